@@ -1,0 +1,173 @@
+/*
+ * casgd.h -- C ABI of libcasgd.so: one communication-avoiding SGD (CA-SGD) outer
+ * iteration for generalized linear models on one NVIDIA B200 (sm_100a).
+ *
+ * Method: "Mixed-Precision Communication-Avoiding SGD for Generalized Linear
+ * Models on GPUs" (arxiv/paper_2606_18463). Citations "PAPER.md:L<n>" are lines
+ * of the paper's text; DESIGN.md lists every reading taken where the text is
+ * silent or garbled. Scope: P = 1 (one GPU, Alg. 1 line 5's AllReduce is the
+ * identity), Recipe C of Table 3 with r and u kept in FP32.
+ *
+ * Notation (sec. 3.1): A is the m x n data matrix (BF16), y the
+ * m labels (FP32), x the n weights (FP32 master), b the mini-batch size, s the
+ * number of inner steps, alpha = eta / b. One outer iteration takes sb = s*b row
+ * indices I = I_0 u ... u I_{s-1} and computes (u = dL/dr = -delta):
+ *
+ *   Y   = A[I, :]                                   Alg. 1 line 2  (L113)   bit-exact
+ *   r   = Y bf16(x)                                 line 3         (L114)   BF16 in, FP32 acc/out
+ *   G   = Y Y^T   (blocks below the block diagonal) line 4         (L116)   BF16 in, FP32 acc/out
+ *   z_j = r_j - alpha * sum_{k<j} G_{jk} u_k        lines 6-15     (L120-L132)   FP32
+ *   u_j = l'(z_j, y_{I_j})                                                  FP32
+ *   x  <- x - alpha * Y^T u                         lines 16-17    (L133-L135)   FP32 master
+ *   bf16(x) refreshed for the next iteration        (L231)
+ *
+ * Conventions for every entry point
+ *   - Pointers are DEVICE pointers on the context's GPU unless the parameter name
+ *     ends in `_host`. Nothing is copied or retained beyond what is stated.
+ *   - Every call returns a casgd_status. On failure casgd_last_error() gives a
+ *     message. Nothing prints, throws or aborts. There is no CPU fallback: on a
+ *     device that is not compute capability 10.x casgd_init returns CASGD_EARCH.
+ *   - Calls that only enqueue work on the context's stream say "asynchronous";
+ *     the others synchronise that stream before returning.
+ *   - A context is not thread-safe; use one per host thread or lock around it.
+ */
+#ifndef CASGD_H
+#define CASGD_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct casgd_ctx casgd_ctx; /* opaque; one per (A, y) dataset and CUDA device */
+
+/* Loss family, sec. 2.1 (L) and L59 sec. 3.1 (delta = -dL/dr):
+ *   LOGISTIC  L = log(1 + exp(-y r)),  u = -y / (1 + exp(y r)),  y in {-1, +1}
+ *   LINEAR    L = (r - y)^2 / 2,       u = r - y
+ *   POISSON   L = exp(r) - y r,        u = exp(r) - y,           y in {0, 1, 2, ...} */
+typedef enum { CASGD_LOGISTIC = 0, CASGD_LINEAR = 1, CASGD_POISSON = 2 } casgd_loss_kind;
+
+typedef enum {
+    CASGD_OK = 0,
+    CASGD_EINVAL = 1, /* bad argument (null, s < 1, b < 1, s*b > CASGD_MAX_SB, unknown loss/option, ...) */
+    CASGD_ENOMEM = 2, /* device or host allocation failed */
+    CASGD_ECUDA = 3,  /* a CUDA call or kernel failed; casgd_last_error() has the CUDA message */
+    CASGD_EARCH = 4,  /* the current device is not sm_100 (B200) */
+    CASGD_EINDEX = 5  /* a row index outside [0, m) was seen by a gather (sticky until casgd_sync) */
+} casgd_status;
+
+/* Largest s*b accepted: the paper's largest block, "sb <= 16384". */
+#define CASGD_MAX_SB 16384
+
+/* Create a context for the dataset (A, y).
+ *   X_bf16  m x n BF16 bit patterns, row-major, row stride `ldx` elements (ldx >= n). BORROWED for the
+ *           context's lifetime when it can be used in place (16-byte aligned base, ldx % 8 == 0);
+ *           otherwise (e.g. n = 18, ldx = 18) the library makes its own zero-padded copy during this
+ *           call and does not touch X_bf16 again.
+ *   y       m FP32 labels (Table 1: labels are FP32 throughout). BORROWED.
+ *   loss    a casgd_loss_kind.
+ *   cuda_stream  a cudaStream_t (NULL = the legacy default stream). All work of this context is
+ *           enqueued on it. BORROWED.
+ * Synchronises `cuda_stream` if it had to copy X. The context allocates its workspaces lazily,
+ * sized to the largest s*b seen. */
+int casgd_init(casgd_ctx **out, const uint16_t *X_bf16, int64_t ldx, const float *y, int64_t m, int32_t n,
+               int loss, void *cuda_stream);
+
+/* One CA-SGD outer iteration, Algorithm 1 at P = 1. ASYNCHRONOUS.
+ *   idx  s*b row indices in [0, m), int32; idx[j*b + i] is row i of mini-batch j. Any multiset is
+ *        accepted (the paper samples with replacement, L111). An out-of-range index makes that
+ *        row read as zeros with label 0 and raises the sticky CASGD_EINDEX flag.
+ *   x    n FP32 master weights, updated in place: x <- x - (eta/b) Y^T u.
+ * The BF16 shadow of x used by the margin (L231) is owned by the context. It is rebuilt from `x`
+ * when the context has no valid shadow for this `x` pointer (first call, pointer change, after
+ * casgd_sgd_step_fp32 or casgd_invalidate_shadow) and otherwise kept current by the fused update;
+ * a caller that modifies x between calls must call casgd_invalidate_shadow. */
+int casgd_outer_step(casgd_ctx *c, const int32_t *idx, float *x, int32_t s, int32_t b, float eta);
+
+/* n_steps consecutive outer iterations; step h uses idx[h*s*b .. (h+1)*s*b). ASYNCHRONOUS.
+ * Same result as n_steps calls of casgd_outer_step, without per-call launch cost (the step's
+ * kernels are replayed from a CUDA graph). An extension of the paper's two CUDA graphs (L278). */
+int casgd_outer_steps(casgd_ctx *c, const int32_t *idx, int64_t n_steps, float *x, int32_t s, int32_t b,
+                      float eta);
+
+/* The same through HOST buffers: copies idx_host (n_steps*s*b int32) and x_host (n FP32) to the
+ * device, runs the steps, copies x back into x_host, and synchronises. Pinned host memory makes the
+ * copies asynchronous with respect to the host but the call still returns only when x_host is valid. */
+int casgd_outer_steps_host(casgd_ctx *c, const int32_t *idx_host, int64_t n_steps, float *x_host, int32_t s,
+                           int32_t b, float eta);
+
+/* In-library baseline: one all-FP32 mini-batch SGD step, i.e. Alg. 1 with s = 1 and every
+ * precision slot FP32 ("Recipe A", Table 3): x <- x - (eta/b) Y32^T l'(Y32 x, y_I), with
+ * Y32 the exact FP32 widening of the BF16 rows. The first call allocates the m x n FP32 copy of A.
+ * `idx` holds b indices; casgd_sgd_steps_fp32 runs n_steps of them. ASYNCHRONOUS. */
+int casgd_sgd_step_fp32(casgd_ctx *c, const int32_t *idx, float *x, int32_t b, float eta);
+int casgd_sgd_steps_fp32(casgd_ctx *c, const int32_t *idx, int64_t n_steps, float *x, int32_t b, float eta);
+
+/* F(x) = (1/m) sum_i L(a_i^T x, y_i) over the whole dataset: BF16 A, FP32 x (the master,
+ * not the shadow), FP32 margins and per-row losses, FP64 sum. Writes one double to *loss_host.
+ * Synchronises. */
+int casgd_loss(casgd_ctx *c, const float *x, double *loss_host);
+
+/* Drop the BF16 shadow so the next outer step rebuilds it from x. */
+int casgd_invalidate_shadow(casgd_ctx *c);
+
+/* Wait for the context's stream; returns CASGD_EINDEX (and clears the flag) if any gather since the
+ * last casgd_sync saw an out-of-range index, CASGD_ECUDA if the stream failed. */
+int casgd_sync(casgd_ctx *c);
+
+/* Intermediates of the LAST outer step (casgd_outer_step, or the last step of casgd_outer_steps),
+ * copied to HOST memory `dst_host`; synchronises. Layouts (sb = s*b of that step):
+ *   CASGD_DBG_Y    sb x n  BF16 bits (uint16), packed row-major         (the gathered rows)
+ *   CASGD_DBG_YLAB sb      FP32                                         (y_I)
+ *   CASGD_DBG_G    sb x sb FP32 packed row-major. Valid entries: G[i][k] with block(k) < block(i)
+ *                  always; every k <= i when CASGD_OPT_GRAM_FULL_LOWER is set. The rest is unspecified.
+ *   CASGD_DBG_R    sb FP32   CASGD_DBG_Z sb FP32   CASGD_DBG_U sb FP32
+ *   CASGD_DBG_XBF  n  BF16 bits: the shadow AFTER the step (bf16 of the updated x)
+ * dst_bytes must equal the size implied above, else CASGD_EINVAL. */
+typedef enum {
+    CASGD_DBG_Y = 0, CASGD_DBG_YLAB = 1, CASGD_DBG_G = 2, CASGD_DBG_R = 3, CASGD_DBG_Z = 4,
+    CASGD_DBG_U = 5, CASGD_DBG_XBF = 6
+} casgd_debug_what;
+int casgd_debug_export(casgd_ctx *c, int what, void *dst_host, int64_t dst_bytes);
+
+/* Options (all default 0 unless stated).
+ *   CASGD_OPT_GRAM_IMPL        0 = tcgen05 tensor-core kernel (default), 1 = plain FP32-FMA CUDA-core kernel
+ *                              (bring-up reference, same BF16 inputs and FP32 accumulation).
+ *   CASGD_OPT_GRAM_FULL_LOWER  1 = also compute the tiles on the block diagonal, so that the whole lower
+ *                              triangle of CASGD_DBG_G is valid (the recurrence never reads them).
+ *   CASGD_OPT_PROFILE          1 = record CUDA events around each stage of casgd_outer_step(s) (disables
+ *                              graph replay); read with casgd_stage_times.
+ *   CASGD_OPT_NO_GRAPH         1 = casgd_outer_steps launches kernels directly instead of replaying a graph. */
+typedef enum {
+    CASGD_OPT_GRAM_IMPL = 0, CASGD_OPT_GRAM_FULL_LOWER = 1, CASGD_OPT_PROFILE = 2, CASGD_OPT_NO_GRAPH = 3
+} casgd_option;
+int casgd_set_option(casgd_ctx *c, int option, int64_t value);
+
+/* Stages of an outer step, for casgd_stage_times and casgd_launch_count. */
+typedef enum {
+    CASGD_STAGE_GATHER = 0, CASGD_STAGE_GRAM = 1, CASGD_STAGE_RECURRENCE = 2, CASGD_STAGE_GRADIENT = 3,
+    CASGD_STAGE_OTHER = 4, CASGD_NUM_STAGES = 5
+} casgd_stage;
+
+/* With CASGD_OPT_PROFILE set: total device milliseconds and launch counts per stage accumulated since
+ * the option was set (or since the last call with reset != 0). ms_host and launches_host each hold
+ * CASGD_NUM_STAGES entries. Synchronises. */
+int casgd_stage_times(casgd_ctx *c, double *ms_host, int64_t *launches_host, int reset);
+
+/* Number of kernels this context has launched (graph replays count their kernel nodes). */
+int64_t casgd_launch_count(const casgd_ctx *c);
+
+/* Message for the last non-OK status returned on this context ("" if none). Owned by the context. */
+const char *casgd_last_error(const casgd_ctx *c);
+
+/* Free everything the context owns (never X_bf16, y, idx, x). Synchronises. NULL is allowed. */
+void casgd_destroy(casgd_ctx *c);
+
+/* Library version string, and the SM architecture the kernels were compiled for ("sm_100a"). */
+const char *casgd_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* CASGD_H */

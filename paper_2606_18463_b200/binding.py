@@ -1,0 +1,221 @@
+"""Thin ctypes binding of libcasgd.so (C ABI: include/casgd.h). Argument marshalling only.
+
+PyTorch is used for device memory and streams; every step of the path runs in the library's
+CUDA kernels. There is no CPU path: if the library is missing or cannot be loaded, `load()`
+raises, and so does everything that needs it.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+from typing import Optional
+
+import numpy as np
+import torch
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libcasgd.so")
+
+LOGISTIC, LINEAR, POISSON = 0, 1, 2
+OK, EINVAL, ENOMEM, ECUDA, EARCH, EINDEX = range(6)
+STATUS_NAMES = ("CASGD_OK", "CASGD_EINVAL", "CASGD_ENOMEM", "CASGD_ECUDA", "CASGD_EARCH", "CASGD_EINDEX")
+DBG_Y, DBG_YLAB, DBG_G, DBG_R, DBG_Z, DBG_U, DBG_XBF = range(7)
+OPT_GRAM_IMPL, OPT_GRAM_FULL_LOWER, OPT_PROFILE, OPT_NO_GRAPH = range(4)
+STAGES = ("gather", "gram", "recurrence", "gradient", "other")
+MAX_SB = 16384
+
+# every symbol include/casgd.h declares
+EXPORTS = (
+    "casgd_init", "casgd_outer_step", "casgd_outer_steps", "casgd_outer_steps_host", "casgd_sgd_step_fp32",
+    "casgd_sgd_steps_fp32", "casgd_loss", "casgd_invalidate_shadow", "casgd_sync", "casgd_debug_export",
+    "casgd_set_option", "casgd_stage_times", "casgd_launch_count", "casgd_last_error", "casgd_destroy",
+    "casgd_version",
+)
+
+
+class CasgdError(RuntimeError):
+    def __init__(self, status: int, message: str):
+        super().__init__(f"{STATUS_NAMES[status] if 0 <= status < 6 else status}: {message}")
+        self.status = status
+
+
+_lib = None
+
+
+def load() -> ctypes.CDLL:
+    """dlopen libcasgd.so and declare the prototypes. Raises if the library has not been built."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(LIB_PATH):
+        raise FileNotFoundError(
+            f"{LIB_PATH} is missing: build it with `python -m paper_2606_18463_b200.build` "
+            "(or __graft_entry__.build()). There is no CPU fallback.")
+    lib = ctypes.CDLL(LIB_PATH)
+    vp, i64, i32, f32 = ctypes.c_void_p, ctypes.c_int64, ctypes.c_int32, ctypes.c_float
+    lib.casgd_init.restype = ctypes.c_int
+    lib.casgd_init.argtypes = [ctypes.POINTER(vp), vp, i64, vp, i64, i32, ctypes.c_int, vp]
+    lib.casgd_outer_step.restype = ctypes.c_int
+    lib.casgd_outer_step.argtypes = [vp, vp, vp, i32, i32, f32]
+    lib.casgd_outer_steps.restype = ctypes.c_int
+    lib.casgd_outer_steps.argtypes = [vp, vp, i64, vp, i32, i32, f32]
+    lib.casgd_outer_steps_host.restype = ctypes.c_int
+    lib.casgd_outer_steps_host.argtypes = [vp, vp, i64, vp, i32, i32, f32]
+    lib.casgd_sgd_step_fp32.restype = ctypes.c_int
+    lib.casgd_sgd_step_fp32.argtypes = [vp, vp, vp, i32, f32]
+    lib.casgd_sgd_steps_fp32.restype = ctypes.c_int
+    lib.casgd_sgd_steps_fp32.argtypes = [vp, vp, i64, vp, i32, f32]
+    lib.casgd_loss.restype = ctypes.c_int
+    lib.casgd_loss.argtypes = [vp, vp, ctypes.POINTER(ctypes.c_double)]
+    lib.casgd_invalidate_shadow.restype = ctypes.c_int
+    lib.casgd_invalidate_shadow.argtypes = [vp]
+    lib.casgd_sync.restype = ctypes.c_int
+    lib.casgd_sync.argtypes = [vp]
+    lib.casgd_debug_export.restype = ctypes.c_int
+    lib.casgd_debug_export.argtypes = [vp, ctypes.c_int, vp, i64]
+    lib.casgd_set_option.restype = ctypes.c_int
+    lib.casgd_set_option.argtypes = [vp, ctypes.c_int, i64]
+    lib.casgd_stage_times.restype = ctypes.c_int
+    lib.casgd_stage_times.argtypes = [vp, ctypes.POINTER(ctypes.c_double), ctypes.POINTER(i64), ctypes.c_int]
+    lib.casgd_launch_count.restype = i64
+    lib.casgd_launch_count.argtypes = [vp]
+    lib.casgd_last_error.restype = ctypes.c_char_p
+    lib.casgd_last_error.argtypes = [vp]
+    lib.casgd_destroy.restype = None
+    lib.casgd_destroy.argtypes = [vp]
+    lib.casgd_version.restype = ctypes.c_char_p
+    lib.casgd_version.argtypes = []
+    _lib = lib
+    return lib
+
+
+def version() -> str:
+    return load().casgd_version().decode()
+
+
+def _dev_ptr(t: torch.Tensor) -> int:
+    assert t.is_cuda and t.is_contiguous(), "device tensors must be contiguous CUDA tensors"
+    return t.data_ptr()
+
+
+class Casgd:
+    """One context per (A, y) dataset: the calls of include/casgd.h with torch tensors for memory.
+
+    X_bf16: [m, n] torch.bfloat16 CUDA tensor (row stride may exceed n); y: [m] float32 CUDA tensor.
+    Both are borrowed: keep them alive as long as this object (it holds references)."""
+
+    def __init__(self, X_bf16: torch.Tensor, y: torch.Tensor, loss: int, stream: Optional[torch.cuda.Stream] = None):
+        lib = load()
+        assert X_bf16.is_cuda and X_bf16.dtype == torch.bfloat16 and X_bf16.dim() == 2 and X_bf16.stride(1) == 1
+        assert y.is_cuda and y.dtype == torch.float32 and y.dim() == 1 and y.is_contiguous()
+        assert y.shape[0] == X_bf16.shape[0]
+        self._lib = lib
+        self.X, self.y = X_bf16, y
+        self.m, self.n = X_bf16.shape
+        self.loss_kind = int(loss)
+        self.stream = stream if stream is not None else torch.cuda.current_stream(X_bf16.device)
+        self._ctx = ctypes.c_void_p()
+        with torch.cuda.device(X_bf16.device):
+            rc = lib.casgd_init(ctypes.byref(self._ctx), X_bf16.data_ptr(), X_bf16.stride(0), y.data_ptr(),
+                                self.m, self.n, self.loss_kind, self.stream.cuda_stream)
+        if rc != OK:
+            self._ctx = ctypes.c_void_p()
+            raise CasgdError(rc, "casgd_init failed (device not sm_100, bad arguments or out of memory)")
+        self._last_sb = 0
+
+    # -- plumbing ---------------------------------------------------------------------------
+    def _check(self, rc: int):
+        if rc != OK:
+            raise CasgdError(rc, self._lib.casgd_last_error(self._ctx).decode())
+
+    def close(self):
+        if getattr(self, "_ctx", None) is not None and self._ctx.value:
+            self._lib.casgd_destroy(self._ctx)
+            self._ctx = ctypes.c_void_p()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def __enter__(self):
+        return self
+
+    def __exit__(self, *exc):
+        self.close()
+
+    # -- the path -----------------------------------------------------------------------------
+    def outer_step(self, idx: torch.Tensor, x: torch.Tensor, s: int, b: int, eta: float):
+        """casgd_outer_step: idx int32 [s*b] (device), x float32 [n] (device, updated in place)."""
+        assert idx.dtype == torch.int32 and idx.numel() == s * b and x.dtype == torch.float32 and x.numel() == self.n
+        self._check(self._lib.casgd_outer_step(self._ctx, _dev_ptr(idx), _dev_ptr(x), s, b, eta))
+        self._last_sb = s * b
+
+    def outer_steps(self, idx: torch.Tensor, x: torch.Tensor, s: int, b: int, eta: float, n_steps: Optional[int] = None):
+        """casgd_outer_steps: idx int32 [n_steps*s*b] (device)."""
+        assert idx.dtype == torch.int32 and x.dtype == torch.float32 and x.numel() == self.n
+        if n_steps is None:
+            assert idx.numel() % (s * b) == 0
+            n_steps = idx.numel() // (s * b)
+        assert idx.numel() >= n_steps * s * b
+        self._check(self._lib.casgd_outer_steps(self._ctx, _dev_ptr(idx), n_steps, _dev_ptr(x), s, b, eta))
+        if n_steps:
+            self._last_sb = s * b
+
+    def outer_steps_host(self, idx_host: torch.Tensor, x_host: torch.Tensor, s: int, b: int, eta: float,
+                         n_steps: Optional[int] = None):
+        """casgd_outer_steps_host: idx_host int32 and x_host float32 are HOST tensors (pinned for async copies)."""
+        assert not idx_host.is_cuda and not x_host.is_cuda
+        assert idx_host.dtype == torch.int32 and idx_host.is_contiguous()
+        assert x_host.dtype == torch.float32 and x_host.is_contiguous() and x_host.numel() == self.n
+        if n_steps is None:
+            n_steps = idx_host.numel() // (s * b)
+        assert idx_host.numel() >= n_steps * s * b
+        self._check(self._lib.casgd_outer_steps_host(self._ctx, idx_host.data_ptr(), n_steps, x_host.data_ptr(), s, b, eta))
+        if n_steps:
+            self._last_sb = s * b
+
+    def sgd_steps_fp32(self, idx: torch.Tensor, x: torch.Tensor, b: int, eta: float, n_steps: Optional[int] = None):
+        """casgd_sgd_steps_fp32: the all-FP32 s = 1 baseline."""
+        assert idx.dtype == torch.int32 and x.dtype == torch.float32 and x.numel() == self.n
+        if n_steps is None:
+            n_steps = idx.numel() // b
+        assert idx.numel() >= n_steps * b
+        self._check(self._lib.casgd_sgd_steps_fp32(self._ctx, _dev_ptr(idx), n_steps, _dev_ptr(x), b, eta))
+
+    def loss(self, x: torch.Tensor) -> float:
+        """casgd_loss: F(x) over the whole dataset."""
+        assert x.dtype == torch.float32 and x.numel() == self.n
+        out = ctypes.c_double()
+        self._check(self._lib.casgd_loss(self._ctx, _dev_ptr(x), ctypes.byref(out)))
+        return out.value
+
+    def sync(self):
+        self._check(self._lib.casgd_sync(self._ctx))
+
+    def invalidate_shadow(self):
+        self._check(self._lib.casgd_invalidate_shadow(self._ctx))
+
+    def set_option(self, option: int, value: int):
+        self._check(self._lib.casgd_set_option(self._ctx, option, value))
+
+    def launch_count(self) -> int:
+        return int(self._lib.casgd_launch_count(self._ctx))
+
+    def stage_times(self, reset: bool = False):
+        ms = (ctypes.c_double * len(STAGES))()
+        cnt = (ctypes.c_int64 * len(STAGES))()
+        self._check(self._lib.casgd_stage_times(self._ctx, ms, cnt, int(reset)))
+        return {name: (ms[i], int(cnt[i])) for i, name in enumerate(STAGES)}
+
+    def debug(self, what: int, sb: Optional[int] = None) -> np.ndarray:
+        """casgd_debug_export into a fresh numpy array (see include/casgd.h for layouts)."""
+        sb = self._last_sb if sb is None else sb
+        shapes = {DBG_Y: ((sb, self.n), np.uint16), DBG_YLAB: ((sb,), np.float32), DBG_G: ((sb, sb), np.float32),
+                  DBG_R: ((sb,), np.float32), DBG_Z: ((sb,), np.float32), DBG_U: ((sb,), np.float32),
+                  DBG_XBF: ((self.n,), np.uint16)}
+        shape, dt = shapes[what]
+        out = np.empty(shape, dt)
+        self._check(self._lib.casgd_debug_export(self._ctx, what, out.ctypes.data, out.nbytes))
+        return out

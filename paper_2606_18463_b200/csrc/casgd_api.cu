@@ -1,0 +1,544 @@
+// casgd_api.cu -- the C ABI of include/casgd.h: argument checks, workspace ownership, stage
+// sequencing, CUDA-graph replay and the host-buffer entry point. No arithmetic of the method
+// lives here; every step of the path runs in the kernels of this directory.
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <map>
+#include <new>
+#include <tuple>
+#include <vector>
+
+#include "common.cuh"
+
+using namespace casgd;
+
+namespace {
+
+struct StageEvent {
+    int stage;
+    cudaEvent_t start, stop;
+};
+
+struct GraphKey {
+    int32_t s, b;
+    uint32_t eta_bits;
+    int32_t len;
+    bool operator<(const GraphKey &o) const
+    {
+        return std::tie(s, b, eta_bits, len) < std::tie(o.s, o.b, o.eta_bits, o.len);
+    }
+};
+
+struct GraphEntry {
+    cudaGraphExec_t exec;
+    int64_t kernels;
+};
+
+inline int64_t round_up(int64_t v, int64_t q) { return (v + q - 1) / q * q; }
+
+}  // namespace
+
+struct casgd_ctx {
+    int device = 0;
+    cudaStream_t stream = nullptr;
+    // dataset
+    const uint16_t *A = nullptr;      // BF16 bits, row stride lda (borrowed or owned)
+    uint16_t *A_owned = nullptr;
+    int64_t lda = 0;
+    const float *y = nullptr;
+    int64_t m = 0;
+    int32_t n = 0;
+    int loss = 0;
+    float *A32 = nullptr;             // lazy FP32 widening for the baseline
+    // per-step workspaces, sized for rows_alloc rows
+    int32_t rows_alloc = 0;
+    int32_t ldy = 0, ldg = 0;
+    uint16_t *Y = nullptr;
+    float *yI = nullptr, *G = nullptr, *r = nullptr, *z = nullptr, *u = nullptr;
+    uint16_t *xbf = nullptr;          // BF16 shadow of x, zero padded
+    const float *shadow_of = nullptr;
+    bool shadow_valid = false;
+    GradWorkspace gws{};
+    StepParams *ind = nullptr;
+    int *err_flag = nullptr;
+    int *err_flag_host = nullptr;     // pinned
+    double *loss_partials = nullptr, *loss_result = nullptr;
+    double *loss_result_host = nullptr;   // pinned
+    int32_t loss_max_blocks = 0;
+    // host-buffer entry point staging
+    int32_t *idx_stage = nullptr;
+    int64_t idx_stage_cap = 0;
+    float *x_stage = nullptr;
+    // last step, for debug export
+    int32_t last_s = 0, last_b = 0;
+    // options
+    int64_t opt_gram_impl = 0, opt_full_lower = 0, opt_profile = 0, opt_no_graph = 0;
+    GramTcPlan *tc_plan = nullptr;
+    std::map<GraphKey, GraphEntry> graphs;
+    std::vector<StageEvent> events;
+    double stage_ms[CASGD_NUM_STAGES] = {};
+    int64_t stage_launches[CASGD_NUM_STAGES] = {};
+    int64_t launches = 0;
+    char err[512] = "";
+};
+
+namespace {
+
+int fail(casgd_ctx *c, int code, const char *fmt, ...)
+{
+    if (c) {
+        va_list ap;
+        va_start(ap, fmt);
+        vsnprintf(c->err, sizeof c->err, fmt, ap);
+        va_end(ap);
+    }
+    return code;
+}
+
+#define CK(call)                                                                                       \
+    do {                                                                                               \
+        cudaError_t e_ = (call);                                                                       \
+        if (e_ != cudaSuccess)                                                                         \
+            return fail(c, e_ == cudaErrorMemoryAllocation ? CASGD_ENOMEM : CASGD_ECUDA, "%s: %s", #call, \
+                        cudaGetErrorString(e_));                                                       \
+    } while (0)
+
+void drop_graphs(casgd_ctx *c)
+{
+    for (auto &kv : c->graphs) cudaGraphExecDestroy(kv.second.exec);
+    c->graphs.clear();
+}
+
+void free_step_workspace(casgd_ctx *c)
+{
+    drop_graphs(c);
+    if (c->tc_plan) { gram_tc_plan_destroy(c->tc_plan); c->tc_plan = nullptr; }
+    cudaFree(c->Y); cudaFree(c->yI); cudaFree(c->G); cudaFree(c->r); cudaFree(c->z); cudaFree(c->u);
+    c->Y = nullptr; c->yI = c->G = c->r = c->z = c->u = nullptr;
+    c->rows_alloc = 0;
+}
+
+int ensure_workspace(casgd_ctx *c, int32_t sb)
+{
+    if (sb <= c->rows_alloc) return CASGD_OK;
+    CK(cudaStreamSynchronize(c->stream));
+    free_step_workspace(c);
+    const int32_t rows = (int32_t)round_up(sb, kTile);
+    c->ldg = rows;
+    CK(cudaMalloc(&c->Y, sizeof(uint16_t) * (size_t)rows * c->ldy));
+    CK(cudaMalloc(&c->yI, sizeof(float) * rows));
+    CK(cudaMalloc(&c->G, sizeof(float) * (size_t)rows * rows));
+    CK(cudaMalloc(&c->r, sizeof(float) * rows));
+    CK(cudaMalloc(&c->z, sizeof(float) * rows));
+    CK(cudaMalloc(&c->u, sizeof(float) * rows));
+    CK(cudaMemsetAsync(c->Y, 0, sizeof(uint16_t) * (size_t)rows * c->ldy, c->stream));
+    CK(cudaMemsetAsync(c->G, 0, sizeof(float) * (size_t)rows * rows, c->stream));
+    CK(cudaMemsetAsync(c->yI, 0, sizeof(float) * rows, c->stream));
+    CK(cudaMemsetAsync(c->r, 0, sizeof(float) * rows, c->stream));
+    CK(cudaMemsetAsync(c->z, 0, sizeof(float) * rows, c->stream));
+    CK(cudaMemsetAsync(c->u, 0, sizeof(float) * rows, c->stream));
+    c->rows_alloc = rows;
+    return CASGD_OK;
+}
+
+int check_step_args(casgd_ctx *c, const void *idx, const void *x, int64_t n_steps, int32_t s, int32_t b, float eta)
+{
+    if (!c) return CASGD_EINVAL;
+    if (!idx || !x) return fail(c, CASGD_EINVAL, "idx and x must not be null");
+    if (n_steps < 0) return fail(c, CASGD_EINVAL, "n_steps = %lld < 0", (long long)n_steps);
+    if (s < 1 || b < 1) return fail(c, CASGD_EINVAL, "s = %d and b = %d must be >= 1", s, b);
+    if ((int64_t)s * b > CASGD_MAX_SB) return fail(c, CASGD_EINVAL, "s*b = %lld exceeds CASGD_MAX_SB = %d", (long long)s * b, CASGD_MAX_SB);
+    if (!(eta == eta)) return fail(c, CASGD_EINVAL, "eta is NaN");
+    return CASGD_OK;
+}
+
+struct StageTimer {
+    casgd_ctx *c;
+    int stage;
+    StageEvent ev{};
+    bool on;
+    StageTimer(casgd_ctx *c_, int stage_) : c(c_), stage(stage_), on(c_->opt_profile != 0)
+    {
+        if (!on) return;
+        ev.stage = stage;
+        cudaEventCreate(&ev.start);
+        cudaEventCreate(&ev.stop);
+        cudaEventRecord(ev.start, c->stream);
+    }
+    void done(int launches)
+    {
+        c->launches += launches;
+        if (!on) return;
+        cudaEventRecord(ev.stop, c->stream);
+        c->events.push_back(ev);
+        c->stage_launches[stage] += launches;
+    }
+};
+
+// Enqueue one outer iteration (Alg. 1 lines 2-17). `ind` non-null: graph-replay addressing.
+int enqueue_step(casgd_ctx *c, const int32_t *idx, const StepParams *ind, int64_t idx_off, float *x, int32_t s,
+                 int32_t b, float eta, int64_t *kernels)
+{
+    const int32_t sb = s * b;
+    const float alpha = eta / (float)b;
+    int k;
+    {
+        StageTimer t(c, CASGD_STAGE_GATHER);
+        k = launch_gather(c->stream, c->A, c->lda, c->y, c->m, c->n, idx, ind, idx_off, sb, c->Y, c->ldy, c->yI, c->err_flag);
+        t.done(k); *kernels += k;
+    }
+    {
+        StageTimer t(c, CASGD_STAGE_GRAM);
+        if (c->opt_gram_impl == 1) {
+            k = launch_gram_simt(c->stream, c->Y, c->ldy, c->n, sb, b, c->xbf, c->G, c->ldg, c->r, (int)c->opt_full_lower);
+        } else {
+            if (!c->tc_plan) {
+                c->tc_plan = gram_tc_plan_create(c->Y, c->ldy, c->n, c->rows_alloc, c->xbf, c->err, sizeof c->err);
+                if (!c->tc_plan) return CASGD_ECUDA;
+            }
+            k = launch_gram_tc(c->stream, c->tc_plan, sb, b, c->G, c->ldg, c->r, (int)c->opt_full_lower, c->err, sizeof c->err);
+            if (k < 0) return CASGD_ECUDA;
+        }
+        t.done(k); *kernels += k;
+    }
+    {
+        StageTimer t(c, CASGD_STAGE_RECURRENCE);
+        k = launch_recurrence(c->stream, c->G, c->ldg, c->r, c->yI, s, b, alpha, c->loss, c->z, c->u);
+        t.done(k); *kernels += k;
+    }
+    {
+        StageTimer t(c, CASGD_STAGE_GRADIENT);
+        k = launch_gradient_bf16(c->stream, c->Y, c->ldy, c->n, sb, c->u, alpha, x, ind, c->xbf, c->gws);
+        t.done(k); *kernels += k;
+    }
+    return CASGD_OK;
+}
+
+int ensure_shadow(casgd_ctx *c, const float *x)
+{
+    if (c->shadow_valid && c->shadow_of == x) return CASGD_OK;
+    StageTimer t(c, CASGD_STAGE_OTHER);
+    int k = launch_shadow(c->stream, x, nullptr, c->n, c->xbf);
+    t.done(k);
+    c->shadow_of = x;
+    c->shadow_valid = true;
+    return CASGD_OK;
+}
+
+int get_graph(casgd_ctx *c, int32_t s, int32_t b, float eta, int32_t len, GraphEntry *out)
+{
+    GraphKey key{s, b, 0u, len};
+    memcpy(&key.eta_bits, &eta, sizeof eta);
+    auto it = c->graphs.find(key);
+    if (it != c->graphs.end()) { *out = it->second; return CASGD_OK; }
+    cudaGraph_t graph = nullptr;
+    CK(cudaStreamBeginCapture(c->stream, cudaStreamCaptureModeThreadLocal));
+    int64_t kernels = 0;
+    int rc = CASGD_OK;
+    const int64_t saved = c->launches;
+    for (int32_t h = 0; h < len && rc == CASGD_OK; ++h)
+        rc = enqueue_step(c, nullptr, c->ind, (int64_t)h * s * b, nullptr, s, b, eta, &kernels);
+    c->launches = saved;                      // capture launches nothing; replays are counted
+    cudaError_t e = cudaStreamEndCapture(c->stream, &graph);
+    if (rc != CASGD_OK) { if (graph) cudaGraphDestroy(graph); return rc; }
+    if (e != cudaSuccess) return fail(c, CASGD_ECUDA, "cudaStreamEndCapture: %s", cudaGetErrorString(e));
+    GraphEntry ge{nullptr, kernels};
+    e = cudaGraphInstantiate(&ge.exec, graph, 0);
+    cudaGraphDestroy(graph);
+    if (e != cudaSuccess) return fail(c, CASGD_ECUDA, "cudaGraphInstantiate: %s", cudaGetErrorString(e));
+    c->graphs[key] = ge;
+    *out = ge;
+    return CASGD_OK;
+}
+
+int collect_events(casgd_ctx *c)
+{
+    for (auto &ev : c->events) {
+        float ms = 0.f;
+        cudaError_t e = cudaEventElapsedTime(&ms, ev.start, ev.stop);
+        if (e == cudaSuccess) c->stage_ms[ev.stage] += ms;
+        cudaEventDestroy(ev.start);
+        cudaEventDestroy(ev.stop);
+    }
+    c->events.clear();
+    return CASGD_OK;
+}
+
+int run_steps(casgd_ctx *c, const int32_t *idx, int64_t n_steps, float *x, int32_t s, int32_t b, float eta,
+              bool allow_graph)
+{
+    const int32_t sb = s * b;
+    int rc = ensure_workspace(c, sb);
+    if (rc) return rc;
+    rc = ensure_shadow(c, x);
+    if (rc) return rc;
+    c->last_s = s;
+    c->last_b = b;
+    int64_t done = 0;
+    if (allow_graph && !c->opt_profile && !c->opt_no_graph && n_steps >= 2) {
+        static const int32_t lens[3] = {64, 8, 1};
+        for (int li = 0; li < 3; ++li) {
+            const int32_t len = lens[li];
+            if (n_steps - done < len) continue;
+            GraphEntry ge;
+            rc = get_graph(c, s, b, eta, len, &ge);
+            if (rc) return rc;
+            while (n_steps - done >= len) {
+                c->launches += launch_set_params(c->stream, c->ind, idx + done * sb, x);
+                CK(cudaGraphLaunch(ge.exec, c->stream));
+                c->launches += ge.kernels;
+                done += len;
+            }
+        }
+    }
+    for (; done < n_steps; ++done) {
+        int64_t kernels = 0;
+        rc = enqueue_step(c, idx + done * sb, nullptr, 0, x, s, b, eta, &kernels);
+        if (rc) return rc;
+    }
+    CK(cudaGetLastError());
+    return CASGD_OK;
+}
+
+}  // namespace
+
+// ------------------------------------------------------------------------- C ABI ---
+
+extern "C" {
+
+const char *casgd_version(void) { return "casgd-b200 0.1 (sm_100a)"; }
+
+int casgd_init(casgd_ctx **out, const uint16_t *X_bf16, int64_t ldx, const float *y, int64_t m, int32_t n, int loss,
+               void *cuda_stream)
+{
+    if (!out) return CASGD_EINVAL;
+    *out = nullptr;
+    if (!X_bf16 || !y || m < 1 || n < 1 || ldx < n || loss < 0 || loss > 2) return CASGD_EINVAL;
+    casgd_ctx *c = new (std::nothrow) casgd_ctx;
+    if (!c) return CASGD_ENOMEM;
+    auto bail = [&](int code) { casgd_destroy(c); return code; };
+    cudaDeviceProp prop;
+    if (cudaGetDevice(&c->device) != cudaSuccess || cudaGetDeviceProperties(&prop, c->device) != cudaSuccess)
+        return bail(CASGD_ECUDA);
+    if (prop.major != 10) return bail(CASGD_EARCH);
+    c->stream = (cudaStream_t)cuda_stream;
+    c->y = y; c->m = m; c->n = n; c->loss = loss;
+    c->ldy = (int32_t)round_up(n, 8);
+
+    auto ck = [&](cudaError_t e) { return e == cudaSuccess; };
+    const bool in_place = (ldx % 8 == 0) && ((uintptr_t)X_bf16 % 16 == 0);
+    if (in_place) {
+        c->A = X_bf16;
+        c->lda = ldx;
+    } else {
+        // narrow rows get a power-of-two stride so that no row straddles a 128-byte line
+        int64_t lda = round_up(n, 8);
+        if (lda < 64) { int64_t p = 8; while (p < lda) p <<= 1; lda = p; }
+        if (!ck(cudaMalloc(&c->A_owned, sizeof(uint16_t) * (size_t)m * lda))) return bail(CASGD_ENOMEM);
+        c->launches += launch_repack(c->stream, X_bf16, ldx, m, n, c->A_owned, lda);
+        if (!ck(cudaStreamSynchronize(c->stream))) return bail(CASGD_ECUDA);
+        c->A = c->A_owned;
+        c->lda = lda;
+    }
+    const size_t xbf_elems = (size_t)round_up(n, 64) + 64;
+    c->gws.ldp = c->ldy;
+    c->gws.max_splits = 128;
+    c->loss_max_blocks = kNumSMsB200 * 4;
+    const int n_counters = 8192;
+    bool ok = ck(cudaMalloc(&c->xbf, sizeof(uint16_t) * xbf_elems)) &&
+              ck(cudaMemsetAsync(c->xbf, 0, sizeof(uint16_t) * xbf_elems, c->stream)) &&
+              ck(cudaMalloc(&c->gws.partial, sizeof(float) * (size_t)c->gws.max_splits * c->gws.ldp)) &&
+              ck(cudaMalloc(&c->gws.counters, sizeof(unsigned) * n_counters)) &&
+              ck(cudaMemsetAsync(c->gws.counters, 0, sizeof(unsigned) * n_counters, c->stream)) &&
+              ck(cudaMalloc(&c->ind, sizeof(StepParams))) &&
+              ck(cudaMalloc(&c->err_flag, sizeof(int))) &&
+              ck(cudaMemsetAsync(c->err_flag, 0, sizeof(int), c->stream)) &&
+              ck(cudaMallocHost(&c->err_flag_host, sizeof(int))) &&
+              ck(cudaMalloc(&c->loss_partials, sizeof(double) * c->loss_max_blocks)) &&
+              ck(cudaMalloc(&c->loss_result, sizeof(double))) &&
+              ck(cudaMallocHost(&c->loss_result_host, sizeof(double))) &&
+              ck(cudaMalloc(&c->x_stage, sizeof(float) * (size_t)n));
+    if (!ok) return bail(CASGD_ENOMEM);
+    *out = c;
+    return CASGD_OK;
+}
+
+int casgd_outer_step(casgd_ctx *c, const int32_t *idx, float *x, int32_t s, int32_t b, float eta)
+{
+    int rc = check_step_args(c, idx, x, 1, s, b, eta);
+    if (rc) return rc;
+    return run_steps(c, idx, 1, x, s, b, eta, false);
+}
+
+int casgd_outer_steps(casgd_ctx *c, const int32_t *idx, int64_t n_steps, float *x, int32_t s, int32_t b, float eta)
+{
+    int rc = check_step_args(c, idx, x, n_steps, s, b, eta);
+    if (rc) return rc;
+    return run_steps(c, idx, n_steps, x, s, b, eta, true);
+}
+
+int casgd_outer_steps_host(casgd_ctx *c, const int32_t *idx_host, int64_t n_steps, float *x_host, int32_t s, int32_t b,
+                           float eta)
+{
+    int rc = check_step_args(c, idx_host, x_host, n_steps, s, b, eta);
+    if (rc) return rc;
+    const int64_t count = n_steps * s * b;
+    if (count > c->idx_stage_cap) {
+        CK(cudaStreamSynchronize(c->stream));
+        cudaFree(c->idx_stage);
+        c->idx_stage = nullptr;
+        c->idx_stage_cap = 0;
+        CK(cudaMalloc(&c->idx_stage, sizeof(int32_t) * (size_t)count));
+        c->idx_stage_cap = count;
+    }
+    if (count > 0) CK(cudaMemcpyAsync(c->idx_stage, idx_host, sizeof(int32_t) * (size_t)count, cudaMemcpyHostToDevice, c->stream));
+    CK(cudaMemcpyAsync(c->x_stage, x_host, sizeof(float) * (size_t)c->n, cudaMemcpyHostToDevice, c->stream));
+    c->shadow_valid = false;                  // x_stage was overwritten from the host
+    rc = run_steps(c, c->idx_stage, n_steps, c->x_stage, s, b, eta, true);
+    if (rc) return rc;
+    CK(cudaMemcpyAsync(x_host, c->x_stage, sizeof(float) * (size_t)c->n, cudaMemcpyDeviceToHost, c->stream));
+    CK(cudaStreamSynchronize(c->stream));
+    return CASGD_OK;
+}
+
+int casgd_sgd_steps_fp32(casgd_ctx *c, const int32_t *idx, int64_t n_steps, float *x, int32_t b, float eta)
+{
+    int rc = check_step_args(c, idx, x, n_steps, 1, b, eta);
+    if (rc) return rc;
+    if (!c->A32) {
+        CK(cudaMalloc(&c->A32, sizeof(float) * (size_t)c->m * c->lda));
+        c->launches += launch_widen(c->stream, c->A, c->lda, c->m, c->n, c->A32, c->lda);
+    }
+    rc = ensure_workspace(c, b);
+    if (rc) return rc;
+    c->shadow_valid = false;                  // x changes without the shadow following
+    const float alpha = eta / (float)b;
+    for (int64_t h = 0; h < n_steps; ++h)
+        c->launches += launch_sgd32_step(c->stream, c->A32, c->lda, c->y, c->m, c->n, idx + h * b, b, alpha, c->loss, x,
+                                         c->u, c->z, c->err_flag, c->gws);
+    CK(cudaGetLastError());
+    return CASGD_OK;
+}
+
+int casgd_sgd_step_fp32(casgd_ctx *c, const int32_t *idx, float *x, int32_t b, float eta)
+{
+    return casgd_sgd_steps_fp32(c, idx, 1, x, b, eta);
+}
+
+int casgd_loss(casgd_ctx *c, const float *x, double *loss_host)
+{
+    if (!c) return CASGD_EINVAL;
+    if (!x || !loss_host) return fail(c, CASGD_EINVAL, "x and loss_host must not be null");
+    c->launches += launch_loss(c->stream, c->A, c->lda, c->y, c->m, c->n, c->loss, x, c->loss_partials,
+                               c->loss_max_blocks, c->loss_result);
+    CK(cudaGetLastError());
+    CK(cudaMemcpyAsync(c->loss_result_host, c->loss_result, sizeof(double), cudaMemcpyDeviceToHost, c->stream));
+    CK(cudaStreamSynchronize(c->stream));
+    *loss_host = *c->loss_result_host;
+    return CASGD_OK;
+}
+
+int casgd_invalidate_shadow(casgd_ctx *c)
+{
+    if (!c) return CASGD_EINVAL;
+    c->shadow_valid = false;
+    return CASGD_OK;
+}
+
+int casgd_sync(casgd_ctx *c)
+{
+    if (!c) return CASGD_EINVAL;
+    CK(cudaMemcpyAsync(c->err_flag_host, c->err_flag, sizeof(int), cudaMemcpyDeviceToHost, c->stream));
+    CK(cudaStreamSynchronize(c->stream));
+    if (*c->err_flag_host) {
+        CK(cudaMemsetAsync(c->err_flag, 0, sizeof(int), c->stream));
+        return fail(c, CASGD_EINDEX, "a row index outside [0, %lld) was gathered", (long long)c->m);
+    }
+    return CASGD_OK;
+}
+
+int casgd_debug_export(casgd_ctx *c, int what, void *dst_host, int64_t dst_bytes)
+{
+    if (!c) return CASGD_EINVAL;
+    if (!dst_host) return fail(c, CASGD_EINVAL, "dst_host is null");
+    const int64_t sb = (int64_t)c->last_s * c->last_b;
+    if (sb == 0 && what != CASGD_DBG_XBF) return fail(c, CASGD_EINVAL, "no outer step has run yet");
+    CK(cudaStreamSynchronize(c->stream));
+    auto need = [&](int64_t bytes) { return dst_bytes == bytes; };
+    switch (what) {
+    case CASGD_DBG_Y:
+        if (!need(sb * c->n * 2)) break;
+        CK(cudaMemcpy2D(dst_host, (size_t)c->n * 2, c->Y, (size_t)c->ldy * 2, (size_t)c->n * 2, (size_t)sb, cudaMemcpyDeviceToHost));
+        return CASGD_OK;
+    case CASGD_DBG_G:
+        if (!need(sb * sb * 4)) break;
+        CK(cudaMemcpy2D(dst_host, (size_t)sb * 4, c->G, (size_t)c->ldg * 4, (size_t)sb * 4, (size_t)sb, cudaMemcpyDeviceToHost));
+        return CASGD_OK;
+    case CASGD_DBG_YLAB: case CASGD_DBG_R: case CASGD_DBG_Z: case CASGD_DBG_U: {
+        if (!need(sb * 4)) break;
+        const float *src = what == CASGD_DBG_YLAB ? c->yI : what == CASGD_DBG_R ? c->r : what == CASGD_DBG_Z ? c->z : c->u;
+        CK(cudaMemcpy(dst_host, src, (size_t)sb * 4, cudaMemcpyDeviceToHost));
+        return CASGD_OK;
+    }
+    case CASGD_DBG_XBF:
+        if (!need((int64_t)c->n * 2)) break;
+        CK(cudaMemcpy(dst_host, c->xbf, (size_t)c->n * 2, cudaMemcpyDeviceToHost));
+        return CASGD_OK;
+    default:
+        return fail(c, CASGD_EINVAL, "unknown debug item %d", what);
+    }
+    return fail(c, CASGD_EINVAL, "dst_bytes = %lld does not match item %d of the last step (s = %d, b = %d, n = %d)",
+                (long long)dst_bytes, what, c->last_s, c->last_b, c->n);
+}
+
+int casgd_set_option(casgd_ctx *c, int option, int64_t value)
+{
+    if (!c) return CASGD_EINVAL;
+    switch (option) {
+    case CASGD_OPT_GRAM_IMPL:
+        if (value != 0 && value != 1) return fail(c, CASGD_EINVAL, "CASGD_OPT_GRAM_IMPL must be 0 or 1");
+        c->opt_gram_impl = value; break;
+    case CASGD_OPT_GRAM_FULL_LOWER: c->opt_full_lower = value != 0; break;
+    case CASGD_OPT_PROFILE:
+        c->opt_profile = value != 0;
+        break;
+    case CASGD_OPT_NO_GRAPH: c->opt_no_graph = value != 0; break;
+    default: return fail(c, CASGD_EINVAL, "unknown option %d", option);
+    }
+    drop_graphs(c);
+    return CASGD_OK;
+}
+
+int casgd_stage_times(casgd_ctx *c, double *ms_host, int64_t *launches_host, int reset)
+{
+    if (!c) return CASGD_EINVAL;
+    CK(cudaStreamSynchronize(c->stream));
+    collect_events(c);
+    for (int i = 0; i < CASGD_NUM_STAGES; ++i) {
+        if (ms_host) ms_host[i] = c->stage_ms[i];
+        if (launches_host) launches_host[i] = c->stage_launches[i];
+        if (reset) { c->stage_ms[i] = 0.0; c->stage_launches[i] = 0; }
+    }
+    return CASGD_OK;
+}
+
+int64_t casgd_launch_count(const casgd_ctx *c) { return c ? c->launches : 0; }
+
+const char *casgd_last_error(const casgd_ctx *c) { return c ? c->err : "null context"; }
+
+void casgd_destroy(casgd_ctx *c)
+{
+    if (!c) return;
+    cudaStreamSynchronize(c->stream);
+    collect_events(c);
+    free_step_workspace(c);
+    cudaFree(c->A_owned); cudaFree(c->A32); cudaFree(c->xbf);
+    cudaFree(c->gws.partial); cudaFree(c->gws.counters); cudaFree(c->ind); cudaFree(c->err_flag);
+    cudaFree(c->loss_partials); cudaFree(c->loss_result); cudaFree(c->idx_stage); cudaFree(c->x_stage);
+    if (c->err_flag_host) cudaFreeHost(c->err_flag_host);
+    if (c->loss_result_host) cudaFreeHost(c->loss_result_host);
+    delete c;
+}
+
+}  // extern "C"

@@ -1,0 +1,151 @@
+// common.cuh -- shared declarations of libcasgd.so (device helpers, context, launch prototypes).
+// Notation follows the paper (arxiv/paper_2606_18463): A, y, x, Y, G, r, z, u, b, s, alpha = eta/b.
+#pragma once
+
+#include <cuda_bf16.h>
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "../../include/casgd.h"
+
+namespace casgd {
+
+constexpr int kTile = 128;            // Gram tile edge (rows of Y per tcgen05 operand tile)
+constexpr int kNumSMsB200 = 148;
+
+// Device-side indirection block: lets kernels baked into a CUDA graph follow a base pointer
+// that changes between replays (casgd_outer_steps).
+struct StepParams {
+    const int32_t *idx;   // first index of the current replay
+    float *x;             // master weights
+};
+
+// ---------------------------------------------------------------- device math ---
+
+__device__ __forceinline__ float bf16_bits_to_f32(uint16_t h) { return __uint_as_float(((uint32_t)h) << 16); }
+__device__ __forceinline__ float bf16lo(uint32_t w) { return __uint_as_float(w << 16); }
+__device__ __forceinline__ float bf16hi(uint32_t w) { return __uint_as_float(w & 0xffff0000u); }
+
+__device__ __forceinline__ uint16_t f32_to_bf16_bits_rn(float f)
+{
+    return __bfloat16_as_ushort(__float2bfloat16_rn(f));
+}
+
+// u = dL/dr = -delta. Accurate expf (not __expf): Poisson amplifies margin error by e^z.
+template <int LOSS>
+__device__ __forceinline__ float lprime(float z, float y)
+{
+    if (LOSS == CASGD_LOGISTIC) {
+        float t = y * z;
+        float e = expf(-fabsf(t));                   // in (0, 1]
+        float sig_neg = (t >= 0.f) ? e / (1.f + e) : 1.f / (1.f + e);   // 1 / (1 + e^{t})
+        return -y * sig_neg;
+    } else if (LOSS == CASGD_LINEAR) {
+        return z - y;
+    } else {
+        return expf(z) - y;
+    }
+}
+
+__device__ __forceinline__ float lprime_rt(int loss, float z, float y)
+{
+    return loss == CASGD_LOGISTIC ? lprime<CASGD_LOGISTIC>(z, y)
+         : loss == CASGD_LINEAR  ? lprime<CASGD_LINEAR>(z, y)
+                                 : lprime<CASGD_POISSON>(z, y);
+}
+
+// L(r, y) in FP32; logistic as max(-t, 0) + log1p(exp(-|t|)).
+__device__ __forceinline__ float loss_value_rt(int loss, float r, float y)
+{
+    if (loss == CASGD_LOGISTIC) {
+        float t = y * r;
+        return fmaxf(-t, 0.f) + log1pf(expf(-fabsf(t)));
+    } else if (loss == CASGD_LINEAR) {
+        float d = r - y;
+        return 0.5f * d * d;
+    }
+    return expf(r) - y * r;
+}
+
+__device__ __forceinline__ float warp_sum(float v)
+{
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    return v;
+}
+
+__device__ __forceinline__ double warp_sum(double v)
+{
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    return v;
+}
+
+// dot of 8 BF16 (one 16-byte vector) with 8 FP32
+__device__ __forceinline__ float dot8(const uint4 &a, const float4 &x0, const float4 &x1, float acc)
+{
+    acc = fmaf(bf16lo(a.x), x0.x, acc);
+    acc = fmaf(bf16hi(a.x), x0.y, acc);
+    acc = fmaf(bf16lo(a.y), x0.z, acc);
+    acc = fmaf(bf16hi(a.y), x0.w, acc);
+    acc = fmaf(bf16lo(a.z), x1.x, acc);
+    acc = fmaf(bf16hi(a.z), x1.y, acc);
+    acc = fmaf(bf16lo(a.w), x1.z, acc);
+    acc = fmaf(bf16hi(a.w), x1.w, acc);
+    return acc;
+}
+
+__device__ __forceinline__ uint4 ldg_nc_v4(const void *p)
+{
+    uint4 r;
+    asm volatile("ld.global.nc.L1::no_allocate.v4.u32 {%0, %1, %2, %3}, [%4];"
+                 : "=r"(r.x), "=r"(r.y), "=r"(r.z), "=r"(r.w) : "l"(p));
+    return r;
+}
+
+// ------------------------------------------------------------ launch prototypes ---
+// Every launcher enqueues on `st` and returns the number of kernels it launched.
+// `ind`, when non-null, overrides idx / x with ind->idx + idx_off / ind->x (graph replay).
+
+int launch_gather(cudaStream_t st, const uint16_t *A, int64_t lda, const float *y, int64_t m, int32_t n,
+                  const int32_t *idx, const StepParams *ind, int64_t idx_off, int32_t sb, uint16_t *Y, int32_t ldy,
+                  float *yI, int *err_flag);
+
+int launch_gram_simt(cudaStream_t st, const uint16_t *Y, int32_t ldy, int32_t n, int32_t sb, int32_t b,
+                     const uint16_t *xbf, float *G, int32_t ldg, float *r, int full_lower);
+
+int launch_recurrence(cudaStream_t st, const float *G, int32_t ldg, const float *r, const float *yI, int32_t s,
+                      int32_t b, float alpha, int loss, float *z, float *u);
+
+struct GradWorkspace {
+    float *partial;        // [row_splits x ldp] partial column sums
+    int32_t ldp;
+    unsigned *counters;    // one per column tile, zero between launches
+    int32_t max_splits;
+};
+
+int launch_gradient_bf16(cudaStream_t st, const uint16_t *Y, int32_t ldy, int32_t n, int32_t sb, const float *u,
+                         float alpha, float *x, const StepParams *ind, uint16_t *xbf, const GradWorkspace &ws);
+
+int launch_sgd32_step(cudaStream_t st, const float *A32, int64_t lda32, const float *y, int64_t m, int32_t n,
+                      const int32_t *idx, int32_t b, float alpha, int loss, float *x, float *u, float *z,
+                      int *err_flag, const GradWorkspace &ws);
+
+int launch_loss(cudaStream_t st, const uint16_t *A, int64_t lda, const float *y, int64_t m, int32_t n, int loss,
+                const float *x, double *block_partials, int32_t max_blocks, double *result_dev);
+
+int launch_shadow(cudaStream_t st, const float *x, const StepParams *ind, int32_t n, uint16_t *xbf);
+int launch_widen(cudaStream_t st, const uint16_t *A, int64_t lda, int64_t m, int32_t n, float *A32, int64_t lda32);
+int launch_repack(cudaStream_t st, const uint16_t *X, int64_t ldx, int64_t m, int32_t n, uint16_t *A, int64_t lda);
+int launch_set_params(cudaStream_t st, StepParams *ind, const int32_t *idx, float *x);
+
+// tcgen05 Gram + margin (gram_tc.cu). `tmaps` points at device-visible-by-value tensor maps owned by
+// the caller (see casgd_api.cu); returns 0 launches and sets *unsupported when the shape is not handled.
+struct GramTcPlan;
+GramTcPlan *gram_tc_plan_create(const uint16_t *Y, int32_t ldy, int32_t n, int32_t sb_rows_alloc,
+                                const uint16_t *xbf, char *err, int errlen);
+void gram_tc_plan_destroy(GramTcPlan *p);
+int launch_gram_tc(cudaStream_t st, GramTcPlan *plan, int32_t sb, int32_t b, float *G, int32_t ldg, float *r,
+                   int full_lower, char *err, int errlen);
+
+}  // namespace casgd
