@@ -138,16 +138,19 @@ int casgd_debug_export(casgd_ctx *c, int what, void *dst_host, int64_t dst_bytes
  *                              triangle of CASGD_DBG_G is valid (the recurrence never reads them).
  *   CASGD_OPT_PROFILE          1 = record CUDA events around each stage of casgd_outer_step(s) (disables
  *                              graph replay); read with casgd_stage_times.
- *   CASGD_OPT_NO_GRAPH         1 = casgd_outer_steps launches kernels directly instead of replaying a graph. */
+ *   CASGD_OPT_NO_GRAPH         1 = casgd_outer_steps launches kernels directly instead of replaying a graph.
+ *   CASGD_OPT_GRAM_KSPLIT      0 = the tcgen05 Gram kernel chooses how many slices to cut K (= n) into so that
+ *                              few-tile shapes still fill the GPU; k in [1, 64] forces k slices. */
 typedef enum {
-    CASGD_OPT_GRAM_IMPL = 0, CASGD_OPT_GRAM_FULL_LOWER = 1, CASGD_OPT_PROFILE = 2, CASGD_OPT_NO_GRAPH = 3
+    CASGD_OPT_GRAM_IMPL = 0, CASGD_OPT_GRAM_FULL_LOWER = 1, CASGD_OPT_PROFILE = 2, CASGD_OPT_NO_GRAPH = 3,
+    CASGD_OPT_GRAM_KSPLIT = 4
 } casgd_option;
 int casgd_set_option(casgd_ctx *c, int option, int64_t value);
 
-/* Stages of an outer step, for casgd_stage_times and casgd_launch_count. */
+/* Stages of an outer step (plus shadow rebuilds = OTHER, and casgd_loss), for casgd_stage_times. */
 typedef enum {
     CASGD_STAGE_GATHER = 0, CASGD_STAGE_GRAM = 1, CASGD_STAGE_RECURRENCE = 2, CASGD_STAGE_GRADIENT = 3,
-    CASGD_STAGE_OTHER = 4, CASGD_NUM_STAGES = 5
+    CASGD_STAGE_OTHER = 4, CASGD_STAGE_LOSS = 5, CASGD_NUM_STAGES = 6
 } casgd_stage;
 
 /* With CASGD_OPT_PROFILE set: total device milliseconds and launch counts per stage accumulated since

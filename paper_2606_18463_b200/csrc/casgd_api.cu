@@ -42,6 +42,7 @@ inline int64_t round_up(int64_t v, int64_t q) { return (v + q - 1) / q * q; }
 struct casgd_ctx {
     int device = 0;
     cudaStream_t stream = nullptr;
+    cudaStream_t capture_stream = nullptr;
     // dataset
     const uint16_t *A = nullptr;      // BF16 bits, row stride lda (borrowed or owned)
     uint16_t *A_owned = nullptr;
@@ -56,7 +57,8 @@ struct casgd_ctx {
     int32_t ldy = 0, ldg = 0;
     uint16_t *Y = nullptr;
     float *yI = nullptr, *G = nullptr, *r = nullptr, *z = nullptr, *u = nullptr;
-    uint16_t *xbf = nullptr;          // BF16 shadow of x, zero padded
+    uint16_t *xbf = nullptr;          // BF16 shadow of x: [16 x ldxb], row 0 = bf16(x), the rest zero
+    int32_t ldxb = 0;
     const float *shadow_of = nullptr;
     bool shadow_valid = false;
     GradWorkspace gws{};
@@ -73,7 +75,7 @@ struct casgd_ctx {
     // last step, for debug export
     int32_t last_s = 0, last_b = 0;
     // options
-    int64_t opt_gram_impl = 0, opt_full_lower = 0, opt_profile = 0, opt_no_graph = 0;
+    int64_t opt_gram_impl = 0, opt_full_lower = 0, opt_profile = 0, opt_no_graph = 0, opt_ksplit = 0;
     GramTcPlan *tc_plan = nullptr;
     std::map<GraphKey, GraphEntry> graphs;
     std::vector<StageEvent> events;
@@ -177,39 +179,39 @@ struct StageTimer {
 };
 
 // Enqueue one outer iteration (Alg. 1 lines 2-17). `ind` non-null: graph-replay addressing.
-int enqueue_step(casgd_ctx *c, const int32_t *idx, const StepParams *ind, int64_t idx_off, float *x, int32_t s,
-                 int32_t b, float eta, int64_t *kernels)
+int enqueue_step(casgd_ctx *c, cudaStream_t st, const int32_t *idx, const StepParams *ind, int64_t idx_off, float *x,
+                 int32_t s, int32_t b, float eta, int64_t *kernels)
 {
     const int32_t sb = s * b;
     const float alpha = eta / (float)b;
     int k;
     {
         StageTimer t(c, CASGD_STAGE_GATHER);
-        k = launch_gather(c->stream, c->A, c->lda, c->y, c->m, c->n, idx, ind, idx_off, sb, c->Y, c->ldy, c->yI, c->err_flag);
+        k = launch_gather(st, c->A, c->lda, c->y, c->m, c->n, idx, ind, idx_off, sb, c->Y, c->ldy, c->yI, c->err_flag);
         t.done(k); *kernels += k;
     }
     {
         StageTimer t(c, CASGD_STAGE_GRAM);
         if (c->opt_gram_impl == 1) {
-            k = launch_gram_simt(c->stream, c->Y, c->ldy, c->n, sb, b, c->xbf, c->G, c->ldg, c->r, (int)c->opt_full_lower);
+            k = launch_gram_simt(st, c->Y, c->ldy, c->n, sb, b, c->xbf, c->G, c->ldg, c->r, (int)c->opt_full_lower);
         } else {
             if (!c->tc_plan) {
-                c->tc_plan = gram_tc_plan_create(c->Y, c->ldy, c->n, c->rows_alloc, c->xbf, c->err, sizeof c->err);
+                c->tc_plan = gram_tc_plan_create(c->Y, c->ldy, c->n, c->rows_alloc, c->xbf, c->ldxb, c->err, sizeof c->err);
                 if (!c->tc_plan) return CASGD_ECUDA;
             }
-            k = launch_gram_tc(c->stream, c->tc_plan, sb, b, c->G, c->ldg, c->r, (int)c->opt_full_lower, c->err, sizeof c->err);
+            k = launch_gram_tc(st, c->tc_plan, sb, b, c->G, c->ldg, c->r, (int)c->opt_full_lower, (int)c->opt_ksplit, c->err, sizeof c->err);
             if (k < 0) return CASGD_ECUDA;
         }
         t.done(k); *kernels += k;
     }
     {
         StageTimer t(c, CASGD_STAGE_RECURRENCE);
-        k = launch_recurrence(c->stream, c->G, c->ldg, c->r, c->yI, s, b, alpha, c->loss, c->z, c->u);
+        k = launch_recurrence(st, c->G, c->ldg, c->r, c->yI, s, b, alpha, c->loss, c->z, c->u);
         t.done(k); *kernels += k;
     }
     {
         StageTimer t(c, CASGD_STAGE_GRADIENT);
-        k = launch_gradient_bf16(c->stream, c->Y, c->ldy, c->n, sb, c->u, alpha, x, ind, c->xbf, c->gws);
+        k = launch_gradient_bf16(st, c->Y, c->ldy, c->n, sb, c->u, alpha, x, ind, c->xbf, c->gws);
         t.done(k); *kernels += k;
     }
     return CASGD_OK;
@@ -233,14 +235,17 @@ int get_graph(casgd_ctx *c, int32_t s, int32_t b, float eta, int32_t len, GraphE
     auto it = c->graphs.find(key);
     if (it != c->graphs.end()) { *out = it->second; return CASGD_OK; }
     cudaGraph_t graph = nullptr;
-    CK(cudaStreamBeginCapture(c->stream, cudaStreamCaptureModeThreadLocal));
+    // captured on a stream of the library's own (the caller's may be the legacy default stream, which cannot
+    // be captured); nothing runs during capture, and replays are launched on the caller's stream
+    if (!c->capture_stream) CK(cudaStreamCreateWithFlags(&c->capture_stream, cudaStreamNonBlocking));
+    CK(cudaStreamBeginCapture(c->capture_stream, cudaStreamCaptureModeThreadLocal));
     int64_t kernels = 0;
     int rc = CASGD_OK;
     const int64_t saved = c->launches;
     for (int32_t h = 0; h < len && rc == CASGD_OK; ++h)
-        rc = enqueue_step(c, nullptr, c->ind, (int64_t)h * s * b, nullptr, s, b, eta, &kernels);
+        rc = enqueue_step(c, c->capture_stream, nullptr, c->ind, (int64_t)h * s * b, nullptr, s, b, eta, &kernels);
     c->launches = saved;                      // capture launches nothing; replays are counted
-    cudaError_t e = cudaStreamEndCapture(c->stream, &graph);
+    cudaError_t e = cudaStreamEndCapture(c->capture_stream, &graph);
     if (rc != CASGD_OK) { if (graph) cudaGraphDestroy(graph); return rc; }
     if (e != cudaSuccess) return fail(c, CASGD_ECUDA, "cudaStreamEndCapture: %s", cudaGetErrorString(e));
     GraphEntry ge{nullptr, kernels};
@@ -269,6 +274,7 @@ int run_steps(casgd_ctx *c, const int32_t *idx, int64_t n_steps, float *x, int32
               bool allow_graph)
 {
     const int32_t sb = s * b;
+    if (n_steps == 0) return CASGD_OK;
     int rc = ensure_workspace(c, sb);
     if (rc) return rc;
     rc = ensure_shadow(c, x);
@@ -294,7 +300,7 @@ int run_steps(casgd_ctx *c, const int32_t *idx, int64_t n_steps, float *x, int32
     }
     for (; done < n_steps; ++done) {
         int64_t kernels = 0;
-        rc = enqueue_step(c, idx + done * sb, nullptr, 0, x, s, b, eta, &kernels);
+        rc = enqueue_step(c, c->stream, idx + done * sb, nullptr, 0, x, s, b, eta, &kernels);
         if (rc) return rc;
     }
     CK(cudaGetLastError());
@@ -341,7 +347,8 @@ int casgd_init(casgd_ctx **out, const uint16_t *X_bf16, int64_t ldx, const float
         c->A = c->A_owned;
         c->lda = lda;
     }
-    const size_t xbf_elems = (size_t)round_up(n, 64) + 64;
+    c->ldxb = (int32_t)round_up(n, 64);
+    const size_t xbf_elems = (size_t)16 * c->ldxb;
     c->gws.ldp = c->ldy;
     c->gws.max_splits = 128;
     c->loss_max_blocks = kNumSMsB200 * 4;
@@ -430,8 +437,11 @@ int casgd_loss(casgd_ctx *c, const float *x, double *loss_host)
 {
     if (!c) return CASGD_EINVAL;
     if (!x || !loss_host) return fail(c, CASGD_EINVAL, "x and loss_host must not be null");
-    c->launches += launch_loss(c->stream, c->A, c->lda, c->y, c->m, c->n, c->loss, x, c->loss_partials,
-                               c->loss_max_blocks, c->loss_result);
+    {
+        StageTimer t(c, CASGD_STAGE_LOSS);
+        t.done(launch_loss(c->stream, c->A, c->lda, c->y, c->m, c->n, c->loss, x, c->loss_partials,
+                           c->loss_max_blocks, c->loss_result));
+    }
     CK(cudaGetLastError());
     CK(cudaMemcpyAsync(c->loss_result_host, c->loss_result, sizeof(double), cudaMemcpyDeviceToHost, c->stream));
     CK(cudaStreamSynchronize(c->stream));
@@ -504,6 +514,9 @@ int casgd_set_option(casgd_ctx *c, int option, int64_t value)
         c->opt_profile = value != 0;
         break;
     case CASGD_OPT_NO_GRAPH: c->opt_no_graph = value != 0; break;
+    case CASGD_OPT_GRAM_KSPLIT:
+        if (value < 0 || value > 64) return fail(c, CASGD_EINVAL, "CASGD_OPT_GRAM_KSPLIT must be in [0, 64]");
+        c->opt_ksplit = value; break;
     default: return fail(c, CASGD_EINVAL, "unknown option %d", option);
     }
     drop_graphs(c);
@@ -533,6 +546,7 @@ void casgd_destroy(casgd_ctx *c)
     cudaStreamSynchronize(c->stream);
     collect_events(c);
     free_step_workspace(c);
+    if (c->capture_stream) cudaStreamDestroy(c->capture_stream);
     cudaFree(c->A_owned); cudaFree(c->A32); cudaFree(c->xbf);
     cudaFree(c->gws.partial); cudaFree(c->gws.counters); cudaFree(c->ind); cudaFree(c->err_flag);
     cudaFree(c->loss_partials); cudaFree(c->loss_result); cudaFree(c->idx_stage); cudaFree(c->x_stage);

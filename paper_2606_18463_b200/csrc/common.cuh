@@ -6,6 +6,8 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 
+#include <algorithm>
+
 #include "../../include/casgd.h"
 
 namespace casgd {
@@ -139,13 +141,13 @@ int launch_widen(cudaStream_t st, const uint16_t *A, int64_t lda, int64_t m, int
 int launch_repack(cudaStream_t st, const uint16_t *X, int64_t ldx, int64_t m, int32_t n, uint16_t *A, int64_t lda);
 int launch_set_params(cudaStream_t st, StepParams *ind, const int32_t *idx, float *x);
 
-// tcgen05 Gram + margin (gram_tc.cu). `tmaps` points at device-visible-by-value tensor maps owned by
-// the caller (see casgd_api.cu); returns 0 launches and sets *unsupported when the shape is not handled.
+// tcgen05 Gram + margin (gram_tc.cu). The plan owns the TMA tensor maps of the Y workspace and of the
+// BF16 shadow (a [16 x ldxb] buffer: row 0 = x_bf, rows 1..15 zero). ksplit_opt <= 0: choose automatically.
 struct GramTcPlan;
 GramTcPlan *gram_tc_plan_create(const uint16_t *Y, int32_t ldy, int32_t n, int32_t sb_rows_alloc,
-                                const uint16_t *xbf, char *err, int errlen);
+                                const uint16_t *xbf, int32_t ldxb, char *err, int errlen);
 void gram_tc_plan_destroy(GramTcPlan *p);
 int launch_gram_tc(cudaStream_t st, GramTcPlan *plan, int32_t sb, int32_t b, float *G, int32_t ldg, float *r,
-                   int full_lower, char *err, int errlen);
+                   int full_lower, int ksplit_opt, char *err, int errlen);
 
 }  // namespace casgd

@@ -1,13 +1,388 @@
-// gram_tc.cu -- placeholder until the tcgen05 kernel lands (next commit).
+// gram_tc.cu -- Alg. 1 lines 3-4 on the 5th-generation tensor cores:
+//   G = Y Y^T (lower-triangular 128x128 tiles only; BF16 operands, FP32 accumulation in TMEM) with the
+//   margin r = Y x_bf fused in: on the diagonal tile of each row block the B operand carries 16 extra
+//   rows, the first of which is x_bf (BASELINE.json:north_star "carrying x as an extra B-operand column").
+//
+// One persistent CTA per SM, warp-specialised:
+//   warp 0      TMA producer: 128B-swizzled K-major boxes of Y (and of x_bf) into a 5-stage smem ring
+//   warp 1      allocates TMEM, then one lane issues tcgen05.mma (M=128, N=128/144/16, K=16, kind::f16)
+//   warps 2..5  epilogue: tcgen05.ld the FP32 accumulator (two TMEM slots, so the epilogue of tile i
+//               overlaps the MMAs of tile i+1) and store G / r
+// G = Y Y^T is a "TN" product: both operands are K-major tiles of the same matrix, so on diagonal tiles
+// one smem tile serves as A and as B. Few-tile shapes are split along K (partial sums added with red.f32).
+#include <cuda.h>
+
 #include <cstdio>
+#include <cstring>
+
 #include "common.cuh"
+
 namespace casgd {
-struct GramTcPlan { int unused; };
-GramTcPlan *gram_tc_plan_create(const uint16_t *, int32_t, int32_t, int32_t, const uint16_t *, char *err, int errlen)
+
+namespace {
+
+constexpr int BM = 128, BN = 128, BK = 64, XR = 16;
+constexpr int kStages = 5;
+constexpr uint32_t kTileBytes = BM * BK * 2;            // 16384
+constexpr uint32_t kXBytes = XR * BK * 2;               // 2048
+constexpr uint32_t kStageBytes = 2 * kTileBytes + kXBytes;
+constexpr uint32_t kOffB = 0, kOffX = kTileBytes, kOffA = kTileBytes + kXBytes;
+constexpr uint32_t kAccCols = 256;                      // TMEM columns per accumulator slot (144 used)
+constexpr uint32_t kTmemCols = 512;
+constexpr int kThreads = 192;
+constexpr size_t kSmemBytes = 1024 + (size_t)kStages * kStageBytes + 256;
+
+struct GramParams {
+    float *G;
+    float *r;
+    int32_t ldg, sb, b, n, T, ntiles, ksplit, kb_total, full_lower;
+};
+
+// ------------------------------------------------------------------------------------ PTX ---
+
+__device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
+
+__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count)
 {
-    snprintf(err, errlen, "tcgen05 Gram kernel not built yet; set CASGD_OPT_GRAM_IMPL = 1");
-    return nullptr;
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory");
 }
+__device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint32_t bar)
+{
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity)
+{
+    uint32_t ok;
+    do {
+        asm volatile("{\n.reg .pred p;\nmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\nselp.u32 %0, 1, 0, p;\n}"
+                     : "=r"(ok) : "r"(bar), "r"(parity) : "memory");
+    } while (!ok);
+}
+__device__ __forceinline__ void tma_load_2d(uint32_t dst, const CUtensorMap *map, uint32_t bar, int32_t c0, int32_t c1)
+{
+    asm volatile("cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4}], [%2];"
+                 ::"r"(dst), "l"((uint64_t)map), "r"(bar), "r"(c0), "r"(c1) : "memory");
+}
+__device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
+__device__ __forceinline__ void tc_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
+__device__ __forceinline__ void tc_commit(uint32_t bar)
+{
+    asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(bar) : "memory");
+}
+__device__ __forceinline__ void tc_mma_bf16(uint32_t d_tmem, uint64_t adesc, uint64_t bdesc, uint32_t idesc, uint32_t acc)
+{
+    asm volatile("{\n.reg .pred p;\nsetp.ne.b32 p, %4, 0;\n"
+                 "tcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p;\n}"
+                 ::"r"(d_tmem), "l"(adesc), "l"(bdesc), "r"(idesc), "r"(acc) : "memory");
+}
+__device__ __forceinline__ void tc_ld32(uint32_t taddr, uint32_t (&v)[32])
+{
+    asm volatile("tcgen05.ld.sync.aligned.32x32b.x32.b32 "
+                 "{%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, "
+                 "%16, %17, %18, %19, %20, %21, %22, %23, %24, %25, %26, %27, %28, %29, %30, %31}, [%32];"
+                 : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7]),
+                   "=r"(v[8]), "=r"(v[9]), "=r"(v[10]), "=r"(v[11]), "=r"(v[12]), "=r"(v[13]), "=r"(v[14]), "=r"(v[15]),
+                   "=r"(v[16]), "=r"(v[17]), "=r"(v[18]), "=r"(v[19]), "=r"(v[20]), "=r"(v[21]), "=r"(v[22]), "=r"(v[23]),
+                   "=r"(v[24]), "=r"(v[25]), "=r"(v[26]), "=r"(v[27]), "=r"(v[28]), "=r"(v[29]), "=r"(v[30]), "=r"(v[31])
+                 : "r"(taddr) : "memory");
+}
+__device__ __forceinline__ uint32_t tc_ld1(uint32_t taddr)
+{
+    uint32_t v;
+    asm volatile("tcgen05.ld.sync.aligned.32x32b.x1.b32 {%0}, [%1];" : "=r"(v) : "r"(taddr) : "memory");
+    return v;
+}
+__device__ __forceinline__ void tc_wait_ld() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
+
+// K-major, 128-byte swizzle: rows of 64 BF16 (128 B), 8-row groups 1024 B apart (SBO), descriptor version 1.
+__device__ __forceinline__ uint64_t umma_desc_sw128(uint32_t saddr)
+{
+    return (uint64_t)((saddr & 0x3FFFFu) >> 4) | (1ull << 16) | ((uint64_t)(1024 >> 4) << 32) | (1ull << 46) | (2ull << 61);
+}
+// kind::f16 instruction descriptor: D = F32, A = B = BF16, both K-major, M = 128, N = n_cols.
+__device__ __forceinline__ uint32_t umma_idesc(uint32_t n_cols)
+{
+    return (1u << 4) | (1u << 7) | (1u << 10) | ((n_cols >> 3) << 17) | ((uint32_t)(BM >> 4) << 24);
+}
+
+// ------------------------------------------------------------------------- work decoding ---
+
+struct Work {
+    int ti, tj, kb0, kb1;
+    bool diag, need_g, skip;
+};
+
+__device__ __forceinline__ Work decode_work(const GramParams &p, int w)
+{
+    Work k;
+    const int t = w % p.ntiles, ks = w / p.ntiles;
+    if (t < p.T) {
+        k.ti = k.tj = t;
+        k.diag = true;
+    } else {
+        const int q = t - p.T;                          // strictly-lower tiles: q = ti (ti - 1) / 2 + tj, ti >= 1
+        int ti = (int)((1.f + sqrtf(1.f + 8.f * (float)q)) * 0.5f);
+        while (ti * (ti - 1) / 2 > q) --ti;
+        while ((ti + 1) * ti / 2 <= q) ++ti;
+        k.ti = ti;
+        k.tj = q - ti * (ti - 1) / 2;
+        k.diag = false;
+    }
+    const int last_row = min(k.ti * BM + BM, p.sb) - 1;
+    k.need_g = p.full_lower || (last_row / p.b) > ((k.tj * BN) / p.b);      // holds an entry of a block below the block diagonal
+    k.skip = !k.diag && !k.need_g;
+    k.kb0 = (int)(((int64_t)ks * p.kb_total) / p.ksplit);
+    k.kb1 = (int)(((int64_t)(ks + 1) * p.kb_total) / p.ksplit);
+    return k;
+}
+
+// ------------------------------------------------------------------------------- kernel ---
+
+__global__ void __launch_bounds__(kThreads, 1)
+gram_tc_kernel(const __grid_constant__ CUtensorMap tmY, const __grid_constant__ CUtensorMap tmX, const GramParams p)
+{
+    extern __shared__ uint8_t smem_raw[];
+    const uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;
+    const uint32_t bar_base = smem_base + kStages * kStageBytes;
+    auto full_bar = [&](int s) { return bar_base + 8u * s; };
+    auto empty_bar = [&](int s) { return bar_base + 8u * (kStages + s); };
+    auto accf_bar = [&](int s) { return bar_base + 8u * (2 * kStages + s); };
+    auto acce_bar = [&](int s) { return bar_base + 8u * (2 * kStages + 2 + s); };
+    const uint32_t tmem_slot = bar_base + 8u * (2 * kStages + 4);
+    volatile uint32_t *tmem_slot_ptr =
+        reinterpret_cast<volatile uint32_t *>(smem_raw + (tmem_slot - smem_u32(smem_raw)));
+
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int nwork = p.ntiles * p.ksplit;
+
+    if (warp == 0 && lane == 0) {
+        for (int s = 0; s < kStages; ++s) { mbar_init(full_bar(s), 1); mbar_init(empty_bar(s), 1); }
+        for (int s = 0; s < 2; ++s) { mbar_init(accf_bar(s), 1); mbar_init(acce_bar(s), 4); }
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        asm volatile("prefetch.tensormap [%0];" ::"l"((uint64_t)&tmY) : "memory");
+        asm volatile("prefetch.tensormap [%0];" ::"l"((uint64_t)&tmX) : "memory");
+    }
+    if (warp == 1) {
+        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(tmem_slot), "r"(kTmemCols) : "memory");
+        asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+    }
+    tc_fence_before();
+    __syncthreads();
+    tc_fence_after();
+    const uint32_t tmem_base = *tmem_slot_ptr;
+
+    if (warp == 0) {
+        // ===== TMA producer =====
+        if (lane == 0) {
+            int stage = 0;
+            uint32_t phase = 0;
+            for (int w = blockIdx.x; w < nwork; w += gridDim.x) {
+                const Work k = decode_work(p, w);
+                if (k.skip) continue;
+                for (int kb = k.kb0; kb < k.kb1; ++kb) {
+                    mbar_wait(empty_bar(stage), phase ^ 1u);
+                    const uint32_t sbase = smem_base + stage * kStageBytes;
+                    if (k.diag) {
+                        mbar_expect_tx(full_bar(stage), kTileBytes + kXBytes);
+                        tma_load_2d(sbase + kOffB, &tmY, full_bar(stage), kb * BK, k.ti * BM);
+                        tma_load_2d(sbase + kOffX, &tmX, full_bar(stage), kb * BK, 0);
+                    } else {
+                        mbar_expect_tx(full_bar(stage), 2 * kTileBytes);
+                        tma_load_2d(sbase + kOffB, &tmY, full_bar(stage), kb * BK, k.tj * BN);
+                        tma_load_2d(sbase + kOffA, &tmY, full_bar(stage), kb * BK, k.ti * BM);
+                    }
+                    if (++stage == kStages) { stage = 0; phase ^= 1u; }
+                }
+            }
+        }
+    } else if (warp == 1) {
+        // ===== MMA issuer =====
+        if (lane == 0) {
+            int stage = 0;
+            uint32_t phase = 0;
+            int it = 0;
+            for (int w = blockIdx.x; w < nwork; w += gridDim.x) {
+                const Work k = decode_work(p, w);
+                if (k.skip) continue;
+                const int slot = it & 1;
+                const uint32_t acc_phase = (uint32_t)(it >> 1) & 1u;
+                ++it;
+                mbar_wait(acce_bar(slot), acc_phase ^ 1u);
+                tc_fence_after();
+                const uint32_t d_tmem = tmem_base + slot * kAccCols;
+                // diagonal tile: A = B = the same smem tile; N = 144 (G tile + margin rows) or 16 (margin only)
+                const uint32_t ncols = k.diag ? (k.need_g ? (uint32_t)(BN + XR) : (uint32_t)XR) : (uint32_t)BN;
+                const uint32_t idesc = umma_idesc(ncols);
+                for (int kb = k.kb0; kb < k.kb1; ++kb) {
+                    mbar_wait(full_bar(stage), phase);
+                    tc_fence_after();
+                    const uint32_t sbase = smem_base + stage * kStageBytes;
+                    const uint64_t adesc = umma_desc_sw128(sbase + (k.diag ? kOffB : kOffA));
+                    const uint64_t bdesc = umma_desc_sw128(sbase + ((k.diag && !k.need_g) ? kOffX : kOffB));
+                    const int kcols = min(p.n - kb * BK, BK);
+                    const int ksteps = (kcols + 15) >> 4;                  // zero-filled K tail beyond n is skipped
+                    for (int ks = 0; ks < ksteps; ++ks)
+                        tc_mma_bf16(d_tmem, adesc + 2u * ks, bdesc + 2u * ks, idesc, (kb > k.kb0 || ks > 0) ? 1u : 0u);
+                    tc_commit(empty_bar(stage));                           // frees the smem slot when the MMAs retire
+                    if (++stage == kStages) { stage = 0; phase ^= 1u; }
+                }
+                tc_commit(accf_bar(slot));                                 // accumulator ready for the epilogue
+            }
+        }
+    } else {
+        // ===== epilogue warps: TMEM lane group (warp % 4), one accumulator row per thread =====
+        const int q = warp & 3;
+        int it = 0;
+        const bool accumulate = p.ksplit > 1;
+        for (int w = blockIdx.x; w < nwork; w += gridDim.x) {
+            const Work k = decode_work(p, w);
+            if (k.skip) continue;
+            const int slot = it & 1;
+            const uint32_t acc_phase = (uint32_t)(it >> 1) & 1u;
+            ++it;
+            mbar_wait(accf_bar(slot), acc_phase);
+            tc_fence_after();
+            const uint32_t t_row = tmem_base + ((uint32_t)(q * 32) << 16) + slot * kAccCols;
+            const int row = k.ti * BM + q * 32 + lane;
+            const bool row_ok = row < p.sb;
+            if (k.need_g) {
+                float *grow = p.G + (int64_t)row * p.ldg + k.tj * BN;
+#pragma unroll 1
+                for (int c = 0; c < BN / 32; ++c) {
+                    uint32_t v[32];
+                    tc_ld32(t_row + c * 32, v);
+                    tc_wait_ld();
+                    if (row_ok) {
+                        if (!accumulate) {
+#pragma unroll
+                            for (int e = 0; e < 32; e += 4)
+                                *reinterpret_cast<uint4 *>(grow + c * 32 + e) = make_uint4(v[e], v[e + 1], v[e + 2], v[e + 3]);
+                        } else {
+#pragma unroll
+                            for (int e = 0; e < 32; ++e) atomicAdd(grow + c * 32 + e, __uint_as_float(v[e]));
+                        }
+                    }
+                }
+            }
+            if (k.diag) {
+                const uint32_t rv = tc_ld1(t_row + (k.need_g ? BN : 0));
+                tc_wait_ld();
+                if (row_ok) {
+                    if (!accumulate) p.r[row] = __uint_as_float(rv);
+                    else atomicAdd(p.r + row, __uint_as_float(rv));
+                }
+            }
+            tc_fence_before();
+            __syncwarp();
+            if (lane == 0) mbar_arrive(acce_bar(slot));
+        }
+    }
+
+    tc_fence_before();
+    __syncthreads();
+    if (warp == 1) {
+        tc_fence_after();
+        asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "r"(kTmemCols) : "memory");
+    }
+}
+
+typedef CUresult (*EncodeTiledFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *,
+                                  const cuuint64_t *, const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave,
+                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+EncodeTiledFn encode_tiled_fn()
+{
+    static EncodeTiledFn fn = nullptr;
+    if (!fn) {
+        void *sym = nullptr;
+        cudaDriverEntryPointQueryResult qres;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &sym, cudaEnableDefault, &qres) == cudaSuccess &&
+            qres == cudaDriverEntryPointSuccess)
+            fn = (EncodeTiledFn)sym;
+    }
+    return fn;
+}
+
+bool make_bf16_map(CUtensorMap *map, const void *base, uint64_t cols, uint64_t rows, uint64_t row_stride_elems,
+                   uint32_t box_cols, uint32_t box_rows)
+{
+    EncodeTiledFn fn = encode_tiled_fn();
+    if (!fn) return false;
+    cuuint64_t dims[2] = {cols, rows};
+    cuuint64_t strides[1] = {row_stride_elems * 2};
+    cuuint32_t box[2] = {box_cols, box_rows};
+    cuuint32_t estr[2] = {1, 1};
+    return fn(map, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, const_cast<void *>(base), dims, strides, box, estr,
+              CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+              CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+}
+
+}  // namespace
+
+struct GramTcPlan {
+    CUtensorMap tmY, tmX;
+    int32_t n, rows_alloc;
+    bool attr_set;
+};
+
+// Y: [rows_alloc x ldy] BF16 (pad columns zero), xbf: [16 x ldxb] BF16 whose row 0 is the shadow and rows 1..15 zero.
+GramTcPlan *gram_tc_plan_create(const uint16_t *Y, int32_t ldy, int32_t n, int32_t rows_alloc, const uint16_t *xbf,
+                                int32_t ldxb, char *err, int errlen)
+{
+    GramTcPlan *pl = new GramTcPlan;
+    pl->n = n;
+    pl->rows_alloc = rows_alloc;
+    pl->attr_set = false;
+    // inner extent n: the K tail of the last 64-wide box is zero-filled by TMA
+    if (!make_bf16_map(&pl->tmY, Y, (uint64_t)n, (uint64_t)rows_alloc, (uint64_t)ldy, BK, BM) ||
+        !make_bf16_map(&pl->tmX, xbf, (uint64_t)n, (uint64_t)XR, (uint64_t)ldxb, BK, XR)) {
+        snprintf(err, errlen, "cuTensorMapEncodeTiled failed (n = %d, ldy = %d, rows = %d)", n, ldy, rows_alloc);
+        delete pl;
+        return nullptr;
+    }
+    return pl;
+}
+
 void gram_tc_plan_destroy(GramTcPlan *p) { delete p; }
-int launch_gram_tc(cudaStream_t, GramTcPlan *, int32_t, int32_t, float *, int32_t, float *, int, char *, int) { return -1; }
+
+int launch_gram_tc(cudaStream_t st, GramTcPlan *plan, int32_t sb, int32_t b, float *G, int32_t ldg, float *r,
+                   int full_lower, int ksplit_opt, char *err, int errlen)
+{
+    if (!plan->attr_set) {
+        cudaError_t e = cudaFuncSetAttribute(gram_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemBytes);
+        if (e != cudaSuccess) {
+            snprintf(err, errlen, "cudaFuncSetAttribute(gram_tc_kernel): %s", cudaGetErrorString(e));
+            return -1;
+        }
+        plan->attr_set = true;
+    }
+    GramParams p;
+    p.G = G; p.r = r; p.ldg = ldg; p.sb = sb; p.b = b; p.n = plan->n;
+    p.T = (sb + BM - 1) / BM;
+    p.ntiles = p.T * (p.T + 1) / 2;
+    p.kb_total = (plan->n + BK - 1) / BK;
+    p.full_lower = full_lower;
+    int ksplit = ksplit_opt;
+    if (ksplit <= 0) {
+        // fill the 148 SMs when there are few tiles, keeping >= 4 K-blocks (256 columns) per slice
+        ksplit = kNumSMsB200 / p.ntiles;
+        ksplit = std::min(ksplit, p.kb_total / 4);
+    }
+    ksplit = std::max(1, std::min(ksplit, p.kb_total));
+    p.ksplit = ksplit;
+    int launches = 1;
+    if (ksplit > 1) {
+        // partial sums are added with red.global.add.f32: clear the rows of G and r this step writes
+        cudaMemsetAsync(G, 0, sizeof(float) * (size_t)p.T * BM * ldg, st);
+        cudaMemsetAsync(r, 0, sizeof(float) * (size_t)p.T * BM, st);
+    }
+    const int grid = std::min(p.ntiles * ksplit, kNumSMsB200);
+    gram_tc_kernel<<<grid, kThreads, kSmemBytes, st>>>(plan->tmY, plan->tmX, p);
+    return launches;
+}
+
 }  // namespace casgd

@@ -1,0 +1,228 @@
+"""GPU parity: the CUDA path (through the C ABI) against the FP64 oracle, element by element, on the same
+seeded inputs. Sizes here are ones the oracle finishes in seconds and that still span several 128-row
+Gram tiles and a ragged tail; tests/test_gpu_fullsize.py covers BASELINE.json's full sizes on sampled
+outputs. Tolerances: tests/gpu_common.py (BASELINE.json:north_star)."""
+import math
+
+import numpy as np
+import pytest
+import torch
+
+from paper_2606_18463_b200 import synth
+
+from gpu_common import (TOL_FINAL_LOSS, TOL_LOSS_CALL, check_step_against_oracle, device_dataset, random_x,
+                        require_cuda)
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def binding():
+    require_cuda()
+    from paper_2606_18463_b200 import build
+    build.build()
+    from paper_2606_18463_b200 import binding as b
+    b.load()
+    return b
+
+
+# (config index, m, n, s, b): down-sized rows, BASELINE shapes of (n, b); sb spans several tiles + a tail
+SMALL = [
+    (0, 8192, 64, 4, 16),        # configs[0] as is
+    (1, 20000, 18, 4, 64),       # SUSY-shaped: n = 18 goes through the padded repack
+    (1, 20000, 18, 5, 64),       # sb = 320: ragged tail of a 128-row tile
+    (2, 3000, 4096, 3, 128),     # dense linear, full n
+    (3, 5000, 2000, 9, 32),      # epsilon-shaped, n = 2000: ragged K tail (2000 = 31*64 + 16)
+    (4, 6000, 512, 5, 64),       # Poisson
+    (4, 6000, 512, 1, 64),       # s = 1: plain mini-batch SGD with a BF16 shadow
+    (0, 4096, 64, 7, 1),         # b = 1
+    (3, 3000, 203, 11, 13),      # odd n, odd b: nothing aligned
+]
+
+
+@pytest.mark.parametrize("gram_impl", [0, 1], ids=["umma", "simt"])
+@pytest.mark.parametrize("ci,m,n,s,b", SMALL)
+def test_one_outer_step_matches_the_oracle(binding, oracle_mod, ci, m, n, s, b, gram_impl):
+    cfg = synth.config(ci, m=m, n=n)
+    X_d, y_d, A_bits, y = device_dataset(cfg)
+    with binding.Casgd(X_d, y_d, cfg.loss) as cg:
+        cg.set_option(binding.OPT_GRAM_IMPL, gram_impl)
+        idx = np.random.default_rng(42).permutation(m)[: s * b].astype(np.int32)      # without replacement
+        # from x = 0 (first block has the closed form u_0 = l'(0, y)) and from a generic iterate
+        for x0 in (np.zeros(n, np.float32), random_x(n, 7, 0.5 if cfg.loss != synth.POISSON else 0.2)):
+            check_step_against_oracle(oracle_mod, cg, A_bits, y, idx, x0, s, b, cfg.eta, cfg.loss, binding)
+
+
+@pytest.mark.parametrize("gram_impl", [0, 1], ids=["umma", "simt"])
+def test_full_lower_triangle_and_duplicates(binding, oracle_mod, gram_impl):
+    """i.i.d. sampling with replacement (Alg. 1 line 1) gives duplicate rows inside and
+    across blocks; with CASGD_OPT_GRAM_FULL_LOWER the whole lower triangle (diagonal G_ii = ||y_i||^2
+    included) is exported and checked."""
+    cfg = synth.config(3, m=300, n=520)
+    X_d, y_d, A_bits, y = device_dataset(cfg)
+    s, b = 6, 50
+    idx = synth.iid_indices(cfg.m, s * b, 5)
+    assert len(np.unique(idx)) < len(idx)
+    with binding.Casgd(X_d, y_d, cfg.loss) as cg:
+        cg.set_option(binding.OPT_GRAM_IMPL, gram_impl)
+        cg.set_option(binding.OPT_GRAM_FULL_LOWER, 1)
+        check_step_against_oracle(oracle_mod, cg, A_bits, y, idx, random_x(cfg.n, 3), s, b, cfg.eta, cfg.loss,
+                                  binding, full_lower=True)
+
+
+def test_gather_special_index_sets(binding, oracle_mod):
+    """idx = identity gives Y = A[:sb]; a constant idx gives equal rows; a strided X (row stride > n)
+    is used in place."""
+    cfg = synth.config(4, m=1000, n=96)
+    ds = synth.make_dataset(cfg, device="cpu")
+    wide = torch.zeros((cfg.m, 128), dtype=torch.bfloat16)
+    wide[:, :96] = ds.X_bf16
+    wide[:, 96:] = 7.0                                   # junk in the padding must never reach Y
+    X_d = wide.cuda()[:, :96]
+    assert X_d.stride(0) == 128
+    y_d = ds.y.cuda()
+    A_bits = ds.X_bits_numpy()
+    x = torch.zeros(cfg.n, device="cuda")
+    with binding.Casgd(X_d, y_d, cfg.loss) as cg:
+        idx = np.arange(256, dtype=np.int32)
+        cg.outer_step(torch.from_numpy(idx).cuda(), x, 4, 64, 0.0)
+        assert np.array_equal(cg.debug(binding.DBG_Y), A_bits[:256])
+        idx = np.full(256, 17, np.int32)
+        cg.outer_step(torch.from_numpy(idx).cuda(), x, 4, 64, 0.0)
+        Y = cg.debug(binding.DBG_Y)
+        assert np.array_equal(Y, np.broadcast_to(A_bits[17], (256, 96)))
+        assert torch.count_nonzero(x).item() == 0        # eta = 0 leaves x alone
+
+
+def test_out_of_range_index_is_reported_not_read(binding):
+    cfg = synth.config(0, m=512, n=64)
+    X_d, y_d, A_bits, y = device_dataset(cfg)
+    with binding.Casgd(X_d, y_d, cfg.loss) as cg:
+        idx = np.arange(64, dtype=np.int32)
+        idx[5] = cfg.m
+        idx[9] = -1
+        x = torch.zeros(cfg.n, device="cuda")
+        cg.outer_step(torch.from_numpy(idx).cuda(), x, 4, 16, 0.5)
+        with pytest.raises(binding.CasgdError) as e:
+            cg.sync()
+        assert e.value.status == binding.EINDEX
+        Y = cg.debug(binding.DBG_Y)
+        assert not Y[5].any() and not Y[9].any() and np.array_equal(Y[6], A_bits[6])
+        cg.sync()                                        # the flag is cleared by the failing sync
+
+
+def test_bad_arguments_are_rejected_before_any_launch(binding):
+    cfg = synth.config(0, m=256, n=64)
+    X_d, y_d, _, _ = device_dataset(cfg)
+    with binding.Casgd(X_d, y_d, cfg.loss) as cg:
+        x = torch.zeros(cfg.n, device="cuda")
+        idx = torch.zeros(64, dtype=torch.int32, device="cuda")
+        before = cg.launch_count()
+        lib, ctx = cg._lib, cg._ctx
+        assert lib.casgd_outer_step(ctx, idx.data_ptr(), x.data_ptr(), 0, 16, 0.5) == binding.EINVAL
+        assert lib.casgd_outer_step(ctx, idx.data_ptr(), x.data_ptr(), 4, 0, 0.5) == binding.EINVAL
+        assert lib.casgd_outer_step(ctx, None, x.data_ptr(), 4, 16, 0.5) == binding.EINVAL
+        assert lib.casgd_outer_step(ctx, idx.data_ptr(), x.data_ptr(), 4, 16, float("nan")) == binding.EINVAL
+        assert lib.casgd_outer_step(ctx, idx.data_ptr(), x.data_ptr(), 2, binding.MAX_SB, 0.5) == binding.EINVAL
+        assert lib.casgd_outer_steps(ctx, idx.data_ptr(), -1, x.data_ptr(), 4, 16, 0.5) == binding.EINVAL
+        assert cg.launch_count() == before
+        cg.outer_steps(idx, x, 4, 16, 0.5, n_steps=0)    # zero steps: a no-op
+        assert cg.launch_count() == before
+
+
+@pytest.mark.parametrize("ci,m,n", [(0, 8192, 64), (1, 30000, 18), (2, 4000, 1024), (3, 6000, 2000), (4, 20000, 512)])
+def test_full_loss_matches_the_oracle(binding, oracle_mod, ci, m, n):
+    cfg = synth.config(ci, m=m, n=n)
+    X_d, y_d, A_bits, y = device_dataset(cfg)
+    with binding.Casgd(X_d, y_d, cfg.loss) as cg:
+        F0 = cg.loss(torch.zeros(n, device="cuda"))
+        closed = {0: math.log(2.0), 1: float(np.mean(y.astype(np.float64) ** 2) / 2), 2: 1.0}[cfg.loss]
+        assert F0 == pytest.approx(closed, rel=1e-6)                       # F(0) in closed form
+        x = random_x(n, 11, 0.3)
+        F = cg.loss(torch.from_numpy(x).cuda())
+        ref = oracle_mod.full_loss(A_bits, y, x.astype(np.float64), cfg.loss)
+        assert abs(F - ref) <= TOL_LOSS_CALL * abs(ref)
+
+
+@pytest.mark.parametrize("ci,m,n", [(1, 20000, 18), (2, 4200, 4096), (4, 6000, 512)])
+def test_fp32_sgd_baseline_matches_the_oracle(binding, oracle_mod, ci, m, n):
+    """casgd_sgd_steps_fp32 is Alg. 1 with s = 1 and no BF16 shadow (Recipe A): O2 with shadow off."""
+    cfg = synth.config(ci, m=m, n=n)
+    X_d, y_d, A_bits, y = device_dataset(cfg)
+    steps = 6
+    idx = synth.epoch_indices(cfg, 42, 0)[: steps * cfg.b].copy()
+    x0 = random_x(n, 2, 0.1)
+    with binding.Casgd(X_d, y_d, cfg.loss) as cg:
+        x_d = torch.from_numpy(x0.copy()).cuda()
+        cg.sgd_steps_fp32(torch.from_numpy(idx).cuda(), x_d, cfg.b, cfg.eta)
+        cg.sync()
+        ref = oracle_mod.train(A_bits, y, idx, x0.astype(np.float64), 1, cfg.b, cfg.eta, cfg.loss, shadow=False)
+        x1 = x_d.cpu().numpy().astype(np.float64)
+        assert np.linalg.norm(x1 - ref) <= 1e-5 * np.linalg.norm(ref)
+
+
+def test_graph_replay_and_host_entry_point_equal_single_steps(binding):
+    """casgd_outer_steps (CUDA-graph replay) and casgd_outer_steps_host run the same kernels as repeated
+    casgd_outer_step: bitwise-equal x (every reduction in the library has a fixed order)."""
+    cfg = synth.config(4, m=20000, n=512)
+    X_d, y_d, _, _ = device_dataset(cfg)
+    s, b, steps = 8, 64, 21                     # 21 = 8 + 8 + 5 singles: exercises both graph lengths
+    idx = synth.epoch_indices(cfg, 42, 0)[: steps * s * b].copy()
+    idx_d = torch.from_numpy(idx).cuda()
+    with binding.Casgd(X_d, y_d, cfg.loss) as cg:
+        xa = torch.zeros(cfg.n, device="cuda")
+        for h in range(steps):
+            cg.outer_step(idx_d[h * s * b:(h + 1) * s * b], xa, s, b, cfg.eta)
+        xb = torch.zeros(cfg.n, device="cuda")
+        n0 = cg.launch_count()
+        cg.outer_steps(idx_d, xb, s, b, cfg.eta)
+        assert cg.launch_count() > n0
+        cg.sync()
+        assert torch.equal(xa, xb)
+        xh = torch.zeros(cfg.n).pin_memory()
+        cg.outer_steps_host(torch.from_numpy(idx).pin_memory(), xh, s, b, cfg.eta)
+        assert torch.equal(xa.cpu(), xh)
+
+
+def _train_gpu(binding, cg, cfg, idx, s):
+    x = torch.zeros(cfg.n, device="cuda")
+    cg.invalidate_shadow()
+    cg.outer_steps(torch.from_numpy(idx).cuda(), x, s, cfg.b, cfg.eta)
+    cg.sync()
+    return x
+
+
+def test_config1_training_loss_matches_the_trajectory_oracle(binding, oracle_mod):
+    """BASELINE.json:configs[0] in full: 5 epochs = 640 outer steps from x = 0; final F within 0.5 %."""
+    cfg = synth.config(0)
+    X_d, y_d, A_bits, y = device_dataset(cfg)
+    idx = synth.training_indices(cfg, seed=42)
+    s = cfg.s_list[0]
+    with binding.Casgd(X_d, y_d, cfg.loss) as cg:
+        x = _train_gpu(binding, cg, cfg, idx, s)
+        F_gpu = cg.loss(x)
+    x_ref = oracle_mod.train(A_bits, y, idx, np.zeros(cfg.n), s, cfg.b, cfg.eta, cfg.loss, shadow=True, form="gram")
+    F_ref = oracle_mod.full_loss(A_bits, y, x_ref, cfg.loss)
+    assert F_ref < 0.6 * math.log(2.0)                    # it trained
+    assert abs(F_gpu - F_ref) <= TOL_FINAL_LOSS * F_ref
+    # far tighter in practice; the iterate itself stays close too
+    assert np.linalg.norm(x.cpu().numpy() - x_ref) <= 1e-3 * np.linalg.norm(x_ref)
+
+
+@pytest.mark.parametrize("ci,m,n", [(1, 65536, 18), (2, 16384, 1024), (3, 16384, 2000), (4, 32768, 512)])
+def test_downsized_training_loss_across_the_s_sweep(binding, oracle_mod, ci, m, n):
+    """Configs 2-5 with fewer rows, every s of the sweep, the configured epochs: final F within 0.5 % of
+    the trajectory oracle (O2 form), and the losses of different s agree with each other."""
+    cfg = synth.config(ci, m=m, n=n)
+    X_d, y_d, A_bits, y = device_dataset(cfg)
+    idx = synth.training_indices(cfg, seed=42)
+    losses = []
+    with binding.Casgd(X_d, y_d, cfg.loss) as cg:
+        for s in cfg.s_list:
+            x = _train_gpu(binding, cg, cfg, idx, s)
+            F_gpu = cg.loss(x)
+            x_ref = oracle_mod.train(A_bits, y, idx, np.zeros(n), s, cfg.b, cfg.eta, cfg.loss, shadow=True)
+            F_ref = oracle_mod.full_loss(A_bits, y, x_ref, cfg.loss)
+            assert abs(F_gpu - F_ref) <= TOL_FINAL_LOSS * abs(F_ref), (s, F_gpu, F_ref)
+            losses.append(F_gpu)
+    assert max(losses) - min(losses) <= 1e-3 * abs(losses[0])
