@@ -236,6 +236,25 @@ def main_reference(args, cfg, s):
 
 # --------------------------------------------------------------------------------- our arm ---
 
+def replica_seed(rank):
+    """Replicas only: rank r trains its own dataset, drawn from seed 42 + r."""
+    return 42 + rank
+
+
+def max_over_ranks(values, dist, device):
+    """Element-wise MAX over ranks of a list of floats (the timing rule: the slowest rank sets the time)."""
+    if dist is None:
+        return [float(v) for v in values]
+    t = torch.tensor(list(values), dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return [float(v) for v in t.tolist()]
+
+
+def aggregate_rows_per_s(world, steps, sb, ms):
+    """Whole-job rows/s: every rank processed steps*sb rows in (max-over-ranks) ms."""
+    return world * steps * sb / (ms * 1e-3)
+
+
 def time_steps(binding, cg, idx_d, x, s, b, eta, n_steps, stream):
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     with torch.cuda.stream(stream):
@@ -264,7 +283,7 @@ def main_ours(args, cfg, s):
     from paper_2606_18463_b200 import binding
     pk = peaks()
     sb = s * cfg.b
-    seed = 42 + rank                                     # independent replicas
+    seed = replica_seed(rank)                            # independent replicas
     ds = synth.make_dataset(cfg, seed=seed, device="cuda")
     K, W = args.steps, max(args.warmup, 3)
     idx_np = step_indices(cfg, seed, W + K, sb)
@@ -289,9 +308,7 @@ def main_ours(args, cfg, s):
     launches = cg.launch_count() - l0
     if dist:
         dist.barrier()
-        t = torch.tensor([ms], device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms = float(t.item())
+    ms, = max_over_ranks([ms], dist, "cuda")
     cg.sync()
     F_after = cg.loss(x)
 
@@ -316,10 +333,7 @@ def main_ours(args, cfg, s):
         done += c
     e2e64_s = time.perf_counter() - t0
     clk = clocks.stop()
-    if dist:
-        t = torch.tensor([e2e_s, e2e64_s], device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        e2e_s, e2e64_s = (float(v) for v in t.tolist())
+    e2e_s, e2e64_s = max_over_ranks([e2e_s, e2e64_s], dist, "cuda")
 
     # ---- per-stage device times (CUDA events on the library's stream, same kernels launched directly)
     Kp = min(K, 200)
@@ -377,8 +391,8 @@ def main_ours(args, cfg, s):
             ms2 = time_steps(binding, cg, idx2[5 * sb2:], x2, s2, cfg.b, cfg.eta, k2, stream)
             sweep[f"s{s2}"] = dict(rows_per_s=k2 * sb2 / (ms2 * 1e-3), ms_per_outer_step=ms2 / k2)
 
-    value = world * K * sb / (ms * 1e-3)
-    e2e_value = world * Ke * sb / e2e_s
+    value = aggregate_rows_per_s(world, K, sb, ms)
+    e2e_value = aggregate_rows_per_s(world, Ke, sb, e2e_s * 1e3)
     line = dict(metric=METRIC, value=value, unit=UNIT, n_gpus=world, steps=K, warmup=W, ms_per_step=ms / K,
                 higher_is_better=True, scaling="weak", vs_baseline=None, dtype="bf16 in / f32 accumulate",
                 data="synthetic",
@@ -391,7 +405,7 @@ def main_ours(args, cfg, s):
                 clocks=clk,
                 e2e=dict(value=e2e_value, unit=UNIT, h2d_bytes_per_step=sb * 4 + cfg.n * 4,
                          d2h_bytes_per_step=cfg.n * 4, steps=Ke,
-                         batched64=dict(value=world * Ke * sb / e2e64_s, h2d_bytes_per_step=sb * 4 + cfg.n * 4 / 64,
+                         batched64=dict(value=aggregate_rows_per_s(world, Ke, sb, e2e64_s * 1e3), h2d_bytes_per_step=sb * 4 + cfg.n * 4 / 64,
                                         d2h_bytes_per_step=cfg.n * 4 / 64)),
                 gpu_launches=int(launches), roofline=roofline, stages=stages, gemv=gemv, sweep=sweep)
 

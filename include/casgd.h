@@ -140,10 +140,12 @@ int casgd_debug_export(casgd_ctx *c, int what, void *dst_host, int64_t dst_bytes
  *                              graph replay); read with casgd_stage_times.
  *   CASGD_OPT_NO_GRAPH         1 = casgd_outer_steps launches kernels directly instead of replaying a graph.
  *   CASGD_OPT_GRAM_KSPLIT      0 = the tcgen05 Gram kernel chooses how many slices to cut K (= n) into so that
- *                              few-tile shapes still fill the GPU; k in [1, 64] forces k slices. */
+ *                              few-tile shapes still fill the GPU; k in [1, 64] forces k slices.
+ *   CASGD_OPT_RECURRENCE_IMPL  0 = choose by the size of the strict block-lower G (default), 1 = the one-CTA
+ *                              kernel, 2 = the grid-wide kernel (one CTA per SM, cooperative launch). */
 typedef enum {
     CASGD_OPT_GRAM_IMPL = 0, CASGD_OPT_GRAM_FULL_LOWER = 1, CASGD_OPT_PROFILE = 2, CASGD_OPT_NO_GRAPH = 3,
-    CASGD_OPT_GRAM_KSPLIT = 4
+    CASGD_OPT_GRAM_KSPLIT = 4, CASGD_OPT_RECURRENCE_IMPL = 5
 } casgd_option;
 int casgd_set_option(casgd_ctx *c, int option, int64_t value);
 

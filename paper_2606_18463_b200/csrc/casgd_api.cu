@@ -62,6 +62,7 @@ struct casgd_ctx {
     const float *shadow_of = nullptr;
     bool shadow_valid = false;
     GradWorkspace gws{};
+    RecWorkspace rws{};
     StepParams *ind = nullptr;
     int *err_flag = nullptr;
     int *err_flag_host = nullptr;     // pinned
@@ -75,7 +76,7 @@ struct casgd_ctx {
     // last step, for debug export
     int32_t last_s = 0, last_b = 0;
     // options
-    int64_t opt_gram_impl = 0, opt_full_lower = 0, opt_profile = 0, opt_no_graph = 0, opt_ksplit = 0;
+    int64_t opt_gram_impl = 0, opt_full_lower = 0, opt_profile = 0, opt_no_graph = 0, opt_ksplit = 0, opt_rec_impl = 0;
     GramTcPlan *tc_plan = nullptr;
     std::map<GraphKey, GraphEntry> graphs;
     std::vector<StageEvent> events;
@@ -86,6 +87,9 @@ struct casgd_ctx {
 };
 
 namespace {
+
+constexpr int kRecReplicas = 8;
+const unsigned kEpochInit[2] = {1u, 0u};                // {epoch, done}
 
 int fail(casgd_ctx *c, int code, const char *fmt, ...)
 {
@@ -206,7 +210,9 @@ int enqueue_step(casgd_ctx *c, cudaStream_t st, const int32_t *idx, const StepPa
     }
     {
         StageTimer t(c, CASGD_STAGE_RECURRENCE);
-        k = launch_recurrence(st, c->G, c->ldg, c->r, c->yI, s, b, alpha, c->loss, c->z, c->u);
+        k = launch_recurrence(st, c->G, c->ldg, c->r, c->yI, s, b, alpha, c->loss, c->z, c->u, c->rws,
+                              (int)c->opt_rec_impl);
+        if (k < 0) return fail(c, CASGD_ECUDA, "recurrence launch: %s", cudaGetErrorString(cudaGetLastError()));
         t.done(k); *kernels += k;
     }
     {
@@ -359,6 +365,10 @@ int casgd_init(casgd_ctx **out, const uint16_t *X_bf16, int64_t ldx, const float
               ck(cudaMalloc(&c->gws.counters, sizeof(unsigned) * n_counters)) &&
               ck(cudaMemsetAsync(c->gws.counters, 0, sizeof(unsigned) * n_counters, c->stream)) &&
               ck(cudaMalloc(&c->ind, sizeof(StepParams))) &&
+              ck(cudaMalloc(&c->rws.utag, sizeof(unsigned long long) * CASGD_MAX_SB * kRecReplicas)) &&
+              ck(cudaMemsetAsync(c->rws.utag, 0, sizeof(unsigned long long) * CASGD_MAX_SB * kRecReplicas, c->stream)) &&
+              ck(cudaMalloc(&c->rws.epoch, 2 * sizeof(unsigned))) &&
+              ck(cudaMemcpyAsync(c->rws.epoch, kEpochInit, 2 * sizeof(unsigned), cudaMemcpyHostToDevice, c->stream)) &&
               ck(cudaMalloc(&c->err_flag, sizeof(int))) &&
               ck(cudaMemsetAsync(c->err_flag, 0, sizeof(int), c->stream)) &&
               ck(cudaMallocHost(&c->err_flag_host, sizeof(int))) &&
@@ -367,6 +377,11 @@ int casgd_init(casgd_ctx **out, const uint16_t *X_bf16, int64_t ldx, const float
               ck(cudaMallocHost(&c->loss_result_host, sizeof(double))) &&
               ck(cudaMalloc(&c->x_stage, sizeof(float) * (size_t)n));
     if (!ok) return bail(CASGD_ENOMEM);
+    c->rws.done = c->rws.epoch + 1;
+    c->rws.nrep = kRecReplicas;
+    c->rws.max_ctas = recurrence_max_coresident_ctas(prop.multiProcessorCount);
+    c->rws.grid_threshold_bytes = 64 * 1024;
+    if (!ck(cudaStreamSynchronize(c->stream))) return bail(CASGD_ECUDA);   // kEpochInit is consumed
     *out = c;
     return CASGD_OK;
 }
@@ -517,6 +532,9 @@ int casgd_set_option(casgd_ctx *c, int option, int64_t value)
     case CASGD_OPT_GRAM_KSPLIT:
         if (value < 0 || value > 64) return fail(c, CASGD_EINVAL, "CASGD_OPT_GRAM_KSPLIT must be in [0, 64]");
         c->opt_ksplit = value; break;
+    case CASGD_OPT_RECURRENCE_IMPL:
+        if (value < 0 || value > 2) return fail(c, CASGD_EINVAL, "CASGD_OPT_RECURRENCE_IMPL must be 0, 1 or 2");
+        c->opt_rec_impl = value; break;
     default: return fail(c, CASGD_EINVAL, "unknown option %d", option);
     }
     drop_graphs(c);
@@ -549,6 +567,7 @@ void casgd_destroy(casgd_ctx *c)
     if (c->capture_stream) cudaStreamDestroy(c->capture_stream);
     cudaFree(c->A_owned); cudaFree(c->A32); cudaFree(c->xbf);
     cudaFree(c->gws.partial); cudaFree(c->gws.counters); cudaFree(c->ind); cudaFree(c->err_flag);
+    cudaFree(c->rws.utag); cudaFree(c->rws.epoch);
     cudaFree(c->loss_partials); cudaFree(c->loss_result); cudaFree(c->idx_stage); cudaFree(c->x_stage);
     if (c->err_flag_host) cudaFreeHost(c->err_flag_host);
     if (c->loss_result_host) cudaFreeHost(c->loss_result_host);

@@ -116,8 +116,19 @@ int launch_gather(cudaStream_t st, const uint16_t *A, int64_t lda, const float *
 int launch_gram_simt(cudaStream_t st, const uint16_t *Y, int32_t ldy, int32_t n, int32_t sb, int32_t b,
                      const uint16_t *xbf, float *G, int32_t ldg, float *r, int full_lower);
 
+// Cross-SM state of the grid-wide recurrence kernel (recurrence.cu).
+struct RecWorkspace {
+    unsigned long long *utag;      // [nrep x CASGD_MAX_SB] {u value, epoch tag} words, zero at allocation
+    int32_t nrep;                  // replicas of the tagged words (spreads the polling over L2 slices)
+    unsigned *epoch;               // tag of the next launch (starts at 1); retired by the kernel itself
+    unsigned *done;                // CTAs finished in the current launch (0 between launches)
+    int32_t max_ctas;              // CTAs that can be co-resident (one per SM); 0 = grid kernel unavailable
+    int64_t grid_threshold_bytes;  // strict block-lower G at or above this size goes to the grid kernel
+};
+int recurrence_max_coresident_ctas(int num_sms);
+// impl: 0 = choose by size, 1 = one CTA, 2 = all SMs. Returns kernels launched, or -1 on a launch error.
 int launch_recurrence(cudaStream_t st, const float *G, int32_t ldg, const float *r, const float *yI, int32_t s,
-                      int32_t b, float alpha, int loss, float *z, float *u);
+                      int32_t b, float alpha, int loss, float *z, float *u, const RecWorkspace &ws, int impl);
 
 struct GradWorkspace {
     float *partial;        // [row_splits x ldp] partial column sums

@@ -3,12 +3,25 @@
 // All FP32 (the paper requires u_c = u_sigma = FP32: L236, Table 3). Only blocks k < j of G are read
 // ("strict block-lower", L180). The chain is serial in j; inside a step the b rows and the j*b-long
 // dot products are parallel.
+//
+// Two kernels:
+//   recurrence_cta_kernel   one CTA, u in shared memory, __syncthreads per step. For small G_L.
+//   recurrence_grid_kernel  all SMs (cooperative launch, one CTA per SM). Each warp owns a few rows of G
+//       (row i -> warp i mod W, so the b rows of a block sit on b different SMs) and keeps one lane-partial
+//       dot product per row in registers. u_k travels between SMs as 8-byte {value, tag} words through L2
+//       (the tag is a per-launch epoch, so a word is valid the moment it is visible: no flag, no fence,
+//       one L2 round trip per step). When u_k lands every warp adds G[row, block k] . u_k to its rows
+//       (the G loads are issued BEFORE the poll, so they are in flight while it spins), and the warps that own
+//       rows of block k+1 reduce, apply l', and publish. The whole strict block-lower G is read exactly once,
+//       by 148 SMs in parallel, instead of through one SM.
+#include <cuda/atomic>
+
 #include "common.cuh"
 
 namespace casgd {
 
-// v1: one CTA. G_{j,<j} streams from L2/HBM with 16-byte loads, u lives in shared memory,
-// warp-shuffle reductions, the loss's link derivative inlined.
+// ---------------------------------------------------------------------------- one CTA ---
+
 template <int LOSS>
 __global__ void __launch_bounds__(1024)
 recurrence_cta_kernel(const float *__restrict__ G, int32_t ldg, const float *__restrict__ r, const float *__restrict__ yI,
@@ -45,9 +58,236 @@ recurrence_cta_kernel(const float *__restrict__ G, int32_t ldg, const float *__r
     }
 }
 
-int launch_recurrence(cudaStream_t st, const float *G, int32_t ldg, const float *r, const float *yI, int32_t s,
-                      int32_t b, float alpha, int loss, float *z, float *u)
+// --------------------------------------------------------------------------- all SMs ---
+
+constexpr int kRecThreads = 256;
+constexpr int kRecWarps = kRecThreads / 32;
+
+__device__ __forceinline__ void st_tagged(unsigned long long *p, float v, uint32_t tag)
 {
+    const unsigned long long w = ((unsigned long long)tag << 32) | (unsigned long long)__float_as_uint(v);
+    asm volatile("st.relaxed.gpu.global.b64 [%0], %1;" ::"l"(p), "l"(w) : "memory");
+}
+__device__ __forceinline__ void ld_tagged_x4(const unsigned long long *p, uint32_t (&v)[4], uint32_t (&t)[4])
+{
+    // two 16-byte volatile loads: {v0, t0, v1, t1}, {v2, t2, v3, t3}; each 8-byte word was written whole
+    asm volatile("ld.volatile.global.v4.u32 {%0, %1, %2, %3}, [%4];"
+                 : "=r"(v[0]), "=r"(t[0]), "=r"(v[1]), "=r"(t[1]) : "l"(p) : "memory");
+    asm volatile("ld.volatile.global.v4.u32 {%0, %1, %2, %3}, [%4];"
+                 : "=r"(v[2]), "=r"(t[2]), "=r"(v[3]), "=r"(t[3]) : "l"(p + 2) : "memory");
+}
+__device__ __forceinline__ void ld_tagged_x1(const unsigned long long *p, uint32_t &v, uint32_t &t)
+{
+    asm volatile("ld.volatile.global.v2.u32 {%0, %1}, [%2];" : "=r"(v), "=r"(t) : "l"(p) : "memory");
+}
+
+// VEC: b % 4 == 0, so block-column offsets k*b are 16-byte aligned in G (ldg % 4 == 0) and in shared memory;
+// each lane takes 4 consecutive columns per 128-column chunk. Otherwise one column per lane per 32-column
+// chunk. MAXR bounds the rows one warp owns (ceil(sb / W)).
+// Polling: every SM spinning on the same 8 b bytes would queue on the one or two L2 slices that hold them
+// (measured: 5.8 us per step with 1184 polling warps). So (a) a CTA polls each word once -- thread c takes
+// column c and drops the value into shared memory, one __syncthreads, then all warps read it there -- and
+// (b) the producer writes `nrep` replicas 128 KB apart and CTA i polls replica i mod nrep.
+template <int LOSS, int MAXR, bool VEC>
+__global__ void __launch_bounds__(kRecThreads, 1)
+recurrence_grid_kernel(const float *__restrict__ G, int32_t ldg, const float *__restrict__ r,
+                       const float *__restrict__ yI, int32_t s, int32_t b, float alpha, float *__restrict__ z,
+                       float *__restrict__ u, unsigned long long *__restrict__ utag, int32_t nrep,
+                       unsigned *__restrict__ epoch, unsigned *__restrict__ done)
+{
+    extern __shared__ __align__(16) float u_s[];        // [s*b]: u as it arrives
+    __shared__ int s_last;
+    const uint32_t tag = *reinterpret_cast<volatile unsigned *>(epoch);
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int W = gridDim.x * kRecWarps;
+    const int gw = warp * gridDim.x + blockIdx.x;       // consecutive rows sit on different SMs
+    const int sb = s * b;
+    const int R = gw < sb ? (sb - 1 - gw) / W + 1 : 0;  // rows gw, gw + W, ..., gw + (R-1) W
+    const unsigned long long *my_rep = utag + (size_t)(blockIdx.x % nrep) * CASGD_MAX_SB;
+
+    float acc[MAXR], rv[MAXR], yv[MAXR];
+    int blk[MAXR];
+#pragma unroll
+    for (int t = 0; t < MAXR; ++t) {
+        acc[t] = 0.f;
+        const int row = gw + t * W;
+        const bool own = t < R;
+        rv[t] = own ? __ldg(r + row) : 0.f;
+        yv[t] = own ? __ldg(yI + row) : 0.f;
+        blk[t] = own ? row / b : -1;
+    }
+    int last_blk = -1;
+#pragma unroll
+    for (int t = 0; t < MAXR; ++t) last_blk = max(last_blk, blk[t]);
+    if (threadIdx.x == 0) s_last = -1;
+    __syncthreads();
+    if (lane == 0) atomicMax(&s_last, last_blk);
+    __syncthreads();
+    const int cta_last = s_last;                        // this CTA needs u_0 .. u_{cta_last - 1}
+
+    auto finalize = [&](int t, int row) {
+        const float a = warp_sum(acc[t]);               // every lane holds the sum
+        const float zz = fmaf(-alpha, a, rv[t]);
+        const float uu = lprime<LOSS>(zz, yv[t]);
+        if (lane < nrep) st_tagged(utag + (size_t)lane * CASGD_MAX_SB + row, uu, tag);   // what the other SMs wait for
+        if (lane == 0) {
+            z[row] = zz;
+            u[row] = uu;
+        }
+    };
+
+    // rows of block 0 depend on nothing
+#pragma unroll
+    for (int t = 0; t < MAXR; ++t)
+        if (blk[t] == 0) finalize(t, gw + t * W);
+
+    constexpr int CW = VEC ? 128 : 32;                  // columns per chunk
+    for (int k = 0; k < cta_last; ++k) {                // consume u_k; rows of blocks > k need it
+        const int c_first = VEC ? lane * 4 : lane;
+        const int64_t col0 = (int64_t)k * b;
+        // chunk 0 of G for this warp's rows: in flight while the CTA waits for u_k
+        float4 g4[VEC ? MAXR : 1];
+        float g1[VEC ? 1 : MAXR];
+#pragma unroll
+        for (int t = 0; t < MAXR; ++t) {
+            const bool need = blk[t] > k && c_first < b;
+            const float *gp = G + (int64_t)(gw + t * W) * ldg + col0 + c_first;
+            if (VEC) {
+                g4[t] = make_float4(0.f, 0.f, 0.f, 0.f);
+                if (need) {
+                    const uint4 w = ldg_nc_v4(gp);
+                    g4[t] = make_float4(__uint_as_float(w.x), __uint_as_float(w.y), __uint_as_float(w.z),
+                                        __uint_as_float(w.w));
+                }
+            } else {
+                g1[t] = need ? __ldcg(gp) : 0.f;
+            }
+        }
+        // the CTA's one poll of u_k
+        for (int c = threadIdx.x; c < b; c += kRecThreads) {
+            uint32_t v, tg;
+            do { ld_tagged_x1(my_rep + col0 + c, v, tg); } while (tg != tag);
+            u_s[col0 + c] = __uint_as_float(v);
+        }
+        __syncthreads();
+        if (k < last_blk) {
+            if (VEC) {
+                if (c_first < b) {
+                    const float4 uv = *reinterpret_cast<const float4 *>(u_s + col0 + c_first);
+#pragma unroll
+                    for (int t = 0; t < MAXR; ++t) {
+                        acc[t] = fmaf(g4[t].x, uv.x, acc[t]);
+                        acc[t] = fmaf(g4[t].y, uv.y, acc[t]);
+                        acc[t] = fmaf(g4[t].z, uv.z, acc[t]);
+                        acc[t] = fmaf(g4[t].w, uv.w, acc[t]);
+                    }
+                }
+            } else {
+                const float uv = c_first < b ? u_s[col0 + c_first] : 0.f;
+#pragma unroll
+                for (int t = 0; t < MAXR; ++t) acc[t] = fmaf(g1[t], uv, acc[t]);
+            }
+            // wide blocks: the remaining chunks
+            for (int c = CW + c_first; c < b; c += CW) {
+#pragma unroll
+                for (int t = 0; t < MAXR; ++t) {
+                    if (blk[t] <= k) continue;
+                    const float *gp = G + (int64_t)(gw + t * W) * ldg + col0 + c;
+                    if (VEC) {
+                        const uint4 w = ldg_nc_v4(gp);
+                        const float4 uv = *reinterpret_cast<const float4 *>(u_s + col0 + c);
+                        acc[t] = fmaf(__uint_as_float(w.x), uv.x, acc[t]);
+                        acc[t] = fmaf(__uint_as_float(w.y), uv.y, acc[t]);
+                        acc[t] = fmaf(__uint_as_float(w.z), uv.z, acc[t]);
+                        acc[t] = fmaf(__uint_as_float(w.w), uv.w, acc[t]);
+                    } else {
+                        acc[t] = fmaf(__ldcg(gp), u_s[col0 + c], acc[t]);
+                    }
+                }
+            }
+#pragma unroll
+            for (int t = 0; t < MAXR; ++t)
+                if (blk[t] == k + 1) finalize(t, gw + t * W);
+        }
+    }
+
+    // the last CTA to finish retires the epoch, which invalidates every tagged word at once
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        cuda::atomic_ref<unsigned, cuda::thread_scope_device> d(*done);
+        if (d.fetch_add(1u, cuda::memory_order_acq_rel) == gridDim.x - 1) {
+            d.store(0u, cuda::memory_order_relaxed);
+            *epoch = (tag + 1u == 0u) ? 1u : tag + 1u;  // 0 is the value of never-written words
+        }
+    }
+}
+
+int recurrence_grid_ctas(const RecWorkspace &ws, int32_t sb)
+{
+    return std::max(1, std::min(ws.max_ctas, (sb + kRecWarps - 1) / kRecWarps));
+}
+
+template <int LOSS>
+static cudaError_t launch_grid(cudaStream_t st, const float *G, int32_t ldg, const float *r, const float *yI, int32_t s,
+                               int32_t b, float alpha, float *z, float *u, const RecWorkspace &ws)
+{
+    const int sb = s * b;
+    const int grid = recurrence_grid_ctas(ws, sb);
+    const int W = grid * kRecWarps;
+    const int maxr = (sb + W - 1) / W;
+    const bool vec = (b % 4 == 0) && (ldg % 4 == 0);
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3(grid);
+    cfg.blockDim = dim3(kRecThreads);
+    cfg.dynamicSmemBytes = sizeof(float) * (size_t)sb;
+    cfg.stream = st;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeCooperative;        // every CTA must be resident: they wait on each other
+    attr[0].val.cooperative = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    auto go = [&](auto kern) {
+        static bool attr_set = false;
+        if (!attr_set) {
+            cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                                 CASGD_MAX_SB * (int)sizeof(float));
+            if (e != cudaSuccess) return e;
+            attr_set = true;
+        }
+        return cudaLaunchKernelEx(&cfg, kern, G, ldg, r, yI, s, b, alpha, z, u, ws.utag, ws.nrep, ws.epoch, ws.done);
+    };
+    if (maxr <= 2) return vec ? go(recurrence_grid_kernel<LOSS, 2, true>) : go(recurrence_grid_kernel<LOSS, 2, false>);
+    if (maxr <= 4) return vec ? go(recurrence_grid_kernel<LOSS, 4, true>) : go(recurrence_grid_kernel<LOSS, 4, false>);
+    if (maxr <= 8) return vec ? go(recurrence_grid_kernel<LOSS, 8, true>) : go(recurrence_grid_kernel<LOSS, 8, false>);
+    return vec ? go(recurrence_grid_kernel<LOSS, 16, true>) : go(recurrence_grid_kernel<LOSS, 16, false>);
+}
+
+int recurrence_max_coresident_ctas(int num_sms)
+{
+    int per_sm = 0;
+    if (cudaFuncSetAttribute(recurrence_grid_kernel<CASGD_LOGISTIC, 16, true>,
+                             cudaFuncAttributeMaxDynamicSharedMemorySize, CASGD_MAX_SB * (int)sizeof(float)) != cudaSuccess)
+        return 0;
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, recurrence_grid_kernel<CASGD_LOGISTIC, 16, true>,
+                                                      kRecThreads, CASGD_MAX_SB * sizeof(float)) != cudaSuccess || per_sm < 1)
+        return 0;
+    return num_sms;                                     // one CTA per SM
+}
+
+int launch_recurrence(cudaStream_t st, const float *G, int32_t ldg, const float *r, const float *yI, int32_t s,
+                      int32_t b, float alpha, int loss, float *z, float *u, const RecWorkspace &ws, int impl)
+{
+    const int64_t gl_bytes = 2ll * b * b * s * (s - 1);
+    const int sb = s * b;
+    // MAXR = 16 rows per warp covers CASGD_MAX_SB on >= 128 SMs; on fewer co-resident CTAs fall back
+    const bool grid_ok = ws.max_ctas > 0 && (int64_t)ws.max_ctas * kRecWarps * 16 >= sb;
+    const bool use_grid = grid_ok && (impl == 2 || (impl == 0 && gl_bytes >= ws.grid_threshold_bytes));
+    if (use_grid) {
+        cudaError_t e = loss == CASGD_LOGISTIC ? launch_grid<CASGD_LOGISTIC>(st, G, ldg, r, yI, s, b, alpha, z, u, ws)
+                      : loss == CASGD_LINEAR  ? launch_grid<CASGD_LINEAR>(st, G, ldg, r, yI, s, b, alpha, z, u, ws)
+                                              : launch_grid<CASGD_POISSON>(st, G, ldg, r, yI, s, b, alpha, z, u, ws);
+        return e == cudaSuccess ? 1 : -1;
+    }
     const size_t smem = sizeof(float) * (size_t)s * b;
     const int threads = (b >= 32) ? 1024 : 32 * ((b < 4) ? 4 : b);
     auto go = [&](auto kern) {

@@ -70,6 +70,56 @@ def test_full_lower_triangle_and_duplicates(binding, oracle_mod, gram_impl):
                                   binding, full_lower=True)
 
 
+# (config index, m, n, s, b): shapes that stress the recurrence kernels; n kept small so that O1 stays fast
+RECURRENCE = [
+    (2, 6000, 64, 32, 128),      # configs[2]'s largest block: sb = 4096, 31 dependent steps, 4 rows per warp
+    (3, 5000, 40, 64, 32),       # configs[3]: s = 64, b = 32 (a quarter of a 128-column chunk)
+    (1, 20000, 18, 32, 64),      # configs[1]: sb = 2048
+    (0, 9000, 24, 50, 13),       # b % 4 != 0: the one-column-per-lane path, ragged everything
+    (4, 6000, 32, 3, 256),       # b = 256: two 128-column chunks per block
+    (0, 20000, 16, 9, 1300),     # sb = 11700: up to 10 rows per warp
+    (0, 3000, 16, 300, 1),       # b = 1: 299 dependent steps of one column each
+]
+
+
+@pytest.mark.parametrize("rec_impl", [1, 2], ids=["cta", "grid"])
+@pytest.mark.parametrize("ci,m,n,s,b", RECURRENCE)
+def test_recurrence_kernels_match_the_oracle(binding, oracle_mod, ci, m, n, s, b, rec_impl):
+    """Both recurrence kernels (one CTA; all SMs with tagged words through L2) on the same inputs, forced
+    with CASGD_OPT_RECURRENCE_IMPL, twice in a row (the second launch sees the first one's retired epoch)."""
+    cfg = synth.config(ci, m=m, n=n)
+    X_d, y_d, A_bits, y = device_dataset(cfg)
+    eta = cfg.eta if cfg.loss != synth.POISSON else 0.01
+    with binding.Casgd(X_d, y_d, cfg.loss) as cg:
+        cg.set_option(binding.OPT_RECURRENCE_IMPL, rec_impl)
+        for rep in range(2):
+            idx = synth.iid_indices(m, s * b, 100 + rep)
+            x0 = random_x(n, 7 + rep, 0.3 if cfg.loss != synth.POISSON else 0.1)
+            check_step_against_oracle(oracle_mod, cg, A_bits, y, idx, x0, s, b, eta, cfg.loss, binding)
+
+
+def test_grid_recurrence_replays_from_a_graph(binding):
+    """The cooperative grid-wide recurrence inside casgd_outer_steps' CUDA graph gives bitwise the x of
+    single launches, and of the one-CTA kernel up to FP32 summation order."""
+    cfg = synth.config(4, m=30000, n=128)
+    X_d, y_d, _, _ = device_dataset(cfg)
+    s, b, steps = 16, 64, 19
+    idx_d = torch.from_numpy(synth.epoch_indices(cfg, 42, 0)[: steps * s * b].copy()).cuda()
+    xs = {}
+    with binding.Casgd(X_d, y_d, cfg.loss) as cg:
+        for impl in (1, 2):
+            cg.set_option(binding.OPT_RECURRENCE_IMPL, impl)
+            xa = torch.zeros(cfg.n, device="cuda")
+            for h in range(steps):
+                cg.outer_step(idx_d[h * s * b:(h + 1) * s * b], xa, s, b, cfg.eta)
+            xb = torch.zeros(cfg.n, device="cuda")
+            cg.outer_steps(idx_d, xb, s, b, cfg.eta)
+            cg.sync()
+            assert torch.equal(xa, xb)
+            xs[impl] = xa
+    assert torch.linalg.norm(xs[1] - xs[2]) <= 1e-5 * torch.linalg.norm(xs[1])
+
+
 def test_gather_special_index_sets(binding, oracle_mod):
     """idx = identity gives Y = A[:sb]; a constant idx gives equal rows; a strided X (row stride > n)
     is used in place."""
