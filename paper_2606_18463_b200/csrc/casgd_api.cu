@@ -380,6 +380,7 @@ int casgd_init(casgd_ctx **out, const uint16_t *X_bf16, int64_t ldx, const float
     c->rws.done = c->rws.epoch + 1;
     c->rws.nrep = kRecReplicas;
     c->rws.max_ctas = recurrence_max_coresident_ctas(prop.multiProcessorCount);
+    c->rws.cluster = recurrence_cluster_size();
     c->rws.grid_threshold_bytes = 64 * 1024;
     if (!ck(cudaStreamSynchronize(c->stream))) return bail(CASGD_ECUDA);   // kEpochInit is consumed
     *out = c;
@@ -533,7 +534,7 @@ int casgd_set_option(casgd_ctx *c, int option, int64_t value)
         if (value < 0 || value > 64) return fail(c, CASGD_EINVAL, "CASGD_OPT_GRAM_KSPLIT must be in [0, 64]");
         c->opt_ksplit = value; break;
     case CASGD_OPT_RECURRENCE_IMPL:
-        if (value < 0 || value > 2) return fail(c, CASGD_EINVAL, "CASGD_OPT_RECURRENCE_IMPL must be 0, 1 or 2");
+        if (value < 0 || value > 3) return fail(c, CASGD_EINVAL, "CASGD_OPT_RECURRENCE_IMPL must be in [0, 3]");
         c->opt_rec_impl = value; break;
     default: return fail(c, CASGD_EINVAL, "unknown option %d", option);
     }

@@ -123,10 +123,12 @@ struct RecWorkspace {
     unsigned *epoch;               // tag of the next launch (starts at 1); retired by the kernel itself
     unsigned *done;                // CTAs finished in the current launch (0 between launches)
     int32_t max_ctas;              // CTAs that can be co-resident (one per SM); 0 = grid kernel unavailable
-    int64_t grid_threshold_bytes;  // strict block-lower G at or above this size goes to the grid kernel
+    int32_t cluster;               // CTAs per cluster of the cluster kernel (16 or 8); 0 = unavailable
+    int64_t grid_threshold_bytes;  // strict block-lower G at or above this size leaves the one-CTA kernel
 };
+int recurrence_cluster_size();
 int recurrence_max_coresident_ctas(int num_sms);
-// impl: 0 = choose by size, 1 = one CTA, 2 = all SMs. Returns kernels launched, or -1 on a launch error.
+// impl: 0 = choose by size, 1 = one CTA, 2 = all SMs through L2, 3 = one cluster through DSMEM. Returns kernels launched, or -1 on a launch error.
 int launch_recurrence(cudaStream_t st, const float *G, int32_t ldg, const float *r, const float *yI, int32_t s,
                       int32_t b, float alpha, int loss, float *z, float *u, const RecWorkspace &ws, int impl);
 

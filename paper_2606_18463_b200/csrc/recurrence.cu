@@ -222,6 +222,193 @@ recurrence_grid_kernel(const float *__restrict__ G, int32_t ldg, const float *__
     }
 }
 
+// --------------------------------------------------------------- one thread-block cluster ---
+// The chain of s-1 dependent steps is bound by how fast u_k gets from the SMs that produce it to the SMs that
+// need it. Through L2 that hop costs ~1.5 us (measured above); between the CTAs of one cluster it is a remote
+// shared-memory store (~0.1 us). So: one cluster of C (16, else 8) CTAs runs the whole recurrence.
+//   * Every CTA holds all of u in its own shared memory, plus one mbarrier per block k that expects 4b bytes.
+//     A finished u value goes to all C copies with st.async (...mbarrier::complete_tx::bytes): the store and
+//     the barrier's byte count travel together, so consumers sleep in mbarrier.try_wait instead of hammering
+//     shared memory, and a block is usable the moment its last value lands.
+//   * Left-looking: at step j the b rows of block j are dealt to the CTAs (row q -> CTA q mod C); inside a CTA a
+//     row belongs to one warp or, when there are fewer rows than warps, to several warps that split its
+//     128-column chunks and hand their partial sums to the row's lead warp through shared memory. Each warp
+//     walks its columns oldest first, so only the newest block is ever waited for.
+//   * Steps alternate between two groups of warps (even j / odd j): while one group waits for the newest u,
+//     the other is already streaming the older columns of the next step, which hides the L2 latency of G.
+// G streams from L2 (where the Gram kernel just left it) with 4 x 16-byte loads in flight per lane.
+// Needs b % 4 == 0 (16-byte loads at block-column offsets).
+
+constexpr int kChainThreads = 512;
+constexpr int kChainWarps = kChainThreads / 32;
+constexpr int kChainGroups = 2;
+constexpr int kGroupWarps = kChainWarps / kChainGroups;
+constexpr int kChainUnroll = 4;
+
+__device__ __forceinline__ uint32_t cluster_ctarank()
+{
+    uint32_t v;
+    asm volatile("mov.u32 %0, %%cluster_ctarank;" : "=r"(v));
+    return v;
+}
+__device__ __forceinline__ uint32_t cluster_nctarank()
+{
+    uint32_t v;
+    asm volatile("mov.u32 %0, %%cluster_nctarank;" : "=r"(v));
+    return v;
+}
+__device__ __forceinline__ void cluster_sync_all()
+{
+    asm volatile("barrier.cluster.arrive.release.aligned;\n\tbarrier.cluster.wait.acquire.aligned;" ::: "memory");
+}
+__device__ __forceinline__ uint32_t mapa_u32(uint32_t local_saddr, uint32_t cta)
+{
+    uint32_t remote;
+    asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(remote) : "r"(local_saddr), "r"(cta));
+    return remote;
+}
+__device__ __forceinline__ void st_async_b32(uint32_t remote_addr, uint32_t value, uint32_t remote_bar)
+{
+    asm volatile("st.async.weak.shared::cluster.mbarrier::complete_tx::bytes.b32 [%0], %1, [%2];"
+                 ::"r"(remote_addr), "r"(value), "r"(remote_bar) : "memory");
+}
+__device__ __forceinline__ void chain_bar_wait(uint32_t bar)
+{
+    uint32_t ok;
+    do {
+        asm volatile("{\n.reg .pred p;\nmbarrier.try_wait.parity.shared::cta.b64 p, [%1], 0;\nselp.u32 %0, 1, 0, p;\n}"
+                     : "=r"(ok) : "r"(bar) : "memory");
+    } while (!ok);
+}
+
+template <int LOSS>
+__global__ void __launch_bounds__(kChainThreads, 1)
+recurrence_cluster_kernel(const float *__restrict__ G, int32_t ldg, const float *__restrict__ r,
+                          const float *__restrict__ yI, int32_t s, int32_t b, float alpha, float *__restrict__ z,
+                          float *__restrict__ u)
+{
+    extern __shared__ __align__(16) unsigned char chain_smem[];    // u_s[s*b] floats, then bars[s]
+    __shared__ volatile float part[2][kChainWarps];
+    __shared__ volatile int pflag[2][kChainWarps];                 // step whose partial sits in part[.][w]
+    __shared__ volatile int cons[kChainWarps];                     // last step whose partial the lead has read
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int C = (int)cluster_nctarank(), crank = (int)cluster_ctarank();
+    const int sb = s * b;
+    float *u_s = reinterpret_cast<float *>(chain_smem);
+    const uint32_t us_base = (uint32_t)__cvta_generic_to_shared(u_s);
+    const uint32_t bar_base = us_base + 4u * (uint32_t)sb;         // sb % 4 == 0: 8-byte aligned
+    for (int k = threadIdx.x; k < s; k += kChainThreads) {
+        asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(bar_base + 8u * k) : "memory");
+        asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar_base + 8u * k), "r"(4u * b) : "memory");
+    }
+    if (threadIdx.x < kChainWarps) {
+        pflag[0][threadIdx.x] = -1;
+        pflag[1][threadIdx.x] = -1;
+        cons[threadIdx.x] = -1;
+    }
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    __syncthreads();
+    cluster_sync_all();                                 // nobody signals a barrier that is not initialised yet
+
+    int ready = 0;                                      // blocks 0 .. ready-1 of u are complete in u_s (this warp's view)
+
+    // dot of row `row` with u over the 128-column chunks e = first, first + stride, ... counted from the END of
+    // [0, L) (e = 0 is the newest chunk), walked oldest first
+    auto dot_chunks = [&](int row, int L, int first, int stride) -> float {
+        const int nchunks = (L + 127) >> 7;
+        float acc = 0.f;
+        if (first >= nchunks) return acc;
+        const float *g = G + (int64_t)row * ldg + lane * 4;
+        int e = first + ((nchunks - 1 - first) / stride) * stride;          // the oldest of this warp's chunks
+        for (; e >= first; e -= kChainUnroll * stride) {
+            uint4 gv[kChainUnroll];
+#pragma unroll
+            for (int q = 0; q < kChainUnroll; ++q) {
+                const int eq = e - q * stride;
+                const int col = (nchunks - 1 - eq) * 128 + lane * 4;
+                gv[q] = make_uint4(0u, 0u, 0u, 0u);
+                if (eq >= first && col < L) gv[q] = ldg_nc_v4(g + (nchunks - 1 - eq) * 128);
+            }
+#pragma unroll
+            for (int q = 0; q < kChainUnroll; ++q) {
+                const int eq = e - q * stride;
+                if (eq >= first) {                                          // warp-uniform
+                    const int c0 = (nchunks - 1 - eq) * 128;
+                    const int need = (min(c0 + 128, L) - 1) / b;            // newest block this chunk touches
+                    while (ready <= need) { chain_bar_wait(bar_base + 8u * ready); ++ready; }
+                    const int col = c0 + lane * 4;
+                    if (col < L) {
+                        const float4 uv = *reinterpret_cast<const float4 *>(u_s + col);
+                        acc = fmaf(__uint_as_float(gv[q].x), uv.x, acc);
+                        acc = fmaf(__uint_as_float(gv[q].y), uv.y, acc);
+                        acc = fmaf(__uint_as_float(gv[q].z), uv.z, acc);
+                        acc = fmaf(__uint_as_float(gv[q].w), uv.w, acc);
+                    }
+                }
+            }
+        }
+        return acc;
+    };
+
+    auto publish = [&](int j, int row, float total, float rr, float yy) {
+        const float zz = fmaf(-alpha, total, rr);
+        const float uu = lprime<LOSS>(zz, yy);
+        if (lane < C && j + 1 < s)
+            st_async_b32(mapa_u32(us_base + 4u * (uint32_t)row, (uint32_t)lane), __float_as_uint(uu),
+                         mapa_u32(bar_base + 8u * (uint32_t)j, (uint32_t)lane));
+        if (lane == 0) {
+            z[row] = zz;
+            u[row] = uu;
+        }
+    };
+
+    const int nr = crank < b ? (b - crank + C - 1) / C : 0;        // rows of each block dealt to this CTA
+    const int group = warp / kGroupWarps, wg = warp % kGroupWarps;
+    if (nr >= kGroupWarps) {
+        // a warp owns whole rows
+        for (int j = group; j < s; j += kChainGroups) {
+            for (int rho = wg; rho < nr; rho += kGroupWarps) {
+                const int row = j * b + crank + rho * C;
+                const float rr = __ldg(r + row), yy = __ldg(yI + row);
+                const float acc = dot_chunks(row, j * b, 0, 1);
+                publish(j, row, warp_sum(acc), rr, yy);
+            }
+        }
+    } else if (nr > 0) {
+        // wpr warps share a row: warp h of the row takes chunks e = h, h + wpr, ...; h = 0 (which holds the newest
+        // chunk) is the lead and adds the others' partial sums
+        const int wpr = kGroupWarps / nr;
+        const int rho = wg / wpr, h = wg % wpr;
+        if (rho < nr) {
+            for (int j = group, it = 0; j < s; j += kChainGroups, ++it) {
+                const int row = j * b + crank + rho * C;
+                if (h == 0) {
+                    const float rr = __ldg(r + row), yy = __ldg(yI + row);
+                    float acc = dot_chunks(row, j * b, 0, wpr);
+                    if (lane >= 1 && lane < wpr) {                          // lane hh collects helper hh's partial
+                        while (pflag[it & 1][warp + lane] != j) { }
+                        acc += part[it & 1][warp + lane];
+                        cons[warp + lane] = j;
+                    }
+                    __syncwarp();
+                    publish(j, row, warp_sum(acc), rr, yy);
+                } else {
+                    const float p = warp_sum(dot_chunks(row, j * b, h, wpr));
+                    if (lane == 0) {
+                        while (cons[warp] < j - 2 * kChainGroups) { }       // this slot's previous value has been read
+                        part[it & 1][warp] = p;
+                        __threadfence_block();
+                        pflag[it & 1][warp] = j;
+                    }
+                    __syncwarp();
+                }
+            }
+        }
+    }
+    __syncthreads();
+    cluster_sync_all();                                 // no CTA leaves while others may still store into it
+}
+
 int recurrence_grid_ctas(const RecWorkspace &ws, int32_t sb)
 {
     return std::max(1, std::min(ws.max_ctas, (sb + kRecWarps - 1) / kRecWarps));
@@ -262,6 +449,59 @@ static cudaError_t launch_grid(cudaStream_t st, const float *G, int32_t ldg, con
     return vec ? go(recurrence_grid_kernel<LOSS, 16, true>) : go(recurrence_grid_kernel<LOSS, 16, false>);
 }
 
+template <int LOSS>
+static cudaError_t launch_cluster(cudaStream_t st, const float *G, int32_t ldg, const float *r, const float *yI,
+                                  int32_t s, int32_t b, float alpha, float *z, float *u, int cluster)
+{
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3(cluster);
+    cfg.blockDim = dim3(kChainThreads);
+    cfg.dynamicSmemBytes = sizeof(float) * (size_t)s * b + 8 * (size_t)s;
+    cfg.stream = st;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeClusterDimension;
+    attr[0].val.clusterDim.x = cluster;
+    attr[0].val.clusterDim.y = 1;
+    attr[0].val.clusterDim.z = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    return cudaLaunchKernelEx(&cfg, recurrence_cluster_kernel<LOSS>, G, ldg, r, yI, s, b, alpha, z, u);
+}
+
+template <int LOSS>
+static int cluster_size_for()
+{
+    auto kern = recurrence_cluster_kernel<LOSS>;
+    const int smem = CASGD_MAX_SB * (int)sizeof(float) + 8 * (CASGD_MAX_SB / 4);   // u_s + one mbarrier per block
+    if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem) != cudaSuccess) return 0;
+    cudaFuncSetAttribute(kern, cudaFuncAttributeNonPortableClusterSizeAllowed, 1);
+    for (int c : {16, 8}) {
+        cudaLaunchConfig_t cfg = {};
+        cfg.gridDim = dim3(c);
+        cfg.blockDim = dim3(kChainThreads);
+        cfg.dynamicSmemBytes = smem;
+        cudaLaunchAttribute attr[1];
+        attr[0].id = cudaLaunchAttributeClusterDimension;
+        attr[0].val.clusterDim.x = c;
+        attr[0].val.clusterDim.y = 1;
+        attr[0].val.clusterDim.z = 1;
+        cfg.attrs = attr;
+        cfg.numAttrs = 1;
+        int n = 0;
+        if (cudaOccupancyMaxActiveClusters(&n, kern, &cfg) == cudaSuccess && n >= 1) return c;
+    }
+    cudaGetLastError();
+    return 0;
+}
+
+// Largest cluster (16, else 8, else 0) the three instantiations of the cluster kernel can run with.
+int recurrence_cluster_size()
+{
+    const int a = cluster_size_for<CASGD_LOGISTIC>(), b = cluster_size_for<CASGD_LINEAR>(),
+              c = cluster_size_for<CASGD_POISSON>();
+    return std::min(a, std::min(b, c));
+}
+
 int recurrence_max_coresident_ctas(int num_sms)
 {
     int per_sm = 0;
@@ -281,6 +521,14 @@ int launch_recurrence(cudaStream_t st, const float *G, int32_t ldg, const float 
     const int sb = s * b;
     // MAXR = 16 rows per warp covers CASGD_MAX_SB on >= 128 SMs; on fewer co-resident CTAs fall back
     const bool grid_ok = ws.max_ctas > 0 && (int64_t)ws.max_ctas * kRecWarps * 16 >= sb;
+    const bool cluster_ok = ws.cluster > 0 && b % 4 == 0 && ldg % 4 == 0;
+    const bool use_cluster = cluster_ok && (impl == 3 || (impl == 0 && gl_bytes >= ws.grid_threshold_bytes));
+    if (use_cluster) {
+        cudaError_t e = loss == CASGD_LOGISTIC ? launch_cluster<CASGD_LOGISTIC>(st, G, ldg, r, yI, s, b, alpha, z, u, ws.cluster)
+                      : loss == CASGD_LINEAR  ? launch_cluster<CASGD_LINEAR>(st, G, ldg, r, yI, s, b, alpha, z, u, ws.cluster)
+                                              : launch_cluster<CASGD_POISSON>(st, G, ldg, r, yI, s, b, alpha, z, u, ws.cluster);
+        return e == cudaSuccess ? 1 : -1;
+    }
     const bool use_grid = grid_ok && (impl == 2 || (impl == 0 && gl_bytes >= ws.grid_threshold_bytes));
     if (use_grid) {
         cudaError_t e = loss == CASGD_LOGISTIC ? launch_grid<CASGD_LOGISTIC>(st, G, ldg, r, yI, s, b, alpha, z, u, ws)
