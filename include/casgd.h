@@ -144,7 +144,9 @@ int casgd_debug_export(casgd_ctx *c, int what, void *dst_host, int64_t dst_bytes
  *   CASGD_OPT_RECURRENCE_IMPL  0 = choose by the size of the strict block-lower G (default), 1 = the one-CTA
  *                              kernel, 2 = the grid-wide kernel (one CTA per SM, cooperative launch, u through
  *                              L2), 3 = the cluster kernel (one 16-CTA cluster, u through distributed shared
- *                              memory; needs b % 4 == 0, else falls through to 2). */
+ *                              memory, G by plain loads; needs b % 4 == 0, else falls through to 2), 4 = the
+ *                              streaming cluster kernel (same cluster, G through a cp.async.bulk shared-memory
+ *                              ring; needs b % 4 == 0 and b <= 128, else falls through to 3). */
 typedef enum {
     CASGD_OPT_GRAM_IMPL = 0, CASGD_OPT_GRAM_FULL_LOWER = 1, CASGD_OPT_PROFILE = 2, CASGD_OPT_NO_GRAPH = 3,
     CASGD_OPT_GRAM_KSPLIT = 4, CASGD_OPT_RECURRENCE_IMPL = 5

@@ -534,7 +534,7 @@ int casgd_set_option(casgd_ctx *c, int option, int64_t value)
         if (value < 0 || value > 64) return fail(c, CASGD_EINVAL, "CASGD_OPT_GRAM_KSPLIT must be in [0, 64]");
         c->opt_ksplit = value; break;
     case CASGD_OPT_RECURRENCE_IMPL:
-        if (value < 0 || value > 3) return fail(c, CASGD_EINVAL, "CASGD_OPT_RECURRENCE_IMPL must be in [0, 3]");
+        if (value < 0 || value > 4) return fail(c, CASGD_EINVAL, "CASGD_OPT_RECURRENCE_IMPL must be in [0, 4]");
         c->opt_rec_impl = value; break;
     default: return fail(c, CASGD_EINVAL, "unknown option %d", option);
     }

@@ -128,9 +128,15 @@ struct RecWorkspace {
 };
 int recurrence_cluster_size();
 int recurrence_max_coresident_ctas(int num_sms);
-// impl: 0 = choose by size, 1 = one CTA, 2 = all SMs through L2, 3 = one cluster through DSMEM. Returns kernels launched, or -1 on a launch error.
+// impl: 0 = choose by size, 1 = one CTA, 2 = all SMs through L2, 3 = one cluster, G from L2 by plain loads,
+// 4 = one cluster, G through a cp.async.bulk ring (recurrence_stream.cu). Returns kernels launched, or -1 on a launch error.
 int launch_recurrence(cudaStream_t st, const float *G, int32_t ldg, const float *r, const float *yI, int32_t s,
                       int32_t b, float alpha, int loss, float *z, float *u, const RecWorkspace &ws, int impl);
+
+// recurrence_stream.cu: one cluster, G streamed through a shared-memory ring, u through distributed shared memory.
+bool recurrence_stream_ok(int32_t s, int32_t b, int32_t ldg, int cluster);
+int launch_recurrence_stream(cudaStream_t st, const float *G, int32_t ldg, const float *r, const float *yI, int32_t s,
+                             int32_t b, float alpha, int loss, float *z, float *u, int cluster);
 
 struct GradWorkspace {
     float *partial;        // [row_splits x ldp] partial column sums

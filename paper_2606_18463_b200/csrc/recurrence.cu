@@ -522,14 +522,17 @@ int launch_recurrence(cudaStream_t st, const float *G, int32_t ldg, const float 
     // MAXR = 16 rows per warp covers CASGD_MAX_SB on >= 128 SMs; on fewer co-resident CTAs fall back
     const bool grid_ok = ws.max_ctas > 0 && (int64_t)ws.max_ctas * kRecWarps * 16 >= sb;
     const bool cluster_ok = ws.cluster > 0 && b % 4 == 0 && ldg % 4 == 0;
-    const bool use_cluster = cluster_ok && (impl == 3 || (impl == 0 && gl_bytes >= ws.grid_threshold_bytes));
+    const bool stream_ok = (impl == 4 || impl == 0) && recurrence_stream_ok(s, b, ldg, ws.cluster);
+    if (stream_ok && (impl == 4 || gl_bytes >= ws.grid_threshold_bytes))
+        return launch_recurrence_stream(st, G, ldg, r, yI, s, b, alpha, loss, z, u, ws.cluster);
+    const bool use_cluster = cluster_ok && (impl >= 3 || (impl == 0 && gl_bytes >= ws.grid_threshold_bytes));
     if (use_cluster) {
         cudaError_t e = loss == CASGD_LOGISTIC ? launch_cluster<CASGD_LOGISTIC>(st, G, ldg, r, yI, s, b, alpha, z, u, ws.cluster)
                       : loss == CASGD_LINEAR  ? launch_cluster<CASGD_LINEAR>(st, G, ldg, r, yI, s, b, alpha, z, u, ws.cluster)
                                               : launch_cluster<CASGD_POISSON>(st, G, ldg, r, yI, s, b, alpha, z, u, ws.cluster);
         return e == cudaSuccess ? 1 : -1;
     }
-    const bool use_grid = grid_ok && (impl == 2 || (impl == 0 && gl_bytes >= ws.grid_threshold_bytes));
+    const bool use_grid = grid_ok && (impl >= 2 || (impl == 0 && gl_bytes >= ws.grid_threshold_bytes));
     if (use_grid) {
         cudaError_t e = loss == CASGD_LOGISTIC ? launch_grid<CASGD_LOGISTIC>(st, G, ldg, r, yI, s, b, alpha, z, u, ws)
                       : loss == CASGD_LINEAR  ? launch_grid<CASGD_LINEAR>(st, G, ldg, r, yI, s, b, alpha, z, u, ws)

@@ -1,0 +1,505 @@
+// recurrence_stream.cu -- the s-step inner residual correction, Alg. 1 lines 6-15:
+//   for j = 0..s-1:  z_j = r_j - alpha * sum_{k<j} G_{jk} u_k ;  u_j = l'(z_j, y_{I_j})          (all FP32, L236)
+// as ONE thread-block cluster whose critical path never waits for global memory.
+//
+// The chain has s-1 dependent hops; what a hop costs is (a) how fast u_k gets from the SMs that produce it to
+// the SMs that need it and (b) whether the G values the next block needs are already on chip when it lands.
+//   (a) u travels between the CTAs of the cluster with st.async + mbarrier::complete_tx (distributed shared
+//       memory, ~0.1 us) -- every CTA holds all of u in its own shared memory and one mbarrier per block.
+//   (b) every warp streams its own part of G from L2 into a private shared-memory ring with 16-byte cp.async
+//       (LDGSTS: each lane copies, and later reads back, its own 16 bytes, so the ring needs no barrier --
+//       cp.async.wait_group is the only synchronisation), kDepth 512-byte chunks ahead of use and independent
+//       of the chain. 8 warps x kDepth 2 KB units in flight keep one SM's L2 port busy (measured: plain 16-byte
+//       loads from 16 warps reach ~80 B/cycle/SM, a single-thread cp.async.bulk producer only 1-25).
+// Rows: each block's rows are dealt to the CTAs in groups of 4 consecutive rows (group q -> CTA q mod C), so the
+// four u values of a group leave as ONE 16-byte st.async per destination CTA (measured: a hop with 4-byte stores
+// costs 850 cycles in a 16-CTA cluster, with 16-byte stores 540). Work of one CTA at step j:
+//   bulk warps (8)  every 128-column chunk of its rows but the last: these columns belong to blocks <= j-2
+//                   (whenever b divides 128 or 128 divides b), whose u landed a hop earlier -- so this runs one
+//                   hop ahead; per-row partial sums go to shared memory + an mbarrier per step;
+//   critical warps  two per owned group, taking alternate steps: the last chunk (which holds block j-1), the
+//                   bulk partials, one 5-level shuffle reduction for the 4 rows, l', and the broadcast of u.
+//                   They sit on SM sub-partitions of their own (warp id mod 4), away from the bulk warps.
+// The strict block-lower G is read exactly once (L180). Needs b % 4 == 0 and at most 4 groups per CTA.
+#include "common.cuh"
+
+namespace casgd {
+
+namespace {
+
+constexpr int kWarps = 16;
+constexpr int kThreads = 32 * kWarps;
+constexpr int kQuad = 4;                                // rows per row group: one 16-byte remote store carries their u
+constexpr int kMaxQuadsPerCta = 2;                      // row groups of one block owned by one CTA (b <= 8 * C)
+constexpr int kBulkWarps = 8;
+constexpr int kChunk = 128;                             // columns per chunk
+constexpr uint32_t kUnitBytes = kQuad * kChunk * 4u;    // one unit: 4 rows x 128 columns of G = 2 KB
+constexpr int kWin = 2;                                 // chunks of a step the critical warps take: the newest 256 columns
+constexpr int kCritPer = 3;                             // critical warps per row group, taking every third step
+constexpr int kDepth = 4;                               // bulk warp: units in flight (64 KB per CTA)
+constexpr int kCritDepth = 3;                           // critical warp: steps in flight (kWin units each)
+constexpr int kPartDepth = 40;                          // steps of partial sums kept (bulk runs < 128/b + 3 steps ahead)
+
+__device__ __forceinline__ uint32_t cluster_ctarank()
+{
+    uint32_t v;
+    asm volatile("mov.u32 %0, %%cluster_ctarank;" : "=r"(v));
+    return v;
+}
+__device__ __forceinline__ uint32_t cluster_nctarank()
+{
+    uint32_t v;
+    asm volatile("mov.u32 %0, %%cluster_nctarank;" : "=r"(v));
+    return v;
+}
+__device__ __forceinline__ void cluster_sync_all()
+{
+    asm volatile("barrier.cluster.arrive.release.aligned;\n\tbarrier.cluster.wait.acquire.aligned;" ::: "memory");
+}
+__device__ __forceinline__ uint32_t mapa_u32(uint32_t local_saddr, uint32_t cta)
+{
+    uint32_t remote;
+    asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(remote) : "r"(local_saddr), "r"(cta));
+    return remote;
+}
+__device__ __forceinline__ void st_async_b32(uint32_t remote_addr, uint32_t value, uint32_t remote_bar)
+{
+    asm volatile("st.async.weak.shared::cluster.mbarrier::complete_tx::bytes.b32 [%0], %1, [%2];"
+                 ::"r"(remote_addr), "r"(value), "r"(remote_bar) : "memory");
+}
+__device__ __forceinline__ void st_async_v4(uint32_t remote_addr, float v0, float v1, float v2, float v3, uint32_t remote_bar)
+{
+    asm volatile("st.async.weak.shared::cluster.mbarrier::complete_tx::bytes.v4.b32 [%0], {%1, %2, %3, %4}, [%5];"
+                 ::"r"(remote_addr), "r"(__float_as_uint(v0)), "r"(__float_as_uint(v1)), "r"(__float_as_uint(v2)),
+                   "r"(__float_as_uint(v3)), "r"(remote_bar) : "memory");
+}
+__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint32_t bar)
+{
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity)
+{
+    uint32_t ok;
+    do {
+        asm volatile("{\n.reg .pred p;\nmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\nselp.u32 %0, 1, 0, p;\n}"
+                     : "=r"(ok) : "r"(bar), "r"(parity) : "memory");
+    } while (!ok);
+}
+__device__ __forceinline__ void cp_async16(uint32_t dst, const void *src)
+{
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(dst), "l"(src) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+template <int N>
+__device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
+__device__ __forceinline__ float4 lds_f4(uint32_t saddr)
+{
+    float4 v;
+    asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "r"(saddr));
+    return v;
+}
+
+struct StreamLayout {                   // byte offsets into dynamic shared memory (base 128-byte aligned)
+    uint32_t u, ubar, pbar, part, cring, bring, total;
+};
+
+__host__ __device__ inline StreamLayout stream_layout(int s, int b)
+{
+    StreamLayout L;
+    uint32_t o = 0;
+    L.u = o;      o += 4u * (uint32_t)(s * b);
+    o = (o + 7u) & ~7u;
+    L.ubar = o;   o += 8u * (uint32_t)s;
+    L.pbar = o;   o += 8u * (uint32_t)s;
+    o = (o + 15u) & ~15u;
+    L.part = o;   o += 16u * (uint32_t)(kPartDepth * kMaxQuadsPerCta * kBulkWarps);     // [step % depth][quad][bulk warp][4 rows]
+    o = (o + 127u) & ~127u;
+    L.cring = o;  o += (uint32_t)(kCritPer * kMaxQuadsPerCta * kCritDepth * kWin) * kUnitBytes;
+    L.bring = o;  o += (uint32_t)(kBulkWarps * kDepth) * kUnitBytes;
+    L.total = o;
+    return L;
+}
+
+__device__ __forceinline__ int num_chunks(int j, int b) { return (j * b + kChunk - 1) / kChunk; }
+
+#ifdef CASGD_REC_TRACE
+__device__ long long g_rec_trace[8192];
+#define REC_TRACE(i) do { if (crank == 0 && warp == 0 && lane == 0 && (i) < 8192) g_rec_trace[(i)] = clock64(); } while (0)
+#define REC_TRACE_B(i) do { if (crank == 0 && warp == 2 && lane == 0 && (i) < 8192) g_rec_trace[(i)] = clock64(); } while (0)
+#else
+#define REC_TRACE_B(i) do { } while (0)
+#define REC_TRACE(i) do { } while (0)
+#endif
+
+// l' with the fast exponential and reciprocal on the chain's critical path where their error (~2^-21 relative)
+// is far inside the tolerance on u; Poisson keeps the accurate expf (its error is amplified by e^z).
+template <int LOSS>
+__device__ __forceinline__ float lprime_chain(float z, float y)
+{
+    if (LOSS == CASGD_LOGISTIC) {
+        const float t = y * z;
+        const float e = __expf(-fabsf(t));               // in (0, 1]
+        const float num = (t >= 0.f) ? e : 1.f;          // 1 / (1 + e^t) = num / (1 + e)
+        return -y * __fdividef(num, 1.f + e);
+    }
+    return lprime<LOSS>(z, y);
+}
+
+
+// Sum acc[i] (row i of the group) over the 32 lanes in five shuffle levels (six shuffles): afterwards lane l
+// holds the total of row l >> 3.
+__device__ __forceinline__ float quad_reduce(const float (&a)[kQuad], int lane)
+{
+    const bool h16 = lane & 16, h8 = lane & 8;
+    float k0 = h16 ? a[2] : a[0], k1 = h16 ? a[3] : a[1];
+    const float s0 = h16 ? a[0] : a[2], s1 = h16 ? a[1] : a[3];
+    k0 += __shfl_xor_sync(0xffffffffu, s0, 16);
+    k1 += __shfl_xor_sync(0xffffffffu, s1, 16);
+    float k = h8 ? k1 : k0;
+    const float sd = h8 ? k0 : k1;
+    k += __shfl_xor_sync(0xffffffffu, sd, 8);
+    k += __shfl_xor_sync(0xffffffffu, k, 4);
+    k += __shfl_xor_sync(0xffffffffu, k, 2);
+    k += __shfl_xor_sync(0xffffffffu, k, 1);
+    return k;
+}
+
+template <int LOSS>
+__global__ void __launch_bounds__(kThreads, 1)
+recurrence_stream_kernel(const float *__restrict__ G, int32_t ldg, const float *__restrict__ r,
+                         const float *__restrict__ yI, int32_t s, int32_t b, float alpha, float *__restrict__ z,
+                         float *__restrict__ u)
+{
+    extern __shared__ __align__(128) unsigned char rs_smem[];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int C = (int)cluster_nctarank(), crank = (int)cluster_ctarank();
+    REC_TRACE(0);
+    const StreamLayout L = stream_layout(s, b);
+    const uint32_t base = (uint32_t)__cvta_generic_to_shared(rs_smem);
+    const uint32_t us = base + L.u, ubar = base + L.ubar, pbar = base + L.pbar, part = base + L.part;
+
+    // row groups (4 consecutive rows of a block) are dealt to the CTAs: group q -> CTA q mod C
+    const int nquads = b / kQuad;
+    const int qpc = crank < nquads ? (nquads - crank + C - 1) / C : 0;     // groups of each block owned here
+    const int ndst = min(C, nquads);                                       // CTAs that own rows
+    const int bshift = (b & (b - 1)) == 0 ? __ffs(b) - 1 : -1;             // b a power of two: column -> block by shift
+    auto block_of = [&](int col) { return bshift >= 0 ? (col >> bshift) : col / b; };
+
+    for (int k = threadIdx.x; k < s; k += kThreads) {
+        mbar_init(ubar + 8u * k, 1);
+        mbar_expect_tx(ubar + 8u * k, 4u * (uint32_t)b);
+        mbar_init(pbar + 8u * k, kBulkWarps);
+    }
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+
+    // Warp w runs on scheduler w & 3. Critical warps: (group gamma, parity e) -> warp gamma + 4 e, so with up
+    // to two groups they have schedulers 0 and 1 to themselves and the eight bulk warps share 2 and 3: what the
+    // bulk warps issue when u lands (they wake on the same barrier) does not delay the chain.
+    const int wsched = warp & 3, wslot = warp >> 2;
+    const bool is_critical = wslot < kCritPer && wsched < qpc;
+    const bool is_bulk = qpc > 0 && (qpc <= 2 ? wsched >= 2 : warp >= 8);
+    const int li = lane >> 3;                           // the row of a group this lane finalises / reports
+
+    if (is_critical) {
+        // ===== critical warp: row group gamma (4 rows), steps j = e, e + kCritPer, ...; the newest kWin chunks =====
+        // While this warp finishes step j (stores, prefetch) and sets up step j + kCritPer -- including the window's
+        // older chunks, whose u is already there -- the group's next critical warp is waiting for u_j:
+        // a hop is wake + one chunk's dot + reduce + l' + one 16-byte store per CTA.
+        const int gamma = wsched, e = wslot;
+        const int q0 = kQuad * (crank + gamma * C);                 // first row of the group inside a block
+        const uint32_t ring = base + L.cring + (uint32_t)((gamma * kCritPer + e) * kCritDepth * kWin) * kUnitBytes + (uint32_t)lane * 16u;
+        const float *gbase = G + (int64_t)q0 * ldg + lane * 4;
+        // remote addresses are linear in the shared::cluster window: map the two bases once
+        const uint32_t rem_us = mapa_u32(us, (uint32_t)(lane < ndst ? lane : 0));
+        const uint32_t rem_ubar = mapa_u32(ubar, (uint32_t)(lane < ndst ? lane : 0));
+        int pj = e > 0 ? e : kCritPer, pslot = 0;       // next step to prefetch (step 0 has no chunk)
+        auto prefetch_step = [&]() {
+            if (pj < s) {
+                const int len = pj * b;
+                const int nch = num_chunks(pj, b);
+                const float *src = gbase + (int64_t)len * ldg;
+#pragma unroll
+                for (int w = 0; w < kWin; ++w) {
+                    const int c = nch - kWin + w;
+                    if (c >= 0 && c * kChunk + lane * 4 < len) {
+#pragma unroll
+                        for (int i = 0; i < kQuad; ++i)
+                            cp_async16(ring + (uint32_t)(pslot * kWin + w) * kUnitBytes + (uint32_t)i * (kChunk * 4u),
+                                       src + (int64_t)i * ldg + c * kChunk);
+                    }
+                }
+                pj += kCritPer;
+            }
+            cp_async_commit();                          // always: wait_group counts groups, empty ones included
+            pslot = (pslot + 1 == kCritDepth) ? 0 : pslot + 1;
+        };
+#pragma unroll 1
+        for (int i = 0; i < kCritDepth - 1; ++i) prefetch_step();
+        float rr = 0.f, yy = 0.f;
+        if (e < s) { rr = __ldg(r + e * b + q0 + li); yy = __ldg(yI + e * b + q0 + li); }
+
+        __syncthreads();
+        cluster_sync_all();                             // nobody signals a barrier that is not initialised yet
+        REC_TRACE(1);
+
+        int slot = 0, ready = 0;                        // blocks 0 .. ready-1 of u are complete in u_s (this warp's view)
+#pragma unroll 1
+        for (int j = e; j < s; j += kCritPer) {
+            const int row = j * b + q0;
+            float rr_next = 0.f, yy_next = 0.f;
+            if (j + kCritPer < s) {
+                rr_next = __ldg(r + row + kCritPer * b + li);
+                yy_next = __ldg(yI + row + kCritPer * b + li);
+            }
+            float acc[kQuad] = {0.f, 0.f, 0.f, 0.f};
+            if (j > 0) {
+                const int len = j * b;
+                const int nch = num_chunks(j, b);
+                cp_async_wait<kCritDepth - 2>();        // the oldest outstanding step (this one) has landed
+                const uint32_t sbase = ring + (uint32_t)(slot * kWin) * kUnitBytes;
+                slot = (slot + 1 == kCritDepth) ? 0 : slot + 1;
+                // the newest chunk's G: in registers before the wait
+                const int cl = nch - 1;
+                const bool mine = cl * kChunk + lane * 4 < len;
+                float4 gl[kQuad];
+#pragma unroll
+                for (int i = 0; i < kQuad; ++i) {
+                    gl[i] = make_float4(0.f, 0.f, 0.f, 0.f);
+                    if (mine) gl[i] = lds_f4(sbase + (uint32_t)(kWin - 1) * kUnitBytes + (uint32_t)i * (kChunk * 4u));
+                }
+                if (nch > kWin) {
+                    // lane (li, gg): the partial sum of row li from bulk warp gg of this group
+                    mbar_wait(pbar + 8u * j, 0u);
+                    float p = 0.f;
+                    if ((lane & 7) < kBulkWarps / qpc)
+                        asm volatile("ld.shared.f32 %0, [%1];" : "=f"(p)
+                                 : "r"(part + 16u * (uint32_t)(((j % kPartDepth) * kMaxQuadsPerCta + gamma) * kBulkWarps + (lane & 7)) + 4u * (uint32_t)li));
+#pragma unroll
+                    for (int i = 0; i < kQuad; ++i) acc[i] = (i == li) ? p : 0.f;
+                }
+                // the window's older chunks (full ones): their blocks are at most j - 2, normally long there
+#pragma unroll 1
+                for (int w = max(0, kWin - nch); w < kWin - 1; ++w) {
+                    const int c = nch - kWin + w;
+                    const int need = block_of(c * kChunk + kChunk - 1);
+                    while (ready <= need) { mbar_wait(ubar + 8u * ready, 0u); ++ready; }
+                    const float4 uv = lds_f4(us + 4u * (uint32_t)(c * kChunk + lane * 4));
+#pragma unroll
+                    for (int i = 0; i < kQuad; ++i) {
+                        const float4 gv = lds_f4(sbase + (uint32_t)w * kUnitBytes + (uint32_t)i * (kChunk * 4u));
+                        acc[i] = fmaf(gv.x, uv.x, acc[i]);
+                        acc[i] = fmaf(gv.y, uv.y, acc[i]);
+                        acc[i] = fmaf(gv.z, uv.z, acc[i]);
+                        acc[i] = fmaf(gv.w, uv.w, acc[i]);
+                    }
+                }
+                REC_TRACE(8 + 4 * j);
+                // every block the newest chunk touches must have landed HERE (completion of a later block in
+                // another CTA says nothing about what has reached this one)
+                ready = max(ready, block_of(cl * kChunk));
+                while (ready < j) { mbar_wait(ubar + 8u * ready, 0u); ++ready; }
+                REC_TRACE(9 + 4 * j);
+                if (mine) {
+                    const float4 uv = lds_f4(us + 4u * (uint32_t)(cl * kChunk + lane * 4));
+#pragma unroll
+                    for (int i = 0; i < kQuad; ++i) {
+                        acc[i] = fmaf(gl[i].x, uv.x, acc[i]);
+                        acc[i] = fmaf(gl[i].y, uv.y, acc[i]);
+                        acc[i] = fmaf(gl[i].z, uv.z, acc[i]);
+                        acc[i] = fmaf(gl[i].w, uv.w, acc[i]);
+                    }
+                }
+            }
+            const float tot = (j > 0) ? quad_reduce(acc, lane) : 0.f;       // lane l: row l >> 3
+            const float zz = fmaf(-alpha, tot, rr);
+            const float uu = lprime_chain<LOSS>(zz, yy);
+            if (j + 1 < s) {
+                const float u0 = __shfl_sync(0xffffffffu, uu, 0), u1 = __shfl_sync(0xffffffffu, uu, 8);
+                const float u2 = __shfl_sync(0xffffffffu, uu, 16), u3 = __shfl_sync(0xffffffffu, uu, 24);
+                if (lane < ndst) st_async_v4(rem_us + 4u * (uint32_t)row, u0, u1, u2, u3, rem_ubar + 8u * (uint32_t)j);
+            }
+            REC_TRACE(10 + 4 * j);
+            if ((lane & 7) == 0) {
+                z[row + li] = zz;
+                u[row + li] = uu;
+            }
+            if (j > 0) prefetch_step();                 // refills the slot consumed one step ago
+            REC_TRACE(11 + 4 * j);
+            rr = rr_next;
+            yy = yy_next;
+        }
+    }
+    else if (is_bulk) {
+        // ===== bulk warp: group gamma, lane cidx of nw; chunks c = cidx, cidx + nw, ... < nch(j) - kWin of every step =====
+        // These columns belong to blocks that landed (kWin - 1) * 128 / b hops ago, so the bulk warps run
+        // several steps ahead of the chain and are bound only by the SM's L2 bandwidth.
+        const int g = qpc <= 2 ? wslot * 2 + (wsched - 2) : warp - 8;
+        const int nw = kBulkWarps / qpc;                // bulk warps per owned group
+        const int gamma = g / nw, cidx = g % nw;
+        const uint32_t ring = base + L.bring + (uint32_t)(g * kDepth) * kUnitBytes + (uint32_t)lane * 16u;
+        const float *gbase = G + (int64_t)(kQuad * (crank + gamma * C)) * ldg + lane * 4;   // + j b ldg + c * 128
+        int pj = 1, pc = cidx, pslot = 0;               // next unit to prefetch
+        auto cursor_norm = [&]() {
+            while (pj < s && pc >= num_chunks(pj, b) - kWin) { ++pj; pc = cidx; }
+        };
+        auto prefetch_unit = [&]() {
+            if (pj < s) {
+                const float *src = gbase + (int64_t)pj * b * ldg + pc * kChunk;
+#pragma unroll
+                for (int i = 0; i < kQuad; ++i)
+                    cp_async16(ring + (uint32_t)pslot * kUnitBytes + (uint32_t)i * (kChunk * 4u), src + (int64_t)i * ldg);
+                pc += nw;
+                cursor_norm();
+            }
+            cp_async_commit();
+            pslot = (pslot + 1 == kDepth) ? 0 : pslot + 1;
+        };
+        cursor_norm();
+#pragma unroll 1
+        for (int i = 0; i < kDepth - 1; ++i) prefetch_unit();
+
+        __syncthreads();
+        cluster_sync_all();
+
+        int slot = 0, ready = 0;
+#pragma unroll 1
+        for (int j = 1; j < s; ++j) {
+            const int nb = num_chunks(j, b) - kWin;
+            if (nb <= 0) continue;
+            // a warp with nothing to do must not run ahead into partial-sum slots that are still being read
+            if (j >= kPartDepth - 4) {
+                const int k = j - (kPartDepth - 4);
+                if (ready <= k) mbar_wait(ubar + 8u * k, 0u);
+            }
+            REC_TRACE_B(6000 + 4 * j);
+            float acc[kQuad] = {0.f, 0.f, 0.f, 0.f};
+#pragma unroll 1
+            for (int c = cidx; c < nb; c += nw) {
+                cp_async_wait<kDepth - 2>();
+                float4 gv[kQuad];
+#pragma unroll
+                for (int i = 0; i < kQuad; ++i) gv[i] = lds_f4(ring + (uint32_t)slot * kUnitBytes + (uint32_t)i * (kChunk * 4u));
+                slot = (slot + 1 == kDepth) ? 0 : slot + 1;
+                const int need = block_of(c * kChunk + kChunk - 1);         // newest block this chunk touches
+                while (ready <= need) { mbar_wait(ubar + 8u * ready, 0u); ++ready; }
+                const float4 uv = lds_f4(us + 4u * (uint32_t)(c * kChunk + lane * 4));
+#pragma unroll
+                for (int i = 0; i < kQuad; ++i) {
+                    acc[i] = fmaf(gv[i].x, uv.x, acc[i]);
+                    acc[i] = fmaf(gv[i].y, uv.y, acc[i]);
+                    acc[i] = fmaf(gv[i].z, uv.z, acc[i]);
+                    acc[i] = fmaf(gv[i].w, uv.w, acc[i]);
+                }
+                prefetch_unit();
+            }
+            const float tot = quad_reduce(acc, lane);
+            if ((lane & 7) == 0)
+                asm volatile("st.shared.f32 [%0], %1;"
+                             ::"r"(part + 16u * (uint32_t)(((j % kPartDepth) * kMaxQuadsPerCta + gamma) * kBulkWarps + cidx) + 4u * (uint32_t)li), "f"(tot) : "memory");
+            __syncwarp();
+            if (lane == 0) mbar_arrive(pbar + 8u * j);
+            REC_TRACE_B(6001 + 4 * j);
+        }
+    } else {
+        __syncthreads();
+        cluster_sync_all();
+    }
+    cp_async_wait<0>();
+    REC_TRACE(2);
+    __syncthreads();
+    cluster_sync_all();                                 // no CTA leaves while others may still store into it
+    REC_TRACE(3);
+}
+
+int stream_smem_bytes(int s, int b)
+{
+    static int max_optin = -1;
+    if (max_optin < 0) {
+        int dev = 0;
+        cudaGetDevice(&dev);
+        if (cudaDeviceGetAttribute(&max_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev) != cudaSuccess) max_optin = 0;
+    }
+    const int need = (int)stream_layout(s, b).total;
+    return need <= max_optin ? need : 0;
+}
+
+// Cluster size for block size b: the largest power of two <= min(cluster_max, b / 4), so that every CTA owns
+// at least one row group.
+int stream_cluster_for(int b, int cluster_max)
+{
+    int c = 1;
+    while (2 * c <= cluster_max && 2 * c <= b / kQuad) c *= 2;
+    return c;
+}
+
+template <int LOSS>
+cudaError_t launch_stream(cudaStream_t st, const float *G, int32_t ldg, const float *r, const float *yI, int32_t s,
+                          int32_t b, float alpha, float *z, float *u, int cluster_max)
+{
+    static bool attr_set = false;
+    const int smem = stream_smem_bytes(s, b);
+    if (smem == 0) return cudaErrorInvalidConfiguration;
+    auto kern = recurrence_stream_kernel<LOSS>;
+    if (!attr_set) {
+        int dev = 0, max_optin = 0;
+        cudaGetDevice(&dev);
+        cudaDeviceGetAttribute(&max_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev);
+        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, max_optin);
+        if (e != cudaSuccess) return e;
+        e = cudaFuncSetAttribute(kern, cudaFuncAttributeNonPortableClusterSizeAllowed, 1);
+        if (e != cudaSuccess) return e;
+        attr_set = true;
+    }
+    const int cluster = stream_cluster_for(b, cluster_max);
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3(cluster);
+    cfg.blockDim = dim3(kThreads);
+    cfg.dynamicSmemBytes = (size_t)smem;
+    cfg.stream = st;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeClusterDimension;
+    attr[0].val.clusterDim.x = cluster;
+    attr[0].val.clusterDim.y = 1;
+    attr[0].val.clusterDim.z = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    return cudaLaunchKernelEx(&cfg, kern, G, ldg, r, yI, s, b, alpha, z, u);
+}
+
+}  // namespace
+
+// Can the stream kernel run this shape in a cluster of at most `cluster` CTAs?
+bool recurrence_stream_ok(int32_t s, int32_t b, int32_t ldg, int cluster)
+{
+    if (cluster <= 0 || b % 4 != 0 || ldg % 4 != 0 || s < 2) return false;
+    const int c = stream_cluster_for(b, cluster);
+    if ((b / kQuad + c - 1) / c > kMaxQuadsPerCta) return false;
+    return stream_smem_bytes(s, b) > 0;
+}
+
+int launch_recurrence_stream(cudaStream_t st, const float *G, int32_t ldg, const float *r, const float *yI, int32_t s,
+                             int32_t b, float alpha, int loss, float *z, float *u, int cluster)
+{
+    cudaError_t e = loss == CASGD_LOGISTIC ? launch_stream<CASGD_LOGISTIC>(st, G, ldg, r, yI, s, b, alpha, z, u, cluster)
+                  : loss == CASGD_LINEAR  ? launch_stream<CASGD_LINEAR>(st, G, ldg, r, yI, s, b, alpha, z, u, cluster)
+                                          : launch_stream<CASGD_POISSON>(st, G, ldg, r, yI, s, b, alpha, z, u, cluster);
+    return e == cudaSuccess ? 1 : -1;
+}
+
+#ifdef CASGD_REC_TRACE
+extern "C" int casgd_rec_trace_dump(long long *dst_host, int n)
+{
+    cudaDeviceSynchronize();
+    return (int)cudaMemcpyFromSymbol(dst_host, g_rec_trace, sizeof(long long) * (size_t)n);
+}
+#endif
+
+}  // namespace casgd

@@ -79,14 +79,19 @@ RECURRENCE = [
     (4, 6000, 32, 3, 256),       # b = 256: two 128-column chunks per block
     (0, 20000, 16, 9, 1300),     # sb = 11700: up to 10 rows per warp
     (0, 3000, 16, 300, 1),       # b = 1: 299 dependent steps of one column each
+    (0, 9000, 24, 21, 20),       # b = 20: blocks straddle the 128-column chunks; CTAs own 2 or 1 rows per block
+    (3, 5000, 40, 130, 16),      # b = 16: one row per CTA, 129 hops, eight blocks per chunk
+    (0, 9000, 24, 40, 96),       # b = 96: a "bulk" chunk can hold part of the newest block
 ]
 
 
-@pytest.mark.parametrize("rec_impl", [1, 2, 3], ids=["cta", "grid", "cluster"])
+@pytest.mark.parametrize("rec_impl", [1, 2, 3, 4], ids=["cta", "grid", "cluster", "stream"])
 @pytest.mark.parametrize("ci,m,n,s,b", RECURRENCE)
 def test_recurrence_kernels_match_the_oracle(binding, oracle_mod, ci, m, n, s, b, rec_impl):
-    """Both recurrence kernels (one CTA; all SMs with tagged words through L2) on the same inputs, forced
-    with CASGD_OPT_RECURRENCE_IMPL, twice in a row (the second launch sees the first one's retired epoch)."""
+    """Every recurrence kernel (one CTA; all SMs with tagged words through L2; one cluster with plain loads of G;
+    one cluster with G streamed through a shared-memory ring) on the same inputs, forced with
+    CASGD_OPT_RECURRENCE_IMPL, twice in a row (the second launch sees the first one's retired epoch). Shapes a
+    kernel does not take (b % 4 != 0, more than 8 rows of a block per CTA) fall through to the next one."""
     cfg = synth.config(ci, m=m, n=n)
     X_d, y_d, A_bits, y = device_dataset(cfg)
     eta = cfg.eta if cfg.loss != synth.POISSON else 0.01
@@ -107,7 +112,7 @@ def test_grid_recurrence_replays_from_a_graph(binding):
     idx_d = torch.from_numpy(synth.epoch_indices(cfg, 42, 0)[: steps * s * b].copy()).cuda()
     xs = {}
     with binding.Casgd(X_d, y_d, cfg.loss) as cg:
-        for impl in (1, 2, 3):
+        for impl in (1, 2, 3, 4):
             cg.set_option(binding.OPT_RECURRENCE_IMPL, impl)
             xa = torch.zeros(cfg.n, device="cuda")
             for h in range(steps):
@@ -117,7 +122,7 @@ def test_grid_recurrence_replays_from_a_graph(binding):
             cg.sync()
             assert torch.equal(xa, xb)
             xs[impl] = xa
-    for impl in (2, 3):
+    for impl in (2, 3, 4):
         assert torch.linalg.norm(xs[1] - xs[impl]) <= 1e-5 * torch.linalg.norm(xs[1])
 
 
