@@ -47,6 +47,8 @@ struct casgd_ctx {
     const uint16_t *A = nullptr;      // BF16 bits, row stride lda (borrowed or owned)
     uint16_t *A_owned = nullptr;
     int64_t lda = 0;
+    const uint16_t *X_caller = nullptr;   // the caller's matrix when A is a repacked copy (casgd_loss streams narrow rows from it)
+    int64_t ldx_caller = 0;
     const float *y = nullptr;
     int64_t m = 0;
     int32_t n = 0;
@@ -76,7 +78,7 @@ struct casgd_ctx {
     // last step, for debug export
     int32_t last_s = 0, last_b = 0;
     // options
-    int64_t opt_gram_impl = 0, opt_full_lower = 0, opt_profile = 0, opt_no_graph = 0, opt_ksplit = 0, opt_rec_impl = 0;
+    int64_t opt_gram_impl = 0, opt_full_lower = 0, opt_profile = 0, opt_no_graph = 0, opt_ksplit = 0, opt_rec_impl = 0, opt_loss_impl = 0;
     GramTcPlan *tc_plan = nullptr;
     std::map<GraphKey, GraphEntry> graphs;
     std::vector<StageEvent> events;
@@ -352,13 +354,15 @@ int casgd_init(casgd_ctx **out, const uint16_t *X_bf16, int64_t ldx, const float
         if (!ck(cudaStreamSynchronize(c->stream))) return bail(CASGD_ECUDA);
         c->A = c->A_owned;
         c->lda = lda;
+        c->X_caller = X_bf16;
+        c->ldx_caller = ldx;
     }
     c->ldxb = (int32_t)round_up(n, 64);
     const size_t xbf_elems = (size_t)16 * c->ldxb;
     c->gws.ldp = c->ldy;
     c->gws.max_splits = 128;
     c->loss_max_blocks = kNumSMsB200 * 4;
-    const int n_counters = 8192;
+    const int n_counters = 8192 + 1;              // gradient column tiles, plus casgd_loss's finished-CTA counter
     bool ok = ck(cudaMalloc(&c->xbf, sizeof(uint16_t) * xbf_elems)) &&
               ck(cudaMemsetAsync(c->xbf, 0, sizeof(uint16_t) * xbf_elems, c->stream)) &&
               ck(cudaMalloc(&c->gws.partial, sizeof(float) * (size_t)c->gws.max_splits * c->gws.ldp)) &&
@@ -455,8 +459,9 @@ int casgd_loss(casgd_ctx *c, const float *x, double *loss_host)
     if (!x || !loss_host) return fail(c, CASGD_EINVAL, "x and loss_host must not be null");
     {
         StageTimer t(c, CASGD_STAGE_LOSS);
-        t.done(launch_loss(c->stream, c->A, c->lda, c->y, c->m, c->n, c->loss, x, c->loss_partials,
-                           c->loss_max_blocks, c->loss_result));
+        t.done(launch_loss(c->stream, c->A, c->lda, c->X_caller, c->ldx_caller, c->y, c->m, c->n, c->loss, x,
+                           c->loss_partials, c->loss_max_blocks, c->loss_result, c->gws.counters + 8192,
+                           (int)c->opt_loss_impl));
     }
     CK(cudaGetLastError());
     CK(cudaMemcpyAsync(c->loss_result_host, c->loss_result, sizeof(double), cudaMemcpyDeviceToHost, c->stream));
@@ -536,6 +541,9 @@ int casgd_set_option(casgd_ctx *c, int option, int64_t value)
     case CASGD_OPT_RECURRENCE_IMPL:
         if (value < 0 || value > 4) return fail(c, CASGD_EINVAL, "CASGD_OPT_RECURRENCE_IMPL must be in [0, 4]");
         c->opt_rec_impl = value; break;
+    case CASGD_OPT_LOSS_IMPL:
+        if (value != 0 && value != 1) return fail(c, CASGD_EINVAL, "CASGD_OPT_LOSS_IMPL must be 0 or 1");
+        c->opt_loss_impl = value; break;
     default: return fail(c, CASGD_EINVAL, "unknown option %d", option);
     }
     drop_graphs(c);

@@ -105,6 +105,41 @@ __device__ __forceinline__ uint4 ldg_nc_v4(const void *p)
     return r;
 }
 
+// ------------------------------------------------- programmatic dependent launch ---
+// The four kernels of an outer step are chained with programmatic stream serialisation: a kernel's CTAs are
+// scheduled (and run their prologue) while the previous kernel drains, and block in pdl_wait() until it has
+// completed and its writes are visible. Every kernel of the step path calls pdl_trigger() first thing and
+// pdl_wait() before it touches anything another kernel of the chain writes or reads.
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+__device__ __forceinline__ void pdl_trigger() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+
+// cudaLaunchKernelEx with the programmatic-serialisation attribute (and a cluster dimension when cluster > 1).
+template <typename... KArgs, typename... Args>
+inline cudaError_t launch_pdl(void (*kern)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t st, int cluster,
+                              Args... args)
+{
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = grid;
+    cfg.blockDim = block;
+    cfg.dynamicSmemBytes = smem;
+    cfg.stream = st;
+    cudaLaunchAttribute attr[2];
+    int na = 0;
+    attr[na].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[na].val.programmaticStreamSerializationAllowed = 1;
+    ++na;
+    if (cluster > 1) {
+        attr[na].id = cudaLaunchAttributeClusterDimension;
+        attr[na].val.clusterDim.x = (unsigned)cluster;
+        attr[na].val.clusterDim.y = 1;
+        attr[na].val.clusterDim.z = 1;
+        ++na;
+    }
+    cfg.attrs = attr;
+    cfg.numAttrs = na;
+    return cudaLaunchKernelEx(&cfg, kern, KArgs(args)...);
+}
+
 // ------------------------------------------------------------ launch prototypes ---
 // Every launcher enqueues on `st` and returns the number of kernels it launched.
 // `ind`, when non-null, overrides idx / x with ind->idx + idx_off / ind->x (graph replay).
@@ -152,8 +187,9 @@ int launch_sgd32_step(cudaStream_t st, const float *A32, int64_t lda32, const fl
                       const int32_t *idx, int32_t b, float alpha, int loss, float *x, float *u, float *z,
                       int *err_flag, const GradWorkspace &ws);
 
-int launch_loss(cudaStream_t st, const uint16_t *A, int64_t lda, const float *y, int64_t m, int32_t n, int loss,
-                const float *x, double *block_partials, int32_t max_blocks, double *result_dev);
+int launch_loss(cudaStream_t st, const uint16_t *A, int64_t lda, const uint16_t *X, int64_t ldx, const float *y, int64_t m,
+                int32_t n, int loss, const float *x, double *block_partials, int32_t max_blocks, double *result_dev,
+                unsigned *done_counter, int impl);
 
 int launch_shadow(cudaStream_t st, const float *x, const StepParams *ind, int32_t n, uint16_t *xbf);
 int launch_widen(cudaStream_t st, const uint16_t *A, int64_t lda, int64_t m, int32_t n, float *A32, int64_t lda32);

@@ -12,6 +12,8 @@ gather_rows_kernel(const uint16_t *__restrict__ A, int64_t lda, const float *__r
                    const int32_t *__restrict__ idx, const StepParams *__restrict__ ind, int64_t idx_off, int32_t sb,
                    uint16_t *__restrict__ Y, int32_t ldy, float *__restrict__ yI, int *__restrict__ err_flag)
 {
+    pdl_trigger();
+    pdl_wait();                                     // Y is still being read by the previous step's gradient
     const int32_t chunks = ldy >> 3;
     const int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     const int64_t row = t / chunks;
@@ -49,7 +51,8 @@ int launch_gather(cudaStream_t st, const uint16_t *A, int64_t lda, const float *
     const int64_t total = (int64_t)sb * (ldy >> 3);
     const int threads = 256;
     const unsigned blocks = (unsigned)((total + threads - 1) / threads);
-    gather_rows_kernel<<<blocks, threads, 0, st>>>(A, lda, y, m, n, idx, ind, idx_off, sb, Y, ldy, yI, err_flag);
+    launch_pdl(gather_rows_kernel, dim3(blocks), dim3(threads), 0, st, 1, A, lda, y, m, n, idx, ind, idx_off, sb, Y, ldy, yI,
+               err_flag);
     return 1;
 }
 
@@ -57,6 +60,8 @@ int launch_gather(cudaStream_t st, const uint16_t *A, int64_t lda, const float *
 __global__ void shadow_kernel(const float *__restrict__ x, const StepParams *__restrict__ ind, int32_t n,
                               uint16_t *__restrict__ xbf)
 {
+    pdl_trigger();
+    pdl_wait();
     const float *xs = ind ? ind->x : x;
     int32_t k = blockIdx.x * blockDim.x + threadIdx.x;
     if (k < n) xbf[k] = f32_to_bf16_bits_rn(xs[k]);
@@ -64,7 +69,7 @@ __global__ void shadow_kernel(const float *__restrict__ x, const StepParams *__r
 
 int launch_shadow(cudaStream_t st, const float *x, const StepParams *ind, int32_t n, uint16_t *xbf)
 {
-    shadow_kernel<<<(n + 255) / 256, 256, 0, st>>>(x, ind, n, xbf);
+    launch_pdl(shadow_kernel, dim3((n + 255) / 256), dim3(256), 0, st, 1, x, ind, n, xbf);
     return 1;
 }
 
@@ -106,13 +111,15 @@ int launch_repack(cudaStream_t st, const uint16_t *X, int64_t ldx, int64_t m, in
 
 __global__ void set_params_kernel(StepParams *ind, const int32_t *idx, float *x)
 {
+    pdl_trigger();
+    pdl_wait();                                     // the previous replay may still be reading the block
     ind->idx = idx;
     ind->x = x;
 }
 
 int launch_set_params(cudaStream_t st, StepParams *ind, const int32_t *idx, float *x)
 {
-    set_params_kernel<<<1, 1, 0, st>>>(ind, idx, x);
+    launch_pdl(set_params_kernel, dim3(1), dim3(1), 0, st, 1, ind, idx, x);
     return 1;
 }
 

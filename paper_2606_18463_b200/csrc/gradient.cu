@@ -41,6 +41,8 @@ gradient_update_kernel(const T *__restrict__ base, int64_t ld, const int32_t *__
                        float *__restrict__ partial, int32_t ldp, unsigned *__restrict__ counters)
 {
     constexpr int kVec = VecTraits<T>::kVec;
+    pdl_trigger();
+    pdl_wait();
     __shared__ float red[kGradThreads * kVec];
     __shared__ bool s_last;
     const int tid = threadIdx.x;
@@ -127,8 +129,8 @@ static int launch_gradient_any(cudaStream_t st, const T *base, int64_t ld, const
     const int rows_per_split = (rows + splits - 1) / splits;
     splits = (rows + rows_per_split - 1) / rows_per_split;
     dim3 grid(col_tiles, splits);
-    gradient_update_kernel<T, GATHER, SHADOW><<<grid, kGradThreads, 0, st>>>(
-        base, ld, idx, m, n, rows, rows_per_split, CV, u, alpha, x, ind, xbf, ws.partial, ws.ldp, ws.counters);
+    launch_pdl(gradient_update_kernel<T, GATHER, SHADOW>, grid, dim3(kGradThreads), 0, st, 1, base, ld, idx, m, n, rows,
+               rows_per_split, CV, u, alpha, x, ind, xbf, ws.partial, ws.ldp, ws.counters);
     return 1;
 }
 
@@ -146,6 +148,8 @@ sgd32_margin_kernel(const float *__restrict__ A32, int64_t lda32, const float *_
                     const int32_t *__restrict__ idx, int32_t b, int loss, const float *__restrict__ x, float *__restrict__ z,
                     float *__restrict__ u, int *__restrict__ err_flag)
 {
+    pdl_trigger();
+    pdl_wait();
     const int warp = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
     if (warp >= b) return;
     const int64_t src = idx[warp];
@@ -174,7 +178,8 @@ int launch_sgd32_step(cudaStream_t st, const float *A32, int64_t lda32, const fl
                       const int32_t *idx, int32_t b, float alpha, int loss, float *x, float *u, float *z,
                       int *err_flag, const GradWorkspace &ws)
 {
-    sgd32_margin_kernel<<<(b * 32 + 255) / 256, 256, 0, st>>>(A32, lda32, y, m, n, idx, b, loss, x, z, u, err_flag);
+    launch_pdl(sgd32_margin_kernel, dim3((b * 32 + 255) / 256), dim3(256), 0, st, 1, A32, lda32, y, m, n, idx, b, loss,
+               (const float *)x, z, u, err_flag);
     launch_gradient_any<float, true, false>(st, A32, lda32, idx, m, n, b, u, alpha, x, nullptr, nullptr, ws);
     return 2;
 }

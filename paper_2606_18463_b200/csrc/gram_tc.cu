@@ -158,6 +158,7 @@ gram_tc_kernel(const __grid_constant__ CUtensorMap tmY, const __grid_constant__ 
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int nwork = p.ntiles * p.ksplit;
+    pdl_trigger();
 
     if (warp == 0 && lane == 0) {
         for (int s = 0; s < kStages; ++s) { mbar_init(full_bar(s), 1); mbar_init(empty_bar(s), 1); }
@@ -174,6 +175,7 @@ gram_tc_kernel(const __grid_constant__ CUtensorMap tmY, const __grid_constant__ 
     __syncthreads();
     tc_fence_after();
     const uint32_t tmem_base = *tmem_slot_ptr;
+    pdl_wait();                                     // Y and x_bf come from the gather / the previous gradient
 
     if (warp == 0) {
         // ===== TMA producer =====
@@ -381,7 +383,7 @@ int launch_gram_tc(cudaStream_t st, GramTcPlan *plan, int32_t sb, int32_t b, flo
         cudaMemsetAsync(r, 0, sizeof(float) * (size_t)p.T * BM, st);
     }
     const int grid = std::min(p.ntiles * ksplit, kNumSMsB200);
-    gram_tc_kernel<<<grid, kThreads, kSmemBytes, st>>>(plan->tmY, plan->tmX, p);
+    launch_pdl(gram_tc_kernel, dim3(grid), dim3(kThreads), kSmemBytes, st, 1, plan->tmY, plan->tmX, p);
     return launches;
 }
 

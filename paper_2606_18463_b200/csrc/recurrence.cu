@@ -28,6 +28,8 @@ recurrence_cta_kernel(const float *__restrict__ G, int32_t ldg, const float *__r
                       int32_t s, int32_t b, float alpha, float *__restrict__ z, float *__restrict__ u)
 {
     extern __shared__ float u_s[];                    // [s*b]
+    pdl_trigger();
+    pdl_wait();
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarps = blockDim.x >> 5;
     for (int j = 0; j < s; ++j) {
         const int len = j * b;
@@ -291,6 +293,8 @@ recurrence_cluster_kernel(const float *__restrict__ G, int32_t ldg, const float 
     __shared__ volatile float part[2][kChainWarps];
     __shared__ volatile int pflag[2][kChainWarps];                 // step whose partial sits in part[.][w]
     __shared__ volatile int cons[kChainWarps];                     // last step whose partial the lead has read
+    pdl_trigger();
+    pdl_wait();
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int C = (int)cluster_nctarank(), crank = (int)cluster_ctarank();
     const int sb = s * b;
@@ -453,19 +457,8 @@ template <int LOSS>
 static cudaError_t launch_cluster(cudaStream_t st, const float *G, int32_t ldg, const float *r, const float *yI,
                                   int32_t s, int32_t b, float alpha, float *z, float *u, int cluster)
 {
-    cudaLaunchConfig_t cfg = {};
-    cfg.gridDim = dim3(cluster);
-    cfg.blockDim = dim3(kChainThreads);
-    cfg.dynamicSmemBytes = sizeof(float) * (size_t)s * b + 8 * (size_t)s;
-    cfg.stream = st;
-    cudaLaunchAttribute attr[1];
-    attr[0].id = cudaLaunchAttributeClusterDimension;
-    attr[0].val.clusterDim.x = cluster;
-    attr[0].val.clusterDim.y = 1;
-    attr[0].val.clusterDim.z = 1;
-    cfg.attrs = attr;
-    cfg.numAttrs = 1;
-    return cudaLaunchKernelEx(&cfg, recurrence_cluster_kernel<LOSS>, G, ldg, r, yI, s, b, alpha, z, u);
+    return launch_pdl(recurrence_cluster_kernel<LOSS>, dim3(cluster), dim3(kChainThreads),
+                      sizeof(float) * (size_t)s * b + 8 * (size_t)s, st, cluster, G, ldg, r, yI, s, b, alpha, z, u);
 }
 
 template <int LOSS>
@@ -547,7 +540,7 @@ int launch_recurrence(cudaStream_t st, const float *G, int32_t ldg, const float 
             cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, CASGD_MAX_SB * (int)sizeof(float));
             attr_set = true;
         }
-        kern<<<1, threads, smem, st>>>(G, ldg, r, yI, s, b, alpha, z, u);
+        launch_pdl(kern, dim3(1), dim3(threads), smem, st, 1, G, ldg, r, yI, s, b, alpha, z, u);
     };
     if (loss == CASGD_LOGISTIC) go(recurrence_cta_kernel<CASGD_LOGISTIC>);
     else if (loss == CASGD_LINEAR) go(recurrence_cta_kernel<CASGD_LINEAR>);

@@ -181,6 +181,7 @@ recurrence_stream_kernel(const float *__restrict__ G, int32_t ldg, const float *
     extern __shared__ __align__(128) unsigned char rs_smem[];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int C = (int)cluster_nctarank(), crank = (int)cluster_ctarank();
+    pdl_trigger();
     REC_TRACE(0);
     const StreamLayout L = stream_layout(s, b);
     const uint32_t base = (uint32_t)__cvta_generic_to_shared(rs_smem);
@@ -199,6 +200,7 @@ recurrence_stream_kernel(const float *__restrict__ G, int32_t ldg, const float *
         mbar_init(pbar + 8u * k, kBulkWarps);
     }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    pdl_wait();                                         // G, r and y_I come from the Gram and gather kernels
 
     // Warp w runs on scheduler w & 3. Critical warps: (group gamma, parity e) -> warp gamma + 4 e, so with up
     // to two groups they have schedulers 0 and 1 to themselves and the eight bulk warps share 2 and 3: what the
@@ -459,19 +461,7 @@ cudaError_t launch_stream(cudaStream_t st, const float *G, int32_t ldg, const fl
         attr_set = true;
     }
     const int cluster = stream_cluster_for(b, cluster_max);
-    cudaLaunchConfig_t cfg = {};
-    cfg.gridDim = dim3(cluster);
-    cfg.blockDim = dim3(kThreads);
-    cfg.dynamicSmemBytes = (size_t)smem;
-    cfg.stream = st;
-    cudaLaunchAttribute attr[1];
-    attr[0].id = cudaLaunchAttributeClusterDimension;
-    attr[0].val.clusterDim.x = cluster;
-    attr[0].val.clusterDim.y = 1;
-    attr[0].val.clusterDim.z = 1;
-    cfg.attrs = attr;
-    cfg.numAttrs = 1;
-    return cudaLaunchKernelEx(&cfg, kern, G, ldg, r, yI, s, b, alpha, z, u);
+    return launch_pdl(kern, dim3(cluster), dim3(kThreads), (size_t)smem, st, cluster, G, ldg, r, yI, s, b, alpha, z, u);
 }
 
 }  // namespace

@@ -186,11 +186,20 @@ def test_bad_arguments_are_rejected_before_any_launch(binding):
         assert cg.launch_count() == before
 
 
-@pytest.mark.parametrize("ci,m,n", [(0, 8192, 64), (1, 30000, 18), (2, 4000, 1024), (3, 6000, 2000), (4, 20000, 512)])
-def test_full_loss_matches_the_oracle(binding, oracle_mod, ci, m, n):
+# shapes: the five configs' n, plus ragged ones -- odd n and odd row counts (unaligned narrow rows, a last slot
+# that is not a multiple of 16 bytes), n just past a 2 KB segment, one row, fewer rows than warps
+LOSS_SHAPES = [(0, 8192, 64), (1, 30000, 18), (2, 4000, 1024), (3, 6000, 2000), (4, 20000, 512), (2, 1501, 4096),
+               (1, 30001, 18), (0, 7777, 19), (0, 5003, 7), (4, 3001, 1032), (3, 999, 1001), (0, 1, 64), (1, 37, 18),
+               (4, 4099, 40), (2, 300, 8200)]
+
+
+@pytest.mark.parametrize("impl", [0, 1], ids=["stream", "plain"])
+@pytest.mark.parametrize("ci,m,n", LOSS_SHAPES)
+def test_full_loss_matches_the_oracle(binding, oracle_mod, ci, m, n, impl):
     cfg = synth.config(ci, m=m, n=n)
     X_d, y_d, A_bits, y = device_dataset(cfg)
     with binding.Casgd(X_d, y_d, cfg.loss) as cg:
+        cg.set_option(binding.OPT_LOSS_IMPL, impl)
         F0 = cg.loss(torch.zeros(n, device="cuda"))
         closed = {0: math.log(2.0), 1: float(np.mean(y.astype(np.float64) ** 2) / 2), 2: 1.0}[cfg.loss]
         assert F0 == pytest.approx(closed, rel=1e-6)                       # F(0) in closed form
