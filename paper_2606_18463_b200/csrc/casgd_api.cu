@@ -80,6 +80,9 @@ struct casgd_ctx {
     // options
     int64_t opt_gram_impl = 0, opt_full_lower = 0, opt_profile = 0, opt_no_graph = 0, opt_ksplit = 0, opt_rec_impl = 0, opt_loss_impl = 0;
     GramTcPlan *tc_plan = nullptr;
+    GramPairPlan *pair_plan = nullptr;
+    int num_sms = 0;
+    int cur_gram = 0, cur_bn = 0;     // Gram kernel of the shape being enqueued: 1 = CUDA cores, 2 = 128x128 tiles, 3 = CTA pairs
     std::map<GraphKey, GraphEntry> graphs;
     std::vector<StageEvent> events;
     double stage_ms[CASGD_NUM_STAGES] = {};
@@ -122,6 +125,7 @@ void free_step_workspace(casgd_ctx *c)
 {
     drop_graphs(c);
     if (c->tc_plan) { gram_tc_plan_destroy(c->tc_plan); c->tc_plan = nullptr; }
+    if (c->pair_plan) { gram_pair_plan_destroy(c->pair_plan); c->pair_plan = nullptr; }
     cudaFree(c->Y); cudaFree(c->yI); cudaFree(c->G); cudaFree(c->r); cudaFree(c->z); cudaFree(c->u);
     c->Y = nullptr; c->yI = c->G = c->r = c->z = c->u = nullptr;
     c->rows_alloc = 0;
@@ -198,8 +202,12 @@ int enqueue_step(casgd_ctx *c, cudaStream_t st, const int32_t *idx, const StepPa
     }
     {
         StageTimer t(c, CASGD_STAGE_GRAM);
-        if (c->opt_gram_impl == 1) {
+        if (c->cur_gram == 1) {
             k = launch_gram_simt(st, c->Y, c->ldy, c->n, sb, b, c->xbf, c->G, c->ldg, c->r, (int)c->opt_full_lower);
+        } else if (c->cur_gram == 3) {
+            k = launch_gram_pair(st, c->pair_plan, sb, b, c->G, c->ldg, c->r, (int)c->opt_full_lower, c->cur_bn,
+                                 (int)c->opt_ksplit, c->err, sizeof c->err);
+            if (k < 0) return CASGD_ECUDA;
         } else {
             if (!c->tc_plan) {
                 c->tc_plan = gram_tc_plan_create(c->Y, c->ldy, c->n, c->rows_alloc, c->xbf, c->ldxb, c->err, sizeof c->err);
@@ -222,6 +230,46 @@ int enqueue_step(casgd_ctx *c, cudaStream_t st, const int32_t *idx, const StepPa
         k = launch_gradient_bf16(st, c->Y, c->ldy, c->n, sb, c->u, alpha, x, ind, c->xbf, c->gws);
         t.done(k); *kernels += k;
     }
+    return CASGD_OK;
+}
+
+// Pick the Gram kernel for this shape (outside stream capture: the pair kernel's work list is uploaded here).
+// CASGD_OPT_GRAM_IMPL: 0 = by the cost model, 1 = CUDA cores, 2 = 128x128 tcgen05 tiles, 3 / 4 = CTA pairs with
+// 256 / 512-column tiles.
+int choose_gram(casgd_ctx *c, int32_t s, int32_t b)
+{
+    const int32_t sb = s * b;
+    const int64_t opt = c->opt_gram_impl;
+    c->cur_gram = opt == 1 ? 1 : 2;
+    c->cur_bn = 0;
+    if (opt == 1 || opt == 2 || c->num_sms < 2) return CASGD_OK;
+    if (opt == 0 && (sb < 512 || c->n < 256)) return CASGD_OK;      // too little work for 256-row tiles
+    if (!c->pair_plan) {
+        c->pair_plan = gram_pair_plan_create(c->Y, c->ldy, c->n, c->rows_alloc, c->xbf, c->ldxb, c->num_sms);
+        if (!c->pair_plan) return fail(c, CASGD_ECUDA, "cuTensorMapEncodeTiled failed for the pair Gram kernel");
+    }
+    int bn = 0;
+    const int64_t span = gram_pair_prepare(c->pair_plan, sb, b, (int)c->opt_full_lower, opt == 3 ? 256 : opt == 4 ? 512 : 0,
+                                           (int)c->opt_ksplit, &bn);
+    if (span < 0) {
+        if (opt >= 3) return fail(c, CASGD_EINVAL, "the pair Gram kernel cannot run s*b = %d (work list too long)", sb);
+        return CASGD_OK;
+    }
+    if (opt == 0) {
+        // 128x128 tiles: 32 KB per K block per SM at the L2 cap of ~42.6 B/cycle/SM = 770 cycles
+        const int64_t T = (sb + kTile - 1) / kTile, kbt = (c->n + 63) / 64;
+        int64_t tiles = 0;
+        for (int64_t ti = 0; ti < T; ++ti)
+            for (int64_t tj = 0; tj <= ti; ++tj) {
+                const int64_t last_row = std::min<int64_t>(ti * kTile + kTile, sb) - 1;
+                tiles += (ti == tj) || c->opt_full_lower || (last_row / b) > (tj * kTile / b);
+            }
+        int64_t ks = std::max<int64_t>(1, std::min<int64_t>(c->num_sms / std::max<int64_t>(tiles, 1), kbt / 4));
+        const int64_t span_tc = (tiles * ks + c->num_sms - 1) / c->num_sms * ((kbt + ks - 1) / ks) * 770 + 2600;
+        if (span * 10 > span_tc * 9) return CASGD_OK;               // not clearly better: stay with the simpler kernel
+    }
+    c->cur_gram = 3;
+    c->cur_bn = bn;
     return CASGD_OK;
 }
 
@@ -285,6 +333,8 @@ int run_steps(casgd_ctx *c, const int32_t *idx, int64_t n_steps, float *x, int32
     if (n_steps == 0) return CASGD_OK;
     int rc = ensure_workspace(c, sb);
     if (rc) return rc;
+    rc = choose_gram(c, s, b);
+    if (rc) return rc;
     rc = ensure_shadow(c, x);
     if (rc) return rc;
     c->last_s = s;
@@ -336,6 +386,7 @@ int casgd_init(casgd_ctx **out, const uint16_t *X_bf16, int64_t ldx, const float
     if (cudaGetDevice(&c->device) != cudaSuccess || cudaGetDeviceProperties(&prop, c->device) != cudaSuccess)
         return bail(CASGD_ECUDA);
     if (prop.major != 10) return bail(CASGD_EARCH);
+    c->num_sms = prop.multiProcessorCount;
     c->stream = (cudaStream_t)cuda_stream;
     c->y = y; c->m = m; c->n = n; c->loss = loss;
     c->ldy = (int32_t)round_up(n, 8);
@@ -528,7 +579,7 @@ int casgd_set_option(casgd_ctx *c, int option, int64_t value)
     if (!c) return CASGD_EINVAL;
     switch (option) {
     case CASGD_OPT_GRAM_IMPL:
-        if (value != 0 && value != 1) return fail(c, CASGD_EINVAL, "CASGD_OPT_GRAM_IMPL must be 0 or 1");
+        if (value < 0 || value > 4) return fail(c, CASGD_EINVAL, "CASGD_OPT_GRAM_IMPL must be in [0, 4]");
         c->opt_gram_impl = value; break;
     case CASGD_OPT_GRAM_FULL_LOWER: c->opt_full_lower = value != 0; break;
     case CASGD_OPT_PROFILE:

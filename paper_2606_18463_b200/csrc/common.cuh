@@ -205,4 +205,14 @@ void gram_tc_plan_destroy(GramTcPlan *p);
 int launch_gram_tc(cudaStream_t st, GramTcPlan *plan, int32_t sb, int32_t b, float *G, int32_t ldg, float *r,
                    int full_lower, int ksplit_opt, char *err, int errlen);
 
+// cta_group::2 Gram + margin for large shapes (gram_pair.cu): 256 x 256 / 256 x 512 tiles on CTA pairs, work lists
+// built on the host. gram_pair_prepare (outside stream capture) returns the estimated cycles, or -1.
+struct GramPairPlan;
+GramPairPlan *gram_pair_plan_create(const uint16_t *Y, int32_t ldy, int32_t n, int32_t rows_alloc, const uint16_t *xbf,
+                                    int32_t ldxb, int num_sms);
+void gram_pair_plan_destroy(GramPairPlan *p);
+int64_t gram_pair_prepare(GramPairPlan *pl, int32_t sb, int32_t b, int full_lower, int bn, int ksplit_opt, int *bn_out);
+int launch_gram_pair(cudaStream_t st, GramPairPlan *pl, int32_t sb, int32_t b, float *G, int32_t ldg, float *r,
+                     int full_lower, int bn, int ksplit_opt, char *err, int errlen);
+
 }  // namespace casgd

@@ -40,7 +40,10 @@ SMALL = [
 ]
 
 
-@pytest.mark.parametrize("gram_impl", [0, 1], ids=["umma", "simt"])
+GRAM_IMPLS = dict(argvalues=[0, 1, 2, 3, 4], ids=["auto", "simt", "tile128", "pair256", "pair512"])
+
+
+@pytest.mark.parametrize("gram_impl", **GRAM_IMPLS)
 @pytest.mark.parametrize("ci,m,n,s,b", SMALL)
 def test_one_outer_step_matches_the_oracle(binding, oracle_mod, ci, m, n, s, b, gram_impl):
     cfg = synth.config(ci, m=m, n=n)
@@ -53,7 +56,33 @@ def test_one_outer_step_matches_the_oracle(binding, oracle_mod, ci, m, n, s, b, 
             check_step_against_oracle(oracle_mod, cg, A_bits, y, idx, x0, s, b, cfg.eta, cfg.loss, binding)
 
 
-@pytest.mark.parametrize("gram_impl", [0, 1], ids=["umma", "simt"])
+# shapes that span several 256-row pair tiles with a ragged tail, for the cta_group::2 Gram kernel
+PAIR_SHAPES = [
+    (4, 6000, 512, 9, 128),      # sb = 1152 = 4.5 pair tiles; b = 128: the block diagonal cuts every diagonal tile
+    (3, 5000, 336, 40, 32),      # sb = 1280, K tail (336 = 5*64 + 16)
+    (2, 4000, 1024, 17, 64),     # sb = 1088: a 64-row tail
+]
+
+
+@pytest.mark.parametrize("ksplit", [0, 3])
+@pytest.mark.parametrize("gram_impl", [0, 2, 3, 4], ids=["auto", "tile128", "pair256", "pair512"])
+@pytest.mark.parametrize("ci,m,n,s,b", PAIR_SHAPES)
+def test_pair_gram_kernel_matches_the_oracle(binding, oracle_mod, ci, m, n, s, b, gram_impl, ksplit):
+    cfg = synth.config(ci, m=m, n=n)
+    X_d, y_d, A_bits, y = device_dataset(cfg)
+    eta = cfg.eta if cfg.loss != synth.POISSON else 0.01
+    with binding.Casgd(X_d, y_d, cfg.loss) as cg:
+        cg.set_option(binding.OPT_GRAM_IMPL, gram_impl)
+        cg.set_option(binding.OPT_GRAM_KSPLIT, ksplit)
+        for rep, full in enumerate((0, 1)):
+            cg.set_option(binding.OPT_GRAM_FULL_LOWER, full)
+            idx = synth.iid_indices(m, s * b, 200 + rep)
+            x0 = random_x(n, 17 + rep, 0.3 if cfg.loss != synth.POISSON else 0.1)
+            check_step_against_oracle(oracle_mod, cg, A_bits, y, idx, x0, s, b, eta, cfg.loss, binding,
+                                      full_lower=bool(full))
+
+
+@pytest.mark.parametrize("gram_impl", **GRAM_IMPLS)
 def test_full_lower_triangle_and_duplicates(binding, oracle_mod, gram_impl):
     """i.i.d. sampling with replacement (Alg. 1 line 1) gives duplicate rows inside and
     across blocks; with CASGD_OPT_GRAM_FULL_LOWER the whole lower triangle (diagonal G_ii = ||y_i||^2
