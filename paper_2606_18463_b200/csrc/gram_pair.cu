@@ -507,7 +507,7 @@ int64_t gram_pair_prepare(GramPairPlan *pl, int32_t sb, int32_t b, int full_lowe
             // K split: try the candidates and keep the shortest estimated makespan
             for (int ks = 1; ks <= std::min(kbt, 16); ++ks) {
                 if (ksplit_opt > 0 && ks != std::min(ksplit_opt, kbt)) continue;
-                if (ksplit_opt <= 0 && ks > 1 && kbt / ks < 4) break;       // keep >= 4 K blocks per slice
+                if (ksplit_opt <= 0 && ks > 1 && kbt / ks < 16) break;      // keep >= 16 K blocks per slice
                 if (ksplit_opt <= 0 && ks > 1 && n_g_items * (ks - 1) >= pl->npairs) break;   // split only to fill idle pairs
                 int64_t sp = 0;
                 if (!build_items(sb, b, pl->n, full_lower, cand, ks, pl->npairs, per_pair, &sp)) continue;

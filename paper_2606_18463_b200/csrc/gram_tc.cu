@@ -30,7 +30,9 @@ constexpr uint32_t kOffB = 0, kOffX = kTileBytes, kOffA = kTileBytes + kXBytes;
 constexpr uint32_t kAccCols = 256;                      // TMEM columns per accumulator slot (144 used)
 constexpr uint32_t kTmemCols = 512;
 constexpr int kThreads = 192;
-constexpr size_t kSmemBytes = 1024 + (size_t)kStages * kStageBytes + 256;
+constexpr int kEpiStride = 36;                          // floats per row of an epilogue transpose buffer (conflict-free)
+constexpr uint32_t kEpiBufB = 32 * kEpiStride * 4;       // per epilogue warp
+constexpr size_t kSmemBytes = 1024 + (size_t)kStages * kStageBytes + 256 + 4 * kEpiBufB;
 
 struct GramParams {
     float *G;
@@ -66,6 +68,12 @@ __device__ __forceinline__ void tma_load_2d(uint32_t dst, const CUtensorMap *map
 {
     asm volatile("cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4}], [%2];"
                  ::"r"(dst), "l"((uint64_t)map), "r"(bar), "r"(c0), "r"(c1) : "memory");
+}
+__device__ __forceinline__ bool elect_one()
+{
+    uint32_t pred;
+    asm volatile("{\n.reg .pred P;\nelect.sync _|P, 0xffffffff;\nselp.u32 %0, 1, 0, P;\n}" : "=r"(pred));
+    return pred != 0;
 }
 __device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
 __device__ __forceinline__ void tc_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
@@ -202,8 +210,10 @@ gram_tc_kernel(const __grid_constant__ CUtensorMap tmY, const __grid_constant__ 
             }
         }
     } else if (warp == 1) {
-        // ===== MMA issuer =====
-        if (lane == 0) {
+        // ===== MMA issuer: the whole warp runs the loops (uniform control flow keeps the descriptors in uniform
+        // registers), one elected lane issues. With a lane-0-only branch every operand is a per-thread register
+        // that has to be moved to a uniform register around each tcgen05.mma (measured: ~2x the 64-cycle floor). =====
+        {
             int stage = 0;
             uint32_t phase = 0;
             int it = 0;
@@ -219,20 +229,32 @@ gram_tc_kernel(const __grid_constant__ CUtensorMap tmY, const __grid_constant__ 
                 // diagonal tile: A = B = the same smem tile; N = 144 (G tile + margin rows) or 16 (margin only)
                 const uint32_t ncols = k.diag ? (k.need_g ? (uint32_t)(BN + XR) : (uint32_t)XR) : (uint32_t)BN;
                 const uint32_t idesc = umma_idesc(ncols);
+                const uint32_t offa = k.diag ? kOffB : kOffA, offb = (k.diag && !k.need_g) ? kOffX : kOffB;
                 for (int kb = k.kb0; kb < k.kb1; ++kb) {
                     mbar_wait(full_bar(stage), phase);
                     tc_fence_after();
                     const uint32_t sbase = smem_base + stage * kStageBytes;
-                    const uint64_t adesc = umma_desc_sw128(sbase + (k.diag ? kOffB : kOffA));
-                    const uint64_t bdesc = umma_desc_sw128(sbase + ((k.diag && !k.need_g) ? kOffX : kOffB));
+                    const uint64_t adesc = umma_desc_sw128(sbase + offa);
+                    const uint64_t bdesc = umma_desc_sw128(sbase + offb);
                     const int kcols = min(p.n - kb * BK, BK);
                     const int ksteps = (kcols + 15) >> 4;                  // zero-filled K tail beyond n is skipped
-                    for (int ks = 0; ks < ksteps; ++ks)
-                        tc_mma_bf16(d_tmem, adesc + 2u * ks, bdesc + 2u * ks, idesc, (kb > k.kb0 || ks > 0) ? 1u : 0u);
-                    tc_commit(empty_bar(stage));                           // frees the smem slot when the MMAs retire
+                    const uint32_t first = kb > k.kb0 ? 1u : 0u;
+                    if (elect_one()) {
+                        if (ksteps == 4) {                                 // a full K block: straight-line issue
+                            tc_mma_bf16(d_tmem, adesc, bdesc, idesc, first);
+                            tc_mma_bf16(d_tmem, adesc + 2u, bdesc + 2u, idesc, 1u);
+                            tc_mma_bf16(d_tmem, adesc + 4u, bdesc + 4u, idesc, 1u);
+                            tc_mma_bf16(d_tmem, adesc + 6u, bdesc + 6u, idesc, 1u);
+                        } else {
+                            for (int ks = 0; ks < ksteps; ++ks)
+                                tc_mma_bf16(d_tmem, adesc + 2u * ks, bdesc + 2u * ks, idesc, ks > 0 ? 1u : first);
+                        }
+                        tc_commit(empty_bar(stage));                       // frees the smem slot when the MMAs retire
+                        if (kb == k.kb1 - 1) tc_commit(accf_bar(slot));    // accumulator ready for the epilogue
+                    }
+                    __syncwarp();
                     if (++stage == kStages) { stage = 0; phase ^= 1u; }
                 }
-                tc_commit(accf_bar(slot));                                 // accumulator ready for the epilogue
             }
         }
     } else {
@@ -240,6 +262,7 @@ gram_tc_kernel(const __grid_constant__ CUtensorMap tmY, const __grid_constant__ 
         const int q = warp & 3;
         int it = 0;
         const bool accumulate = p.ksplit > 1;
+        const uint32_t ebuf = bar_base + 256 + (uint32_t)(warp - 2) * kEpiBufB;
         for (int w = blockIdx.x; w < nwork; w += gridDim.x) {
             const Work k = decode_work(p, w);
             if (k.skip) continue;
@@ -252,22 +275,33 @@ gram_tc_kernel(const __grid_constant__ CUtensorMap tmY, const __grid_constant__ 
             const int row = k.ti * BM + q * 32 + lane;
             const bool row_ok = row < p.sb;
             if (k.need_g) {
-                float *grow = p.G + (int64_t)row * p.ldg + k.tj * BN;
 #pragma unroll 1
                 for (int c = 0; c < BN / 32; ++c) {
                     uint32_t v[32];
                     tc_ld32(t_row + c * 32, v);
                     tc_wait_ld();
-                    if (row_ok) {
-                        if (!accumulate) {
+                    // transpose through shared memory so that every store instruction writes whole 128-byte lines
 #pragma unroll
-                            for (int e = 0; e < 32; e += 4)
-                                *reinterpret_cast<uint4 *>(grow + c * 32 + e) = make_uint4(v[e], v[e + 1], v[e + 2], v[e + 3]);
-                        } else {
+                    for (int e = 0; e < 32; e += 4)
+                        asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(ebuf + (uint32_t)(lane * kEpiStride + e) * 4u),
+                                     "r"(v[e]), "r"(v[e + 1]), "r"(v[e + 2]), "r"(v[e + 3]) : "memory");
+                    __syncwarp();
+                    const int c4 = (lane & 7) * 4;
 #pragma unroll
-                            for (int e = 0; e < 32; ++e) atomicAdd(grow + c * 32 + e, __uint_as_float(v[e]));
+                    for (int i = 0; i < 8; ++i) {
+                        const int rl = 4 * i + (lane >> 3);
+                        uint32_t o0, o1, o2, o3;
+                        asm volatile("ld.shared.v4.b32 {%0, %1, %2, %3}, [%4];" : "=r"(o0), "=r"(o1), "=r"(o2), "=r"(o3)
+                                     : "r"(ebuf + (uint32_t)(rl * kEpiStride + c4) * 4u) : "memory");
+                        const int orow = k.ti * BM + q * 32 + rl;
+                        if (orow < p.sb) {
+                            float *dst = p.G + (int64_t)orow * p.ldg + k.tj * BN + c * 32 + c4;
+                            if (!accumulate) *reinterpret_cast<uint4 *>(dst) = make_uint4(o0, o1, o2, o3);
+                            else asm volatile("red.global.add.v4.f32 [%0], {%1, %2, %3, %4};" ::"l"(dst), "f"(__uint_as_float(o0)),
+                                              "f"(__uint_as_float(o1)), "f"(__uint_as_float(o2)), "f"(__uint_as_float(o3)) : "memory");
                         }
                     }
+                    __syncwarp();
                 }
             }
             if (k.diag) {
@@ -370,9 +404,10 @@ int launch_gram_tc(cudaStream_t st, GramTcPlan *plan, int32_t sb, int32_t b, flo
     p.full_lower = full_lower;
     int ksplit = ksplit_opt;
     if (ksplit <= 0) {
-        // fill the 148 SMs when there are few tiles, keeping >= 4 K-blocks (256 columns) per slice
+        // fill the 148 SMs when there are few tiles -- but the cleared G, its memset node and the red.add epilogue
+        // cost several microseconds, so only when a slice still holds >= 16 K blocks (1024 columns)
         ksplit = kNumSMsB200 / p.ntiles;
-        ksplit = std::min(ksplit, p.kb_total / 4);
+        ksplit = std::min(ksplit, p.kb_total / 16);
     }
     ksplit = std::max(1, std::min(ksplit, p.kb_total));
     p.ksplit = ksplit;
