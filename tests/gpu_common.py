@@ -54,19 +54,24 @@ def block_lower_mask(s, b):
 def check_step_against_oracle(oracle, cg, A_bits, y, idx, x0, s, b, eta, loss, binding, full_lower=False,
                               check_g=True, tol_scale=1.0):
     """Run one casgd_outer_step from the FP32 bits x0 and compare every exported intermediate with O1."""
-    sb = s * b
-    n = A_bits.shape[1]
     idx_d = torch.from_numpy(idx).cuda()
     x_d = torch.from_numpy(x0.copy()).cuda()
     cg.invalidate_shadow()
     cg.outer_step(idx_d, x_d, s, b, eta)
     cg.sync()
     ref = oracle.outer_step_gram(A_bits, y, idx, x0.astype(np.float64), s, b, eta, loss, shadow=True)
+    return compare_last_step(oracle, cg, ref, y[idx], x0, x_d, s, b, eta, loss, binding, full_lower, check_g, tol_scale)
 
+
+def compare_last_step(oracle, cg, ref, y_idx, x0, x_d, s, b, eta, loss, binding, full_lower=False, check_g=True,
+                      tol_scale=1.0):
+    """Compare the intermediates of the LAST outer step the context ran (casgd_debug_export) and the iterate
+    `x_d` it left with `ref`, oracle O1's result for the same rows, labels `y_idx`, indices and FP32 x0 bits."""
+    sb = s * b
     # gather: bit-exact rows and labels (Alg. 1 line 2)
     Y = cg.debug(binding.DBG_Y)
     assert Y.dtype == np.uint16 and np.array_equal(Y, ref.Y_bits), "gathered rows differ bitwise"
-    assert np.array_equal(cg.debug(binding.DBG_YLAB), y[idx]), "gathered labels differ bitwise"
+    assert np.array_equal(cg.debug(binding.DBG_YLAB), y_idx), "gathered labels differ bitwise"
 
     Yf = oracle.bf16_to_f64(ref.Y_bits)
     norms = np.sqrt((Yf * Yf).sum(axis=1))

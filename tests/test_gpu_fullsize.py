@@ -1,0 +1,122 @@
+"""GPU parity at BASELINE.json's FULL sizes, in the launch configuration bench.py times.
+
+bench.py times casgd_outer_steps (CUDA-graph replay, programmatic dependent launch) on the full-size synthetic
+datasets drawn on the GPU generator. Here the same call runs two outer iterations from x = 0 on those datasets;
+the SECOND iteration (a generic iterate, BF16 shadow maintained by the fused update, kernels replayed from the
+graph) is compared element by element with oracle O1 started from the first iteration's FP32 x bits:
+gathered rows and labels bit-exact, G, r, z, u, x and the shadow within tests/gpu_common.py's tolerances.
+Only the rows the step touches are brought to the host (the oracle sees the same BF16 bits, labels, indices).
+casgd_loss is checked at full size too (second test): F(0) in closed form, and for a generic x the full-matrix F
+against the row-weighted mean of F over a partition of the rows, one slice of which goes through the oracle.
+"""
+import math
+
+import numpy as np
+import pytest
+import torch
+
+from paper_2606_18463_b200 import synth
+
+from gpu_common import TOL_LOSS_CALL, compare_last_step, require_cuda
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def binding():
+    require_cuda()
+    from paper_2606_18463_b200 import build
+    build.build()
+    from paper_2606_18463_b200 import binding as b
+    b.load()
+    return b
+
+
+def _host_rows(ds, idx):
+    """The rows of the device dataset that `idx` touches: compact BF16 bits, labels, and idx remapped to them."""
+    uniq, inv = np.unique(idx, return_inverse=True)
+    sel = torch.from_numpy(uniq.astype(np.int64)).to(ds.X_bf16.device)
+    A_bits = ds.X_bf16[sel].contiguous().view(torch.int16).cpu().numpy().view(np.uint16)
+    y = ds.y[sel].cpu().numpy()
+    return A_bits, y, inv.astype(np.int32)
+
+
+# (config index, s): every config at its headline s of bench.py, plus the largest s of the two tensor-bound sweeps
+FULL = [(0, 4), (1, 16), (1, 32), (2, 32), (3, 16), (3, 64), (4, 32)]
+
+
+@pytest.mark.parametrize("ci,s", FULL)
+def test_second_graph_step_at_full_size_matches_the_oracle(binding, oracle_mod, ci, s):
+    cfg = synth.config(ci)
+    need = cfg.m * max(cfg.n, 32) * 2 * 1.3 + (1 << 30)
+    free, _ = torch.cuda.mem_get_info()
+    assert free > need, f"{cfg.name} needs {need / 1e9:.1f} GB of device memory, {free / 1e9:.1f} GB free"
+    ds = synth.make_dataset(cfg, seed=42, device="cuda")
+    b, sb = cfg.b, s * cfg.b
+    idx = synth.epoch_indices(cfg, 42, 0)[: 2 * sb].copy()
+    idx_d = torch.from_numpy(idx).cuda()
+    stream = torch.cuda.Stream()
+    with torch.cuda.stream(stream):
+        cg = binding.Casgd(ds.X_bf16, ds.y, cfg.loss, stream=stream)
+    try:
+        # the first iteration alone (direct launches), to learn the FP32 bits the second one starts from
+        x1 = torch.zeros(cfg.n, device="cuda")
+        cg.outer_step(idx_d[:sb], x1, s, b, cfg.eta)
+        cg.sync()
+        x1_host = x1.cpu().numpy().copy()
+        # both iterations the way bench.py runs them: one casgd_outer_steps call, replayed from a CUDA graph
+        x2 = torch.zeros(cfg.n, device="cuda")
+        n0 = cg.launch_count()
+        cg.outer_steps(idx_d, x2, s, b, cfg.eta, n_steps=2)
+        cg.sync()
+        assert cg.launch_count() - n0 >= 8
+        A_bits, y, local = _host_rows(ds, idx[sb:])
+        ref = oracle_mod.outer_step_gram(A_bits, y, local, x1_host.astype(np.float64), s, b, cfg.eta, cfg.loss, shadow=True)
+        compare_last_step(oracle_mod, cg, ref, y[local], x1_host, x2, s, b, cfg.eta, cfg.loss, binding)
+        # the first iteration from x = 0 has a closed form for its first block (r = 0): u_0 = l'(0, y)
+        y0 = ds.y[torch.from_numpy(idx[:b].astype(np.int64)).cuda()].cpu().numpy().astype(np.float64)
+        u0 = {0: -y0 / 2, 1: -y0, 2: 1 - y0}[cfg.loss]
+        xs = torch.zeros(cfg.n, device="cuda")
+        cg.invalidate_shadow()
+        cg.outer_step(idx_d[:b], xs, 1, b, cfg.eta)
+        cg.sync()
+        assert np.allclose(cg.debug(binding.DBG_U).astype(np.float64), u0, rtol=1e-6, atol=1e-7)
+    finally:
+        cg.close()
+        del ds
+
+
+@pytest.mark.parametrize("ci", [1, 2, 3, 4])
+def test_full_size_loss_is_the_row_weighted_mean_of_slice_losses(binding, oracle_mod, ci):
+    """casgd_loss over all m rows (the streaming kernel at the size bench.py's GEMV line times) against what is
+    unique about it: F(0) in closed form, and for a generic x the row-weighted mean of F over a partition of the
+    rows into slices, where the slice that is small enough for the host goes through the ORACLE and the rest
+    through contexts of their own (so every row of the full matrix is summed by the kernel under test twice, in
+    two different launch geometries, and one slice by the oracle)."""
+    cfg = synth.config(ci)
+    ds = synth.make_dataset(cfg, seed=42, device="cuda")
+    try:
+        x = (torch.randn(cfg.n, generator=torch.Generator().manual_seed(5)) * 0.2).cuda()
+        with binding.Casgd(ds.X_bf16, ds.y, cfg.loss) as cg:
+            F0 = cg.loss(torch.zeros(cfg.n, device="cuda"))
+            F = cg.loss(x)
+        ymean2 = float((ds.y.double() ** 2).mean().item()) / 2
+        closed = {0: math.log(2.0), 1: ymean2, 2: 1.0}[cfg.loss]
+        assert F0 == pytest.approx(closed, rel=1e-6)
+        # partition: an oracle slice of ~64 MB of BF16 at an odd offset, and the two device slices around it
+        rows_o = max(1, min(cfg.m // 3, (64 << 20) // (2 * cfg.n)))
+        lo = (cfg.m // 2) | 1
+        hi = lo + rows_o
+        parts = []
+        A_bits = ds.X_bf16[lo:hi].contiguous().view(torch.int16).cpu().numpy().view(np.uint16)
+        F_o = oracle_mod.full_loss(A_bits, ds.y[lo:hi].cpu().numpy(), x.cpu().numpy().astype(np.float64), cfg.loss)
+        parts.append((rows_o, F_o))
+        with binding.Casgd(ds.X_bf16[lo:hi].contiguous(), ds.y[lo:hi].contiguous(), cfg.loss) as cs:
+            assert abs(cs.loss(x) - F_o) <= TOL_LOSS_CALL * abs(F_o)       # the kernel on the oracle's slice
+        for a, e in ((0, lo), (hi, cfg.m)):
+            with binding.Casgd(ds.X_bf16[a:e], ds.y[a:e], cfg.loss) as cs:   # row slices are contiguous views
+                parts.append((e - a, cs.loss(x)))
+        F_parts = sum(r * f for r, f in parts) / cfg.m
+        assert abs(F - F_parts) <= 2 * TOL_LOSS_CALL * abs(F_parts)
+    finally:
+        del ds
