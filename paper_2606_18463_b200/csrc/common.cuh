@@ -110,7 +110,16 @@ __device__ __forceinline__ uint4 ldg_nc_v4(const void *p)
 // scheduled (and run their prologue) while the previous kernel drains, and block in pdl_wait() until it has
 // completed and its writes are visible. Every kernel of the step path calls pdl_trigger() first thing and
 // pdl_wait() before it touches anything another kernel of the chain writes or reads.
+// IMPORTANT: what another kernel of the chain wrote must NOT be read through a `const T *__restrict__` pointer or
+// __ldg: the compiler treats such data as read-only for the whole kernel and may hoist the load ABOVE pdl_wait()
+// (seen: a gradient kernel summing the previous step's u). Such inputs are plain pointers, or go through ld_dep().
 __device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+__device__ __forceinline__ float ld_dep(const float *p)
+{
+    float v;
+    asm volatile("ld.global.f32 %0, [%1];" : "=f"(v) : "l"(p) : "memory");
+    return v;
+}
 __device__ __forceinline__ void pdl_trigger() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
 
 // cudaLaunchKernelEx with the programmatic-serialisation attribute (and a cluster dimension when cluster > 1).

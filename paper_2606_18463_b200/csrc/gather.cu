@@ -9,8 +9,8 @@ namespace casgd {
 // masked to n so that the pad columns [n, ldy) of Y are always zero whatever A's padding holds.
 __global__ void __launch_bounds__(256)
 gather_rows_kernel(const uint16_t *__restrict__ A, int64_t lda, const float *__restrict__ y, int64_t m, int32_t n,
-                   const int32_t *__restrict__ idx, const StepParams *__restrict__ ind, int64_t idx_off, int32_t sb,
-                   uint16_t *__restrict__ Y, int32_t ldy, float *__restrict__ yI, int *__restrict__ err_flag)
+                   const int32_t *idx, const StepParams *ind, int64_t idx_off, int32_t sb,
+                   uint16_t *Y, int32_t ldy, float *yI, int *err_flag)
 {
     pdl_trigger();
     pdl_wait();                                     // Y is still being read by the previous step's gradient
@@ -44,10 +44,126 @@ gather_rows_kernel(const uint16_t *__restrict__ A, int64_t lda, const float *__r
     }
 }
 
+// Wide rows (n % 8 == 0, >= 512 bytes): the gather is pure data movement, so it is done by the copy engine alone.
+// One lane per warp drives a ring of kGbDepth 4 KB shared-memory slots (kGbAhead loads in flight): cp.async.bulk global -> shared for a piece
+// of a sampled row, then cp.async.bulk shared -> global into the Y stage; no byte passes through a register, and
+// each SM keeps ~100 KB of reads in flight. The row indices of a warp's next 32 rows are loaded by its 32 lanes
+// at once. Labels and the out-of-range check are done by the first warps of the grid, element-wise.
+constexpr int kGbWarps = 8, kGbDepth = 6, kGbAhead = 4;
+constexpr uint32_t kGbSlot = 4096;
+
+__global__ void __launch_bounds__(32 * kGbWarps, 1)
+gather_bulk_kernel(const uint16_t *__restrict__ A, int64_t lda, const float *__restrict__ y, int64_t m, int32_t n,
+                   const int32_t *idx, const StepParams *ind, int64_t idx_off, int32_t sb,
+                   uint16_t *Y, int32_t ldy, float *yI, int *err_flag)
+{
+    extern __shared__ __align__(128) unsigned char gb_smem[];
+    __shared__ __align__(8) unsigned long long bars[kGbWarps * kGbDepth];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    pdl_trigger();
+    const uint32_t ring = (uint32_t)__cvta_generic_to_shared(gb_smem) + (uint32_t)warp * (kGbDepth * kGbSlot);
+    const uint32_t bar0 = (uint32_t)__cvta_generic_to_shared(bars) + 8u * (uint32_t)(warp * kGbDepth);
+    if (lane == 0) {
+#pragma unroll
+        for (int d = 0; d < kGbDepth; ++d)
+            asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(bar0 + 8u * d) : "memory");
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncwarp();
+    pdl_wait();                                     // Y is still being read by the previous step's gradient
+    const int32_t *I = ind ? ind->idx + idx_off : idx;
+    const int gw = blockIdx.x * kGbWarps + warp, W = gridDim.x * kGbWarps;
+
+    // labels (and the range check): one thread per sampled row
+    for (int row = blockIdx.x * blockDim.x + threadIdx.x; row < sb; row += gridDim.x * blockDim.x) {
+        const int64_t src = I[row];
+        const bool ok = src >= 0 && src < m;
+        yI[row] = ok ? y[src] : 0.f;
+        if (!ok) atomicOr(err_flag, 1);
+    }
+
+    const uint32_t rowB = (uint32_t)n * 2u;                                 // a multiple of 16
+    const int ppr = (int)((rowB + kGbSlot - 1) / kGbSlot);                  // pieces per row
+    const int my_rows = gw < sb ? (sb - 1 - gw) / W + 1 : 0;                // rows gw, gw + W, ...
+    const int total = my_rows * ppr;
+    int64_t src_row = 0, src_prev = 0;                                      // lane k: source row of the k-th row of this / the previous batch of 32
+    uint32_t phase_bits = 0;                                                // per-slot parity of the full barriers
+    // software pipeline over pieces: loads run kGbAhead pieces ahead of the stores; a slot is loaded again
+    // kGbDepth - kGbAhead iterations after its store was committed
+    for (int p = 0; p < total + kGbAhead; ++p) {
+        if (p < total) {
+            const int k = p / ppr, piece = p - k * ppr;
+            if (piece == 0 && (k & 31) == 0) {                              // a new batch of 32 rows: one index per lane
+                const int kk = k + lane;
+                src_prev = src_row;
+                src_row = kk < my_rows ? (int64_t)I[gw + kk * W] : 0;
+            }
+            const int64_t src = __shfl_sync(0xffffffffu, src_row, k & 31);
+            const bool ok = src >= 0 && src < m;
+            const uint32_t off = (uint32_t)piece * kGbSlot, bytes = min(kGbSlot, rowB - off);
+            const int slot = p % kGbDepth;
+            const uint32_t dst = ring + (uint32_t)slot * kGbSlot, bar = bar0 + 8u * slot;
+            if (ok) {
+                if (lane == 0) {
+                    // the store that last read this slot has finished reading it
+                    asm volatile("cp.async.bulk.wait_group.read %0;" ::"n"(kGbDepth - kGbAhead - 1) : "memory");
+                    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+                    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                                 ::"r"(dst), "l"(A + src * lda + off / 2), "r"(bytes), "r"(bar) : "memory");
+                }
+            } else {
+                // an out-of-range index reads as a zero row: written by the lanes, nothing goes through the ring
+                unsigned char *yrow = reinterpret_cast<unsigned char *>(Y + (int64_t)(gw + k * W) * ldy) + off;
+                for (uint32_t e = lane * 16u; e < bytes; e += 512u) *reinterpret_cast<uint4 *>(yrow + e) = make_uint4(0u, 0u, 0u, 0u);
+                if (lane == 0) asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
+            }
+        }
+        const int q = p - kGbAhead;                                         // the piece to store now
+        if (q >= 0) {
+            const int k = q / ppr, piece = q - k * ppr;
+            const int slot = q % kGbDepth;
+            const uint32_t srcs = ring + (uint32_t)slot * kGbSlot, bar = bar0 + 8u * slot;
+            const uint32_t off = (uint32_t)piece * kGbSlot, bytes = min(kGbSlot, rowB - off);
+            const uint32_t parity = (phase_bits >> slot) & 1u;
+            phase_bits ^= 1u << slot;
+            const int k_load = min(p, total - 1) / ppr;                     // the loads are at most one batch ahead
+            const int64_t src = __shfl_sync(0xffffffffu, (k >> 5) == (k_load >> 5) ? src_row : src_prev, k & 31);
+            if (lane == 0) {
+                uint32_t done;
+                do {
+                    asm volatile("{\n.reg .pred p;\nmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\nselp.u32 %0, 1, 0, p;\n}"
+                                 : "=r"(done) : "r"(bar), "r"(parity) : "memory");
+                } while (!done);
+                if (src >= 0 && src < m) {
+                    unsigned char *yrow = reinterpret_cast<unsigned char *>(Y + (int64_t)(gw + k * W) * ldy) + off;
+                    asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;" ::"l"(yrow), "r"(srcs), "r"(bytes) : "memory");
+                }
+                asm volatile("cp.async.bulk.commit_group;" ::: "memory");
+            }
+            __syncwarp();
+        }
+    }
+    if (lane == 0) asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");   // the stores have landed before the CTA exits
+}
+
 int launch_gather(cudaStream_t st, const uint16_t *A, int64_t lda, const float *y, int64_t m, int32_t n,
                   const int32_t *idx, const StepParams *ind, int64_t idx_off, int32_t sb, uint16_t *Y, int32_t ldy,
                   float *yI, int *err_flag)
 {
+    if (n % 8 == 0 && n * 2 >= 512 && ldy == n && (int64_t)sb * n * 2 >= (1 << 20)) {
+        static bool attr_set = false;
+        const size_t smem = (size_t)kGbWarps * kGbDepth * kGbSlot;
+        if (!attr_set) {
+            cudaFuncSetAttribute(gather_bulk_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+            attr_set = true;
+        }
+        const int ppr = (n * 2 + (int)kGbSlot - 1) / (int)kGbSlot;
+        const int64_t pieces = (int64_t)sb * ppr;
+        const int blocks = (int)std::max<int64_t>(1, std::min<int64_t>(kNumSMsB200, (pieces + kGbWarps * 2 - 1) / (kGbWarps * 2)));
+        launch_pdl(gather_bulk_kernel, dim3(blocks), dim3(32 * kGbWarps), smem, st, 1, A, lda, y, m, n, idx, ind, idx_off, sb, Y,
+                   ldy, yI, err_flag);
+        return 1;
+    }
     const int64_t total = (int64_t)sb * (ldy >> 3);
     const int threads = 256;
     const unsigned blocks = (unsigned)((total + threads - 1) / threads);
@@ -57,8 +173,8 @@ int launch_gather(cudaStream_t st, const uint16_t *A, int64_t lda, const float *
 }
 
 // x_bf = bf16_rne(x): the margin kernel's view of the weights.
-__global__ void shadow_kernel(const float *__restrict__ x, const StepParams *__restrict__ ind, int32_t n,
-                              uint16_t *__restrict__ xbf)
+__global__ void shadow_kernel(const float *x, const StepParams *ind, int32_t n,
+                              uint16_t *xbf)
 {
     pdl_trigger();
     pdl_wait();

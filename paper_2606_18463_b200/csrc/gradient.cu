@@ -35,10 +35,10 @@ constexpr int kGradThreads = 256;
 // GATHER: rows are base + idx[row]*ld (FP32 baseline), else base + row*ld (the staged Y).
 template <typename T, bool GATHER, bool SHADOW>
 __global__ void __launch_bounds__(kGradThreads)
-gradient_update_kernel(const T *__restrict__ base, int64_t ld, const int32_t *__restrict__ idx, int64_t m, int32_t n,
-                       int32_t rows, int32_t rows_per_split, int32_t CV, const float *__restrict__ u, float alpha,
-                       float *__restrict__ x_direct, const StepParams *__restrict__ ind, uint16_t *__restrict__ xbf,
-                       float *__restrict__ partial, int32_t ldp, unsigned *__restrict__ counters)
+gradient_update_kernel(const T *base, int64_t ld, const int32_t *idx, int64_t m, int32_t n,
+                       int32_t rows, int32_t rows_per_split, int32_t CV, const float *u, float alpha,
+                       float *x_direct, const StepParams *ind, uint16_t *xbf,
+                       float *partial, int32_t ldp, unsigned *counters)
 {
     constexpr int kVec = VecTraits<T>::kVec;
     pdl_trigger();
@@ -111,6 +111,151 @@ gradient_update_kernel(const T *__restrict__ base, int64_t ld, const int32_t *__
     if (tid == 0) counters[blockIdx.x] = 0u;
 }
 
+// ------------------------------------------------------------------ wide rows: streamed through the copy engine ---
+// For rows of >= 512 bytes the BF16 path uses gradient_stream_kernel: a CTA of 16 warps takes a slab of rows and a
+// segment of 1024 columns; every warp streams its own rows' 2 KB pieces through a private ring of shared-memory
+// slots with cp.async.bulk (lane 0 issues; ~100 KB of reads in flight per SM), each lane keeps 32 column sums in
+// registers (u broadcast by shuffle), the 16 warps' sums are added through shared memory, one partial per CTA is
+// written, and the last CTA of a column segment adds the partials in a fixed order and applies the update.
+constexpr int kGsWarps = 16, kGsDepth = 4, kGsSegCols = 1024;
+constexpr uint32_t kGsPiece = kGsSegCols * 2;                 // bytes of one row piece
+constexpr size_t kGsSmem = (size_t)kGsWarps * kGsDepth * kGsPiece + (size_t)kGsWarps * kGsSegCols * 4;
+
+__global__ void __launch_bounds__(32 * kGsWarps, 1)
+gradient_stream_kernel(const uint16_t *Y, int32_t ldy, int32_t n, int32_t sb, int32_t rpw,
+                       const float *u, float alpha, float *x_direct,
+                       const StepParams *ind, uint16_t *xbf, float *partial,
+                       int32_t ldp, unsigned *counters)
+{
+    extern __shared__ __align__(128) unsigned char gs_smem[];
+    __shared__ __align__(8) unsigned long long bars[kGsWarps * kGsDepth];
+    __shared__ bool s_last;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    pdl_trigger();
+    const uint32_t ring = (uint32_t)__cvta_generic_to_shared(gs_smem) + (uint32_t)warp * (kGsDepth * kGsPiece);
+    float *red = reinterpret_cast<float *>(gs_smem + (size_t)kGsWarps * kGsDepth * kGsPiece);      // [16][1024]
+    const uint32_t bar0 = (uint32_t)__cvta_generic_to_shared(bars) + 8u * (uint32_t)(warp * kGsDepth);
+    if (lane == 0) {
+#pragma unroll
+        for (int d = 0; d < kGsDepth; ++d)
+            asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(bar0 + 8u * d) : "memory");
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncwarp();
+    pdl_wait();
+
+    const int col0 = blockIdx.x * kGsSegCols;
+    const uint32_t segB = min(kGsPiece, (uint32_t)(ldy - col0) * 2u);       // a multiple of 16 (ldy % 8 == 0)
+    const int r0 = min(sb, (blockIdx.y * kGsWarps + warp) * rpw), r1 = min(sb, r0 + rpw);
+    const int nrows = r1 - r0;                                              // <= 32
+    const float u_mine = lane < nrows ? ld_dep(u + r0 + lane) : 0.f;
+    const uint16_t *src = Y + (int64_t)r0 * ldy + col0;
+    auto issue = [&](int k) {
+        if (k < nrows && lane == 0) {
+            const uint32_t bar = bar0 + 8u * (k % kGsDepth);
+            asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(segB) : "memory");
+            asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                         ::"r"(ring + (uint32_t)(k % kGsDepth) * kGsPiece), "l"(src + (int64_t)k * ldy), "r"(segB), "r"(bar) : "memory");
+        }
+    };
+#pragma unroll 1
+    for (int k = 0; k < kGsDepth - 1; ++k) issue(k);
+    float acc[4][8];
+#pragma unroll
+    for (int c = 0; c < 4; ++c)
+#pragma unroll
+        for (int e = 0; e < 8; ++e) acc[c][e] = 0.f;
+#pragma unroll 1
+    for (int k = 0; k < nrows; ++k) {
+        issue(k + kGsDepth - 1);                        // into the slot consumed in the previous iteration
+        const float uu = __shfl_sync(0xffffffffu, u_mine, k);
+        const uint32_t bar = bar0 + 8u * (k % kGsDepth), parity = (uint32_t)(k / kGsDepth) & 1u;
+        uint32_t done;
+        do {
+            asm volatile("{\n.reg .pred p;\nmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\nselp.u32 %0, 1, 0, p;\n}"
+                         : "=r"(done) : "r"(bar), "r"(parity) : "memory");
+        } while (!done);
+        const uint32_t sbase = ring + (uint32_t)(k % kGsDepth) * kGsPiece + (uint32_t)lane * 16u;
+#pragma unroll
+        for (int c = 0; c < 4; ++c) {
+            if ((uint32_t)(lane + 32 * c) * 16u < segB) {
+                uint4 v;
+                asm volatile("ld.shared.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "r"(sbase + 512u * c));
+                VecTraits<uint16_t>::fma_into(acc[c], v, uu);
+            }
+        }
+        __syncwarp();                                   // every lane is done with the slot before it is refilled
+    }
+    // add the 16 warps' column sums: red[warp][col], col = (lane + 32 c) * 8 + e
+#pragma unroll
+    for (int c = 0; c < 4; ++c) {
+        float4 *dst = reinterpret_cast<float4 *>(red + warp * kGsSegCols + (lane + 32 * c) * 8);
+        dst[0] = make_float4(acc[c][0], acc[c][1], acc[c][2], acc[c][3]);
+        dst[1] = make_float4(acc[c][4], acc[c][5], acc[c][6], acc[c][7]);
+    }
+    __syncthreads();
+    const int cl = threadIdx.x * 2;                     // this thread's two columns of the segment
+    const bool mine = col0 + cl < ldy;
+    if (mine) {
+        float sx = 0.f, sy = 0.f;
+#pragma unroll
+        for (int w = 0; w < kGsWarps; ++w) {
+            const float2 v = *reinterpret_cast<const float2 *>(red + w * kGsSegCols + cl);
+            sx += v.x;
+            sy += v.y;
+        }
+        *reinterpret_cast<float2 *>(partial + (int64_t)blockIdx.y * ldp + col0 + cl) = make_float2(sx, sy);
+    }
+    __threadfence();
+    __syncthreads();
+    if (threadIdx.x == 0) s_last = (atomicAdd(&counters[blockIdx.x], 1u) == gridDim.y - 1);
+    __syncthreads();
+    if (!s_last) return;
+    __threadfence();
+    float *x = ind ? ind->x : x_direct;
+    if (mine) {
+        float gx = 0.f, gy = 0.f;
+#pragma unroll 8
+        for (unsigned q = 0; q < gridDim.y; ++q) {
+            const float2 v = __ldcg(reinterpret_cast<const float2 *>(partial + (int64_t)q * ldp + col0 + cl));
+            gx += v.x;
+            gy += v.y;
+        }
+        const int col = col0 + cl;
+        if (col < n) {
+            const float xn = fmaf(-alpha, gx, x[col]);
+            x[col] = xn;
+            xbf[col] = f32_to_bf16_bits_rn(xn);
+        }
+        if (col + 1 < n) {
+            const float xn = fmaf(-alpha, gy, x[col + 1]);
+            x[col + 1] = xn;
+            xbf[col + 1] = f32_to_bf16_bits_rn(xn);
+        }
+    }
+    if (threadIdx.x == 0) counters[blockIdx.x] = 0u;
+}
+
+static int launch_gradient_stream(cudaStream_t st, const uint16_t *Y, int32_t ldy, int32_t n, int32_t sb, const float *u,
+                                  float alpha, float *x, const StepParams *ind, uint16_t *xbf, const GradWorkspace &ws)
+{
+    static bool attr_set = false;
+    if (!attr_set) {
+        cudaFuncSetAttribute(gradient_stream_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kGsSmem);
+        attr_set = true;
+    }
+    const int col_segs = (ldy + kGsSegCols - 1) / kGsSegCols;
+    // rows per warp: at least 8 (fixed costs), at most 32 (one u per lane); about one CTA per SM for large steps
+    const int slabs_target = std::max(1, kNumSMsB200 / col_segs);
+    int rpw = (sb + kGsWarps * slabs_target - 1) / (kGsWarps * slabs_target);
+    rpw = std::min(32, std::max(8, rpw));
+    const int slabs = (sb + kGsWarps * rpw - 1) / (kGsWarps * rpw);
+    if (slabs > ws.max_splits) return 0;
+    launch_pdl(gradient_stream_kernel, dim3(col_segs, slabs), dim3(32 * kGsWarps), kGsSmem, st, 1, Y, ldy, n, sb, rpw, u, alpha, x,
+               ind, xbf, ws.partial, ws.ldp, ws.counters);
+    return 1;
+}
+
 static inline int next_pow2(int v) { int p = 1; while (p < v) p <<= 1; return p; }
 
 template <typename T, bool GATHER, bool SHADOW>
@@ -137,6 +282,7 @@ static int launch_gradient_any(cudaStream_t st, const T *base, int64_t ld, const
 int launch_gradient_bf16(cudaStream_t st, const uint16_t *Y, int32_t ldy, int32_t n, int32_t sb, const float *u,
                          float alpha, float *x, const StepParams *ind, uint16_t *xbf, const GradWorkspace &ws)
 {
+    if (ldy * 2 >= 512 && launch_gradient_stream(st, Y, ldy, n, sb, u, alpha, x, ind, xbf, ws)) return 1;
     return launch_gradient_any<uint16_t, false, true>(st, Y, ldy, nullptr, 0, n, sb, u, alpha, x, ind, xbf, ws);
 }
 
@@ -145,8 +291,8 @@ int launch_gradient_bf16(cudaStream_t st, const uint16_t *Y, int32_t ldy, int32_
 // z_i = a32_{I_i}^T x ; u_i = l'(z_i, y_{I_i}); one warp per row, everything FP32.
 __global__ void __launch_bounds__(256)
 sgd32_margin_kernel(const float *__restrict__ A32, int64_t lda32, const float *__restrict__ y, int64_t m, int32_t n,
-                    const int32_t *__restrict__ idx, int32_t b, int loss, const float *__restrict__ x, float *__restrict__ z,
-                    float *__restrict__ u, int *__restrict__ err_flag)
+                    const int32_t *idx, int32_t b, int loss, const float *x, float *z,
+                    float *u, int *err_flag)
 {
     pdl_trigger();
     pdl_wait();

@@ -24,8 +24,8 @@ namespace casgd {
 
 template <int LOSS>
 __global__ void __launch_bounds__(1024)
-recurrence_cta_kernel(const float *__restrict__ G, int32_t ldg, const float *__restrict__ r, const float *__restrict__ yI,
-                      int32_t s, int32_t b, float alpha, float *__restrict__ z, float *__restrict__ u)
+recurrence_cta_kernel(const float *G, int32_t ldg, const float *r, const float *yI,
+                      int32_t s, int32_t b, float alpha, float *z, float *u)
 {
     extern __shared__ float u_s[];                    // [s*b]
     pdl_trigger();
@@ -92,10 +92,10 @@ __device__ __forceinline__ void ld_tagged_x1(const unsigned long long *p, uint32
 // (b) the producer writes `nrep` replicas 128 KB apart and CTA i polls replica i mod nrep.
 template <int LOSS, int MAXR, bool VEC>
 __global__ void __launch_bounds__(kRecThreads, 1)
-recurrence_grid_kernel(const float *__restrict__ G, int32_t ldg, const float *__restrict__ r,
-                       const float *__restrict__ yI, int32_t s, int32_t b, float alpha, float *__restrict__ z,
-                       float *__restrict__ u, unsigned long long *__restrict__ utag, int32_t nrep,
-                       unsigned *__restrict__ epoch, unsigned *__restrict__ done)
+recurrence_grid_kernel(const float *G, int32_t ldg, const float *r,
+                       const float *yI, int32_t s, int32_t b, float alpha, float *z,
+                       float *u, unsigned long long *utag, int32_t nrep,
+                       unsigned *epoch, unsigned *done)
 {
     extern __shared__ __align__(16) float u_s[];        // [s*b]: u as it arrives
     __shared__ int s_last;
@@ -114,8 +114,8 @@ recurrence_grid_kernel(const float *__restrict__ G, int32_t ldg, const float *__
         acc[t] = 0.f;
         const int row = gw + t * W;
         const bool own = t < R;
-        rv[t] = own ? __ldg(r + row) : 0.f;
-        yv[t] = own ? __ldg(yI + row) : 0.f;
+        rv[t] = own ? ld_dep(r + row) : 0.f;
+        yv[t] = own ? ld_dep(yI + row) : 0.f;
         blk[t] = own ? row / b : -1;
     }
     int last_blk = -1;
@@ -285,9 +285,9 @@ __device__ __forceinline__ void chain_bar_wait(uint32_t bar)
 
 template <int LOSS>
 __global__ void __launch_bounds__(kChainThreads, 1)
-recurrence_cluster_kernel(const float *__restrict__ G, int32_t ldg, const float *__restrict__ r,
-                          const float *__restrict__ yI, int32_t s, int32_t b, float alpha, float *__restrict__ z,
-                          float *__restrict__ u)
+recurrence_cluster_kernel(const float *G, int32_t ldg, const float *r,
+                          const float *yI, int32_t s, int32_t b, float alpha, float *z,
+                          float *u)
 {
     extern __shared__ __align__(16) unsigned char chain_smem[];    // u_s[s*b] floats, then bars[s]
     __shared__ volatile float part[2][kChainWarps];
@@ -373,7 +373,7 @@ recurrence_cluster_kernel(const float *__restrict__ G, int32_t ldg, const float 
         for (int j = group; j < s; j += kChainGroups) {
             for (int rho = wg; rho < nr; rho += kGroupWarps) {
                 const int row = j * b + crank + rho * C;
-                const float rr = __ldg(r + row), yy = __ldg(yI + row);
+                const float rr = ld_dep(r + row), yy = ld_dep(yI + row);
                 const float acc = dot_chunks(row, j * b, 0, 1);
                 publish(j, row, warp_sum(acc), rr, yy);
             }
@@ -387,7 +387,7 @@ recurrence_cluster_kernel(const float *__restrict__ G, int32_t ldg, const float 
             for (int j = group, it = 0; j < s; j += kChainGroups, ++it) {
                 const int row = j * b + crank + rho * C;
                 if (h == 0) {
-                    const float rr = __ldg(r + row), yy = __ldg(yI + row);
+                    const float rr = ld_dep(r + row), yy = ld_dep(yI + row);
                     float acc = dot_chunks(row, j * b, 0, wpr);
                     if (lane >= 1 && lane < wpr) {                          // lane hh collects helper hh's partial
                         while (pflag[it & 1][warp + lane] != j) { }

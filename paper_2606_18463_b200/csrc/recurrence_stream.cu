@@ -174,9 +174,9 @@ __device__ __forceinline__ float quad_reduce(const float (&a)[kQuad], int lane)
 
 template <int LOSS>
 __global__ void __launch_bounds__(kThreads, 1)
-recurrence_stream_kernel(const float *__restrict__ G, int32_t ldg, const float *__restrict__ r,
-                         const float *__restrict__ yI, int32_t s, int32_t b, float alpha, float *__restrict__ z,
-                         float *__restrict__ u)
+recurrence_stream_kernel(const float *G, int32_t ldg, const float *r,
+                         const float *yI, int32_t s, int32_t b, float alpha, float *z,
+                         float *u)
 {
     extern __shared__ __align__(128) unsigned char rs_smem[];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
@@ -246,7 +246,7 @@ recurrence_stream_kernel(const float *__restrict__ G, int32_t ldg, const float *
 #pragma unroll 1
         for (int i = 0; i < kCritDepth - 1; ++i) prefetch_step();
         float rr = 0.f, yy = 0.f;
-        if (e < s) { rr = __ldg(r + e * b + q0 + li); yy = __ldg(yI + e * b + q0 + li); }
+        if (e < s) { rr = ld_dep(r + e * b + q0 + li); yy = ld_dep(yI + e * b + q0 + li); }
 
         __syncthreads();
         cluster_sync_all();                             // nobody signals a barrier that is not initialised yet
@@ -258,8 +258,8 @@ recurrence_stream_kernel(const float *__restrict__ G, int32_t ldg, const float *
             const int row = j * b + q0;
             float rr_next = 0.f, yy_next = 0.f;
             if (j + kCritPer < s) {
-                rr_next = __ldg(r + row + kCritPer * b + li);
-                yy_next = __ldg(yI + row + kCritPer * b + li);
+                rr_next = ld_dep(r + row + kCritPer * b + li);
+                yy_next = ld_dep(yI + row + kCritPer * b + li);
             }
             float acc[kQuad] = {0.f, 0.f, 0.f, 0.f};
             if (j > 0) {

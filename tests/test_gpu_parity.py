@@ -196,6 +196,37 @@ def test_out_of_range_index_is_reported_not_read(binding):
         cg.sync()                                        # the flag is cleared by the failing sync
 
 
+@pytest.mark.parametrize("n,stride", [(1024, 1024), (2040, 2048), (4096, 4096), (520, 520)])
+def test_wide_row_gather_is_bit_exact(binding, n, stride):
+    """Wide rows go through the copy-engine gather (cp.async.bulk global -> shared -> global): duplicates within and
+    across a warp's batches of 32 rows, out-of-range indices (zero rows + CASGD_EINDEX), a row stride larger
+    than n (used in place), row lengths that are not a multiple of the 4 KB slot."""
+    m, sb, b = 3000, 1408, 64
+    rng = np.random.default_rng(n)
+    bits = rng.integers(0, 1 << 16, size=(m, stride), dtype=np.uint16)
+    bits[(bits & 0x7f80) == 0x7f80] = 0x3f80                         # no NaN / Inf patterns: the step also runs the math
+    X_full = torch.from_numpy(bits.view(np.int16)).cuda().view(torch.bfloat16)
+    X_d = X_full[:, :n]
+    y_d = torch.from_numpy(rng.standard_normal(m).astype(np.float32)).cuda()
+    idx = rng.integers(0, m, size=sb).astype(np.int32)
+    idx[100:140] = idx[7]                                             # duplicates
+    bad = [3, 64, 65, 700, sb - 1]
+    idx[bad] = [m, -1, m + 5, -7, 2 ** 31 - 1]
+    x = torch.zeros(n, device="cuda")
+    with binding.Casgd(X_d, y_d, synth.LINEAR) as cg:
+        cg.outer_step(torch.from_numpy(idx).cuda(), x, sb // b, b, 0.0)
+        with pytest.raises(binding.CasgdError) as e:
+            cg.sync()
+        assert e.value.status == binding.EINDEX
+        Y = cg.debug(binding.DBG_Y)
+        ylab = cg.debug(binding.DBG_YLAB)
+        good = np.ones(sb, bool)
+        good[bad] = False
+        assert np.array_equal(Y[good], bits[idx[good], :n])
+        assert not Y[~good].any()
+        assert np.array_equal(ylab[good], y_d.cpu().numpy()[idx[good]]) and not ylab[~good].any()
+
+
 def test_bad_arguments_are_rejected_before_any_launch(binding):
     cfg = synth.config(0, m=256, n=64)
     X_d, y_d, _, _ = device_dataset(cfg)
