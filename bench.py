@@ -92,6 +92,20 @@ def stage_work(n, s, b, pk):
     return w
 
 
+def ncu_traffic(workload, s, stage):
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch of a stage's kernel, from the committed ncu
+    --set full summaries (profiles/r1_traffic.csv: workload,s,stage,kernel,dram_read_bytes,dram_write_bytes,report)."""
+    path = os.path.join(ROOT, "profiles", "r1_traffic.csv")
+    if not os.path.exists(path):
+        return None
+    import csv
+    with open(path) as f:
+        for row in csv.DictReader(f):
+            if row["workload"] == workload and int(row["s"]) == s and row["stage"] == stage:
+                return int(float(row["dram_read_bytes"]) + float(row["dram_write_bytes"]))
+    return None
+
+
 def roofline_of(stage, work, ms, pk, traffic=None):
     if ms <= 0:
         return None
@@ -348,7 +362,7 @@ def main_ours(args, cfg, s):
     for name, wk in work.items():
         tot_ms, cnt = st[name]
         per_step = tot_ms / Kp
-        rl = roofline_of(name, wk, per_step, pk) if cnt else None
+        rl = roofline_of(name, wk, per_step, pk, ncu_traffic(cfg.name, s, name)) if cnt else None
         stages[name] = dict(ms_per_step=round(per_step, 6), launches_per_step=cnt / Kp, roofline=rl,
                             alg_bytes=wk["bytes"], alg_flops=wk["flops"])
     dominant = max(stages, key=lambda k: stages[k]["ms_per_step"])
@@ -366,7 +380,7 @@ def main_ours(args, cfg, s):
     loss_bytes = 2 * cfg.m * cfg.n + 4 * cfg.m
     gemv = dict(kernel="casgd_loss", bound="hbm", achieved=round(loss_bytes / loss_ms / 1e6, 2), peak=pk["hbm"],
                 unit="GB/s", frac=round(loss_bytes / loss_ms / 1e6 / pk["hbm"], 4), avg_call_ms=round(loss_ms, 5),
-                peak_source=pk["source"])
+                traffic=ncu_traffic(cfg.name, 0, "loss"), peak_source=pk["source"])
 
     # ---- in-library FP32 s = 1 SGD baseline (Recipe A) and the s sweep, same index stream
     sweep = {}

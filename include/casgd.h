@@ -149,11 +149,14 @@ int casgd_debug_export(casgd_ctx *c, int what, void *dst_host, int64_t dst_bytes
  *                              memory, G by plain loads; needs b % 4 == 0, else falls through to 2), 4 = the
  *                              streaming cluster kernel (same cluster, G through a cp.async.bulk shared-memory
  *                              ring; needs b % 4 == 0 and b <= 128, else falls through to 3).
+ *   CASGD_OPT_NO_FUSED_UPDATE  1 = the outer update always runs as its own kernel. Default 0: for small steps
+ *                              (Y of at most 256 KB and 512 columns) the streaming recurrence kernel's cluster does
+ *                              g = Y^T u, the update of x and the shadow itself, right after the chain.
  *   CASGD_OPT_LOSS_IMPL        0 = casgd_loss streams A through per-warp cp.async.bulk shared-memory rings
  *                              (default; n <= 8192), 1 = the plain 16-byte-load kernel. */
 typedef enum {
     CASGD_OPT_GRAM_IMPL = 0, CASGD_OPT_GRAM_FULL_LOWER = 1, CASGD_OPT_PROFILE = 2, CASGD_OPT_NO_GRAPH = 3,
-    CASGD_OPT_GRAM_KSPLIT = 4, CASGD_OPT_RECURRENCE_IMPL = 5, CASGD_OPT_LOSS_IMPL = 6
+    CASGD_OPT_GRAM_KSPLIT = 4, CASGD_OPT_RECURRENCE_IMPL = 5, CASGD_OPT_LOSS_IMPL = 6, CASGD_OPT_NO_FUSED_UPDATE = 7
 } casgd_option;
 int casgd_set_option(casgd_ctx *c, int option, int64_t value);
 

@@ -78,7 +78,7 @@ struct casgd_ctx {
     // last step, for debug export
     int32_t last_s = 0, last_b = 0;
     // options
-    int64_t opt_gram_impl = 0, opt_full_lower = 0, opt_profile = 0, opt_no_graph = 0, opt_ksplit = 0, opt_rec_impl = 0, opt_loss_impl = 0;
+    int64_t opt_gram_impl = 0, opt_full_lower = 0, opt_profile = 0, opt_no_graph = 0, opt_ksplit = 0, opt_rec_impl = 0, opt_loss_impl = 0, opt_no_fuse = 0;
     GramTcPlan *tc_plan = nullptr;
     GramPairPlan *pair_plan = nullptr;
     int num_sms = 0;
@@ -218,14 +218,16 @@ int enqueue_step(casgd_ctx *c, cudaStream_t st, const int32_t *idx, const StepPa
         }
         t.done(k); *kernels += k;
     }
+    const bool fused = !c->opt_no_fuse && recurrence_fuses_update(s, b, c->ldg, c->ldy, c->rws, (int)c->opt_rec_impl);
     {
         StageTimer t(c, CASGD_STAGE_RECURRENCE);
+        const FusedUpdate fu{c->Y, c->ldy, c->n, x, ind, c->xbf};
         k = launch_recurrence(st, c->G, c->ldg, c->r, c->yI, s, b, alpha, c->loss, c->z, c->u, c->rws,
-                              (int)c->opt_rec_impl);
+                              (int)c->opt_rec_impl, fused ? &fu : nullptr);
         if (k < 0) return fail(c, CASGD_ECUDA, "recurrence launch: %s", cudaGetErrorString(cudaGetLastError()));
         t.done(k); *kernels += k;
     }
-    {
+    if (!fused) {
         StageTimer t(c, CASGD_STAGE_GRADIENT);
         k = launch_gradient_bf16(st, c->Y, c->ldy, c->n, sb, c->u, alpha, x, ind, c->xbf, c->gws);
         t.done(k); *kernels += k;
@@ -592,6 +594,7 @@ int casgd_set_option(casgd_ctx *c, int option, int64_t value)
     case CASGD_OPT_RECURRENCE_IMPL:
         if (value < 0 || value > 4) return fail(c, CASGD_EINVAL, "CASGD_OPT_RECURRENCE_IMPL must be in [0, 4]");
         c->opt_rec_impl = value; break;
+    case CASGD_OPT_NO_FUSED_UPDATE: c->opt_no_fuse = value != 0; break;
     case CASGD_OPT_LOSS_IMPL:
         if (value != 0 && value != 1) return fail(c, CASGD_EINVAL, "CASGD_OPT_LOSS_IMPL must be 0 or 1");
         c->opt_loss_impl = value; break;

@@ -174,13 +174,26 @@ int recurrence_cluster_size();
 int recurrence_max_coresident_ctas(int num_sms);
 // impl: 0 = choose by size, 1 = one CTA, 2 = all SMs through L2, 3 = one cluster, G from L2 by plain loads,
 // 4 = one cluster, G through a cp.async.bulk ring (recurrence_stream.cu). Returns kernels launched, or -1 on a launch error.
+// `fu` (optional): the outer update of the same step (Alg. 1 lines 16-17), which the streaming cluster kernel can do
+// itself when Y is small; recurrence_fuses_update() tells whether launch_recurrence will honour it for this shape
+// (the caller then skips the gradient kernel).
+struct FusedUpdate {
+    const uint16_t *Y;
+    int32_t ldy, n;
+    float *x;
+    const StepParams *ind;
+    uint16_t *xbf;
+};
+bool recurrence_fuses_update(int32_t s, int32_t b, int32_t ldg, int32_t ldy, const RecWorkspace &ws, int impl);
 int launch_recurrence(cudaStream_t st, const float *G, int32_t ldg, const float *r, const float *yI, int32_t s,
-                      int32_t b, float alpha, int loss, float *z, float *u, const RecWorkspace &ws, int impl);
+                      int32_t b, float alpha, int loss, float *z, float *u, const RecWorkspace &ws, int impl,
+                      const FusedUpdate *fu);
 
 // recurrence_stream.cu: one cluster, G streamed through a shared-memory ring, u through distributed shared memory.
 bool recurrence_stream_ok(int32_t s, int32_t b, int32_t ldg, int cluster);
+bool recurrence_stream_fuses_update(int32_t s, int32_t b, int32_t ldy);
 int launch_recurrence_stream(cudaStream_t st, const float *G, int32_t ldg, const float *r, const float *yI, int32_t s,
-                             int32_t b, float alpha, int loss, float *z, float *u, int cluster);
+                             int32_t b, float alpha, int loss, float *z, float *u, int cluster, const FusedUpdate *fu);
 
 struct GradWorkspace {
     float *partial;        // [row_splits x ldp] partial column sums

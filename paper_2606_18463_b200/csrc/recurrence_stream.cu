@@ -107,6 +107,19 @@ __device__ __forceinline__ float4 lds_f4(uint32_t saddr)
     return v;
 }
 
+// Fused outer update for small steps (Alg. 1 lines 16-17): when Y is small, g = Y^T u, x <- x - alpha g and the
+// BF16 shadow are done by this kernel's cluster right after the chain -- every CTA already holds all of u in shared
+// memory -- instead of by a fourth kernel: each CTA sums its slice of the rows, the per-CTA column sums meet in
+// CTA 0's shared memory (distributed shared memory stores), and CTA 0 adds them in a fixed order and updates x.
+struct FusedGrad {
+    const uint16_t *Y;          // [sb x ldy] staged rows (null: no fusion)
+    int32_t ldy, n;
+    float *x_direct;
+    const StepParams *ind;
+    uint16_t *xbf;
+};
+constexpr int kFgMaxLdy = 512;                          // columns (padded) the fused update handles
+
 struct StreamLayout {                   // byte offsets into dynamic shared memory (base 128-byte aligned)
     uint32_t u, ubar, pbar, part, cring, bring, total;
 };
@@ -176,7 +189,7 @@ template <int LOSS>
 __global__ void __launch_bounds__(kThreads, 1)
 recurrence_stream_kernel(const float *G, int32_t ldg, const float *r,
                          const float *yI, int32_t s, int32_t b, float alpha, float *z,
-                         float *u)
+                         float *u, const FusedGrad fg)
 {
     extern __shared__ __align__(128) unsigned char rs_smem[];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
@@ -323,7 +336,7 @@ recurrence_stream_kernel(const float *G, int32_t ldg, const float *r,
             const float tot = (j > 0) ? quad_reduce(acc, lane) : 0.f;       // lane l: row l >> 3
             const float zz = fmaf(-alpha, tot, rr);
             const float uu = lprime_chain<LOSS>(zz, yy);
-            if (j + 1 < s) {
+            if (j + 1 < s || fg.Y) {                     // (the fused update needs the last block everywhere too)
                 const float u0 = __shfl_sync(0xffffffffu, uu, 0), u1 = __shfl_sync(0xffffffffu, uu, 8);
                 const float u2 = __shfl_sync(0xffffffffu, uu, 16), u3 = __shfl_sync(0xffffffffu, uu, 24);
                 if (lane < ndst) st_async_v4(rem_us + 4u * (uint32_t)row, u0, u1, u2, u3, rem_ubar + 8u * (uint32_t)j);
@@ -416,6 +429,63 @@ recurrence_stream_kernel(const float *G, int32_t ldg, const float *r,
     }
     cp_async_wait<0>();
     REC_TRACE(2);
+    if (fg.Y) {
+        // ===== fused g = Y^T u, x <- x - alpha g, shadow =====
+        // all of u is in this CTA's shared memory once every block's barrier has completed
+        for (int k = threadIdx.x; k < s; k += kThreads) mbar_wait(ubar + 8u * k, 0u);
+        __syncthreads();                                // ... and the rings are free: they become reduction buffers
+        const int sb = s * b, ldy = fg.ldy;
+        const int nvec = ldy >> 3;                      // 16-byte vectors per row (pad columns of Y are zero)
+        int CV = 1;
+        while (CV < nvec && CV < 64) CV <<= 1;          // threads side by side on a row
+        const int RL = kThreads / CV;                   // rows in flight
+        const int cvl = threadIdx.x % CV, rl = threadIdx.x / CV;
+        const int rows_per_cta = (sb + C - 1) / C;
+        const int r0 = crank * rows_per_cta, r1 = min(sb, r0 + rows_per_cta);
+        float *red = reinterpret_cast<float *>(rs_smem + L.cring);                     // [RL][CV * 8]
+        float *gbuf = reinterpret_cast<float *>(rs_smem + L.cring + kThreads * 8 * 4);   // CTA 0: [C][ldy]
+        const float *u_loc = reinterpret_cast<const float *>(rs_smem + L.u);
+        for (int cv0 = 0; cv0 < nvec; cv0 += CV) {      // (one pass unless ldy > 512)
+            const int cv = cv0 + cvl;
+            float acc[8] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
+            if (cv < nvec) {
+                for (int row = r0 + rl; row < r1; row += RL) {
+                    const uint4 v = ldg_nc_v4(fg.Y + (int64_t)row * ldy + cv * 8);
+                    const float uu = u_loc[row];
+                    acc[0] = fmaf(bf16lo(v.x), uu, acc[0]); acc[1] = fmaf(bf16hi(v.x), uu, acc[1]);
+                    acc[2] = fmaf(bf16lo(v.y), uu, acc[2]); acc[3] = fmaf(bf16hi(v.y), uu, acc[3]);
+                    acc[4] = fmaf(bf16lo(v.z), uu, acc[4]); acc[5] = fmaf(bf16hi(v.z), uu, acc[5]);
+                    acc[6] = fmaf(bf16lo(v.w), uu, acc[6]); acc[7] = fmaf(bf16hi(v.w), uu, acc[7]);
+                }
+            }
+#pragma unroll
+            for (int e = 0; e < 8; ++e) red[rl * (CV * 8) + cvl * 8 + e] = acc[e];
+            __syncthreads();
+            // column sums of this CTA, in a fixed order, straight into CTA 0's gbuf[crank][col]
+            const uint32_t gbuf0 = mapa_u32((uint32_t)__cvta_generic_to_shared(gbuf), 0u);
+            for (int t = threadIdx.x; t < CV * 8; t += kThreads) {
+                float sum = 0.f;
+                for (int q = 0; q < RL; ++q) sum += red[q * (CV * 8) + t];
+                const int col = cv0 * 8 + t;
+                if (col < ldy)
+                    asm volatile("st.shared::cluster.f32 [%0], %1;" ::"r"(gbuf0 + 4u * (uint32_t)(crank * ldy + col)), "f"(sum) : "memory");
+            }
+            __syncthreads();
+        }
+        cluster_sync_all();                             // every CTA's sums are in CTA 0; nobody stores into a CTA any more
+        if (crank == 0) {
+            float *x = fg.ind ? fg.ind->x : fg.x_direct;
+            for (int col = threadIdx.x; col < fg.n; col += kThreads) {
+                float g = 0.f;
+                for (int q = 0; q < C; ++q) g += gbuf[q * ldy + col];
+                const float xn = fmaf(-alpha, g, x[col]);
+                x[col] = xn;
+                fg.xbf[col] = f32_to_bf16_bits_rn(xn);
+            }
+        }
+        REC_TRACE(3);
+        return;
+    }
     __syncthreads();
     cluster_sync_all();                                 // no CTA leaves while others may still store into it
     REC_TRACE(3);
@@ -444,7 +514,7 @@ int stream_cluster_for(int b, int cluster_max)
 
 template <int LOSS>
 cudaError_t launch_stream(cudaStream_t st, const float *G, int32_t ldg, const float *r, const float *yI, int32_t s,
-                          int32_t b, float alpha, float *z, float *u, int cluster_max)
+                          int32_t b, float alpha, float *z, float *u, int cluster_max, const FusedGrad &fg)
 {
     static bool attr_set = false;
     const int smem = stream_smem_bytes(s, b);
@@ -461,7 +531,7 @@ cudaError_t launch_stream(cudaStream_t st, const float *G, int32_t ldg, const fl
         attr_set = true;
     }
     const int cluster = stream_cluster_for(b, cluster_max);
-    return launch_pdl(kern, dim3(cluster), dim3(kThreads), (size_t)smem, st, cluster, G, ldg, r, yI, s, b, alpha, z, u);
+    return launch_pdl(kern, dim3(cluster), dim3(kThreads), (size_t)smem, st, cluster, G, ldg, r, yI, s, b, alpha, z, u, fg);
 }
 
 }  // namespace
@@ -475,12 +545,20 @@ bool recurrence_stream_ok(int32_t s, int32_t b, int32_t ldg, int cluster)
     return stream_smem_bytes(s, b) > 0;
 }
 
-int launch_recurrence_stream(cudaStream_t st, const float *G, int32_t ldg, const float *r, const float *yI, int32_t s,
-                             int32_t b, float alpha, int loss, float *z, float *u, int cluster)
+// Can the streaming kernel also do the outer update of this step (small Y)?
+bool recurrence_stream_fuses_update(int32_t s, int32_t b, int32_t ldy)
 {
-    cudaError_t e = loss == CASGD_LOGISTIC ? launch_stream<CASGD_LOGISTIC>(st, G, ldg, r, yI, s, b, alpha, z, u, cluster)
-                  : loss == CASGD_LINEAR  ? launch_stream<CASGD_LINEAR>(st, G, ldg, r, yI, s, b, alpha, z, u, cluster)
-                                          : launch_stream<CASGD_POISSON>(st, G, ldg, r, yI, s, b, alpha, z, u, cluster);
+    return ldy <= kFgMaxLdy && (int64_t)s * b * ldy * 2 <= 256 * 1024;
+}
+
+int launch_recurrence_stream(cudaStream_t st, const float *G, int32_t ldg, const float *r, const float *yI, int32_t s,
+                             int32_t b, float alpha, int loss, float *z, float *u, int cluster, const FusedUpdate *fu)
+{
+    FusedGrad fg{};
+    if (fu) fg = FusedGrad{fu->Y, fu->ldy, fu->n, fu->x, fu->ind, fu->xbf};
+    cudaError_t e = loss == CASGD_LOGISTIC ? launch_stream<CASGD_LOGISTIC>(st, G, ldg, r, yI, s, b, alpha, z, u, cluster, fg)
+                  : loss == CASGD_LINEAR  ? launch_stream<CASGD_LINEAR>(st, G, ldg, r, yI, s, b, alpha, z, u, cluster, fg)
+                                          : launch_stream<CASGD_POISSON>(st, G, ldg, r, yI, s, b, alpha, z, u, cluster, fg);
     return e == cudaSuccess ? 1 : -1;
 }
 
