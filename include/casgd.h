@@ -135,7 +135,9 @@ int casgd_debug_export(casgd_ctx *c, int what, void *dst_host, int64_t dst_bytes
  *   CASGD_OPT_GRAM_IMPL        0 = choose by a cost model (default), 1 = plain FP32-FMA CUDA-core kernel (bring-up
  *                              reference, same BF16 inputs and FP32 accumulation), 2 = tcgen05 kernel with 128 x 128
  *                              tiles, one CTA each, 3 / 4 = tcgen05 kernel on CTA pairs (cta_group::2) with
- *                              256 x 256 / 256 x 512 tiles (large shapes: fewer operand bytes per flop).
+ *                              256 x 256 / 256 x 512 tiles (large shapes: fewer operand bytes per flop), 5 = gather and
+ *                              Gram in ONE kernel, one CTA per 128 x 128 tile, rows pulled straight from A into the
+ *                              swizzled operand layout (n <= 64 only; what 0 picks there).
  *   CASGD_OPT_GRAM_FULL_LOWER  1 = also compute the tiles on the block diagonal, so that the whole lower
  *                              triangle of CASGD_DBG_G is valid (the recurrence never reads them).
  *   CASGD_OPT_PROFILE          1 = record CUDA events around each stage of casgd_outer_step(s) (disables

@@ -195,14 +195,18 @@ int enqueue_step(casgd_ctx *c, cudaStream_t st, const int32_t *idx, const StepPa
     const int32_t sb = s * b;
     const float alpha = eta / (float)b;
     int k;
-    {
+    if (c->cur_gram != 4) {
         StageTimer t(c, CASGD_STAGE_GATHER);
         k = launch_gather(st, c->A, c->lda, c->y, c->m, c->n, idx, ind, idx_off, sb, c->Y, c->ldy, c->yI, c->err_flag);
         t.done(k); *kernels += k;
     }
     {
         StageTimer t(c, CASGD_STAGE_GRAM);
-        if (c->cur_gram == 1) {
+        if (c->cur_gram == 4) {
+            k = launch_gram_narrow(st, c->A, c->lda, c->y, c->m, c->n, idx, ind, idx_off, sb, b, c->xbf, c->ldxb, c->Y, c->ldy,
+                                   c->yI, c->G, c->ldg, c->r, (int)c->opt_full_lower, c->err_flag);
+            if (k < 0) return fail(c, CASGD_ECUDA, "gram_narrow launch: %s", cudaGetErrorString(cudaGetLastError()));
+        } else if (c->cur_gram == 1) {
             k = launch_gram_simt(st, c->Y, c->ldy, c->n, sb, b, c->xbf, c->G, c->ldg, c->r, (int)c->opt_full_lower);
         } else if (c->cur_gram == 3) {
             k = launch_gram_pair(st, c->pair_plan, sb, b, c->G, c->ldg, c->r, (int)c->opt_full_lower, c->cur_bn,
@@ -244,6 +248,9 @@ int choose_gram(casgd_ctx *c, int32_t s, int32_t b)
     const int64_t opt = c->opt_gram_impl;
     c->cur_gram = opt == 1 ? 1 : 2;
     c->cur_bn = 0;
+    // gather + Gram in one kernel: wins while the tiles fit in about half a wave (measured: sb = 2048 is 4 us slower)
+    if ((opt == 5 || (opt == 0 && sb <= 1280)) && c->n <= 64) { c->cur_gram = 4; return CASGD_OK; }
+    if (opt == 5) return fail(c, CASGD_EINVAL, "the fused gather + Gram kernel needs n <= 64");
     if (opt == 1 || opt == 2 || c->num_sms < 2) return CASGD_OK;
     if (opt == 0 && (sb < 512 || c->n < 256)) return CASGD_OK;      // too little work for 256-row tiles
     if (!c->pair_plan) {
@@ -581,7 +588,7 @@ int casgd_set_option(casgd_ctx *c, int option, int64_t value)
     if (!c) return CASGD_EINVAL;
     switch (option) {
     case CASGD_OPT_GRAM_IMPL:
-        if (value < 0 || value > 4) return fail(c, CASGD_EINVAL, "CASGD_OPT_GRAM_IMPL must be in [0, 4]");
+        if (value < 0 || value > 5) return fail(c, CASGD_EINVAL, "CASGD_OPT_GRAM_IMPL must be in [0, 5]");
         c->opt_gram_impl = value; break;
     case CASGD_OPT_GRAM_FULL_LOWER: c->opt_full_lower = value != 0; break;
     case CASGD_OPT_PROFILE:

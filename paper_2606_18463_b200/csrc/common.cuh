@@ -227,6 +227,12 @@ void gram_tc_plan_destroy(GramTcPlan *p);
 int launch_gram_tc(cudaStream_t st, GramTcPlan *plan, int32_t sb, int32_t b, float *G, int32_t ldg, float *r,
                    int full_lower, int ksplit_opt, char *err, int errlen);
 
+// gather + Gram + margin in one kernel for narrow rows (n <= 64): gram_tc.cu
+int launch_gram_narrow(cudaStream_t st, const uint16_t *A, int64_t lda, const float *y, int64_t m, int32_t n,
+                       const int32_t *idx, const StepParams *ind, int64_t idx_off, int32_t sb, int32_t b,
+                       const uint16_t *xbf, int32_t ldxb, uint16_t *Y, int32_t ldy, float *yI, float *G, int32_t ldg,
+                       float *r, int full_lower, int *err_flag);
+
 // cta_group::2 Gram + margin for large shapes (gram_pair.cu): 256 x 256 / 256 x 512 tiles on CTA pairs, work lists
 // built on the host. gram_pair_prepare (outside stream capture) returns the estimated cycles, or -1.
 struct GramPairPlan;

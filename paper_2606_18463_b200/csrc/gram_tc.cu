@@ -326,6 +326,182 @@ gram_tc_kernel(const __grid_constant__ CUtensorMap tmY, const __grid_constant__ 
     }
 }
 
+// ------------------------------------------------------------------ narrow rows: gather + Gram in one kernel ---
+// For n <= 64 (configs[0], configs[1]) a Gram tile has ONE K block and the step is pure latency, so the gather
+// (Alg. 1 line 2) and the Gram + margin (lines 3-4) are one kernel with one CTA per 128x128 tile: its 128 threads
+// read the tile's row indices, pull the rows straight from A with 16-byte loads and write them into shared memory
+// in the 128-byte-swizzled K-major layout tcgen05 expects (chunk c of row r at r * 128 + ((c ^ (r & 7)) << 4)) --
+// no TMA descriptor, no Y round trip through L2 before the MMA. Diagonal tiles also write the Y stage and y_I
+// (the gradient's second pass and casgd_debug_export read them) and carry x_bf as 16 extra B rows for the margin.
+constexpr int kNwThreads = 128;
+constexpr uint32_t kNwOffT0 = 0, kNwOffX = kTileBytes, kNwOffT1 = kTileBytes + kXBytes;
+constexpr size_t kNwSmem = 1024 + 2 * kTileBytes + kXBytes + 64 + 4 * kEpiBufB;
+
+struct NarrowParams {
+    const uint16_t *A;
+    int64_t lda, m;
+    const float *y;
+    const int32_t *idx;
+    const StepParams *ind;
+    int64_t idx_off;
+    const uint16_t *xbf;
+    int32_t ldxb;
+    uint16_t *Y;
+    float *yI, *G, *r;
+    int *err_flag;
+    int32_t ldy, ldg, sb, b, n, T, full_lower;
+};
+
+__global__ void __launch_bounds__(kNwThreads)
+gram_narrow_kernel(const NarrowParams p)
+{
+    extern __shared__ uint8_t smem_raw[];
+    const uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;
+    const uint32_t bar = smem_base + 2 * kTileBytes + kXBytes, tmem_slot = bar + 8u;
+    const uint32_t ebuf0 = bar + 64u;
+    volatile uint32_t *tmem_slot_ptr = reinterpret_cast<volatile uint32_t *>(smem_raw + (tmem_slot - smem_u32(smem_raw)));
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    pdl_trigger();
+
+    // tile of this CTA: the T diagonal tiles first, then the strictly lower ones
+    int ti, tj;
+    if ((int)blockIdx.x < p.T) {
+        ti = tj = blockIdx.x;
+    } else {
+        const int q = (int)blockIdx.x - p.T;
+        ti = (int)((1.f + sqrtf(1.f + 8.f * (float)q)) * 0.5f);
+        while (ti * (ti - 1) / 2 > q) --ti;
+        while ((ti + 1) * ti / 2 <= q) ++ti;
+        tj = q - ti * (ti - 1) / 2;
+    }
+    const bool diag = ti == tj;
+    const int last_row = min(ti * BM + BM, p.sb) - 1;
+    const bool need_g = p.full_lower || (last_row / p.b) > ((tj * BN) / p.b);
+    if (!diag && !need_g) return;
+
+    if (threadIdx.x == 0) {
+        mbar_init(bar, 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    if (warp == 0) {
+        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(tmem_slot), "r"(256u) : "memory");
+        asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+    }
+    pdl_wait();                                     // x_bf and the Y stage belong to the previous step until now
+
+    // ---- gather: thread t owns row t of each operand tile
+    const int32_t *I = p.ind ? p.ind->idx + p.idx_off : p.idx;
+    const int ksteps = (p.n + 15) >> 4;             // K = 16 steps that hold data
+    const int nfill = 2 * ksteps;                   // 16-byte chunks of a tile row the MMAs read
+    for (int op = 0; op < (diag ? 1 : 2); ++op) {
+        const int trow = (op == 0 ? ti : tj) * BM + (int)threadIdx.x;
+        int64_t src = -1;
+        if (trow < p.sb) {
+            src = I[trow];
+            if (src < 0 || src >= p.m) { src = -1; if (diag) atomicOr(p.err_flag, 1); }
+        }
+        const uint32_t trow_s = smem_base + (op == 0 ? kNwOffT0 : kNwOffT1) + threadIdx.x * 128u;
+        uint4 v[8];
+#pragma unroll
+        for (int c = 0; c < 8; ++c) {
+            v[c] = make_uint4(0u, 0u, 0u, 0u);
+            if (c < nfill && src >= 0 && c * 8 < p.n) {
+                v[c] = ldg_nc_v4(p.A + src * p.lda + c * 8);
+                const int valid = p.n - c * 8;
+                if (valid < 8) {
+                    uint32_t w[4] = {v[c].x, v[c].y, v[c].z, v[c].w};
+#pragma unroll
+                    for (int q = 0; q < 4; ++q) {
+                        if (2 * q >= valid) w[q] = 0u;
+                        else if (2 * q + 1 >= valid) w[q] &= 0x0000ffffu;
+                    }
+                    v[c] = make_uint4(w[0], w[1], w[2], w[3]);
+                }
+            }
+        }
+#pragma unroll
+        for (int c = 0; c < 8; ++c)
+            if (c < nfill)
+                asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(trow_s + (uint32_t)((c ^ (threadIdx.x & 7)) << 4)),
+                             "r"(v[c].x), "r"(v[c].y), "r"(v[c].z), "r"(v[c].w) : "memory");
+        if (diag && trow < p.sb) {                  // the Y stage and the labels of these 128 rows
+#pragma unroll
+            for (int c = 0; c < 8; ++c)
+                if (c * 8 < p.ldy) *reinterpret_cast<uint4 *>(p.Y + (int64_t)trow * p.ldy + c * 8) = v[c];
+            p.yI[trow] = src >= 0 ? p.y[src] : 0.f;
+        }
+    }
+    if (diag) {                                     // x_bf: 16 rows x 64 columns right behind the B tile (rows 1..15 are zero)
+        const int xr = threadIdx.x >> 3, c = threadIdx.x & 7;
+        uint4 v = make_uint4(0u, 0u, 0u, 0u);
+        if (c * 8 < p.ldxb) v = *reinterpret_cast<const uint4 *>(p.xbf + (int64_t)xr * p.ldxb + c * 8);
+        asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(smem_base + kNwOffX + (uint32_t)xr * 128u + (uint32_t)((c ^ (xr & 7)) << 4)),
+                     "r"(v.x), "r"(v.y), "r"(v.z), "r"(v.w) : "memory");
+    }
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");   // generic-proxy writes -> visible to the tensor core
+    tc_fence_before();
+    __syncthreads();
+    tc_fence_after();
+    const uint32_t tmem_base = *tmem_slot_ptr;
+
+    // ---- MMA: one K block
+    if (warp == 0) {
+        const uint32_t ncols = diag ? (need_g ? (uint32_t)(BN + XR) : (uint32_t)XR) : (uint32_t)BN;
+        const uint32_t idesc = umma_idesc(ncols);
+        const uint64_t adesc = umma_desc_sw128(smem_base + kNwOffT0);
+        const uint64_t bdesc = umma_desc_sw128(smem_base + (diag ? (need_g ? kNwOffT0 : kNwOffX) : kNwOffT1));
+        if (elect_one()) {
+            for (int ks = 0; ks < ksteps; ++ks) tc_mma_bf16(tmem_base, adesc + 2u * ks, bdesc + 2u * ks, idesc, ks > 0 ? 1u : 0u);
+            tc_commit(bar);
+        }
+        __syncwarp();
+    }
+    mbar_wait(bar, 0u);
+    tc_fence_after();
+
+    // ---- epilogue: TMEM lane group = warp; transposed through shared memory, whole-line stores
+    const uint32_t t_row = tmem_base + ((uint32_t)(warp * 32) << 16);
+    const uint32_t ebuf = ebuf0 + (uint32_t)warp * kEpiBufB;
+    if (need_g) {
+#pragma unroll 1
+        for (int c = 0; c < BN / 32; ++c) {
+            if (tj * BN + c * 32 > last_row) break;   // columns beyond the tile's last row are above the diagonal
+            uint32_t v[32];
+            tc_ld32(t_row + c * 32, v);
+            tc_wait_ld();
+#pragma unroll
+            for (int e = 0; e < 32; e += 4)
+                asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(ebuf + (uint32_t)(lane * kEpiStride + e) * 4u),
+                             "r"(v[e]), "r"(v[e + 1]), "r"(v[e + 2]), "r"(v[e + 3]) : "memory");
+            __syncwarp();
+            const int c4 = (lane & 7) * 4;
+#pragma unroll
+            for (int i = 0; i < 8; ++i) {
+                const int rl = 4 * i + (lane >> 3);
+                uint32_t o0, o1, o2, o3;
+                asm volatile("ld.shared.v4.b32 {%0, %1, %2, %3}, [%4];" : "=r"(o0), "=r"(o1), "=r"(o2), "=r"(o3)
+                             : "r"(ebuf + (uint32_t)(rl * kEpiStride + c4) * 4u) : "memory");
+                const int orow = ti * BM + warp * 32 + rl;
+                if (orow < p.sb)
+                    *reinterpret_cast<uint4 *>(p.G + (int64_t)orow * p.ldg + tj * BN + c * 32 + c4) = make_uint4(o0, o1, o2, o3);
+            }
+            __syncwarp();
+        }
+    }
+    if (diag) {
+        const uint32_t rv = tc_ld1(t_row + (need_g ? BN : 0));
+        tc_wait_ld();
+        const int row = ti * BM + warp * 32 + lane;
+        if (row < p.sb) p.r[row] = __uint_as_float(rv);
+    }
+    tc_fence_before();
+    __syncthreads();
+    if (warp == 0) {
+        tc_fence_after();
+        asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "r"(256u) : "memory");
+    }
+}
+
 typedef CUresult (*EncodeTiledFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *,
                                   const cuuint64_t *, const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave,
                                   CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
@@ -420,6 +596,26 @@ int launch_gram_tc(cudaStream_t st, GramTcPlan *plan, int32_t sb, int32_t b, flo
     const int grid = std::min(p.ntiles * ksplit, kNumSMsB200);
     launch_pdl(gram_tc_kernel, dim3(grid), dim3(kThreads), kSmemBytes, st, 1, plan->tmY, plan->tmX, p);
     return launches;
+}
+
+// Gather + Gram + margin in one kernel for n <= 64 (replaces launch_gather + launch_gram_tc for the step).
+int launch_gram_narrow(cudaStream_t st, const uint16_t *A, int64_t lda, const float *y, int64_t m, int32_t n,
+                       const int32_t *idx, const StepParams *ind, int64_t idx_off, int32_t sb, int32_t b,
+                       const uint16_t *xbf, int32_t ldxb, uint16_t *Y, int32_t ldy, float *yI, float *G, int32_t ldg,
+                       float *r, int full_lower, int *err_flag)
+{
+    static bool attr_set = false;
+    if (!attr_set) {
+        if (cudaFuncSetAttribute(gram_narrow_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kNwSmem) != cudaSuccess) return -1;
+        attr_set = true;
+    }
+    NarrowParams p;
+    p.A = A; p.lda = lda; p.m = m; p.y = y; p.idx = idx; p.ind = ind; p.idx_off = idx_off; p.xbf = xbf; p.ldxb = ldxb;
+    p.Y = Y; p.yI = yI; p.G = G; p.r = r; p.err_flag = err_flag; p.ldy = ldy; p.ldg = ldg; p.sb = sb; p.b = b; p.n = n;
+    p.T = (sb + BM - 1) / BM;
+    p.full_lower = full_lower;
+    const int tiles = p.T * (p.T + 1) / 2;
+    return launch_pdl(gram_narrow_kernel, dim3(tiles), dim3(kNwThreads), kNwSmem, st, 1, p) == cudaSuccess ? 1 : -1;
 }
 
 }  // namespace casgd

@@ -40,7 +40,7 @@ SMALL = [
 ]
 
 
-GRAM_IMPLS = dict(argvalues=[0, 1, 2, 3, 4], ids=["auto", "simt", "tile128", "pair256", "pair512"])
+GRAM_IMPLS = dict(argvalues=[0, 1, 2, 3, 4, 5], ids=["auto", "simt", "tile128", "pair256", "pair512", "narrow"])
 
 
 @pytest.mark.parametrize("gram_impl", **GRAM_IMPLS)
@@ -48,6 +48,8 @@ GRAM_IMPLS = dict(argvalues=[0, 1, 2, 3, 4], ids=["auto", "simt", "tile128", "pa
 def test_one_outer_step_matches_the_oracle(binding, oracle_mod, ci, m, n, s, b, gram_impl):
     cfg = synth.config(ci, m=m, n=n)
     X_d, y_d, A_bits, y = device_dataset(cfg)
+    if gram_impl == 5 and n > 64:
+        gram_impl = 2                                   # the fused gather + Gram kernel takes n <= 64 only
     with binding.Casgd(X_d, y_d, cfg.loss) as cg:
         cg.set_option(binding.OPT_GRAM_IMPL, gram_impl)
         idx = np.random.default_rng(42).permutation(m)[: s * b].astype(np.int32)      # without replacement
@@ -92,6 +94,9 @@ def test_full_lower_triangle_and_duplicates(binding, oracle_mod, gram_impl):
     s, b = 6, 50
     idx = synth.iid_indices(cfg.m, s * b, 5)
     assert len(np.unique(idx)) < len(idx)
+    if gram_impl == 5:
+        cfg = synth.config(3, m=300, n=52)              # the fused gather + Gram kernel takes n <= 64 only
+        X_d, y_d, A_bits, y = device_dataset(cfg)
     with binding.Casgd(X_d, y_d, cfg.loss) as cg:
         cg.set_option(binding.OPT_GRAM_IMPL, gram_impl)
         cg.set_option(binding.OPT_GRAM_FULL_LOWER, 1)
