@@ -31,7 +31,7 @@ constexpr int kWarps = 16;
 constexpr int kThreads = 32 * kWarps;
 constexpr int kQuad = 4;                                // rows per row group: one 16-byte remote store carries their u
 constexpr int kMaxQuadsPerCta = 2;                      // row groups of one block owned by one CTA (b <= 8 * C)
-constexpr int kBulkWarps = 8;
+constexpr int kBulkWarps = 12;                          // bulk warps per CTA at most: every warp that is not critical (12 with one row group, 10 with two)
 constexpr int kChunk = 128;                             // columns per chunk
 constexpr uint32_t kUnitBytes = kQuad * kChunk * 4u;    // one unit: 4 rows x 128 columns of G = 2 KB
 constexpr int kWin = 2;                                 // chunks of a step the critical warps take: the newest 256 columns
@@ -207,20 +207,23 @@ recurrence_stream_kernel(const float *G, int32_t ldg, const float *r,
     const int bshift = (b & (b - 1)) == 0 ? __ffs(b) - 1 : -1;             // b a power of two: column -> block by shift
     auto block_of = [&](int col) { return bshift >= 0 ? (col >> bshift) : col / b; };
 
+    const int nbulk = qpc == 1 ? 12 : 10;               // 16 warps - 3 critical warps per owned row group, rounded to a multiple of qpc
     for (int k = threadIdx.x; k < s; k += kThreads) {
         mbar_init(ubar + 8u * k, 1);
         mbar_expect_tx(ubar + 8u * k, 4u * (uint32_t)b);
-        mbar_init(pbar + 8u * k, kBulkWarps);
+        mbar_init(pbar + 8u * k, (uint32_t)nbulk);
     }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     pdl_wait();                                         // G, r and y_I come from the Gram and gather kernels
 
-    // Warp w runs on scheduler w & 3. Critical warps: (group gamma, parity e) -> warp gamma + 4 e, so with up
-    // to two groups they have schedulers 0 and 1 to themselves and the eight bulk warps share 2 and 3: what the
-    // bulk warps issue when u lands (they wake on the same barrier) does not delay the chain.
+    // Warp w runs on scheduler w & 3. Critical warps: (group gamma, parity e) -> warp gamma + 4 e.
     const int wsched = warp & 3, wslot = warp >> 2;
     const bool is_critical = wslot < kCritPer && wsched < qpc;
-    const bool is_bulk = qpc > 0 && (qpc <= 2 ? wsched >= 2 : warp >= 8);
+    // bulk warps: the non-critical warps, on all four schedulers (the chain's instructions are few; what bounded the
+    // late steps was the bulk warps' own issue rate, 8 warps on 2 schedulers: ~33 B/cycle/SM out of L2)
+    const int ncrit_below = min(wslot, kCritPer) * qpc + (wslot < kCritPer ? min(wsched, qpc) : 0);
+    const int brank = warp - ncrit_below;               // rank among the non-critical warps
+    const bool is_bulk = qpc > 0 && !is_critical && brank < nbulk;
     const int li = lane >> 3;                           // the row of a group this lane finalises / reports
 
     if (is_critical) {
@@ -294,9 +297,12 @@ recurrence_stream_kernel(const float *G, int32_t ldg, const float *r,
                     // lane (li, gg): the partial sum of row li from bulk warp gg of this group
                     mbar_wait(pbar + 8u * j, 0u);
                     float p = 0.f;
-                    if ((lane & 7) < kBulkWarps / qpc)
-                        asm volatile("ld.shared.f32 %0, [%1];" : "=f"(p)
-                                 : "r"(part + 16u * (uint32_t)(((j % kPartDepth) * kMaxQuadsPerCta + gamma) * kBulkWarps + (lane & 7)) + 4u * (uint32_t)li));
+                    for (int gg = lane & 7; gg < nbulk / qpc; gg += 8) {    // at most two partials per lane
+                        float pv;
+                        asm volatile("ld.shared.f32 %0, [%1];" : "=f"(pv)
+                                     : "r"(part + 16u * (uint32_t)(((j % kPartDepth) * kMaxQuadsPerCta + gamma) * kBulkWarps + gg) + 4u * (uint32_t)li));
+                        p += pv;
+                    }
 #pragma unroll
                     for (int i = 0; i < kQuad; ++i) acc[i] = (i == li) ? p : 0.f;
                 }
@@ -356,8 +362,8 @@ recurrence_stream_kernel(const float *G, int32_t ldg, const float *r,
         // ===== bulk warp: group gamma, lane cidx of nw; chunks c = cidx, cidx + nw, ... < nch(j) - kWin of every step =====
         // These columns belong to blocks that landed (kWin - 1) * 128 / b hops ago, so the bulk warps run
         // several steps ahead of the chain and are bound only by the SM's L2 bandwidth.
-        const int g = qpc <= 2 ? wslot * 2 + (wsched - 2) : warp - 8;
-        const int nw = kBulkWarps / qpc;                // bulk warps per owned group
+        const int g = brank;
+        const int nw = nbulk / qpc;                     // bulk warps per owned group
         const int gamma = g / nw, cidx = g % nw;
         const uint32_t ring = base + L.bring + (uint32_t)(g * kDepth) * kUnitBytes + (uint32_t)lane * 16u;
         const float *gbase = G + (int64_t)(kQuad * (crank + gamma * C)) * ldg + lane * 4;   // + j b ldg + c * 128
