@@ -195,6 +195,9 @@ int enqueue_step(casgd_ctx *c, cudaStream_t st, const int32_t *idx, const StepPa
     const int32_t sb = s * b;
     const float alpha = eta / (float)b;
     int k;
+    // s = 1: no correction, u = l'(r, y_I): applied by the Gram kernel's margin epilogue (no recurrence kernel)
+    const bool s1 = s == 1 && !c->opt_no_fuse && (c->cur_gram == 4 || (c->cur_gram == 2 && c->n <= 1024 && c->opt_ksplit <= 1));
+    const S1Fuse s1f{c->loss, c->yI, c->z, c->u};
     if (c->cur_gram != 4) {
         StageTimer t(c, CASGD_STAGE_GATHER);
         k = launch_gather(st, c->A, c->lda, c->y, c->m, c->n, idx, ind, idx_off, sb, c->Y, c->ldy, c->yI, c->err_flag);
@@ -204,7 +207,7 @@ int enqueue_step(casgd_ctx *c, cudaStream_t st, const int32_t *idx, const StepPa
         StageTimer t(c, CASGD_STAGE_GRAM);
         if (c->cur_gram == 4) {
             k = launch_gram_narrow(st, c->A, c->lda, c->y, c->m, c->n, idx, ind, idx_off, sb, b, c->xbf, c->ldxb, c->Y, c->ldy,
-                                   c->yI, c->G, c->ldg, c->r, (int)c->opt_full_lower, c->err_flag);
+                                   c->yI, c->G, c->ldg, c->r, (int)c->opt_full_lower, c->err_flag, s1 ? &s1f : nullptr);
             if (k < 0) return fail(c, CASGD_ECUDA, "gram_narrow launch: %s", cudaGetErrorString(cudaGetLastError()));
         } else if (c->cur_gram == 1) {
             k = launch_gram_simt(st, c->Y, c->ldy, c->n, sb, b, c->xbf, c->G, c->ldg, c->r, (int)c->opt_full_lower);
@@ -217,13 +220,14 @@ int enqueue_step(casgd_ctx *c, cudaStream_t st, const int32_t *idx, const StepPa
                 c->tc_plan = gram_tc_plan_create(c->Y, c->ldy, c->n, c->rows_alloc, c->xbf, c->ldxb, c->err, sizeof c->err);
                 if (!c->tc_plan) return CASGD_ECUDA;
             }
-            k = launch_gram_tc(st, c->tc_plan, sb, b, c->G, c->ldg, c->r, (int)c->opt_full_lower, (int)c->opt_ksplit, c->err, sizeof c->err);
+            k = launch_gram_tc(st, c->tc_plan, sb, b, c->G, c->ldg, c->r, (int)c->opt_full_lower, (int)c->opt_ksplit, c->err, sizeof c->err,
+                               s1 ? &s1f : nullptr);
             if (k < 0) return CASGD_ECUDA;
         }
         t.done(k); *kernels += k;
     }
     const bool fused = !c->opt_no_fuse && recurrence_fuses_update(s, b, c->ldg, c->ldy, c->rws, (int)c->opt_rec_impl);
-    {
+    if (!s1) {
         StageTimer t(c, CASGD_STAGE_RECURRENCE);
         const FusedUpdate fu{c->Y, c->ldy, c->n, x, ind, c->xbf};
         k = launch_recurrence(st, c->G, c->ldg, c->r, c->yI, s, b, alpha, c->loss, c->z, c->u, c->rws,

@@ -220,18 +220,24 @@ int launch_set_params(cudaStream_t st, StepParams *ind, const int32_t *idx, floa
 
 // tcgen05 Gram + margin (gram_tc.cu). The plan owns the TMA tensor maps of the Y workspace and of the
 // BF16 shadow (a [16 x ldxb] buffer: row 0 = x_bf, rows 1..15 zero). ksplit_opt <= 0: choose automatically.
+// s = 1: there is no correction, u = l'(r, y_I) -- the Gram kernels' margin epilogue can apply l' itself.
+struct S1Fuse {
+    int loss;
+    const float *yI;
+    float *z, *u;
+};
 struct GramTcPlan;
 GramTcPlan *gram_tc_plan_create(const uint16_t *Y, int32_t ldy, int32_t n, int32_t sb_rows_alloc,
                                 const uint16_t *xbf, int32_t ldxb, char *err, int errlen);
 void gram_tc_plan_destroy(GramTcPlan *p);
 int launch_gram_tc(cudaStream_t st, GramTcPlan *plan, int32_t sb, int32_t b, float *G, int32_t ldg, float *r,
-                   int full_lower, int ksplit_opt, char *err, int errlen);
+                   int full_lower, int ksplit_opt, char *err, int errlen, const S1Fuse *s1);
 
 // gather + Gram + margin in one kernel for narrow rows (n <= 64): gram_tc.cu
 int launch_gram_narrow(cudaStream_t st, const uint16_t *A, int64_t lda, const float *y, int64_t m, int32_t n,
                        const int32_t *idx, const StepParams *ind, int64_t idx_off, int32_t sb, int32_t b,
                        const uint16_t *xbf, int32_t ldxb, uint16_t *Y, int32_t ldy, float *yI, float *G, int32_t ldg,
-                       float *r, int full_lower, int *err_flag);
+                       float *r, int full_lower, int *err_flag, const S1Fuse *s1);
 
 // cta_group::2 Gram + margin for large shapes (gram_pair.cu): 256 x 256 / 256 x 512 tiles on CTA pairs, work lists
 // built on the host. gram_pair_prepare (outside stream capture) returns the estimated cycles, or -1.

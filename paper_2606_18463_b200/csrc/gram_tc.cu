@@ -38,6 +38,10 @@ struct GramParams {
     float *G;
     float *r;
     int32_t ldg, sb, b, n, T, ntiles, ksplit, kb_total, full_lower;
+    // s = 1 (one block: u = l'(r, y_I), no correction): the margin epilogue applies l' itself, no recurrence kernel
+    int32_t s1_loss;                    // -1: off
+    const float *yI;
+    float *z, *u;
 };
 
 // ------------------------------------------------------------------------------------ PTX ---
@@ -308,8 +312,16 @@ gram_tc_kernel(const __grid_constant__ CUtensorMap tmY, const __grid_constant__ 
                 const uint32_t rv = tc_ld1(t_row + (k.need_g ? BN : 0));
                 tc_wait_ld();
                 if (row_ok) {
-                    if (!accumulate) p.r[row] = __uint_as_float(rv);
-                    else atomicAdd(p.r + row, __uint_as_float(rv));
+                    if (!accumulate) {
+                        p.r[row] = __uint_as_float(rv);
+                        if (p.s1_loss >= 0) {
+                            const float zz = __uint_as_float(rv);
+                            p.z[row] = zz;
+                            p.u[row] = lprime_rt(p.s1_loss, zz, ld_dep(p.yI + row));
+                        }
+                    } else {
+                        atomicAdd(p.r + row, __uint_as_float(rv));
+                    }
                 }
             }
             tc_fence_before();
@@ -350,6 +362,8 @@ struct NarrowParams {
     float *yI, *G, *r;
     int *err_flag;
     int32_t ldy, ldg, sb, b, n, T, full_lower;
+    int32_t s1_loss;                    // >= 0 (s = 1): the epilogue also writes z = r and u = l'(r, y_I)
+    float *z, *u;
 };
 
 __global__ void __launch_bounds__(kNwThreads)
@@ -393,6 +407,7 @@ gram_narrow_kernel(const NarrowParams p)
     const int32_t *I = p.ind ? p.ind->idx + p.idx_off : p.idx;
     const int ksteps = (p.n + 15) >> 4;             // K = 16 steps that hold data
     const int nfill = 2 * ksteps;                   // 16-byte chunks of a tile row the MMAs read
+    float ylab = 0.f;                               // label of row ti * 128 + threadIdx.x (diagonal tiles)
     for (int op = 0; op < (diag ? 1 : 2); ++op) {
         const int trow = (op == 0 ? ti : tj) * BM + (int)threadIdx.x;
         int64_t src = -1;
@@ -428,7 +443,8 @@ gram_narrow_kernel(const NarrowParams p)
 #pragma unroll
             for (int c = 0; c < 8; ++c)
                 if (c * 8 < p.ldy) *reinterpret_cast<uint4 *>(p.Y + (int64_t)trow * p.ldy + c * 8) = v[c];
-            p.yI[trow] = src >= 0 ? p.y[src] : 0.f;
+            ylab = src >= 0 ? p.y[src] : 0.f;
+            p.yI[trow] = ylab;
         }
     }
     if (diag) {                                     // x_bf: 16 rows x 64 columns right behind the B tile (rows 1..15 are zero)
@@ -492,7 +508,13 @@ gram_narrow_kernel(const NarrowParams p)
         const uint32_t rv = tc_ld1(t_row + (need_g ? BN : 0));
         tc_wait_ld();
         const int row = ti * BM + warp * 32 + lane;
-        if (row < p.sb) p.r[row] = __uint_as_float(rv);
+        if (row < p.sb) {
+            p.r[row] = __uint_as_float(rv);
+            if (p.s1_loss >= 0) {                   // this thread gathered this very row: its label is in a register
+                p.z[row] = __uint_as_float(rv);
+                p.u[row] = lprime_rt(p.s1_loss, __uint_as_float(rv), ylab);
+            }
+        }
     }
     tc_fence_before();
     __syncthreads();
@@ -562,7 +584,7 @@ GramTcPlan *gram_tc_plan_create(const uint16_t *Y, int32_t ldy, int32_t n, int32
 void gram_tc_plan_destroy(GramTcPlan *p) { delete p; }
 
 int launch_gram_tc(cudaStream_t st, GramTcPlan *plan, int32_t sb, int32_t b, float *G, int32_t ldg, float *r,
-                   int full_lower, int ksplit_opt, char *err, int errlen)
+                   int full_lower, int ksplit_opt, char *err, int errlen, const S1Fuse *s1)
 {
     if (!plan->attr_set) {
         cudaError_t e = cudaFuncSetAttribute(gram_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemBytes);
@@ -578,6 +600,11 @@ int launch_gram_tc(cudaStream_t st, GramTcPlan *plan, int32_t sb, int32_t b, flo
     p.ntiles = p.T * (p.T + 1) / 2;
     p.kb_total = (plan->n + BK - 1) / BK;
     p.full_lower = full_lower;
+    p.s1_loss = s1 ? s1->loss : -1;
+    p.yI = s1 ? s1->yI : nullptr;
+    p.z = s1 ? s1->z : nullptr;
+    p.u = s1 ? s1->u : nullptr;
+    if (s1) ksplit_opt = 1;                             // l' needs the whole margin in one accumulator
     int ksplit = ksplit_opt;
     if (ksplit <= 0) {
         // fill the 148 SMs when there are few tiles -- but the cleared G, its memset node and the red.add epilogue
@@ -602,7 +629,7 @@ int launch_gram_tc(cudaStream_t st, GramTcPlan *plan, int32_t sb, int32_t b, flo
 int launch_gram_narrow(cudaStream_t st, const uint16_t *A, int64_t lda, const float *y, int64_t m, int32_t n,
                        const int32_t *idx, const StepParams *ind, int64_t idx_off, int32_t sb, int32_t b,
                        const uint16_t *xbf, int32_t ldxb, uint16_t *Y, int32_t ldy, float *yI, float *G, int32_t ldg,
-                       float *r, int full_lower, int *err_flag)
+                       float *r, int full_lower, int *err_flag, const S1Fuse *s1)
 {
     static bool attr_set = false;
     if (!attr_set) {
@@ -614,6 +641,9 @@ int launch_gram_narrow(cudaStream_t st, const uint16_t *A, int64_t lda, const fl
     p.Y = Y; p.yI = yI; p.G = G; p.r = r; p.err_flag = err_flag; p.ldy = ldy; p.ldg = ldg; p.sb = sb; p.b = b; p.n = n;
     p.T = (sb + BM - 1) / BM;
     p.full_lower = full_lower;
+    p.s1_loss = s1 ? s1->loss : -1;
+    p.z = s1 ? s1->z : nullptr;
+    p.u = s1 ? s1->u : nullptr;
     const int tiles = p.T * (p.T + 1) / 2;
     return launch_pdl(gram_narrow_kernel, dim3(tiles), dim3(kNwThreads), kNwSmem, st, 1, p) == cudaSuccess ? 1 : -1;
 }
