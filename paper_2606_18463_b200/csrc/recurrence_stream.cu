@@ -368,16 +368,24 @@ recurrence_stream_kernel(const float *G, int32_t ldg, const float *r,
         const uint32_t ring = base + L.bring + (uint32_t)(g * kDepth) * kUnitBytes + (uint32_t)lane * 16u;
         const float *gbase = G + (int64_t)(kQuad * (crank + gamma * C)) * ldg + lane * 4;   // + j b ldg + c * 128
         int pj = 1, pc = cidx, pslot = 0;               // next unit to prefetch
+        // running pointers instead of a 64-bit multiply per unit (the bulk warps are bound by their own issue rate)
+        const int64_t step_stride = (int64_t)b * ldg;   // floats between the same row of consecutive blocks
+        const float *prow = gbase + step_stride;        // row group of block pj, column 0
+        const float *psrc = prow + cidx * kChunk;       // ... chunk pc
         auto cursor_norm = [&]() {
-            while (pj < s && pc >= num_chunks(pj, b) - kWin) { ++pj; pc = cidx; }
+            while (pj < s && pc >= num_chunks(pj, b) - kWin) { ++pj; pc = cidx; prow += step_stride; psrc = prow + cidx * kChunk; }
         };
         auto prefetch_unit = [&]() {
             if (pj < s) {
-                const float *src = gbase + (int64_t)pj * b * ldg + pc * kChunk;
+                const uint32_t dst = ring + (uint32_t)pslot * kUnitBytes;
+                const float *src = psrc;
 #pragma unroll
-                for (int i = 0; i < kQuad; ++i)
-                    cp_async16(ring + (uint32_t)pslot * kUnitBytes + (uint32_t)i * (kChunk * 4u), src + (int64_t)i * ldg);
+                for (int i = 0; i < kQuad; ++i) {
+                    cp_async16(dst + (uint32_t)i * (kChunk * 4u), src);
+                    src += ldg;
+                }
                 pc += nw;
+                psrc += nw * kChunk;
                 cursor_norm();
             }
             cp_async_commit();
