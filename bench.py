@@ -132,7 +132,7 @@ class ClockSampler:
         self.f = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
         try:
             self.p = subprocess.Popen(["nvidia-smi", f"--id={index}", f"--query-gpu={self.Q}",
-                                       "--format=csv,noheader,nounits", "-lms", "100"],
+                                       "--format=csv,noheader,nounits", "-lms", "20"],
                                       stdout=self.f, stderr=subprocess.DEVNULL)
         except OSError:
             self.p = None
@@ -358,11 +358,24 @@ def main_ours(args, cfg, s):
     st = cg.stage_times(reset=True)
     cg.set_option(binding.OPT_PROFILE, 0)
     work = stage_work(cfg.n, s, cfg.b, pk)
+    # fused stages: a stage with no launch of its own ran inside its neighbour (n <= 64: gather inside the Gram
+    # kernel; small steps: gradient + update inside the recurrence kernel; s = 1: l' inside the Gram epilogue)
+    for absent, host in (("gather", "gram"), ("gradient", "recurrence"), ("recurrence", "gram")):
+        if st[absent][1] == 0 and st[host][1] > 0:
+            work[host]["bytes"] += work[absent]["bytes"]
+            work[host]["flops"] += work[absent]["flops"]
+            work[host]["fused"] = work[host].get("fused", []) + [absent]
     stages = {}
     for name, wk in work.items():
         tot_ms, cnt = st[name]
         per_step = tot_ms / Kp
         rl = roofline_of(name, wk, per_step, pk, ncu_traffic(cfg.name, s, name)) if cnt else None
+        if rl and name == "recurrence" and s > 1:
+            # the chain is s - 1 dependent hops of one distributed-shared-memory broadcast each: its own floor
+            rl["chain"] = dict(hops=s - 1, us_per_hop=round(per_step * 1e3 / (s - 1), 3),
+                               note="latency chain: ~0.42 us per hop measured at best (DESIGN.md section 6)")
+        if rl and wk.get("fused"):
+            rl["includes"] = wk["fused"]
         stages[name] = dict(ms_per_step=round(per_step, 6), launches_per_step=cnt / Kp, roofline=rl,
                             alg_bytes=wk["bytes"], alg_flops=wk["flops"])
     dominant = max(stages, key=lambda k: stages[k]["ms_per_step"])
