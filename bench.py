@@ -372,8 +372,10 @@ def main_ours(args, cfg, s):
         rl = roofline_of(name, wk, per_step, pk, ncu_traffic(cfg.name, s, name)) if cnt else None
         if rl and name == "recurrence" and s > 1:
             # the chain is s - 1 dependent hops of one distributed-shared-memory broadcast each: its own floor
-            rl["chain"] = dict(hops=s - 1, us_per_hop=round(per_step * 1e3 / (s - 1), 3),
-                               note="latency chain: ~0.42 us per hop measured at best (DESIGN.md section 6)")
+            rl["chain"] = dict(hops=s - 1, kernel_us_per_hop=round(per_step * 1e3 / (s - 1), 3),
+                               note="latency chain: the kernel's time over its s - 1 dependent hops (start-up, launch "
+                                    "latency and any fused update included); ~0.42 us per hop in steady state "
+                                    "(DESIGN.md section 6)")
         if rl and wk.get("fused"):
             rl["includes"] = wk["fused"]
         stages[name] = dict(ms_per_step=round(per_step, 6), launches_per_step=cnt / Kp, roofline=rl,

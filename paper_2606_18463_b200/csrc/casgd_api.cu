@@ -195,15 +195,22 @@ int enqueue_step(casgd_ctx *c, cudaStream_t st, const int32_t *idx, const StepPa
     const int32_t sb = s * b;
     const float alpha = eta / (float)b;
     int k;
-    // s = 1: no correction, u = l'(r, y_I): applied by the Gram kernel's margin epilogue (no recurrence kernel)
-    const bool s1 = s == 1 && !c->opt_no_fuse && (c->cur_gram == 4 || (c->cur_gram == 2 && c->n <= 1024 && c->opt_ksplit <= 1));
+    // s = 1: no Gram, no correction, u = l'(r, y_I): one kernel computes the margin and applies l' (the fused
+    // gather + Gram kernel's epilogue for n <= 64, a warp-per-row kernel otherwise); a forced Gram kernel still runs
+    const bool s1 = s == 1 && !c->opt_no_fuse && (c->cur_gram == 4 || c->opt_gram_impl == 0);
     const S1Fuse s1f{c->loss, c->yI, c->z, c->u};
-    if (c->cur_gram != 4) {
+    if (s1 && c->cur_gram != 4) {
+        // wide rows: gather + margin + l' in one warp-per-row kernel (there is no Gram at s = 1)
+        StageTimer t(c, CASGD_STAGE_GRAM);
+        k = launch_margin_s1(st, c->A, c->lda, c->y, c->m, c->n, idx, ind, idx_off, b, c->loss, c->xbf, c->Y, c->ldy, c->yI,
+                             c->r, c->z, c->u, c->err_flag);
+        t.done(k); *kernels += k;
+    } else if (c->cur_gram != 4) {
         StageTimer t(c, CASGD_STAGE_GATHER);
         k = launch_gather(st, c->A, c->lda, c->y, c->m, c->n, idx, ind, idx_off, sb, c->Y, c->ldy, c->yI, c->err_flag);
         t.done(k); *kernels += k;
     }
-    {
+    if (!(s1 && c->cur_gram != 4)) {
         StageTimer t(c, CASGD_STAGE_GRAM);
         if (c->cur_gram == 4) {
             k = launch_gram_narrow(st, c->A, c->lda, c->y, c->m, c->n, idx, ind, idx_off, sb, b, c->xbf, c->ldxb, c->Y, c->ldy,
@@ -220,8 +227,7 @@ int enqueue_step(casgd_ctx *c, cudaStream_t st, const int32_t *idx, const StepPa
                 c->tc_plan = gram_tc_plan_create(c->Y, c->ldy, c->n, c->rows_alloc, c->xbf, c->ldxb, c->err, sizeof c->err);
                 if (!c->tc_plan) return CASGD_ECUDA;
             }
-            k = launch_gram_tc(st, c->tc_plan, sb, b, c->G, c->ldg, c->r, (int)c->opt_full_lower, (int)c->opt_ksplit, c->err, sizeof c->err,
-                               s1 ? &s1f : nullptr);
+            k = launch_gram_tc(st, c->tc_plan, sb, b, c->G, c->ldg, c->r, (int)c->opt_full_lower, (int)c->opt_ksplit, c->err, sizeof c->err);
             if (k < 0) return CASGD_ECUDA;
         }
         t.done(k); *kernels += k;

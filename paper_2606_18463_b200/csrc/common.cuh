@@ -114,6 +114,12 @@ __device__ __forceinline__ uint4 ldg_nc_v4(const void *p)
 // __ldg: the compiler treats such data as read-only for the whole kernel and may hoist the load ABOVE pdl_wait()
 // (seen: a gradient kernel summing the previous step's u). Such inputs are plain pointers, or go through ld_dep().
 __device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+__device__ __forceinline__ uint4 ld_dep_v4(const void *p)
+{
+    uint4 r;
+    asm volatile("ld.global.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(r.x), "=r"(r.y), "=r"(r.z), "=r"(r.w) : "l"(p) : "memory");
+    return r;
+}
 __device__ __forceinline__ float ld_dep(const float *p)
 {
     float v;
@@ -205,6 +211,11 @@ struct GradWorkspace {
 int launch_gradient_bf16(cudaStream_t st, const uint16_t *Y, int32_t ldy, int32_t n, int32_t sb, const float *u,
                          float alpha, float *x, const StepParams *ind, uint16_t *xbf, const GradWorkspace &ws);
 
+// s = 1 with wide rows: gather + margin + l' in one warp-per-row kernel (no Gram exists at s = 1); gradient.cu
+int launch_margin_s1(cudaStream_t st, const uint16_t *A, int64_t lda, const float *y, int64_t m, int32_t n,
+                     const int32_t *idx, const StepParams *ind, int64_t idx_off, int32_t b, int loss, const uint16_t *xbf,
+                     uint16_t *Y, int32_t ldy, float *yI, float *r, float *z, float *u, int *err_flag);
+
 int launch_sgd32_step(cudaStream_t st, const float *A32, int64_t lda32, const float *y, int64_t m, int32_t n,
                       const int32_t *idx, int32_t b, float alpha, int loss, float *x, float *u, float *z,
                       int *err_flag, const GradWorkspace &ws);
@@ -231,7 +242,7 @@ GramTcPlan *gram_tc_plan_create(const uint16_t *Y, int32_t ldy, int32_t n, int32
                                 const uint16_t *xbf, int32_t ldxb, char *err, int errlen);
 void gram_tc_plan_destroy(GramTcPlan *p);
 int launch_gram_tc(cudaStream_t st, GramTcPlan *plan, int32_t sb, int32_t b, float *G, int32_t ldg, float *r,
-                   int full_lower, int ksplit_opt, char *err, int errlen, const S1Fuse *s1);
+                   int full_lower, int ksplit_opt, char *err, int errlen);
 
 // gather + Gram + margin in one kernel for narrow rows (n <= 64): gram_tc.cu
 int launch_gram_narrow(cudaStream_t st, const uint16_t *A, int64_t lda, const float *y, int64_t m, int32_t n,

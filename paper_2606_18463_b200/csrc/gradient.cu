@@ -286,6 +286,80 @@ int launch_gradient_bf16(cudaStream_t st, const uint16_t *Y, int32_t ldy, int32_
     return launch_gradient_any<uint16_t, false, true>(st, Y, ldy, nullptr, 0, n, sb, u, alpha, x, ind, xbf, ws);
 }
 
+// ------------------------------------------------------------- s = 1 with BF16 rows ---
+// At s = 1 there is no Gram matrix and no correction: the step is plain mini-batch SGD on BF16 rows with a BF16
+// shadow of x (Alg. 1 with s = 1, L99). One warp per sampled row gathers the row from A (16-byte loads), writes it
+// to the Y stage (the gradient's second pass and casgd_debug_export read it), forms r = y_i . x_bf in FP32 and
+// applies l': gather + margin + residual in one kernel instead of three.
+__global__ void __launch_bounds__(256)
+margin_s1_kernel(const uint16_t *__restrict__ A, int64_t lda, const float *__restrict__ y, int64_t m, int32_t n,
+                 const int32_t *idx, const StepParams *ind, int64_t idx_off, int32_t b, int loss, const uint16_t *xbf,
+                 uint16_t *Y, int32_t ldy, float *yI, float *r, float *z, float *u, int *err_flag)
+{
+    pdl_trigger();
+    pdl_wait();                                     // x_bf comes from the previous gradient; Y is read by it until now
+    const int row = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
+    if (row >= b) return;
+    const int32_t *I = ind ? ind->idx + idx_off : idx;
+    int64_t src = I[row];
+    const bool ok = src >= 0 && src < m;
+    float acc = 0.f;
+    const int nvec = ldy >> 3;
+    for (int cv0 = lane; cv0 < nvec; cv0 += 128) {   // four 16-byte loads of the row in flight per lane
+        uint4 v[4], xv[4];
+#pragma unroll
+        for (int q = 0; q < 4; ++q) {
+            const int col = (cv0 + 32 * q) * 8;
+            v[q] = make_uint4(0u, 0u, 0u, 0u);
+            if (ok && col < n) v[q] = ldg_nc_v4(A + src * lda + col);
+        }
+#pragma unroll
+        for (int q = 0; q < 4; ++q) {
+            const int col = (cv0 + 32 * q) * 8;
+            xv[q] = make_uint4(0u, 0u, 0u, 0u);
+            if (col < ldy) xv[q] = ld_dep_v4(xbf + col);     // the shadow buffer is padded to 64 columns with zeros
+        }
+#pragma unroll
+        for (int q = 0; q < 4; ++q) {
+            const int col = (cv0 + 32 * q) * 8;
+            if (col >= ldy) continue;
+            const int valid = n - col;
+            if (valid < 8) {                         // the last chunk of the row: pad columns of Y are zero
+                uint32_t w[4] = {v[q].x, v[q].y, v[q].z, v[q].w};
+#pragma unroll
+                for (int e = 0; e < 4; ++e) {
+                    if (2 * e >= valid) w[e] = 0u;
+                    else if (2 * e + 1 >= valid) w[e] &= 0x0000ffffu;
+                }
+                v[q] = make_uint4(w[0], w[1], w[2], w[3]);
+            }
+            *reinterpret_cast<uint4 *>(Y + (int64_t)row * ldy + col) = v[q];
+            acc = fmaf(bf16lo(v[q].x), bf16lo(xv[q].x), acc); acc = fmaf(bf16hi(v[q].x), bf16hi(xv[q].x), acc);
+            acc = fmaf(bf16lo(v[q].y), bf16lo(xv[q].y), acc); acc = fmaf(bf16hi(v[q].y), bf16hi(xv[q].y), acc);
+            acc = fmaf(bf16lo(v[q].z), bf16lo(xv[q].z), acc); acc = fmaf(bf16hi(v[q].z), bf16hi(xv[q].z), acc);
+            acc = fmaf(bf16lo(v[q].w), bf16lo(xv[q].w), acc); acc = fmaf(bf16hi(v[q].w), bf16hi(xv[q].w), acc);
+        }
+    }
+    acc = warp_sum(acc);
+    if (lane == 0) {
+        const float ylab = ok ? y[src] : 0.f;
+        if (!ok) atomicOr(err_flag, 1);
+        yI[row] = ylab;
+        r[row] = acc;
+        z[row] = acc;
+        u[row] = lprime_rt(loss, acc, ylab);
+    }
+}
+
+int launch_margin_s1(cudaStream_t st, const uint16_t *A, int64_t lda, const float *y, int64_t m, int32_t n,
+                     const int32_t *idx, const StepParams *ind, int64_t idx_off, int32_t b, int loss, const uint16_t *xbf,
+                     uint16_t *Y, int32_t ldy, float *yI, float *r, float *z, float *u, int *err_flag)
+{
+    launch_pdl(margin_s1_kernel, dim3((b * 32 + 255) / 256), dim3(256), 0, st, 1, A, lda, y, m, n, idx, ind, idx_off, b, loss, xbf, Y,
+               ldy, yI, r, z, u, err_flag);
+    return 1;
+}
+
 // ------------------------------------------------------------- FP32 s = 1 baseline ---
 
 // z_i = a32_{I_i}^T x ; u_i = l'(z_i, y_{I_i}); one warp per row, everything FP32.

@@ -38,10 +38,6 @@ struct GramParams {
     float *G;
     float *r;
     int32_t ldg, sb, b, n, T, ntiles, ksplit, kb_total, full_lower;
-    // s = 1 (one block: u = l'(r, y_I), no correction): the margin epilogue applies l' itself, no recurrence kernel
-    int32_t s1_loss;                    // -1: off
-    const float *yI;
-    float *z, *u;
 };
 
 // ------------------------------------------------------------------------------------ PTX ---
@@ -312,16 +308,8 @@ gram_tc_kernel(const __grid_constant__ CUtensorMap tmY, const __grid_constant__ 
                 const uint32_t rv = tc_ld1(t_row + (k.need_g ? BN : 0));
                 tc_wait_ld();
                 if (row_ok) {
-                    if (!accumulate) {
-                        p.r[row] = __uint_as_float(rv);
-                        if (p.s1_loss >= 0) {
-                            const float zz = __uint_as_float(rv);
-                            p.z[row] = zz;
-                            p.u[row] = lprime_rt(p.s1_loss, zz, ld_dep(p.yI + row));
-                        }
-                    } else {
-                        atomicAdd(p.r + row, __uint_as_float(rv));
-                    }
+                    if (!accumulate) p.r[row] = __uint_as_float(rv);
+                    else atomicAdd(p.r + row, __uint_as_float(rv));
                 }
             }
             tc_fence_before();
@@ -584,7 +572,7 @@ GramTcPlan *gram_tc_plan_create(const uint16_t *Y, int32_t ldy, int32_t n, int32
 void gram_tc_plan_destroy(GramTcPlan *p) { delete p; }
 
 int launch_gram_tc(cudaStream_t st, GramTcPlan *plan, int32_t sb, int32_t b, float *G, int32_t ldg, float *r,
-                   int full_lower, int ksplit_opt, char *err, int errlen, const S1Fuse *s1)
+                   int full_lower, int ksplit_opt, char *err, int errlen)
 {
     if (!plan->attr_set) {
         cudaError_t e = cudaFuncSetAttribute(gram_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemBytes);
@@ -600,11 +588,6 @@ int launch_gram_tc(cudaStream_t st, GramTcPlan *plan, int32_t sb, int32_t b, flo
     p.ntiles = p.T * (p.T + 1) / 2;
     p.kb_total = (plan->n + BK - 1) / BK;
     p.full_lower = full_lower;
-    p.s1_loss = s1 ? s1->loss : -1;
-    p.yI = s1 ? s1->yI : nullptr;
-    p.z = s1 ? s1->z : nullptr;
-    p.u = s1 ? s1->u : nullptr;
-    if (s1) ksplit_opt = 1;                             // l' needs the whole margin in one accumulator
     int ksplit = ksplit_opt;
     if (ksplit <= 0) {
         // fill the 148 SMs when there are few tiles -- but the cleared G, its memset node and the red.add epilogue

@@ -507,16 +507,10 @@ int recurrence_max_coresident_ctas(int num_sms)
     return num_sms;                                     // one CTA per SM
 }
 
-static bool uses_stream(int32_t s, int32_t b, int32_t ldg, const RecWorkspace &ws, int impl)
-{
-    const int64_t gl_bytes = 2ll * b * b * s * (s - 1);
-    const bool stream_ok = (impl == 4 || impl == 0) && recurrence_stream_ok(s, b, ldg, ws.cluster);
-    return stream_ok && (impl == 4 || gl_bytes >= ws.grid_threshold_bytes);
-}
-
 bool recurrence_fuses_update(int32_t s, int32_t b, int32_t ldg, int32_t ldy, const RecWorkspace &ws, int impl)
 {
-    return uses_stream(s, b, ldg, ws, impl) && recurrence_stream_fuses_update(s, b, ldy);
+    // with the update fused in, the cluster kernel beats the one-CTA kernel + a gradient kernel even for tiny G (measured)
+    return (impl == 4 || impl == 0) && recurrence_stream_ok(s, b, ldg, ws.cluster) && recurrence_stream_fuses_update(s, b, ldy);
 }
 
 int launch_recurrence(cudaStream_t st, const float *G, int32_t ldg, const float *r, const float *yI, int32_t s,
@@ -529,7 +523,7 @@ int launch_recurrence(cudaStream_t st, const float *G, int32_t ldg, const float 
     const bool grid_ok = ws.max_ctas > 0 && (int64_t)ws.max_ctas * kRecWarps * 16 >= sb;
     const bool cluster_ok = ws.cluster > 0 && b % 4 == 0 && ldg % 4 == 0;
     const bool stream_ok = (impl == 4 || impl == 0) && recurrence_stream_ok(s, b, ldg, ws.cluster);
-    if (stream_ok && (impl == 4 || gl_bytes >= ws.grid_threshold_bytes))
+    if (stream_ok && (impl == 4 || gl_bytes >= ws.grid_threshold_bytes || fu))
         return launch_recurrence_stream(st, G, ldg, r, yI, s, b, alpha, loss, z, u, ws.cluster, fu);
     const bool use_cluster = cluster_ok && (impl >= 3 || (impl == 0 && gl_bytes >= ws.grid_threshold_bytes));
     if (use_cluster) {
