@@ -133,7 +133,7 @@ __host__ __device__ inline StreamLayout stream_layout(int s, int b)
     L.ubar = o;   o += 8u * (uint32_t)s;
     L.pbar = o;   o += 8u * (uint32_t)s;
     o = (o + 15u) & ~15u;
-    L.part = o;   o += 16u * (uint32_t)(kPartDepth * kMaxQuadsPerCta * kBulkWarps);     // [step % depth][quad][bulk warp][4 rows]
+    L.part = o;   o += 16u * (uint32_t)(kPartDepth * kMaxQuadsPerCta);                  // [step % depth][quad][4 rows]
     o = (o + 127u) & ~127u;
     L.cring = o;  o += (uint32_t)(kCritPer * kMaxQuadsPerCta * kCritDepth * kWin) * kUnitBytes;
     L.bring = o;  o += (uint32_t)(kBulkWarps * kDepth) * kUnitBytes;
@@ -211,7 +211,7 @@ recurrence_stream_kernel(const float *G, int32_t ldg, const float *r,
     for (int k = threadIdx.x; k < s; k += kThreads) {
         mbar_init(ubar + 8u * k, 1);
         mbar_expect_tx(ubar + 8u * k, 4u * (uint32_t)b);
-        mbar_init(pbar + 8u * k, (uint32_t)nbulk);
+        mbar_init(pbar + 8u * k, (uint32_t)max(qpc, 1));      // one bulk warp per owned row group reports per step
     }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     pdl_wait();                                         // G, r and y_I come from the Gram and gather kernels
@@ -296,13 +296,10 @@ recurrence_stream_kernel(const float *G, int32_t ldg, const float *r,
                 if (nch > kWin) {
                     // lane (li, gg): the partial sum of row li from bulk warp gg of this group
                     mbar_wait(pbar + 8u * j, 0u);
-                    float p = 0.f;
-                    for (int gg = lane & 7; gg < nbulk / qpc; gg += 8) {    // at most two partials per lane
-                        float pv;
-                        asm volatile("ld.shared.f32 %0, [%1];" : "=f"(pv)
-                                     : "r"(part + 16u * (uint32_t)(((j % kPartDepth) * kMaxQuadsPerCta + gamma) * kBulkWarps + gg) + 4u * (uint32_t)li));
-                        p += pv;
-                    }
+                    float p = 0.f;                      // lane 8 li carries row li's partial sum into the reduction
+                    if ((lane & 7) == 0)
+                        asm volatile("ld.shared.f32 %0, [%1];" : "=f"(p)
+                                     : "r"(part + 16u * (uint32_t)((j % kPartDepth) * kMaxQuadsPerCta + gamma) + 4u * (uint32_t)li));
 #pragma unroll
                     for (int i = 0; i < kQuad; ++i) acc[i] = (i == li) ? p : 0.f;
                 }
@@ -359,21 +356,23 @@ recurrence_stream_kernel(const float *G, int32_t ldg, const float *r,
         }
     }
     else if (is_bulk) {
-        // ===== bulk warp: group gamma, lane cidx of nw; chunks c = cidx, cidx + nw, ... < nch(j) - kWin of every step =====
-        // These columns belong to blocks that landed (kWin - 1) * 128 / b hops ago, so the bulk warps run
-        // several steps ahead of the chain and are bound only by the SM's L2 bandwidth.
+        // ===== bulk warp: every 128-column chunk of a step's rows but the newest kWin =====
+        // These columns belong to blocks that landed (kWin - 1) * 128 / b hops ago, so a bulk warp can be several
+        // steps ahead of the chain; it is bound by its own issue rate and the SM's L2 bandwidth.
         const int g = brank;
         const int nw = nbulk / qpc;                     // bulk warps per owned group
-        const int gamma = g / nw, cidx = g % nw;
+        const int gamma = g / nw, widx = g % nw;
+        // Warp widx of a row group takes WHOLE steps j = 1 + widx, 1 + widx + nw, ...: all bulk chunks of the step,
+        // one reduction and one hand-over per step (splitting every step over all warps cost a 6-shuffle reduction,
+        // a barrier arrive and the loop set-up per 2-3 units). It has nw hops to finish a step.
         const uint32_t ring = base + L.bring + (uint32_t)(g * kDepth) * kUnitBytes + (uint32_t)lane * 16u;
         const float *gbase = G + (int64_t)(kQuad * (crank + gamma * C)) * ldg + lane * 4;   // + j b ldg + c * 128
-        int pj = 1, pc = cidx, pslot = 0;               // next unit to prefetch
-        // running pointers instead of a 64-bit multiply per unit (the bulk warps are bound by their own issue rate)
+        int pj = 1 + widx, pc = 0, pslot = 0;           // next unit to prefetch
         const int64_t step_stride = (int64_t)b * ldg;   // floats between the same row of consecutive blocks
-        const float *prow = gbase + step_stride;        // row group of block pj, column 0
-        const float *psrc = prow + cidx * kChunk;       // ... chunk pc
+        const float *prow = gbase + (int64_t)pj * step_stride;   // row group of block pj, column 0
+        const float *psrc = prow;                       // ... chunk pc
         auto cursor_norm = [&]() {
-            while (pj < s && pc >= num_chunks(pj, b) - kWin) { ++pj; pc = cidx; prow += step_stride; psrc = prow + cidx * kChunk; }
+            while (pj < s && pc >= num_chunks(pj, b) - kWin) { pj += nw; pc = 0; prow += nw * step_stride; psrc = prow; }
         };
         auto prefetch_unit = [&]() {
             if (pj < s) {
@@ -384,8 +383,8 @@ recurrence_stream_kernel(const float *G, int32_t ldg, const float *r,
                     cp_async16(dst + (uint32_t)i * (kChunk * 4u), src);
                     src += ldg;
                 }
-                pc += nw;
-                psrc += nw * kChunk;
+                pc += 1;
+                psrc += kChunk;
                 cursor_norm();
             }
             cp_async_commit();
@@ -400,18 +399,13 @@ recurrence_stream_kernel(const float *G, int32_t ldg, const float *r,
 
         int slot = 0, ready = 0;
 #pragma unroll 1
-        for (int j = 1; j < s; ++j) {
+        for (int j = 1 + widx; j < s; j += nw) {
             const int nb = num_chunks(j, b) - kWin;
             if (nb <= 0) continue;
-            // a warp with nothing to do must not run ahead into partial-sum slots that are still being read
-            if (j >= kPartDepth - 4) {
-                const int k = j - (kPartDepth - 4);
-                if (ready <= k) mbar_wait(ubar + 8u * k, 0u);
-            }
             REC_TRACE_B(6000 + 4 * j);
             float acc[kQuad] = {0.f, 0.f, 0.f, 0.f};
 #pragma unroll 1
-            for (int c = cidx; c < nb; c += nw) {
+            for (int c = 0; c < nb; ++c) {
                 cp_async_wait<kDepth - 2>();
                 float4 gv[kQuad];
 #pragma unroll
@@ -432,7 +426,7 @@ recurrence_stream_kernel(const float *G, int32_t ldg, const float *r,
             const float tot = quad_reduce(acc, lane);
             if ((lane & 7) == 0)
                 asm volatile("st.shared.f32 [%0], %1;"
-                             ::"r"(part + 16u * (uint32_t)(((j % kPartDepth) * kMaxQuadsPerCta + gamma) * kBulkWarps + cidx) + 4u * (uint32_t)li), "f"(tot) : "memory");
+                             ::"r"(part + 16u * (uint32_t)((j % kPartDepth) * kMaxQuadsPerCta + gamma) + 4u * (uint32_t)li), "f"(tot) : "memory");
             __syncwarp();
             if (lane == 0) mbar_arrive(pbar + 8u * j);
             REC_TRACE_B(6001 + 4 * j);
