@@ -35,6 +35,8 @@ SMALL = [
     (3, 5000, 2000, 9, 32),      # epsilon-shaped, n = 2000: ragged K tail (2000 = 31*64 + 16)
     (4, 6000, 512, 5, 64),       # Poisson
     (4, 6000, 512, 1, 64),       # s = 1: plain mini-batch SGD with a BF16 shadow
+    (2, 3000, 4096, 1, 128),     # s = 1, wide rows: the warp-per-row gather + margin + l' kernel
+    (3, 3000, 203, 1, 13),       # s = 1, odd n, odd b
     (0, 4096, 64, 7, 1),         # b = 1
     (3, 3000, 203, 11, 13),      # odd n, odd b: nothing aligned
 ]
