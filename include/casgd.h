@@ -61,10 +61,11 @@ typedef enum {
 #define CASGD_MAX_SB 16384
 
 /* Create a context for the dataset (A, y).
- *   X_bf16  m x n BF16 bit patterns, row-major, row stride `ldx` elements (ldx >= n). BORROWED for the
- *           context's lifetime when it can be used in place (16-byte aligned base, ldx % 8 == 0);
- *           otherwise (e.g. n = 18, ldx = 18) the library makes its own zero-padded copy during this
- *           call and does not touch X_bf16 again.
+ *   X_bf16  m x n BF16 bit patterns, row-major, row stride `ldx` elements (ldx >= n); all m * ldx elements
+ *           must be readable. BORROWED for the context's lifetime: it is used in place when it can be
+ *           (16-byte aligned base, ldx % 8 == 0); otherwise (e.g. n = 18, ldx = 18) the outer steps work on
+ *           the library's own zero-padded copy, made during this call, and casgd_loss still streams the
+ *           caller's (narrower) rows.
  *   y       m FP32 labels (Table 1: labels are FP32 throughout). BORROWED.
  *   loss    a casgd_loss_kind.
  *   cuda_stream  a cudaStream_t (NULL = the legacy default stream). All work of this context is
