@@ -153,7 +153,7 @@ int casgd_debug_export(casgd_ctx *c, int what, void *dst_host, int64_t dst_bytes
  *                              streaming cluster kernel (same cluster, G through a cp.async.bulk shared-memory
  *                              ring; needs b % 4 == 0 and b <= 128, else falls through to 3).
  *   CASGD_OPT_NO_FUSED_UPDATE  1 = the outer update always runs as its own kernel. Default 0: for small steps
- *                              (Y of at most 256 KB and 512 columns) the streaming recurrence kernel's cluster does
+ *                              (at most 136 KB of Y per CTA of the cluster, 2048 columns) the streaming recurrence kernel's cluster does
  *                              g = Y^T u, the update of x and the shadow itself, right after the chain.
  *   CASGD_OPT_LOSS_IMPL        0 = casgd_loss streams A through per-warp cp.async.bulk shared-memory rings
  *                              (default; n <= 8192), 1 = the plain 16-byte-load kernel. */

@@ -197,7 +197,7 @@ int launch_recurrence(cudaStream_t st, const float *G, int32_t ldg, const float 
 
 // recurrence_stream.cu: one cluster, G streamed through a shared-memory ring, u through distributed shared memory.
 bool recurrence_stream_ok(int32_t s, int32_t b, int32_t ldg, int cluster);
-bool recurrence_stream_fuses_update(int32_t s, int32_t b, int32_t ldy);
+bool recurrence_stream_fuses_update(int32_t s, int32_t b, int32_t ldy, int cluster_max);
 int launch_recurrence_stream(cudaStream_t st, const float *G, int32_t ldg, const float *r, const float *yI, int32_t s,
                              int32_t b, float alpha, int loss, float *z, float *u, int cluster, const FusedUpdate *fu);
 

@@ -510,7 +510,7 @@ int recurrence_max_coresident_ctas(int num_sms)
 bool recurrence_fuses_update(int32_t s, int32_t b, int32_t ldg, int32_t ldy, const RecWorkspace &ws, int impl)
 {
     // with the update fused in, the cluster kernel beats the one-CTA kernel + a gradient kernel even for tiny G (measured)
-    return (impl == 4 || impl == 0) && recurrence_stream_ok(s, b, ldg, ws.cluster) && recurrence_stream_fuses_update(s, b, ldy);
+    return (impl == 4 || impl == 0) && recurrence_stream_ok(s, b, ldg, ws.cluster) && recurrence_stream_fuses_update(s, b, ldy, ws.cluster);
 }
 
 int launch_recurrence(cudaStream_t st, const float *G, int32_t ldg, const float *r, const float *yI, int32_t s,

@@ -107,7 +107,7 @@ __device__ __forceinline__ float4 lds_f4(uint32_t saddr)
     return v;
 }
 
-// Fused outer update for small steps (Alg. 1 lines 16-17): when Y is small, g = Y^T u, x <- x - alpha g and the
+// Fused outer update for small steps (Alg. 1 lines 16-17): when a CTA's slice of Y is small (<= 136 KB, <= 2048 columns), g = Y^T u, x <- x - alpha g and the
 // BF16 shadow are done by this kernel's cluster right after the chain -- every CTA already holds all of u in shared
 // memory -- instead of by a fourth kernel: each CTA sums its slice of the rows, the per-CTA column sums meet in
 // CTA 0's shared memory (distributed shared memory stores), and CTA 0 adds them in a fixed order and updates x.
@@ -118,7 +118,7 @@ struct FusedGrad {
     const StepParams *ind;
     uint16_t *xbf;
 };
-constexpr int kFgMaxLdy = 512;                          // columns (padded) the fused update handles
+constexpr int kFgMaxLdy = 2048;                          // columns (padded) the fused update handles
 
 struct StreamLayout {                   // byte offsets into dynamic shared memory (base 128-byte aligned)
     uint32_t u, ubar, pbar, part, cring, bring, total;
@@ -554,9 +554,12 @@ bool recurrence_stream_ok(int32_t s, int32_t b, int32_t ldg, int cluster)
 }
 
 // Can the streaming kernel also do the outer update of this step (small Y)?
-bool recurrence_stream_fuses_update(int32_t s, int32_t b, int32_t ldy)
+bool recurrence_stream_fuses_update(int32_t s, int32_t b, int32_t ldy, int cluster_max)
 {
-    return ldy <= kFgMaxLdy && (int64_t)s * b * ldy * 2 <= 256 * 1024;
+    const int cluster = stream_cluster_for(b, cluster_max);
+    // measured: worth it while a CTA's slice of Y stays below ~136 KB (poisson-synth s=32: 131 KB per CTA, 32.1 -> 30.4 us;
+    // epsilon-shaped s=16 on 8 CTAs: 256 KB per CTA, 34.7 -> 36.9 us)
+    return ldy <= kFgMaxLdy && (int64_t)s * b * ldy * 2 <= (int64_t)136 * 1024 * cluster;
 }
 
 int launch_recurrence_stream(cudaStream_t st, const float *G, int32_t ldg, const float *r, const float *yI, int32_t s,
