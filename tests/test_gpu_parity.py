@@ -312,8 +312,14 @@ def test_graph_replay_and_host_entry_point_equal_single_steps(binding):
         cg.sync()
         assert torch.equal(xa, xb)
         xh = torch.zeros(cfg.n).pin_memory()
-        cg.outer_steps_host(torch.from_numpy(idx).pin_memory(), xh, s, b, cfg.eta)
+        idx_h = torch.from_numpy(idx).pin_memory()
+        cg.outer_steps_host(idx_h, xh, s, b, cfg.eta)
         assert torch.equal(xa.cpu(), xh)
+        # one step per call (the static host graph: staging copies, shadow rebuild, step, copy back), from pageable memory too
+        x1 = torch.zeros(cfg.n)
+        for h in range(steps):
+            cg.outer_steps_host(torch.from_numpy(idx[h * s * b:(h + 1) * s * b].copy()), x1, s, b, cfg.eta, n_steps=1)
+        assert torch.equal(xa.cpu(), x1)
 
 
 def _train_gpu(binding, cg, cfg, idx, s):
