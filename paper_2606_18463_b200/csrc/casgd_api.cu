@@ -286,7 +286,9 @@ int choose_gram(casgd_ctx *c, int32_t s, int32_t b)
         int64_t ks = std::max<int64_t>(1, std::min<int64_t>(c->num_sms / std::max<int64_t>(tiles, 1), kbt / 16));
         if (ks > 1 && kbt - kbt / ks < 24) ks = 1;
         const int64_t span_tc = (tiles * ks + c->num_sms - 1) / c->num_sms * ((kbt + ks - 1) / ks) * 770 + 2600 + (ks > 1 ? 12000 : 0);
-        if (span * 10 > span_tc * 9) return CASGD_OK;               // not clearly better: stay with the simpler kernel
+        // + the pair kernel's fixed cost (cluster launch, two cluster barriers, an epilogue nothing overlaps): ~12k cycles,
+        // measured on one-tile-per-pair shapes (n = 2000, sb = 2048: 23 us against 18.8 us for the 128-tile kernel)
+        if ((span + 12000) * 10 > span_tc * 9) return CASGD_OK;     // not clearly better: stay with the simpler kernel
     }
     c->cur_gram = 3;
     c->cur_bn = bn;

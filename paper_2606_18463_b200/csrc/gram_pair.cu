@@ -61,6 +61,10 @@ struct PairParams {
     const PairItem *items;              // [npairs x kMaxItemsPerPair]
     const int32_t *counts;              // [npairs]
     int32_t ldg, sb, b, n, full_lower, bn, nslots, accumulate;
+    // margin items cut along K into mslices pieces: partial sums per slice, summed in slice order by the last to finish
+    float *rpart;                       // [mslices x ldr]
+    unsigned *rcount;                   // [2 x row tiles], zero between launches
+    int32_t mslices, ldr;
 };
 
 // ------------------------------------------------------------------------------------ PTX ---
@@ -185,6 +189,7 @@ gram_pair_kernel(const __grid_constant__ CUtensorMap tmY, const __grid_constant_
     const uint32_t tmem_slot = bar_base + 8u * (2 * kStagesP + 4);
     volatile uint32_t *tmem_slot_ptr =
         reinterpret_cast<volatile uint32_t *>(smem_raw + (tmem_slot - smem_u32(smem_raw)));
+    volatile uint32_t *s_last_ptr = tmem_slot_ptr + 1;
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const uint32_t rank = cta_rank();
@@ -353,7 +358,29 @@ gram_pair_kernel(const __grid_constant__ CUtensorMap tmY, const __grid_constant_
             } else {
                 const uint32_t rv = tc_ld1(t_row);                         // column 0 of the N = 16 accumulator: Y x_bf
                 tc_wait_ld();
-                if (row_ok) p.r[row] = __uint_as_float(rv);
+                if (p.mslices == 1) {
+                    if (row_ok) p.r[row] = __uint_as_float(rv);
+                } else {
+                    // a K slice of the margin (slice index in w.J): park the partial sum; the slice that finishes last
+                    // adds the parts in slice order (deterministic) and writes r
+                    if (row_ok) p.rpart[(int64_t)w.J * p.ldr + row] = __uint_as_float(rv);
+                    __threadfence();
+                    asm volatile("bar.sync 1, 128;" ::: "memory");             // the four epilogue warps
+                    if (warp == 2 && lane == 0) {
+                        const unsigned old = atomicAdd(p.rcount + 2 * w.I + rank, 1u);
+                        const bool last = old == (unsigned)p.mslices - 1u;
+                        if (last) p.rcount[2 * w.I + rank] = 0u;
+                        *s_last_ptr = last ? 1u : 0u;
+                    }
+                    asm volatile("bar.sync 1, 128;" ::: "memory");
+                    if (*s_last_ptr && row_ok) {
+                        __threadfence();
+                        float sum = 0.f;
+                        for (int ks = 0; ks < p.mslices; ++ks) sum += __ldcg(p.rpart + (int64_t)ks * p.ldr + row);
+                        p.r[row] = sum;
+                    }
+                    asm volatile("bar.sync 1, 128;" ::: "memory");             // s_last is rewritten by the next margin item
+                }
             }
             tc_fence_before();
             __syncwarp();
@@ -395,14 +422,19 @@ bool make_bf16_map_p(CUtensorMap *map, const void *base, uint64_t cols, uint64_t
               CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
 }
 
-// Cost model (cycles), from the measured L2 cap of ~42.6 B/cycle/SM: a K block of a G item moves
-// (1 + nsub) * 16 KB per CTA and takes nsub * 512 MMA cycles, whichever is longer.
-inline int64_t kblock_cost(int nsub) { return std::max<int64_t>(512 * nsub, (int64_t)(1 + nsub) * 385); }
+// Cost model (cycles per 64-column K block), measured: a 256 x 256 item runs at the tensor pipe's floor (4 MMAs of
+// 128 cycles: 519 measured); a 256 x 512 item moves 48 KB per K block and has a single accumulator (no overlap of
+// its epilogue): ~1300; a margin item (N = 16) is bound by its operand loads: ~410.
+inline int64_t kblock_cost(int nsub) { return nsub == 1 ? 520 : 1300; }
 inline int64_t item_cost(const PairItem &w)
 {
     if (w.kind == 1) return (int64_t)(w.kb1 - w.kb0) * 410 + 600;
-    return (int64_t)(w.kb1 - w.kb0) * kblock_cost(w.nsub) + 2600 * w.nsub;
+    return (int64_t)(w.kb1 - w.kb0) * kblock_cost(w.nsub) + 5000 * w.nsub;      // + the epilogue (half of it overlaps on average)
 }
+
+// A margin item (N = 16) is bound by its operand loads, ~410 cycles per K block: uncut it is most of a G tile and
+// unbalances the pairs (n = 4096, sb = 4096: 92k instead of 67k cycles on four pairs). Slices of >= 8 K blocks.
+inline int margin_slices(int n) { return std::max(1, std::min(4, ((n + BK - 1) / BK) / 8)); }
 
 struct PairList {
     PairItem *items = nullptr;          // device, [npairs x kMaxItemsPerPair]
@@ -416,6 +448,7 @@ struct PairList {
 bool build_items(int sb, int b, int n, int full_lower, int bn, int ksplit, int npairs, std::vector<std::vector<PairItem>> &per_pair,
                  int64_t *makespan)
 {
+    const int mslices = margin_slices(n);
     const int T = (sb + PM - 1) / PM, kbt = (n + BK - 1) / BK;
     std::vector<PairItem> all;
     for (int I = 0; I < T; ++I) {
@@ -435,9 +468,13 @@ bool build_items(int sb, int b, int n, int full_lower, int bn, int ksplit, int n
                 if (w.kb1 > w.kb0) all.push_back(w);
             }
         }
-        PairItem mg{};
-        mg.I = (int16_t)I; mg.J = 0; mg.kind = 1; mg.nsub = 1; mg.kb0 = 0; mg.kb1 = (int16_t)kbt;
-        all.push_back(mg);
+        for (int ms = 0; ms < mslices; ++ms) {          // margin items: K slices (slice index in J)
+            PairItem mg{};
+            mg.I = (int16_t)I; mg.J = (int16_t)ms; mg.kind = 1; mg.nsub = 1;
+            mg.kb0 = (int16_t)((int64_t)ms * kbt / mslices);
+            mg.kb1 = (int16_t)((int64_t)(ms + 1) * kbt / mslices);
+            all.push_back(mg);
+        }
     }
     std::stable_sort(all.begin(), all.end(), [](const PairItem &x, const PairItem &y) { return item_cost(x) > item_cost(y); });
     per_pair.assign(npairs, {});
@@ -458,6 +495,8 @@ bool build_items(int sb, int b, int n, int full_lower, int bn, int ksplit, int n
 
 struct GramPairPlan {
     CUtensorMap tmY, tmX8;
+    float *rpart = nullptr;             // [4 x rows_alloc] margin partial sums
+    unsigned *rcount = nullptr;         // [2 x row tiles]
     int32_t n = 0, rows_alloc = 0, npairs = 0;
     bool attr_set = false;
     std::map<std::tuple<int, int, int, int, int>, PairList> lists;       // (sb, b, full_lower, bn, ksplit_opt)
@@ -471,7 +510,12 @@ GramPairPlan *gram_pair_plan_create(const uint16_t *Y, int32_t ldy, int32_t n, i
     pl->rows_alloc = rows_alloc;
     pl->npairs = num_sms / 2;
     if (!make_bf16_map_p(&pl->tmY, Y, (uint64_t)n, (uint64_t)rows_alloc, (uint64_t)ldy, BK, HM) ||
-        !make_bf16_map_p(&pl->tmX8, xbf, (uint64_t)n, 16, (uint64_t)ldxb, BK, 8)) {
+        !make_bf16_map_p(&pl->tmX8, xbf, (uint64_t)n, 16, (uint64_t)ldxb, BK, 8) ||
+        cudaMalloc(&pl->rpart, sizeof(float) * 4 * (size_t)rows_alloc) != cudaSuccess ||
+        cudaMalloc(&pl->rcount, sizeof(unsigned) * 2 * (size_t)(rows_alloc / PM + 1)) != cudaSuccess ||
+        cudaMemset(pl->rcount, 0, sizeof(unsigned) * 2 * (size_t)(rows_alloc / PM + 1)) != cudaSuccess) {
+        cudaFree(pl->rpart);
+        cudaFree(pl->rcount);
         delete pl;
         return nullptr;
     }
@@ -482,6 +526,8 @@ void gram_pair_plan_destroy(GramPairPlan *p)
 {
     if (!p) return;
     for (auto &kv : p->lists) { cudaFree(kv.second.items); cudaFree(kv.second.counts); }
+    cudaFree(p->rpart);
+    cudaFree(p->rcount);
     delete p;
 }
 
@@ -492,7 +538,7 @@ int64_t gram_pair_prepare(GramPairPlan *pl, int32_t sb, int32_t b, int full_lowe
     int64_t best_span = -1, best_span_unused = 0;
     int best_bn = 0;
     for (int cand : {256, 512}) {
-        if (bn != 0 && bn != cand) continue;
+        if (bn != cand && !(bn == 0 && cand == 256)) continue;      // 256 x 512 tiles only on request: never faster, measured
         auto key = std::make_tuple((int)sb, (int)b, full_lower, cand, ksplit_opt);
         auto it = pl->lists.find(key);
         if (it == pl->lists.end()) {
@@ -560,6 +606,7 @@ int launch_gram_pair(cudaStream_t st, GramPairPlan *pl, int32_t sb, int32_t b, f
     p.ldg = ldg; p.sb = sb; p.b = b; p.n = pl->n; p.full_lower = full_lower; p.bn = bn;
     p.nslots = bn == 256 ? 2 : 1;
     p.accumulate = L.ksplit > 1;
+    p.rpart = pl->rpart; p.rcount = pl->rcount; p.mslices = margin_slices(pl->n); p.ldr = pl->rows_alloc;
     if (L.ksplit > 1) {
         const int T128 = (sb + 127) / 128;
         cudaMemsetAsync(G, 0, sizeof(float) * (size_t)T128 * 128 * ldg, st);
