@@ -279,6 +279,14 @@ def time_steps(binding, cg, idx_d, x, s, b, eta, n_steps, stream):
     return e0.elapsed_time(e1)
 
 
+def prime_graphs(cg, cfg, seed, s, sb):
+    """Make the library capture and instantiate every graph length it replays (64 + 8 + 1 steps), on a scratch x."""
+    idx_p = torch.from_numpy(step_indices(cfg, seed, 73, sb)).cuda()
+    cg.outer_steps(idx_p, torch.zeros(cfg.n, device="cuda"), s, cfg.b, cfg.eta, n_steps=73)
+    cg.sync()
+    cg.invalidate_shadow()
+
+
 def main_ours(args, cfg, s):
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
@@ -309,6 +317,9 @@ def main_ours(args, cfg, s):
     x = torch.zeros(cfg.n, device="cuda")
     torch.cuda.synchronize()
 
+    # ---- graph instantiation is not a step: casgd_outer_steps captures its 64 / 8 / 1-step CUDA graphs on first use,
+    # so run 73 steps on a scratch iterate first (untimed, x untouched), then the W warm-up steps proper
+    prime_graphs(cg, cfg, seed, s, sb)
     # ---- warm-up, then the timed region: K outer steps, device-resident inputs
     cg.outer_steps(idx_d[: W * sb], x, s, cfg.b, cfg.eta, n_steps=W)
     cg.sync()
@@ -415,6 +426,7 @@ def main_ours(args, cfg, s):
             sb2 = s2 * cfg.b
             k2 = max(20, min(2000, (K * sb) // sb2))
             idx2 = torch.from_numpy(step_indices(cfg, seed, k2 + 5, sb2)).cuda()
+            prime_graphs(cg, cfg, seed, s2, sb2)
             x2 = torch.zeros(cfg.n, device="cuda")
             cg.outer_steps(idx2[: 5 * sb2], x2, s2, cfg.b, cfg.eta, n_steps=5)
             ms2 = time_steps(binding, cg, idx2[5 * sb2:], x2, s2, cfg.b, cfg.eta, k2, stream)
