@@ -60,6 +60,19 @@ def test_one_outer_step_matches_the_oracle(binding, oracle_mod, ci, m, n, s, b, 
             check_step_against_oracle(oracle_mod, cg, A_bits, y, idx, x0, s, b, cfg.eta, cfg.loss, binding)
 
 
+@pytest.mark.parametrize("ci,m,n,s,b", [(0, 8192, 64, 4, 16), (1, 20000, 18, 5, 64), (4, 6000, 512, 1, 64), (4, 6000, 512, 6, 64)])
+def test_unfused_kernels_match_the_oracle(binding, oracle_mod, ci, m, n, s, b):
+    """CASGD_OPT_NO_FUSED_UPDATE: the outer update as its own kernel after the recurrence, and at s = 1 the margin through
+    the Gram kernel followed by the recurrence kernel -- the paths the fused kernels replace by default."""
+    cfg = synth.config(ci, m=m, n=n)
+    X_d, y_d, A_bits, y = device_dataset(cfg)
+    eta = cfg.eta if cfg.loss != synth.POISSON else 0.01
+    with binding.Casgd(X_d, y_d, cfg.loss) as cg:
+        cg.set_option(binding.OPT_NO_FUSED_UPDATE, 1)
+        idx = synth.iid_indices(m, s * b, 77)
+        check_step_against_oracle(oracle_mod, cg, A_bits, y, idx, random_x(n, 5, 0.2), s, b, eta, cfg.loss, binding)
+
+
 # shapes that span several 256-row pair tiles with a ragged tail, for the cta_group::2 Gram kernel
 PAIR_SHAPES = [
     (4, 6000, 512, 9, 128),      # sb = 1152 = 4.5 pair tiles; b = 128: the block diagonal cuts every diagonal tile
