@@ -466,14 +466,22 @@ recurrence_stream_kernel(const float *G, int32_t ldg, const float *r,
                     acc[6] = fmaf(bf16lo(v.w), uu, acc[6]); acc[7] = fmaf(bf16hi(v.w), uu, acc[7]);
                 }
             }
+            // rows first meet inside a warp (lanes CV apart hold the same columns), then the 16 warps' sums in shared
+            // memory: a serial sum over all RL row lanes by CV * 8 threads was half of this tail
+            for (int o = CV; o < 32; o <<= 1)
 #pragma unroll
-            for (int e = 0; e < 8; ++e) red[rl * (CV * 8) + cvl * 8 + e] = acc[e];
+                for (int e = 0; e < 8; ++e) acc[e] += __shfl_xor_sync(0xffffffffu, acc[e], o);
+            const int groups = CV <= 32 ? kWarps : RL, gidx = CV <= 32 ? warp : rl;
+            if (CV > 32 || lane < CV) {
+#pragma unroll
+                for (int e = 0; e < 8; ++e) red[gidx * (CV * 8) + cvl * 8 + e] = acc[e];
+            }
             __syncthreads();
             // column sums of this CTA, in a fixed order, straight into CTA 0's gbuf[crank][col]
             const uint32_t gbuf0 = mapa_u32((uint32_t)__cvta_generic_to_shared(gbuf), 0u);
             for (int t = threadIdx.x; t < CV * 8; t += kThreads) {
                 float sum = 0.f;
-                for (int q = 0; q < RL; ++q) sum += red[q * (CV * 8) + t];
+                for (int q = 0; q < groups; ++q) sum += red[q * (CV * 8) + t];
                 const int col = cv0 * 8 + t;
                 if (col < ldy)
                     asm volatile("st.shared::cluster.f32 [%0], %1;" ::"r"(gbuf0 + 4u * (uint32_t)(crank * ldy + col)), "f"(sum) : "memory");
