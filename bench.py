@@ -337,6 +337,19 @@ def main_ours(args, cfg, s):
     cg.sync()
     F_after = cg.loss(x)
 
+    # ---- the same K steps with the indices drawn on the device (Alg. 1 line 1 as the paper states it: i.i.d. with
+    # replacement, Philox4x32-10; casgd_outer_steps_sampled) -- no index buffer at all
+    xs_ = torch.zeros(cfg.n, device="cuda")
+    cg.outer_steps_sampled(xs_, s, cfg.b, cfg.eta, n_steps=W, seed=seed, first_step=0)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    with torch.cuda.stream(stream):
+        e0.record(stream)
+        cg.outer_steps_sampled(xs_, s, cfg.b, cfg.eta, n_steps=K, seed=seed, first_step=W)
+        e1.record(stream)
+    stream.synchronize()
+    sampled_ms, = max_over_ranks([e0.elapsed_time(e1)], dist, "cuda")
+    cg.invalidate_shadow()
+
     # ---- end to end through the C ABI with HOST buffers: every step copies its indices and x in, x out
     idx_h = torch.from_numpy(idx_np[W * sb:]).pin_memory()
     x_h = torch.zeros(cfg.n).pin_memory()
@@ -448,7 +461,10 @@ def main_ours(args, cfg, s):
                          d2h_bytes_per_step=cfg.n * 4, steps=Ke,
                          batched64=dict(value=aggregate_rows_per_s(world, Ke, sb, e2e64_s * 1e3), h2d_bytes_per_step=sb * 4 + cfg.n * 4 / 64,
                                         d2h_bytes_per_step=cfg.n * 4 / 64)),
-                gpu_launches=int(launches), roofline=roofline, stages=stages, gemv=gemv, sweep=sweep)
+                gpu_launches=int(launches),
+                sampled_on_device=dict(value=aggregate_rows_per_s(world, K, sb, sampled_ms), unit=UNIT, ms_per_step=sampled_ms / K,
+                                       sampler="Philox4x32-10, i.i.d. with replacement (PAPER.md:L111)"),
+                roofline=roofline, stages=stages, gemv=gemv, sweep=sweep)
 
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         v, steps_o, t_o, cores = oracle_rows_per_s(cfg, s, ds.X_bf16, ds.y, idx_np, seed)

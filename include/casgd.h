@@ -92,6 +92,15 @@ int casgd_outer_step(casgd_ctx *c, const int32_t *idx, float *x, int32_t s, int3
 int casgd_outer_steps(casgd_ctx *c, const int32_t *idx, int64_t n_steps, float *x, int32_t s, int32_t b,
                       float eta);
 
+/* n_steps outer iterations whose row indices are drawn ON THE DEVICE, i.i.d. uniformly with replacement as in
+ * Alg. 1 line 1 -- no index upload. Counter-based: the indices of a step depend only on
+ * (seed, step number, position), step h of this call being number first_step + h:
+ *   index t:  counter = (t / 4, step mod 2^32, step div 2^32, 0xCA5D), key = (seed mod 2^32, seed div 2^32),
+ *             w = Philox4x32-10(counter, key)[t mod 4],  idx = floor(w * m / 2^32)        (needs m < 2^32)
+ * (Salmon et al., SC'11). Otherwise exactly casgd_outer_steps on those indices. ASYNCHRONOUS. */
+int casgd_outer_steps_sampled(casgd_ctx *c, int64_t n_steps, float *x, int32_t s, int32_t b, float eta, uint64_t seed,
+                              uint64_t first_step);
+
 /* The same through HOST buffers: copies idx_host (n_steps*s*b int32) and x_host (n FP32) to the
  * device, runs the steps, copies x back into x_host, and synchronises. Pinned host memory makes the
  * copies asynchronous with respect to the host but the call still returns only when x_host is valid. */

@@ -228,3 +228,47 @@ def gram_entries(A_bits, idx, pairs):
                                     _p(idx, ctypes.c_int32), idx.shape[0], _p(pairs, ctypes.c_int64),
                                     pairs.shape[0], _p(out, ctypes.c_double), _p(norms, ctypes.c_double)))
     return out, norms
+
+
+# ---------------------------------------------------------------- index sampling (Alg. 1 line 1) ---
+# The paper samples the s*b row indices of an outer step i.i.d. uniformly WITH replacement (PAPER.md:L111-L112,
+# L59). For the on-device sampler (include/casgd.h: casgd_outer_steps_sampled) both sides implement the same
+# counter-based generator, Philox4x32-10 (Salmon, Moraes, Dror, Shaw: "Parallel random numbers: as easy as 1, 2, 3",
+# SC'11), written here from the paper's definition in plain numpy integer arithmetic:
+#   index t of outer step h:  counter = (t // 4, h mod 2^32, h div 2^32, 0xCA5D), key = (seed mod 2^32, seed div 2^32),
+#   w = Philox4x32-10(counter, key)[t mod 4],  idx = floor(w * m / 2^32)     (multiply-shift: bias < m / 2^32)
+_PHILOX_M0, _PHILOX_M1 = np.uint64(0xD2511F53), np.uint64(0xCD9E8D57)
+_PHILOX_W0, _PHILOX_W1 = 0x9E3779B9, 0xBB67AE85
+_MASK32 = np.uint64(0xFFFFFFFF)
+SAMPLING_DOMAIN = 0xCA5D
+
+
+def philox4x32_10(counter, key):
+    """Philox4x32 with 10 rounds. counter: [..., 4] and key: [..., 2] arrays of values < 2^32; returns uint32 [..., 4]."""
+    c = np.asarray(counter, dtype=np.uint64) & _MASK32
+    k = np.asarray(key, dtype=np.uint64) & _MASK32
+    c0, c1, c2, c3 = (c[..., i].copy() for i in range(4))
+    k0, k1 = k[..., 0].copy(), k[..., 1].copy()
+    for _ in range(10):
+        p0 = _PHILOX_M0 * c0                      # 32 x 32 -> 64 bit products
+        p1 = _PHILOX_M1 * c2
+        hi0, lo0 = p0 >> np.uint64(32), p0 & _MASK32
+        hi1, lo1 = p1 >> np.uint64(32), p1 & _MASK32
+        c0, c1, c2, c3 = hi1 ^ c1 ^ k0, lo1, hi0 ^ c3 ^ k1, lo0
+        k0 = (k0 + np.uint64(_PHILOX_W0)) & _MASK32
+        k1 = (k1 + np.uint64(_PHILOX_W1)) & _MASK32
+    return np.stack([c0, c1, c2, c3], axis=-1).astype(np.uint32)
+
+
+def sample_indices(seed: int, step: int, sb: int, m: int) -> np.ndarray:
+    """The s*b row indices of outer step `step` under `seed`: i.i.d. uniform on [0, m), with replacement. int32 [sb]."""
+    t = np.arange(sb, dtype=np.uint64)
+    nblk = (sb + 3) // 4
+    ctr = np.zeros((nblk, 4), dtype=np.uint64)
+    ctr[:, 0] = np.arange(nblk, dtype=np.uint64)
+    ctr[:, 1] = step & 0xFFFFFFFF
+    ctr[:, 2] = (step >> 32) & 0xFFFFFFFF
+    ctr[:, 3] = SAMPLING_DOMAIN
+    key = np.array([seed & 0xFFFFFFFF, (seed >> 32) & 0xFFFFFFFF], dtype=np.uint64)
+    w = philox4x32_10(ctr, np.broadcast_to(key, (nblk, 2))).reshape(-1)[:sb].astype(np.uint64)
+    return ((w * np.uint64(m)) >> np.uint64(32)).astype(np.int32)

@@ -26,7 +26,8 @@ MAX_SB = 16384
 
 # every symbol include/casgd.h declares
 EXPORTS = (
-    "casgd_init", "casgd_outer_step", "casgd_outer_steps", "casgd_outer_steps_host", "casgd_sgd_step_fp32",
+    "casgd_init", "casgd_outer_step", "casgd_outer_steps", "casgd_outer_steps_sampled", "casgd_outer_steps_host",
+    "casgd_sgd_step_fp32",
     "casgd_sgd_steps_fp32", "casgd_loss", "casgd_invalidate_shadow", "casgd_sync", "casgd_debug_export",
     "casgd_set_option", "casgd_stage_times", "casgd_launch_count", "casgd_last_error", "casgd_destroy",
     "casgd_version",
@@ -59,6 +60,8 @@ def load() -> ctypes.CDLL:
     lib.casgd_outer_step.argtypes = [vp, vp, vp, i32, i32, f32]
     lib.casgd_outer_steps.restype = ctypes.c_int
     lib.casgd_outer_steps.argtypes = [vp, vp, i64, vp, i32, i32, f32]
+    lib.casgd_outer_steps_sampled.restype = ctypes.c_int
+    lib.casgd_outer_steps_sampled.argtypes = [vp, i64, vp, i32, i32, f32, ctypes.c_uint64, ctypes.c_uint64]
     lib.casgd_outer_steps_host.restype = ctypes.c_int
     lib.casgd_outer_steps_host.argtypes = [vp, vp, i64, vp, i32, i32, f32]
     lib.casgd_sgd_step_fp32.restype = ctypes.c_int
@@ -160,6 +163,13 @@ class Casgd:
             n_steps = idx.numel() // (s * b)
         assert idx.numel() >= n_steps * s * b
         self._check(self._lib.casgd_outer_steps(self._ctx, _dev_ptr(idx), n_steps, _dev_ptr(x), s, b, eta))
+        if n_steps:
+            self._last_sb = s * b
+
+    def outer_steps_sampled(self, x: torch.Tensor, s: int, b: int, eta: float, n_steps: int, seed: int, first_step: int = 0):
+        """casgd_outer_steps_sampled: indices drawn on the device (Philox4x32-10, with replacement)."""
+        assert x.dtype == torch.float32 and x.numel() == self.n
+        self._check(self._lib.casgd_outer_steps_sampled(self._ctx, n_steps, _dev_ptr(x), s, b, eta, seed, first_step))
         if n_steps:
             self._last_sb = s * b
 

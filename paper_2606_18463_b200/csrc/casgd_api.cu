@@ -502,6 +502,26 @@ int casgd_outer_steps_host(casgd_ctx *c, const int32_t *idx_host, int64_t n_step
     return CASGD_OK;
 }
 
+int casgd_outer_steps_sampled(casgd_ctx *c, int64_t n_steps, float *x, int32_t s, int32_t b, float eta, uint64_t seed,
+                              uint64_t first_step)
+{
+    int dummy = 0;
+    int rc = check_step_args(c, &dummy, x, n_steps, s, b, eta);
+    if (rc) return rc;
+    if (c->m >= (1ll << 32)) return fail(c, CASGD_EINVAL, "the on-device sampler needs m < 2^32");
+    const int64_t count = n_steps * s * b;
+    if (count > c->idx_stage_cap) {
+        CK(cudaStreamSynchronize(c->stream));
+        cudaFree(c->idx_stage);
+        c->idx_stage = nullptr;
+        c->idx_stage_cap = 0;
+        CK(cudaMalloc(&c->idx_stage, sizeof(int32_t) * (size_t)count));
+        c->idx_stage_cap = count;
+    }
+    if (count > 0) c->launches += launch_sample_indices(c->stream, c->idx_stage, n_steps, s * b, c->m, seed, first_step);
+    return run_steps(c, c->idx_stage, n_steps, x, s, b, eta, true);
+}
+
 int casgd_sgd_steps_fp32(casgd_ctx *c, const int32_t *idx, int64_t n_steps, float *x, int32_t b, float eta)
 {
     int rc = check_step_args(c, idx, x, n_steps, 1, b, eta);

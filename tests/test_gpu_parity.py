@@ -335,6 +335,39 @@ def test_graph_replay_and_host_entry_point_equal_single_steps(binding):
         assert torch.equal(xa.cpu(), x1)
 
 
+@pytest.mark.parametrize("ci,m,n,s,b", [(1, 20000, 18, 5, 64), (4, 6000, 512, 3, 64), (0, 4097, 64, 7, 13)])
+def test_on_device_sampling_matches_the_oracle_sampler(binding, oracle_mod, ci, m, n, s, b):
+    """casgd_outer_steps_sampled draws Alg. 1 line 1's indices on the device (Philox4x32-10, with replacement): the rows it
+    gathers are exactly A[oracle.sample_indices(...)], and the iterate equals casgd_outer_steps on those indices bit
+    for bit; step numbers continue across calls (first_step)."""
+    cfg = synth.config(ci, m=m, n=n)
+    X_d, y_d, A_bits, y = device_dataset(cfg)
+    seed, steps, sb = 0xC0FFEE1234, 11, s * b
+    idx = np.concatenate([oracle_mod.sample_indices(seed, h, sb, m) for h in range(steps)])
+    assert len(np.unique(idx)) < len(idx) or m > 50 * len(idx)             # with replacement
+    eta = cfg.eta if cfg.loss != synth.POISSON else 0.01
+    with binding.Casgd(X_d, y_d, cfg.loss) as cg:
+        xa = torch.zeros(n, device="cuda")
+        cg.outer_steps(torch.from_numpy(idx).cuda(), xa, s, b, eta)
+        cg.sync()
+        xb = torch.zeros(n, device="cuda")
+        cg.outer_steps_sampled(xb, s, b, eta, n_steps=4, seed=seed, first_step=0)
+        cg.outer_steps_sampled(xb, s, b, eta, n_steps=steps - 4, seed=seed, first_step=4)
+        cg.sync()
+        assert torch.equal(xa, xb)
+        assert np.array_equal(cg.debug(binding.DBG_Y), A_bits[idx[-sb:]])   # the last step's gathered rows
+        # and one sampled step against the oracle itself
+        x0 = random_x(n, 9, 0.2)
+        xc = torch.from_numpy(x0.copy()).cuda()
+        cg.invalidate_shadow()
+        cg.outer_steps_sampled(xc, s, b, eta, n_steps=1, seed=seed, first_step=(1 << 40) + 3)
+        cg.sync()
+        idx1 = oracle_mod.sample_indices(seed, (1 << 40) + 3, sb, m)
+        ref = oracle_mod.outer_step_gram(A_bits, y, idx1, x0.astype(np.float64), s, b, eta, cfg.loss, shadow=True)
+        from gpu_common import compare_last_step
+        compare_last_step(oracle_mod, cg, ref, y[idx1], x0, xc, s, b, eta, cfg.loss, binding)
+
+
 def _train_gpu(binding, cg, cfg, idx, s):
     x = torch.zeros(cfg.n, device="cuda")
     cg.invalidate_shadow()
