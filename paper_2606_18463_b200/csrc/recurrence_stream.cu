@@ -124,7 +124,8 @@ struct StreamLayout {                   // byte offsets into dynamic shared memo
     uint32_t u, ubar, pbar, part, cring, bring, total;
 };
 
-__host__ __device__ inline StreamLayout stream_layout(int s, int b)
+// qmax = row groups of a block per CTA at most (1 or 2): the rings are sized for it, so that s*b = 16384 still fits
+__host__ __device__ inline StreamLayout stream_layout(int s, int b, int qmax)
 {
     StreamLayout L;
     uint32_t o = 0;
@@ -133,10 +134,10 @@ __host__ __device__ inline StreamLayout stream_layout(int s, int b)
     L.ubar = o;   o += 8u * (uint32_t)s;
     L.pbar = o;   o += 8u * (uint32_t)s;
     o = (o + 15u) & ~15u;
-    L.part = o;   o += 16u * (uint32_t)(kPartDepth * kMaxQuadsPerCta);                  // [step % depth][quad][4 rows]
+    L.part = o;   o += 16u * (uint32_t)(kPartDepth * qmax);                             // [step % depth][quad][4 rows]
     o = (o + 127u) & ~127u;
-    L.cring = o;  o += (uint32_t)(kCritPer * kMaxQuadsPerCta * kCritDepth * kWin) * kUnitBytes;
-    L.bring = o;  o += (uint32_t)(kBulkWarps * kDepth) * kUnitBytes;
+    L.cring = o;  o += (uint32_t)(kCritPer * qmax * kCritDepth * kWin) * kUnitBytes;
+    L.bring = o;  o += (uint32_t)((qmax == 1 ? 12 : 10) * kDepth) * kUnitBytes;         // one ring per bulk warp
     L.total = o;
     return L;
 }
@@ -196,7 +197,8 @@ recurrence_stream_kernel(const float *G, int32_t ldg, const float *r,
     const int C = (int)cluster_nctarank(), crank = (int)cluster_ctarank();
     pdl_trigger();
     REC_TRACE(0);
-    const StreamLayout L = stream_layout(s, b);
+    const int qmax = (b / kQuad + C - 1) / C;           // row groups of a block per CTA at most
+    const StreamLayout L = stream_layout(s, b, qmax);
     const uint32_t base = (uint32_t)__cvta_generic_to_shared(rs_smem);
     const uint32_t us = base + L.u, ubar = base + L.ubar, pbar = base + L.pbar, part = base + L.part;
 
@@ -207,7 +209,7 @@ recurrence_stream_kernel(const float *G, int32_t ldg, const float *r,
     const int bshift = (b & (b - 1)) == 0 ? __ffs(b) - 1 : -1;             // b a power of two: column -> block by shift
     auto block_of = [&](int col) { return bshift >= 0 ? (col >> bshift) : col / b; };
 
-    const int nbulk = qpc == 1 ? 12 : 10;               // 16 warps - 3 critical warps per owned row group, rounded to a multiple of qpc
+    const int nbulk = qmax == 1 ? 12 : 10;              // 16 warps - 3 critical warps per row group, rounded to a multiple of qmax
     for (int k = threadIdx.x; k < s; k += kThreads) {
         mbar_init(ubar + 8u * k, 1);
         mbar_expect_tx(ubar + 8u * k, 4u * (uint32_t)b);
@@ -299,7 +301,7 @@ recurrence_stream_kernel(const float *G, int32_t ldg, const float *r,
                     float p = 0.f;                      // lane 8 li carries row li's partial sum into the reduction
                     if ((lane & 7) == 0)
                         asm volatile("ld.shared.f32 %0, [%1];" : "=f"(p)
-                                     : "r"(part + 16u * (uint32_t)((j % kPartDepth) * kMaxQuadsPerCta + gamma) + 4u * (uint32_t)li));
+                                     : "r"(part + 16u * (uint32_t)((j % kPartDepth) * qmax + gamma) + 4u * (uint32_t)li));
 #pragma unroll
                     for (int i = 0; i < kQuad; ++i) acc[i] = (i == li) ? p : 0.f;
                 }
@@ -426,7 +428,7 @@ recurrence_stream_kernel(const float *G, int32_t ldg, const float *r,
             const float tot = quad_reduce(acc, lane);
             if ((lane & 7) == 0)
                 asm volatile("st.shared.f32 [%0], %1;"
-                             ::"r"(part + 16u * (uint32_t)((j % kPartDepth) * kMaxQuadsPerCta + gamma) + 4u * (uint32_t)li), "f"(tot) : "memory");
+                             ::"r"(part + 16u * (uint32_t)((j % kPartDepth) * qmax + gamma) + 4u * (uint32_t)li), "f"(tot) : "memory");
             __syncwarp();
             if (lane == 0) mbar_arrive(pbar + 8u * j);
             REC_TRACE_B(6001 + 4 * j);
@@ -507,7 +509,9 @@ recurrence_stream_kernel(const float *G, int32_t ldg, const float *r,
     REC_TRACE(3);
 }
 
-int stream_smem_bytes(int s, int b)
+int stream_cluster_for(int b, int cluster_max);
+
+int stream_smem_bytes(int s, int b, int cluster_max)
 {
     static int max_optin = -1;
     if (max_optin < 0) {
@@ -515,7 +519,8 @@ int stream_smem_bytes(int s, int b)
         cudaGetDevice(&dev);
         if (cudaDeviceGetAttribute(&max_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev) != cudaSuccess) max_optin = 0;
     }
-    const int need = (int)stream_layout(s, b).total;
+    const int c = stream_cluster_for(b, cluster_max);
+    const int need = (int)stream_layout(s, b, (b / kQuad + c - 1) / c).total;
     return need <= max_optin ? need : 0;
 }
 
@@ -533,7 +538,7 @@ cudaError_t launch_stream(cudaStream_t st, const float *G, int32_t ldg, const fl
                           int32_t b, float alpha, float *z, float *u, int cluster_max, const FusedGrad &fg)
 {
     static bool attr_set = false;
-    const int smem = stream_smem_bytes(s, b);
+    const int smem = stream_smem_bytes(s, b, cluster_max);
     if (smem == 0) return cudaErrorInvalidConfiguration;
     auto kern = recurrence_stream_kernel<LOSS>;
     if (!attr_set) {
@@ -558,7 +563,7 @@ bool recurrence_stream_ok(int32_t s, int32_t b, int32_t ldg, int cluster)
     if (cluster <= 0 || b % 4 != 0 || ldg % 4 != 0 || s < 2) return false;
     const int c = stream_cluster_for(b, cluster);
     if ((b / kQuad + c - 1) / c > kMaxQuadsPerCta) return false;
-    return stream_smem_bytes(s, b) > 0;
+    return stream_smem_bytes(s, b, cluster) > 0;
 }
 
 // Can the streaming kernel also do the outer update of this step (small Y)?
@@ -567,7 +572,9 @@ bool recurrence_stream_fuses_update(int32_t s, int32_t b, int32_t ldy, int clust
     const int cluster = stream_cluster_for(b, cluster_max);
     // measured: worth it while a CTA's slice of Y stays below ~136 KB (poisson-synth s=32: 131 KB per CTA, 32.1 -> 30.4 us;
     // epsilon-shaped s=16 on 8 CTAs: 256 KB per CTA, 34.7 -> 36.9 us)
-    return ldy <= kFgMaxLdy && (int64_t)s * b * ldy * 2 <= (int64_t)136 * 1024 * cluster;
+    const StreamLayout L = stream_layout(s, b, (b / kQuad + cluster - 1) / cluster);
+    const int64_t buffers = (int64_t)kThreads * 8 * 4 + (int64_t)cluster * ldy * 4;      // red + CTA 0's gbuf, over the rings
+    return ldy <= kFgMaxLdy && (int64_t)s * b * ldy * 2 <= (int64_t)136 * 1024 * cluster && buffers <= (int64_t)(L.total - L.cring);
 }
 
 int launch_recurrence_stream(cudaStream_t st, const float *G, int32_t ldg, const float *r, const float *yI, int32_t s,
