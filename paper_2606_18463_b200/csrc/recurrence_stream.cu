@@ -9,18 +9,21 @@
 //   (b) every warp streams its own part of G from L2 into a private shared-memory ring with 16-byte cp.async
 //       (LDGSTS: each lane copies, and later reads back, its own 16 bytes, so the ring needs no barrier --
 //       cp.async.wait_group is the only synchronisation), kDepth 512-byte chunks ahead of use and independent
-//       of the chain. 8 warps x kDepth 2 KB units in flight keep one SM's L2 port busy (measured: plain 16-byte
-//       loads from 16 warps reach ~80 B/cycle/SM, a single-thread cp.async.bulk producer only 1-25).
+//       of the chain (measured: plain 16-byte loads from 16 warps reach ~80 B/cycle/SM, a single-thread
+//       cp.async.bulk producer only 1-25).
 // Rows: each block's rows are dealt to the CTAs in groups of 4 consecutive rows (group q -> CTA q mod C), so the
 // four u values of a group leave as ONE 16-byte st.async per destination CTA (measured: a hop with 4-byte stores
-// costs 850 cycles in a 16-CTA cluster, with 16-byte stores 540). Work of one CTA at step j:
-//   bulk warps (8)  every 128-column chunk of its rows but the last: these columns belong to blocks <= j-2
-//                   (whenever b divides 128 or 128 divides b), whose u landed a hop earlier -- so this runs one
-//                   hop ahead; per-row partial sums go to shared memory + an mbarrier per step;
-//   critical warps  two per owned group, taking alternate steps: the last chunk (which holds block j-1), the
-//                   bulk partials, one 5-level shuffle reduction for the 4 rows, l', and the broadcast of u.
-//                   They sit on SM sub-partitions of their own (warp id mod 4), away from the bulk warps.
-// The strict block-lower G is read exactly once (L180). Needs b % 4 == 0 and at most 4 groups per CTA.
+// costs 850 cycles in a 16-CTA cluster, with 16-byte stores 540). Work of one CTA:
+//   critical warps  three per owned group, taking every third step: the newest kWin = 2 chunks of the step's rows
+//                   (the last one holds block j-1), the bulk partial, one 5-level shuffle reduction for the 4 rows,
+//                   l', and the broadcast of u;
+//   bulk warps      every other warp (12, or 10 when the CTA owns two groups), each taking WHOLE steps in turn: all
+//                   older 128-column chunks of the step's rows -- blocks <= j-2, whose u landed a hop or more
+//                   earlier, so a bulk warp runs ahead of the chain -- then one reduction and one hand-over per
+//                   step through shared memory + an mbarrier. Their issue rate, not L2, bounded the late steps:
+//                   hence running pointers, whole steps per warp and all four schedulers.
+// The strict block-lower G is read exactly once (L180). Needs b % 4 == 0 and at most 2 groups per CTA (b <= 128
+// with 16 CTAs). For small steps the same cluster then applies the outer update (Alg. 1 lines 16-17): see FusedGrad.
 #include "common.cuh"
 
 namespace casgd {
@@ -36,9 +39,9 @@ constexpr int kChunk = 128;                             // columns per chunk
 constexpr uint32_t kUnitBytes = kQuad * kChunk * 4u;    // one unit: 4 rows x 128 columns of G = 2 KB
 constexpr int kWin = 2;                                 // chunks of a step the critical warps take: the newest 256 columns
 constexpr int kCritPer = 3;                             // critical warps per row group, taking every third step
-constexpr int kDepth = 4;                               // bulk warp: units in flight (64 KB per CTA)
+constexpr int kDepth = 4;                               // bulk warp: units of its ring (3 in flight)
 constexpr int kCritDepth = 3;                           // critical warp: steps in flight (kWin units each)
-constexpr int kPartDepth = 40;                          // steps of partial sums kept (bulk runs < 128/b + 3 steps ahead)
+constexpr int kPartDepth = 40;                          // steps of partial sums kept (a bulk warp finishes step j only after u_{j-3} landed)
 
 __device__ __forceinline__ uint32_t cluster_ctarank()
 {
