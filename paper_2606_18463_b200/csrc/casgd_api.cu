@@ -258,8 +258,9 @@ int choose_gram(casgd_ctx *c, int32_t s, int32_t b)
     const int64_t opt = c->opt_gram_impl;
     c->cur_gram = opt == 1 ? 1 : 2;
     c->cur_bn = 0;
-    // gather + Gram in one kernel: wins while the tiles fit in about half a wave (measured: sb = 2048 is 4 us slower)
-    if ((opt == 5 || (opt == 0 && sb <= 1280)) && c->n <= 64) { c->cur_gram = 4; return CASGD_OK; }
+    // gather + Gram in one kernel: wins while the tiles fit in about half a wave (measured at n = 18, b = 64: sb = 1536
+    // 20.7 against 21.8 us per step, sb = 2048 29.8 against 25.7 us)
+    if ((opt == 5 || (opt == 0 && sb <= 1536)) && c->n <= 64) { c->cur_gram = 4; return CASGD_OK; }
     if (opt == 5) return fail(c, CASGD_EINVAL, "the fused gather + Gram kernel needs n <= 64");
     if (opt == 1 || opt == 2 || c->num_sms < 2) return CASGD_OK;
     if (opt == 0 && (sb < 512 || c->n < 256)) return CASGD_OK;      // too little work for 256-row tiles
