@@ -66,6 +66,7 @@ typedef enum {
  *           (16-byte aligned base, ldx % 8 == 0); otherwise (e.g. n = 18, ldx = 18) the outer steps work on
  *           the library's own zero-padded copy, made during this call, and casgd_loss still streams the
  *           caller's (narrower) rows.
+ *   m       rows, 1 <= m < 2^31 (every index buffer of this ABI is int32); n >= 1 columns.
  *   y       m FP32 labels (Table 1: labels are FP32 throughout). BORROWED.
  *   loss    a casgd_loss_kind.
  *   cuda_stream  a cudaStream_t (NULL = the legacy default stream). All work of this context is
@@ -80,10 +81,10 @@ int casgd_init(casgd_ctx **out, const uint16_t *X_bf16, int64_t ldx, const float
  *        accepted (the paper samples with replacement, L111). An out-of-range index makes that
  *        row read as zeros with label 0 and raises the sticky CASGD_EINDEX flag.
  *   x    n FP32 master weights, updated in place: x <- x - (eta/b) Y^T u.
- * The BF16 shadow of x used by the margin (L231) is owned by the context. It is rebuilt from `x`
- * when the context has no valid shadow for this `x` pointer (first call, pointer change, after
- * casgd_sgd_step_fp32 or casgd_invalidate_shadow) and otherwise kept current by the fused update;
- * a caller that modifies x between calls must call casgd_invalidate_shadow. */
+ * The BF16 shadow of x used by the margin (L231) is owned by the context. It is rebuilt from `x` at
+ * the start of every casgd_outer_step / casgd_outer_steps* call (one n-element kernel per call) and kept
+ * current by the fused update between the steps of a call, so a caller may change x, or pass another
+ * x, between calls freely. */
 int casgd_outer_step(casgd_ctx *c, const int32_t *idx, float *x, int32_t s, int32_t b, float eta);
 
 /* n_steps consecutive outer iterations; step h uses idx[h*s*b .. (h+1)*s*b). ASYNCHRONOUS.
@@ -96,7 +97,7 @@ int casgd_outer_steps(casgd_ctx *c, const int32_t *idx, int64_t n_steps, float *
  * Alg. 1 line 1 -- no index upload. Counter-based: the indices of a step depend only on
  * (seed, step number, position), step h of this call being number first_step + h:
  *   index t:  counter = (t / 4, step mod 2^32, step div 2^32, 0xCA5D), key = (seed mod 2^32, seed div 2^32),
- *             w = Philox4x32-10(counter, key)[t mod 4],  idx = floor(w * m / 2^32)        (needs m < 2^32)
+ *             w = Philox4x32-10(counter, key)[t mod 4],  idx = floor(w * m / 2^32)        (m < 2^31 by casgd_init)
  * (Salmon et al., SC'11). Otherwise exactly casgd_outer_steps on those indices. ASYNCHRONOUS. */
 int casgd_outer_steps_sampled(casgd_ctx *c, int64_t n_steps, float *x, int32_t s, int32_t b, float eta, uint64_t seed,
                               uint64_t first_step);
@@ -119,7 +120,7 @@ int casgd_sgd_steps_fp32(casgd_ctx *c, const int32_t *idx, int64_t n_steps, floa
  * Synchronises. */
 int casgd_loss(casgd_ctx *c, const float *x, double *loss_host);
 
-/* Drop the BF16 shadow so the next outer step rebuilds it from x. */
+/* Kept for compatibility: the shadow is rebuilt from x at the start of every outer-step call anyway. */
 int casgd_invalidate_shadow(casgd_ctx *c);
 
 /* Wait for the context's stream; returns CASGD_EINDEX (and clears the flag) if any gather since the
@@ -164,11 +165,18 @@ int casgd_debug_export(casgd_ctx *c, int what, void *dst_host, int64_t dst_bytes
  *   CASGD_OPT_NO_FUSED_UPDATE  1 = the outer update always runs as its own kernel. Default 0: for small steps
  *                              (at most 136 KB of Y per CTA of the cluster, 2048 columns) the streaming recurrence kernel's cluster does
  *                              g = Y^T u, the update of x and the shadow itself, right after the chain.
+ *   CASGD_OPT_STAMPS           1 = every kernel of an outer step records when its first CTA started working (after its
+ *                              programmatic-dependent-launch wait) and when its last CTA finished, in %globaltimer
+ *                              nanoseconds; casgd_stage_times then returns, for the four step stages, the sum over
+ *                              launches of (last end - first start) -- measured INSIDE the CUDA-graph replays that
+ *                              casgd_outer_steps runs (unlike CASGD_OPT_PROFILE, which launches directly). Setting the
+ *                              option (to 0 or 1) clears the totals.
  *   CASGD_OPT_LOSS_IMPL        0 = casgd_loss streams A through per-warp cp.async.bulk shared-memory rings
  *                              (default; n <= 8192), 1 = the plain 16-byte-load kernel. */
 typedef enum {
     CASGD_OPT_GRAM_IMPL = 0, CASGD_OPT_GRAM_FULL_LOWER = 1, CASGD_OPT_PROFILE = 2, CASGD_OPT_NO_GRAPH = 3,
-    CASGD_OPT_GRAM_KSPLIT = 4, CASGD_OPT_RECURRENCE_IMPL = 5, CASGD_OPT_LOSS_IMPL = 6, CASGD_OPT_NO_FUSED_UPDATE = 7
+    CASGD_OPT_GRAM_KSPLIT = 4, CASGD_OPT_RECURRENCE_IMPL = 5, CASGD_OPT_LOSS_IMPL = 6, CASGD_OPT_NO_FUSED_UPDATE = 7,
+    CASGD_OPT_STAMPS = 8
 } casgd_option;
 int casgd_set_option(casgd_ctx *c, int option, int64_t value);
 

@@ -13,6 +13,10 @@
 
 using namespace casgd;
 
+namespace casgd {
+thread_local unsigned long long *g_stamp = nullptr;
+}
+
 namespace {
 
 struct StageEvent {
@@ -78,6 +82,9 @@ struct casgd_ctx {
     // last step, for debug export
     int32_t last_s = 0, last_b = 0;
     // options
+    unsigned long long *stamps = nullptr;     // CASGD_OPT_STAMPS: [kStampSteps * 4][2] slots, then accum_ns[4], count[4]
+    int cur_slot_step = 0;                    // step index (inside the graph being captured) the next stage stamps into
+    int64_t opt_stamps = 0;
     int64_t opt_gram_impl = 0, opt_full_lower = 0, opt_profile = 0, opt_no_graph = 0, opt_ksplit = 0, opt_rec_impl = 0, opt_loss_impl = 0, opt_no_fuse = 0;
     GramTcPlan *tc_plan = nullptr;
     GramPairPlan *pair_plan = nullptr;
@@ -94,6 +101,8 @@ struct casgd_ctx {
 namespace {
 
 constexpr int kRecReplicas = 8;
+constexpr int kStampSteps = 64;                         // the longest graph
+constexpr int kStampWords = kStampSteps * 4 * 2 + 8;    // slots, accum_ns[4], count[4]
 const unsigned kEpochInit[2] = {1u, 0u};                // {epoch, done}
 
 int fail(casgd_ctx *c, int code, const char *fmt, ...)
@@ -172,6 +181,7 @@ struct StageTimer {
     bool on;
     StageTimer(casgd_ctx *c_, int stage_) : c(c_), stage(stage_), on(c_->opt_profile != 0)
     {
+        g_stamp = (c->opt_stamps && c->stamps && stage < 4) ? c->stamps + 2 * (c->cur_slot_step * 4 + stage) : nullptr;
         if (!on) return;
         ev.stage = stage;
         cudaEventCreate(&ev.start);
@@ -180,6 +190,7 @@ struct StageTimer {
     }
     void done(int launches)
     {
+        g_stamp = nullptr;
         c->launches += launches;
         if (!on) return;
         cudaEventRecord(ev.stop, c->stream);
@@ -207,7 +218,7 @@ int enqueue_step(casgd_ctx *c, cudaStream_t st, const int32_t *idx, const StepPa
         t.done(k); *kernels += k;
     } else if (c->cur_gram != 4) {
         StageTimer t(c, CASGD_STAGE_GATHER);
-        k = launch_gather(st, c->A, c->lda, c->y, c->m, c->n, idx, ind, idx_off, sb, c->Y, c->ldy, c->yI, c->err_flag);
+        k = launch_gather(st, c->A, c->lda, c->y, c->m, c->n, idx, ind, idx_off, sb, c->Y, c->ldy, c->yI, c->err_flag, c->num_sms);
         t.done(k); *kernels += k;
     }
     if (!(s1 && c->cur_gram != 4)) {
@@ -227,7 +238,7 @@ int enqueue_step(casgd_ctx *c, cudaStream_t st, const int32_t *idx, const StepPa
                 c->tc_plan = gram_tc_plan_create(c->Y, c->ldy, c->n, c->rows_alloc, c->xbf, c->ldxb, c->err, sizeof c->err);
                 if (!c->tc_plan) return CASGD_ECUDA;
             }
-            k = launch_gram_tc(st, c->tc_plan, sb, b, c->G, c->ldg, c->r, (int)c->opt_full_lower, (int)c->opt_ksplit, c->err, sizeof c->err);
+            k = launch_gram_tc(st, c->tc_plan, sb, b, c->G, c->ldg, c->r, (int)c->opt_full_lower, (int)c->opt_ksplit, c->num_sms, c->err, sizeof c->err);
             if (k < 0) return CASGD_ECUDA;
         }
         t.done(k); *kernels += k;
@@ -296,9 +307,10 @@ int choose_gram(casgd_ctx *c, int32_t s, int32_t b)
     return CASGD_OK;
 }
 
+// The BF16 shadow is rebuilt from x at the start of EVERY casgd_outer_step(s) call (one n-element kernel per call, not
+// per step): a pointer-keyed cache would be fooled by an allocator that hands a new iterate the address of a freed one.
 int ensure_shadow(casgd_ctx *c, const float *x)
 {
-    if (c->shadow_valid && c->shadow_of == x) return CASGD_OK;
     StageTimer t(c, CASGD_STAGE_OTHER);
     int k = launch_shadow(c->stream, x, nullptr, c->n, c->xbf);
     t.done(k);
@@ -321,8 +333,11 @@ int get_graph(casgd_ctx *c, int32_t s, int32_t b, float eta, int32_t len, GraphE
     int64_t kernels = 0;
     int rc = CASGD_OK;
     const int64_t saved = c->launches;
-    for (int32_t h = 0; h < len && rc == CASGD_OK; ++h)
+    for (int32_t h = 0; h < len && rc == CASGD_OK; ++h) {
+        c->cur_slot_step = h;
         rc = enqueue_step(c, c->capture_stream, nullptr, c->ind, (int64_t)h * s * b, nullptr, s, b, eta, &kernels);
+    }
+    c->cur_slot_step = 0;
     c->launches = saved;                      // capture launches nothing; replays are counted
     cudaError_t e = cudaStreamEndCapture(c->capture_stream, &graph);
     if (rc != CASGD_OK) { if (graph) cudaGraphDestroy(graph); return rc; }
@@ -375,6 +390,8 @@ int run_steps(casgd_ctx *c, const int32_t *idx, int64_t n_steps, float *x, int32
                 c->launches += launch_set_params(c->stream, c->ind, idx + done * sb, x);
                 CK(cudaGraphLaunch(ge.exec, c->stream));
                 c->launches += ge.kernels;
+                if (c->opt_stamps)
+                    launch_stamp_collect(c->stream, c->stamps, len * 4, c->stamps + kStampSteps * 8, c->stamps + kStampSteps * 8 + 4);
                 done += len;
             }
         }
@@ -383,6 +400,8 @@ int run_steps(casgd_ctx *c, const int32_t *idx, int64_t n_steps, float *x, int32
         int64_t kernels = 0;
         rc = enqueue_step(c, c->stream, idx + done * sb, nullptr, 0, x, s, b, eta, &kernels);
         if (rc) return rc;
+        if (c->opt_stamps)
+            launch_stamp_collect(c->stream, c->stamps, 4, c->stamps + kStampSteps * 8, c->stamps + kStampSteps * 8 + 4);
     }
     CK(cudaGetLastError());
     return CASGD_OK;
@@ -402,6 +421,7 @@ int casgd_init(casgd_ctx **out, const uint16_t *X_bf16, int64_t ldx, const float
     if (!out) return CASGD_EINVAL;
     *out = nullptr;
     if (!X_bf16 || !y || m < 1 || n < 1 || ldx < n || loss < 0 || loss > 2) return CASGD_EINVAL;
+    if (m >= (1ll << 31)) return CASGD_EINVAL;              // every index buffer of the ABI is int32
     casgd_ctx *c = new (std::nothrow) casgd_ctx;
     if (!c) return CASGD_ENOMEM;
     auto bail = [&](int code) { casgd_destroy(c); return code; };
@@ -410,6 +430,11 @@ int casgd_init(casgd_ctx **out, const uint16_t *X_bf16, int64_t ldx, const float
         return bail(CASGD_ECUDA);
     if (prop.major != 10) return bail(CASGD_EARCH);
     c->num_sms = prop.multiProcessorCount;
+    // opt-in shared-memory sizes and cluster sizes are per-device function attributes: set them on this device
+    if (gather_configure() != cudaSuccess || gradient_configure() != cudaSuccess || gram_tc_configure() != cudaSuccess ||
+        gram_pair_configure() != cudaSuccess || loss_configure() != cudaSuccess || recurrence_configure() != cudaSuccess ||
+        recurrence_stream_configure() != cudaSuccess)
+        return bail(CASGD_ECUDA);
     c->stream = (cudaStream_t)cuda_stream;
     c->y = y; c->m = m; c->n = n; c->loss = loss;
     c->ldy = (int32_t)round_up(n, 8);
@@ -424,7 +449,7 @@ int casgd_init(casgd_ctx **out, const uint16_t *X_bf16, int64_t ldx, const float
         int64_t lda = round_up(n, 8);
         if (lda < 64) { int64_t p = 8; while (p < lda) p <<= 1; lda = p; }
         if (!ck(cudaMalloc(&c->A_owned, sizeof(uint16_t) * (size_t)m * lda))) return bail(CASGD_ENOMEM);
-        c->launches += launch_repack(c->stream, X_bf16, ldx, m, n, c->A_owned, lda);
+        c->launches += launch_repack(c->stream, X_bf16, ldx, m, n, c->A_owned, lda, c->num_sms);
         if (!ck(cudaStreamSynchronize(c->stream))) return bail(CASGD_ECUDA);
         c->A = c->A_owned;
         c->lda = lda;
@@ -435,7 +460,8 @@ int casgd_init(casgd_ctx **out, const uint16_t *X_bf16, int64_t ldx, const float
     const size_t xbf_elems = (size_t)16 * c->ldxb;
     c->gws.ldp = c->ldy;
     c->gws.max_splits = 128;
-    c->loss_max_blocks = kNumSMsB200 * 4;
+    c->gws.num_sms = c->num_sms;
+    c->loss_max_blocks = c->num_sms * 4;
     const int n_counters = 8192 + 1;              // gradient column tiles, plus casgd_loss's finished-CTA counter
     bool ok = ck(cudaMalloc(&c->xbf, sizeof(uint16_t) * xbf_elems)) &&
               ck(cudaMemsetAsync(c->xbf, 0, sizeof(uint16_t) * xbf_elems, c->stream)) &&
@@ -453,7 +479,9 @@ int casgd_init(casgd_ctx **out, const uint16_t *X_bf16, int64_t ldx, const float
               ck(cudaMalloc(&c->loss_partials, sizeof(double) * c->loss_max_blocks)) &&
               ck(cudaMalloc(&c->loss_result, sizeof(double))) &&
               ck(cudaMallocHost(&c->loss_result_host, sizeof(double))) &&
-              ck(cudaMalloc(&c->x_stage, sizeof(float) * (size_t)n));
+              ck(cudaMalloc(&c->x_stage, sizeof(float) * (size_t)n)) &&
+              ck(cudaMalloc(&c->stamps, sizeof(unsigned long long) * kStampWords)) &&
+              ck(cudaMemsetAsync(c->stamps, 0, sizeof(unsigned long long) * kStampWords, c->stream));
     if (!ok) return bail(CASGD_ENOMEM);
     c->rws.done = c->rws.epoch + 1;
     c->rws.nrep = kRecReplicas;
@@ -509,7 +537,6 @@ int casgd_outer_steps_sampled(casgd_ctx *c, int64_t n_steps, float *x, int32_t s
     int dummy = 0;
     int rc = check_step_args(c, &dummy, x, n_steps, s, b, eta);
     if (rc) return rc;
-    if (c->m >= (1ll << 32)) return fail(c, CASGD_EINVAL, "the on-device sampler needs m < 2^32");
     const int64_t count = n_steps * s * b;
     if (count > c->idx_stage_cap) {
         CK(cudaStreamSynchronize(c->stream));
@@ -529,7 +556,7 @@ int casgd_sgd_steps_fp32(casgd_ctx *c, const int32_t *idx, int64_t n_steps, floa
     if (rc) return rc;
     if (!c->A32) {
         CK(cudaMalloc(&c->A32, sizeof(float) * (size_t)c->m * c->lda));
-        c->launches += launch_widen(c->stream, c->A, c->lda, c->m, c->n, c->A32, c->lda);
+        c->launches += launch_widen(c->stream, c->A, c->lda, c->m, c->n, c->A32, c->lda, c->num_sms);
     }
     rc = ensure_workspace(c, b);
     if (rc) return rc;
@@ -555,7 +582,7 @@ int casgd_loss(casgd_ctx *c, const float *x, double *loss_host)
         StageTimer t(c, CASGD_STAGE_LOSS);
         t.done(launch_loss(c->stream, c->A, c->lda, c->X_caller, c->ldx_caller, c->y, c->m, c->n, c->loss, x,
                            c->loss_partials, c->loss_max_blocks, c->loss_result, c->gws.counters + 8192,
-                           (int)c->opt_loss_impl));
+                           (int)c->opt_loss_impl, c->num_sms));
     }
     CK(cudaGetLastError());
     CK(cudaMemcpyAsync(c->loss_result_host, c->loss_result, sizeof(double), cudaMemcpyDeviceToHost, c->stream));
@@ -636,6 +663,13 @@ int casgd_set_option(casgd_ctx *c, int option, int64_t value)
         if (value < 0 || value > 4) return fail(c, CASGD_EINVAL, "CASGD_OPT_RECURRENCE_IMPL must be in [0, 4]");
         c->opt_rec_impl = value; break;
     case CASGD_OPT_NO_FUSED_UPDATE: c->opt_no_fuse = value != 0; break;
+    case CASGD_OPT_STAMPS:
+        c->opt_stamps = value != 0;
+        // arm every slot ({~0, 0}) and clear the totals: a collect pass over all slots, then zero the accumulators
+        CK(cudaStreamSynchronize(c->stream));
+        launch_stamp_collect(c->stream, c->stamps, kStampSteps * 4, c->stamps + kStampSteps * 8, c->stamps + kStampSteps * 8 + 4);
+        CK(cudaMemsetAsync(c->stamps + kStampSteps * 8, 0, sizeof(unsigned long long) * 8, c->stream));
+        break;
     case CASGD_OPT_LOSS_IMPL:
         if (value != 0 && value != 1) return fail(c, CASGD_EINVAL, "CASGD_OPT_LOSS_IMPL must be 0 or 1");
         c->opt_loss_impl = value; break;
@@ -650,6 +684,22 @@ int casgd_stage_times(casgd_ctx *c, double *ms_host, int64_t *launches_host, int
     if (!c) return CASGD_EINVAL;
     CK(cudaStreamSynchronize(c->stream));
     collect_events(c);
+    if (c->opt_stamps) {
+        // in-graph stamps replace the event times of the four step stages
+        unsigned long long acc[8];
+        CK(cudaMemcpy(acc, c->stamps + kStampSteps * 8, sizeof acc, cudaMemcpyDeviceToHost));
+        for (int i = 0; i < 4; ++i) {
+            if (ms_host) ms_host[i] = (double)acc[i] * 1e-6;
+            if (launches_host) launches_host[i] = (int64_t)acc[4 + i];
+        }
+        for (int i = 4; i < CASGD_NUM_STAGES; ++i) {
+            if (ms_host) ms_host[i] = c->stage_ms[i];
+            if (launches_host) launches_host[i] = c->stage_launches[i];
+            if (reset) { c->stage_ms[i] = 0.0; c->stage_launches[i] = 0; }
+        }
+        if (reset) CK(cudaMemset(c->stamps + kStampSteps * 8, 0, sizeof(unsigned long long) * 8));
+        return CASGD_OK;
+    }
     for (int i = 0; i < CASGD_NUM_STAGES; ++i) {
         if (ms_host) ms_host[i] = c->stage_ms[i];
         if (launches_host) launches_host[i] = c->stage_launches[i];
@@ -671,7 +721,7 @@ void casgd_destroy(casgd_ctx *c)
     if (c->capture_stream) cudaStreamDestroy(c->capture_stream);
     cudaFree(c->A_owned); cudaFree(c->A32); cudaFree(c->xbf);
     cudaFree(c->gws.partial); cudaFree(c->gws.counters); cudaFree(c->ind); cudaFree(c->err_flag);
-    cudaFree(c->rws.utag); cudaFree(c->rws.epoch);
+    cudaFree(c->rws.utag); cudaFree(c->rws.epoch); cudaFree(c->stamps);
     cudaFree(c->loss_partials); cudaFree(c->loss_result); cudaFree(c->idx_stage); cudaFree(c->x_stage);
     if (c->err_flag_host) cudaFreeHost(c->err_flag_host);
     if (c->loss_result_host) cudaFreeHost(c->loss_result_host);

@@ -13,7 +13,6 @@
 namespace casgd {
 
 constexpr int kTile = 128;            // Gram tile edge (rows of Y per tcgen05 operand tile)
-constexpr int kNumSMsB200 = 148;
 
 // Device-side indirection block: lets kernels baked into a CUDA graph follow a base pointer
 // that changes between replays (casgd_outer_steps).
@@ -128,6 +127,32 @@ __device__ __forceinline__ float ld_dep(const float *p)
 }
 __device__ __forceinline__ void pdl_trigger() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
 
+// ------------------------------------------------------------- in-graph stage stamps ---
+// CASGD_OPT_STAMPS: every kernel of an outer step records when its first CTA got past pdl_wait() (atomicMin of
+// %globaltimer) and when its last CTA finished (atomicMax) into a {t0, t1} slot of its (step, stage) -- the kernels run
+// exactly as bench.py times them (CUDA-graph replay, programmatic dependent launch), unlike CASGD_OPT_PROFILE's direct
+// launches. The slot pointer is a kernel argument baked into the graph (null = off). A launcher reads it from the
+// thread-local g_stamp, which enqueue_step sets around each stage.
+extern thread_local unsigned long long *g_stamp;
+__device__ __forceinline__ unsigned long long globaltimer_ns()
+{
+    unsigned long long t;
+    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+    return t;
+}
+__device__ __forceinline__ void stamp_begin(unsigned long long *s)
+{
+    if (s && threadIdx.x == 0) atomicMin(s, globaltimer_ns());
+}
+__device__ __forceinline__ void stamp_end(unsigned long long *s)      // by thread 0, after the CTA's last barrier
+{
+    if (s && threadIdx.x == 0) atomicMax(s + 1, globaltimer_ns());
+}
+__device__ __forceinline__ void stamp_end_warp(unsigned long long *s) // by every warp (kernels whose warps end on their own)
+{
+    if (s && (threadIdx.x & 31) == 0) atomicMax(s + 1, globaltimer_ns());
+}
+
 // cudaLaunchKernelEx with the programmatic-serialisation attribute (and a cluster dimension when cluster > 1).
 template <typename... KArgs, typename... Args>
 inline cudaError_t launch_pdl(void (*kern)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t st, int cluster,
@@ -155,13 +180,23 @@ inline cudaError_t launch_pdl(void (*kern)(KArgs...), dim3 grid, dim3 block, siz
     return cudaLaunchKernelEx(&cfg, kern, KArgs(args)...);
 }
 
+// Per-device kernel attributes (opt-in shared memory sizes, non-portable cluster sizes): set for the CURRENT device by
+// casgd_init, every time -- they are per device, so a process with contexts on several GPUs needs them on each.
+cudaError_t gather_configure();
+cudaError_t gradient_configure();
+cudaError_t gram_tc_configure();
+cudaError_t gram_pair_configure();
+cudaError_t loss_configure();
+cudaError_t recurrence_configure();
+cudaError_t recurrence_stream_configure();
+
 // ------------------------------------------------------------ launch prototypes ---
 // Every launcher enqueues on `st` and returns the number of kernels it launched.
 // `ind`, when non-null, overrides idx / x with ind->idx + idx_off / ind->x (graph replay).
 
 int launch_gather(cudaStream_t st, const uint16_t *A, int64_t lda, const float *y, int64_t m, int32_t n,
                   const int32_t *idx, const StepParams *ind, int64_t idx_off, int32_t sb, uint16_t *Y, int32_t ldy,
-                  float *yI, int *err_flag);
+                  float *yI, int *err_flag, int num_sms);
 
 int launch_gram_simt(cudaStream_t st, const uint16_t *Y, int32_t ldy, int32_t n, int32_t sb, int32_t b,
                      const uint16_t *xbf, float *G, int32_t ldg, float *r, int full_lower);
@@ -206,6 +241,7 @@ struct GradWorkspace {
     int32_t ldp;
     unsigned *counters;    // one per column tile, zero between launches
     int32_t max_splits;
+    int32_t num_sms;       // SMs of the context's device (grid sizing)
 };
 
 int launch_gradient_bf16(cudaStream_t st, const uint16_t *Y, int32_t ldy, int32_t n, int32_t sb, const float *u,
@@ -222,14 +258,17 @@ int launch_sgd32_step(cudaStream_t st, const float *A32, int64_t lda32, const fl
 
 int launch_loss(cudaStream_t st, const uint16_t *A, int64_t lda, const uint16_t *X, int64_t ldx, const float *y, int64_t m,
                 int32_t n, int loss, const float *x, double *block_partials, int32_t max_blocks, double *result_dev,
-                unsigned *done_counter, int impl);
+                unsigned *done_counter, int impl, int num_sms);
 
 int launch_sample_indices(cudaStream_t st, int32_t *idx, int64_t n_steps, int32_t sb, int64_t m, uint64_t seed,
                           uint64_t first_step);
 int launch_shadow(cudaStream_t st, const float *x, const StepParams *ind, int32_t n, uint16_t *xbf);
-int launch_widen(cudaStream_t st, const uint16_t *A, int64_t lda, int64_t m, int32_t n, float *A32, int64_t lda32);
-int launch_repack(cudaStream_t st, const uint16_t *X, int64_t ldx, int64_t m, int32_t n, uint16_t *A, int64_t lda);
+int launch_widen(cudaStream_t st, const uint16_t *A, int64_t lda, int64_t m, int32_t n, float *A32, int64_t lda32, int num_sms);
+int launch_repack(cudaStream_t st, const uint16_t *X, int64_t ldx, int64_t m, int32_t n, uint16_t *A, int64_t lda, int num_sms);
 int launch_set_params(cudaStream_t st, StepParams *ind, const int32_t *idx, float *x);
+// slots: [nslots][2] {min start, max end} in %globaltimer ns, slot = 4 * step + stage; accum_ns / count: [4]
+int launch_stamp_collect(cudaStream_t st, unsigned long long *slots, int nslots, unsigned long long *accum_ns,
+                         unsigned long long *count);
 
 // tcgen05 Gram + margin (gram_tc.cu). The plan owns the TMA tensor maps of the Y workspace and of the
 // BF16 shadow (a [16 x ldxb] buffer: row 0 = x_bf, rows 1..15 zero). ksplit_opt <= 0: choose automatically.
@@ -244,7 +283,7 @@ GramTcPlan *gram_tc_plan_create(const uint16_t *Y, int32_t ldy, int32_t n, int32
                                 const uint16_t *xbf, int32_t ldxb, char *err, int errlen);
 void gram_tc_plan_destroy(GramTcPlan *p);
 int launch_gram_tc(cudaStream_t st, GramTcPlan *plan, int32_t sb, int32_t b, float *G, int32_t ldg, float *r,
-                   int full_lower, int ksplit_opt, char *err, int errlen);
+                   int full_lower, int ksplit_opt, int num_sms, char *err, int errlen);
 
 // gather + Gram + margin in one kernel for narrow rows (n <= 64): gram_tc.cu
 int launch_gram_narrow(cudaStream_t st, const uint16_t *A, int64_t lda, const float *y, int64_t m, int32_t n,

@@ -10,10 +10,11 @@ namespace casgd {
 __global__ void __launch_bounds__(256)
 gather_rows_kernel(const uint16_t *__restrict__ A, int64_t lda, const float *__restrict__ y, int64_t m, int32_t n,
                    const int32_t *idx, const StepParams *ind, int64_t idx_off, int32_t sb,
-                   uint16_t *Y, int32_t ldy, float *yI, int *err_flag)
+                   uint16_t *Y, int32_t ldy, float *yI, int *err_flag, unsigned long long *stamp)
 {
     pdl_trigger();
     pdl_wait();                                     // Y is still being read by the previous step's gradient
+    stamp_begin(stamp);
     const int32_t chunks = ldy >> 3;
     const int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     const int64_t row = t / chunks;
@@ -42,6 +43,7 @@ gather_rows_kernel(const uint16_t *__restrict__ A, int64_t lda, const float *__r
         yI[row] = ok ? y[src] : 0.f;
         if (!ok) atomicOr(err_flag, 1);
     }
+    stamp_end_warp(stamp);
 }
 
 // Wide rows (n % 8 == 0, >= 512 bytes): the gather is pure data movement, so it is done by the copy engine alone.
@@ -55,7 +57,7 @@ constexpr uint32_t kGbSlot = 4096;
 __global__ void __launch_bounds__(32 * kGbWarps, 1)
 gather_bulk_kernel(const uint16_t *__restrict__ A, int64_t lda, const float *__restrict__ y, int64_t m, int32_t n,
                    const int32_t *idx, const StepParams *ind, int64_t idx_off, int32_t sb,
-                   uint16_t *Y, int32_t ldy, float *yI, int *err_flag)
+                   uint16_t *Y, int32_t ldy, float *yI, int *err_flag, unsigned long long *stamp)
 {
     extern __shared__ __align__(128) unsigned char gb_smem[];
     __shared__ __align__(8) unsigned long long bars[kGbWarps * kGbDepth];
@@ -71,6 +73,7 @@ gather_bulk_kernel(const uint16_t *__restrict__ A, int64_t lda, const float *__r
     }
     __syncwarp();
     pdl_wait();                                     // Y is still being read by the previous step's gradient
+    stamp_begin(stamp);
     const int32_t *I = ind ? ind->idx + idx_off : idx;
     const int gw = blockIdx.x * kGbWarps + warp, W = gridDim.x * kGbWarps;
 
@@ -144,31 +147,33 @@ gather_bulk_kernel(const uint16_t *__restrict__ A, int64_t lda, const float *__r
         }
     }
     if (lane == 0) asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");   // the stores have landed before the CTA exits
+    stamp_end_warp(stamp);
+}
+
+cudaError_t gather_configure()
+{
+    return cudaFuncSetAttribute(gather_bulk_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                (int)((size_t)kGbWarps * kGbDepth * kGbSlot));
 }
 
 int launch_gather(cudaStream_t st, const uint16_t *A, int64_t lda, const float *y, int64_t m, int32_t n,
                   const int32_t *idx, const StepParams *ind, int64_t idx_off, int32_t sb, uint16_t *Y, int32_t ldy,
-                  float *yI, int *err_flag)
+                  float *yI, int *err_flag, int num_sms)
 {
     if (n % 8 == 0 && n * 2 >= 512 && ldy == n && (int64_t)sb * n * 2 >= (1 << 20)) {
-        static bool attr_set = false;
         const size_t smem = (size_t)kGbWarps * kGbDepth * kGbSlot;
-        if (!attr_set) {
-            cudaFuncSetAttribute(gather_bulk_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-            attr_set = true;
-        }
         const int ppr = (n * 2 + (int)kGbSlot - 1) / (int)kGbSlot;
         const int64_t pieces = (int64_t)sb * ppr;
-        const int blocks = (int)std::max<int64_t>(1, std::min<int64_t>(kNumSMsB200, (pieces + kGbWarps * 2 - 1) / (kGbWarps * 2)));
+        const int blocks = (int)std::max<int64_t>(1, std::min<int64_t>(num_sms, (pieces + kGbWarps * 2 - 1) / (kGbWarps * 2)));
         launch_pdl(gather_bulk_kernel, dim3(blocks), dim3(32 * kGbWarps), smem, st, 1, A, lda, y, m, n, idx, ind, idx_off, sb, Y,
-                   ldy, yI, err_flag);
+                   ldy, yI, err_flag, g_stamp);
         return 1;
     }
     const int64_t total = (int64_t)sb * (ldy >> 3);
     const int threads = 256;
     const unsigned blocks = (unsigned)((total + threads - 1) / threads);
     launch_pdl(gather_rows_kernel, dim3(blocks), dim3(threads), 0, st, 1, A, lda, y, m, n, idx, ind, idx_off, sb, Y, ldy, yI,
-               err_flag);
+               err_flag, g_stamp);
     return 1;
 }
 
@@ -201,9 +206,9 @@ __global__ void widen_kernel(const uint16_t *__restrict__ A, int64_t lda, int64_
     }
 }
 
-int launch_widen(cudaStream_t st, const uint16_t *A, int64_t lda, int64_t m, int32_t n, float *A32, int64_t lda32)
+int launch_widen(cudaStream_t st, const uint16_t *A, int64_t lda, int64_t m, int32_t n, float *A32, int64_t lda32, int num_sms)
 {
-    widen_kernel<<<kNumSMsB200 * 8, 256, 0, st>>>(A, lda, m, n, A32, lda32);
+    widen_kernel<<<num_sms * 8, 256, 0, st>>>(A, lda, m, n, A32, lda32);
     return 1;
 }
 
@@ -219,9 +224,31 @@ __global__ void repack_kernel(const uint16_t *__restrict__ X, int64_t ldx, int64
     }
 }
 
-int launch_repack(cudaStream_t st, const uint16_t *X, int64_t ldx, int64_t m, int32_t n, uint16_t *A, int64_t lda)
+int launch_repack(cudaStream_t st, const uint16_t *X, int64_t ldx, int64_t m, int32_t n, uint16_t *A, int64_t lda, int num_sms)
 {
-    repack_kernel<<<kNumSMsB200 * 8, 256, 0, st>>>(X, ldx, m, n, A, lda);
+    repack_kernel<<<num_sms * 8, 256, 0, st>>>(X, ldx, m, n, A, lda);
+    return 1;
+}
+
+// CASGD_OPT_STAMPS: fold the {first start, last end} slots of the steps just run into per-stage totals and re-arm them.
+__global__ void stamp_collect_kernel(unsigned long long *slots, int nslots, unsigned long long *accum_ns,
+                                     unsigned long long *count)
+{
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= nslots) return;
+    const unsigned long long t0 = slots[2 * i], t1 = slots[2 * i + 1];
+    if (t1 != 0ull && t0 != ~0ull && t1 >= t0) {
+        atomicAdd(accum_ns + (i & 3), t1 - t0);
+        atomicAdd(count + (i & 3), 1ull);
+    }
+    slots[2 * i] = ~0ull;
+    slots[2 * i + 1] = 0ull;
+}
+
+int launch_stamp_collect(cudaStream_t st, unsigned long long *slots, int nslots, unsigned long long *accum_ns,
+                         unsigned long long *count)
+{
+    stamp_collect_kernel<<<(nslots + 255) / 256, 256, 0, st>>>(slots, nslots, accum_ns, count);
     return 1;
 }
 

@@ -38,11 +38,12 @@ __global__ void __launch_bounds__(kGradThreads)
 gradient_update_kernel(const T *base, int64_t ld, const int32_t *idx, int64_t m, int32_t n,
                        int32_t rows, int32_t rows_per_split, int32_t CV, const float *u, float alpha,
                        float *x_direct, const StepParams *ind, uint16_t *xbf,
-                       float *partial, int32_t ldp, unsigned *counters)
+                       float *partial, int32_t ldp, unsigned *counters, unsigned long long *stamp)
 {
     constexpr int kVec = VecTraits<T>::kVec;
     pdl_trigger();
     pdl_wait();
+    stamp_begin(stamp);
     __shared__ float red[kGradThreads * kVec];
     __shared__ bool s_last;
     const int tid = threadIdx.x;
@@ -97,7 +98,7 @@ gradient_update_kernel(const T *base, int64_t ld, const int32_t *idx, int64_t m,
     __syncthreads();
     if (tid == 0) s_last = (atomicAdd(&counters[blockIdx.x], 1u) == gridDim.y - 1);
     __syncthreads();
-    if (!s_last) return;
+    if (!s_last) { stamp_end(stamp); return; }
     __threadfence();
     float *x = ind ? ind->x : x_direct;
     if (tid < tile_cols && col0 + tid < n) {
@@ -109,6 +110,8 @@ gradient_update_kernel(const T *base, int64_t ld, const int32_t *idx, int64_t m,
         if (SHADOW) xbf[col] = f32_to_bf16_bits_rn(xn);
     }
     if (tid == 0) counters[blockIdx.x] = 0u;
+    __syncthreads();
+    stamp_end(stamp);
 }
 
 // ------------------------------------------------------------------ wide rows: streamed through the copy engine ---
@@ -125,7 +128,7 @@ __global__ void __launch_bounds__(32 * kGsWarps, 1)
 gradient_stream_kernel(const uint16_t *Y, int32_t ldy, int32_t n, int32_t sb, int32_t rpw,
                        const float *u, float alpha, float *x_direct,
                        const StepParams *ind, uint16_t *xbf, float *partial,
-                       int32_t ldp, unsigned *counters)
+                       int32_t ldp, unsigned *counters, unsigned long long *stamp)
 {
     extern __shared__ __align__(128) unsigned char gs_smem[];
     __shared__ __align__(8) unsigned long long bars[kGsWarps * kGsDepth];
@@ -143,6 +146,7 @@ gradient_stream_kernel(const uint16_t *Y, int32_t ldy, int32_t n, int32_t sb, in
     }
     __syncwarp();
     pdl_wait();
+    stamp_begin(stamp);
 
     const int col0 = blockIdx.x * kGsSegCols;
     const uint32_t segB = min(kGsPiece, (uint32_t)(ldy - col0) * 2u);       // a multiple of 16 (ldy % 8 == 0)
@@ -210,7 +214,7 @@ gradient_stream_kernel(const uint16_t *Y, int32_t ldy, int32_t n, int32_t sb, in
     __syncthreads();
     if (threadIdx.x == 0) s_last = (atomicAdd(&counters[blockIdx.x], 1u) == gridDim.y - 1);
     __syncthreads();
-    if (!s_last) return;
+    if (!s_last) { stamp_end(stamp); return; }
     __threadfence();
     float *x = ind ? ind->x : x_direct;
     if (mine) {
@@ -234,25 +238,27 @@ gradient_stream_kernel(const uint16_t *Y, int32_t ldy, int32_t n, int32_t sb, in
         }
     }
     if (threadIdx.x == 0) counters[blockIdx.x] = 0u;
+    __syncthreads();
+    stamp_end(stamp);
+}
+
+cudaError_t gradient_configure()
+{
+    return cudaFuncSetAttribute(gradient_stream_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kGsSmem);
 }
 
 static int launch_gradient_stream(cudaStream_t st, const uint16_t *Y, int32_t ldy, int32_t n, int32_t sb, const float *u,
                                   float alpha, float *x, const StepParams *ind, uint16_t *xbf, const GradWorkspace &ws)
 {
-    static bool attr_set = false;
-    if (!attr_set) {
-        cudaFuncSetAttribute(gradient_stream_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kGsSmem);
-        attr_set = true;
-    }
     const int col_segs = (ldy + kGsSegCols - 1) / kGsSegCols;
     // rows per warp: at least 8 (fixed costs), at most 32 (one u per lane); about one CTA per SM for large steps
-    const int slabs_target = std::max(1, kNumSMsB200 / col_segs);
+    const int slabs_target = std::max(1, ws.num_sms / col_segs);
     int rpw = (sb + kGsWarps * slabs_target - 1) / (kGsWarps * slabs_target);
     rpw = std::min(32, std::max(8, rpw));
     const int slabs = (sb + kGsWarps * rpw - 1) / (kGsWarps * rpw);
     if (slabs > ws.max_splits) return 0;
     launch_pdl(gradient_stream_kernel, dim3(col_segs, slabs), dim3(32 * kGsWarps), kGsSmem, st, 1, Y, ldy, n, sb, rpw, u, alpha, x,
-               ind, xbf, ws.partial, ws.ldp, ws.counters);
+               ind, xbf, ws.partial, ws.ldp, ws.counters, g_stamp);
     return 1;
 }
 
@@ -268,14 +274,14 @@ static int launch_gradient_any(cudaStream_t st, const T *base, int64_t ld, const
     const int CV = min(32, next_pow2(nvec));
     const int RL = kGradThreads / CV;
     const int col_tiles = (nvec + CV - 1) / CV;
-    int splits = (4 * kNumSMsB200 + col_tiles - 1) / col_tiles;
+    int splits = (4 * ws.num_sms + col_tiles - 1) / col_tiles;
     splits = min(splits, (rows + RL - 1) / RL);
     splits = max(1, min(splits, ws.max_splits));
     const int rows_per_split = (rows + splits - 1) / splits;
     splits = (rows + rows_per_split - 1) / rows_per_split;
     dim3 grid(col_tiles, splits);
     launch_pdl(gradient_update_kernel<T, GATHER, SHADOW>, grid, dim3(kGradThreads), 0, st, 1, base, ld, idx, m, n, rows,
-               rows_per_split, CV, u, alpha, x, ind, xbf, ws.partial, ws.ldp, ws.counters);
+               rows_per_split, CV, u, alpha, x, ind, xbf, ws.partial, ws.ldp, ws.counters, SHADOW ? g_stamp : nullptr);
     return 1;
 }
 
@@ -294,10 +300,11 @@ int launch_gradient_bf16(cudaStream_t st, const uint16_t *Y, int32_t ldy, int32_
 __global__ void __launch_bounds__(256)
 margin_s1_kernel(const uint16_t *__restrict__ A, int64_t lda, const float *__restrict__ y, int64_t m, int32_t n,
                  const int32_t *idx, const StepParams *ind, int64_t idx_off, int32_t b, int loss, const uint16_t *xbf,
-                 uint16_t *Y, int32_t ldy, float *yI, float *r, float *z, float *u, int *err_flag)
+                 uint16_t *Y, int32_t ldy, float *yI, float *r, float *z, float *u, int *err_flag, unsigned long long *stamp)
 {
     pdl_trigger();
     pdl_wait();                                     // x_bf comes from the previous gradient; Y is read by it until now
+    stamp_begin(stamp);
     const int row = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
     if (row >= b) return;
     const int32_t *I = ind ? ind->idx + idx_off : idx;
@@ -349,6 +356,7 @@ margin_s1_kernel(const uint16_t *__restrict__ A, int64_t lda, const float *__res
         z[row] = acc;
         u[row] = lprime_rt(loss, acc, ylab);
     }
+    stamp_end_warp(stamp);
 }
 
 int launch_margin_s1(cudaStream_t st, const uint16_t *A, int64_t lda, const float *y, int64_t m, int32_t n,
@@ -356,7 +364,7 @@ int launch_margin_s1(cudaStream_t st, const uint16_t *A, int64_t lda, const floa
                      uint16_t *Y, int32_t ldy, float *yI, float *r, float *z, float *u, int *err_flag)
 {
     launch_pdl(margin_s1_kernel, dim3((b * 32 + 255) / 256), dim3(256), 0, st, 1, A, lda, y, m, n, idx, ind, idx_off, b, loss, xbf, Y,
-               ldy, yI, r, z, u, err_flag);
+               ldy, yI, r, z, u, err_flag, g_stamp);
     return 1;
 }
 

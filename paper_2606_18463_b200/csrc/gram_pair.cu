@@ -65,6 +65,7 @@ struct PairParams {
     float *rpart;                       // [mslices x ldr]
     unsigned *rcount;                   // [2 x row tiles], zero between launches
     int32_t mslices, ldr;
+    unsigned long long *stamp;
 };
 
 // ------------------------------------------------------------------------------------ PTX ---
@@ -215,6 +216,7 @@ gram_pair_kernel(const __grid_constant__ CUtensorMap tmY, const __grid_constant_
     tc_fence_after();
     const uint32_t tmem_base = *tmem_slot_ptr;
     pdl_wait();                                         // Y and x_bf come from the gather / the previous gradient
+    stamp_begin(p.stamp);
 
     if (warp == 0) {
         // ===== TMA producer (both CTAs): own half of A, own half of each B sub-tile =====
@@ -395,6 +397,7 @@ gram_pair_kernel(const __grid_constant__ CUtensorMap tmY, const __grid_constant_
         tc_fence_after();
         asm volatile("tcgen05.dealloc.cta_group::2.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "r"(512u) : "memory");
     }
+    stamp_end(p.stamp);
 }
 
 typedef CUresult (*EncodeTiledFnP)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *,
@@ -498,7 +501,6 @@ struct GramPairPlan {
     float *rpart = nullptr;             // [4 x rows_alloc] margin partial sums
     unsigned *rcount = nullptr;         // [2 x row tiles]
     int32_t n = 0, rows_alloc = 0, npairs = 0;
-    bool attr_set = false;
     std::map<std::tuple<int, int, int, int, int>, PairList> lists;       // (sb, b, full_lower, bn, ksplit_opt)
 };
 
@@ -520,6 +522,11 @@ GramPairPlan *gram_pair_plan_create(const uint16_t *Y, int32_t ldy, int32_t n, i
         return nullptr;
     }
     return pl;
+}
+
+cudaError_t gram_pair_configure()
+{
+    return cudaFuncSetAttribute(gram_pair_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemP);
 }
 
 void gram_pair_plan_destroy(GramPairPlan *p)
@@ -593,19 +600,12 @@ int launch_gram_pair(cudaStream_t st, GramPairPlan *pl, int32_t sb, int32_t b, f
         return -1;
     }
     const PairList &L = it->second;
-    if (!pl->attr_set) {
-        cudaError_t e = cudaFuncSetAttribute(gram_pair_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemP);
-        if (e != cudaSuccess) {
-            snprintf(err, errlen, "cudaFuncSetAttribute(gram_pair_kernel): %s", cudaGetErrorString(e));
-            return -1;
-        }
-        pl->attr_set = true;
-    }
     PairParams p;
     p.G = G; p.r = r; p.items = L.items; p.counts = L.counts;
     p.ldg = ldg; p.sb = sb; p.b = b; p.n = pl->n; p.full_lower = full_lower; p.bn = bn;
     p.nslots = bn == 256 ? 2 : 1;
     p.accumulate = L.ksplit > 1;
+    p.stamp = g_stamp;
     p.rpart = pl->rpart; p.rcount = pl->rcount; p.mslices = margin_slices(pl->n); p.ldr = pl->rows_alloc;
     if (L.ksplit > 1) {
         const int T128 = (sb + 127) / 128;

@@ -38,6 +38,7 @@ struct GramParams {
     float *G;
     float *r;
     int32_t ldg, sb, b, n, T, ntiles, ksplit, kb_total, full_lower;
+    unsigned long long *stamp;
 };
 
 // ------------------------------------------------------------------------------------ PTX ---
@@ -184,6 +185,7 @@ gram_tc_kernel(const __grid_constant__ CUtensorMap tmY, const __grid_constant__ 
     tc_fence_after();
     const uint32_t tmem_base = *tmem_slot_ptr;
     pdl_wait();                                     // Y and x_bf come from the gather / the previous gradient
+    stamp_begin(p.stamp);
 
     if (warp == 0) {
         // ===== TMA producer =====
@@ -324,6 +326,7 @@ gram_tc_kernel(const __grid_constant__ CUtensorMap tmY, const __grid_constant__ 
         tc_fence_after();
         asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "r"(kTmemCols) : "memory");
     }
+    stamp_end(p.stamp);
 }
 
 // ------------------------------------------------------------------ narrow rows: gather + Gram in one kernel ---
@@ -352,6 +355,7 @@ struct NarrowParams {
     int32_t ldy, ldg, sb, b, n, T, full_lower;
     int32_t s1_loss;                    // >= 0 (s = 1): the epilogue also writes z = r and u = l'(r, y_I)
     float *z, *u;
+    unsigned long long *stamp;
 };
 
 __global__ void __launch_bounds__(kNwThreads)
@@ -390,6 +394,7 @@ gram_narrow_kernel(const NarrowParams p)
         asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
     }
     pdl_wait();                                     // x_bf and the Y stage belong to the previous step until now
+    stamp_begin(p.stamp);
 
     // ---- gather: thread t owns row t of each operand tile
     const int32_t *I = p.ind ? p.ind->idx + p.idx_off : p.idx;
@@ -510,6 +515,7 @@ gram_narrow_kernel(const NarrowParams p)
         tc_fence_after();
         asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "r"(256u) : "memory");
     }
+    stamp_end(p.stamp);
 }
 
 typedef CUresult (*EncodeTiledFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *,
@@ -548,7 +554,6 @@ bool make_bf16_map(CUtensorMap *map, const void *base, uint64_t cols, uint64_t r
 struct GramTcPlan {
     CUtensorMap tmY, tmX;
     int32_t n, rows_alloc;
-    bool attr_set;
 };
 
 // Y: [rows_alloc x ldy] BF16 (pad columns zero), xbf: [16 x ldxb] BF16 whose row 0 is the shadow and rows 1..15 zero.
@@ -558,7 +563,6 @@ GramTcPlan *gram_tc_plan_create(const uint16_t *Y, int32_t ldy, int32_t n, int32
     GramTcPlan *pl = new GramTcPlan;
     pl->n = n;
     pl->rows_alloc = rows_alloc;
-    pl->attr_set = false;
     // inner extent n: the K tail of the last 64-wide box is zero-filled by TMA
     if (!make_bf16_map(&pl->tmY, Y, (uint64_t)n, (uint64_t)rows_alloc, (uint64_t)ldy, BK, BM) ||
         !make_bf16_map(&pl->tmX, xbf, (uint64_t)n, (uint64_t)XR, (uint64_t)ldxb, BK, XR)) {
@@ -571,28 +575,28 @@ GramTcPlan *gram_tc_plan_create(const uint16_t *Y, int32_t ldy, int32_t n, int32
 
 void gram_tc_plan_destroy(GramTcPlan *p) { delete p; }
 
-int launch_gram_tc(cudaStream_t st, GramTcPlan *plan, int32_t sb, int32_t b, float *G, int32_t ldg, float *r,
-                   int full_lower, int ksplit_opt, char *err, int errlen)
+cudaError_t gram_tc_configure()
 {
-    if (!plan->attr_set) {
-        cudaError_t e = cudaFuncSetAttribute(gram_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemBytes);
-        if (e != cudaSuccess) {
-            snprintf(err, errlen, "cudaFuncSetAttribute(gram_tc_kernel): %s", cudaGetErrorString(e));
-            return -1;
-        }
-        plan->attr_set = true;
-    }
+    cudaError_t e = cudaFuncSetAttribute(gram_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemBytes);
+    if (e != cudaSuccess) return e;
+    return cudaFuncSetAttribute(gram_narrow_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kNwSmem);
+}
+
+int launch_gram_tc(cudaStream_t st, GramTcPlan *plan, int32_t sb, int32_t b, float *G, int32_t ldg, float *r,
+                   int full_lower, int ksplit_opt, int num_sms, char *err, int errlen)
+{
     GramParams p;
     p.G = G; p.r = r; p.ldg = ldg; p.sb = sb; p.b = b; p.n = plan->n;
     p.T = (sb + BM - 1) / BM;
     p.ntiles = p.T * (p.T + 1) / 2;
     p.kb_total = (plan->n + BK - 1) / BK;
     p.full_lower = full_lower;
+    p.stamp = g_stamp;
     int ksplit = ksplit_opt;
     if (ksplit <= 0) {
         // fill the 148 SMs when there are few tiles -- but the cleared G, its memset node and the red.add epilogue
         // cost several microseconds, so only when a slice still holds >= 16 K blocks (1024 columns)
-        ksplit = kNumSMsB200 / p.ntiles;
+        ksplit = num_sms / p.ntiles;
         ksplit = std::min(ksplit, p.kb_total / 16);
         // ... and only when the split takes >= 24 K blocks off the critical path (measured: n = 2000, 32 K blocks:
         // splitting in 2 costs 3 us more than it saves; n = 4096, 64 K blocks: splitting in 4 saves 5 us)
@@ -606,8 +610,12 @@ int launch_gram_tc(cudaStream_t st, GramTcPlan *plan, int32_t sb, int32_t b, flo
         cudaMemsetAsync(G, 0, sizeof(float) * (size_t)p.T * BM * ldg, st);
         cudaMemsetAsync(r, 0, sizeof(float) * (size_t)p.T * BM, st);
     }
-    const int grid = std::min(p.ntiles * ksplit, kNumSMsB200);
-    launch_pdl(gram_tc_kernel, dim3(grid), dim3(kThreads), kSmemBytes, st, 1, plan->tmY, plan->tmX, p);
+    const int grid = std::min(p.ntiles * ksplit, num_sms);
+    cudaError_t e = launch_pdl(gram_tc_kernel, dim3(grid), dim3(kThreads), kSmemBytes, st, 1, plan->tmY, plan->tmX, p);
+    if (e != cudaSuccess) {
+        snprintf(err, errlen, "gram_tc_kernel launch: %s", cudaGetErrorString(e));
+        return -1;
+    }
     return launches;
 }
 
@@ -617,11 +625,6 @@ int launch_gram_narrow(cudaStream_t st, const uint16_t *A, int64_t lda, const fl
                        const uint16_t *xbf, int32_t ldxb, uint16_t *Y, int32_t ldy, float *yI, float *G, int32_t ldg,
                        float *r, int full_lower, int *err_flag, const S1Fuse *s1)
 {
-    static bool attr_set = false;
-    if (!attr_set) {
-        if (cudaFuncSetAttribute(gram_narrow_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kNwSmem) != cudaSuccess) return -1;
-        attr_set = true;
-    }
     NarrowParams p;
     p.A = A; p.lda = lda; p.m = m; p.y = y; p.idx = idx; p.ind = ind; p.idx_off = idx_off; p.xbf = xbf; p.ldxb = ldxb;
     p.Y = Y; p.yI = yI; p.G = G; p.r = r; p.err_flag = err_flag; p.ldy = ldy; p.ldg = ldg; p.sb = sb; p.b = b; p.n = n;
@@ -630,6 +633,7 @@ int launch_gram_narrow(cudaStream_t st, const uint16_t *A, int64_t lda, const fl
     p.s1_loss = s1 ? s1->loss : -1;
     p.z = s1 ? s1->z : nullptr;
     p.u = s1 ? s1->u : nullptr;
+    p.stamp = g_stamp;
     const int tiles = p.T * (p.T + 1) / 2;
     return launch_pdl(gram_narrow_kernel, dim3(tiles), dim3(kNwThreads), kNwSmem, st, 1, p) == cudaSuccess ? 1 : -1;
 }

@@ -440,7 +440,7 @@ __global__ void loss_finish_kernel(const double *__restrict__ block_partials, in
 }
 
 static int launch_loss_rows(cudaStream_t st, const uint16_t *A, int64_t lda, const float *y, int64_t m, int32_t n, int loss,
-                            const float *x, double *block_partials, int32_t max_blocks)
+                            const float *x, double *block_partials, int32_t max_blocks, int num_sms)
 {
     const int nvec = (n + 7) >> 3;
     const size_t smem_x = sizeof(float) * (size_t)nvec * 8;
@@ -450,11 +450,10 @@ static int launch_loss_rows(cudaStream_t st, const uint16_t *A, int64_t lda, con
     int per_sm = 4;
     if (smem > 0) per_sm = (int)std::min<size_t>(4, (200 * 1024) / (smem + 1024));
     per_sm = std::max(per_sm, 1);
-    int blocks = std::min(max_blocks, kNumSMsB200 * per_sm);
+    int blocks = std::min(max_blocks, num_sms * per_sm);
     auto go = [&](auto kern, int gs) {
         int64_t rows_per_pass = (int64_t)blocks * kLossThreads / gs;
         if (rows_per_pass > m) blocks = (int)std::max<int64_t>(1, (m * gs + kLossThreads - 1) / kLossThreads);
-        if (smem > 48 * 1024) cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         kern<<<blocks, kLossThreads, smem, st>>>(A, lda, y, m, n, loss, x, x_in_smem, block_partials);
     };
     if (nvec >= 32) go(loss_rows_kernel<32>, 32);
@@ -466,31 +465,40 @@ static int launch_loss_rows(cudaStream_t st, const uint16_t *A, int64_t lda, con
     return blocks;
 }
 
+cudaError_t loss_configure()
+{
+    // MODE 1 (4 KB slots) takes x up to kLsMaxN floats; MODE 0 / 2 (slots with labels) have n <= 512
+    const int cap = (int)(128 + sizeof(float) * kLsMaxN + 128 + (size_t)kLsWarps * kLsDepth * kLsSlot);
+    cudaError_t e = cudaFuncSetAttribute(loss_stream_kernel<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, cap);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(loss_stream_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, cap);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(loss_stream_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, cap);
+    // the plain-load kernel keeps x in shared memory up to 96 KB
+    const int xcap = 96 * 1024;
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(loss_rows_kernel<32>, cudaFuncAttributeMaxDynamicSharedMemorySize, xcap);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(loss_rows_kernel<16>, cudaFuncAttributeMaxDynamicSharedMemorySize, xcap);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(loss_rows_kernel<8>, cudaFuncAttributeMaxDynamicSharedMemorySize, xcap);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(loss_rows_kernel<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, xcap);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(loss_rows_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, xcap);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(loss_rows_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, xcap);
+    return e;
+}
+
 // A/lda: the library's 16-byte-aligned layout. X/ldx: the caller's own matrix when it was repacked (else null):
 // narrow unaligned rows are streamed from there (fewer bytes). impl: 0 = choose, 1 = plain-load kernel.
 int launch_loss(cudaStream_t st, const uint16_t *A, int64_t lda, const uint16_t *X, int64_t ldx, const float *y, int64_t m,
                 int32_t n, int loss, const float *x, double *block_partials, int32_t max_blocks, double *result_dev,
-                unsigned *done_counter, int impl)
+                unsigned *done_counter, int impl, int num_sms)
 {
     int blocks;
     const int nvec = (n + 7) >> 3;
-    if (impl == 1 || n > kLsMaxN || max_blocks < kNumSMsB200 || (uintptr_t)y % 16 != 0) {
-        blocks = launch_loss_rows(st, A, lda, y, m, n, loss, x, block_partials, max_blocks);
+    if (impl == 1 || n > kLsMaxN || max_blocks < num_sms || (uintptr_t)y % 16 != 0) {
+        blocks = launch_loss_rows(st, A, lda, y, m, n, loss, x, block_partials, max_blocks, num_sms);
         loss_finish_kernel<<<1, 256, 0, st>>>(block_partials, blocks, m, result_dev);
         return 2;
     } else {
         const size_t fixed = 128 + sizeof(float) * (size_t)nvec * 8 + 128;
         auto go = [&](auto kern, const uint16_t *base, int64_t ld, int rows_per_slot, int gs, int64_t nunits, uint32_t slot_bytes) {
-            static bool attr_set = false;               // the three instantiations share one function type: set all at once
-            if (!attr_set) {
-                // MODE 1 (4 KB slots) takes x up to kLsMaxN floats; MODE 0 / 2 (slots with labels) have n <= 512
-                const int cap = (int)(128 + sizeof(float) * kLsMaxN + 128 + (size_t)kLsWarps * kLsDepth * kLsSlot);
-                cudaFuncSetAttribute(loss_stream_kernel<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, cap);
-                cudaFuncSetAttribute(loss_stream_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, cap);
-                cudaFuncSetAttribute(loss_stream_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, cap);
-                attr_set = true;
-            }
-            blocks = (int)std::max<int64_t>(1, std::min<int64_t>(kNumSMsB200, (nunits + kLsWarps - 1) / kLsWarps));
+            blocks = (int)std::max<int64_t>(1, std::min<int64_t>(num_sms, (nunits + kLsWarps - 1) / kLsWarps));
             kern<<<blocks, kLsThreads, fixed + (size_t)kLsWarps * kLsDepth * slot_bytes, st>>>(
                 base, ld, y, m, n, loss, x, rows_per_slot, gs, block_partials, done_counter, result_dev);
         };

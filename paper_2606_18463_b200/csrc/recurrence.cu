@@ -25,11 +25,12 @@ namespace casgd {
 template <int LOSS>
 __global__ void __launch_bounds__(1024)
 recurrence_cta_kernel(const float *G, int32_t ldg, const float *r, const float *yI,
-                      int32_t s, int32_t b, float alpha, float *z, float *u)
+                      int32_t s, int32_t b, float alpha, float *z, float *u, unsigned long long *stamp)
 {
     extern __shared__ float u_s[];                    // [s*b]
     pdl_trigger();
     pdl_wait();
+    stamp_begin(stamp);
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarps = blockDim.x >> 5;
     for (int j = 0; j < s; ++j) {
         const int len = j * b;
@@ -58,6 +59,7 @@ recurrence_cta_kernel(const float *G, int32_t ldg, const float *r, const float *
         }
         __syncthreads();
     }
+    stamp_end(stamp);
 }
 
 // --------------------------------------------------------------------------- all SMs ---
@@ -95,10 +97,11 @@ __global__ void __launch_bounds__(kRecThreads, 1)
 recurrence_grid_kernel(const float *G, int32_t ldg, const float *r,
                        const float *yI, int32_t s, int32_t b, float alpha, float *z,
                        float *u, unsigned long long *utag, int32_t nrep,
-                       unsigned *epoch, unsigned *done)
+                       unsigned *epoch, unsigned *done, unsigned long long *stamp)
 {
     extern __shared__ __align__(16) float u_s[];        // [s*b]: u as it arrives
     __shared__ int s_last;
+    stamp_begin(stamp);
     const uint32_t tag = *reinterpret_cast<volatile unsigned *>(epoch);
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int W = gridDim.x * kRecWarps;
@@ -222,6 +225,7 @@ recurrence_grid_kernel(const float *G, int32_t ldg, const float *r,
             *epoch = (tag + 1u == 0u) ? 1u : tag + 1u;  // 0 is the value of never-written words
         }
     }
+    stamp_end(stamp);
 }
 
 // --------------------------------------------------------------- one thread-block cluster ---
@@ -287,7 +291,7 @@ template <int LOSS>
 __global__ void __launch_bounds__(kChainThreads, 1)
 recurrence_cluster_kernel(const float *G, int32_t ldg, const float *r,
                           const float *yI, int32_t s, int32_t b, float alpha, float *z,
-                          float *u)
+                          float *u, unsigned long long *stamp)
 {
     extern __shared__ __align__(16) unsigned char chain_smem[];    // u_s[s*b] floats, then bars[s]
     __shared__ volatile float part[2][kChainWarps];
@@ -295,6 +299,7 @@ recurrence_cluster_kernel(const float *G, int32_t ldg, const float *r,
     __shared__ volatile int cons[kChainWarps];                     // last step whose partial the lead has read
     pdl_trigger();
     pdl_wait();
+    stamp_begin(stamp);
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int C = (int)cluster_nctarank(), crank = (int)cluster_ctarank();
     const int sb = s * b;
@@ -411,6 +416,7 @@ recurrence_cluster_kernel(const float *G, int32_t ldg, const float *r,
     }
     __syncthreads();
     cluster_sync_all();                                 // no CTA leaves while others may still store into it
+    stamp_end(stamp);
 }
 
 int recurrence_grid_ctas(const RecWorkspace &ws, int32_t sb)
@@ -438,14 +444,7 @@ static cudaError_t launch_grid(cudaStream_t st, const float *G, int32_t ldg, con
     cfg.attrs = attr;
     cfg.numAttrs = 1;
     auto go = [&](auto kern) {
-        static bool attr_set = false;
-        if (!attr_set) {
-            cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                                 CASGD_MAX_SB * (int)sizeof(float));
-            if (e != cudaSuccess) return e;
-            attr_set = true;
-        }
-        return cudaLaunchKernelEx(&cfg, kern, G, ldg, r, yI, s, b, alpha, z, u, ws.utag, ws.nrep, ws.epoch, ws.done);
+        return cudaLaunchKernelEx(&cfg, kern, G, ldg, r, yI, s, b, alpha, z, u, ws.utag, ws.nrep, ws.epoch, ws.done, g_stamp);
     };
     if (maxr <= 2) return vec ? go(recurrence_grid_kernel<LOSS, 2, true>) : go(recurrence_grid_kernel<LOSS, 2, false>);
     if (maxr <= 4) return vec ? go(recurrence_grid_kernel<LOSS, 4, true>) : go(recurrence_grid_kernel<LOSS, 4, false>);
@@ -458,7 +457,7 @@ static cudaError_t launch_cluster(cudaStream_t st, const float *G, int32_t ldg, 
                                   int32_t s, int32_t b, float alpha, float *z, float *u, int cluster)
 {
     return launch_pdl(recurrence_cluster_kernel<LOSS>, dim3(cluster), dim3(kChainThreads),
-                      sizeof(float) * (size_t)s * b + 8 * (size_t)s, st, cluster, G, ldg, r, yI, s, b, alpha, z, u);
+                      sizeof(float) * (size_t)s * b + 8 * (size_t)s, st, cluster, G, ldg, r, yI, s, b, alpha, z, u, g_stamp);
 }
 
 template <int LOSS>
@@ -507,6 +506,30 @@ int recurrence_max_coresident_ctas(int num_sms)
     return num_sms;                                     // one CTA per SM
 }
 
+template <int LOSS>
+static cudaError_t configure_loss()
+{
+    const int cap = CASGD_MAX_SB * (int)sizeof(float);
+    cudaError_t e = cudaFuncSetAttribute(recurrence_cta_kernel<LOSS>, cudaFuncAttributeMaxDynamicSharedMemorySize, cap);
+    auto set = [&](auto kern) {
+        if (e == cudaSuccess) e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, cap);
+    };
+    set(recurrence_grid_kernel<LOSS, 2, true>);  set(recurrence_grid_kernel<LOSS, 2, false>);
+    set(recurrence_grid_kernel<LOSS, 4, true>);  set(recurrence_grid_kernel<LOSS, 4, false>);
+    set(recurrence_grid_kernel<LOSS, 8, true>);  set(recurrence_grid_kernel<LOSS, 8, false>);
+    set(recurrence_grid_kernel<LOSS, 16, true>); set(recurrence_grid_kernel<LOSS, 16, false>);
+    return e;
+}
+
+// (the cluster kernel's attributes are set by recurrence_cluster_size(), which casgd_init calls on every device)
+cudaError_t recurrence_configure()
+{
+    cudaError_t e = configure_loss<CASGD_LOGISTIC>();
+    if (e == cudaSuccess) e = configure_loss<CASGD_LINEAR>();
+    if (e == cudaSuccess) e = configure_loss<CASGD_POISSON>();
+    return e;
+}
+
 bool recurrence_fuses_update(int32_t s, int32_t b, int32_t ldg, int32_t ldy, const RecWorkspace &ws, int impl)
 {
     // with the update fused in, the cluster kernel beats the one-CTA kernel + a gradient kernel even for tiny G (measured)
@@ -542,17 +565,12 @@ int launch_recurrence(cudaStream_t st, const float *G, int32_t ldg, const float 
     const size_t smem = sizeof(float) * (size_t)s * b;
     const int threads = (b >= 32) ? 1024 : 32 * ((b < 4) ? 4 : b);
     auto go = [&](auto kern) {
-        static bool attr_set = false;
-        if (!attr_set) {
-            cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, CASGD_MAX_SB * (int)sizeof(float));
-            attr_set = true;
-        }
-        launch_pdl(kern, dim3(1), dim3(threads), smem, st, 1, G, ldg, r, yI, s, b, alpha, z, u);
+        return launch_pdl(kern, dim3(1), dim3(threads), smem, st, 1, G, ldg, r, yI, s, b, alpha, z, u, g_stamp);
     };
-    if (loss == CASGD_LOGISTIC) go(recurrence_cta_kernel<CASGD_LOGISTIC>);
-    else if (loss == CASGD_LINEAR) go(recurrence_cta_kernel<CASGD_LINEAR>);
-    else go(recurrence_cta_kernel<CASGD_POISSON>);
-    return 1;
+    const cudaError_t e = loss == CASGD_LOGISTIC ? go(recurrence_cta_kernel<CASGD_LOGISTIC>)
+                        : loss == CASGD_LINEAR  ? go(recurrence_cta_kernel<CASGD_LINEAR>)
+                                                : go(recurrence_cta_kernel<CASGD_POISSON>);
+    return e == cudaSuccess ? 1 : -1;
 }
 
 }  // namespace casgd

@@ -193,7 +193,7 @@ template <int LOSS>
 __global__ void __launch_bounds__(kThreads, 1)
 recurrence_stream_kernel(const float *G, int32_t ldg, const float *r,
                          const float *yI, int32_t s, int32_t b, float alpha, float *z,
-                         float *u, const FusedGrad fg)
+                         float *u, const FusedGrad fg, unsigned long long *stamp)
 {
     extern __shared__ __align__(128) unsigned char rs_smem[];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
@@ -220,6 +220,7 @@ recurrence_stream_kernel(const float *G, int32_t ldg, const float *r,
     }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     pdl_wait();                                         // G, r and y_I come from the Gram and gather kernels
+    stamp_begin(stamp);
 
     // Warp w runs on scheduler w & 3. Critical warps: (group gamma, parity e) -> warp gamma + 4 e.
     const int wsched = warp & 3, wslot = warp >> 2;
@@ -505,23 +506,22 @@ recurrence_stream_kernel(const float *G, int32_t ldg, const float *r,
             }
         }
         REC_TRACE(3);
+        __syncthreads();
+        stamp_end(stamp);
         return;
     }
     __syncthreads();
     cluster_sync_all();                                 // no CTA leaves while others may still store into it
     REC_TRACE(3);
+    stamp_end(stamp);
 }
 
 int stream_cluster_for(int b, int cluster_max);
+constexpr int kStreamSmemCap = 227 * 1024;              // sm_100: opt-in shared memory per CTA
 
 int stream_smem_bytes(int s, int b, int cluster_max)
 {
-    static int max_optin = -1;
-    if (max_optin < 0) {
-        int dev = 0;
-        cudaGetDevice(&dev);
-        if (cudaDeviceGetAttribute(&max_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev) != cudaSuccess) max_optin = 0;
-    }
+    const int max_optin = kStreamSmemCap;
     const int c = stream_cluster_for(b, cluster_max);
     const int need = (int)stream_layout(s, b, (b / kQuad + c - 1) / c).total;
     return need <= max_optin ? need : 0;
@@ -540,30 +540,36 @@ template <int LOSS>
 cudaError_t launch_stream(cudaStream_t st, const float *G, int32_t ldg, const float *r, const float *yI, int32_t s,
                           int32_t b, float alpha, float *z, float *u, int cluster_max, const FusedGrad &fg)
 {
-    static bool attr_set = false;
     const int smem = stream_smem_bytes(s, b, cluster_max);
     if (smem == 0) return cudaErrorInvalidConfiguration;
     auto kern = recurrence_stream_kernel<LOSS>;
-    if (!attr_set) {
-        int dev = 0, max_optin = 0;
-        cudaGetDevice(&dev);
-        cudaDeviceGetAttribute(&max_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev);
-        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, max_optin);
-        if (e != cudaSuccess) return e;
-        e = cudaFuncSetAttribute(kern, cudaFuncAttributeNonPortableClusterSizeAllowed, 1);
-        if (e != cudaSuccess) return e;
-        attr_set = true;
-    }
     const int cluster = stream_cluster_for(b, cluster_max);
-    return launch_pdl(kern, dim3(cluster), dim3(kThreads), (size_t)smem, st, cluster, G, ldg, r, yI, s, b, alpha, z, u, fg);
+    return launch_pdl(kern, dim3(cluster), dim3(kThreads), (size_t)smem, st, cluster, G, ldg, r, yI, s, b, alpha, z, u, fg, g_stamp);
 }
 
 }  // namespace
+
+cudaError_t recurrence_stream_configure()
+{
+    cudaError_t e = cudaSuccess;
+    auto set = [&](auto kern) {
+        if (e == cudaSuccess) e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, kStreamSmemCap);
+        if (e == cudaSuccess) e = cudaFuncSetAttribute(kern, cudaFuncAttributeNonPortableClusterSizeAllowed, 1);
+    };
+    set(recurrence_stream_kernel<CASGD_LOGISTIC>);
+    set(recurrence_stream_kernel<CASGD_LINEAR>);
+    set(recurrence_stream_kernel<CASGD_POISSON>);
+    return e;
+}
 
 // Can the stream kernel run this shape in a cluster of at most `cluster` CTAs?
 bool recurrence_stream_ok(int32_t s, int32_t b, int32_t ldg, int cluster)
 {
     if (cluster <= 0 || b % 4 != 0 || ldg % 4 != 0 || s < 2) return false;
+    // part[] slots are recycled every kPartDepth steps with no back-pressure: a bulk warp's last chunk of step J ends up
+    // to 2 * kChunk columns before column J * b, so it can run 2 * kChunk / b blocks ahead of the chain. That lead plus
+    // the kCritPer steps the critical warps have in flight must stay below kPartDepth (b = 4: 64 blocks -- too many).
+    if (2 * kChunk / b + kCritPer >= kPartDepth) return false;
     const int c = stream_cluster_for(b, cluster);
     if ((b / kQuad + c - 1) / c > kMaxQuadsPerCta) return false;
     return stream_smem_bytes(s, b, cluster) > 0;

@@ -17,7 +17,7 @@ import torch
 
 from paper_2606_18463_b200 import synth
 
-from gpu_common import TOL_LOSS_CALL, compare_last_step, require_cuda
+from gpu_common import TOL_FINAL_LOSS, TOL_LOSS_CALL, compare_last_step, require_cuda
 
 pytestmark = pytest.mark.gpu
 
@@ -41,8 +41,10 @@ def _host_rows(ds, idx):
     return A_bits, y, inv.astype(np.int32)
 
 
-# (config index, s): every config at its headline s of bench.py, plus the largest s of the two tensor-bound sweeps
-FULL = [(0, 4), (1, 16), (1, 32), (2, 32), (3, 16), (3, 64), (4, 32)]
+# (config index, s): every s of every config's sweep (s = 1 runs the margin kernels, s = 4 / 8 the narrow and
+# 128-tile Gram kernels, the largest s the pair kernel)
+FULL = [(0, 4), (1, 1), (1, 4), (1, 16), (1, 32), (2, 1), (2, 8), (2, 32), (3, 1), (3, 8), (3, 16), (3, 64), (4, 1), (4, 8),
+        (4, 32)]
 
 
 @pytest.mark.parametrize("ci,s", FULL)
@@ -69,7 +71,7 @@ def test_second_graph_step_at_full_size_matches_the_oracle(binding, oracle_mod, 
         n0 = cg.launch_count()
         cg.outer_steps(idx_d, x2, s, b, cfg.eta, n_steps=2)
         cg.sync()
-        assert cg.launch_count() - n0 >= 4              # at least two kernels per step (gather+Gram, recurrence+update)
+        assert cg.launch_count() - n0 >= 2              # the library's own kernels ran (at least one per step)
         A_bits, y, local = _host_rows(ds, idx[sb:])
         ref = oracle_mod.outer_step_gram(A_bits, y, local, x1_host.astype(np.float64), s, b, cfg.eta, cfg.loss, shadow=True)
         compare_last_step(oracle_mod, cg, ref, y[local], x1_host, x2, s, b, cfg.eta, cfg.loss, binding)
@@ -118,5 +120,41 @@ def test_full_size_loss_is_the_row_weighted_mean_of_slice_losses(binding, oracle
                 parts.append((e - a, cs.loss(x)))
         F_parts = sum(r * f for r, f in parts) / cfg.m
         assert abs(F - F_parts) <= 2 * TOL_LOSS_CALL * abs(F_parts)
+    finally:
+        del ds
+
+
+@pytest.mark.parametrize("ci", [1, 2, 3, 4])
+def test_full_size_training_loss_matches_the_trajectory_oracle(binding, oracle_mod, ci):
+    """BASELINE.json:north_star "the training loss after the configured epochs is within 0.5% of the oracle's"
+    (threshold of PAPER.md:L297 sec. 7.2), at FULL size: configs 2-5, every s of the sweep, the configured epochs,
+    from x = 0, through casgd_outer_steps (CUDA-graph replay, as bench.py runs it). The trajectory oracle is the
+    sequential form O2 (pinned equal to the Gram form O1 in tests/test_oracle_*.py) on the same BF16
+    bits, labels and index stream, the whole matrix brought to the host once. With the epoch rule of DESIGN.md every s
+    consumes the same mini-batches, so the final losses of different s also agree with each other."""
+    cfg = synth.config(ci)
+    free, _ = torch.cuda.mem_get_info()
+    need = cfg.m * max(cfg.n, 32) * 2 * 1.3 + (1 << 30)
+    assert free > need, f"{cfg.name} needs {need / 1e9:.1f} GB of device memory, {free / 1e9:.1f} GB free"
+    ds = synth.make_dataset(cfg, seed=42, device="cuda")
+    try:
+        A_bits, y = ds.X_bits_numpy(), ds.y_numpy()
+        idx = synth.training_indices(cfg, seed=42)
+        idx_d = torch.from_numpy(idx).cuda()
+        F0 = {0: math.log(2.0), 1: float(np.mean(y.astype(np.float64) ** 2) / 2), 2: 1.0}[cfg.loss]
+        losses = []
+        with binding.Casgd(ds.X_bf16, ds.y, cfg.loss) as cg:
+            for s in cfg.s_list:
+                assert len(idx) % (s * cfg.b) == 0
+                x = torch.zeros(cfg.n, device="cuda")
+                cg.outer_steps(idx_d, x, s, cfg.b, cfg.eta)
+                cg.sync()
+                F_gpu = cg.loss(x)
+                x_ref = oracle_mod.train(A_bits, y, idx, np.zeros(cfg.n), s, cfg.b, cfg.eta, cfg.loss, shadow=True)
+                F_ref = oracle_mod.full_loss(A_bits, y, x_ref, cfg.loss)
+                assert F_ref < F0, (s, F_ref, F0)                               # it trained
+                assert abs(F_gpu - F_ref) <= TOL_FINAL_LOSS * abs(F_ref), (cfg.name, s, F_gpu, F_ref)
+                losses.append(F_gpu)
+        assert max(losses) - min(losses) <= 1e-3 * abs(losses[0]), losses
     finally:
         del ds

@@ -131,6 +131,8 @@ RECURRENCE = [
     (0, 9000, 24, 21, 20),       # b = 20: blocks straddle the 128-column chunks; CTAs own 2 or 1 rows per block
     (3, 5000, 40, 130, 16),      # b = 16: one row per CTA, 129 hops, eight blocks per chunk
     (0, 9000, 24, 40, 96),       # b = 96: a "bulk" chunk can hold part of the newest block
+    (0, 3000, 16, 200, 4),       # b = 4: bulk warps run 64 blocks ahead of the chain (the stream kernel declines)
+    (3, 5000, 40, 130, 8),       # b = 8: 32 blocks ahead, inside the stream kernel's partial-sum ring
 ]
 
 
