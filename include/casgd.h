@@ -135,10 +135,13 @@ int casgd_sync(casgd_ctx *c);
  *                  always; every k <= i when CASGD_OPT_GRAM_FULL_LOWER is set. The rest is unspecified.
  *   CASGD_DBG_R    sb FP32   CASGD_DBG_Z sb FP32   CASGD_DBG_U sb FP32
  *   CASGD_DBG_XBF  n  BF16 bits: the shadow AFTER the step (bf16 of the updated x)
+ *   CASGD_DBG_STAMPS  64 x 8 x 2 uint64: with CASGD_OPT_STAMPS, {first-CTA start, last-CTA end} in %globaltimer ns of
+ *                  stage g (CASGD_STAGE_*) of step h of the last graph casgd_outer_steps replayed, at [h][g][0..1];
+ *                  {~0, 0} where a stage did not run
  * dst_bytes must equal the size implied above, else CASGD_EINVAL. */
 typedef enum {
     CASGD_DBG_Y = 0, CASGD_DBG_YLAB = 1, CASGD_DBG_G = 2, CASGD_DBG_R = 3, CASGD_DBG_Z = 4,
-    CASGD_DBG_U = 5, CASGD_DBG_XBF = 6
+    CASGD_DBG_U = 5, CASGD_DBG_XBF = 6, CASGD_DBG_STAMPS = 7
 } casgd_debug_what;
 int casgd_debug_export(casgd_ctx *c, int what, void *dst_host, int64_t dst_bytes);
 
@@ -171,19 +174,31 @@ int casgd_debug_export(casgd_ctx *c, int what, void *dst_host, int64_t dst_bytes
  *                              launches of (last end - first start) -- measured INSIDE the CUDA-graph replays that
  *                              casgd_outer_steps runs (unlike CASGD_OPT_PROFILE, which launches directly). Setting the
  *                              option (to 0 or 1) clears the totals.
+ *   CASGD_OPT_OVERLAP          how the CUDA graphs of casgd_outer_steps schedule consecutive outer iterations (two Y / G
+ *                              stages; results do not depend on the graph length or on single-step calls in a mode):
+ *                              0 = kernels strictly in sequence; 1 = a step that has a gather kernel gathers the NEXT
+ *                              step's rows (Alg. 1 line 2 of iteration t + 1 needs no result of iteration t) on a side
+ *                              branch, beside its own recurrence and update; 2 (default) = pipelined: G(t+1) = Y Y^T
+ *                              needs no result of iteration t either, so gather + Gram of iteration t + 1 run on a side
+ *                              branch (on all but CASGD_OPT_CHAIN_SMS SMs) beside margin -> recurrence -> update of
+ *                              iteration t; the margin r = Y x_bf, which does need x(t+1), is then a kernel of its own
+ *                              (CASGD_STAGE_MARGIN) instead of extra B-operand rows of the Gram.
+ *   CASGD_OPT_CHAIN_SMS        SMs left to the margin / recurrence / update chain in the pipelined schedule (the Gram and
+ *                              gather kernels are sized for the rest). 0 (default) = chosen per shape.
  *   CASGD_OPT_LOSS_IMPL        0 = casgd_loss streams A through per-warp cp.async.bulk shared-memory rings
  *                              (default; n <= 8192), 1 = the plain 16-byte-load kernel. */
 typedef enum {
     CASGD_OPT_GRAM_IMPL = 0, CASGD_OPT_GRAM_FULL_LOWER = 1, CASGD_OPT_PROFILE = 2, CASGD_OPT_NO_GRAPH = 3,
     CASGD_OPT_GRAM_KSPLIT = 4, CASGD_OPT_RECURRENCE_IMPL = 5, CASGD_OPT_LOSS_IMPL = 6, CASGD_OPT_NO_FUSED_UPDATE = 7,
-    CASGD_OPT_STAMPS = 8
+    CASGD_OPT_STAMPS = 8, CASGD_OPT_OVERLAP = 9, CASGD_OPT_CHAIN_SMS = 10
 } casgd_option;
 int casgd_set_option(casgd_ctx *c, int option, int64_t value);
 
-/* Stages of an outer step (plus shadow rebuilds = OTHER, and casgd_loss), for casgd_stage_times. */
+/* Stages of an outer step (plus shadow rebuilds = OTHER, and casgd_loss), for casgd_stage_times. MARGIN has launches of
+ * its own only in the pipelined schedule (CASGD_OPT_OVERLAP = 2); otherwise r comes out of the Gram kernel. */
 typedef enum {
     CASGD_STAGE_GATHER = 0, CASGD_STAGE_GRAM = 1, CASGD_STAGE_RECURRENCE = 2, CASGD_STAGE_GRADIENT = 3,
-    CASGD_STAGE_OTHER = 4, CASGD_STAGE_LOSS = 5, CASGD_NUM_STAGES = 6
+    CASGD_STAGE_MARGIN = 4, CASGD_STAGE_OTHER = 5, CASGD_STAGE_LOSS = 6, CASGD_NUM_STAGES = 7
 } casgd_stage;
 
 /* With CASGD_OPT_PROFILE set: total device milliseconds and launch counts per stage accumulated since

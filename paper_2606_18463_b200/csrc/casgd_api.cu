@@ -4,6 +4,7 @@
 #include <cstdarg>
 #include <cstdio>
 #include <cstring>
+#include <functional>
 #include <map>
 #include <new>
 #include <tuple>
@@ -15,6 +16,8 @@ using namespace casgd;
 
 namespace casgd {
 thread_local unsigned long long *g_stamp = nullptr;
+thread_local bool g_plain_launch = false;
+thread_local cudaEvent_t g_completion_event = nullptr;
 }
 
 namespace {
@@ -37,6 +40,7 @@ struct GraphKey {
 struct GraphEntry {
     cudaGraphExec_t exec;
     int64_t kernels;
+    int last_buf;                       // Y stage its last step used (casgd_debug_export reads that one)
 };
 
 inline int64_t round_up(int64_t v, int64_t q) { return (v + q - 1) / q * q; }
@@ -47,6 +51,9 @@ struct casgd_ctx {
     int device = 0;
     cudaStream_t stream = nullptr;
     cudaStream_t capture_stream = nullptr;
+    cudaStream_t side_stream = nullptr;       // graph capture only: the branch that gathers the next step's rows
+    cudaEvent_t ev_fork = nullptr, ev_join = nullptr;
+    cudaEvent_t ev_gather[2] = {nullptr, nullptr}, ev_gram[2] = {nullptr, nullptr}, ev_grad = nullptr, ev_rec_launch = nullptr;
     // dataset
     const uint16_t *A = nullptr;      // BF16 bits, row stride lda (borrowed or owned)
     uint16_t *A_owned = nullptr;
@@ -61,8 +68,10 @@ struct casgd_ctx {
     // per-step workspaces, sized for rows_alloc rows
     int32_t rows_alloc = 0;
     int32_t ldy = 0, ldg = 0;
-    uint16_t *Y = nullptr;
-    float *yI = nullptr, *G = nullptr, *r = nullptr, *z = nullptr, *u = nullptr;
+    uint16_t *Y = nullptr;            // TWO stages of rows_alloc rows: step h of a graph uses stage h & 1, so that the
+                                      // next step's gather can run beside this step's recurrence and update
+    float *yI = nullptr, *G = nullptr, *r = nullptr, *z = nullptr, *u = nullptr;     // G, y_I: two stages as well
+    float *r_scratch = nullptr;       // pipelined schedule: where the Gram kernels' fused margin (of a stale x) goes
     uint16_t *xbf = nullptr;          // BF16 shadow of x: [16 x ldxb], row 0 = bf16(x), the rest zero
     int32_t ldxb = 0;
     const float *shadow_of = nullptr;
@@ -80,15 +89,17 @@ struct casgd_ctx {
     int64_t idx_stage_cap = 0;
     float *x_stage = nullptr;
     // last step, for debug export
-    int32_t last_s = 0, last_b = 0;
+    int32_t last_s = 0, last_b = 0, last_buf = 0;
     // options
-    unsigned long long *stamps = nullptr;     // CASGD_OPT_STAMPS: [kStampSteps * 4][2] slots, then accum_ns[4], count[4]
+    unsigned long long *stamps = nullptr;     // CASGD_OPT_STAMPS: [kStampSteps * 8][2] slots, accum_ns[8], count[8], raw copy of the slots
     int cur_slot_step = 0;                    // step index (inside the graph being captured) the next stage stamps into
     int64_t opt_stamps = 0;
-    int64_t opt_gram_impl = 0, opt_full_lower = 0, opt_profile = 0, opt_no_graph = 0, opt_ksplit = 0, opt_rec_impl = 0, opt_loss_impl = 0, opt_no_fuse = 0;
+    int64_t opt_gram_impl = 0, opt_full_lower = 0, opt_profile = 0, opt_no_graph = 0, opt_ksplit = 0, opt_rec_impl = 0, opt_loss_impl = 0, opt_no_fuse = 0, opt_overlap = 2, opt_chain_sms = 0;
     GramTcPlan *tc_plan = nullptr;
     GramPairPlan *pair_plan = nullptr;
+    int pair_plan_sms = 0;
     int num_sms = 0;
+    int gram_sms = 0, chain_sms = 0;  // SM budgets of the two branches for the shape being enqueued (both num_sms unless pipelined)
     int cur_gram = 0, cur_bn = 0;     // Gram kernel of the shape being enqueued: 1 = CUDA cores, 2 = 128x128 tiles, 3 = CTA pairs
     std::map<GraphKey, GraphEntry> graphs;
     std::vector<StageEvent> events;
@@ -102,7 +113,11 @@ namespace {
 
 constexpr int kRecReplicas = 8;
 constexpr int kStampSteps = 64;                         // the longest graph
-constexpr int kStampWords = kStampSteps * 4 * 2 + 8;    // slots, accum_ns[4], count[4]
+constexpr int kSlotStages = 8;                          // stamp slots per step (stages 0 .. 4 are stamped)
+constexpr int kStampSlots = kStampSteps * kSlotStages;
+constexpr int kStampAcc = 2 * kStampSlots;              // accum_ns[8], then count[8], then the raw copy of the last collect
+constexpr int kStampRaw = kStampAcc + 16;
+constexpr int kStampWords = kStampRaw + 2 * kStampSlots;
 const unsigned kEpochInit[2] = {1u, 0u};                // {epoch, done}
 
 int fail(casgd_ctx *c, int code, const char *fmt, ...)
@@ -135,8 +150,8 @@ void free_step_workspace(casgd_ctx *c)
     drop_graphs(c);
     if (c->tc_plan) { gram_tc_plan_destroy(c->tc_plan); c->tc_plan = nullptr; }
     if (c->pair_plan) { gram_pair_plan_destroy(c->pair_plan); c->pair_plan = nullptr; }
-    cudaFree(c->Y); cudaFree(c->yI); cudaFree(c->G); cudaFree(c->r); cudaFree(c->z); cudaFree(c->u);
-    c->Y = nullptr; c->yI = c->G = c->r = c->z = c->u = nullptr;
+    cudaFree(c->Y); cudaFree(c->yI); cudaFree(c->G); cudaFree(c->r); cudaFree(c->z); cudaFree(c->u); cudaFree(c->r_scratch);
+    c->Y = nullptr; c->yI = c->G = c->r = c->z = c->u = c->r_scratch = nullptr;
     c->rows_alloc = 0;
 }
 
@@ -145,17 +160,19 @@ int ensure_workspace(casgd_ctx *c, int32_t sb)
     if (sb <= c->rows_alloc) return CASGD_OK;
     CK(cudaStreamSynchronize(c->stream));
     free_step_workspace(c);
-    const int32_t rows = (int32_t)round_up(sb, kTile);
+    const int32_t rows = (int32_t)round_up(sb, 2 * kTile);   // whole 256-row pair tiles: a tile never straddles the two stages
     c->ldg = rows;
-    CK(cudaMalloc(&c->Y, sizeof(uint16_t) * (size_t)rows * c->ldy));
-    CK(cudaMalloc(&c->yI, sizeof(float) * rows));
-    CK(cudaMalloc(&c->G, sizeof(float) * (size_t)rows * rows));
+    CK(cudaMalloc(&c->Y, sizeof(uint16_t) * (size_t)2 * rows * c->ldy));
+    CK(cudaMalloc(&c->yI, sizeof(float) * 2 * rows));
+    CK(cudaMalloc(&c->G, sizeof(float) * (size_t)2 * rows * rows));
     CK(cudaMalloc(&c->r, sizeof(float) * rows));
+    CK(cudaMalloc(&c->r_scratch, sizeof(float) * rows));
     CK(cudaMalloc(&c->z, sizeof(float) * rows));
     CK(cudaMalloc(&c->u, sizeof(float) * rows));
-    CK(cudaMemsetAsync(c->Y, 0, sizeof(uint16_t) * (size_t)rows * c->ldy, c->stream));
-    CK(cudaMemsetAsync(c->G, 0, sizeof(float) * (size_t)rows * rows, c->stream));
-    CK(cudaMemsetAsync(c->yI, 0, sizeof(float) * rows, c->stream));
+    CK(cudaMemsetAsync(c->Y, 0, sizeof(uint16_t) * (size_t)2 * rows * c->ldy, c->stream));
+    CK(cudaMemsetAsync(c->G, 0, sizeof(float) * (size_t)2 * rows * rows, c->stream));
+    CK(cudaMemsetAsync(c->r_scratch, 0, sizeof(float) * rows, c->stream));
+    CK(cudaMemsetAsync(c->yI, 0, sizeof(float) * 2 * rows, c->stream));
     CK(cudaMemsetAsync(c->r, 0, sizeof(float) * rows, c->stream));
     CK(cudaMemsetAsync(c->z, 0, sizeof(float) * rows, c->stream));
     CK(cudaMemsetAsync(c->u, 0, sizeof(float) * rows, c->stream));
@@ -181,7 +198,7 @@ struct StageTimer {
     bool on;
     StageTimer(casgd_ctx *c_, int stage_) : c(c_), stage(stage_), on(c_->opt_profile != 0)
     {
-        g_stamp = (c->opt_stamps && c->stamps && stage < 4) ? c->stamps + 2 * (c->cur_slot_step * 4 + stage) : nullptr;
+        g_stamp = (c->opt_stamps && c->stamps && stage <= CASGD_STAGE_MARGIN) ? c->stamps + 2 * (c->cur_slot_step * kSlotStages + stage) : nullptr;
         if (!on) return;
         ev.stage = stage;
         cudaEventCreate(&ev.start);
@@ -199,65 +216,218 @@ struct StageTimer {
     }
 };
 
-// Enqueue one outer iteration (Alg. 1 lines 2-17). `ind` non-null: graph-replay addressing.
-int enqueue_step(casgd_ctx *c, cudaStream_t st, const int32_t *idx, const StepParams *ind, int64_t idx_off, float *x,
-                 int32_t s, int32_t b, float eta, int64_t *kernels)
+// Where a step finds its rows. `buf`: which of the two Y / y_I / G stages it uses; `gathered`: an earlier step's side branch
+// has already gathered them; `next_idx_off` >= 0: this step gathers the NEXT step's rows (Alg. 1 line 2 of iteration t + 1
+// depends on no result of iteration t) into the other stage on c->side_stream, beside its own recurrence and update.
+struct StepIo {
+    int buf = 0;
+    bool gathered = false;
+    int64_t next_idx_off = -1;
+};
+
+inline bool step_is_s1(const casgd_ctx *c, int32_t s)
 {
-    const int32_t sb = s * b;
-    const float alpha = eta / (float)b;
-    int k;
     // s = 1: no Gram, no correction, u = l'(r, y_I): one kernel computes the margin and applies l' (the fused
     // gather + Gram kernel's epilogue for n <= 64, a warp-per-row kernel otherwise); a forced Gram kernel still runs
-    const bool s1 = s == 1 && !c->opt_no_fuse && (c->cur_gram == 4 || c->opt_gram_impl == 0);
-    const S1Fuse s1f{c->loss, c->yI, c->z, c->u};
-    if (s1 && c->cur_gram != 4) {
-        // wide rows: gather + margin + l' in one warp-per-row kernel (there is no Gram at s = 1)
-        StageTimer t(c, CASGD_STAGE_GRAM);
-        k = launch_margin_s1(st, c->A, c->lda, c->y, c->m, c->n, idx, ind, idx_off, b, c->loss, c->xbf, c->Y, c->ldy, c->yI,
-                             c->r, c->z, c->u, c->err_flag);
-        t.done(k); *kernels += k;
-    } else if (c->cur_gram != 4) {
-        StageTimer t(c, CASGD_STAGE_GATHER);
-        k = launch_gather(st, c->A, c->lda, c->y, c->m, c->n, idx, ind, idx_off, sb, c->Y, c->ldy, c->yI, c->err_flag, c->num_sms);
-        t.done(k); *kernels += k;
-    }
-    if (!(s1 && c->cur_gram != 4)) {
-        StageTimer t(c, CASGD_STAGE_GRAM);
-        if (c->cur_gram == 4) {
-            k = launch_gram_narrow(st, c->A, c->lda, c->y, c->m, c->n, idx, ind, idx_off, sb, b, c->xbf, c->ldxb, c->Y, c->ldy,
-                                   c->yI, c->G, c->ldg, c->r, (int)c->opt_full_lower, c->err_flag, s1 ? &s1f : nullptr);
-            if (k < 0) return fail(c, CASGD_ECUDA, "gram_narrow launch: %s", cudaGetErrorString(cudaGetLastError()));
-        } else if (c->cur_gram == 1) {
-            k = launch_gram_simt(st, c->Y, c->ldy, c->n, sb, b, c->xbf, c->G, c->ldg, c->r, (int)c->opt_full_lower);
-        } else if (c->cur_gram == 3) {
-            k = launch_gram_pair(st, c->pair_plan, sb, b, c->G, c->ldg, c->r, (int)c->opt_full_lower, c->cur_bn,
-                                 (int)c->opt_ksplit, c->err, sizeof c->err);
-            if (k < 0) return CASGD_ECUDA;
-        } else {
-            if (!c->tc_plan) {
-                c->tc_plan = gram_tc_plan_create(c->Y, c->ldy, c->n, c->rows_alloc, c->xbf, c->ldxb, c->err, sizeof c->err);
-                if (!c->tc_plan) return CASGD_ECUDA;
-            }
-            k = launch_gram_tc(st, c->tc_plan, sb, b, c->G, c->ldg, c->r, (int)c->opt_full_lower, (int)c->opt_ksplit, c->num_sms, c->err, sizeof c->err);
-            if (k < 0) return CASGD_ECUDA;
-        }
-        t.done(k); *kernels += k;
-    }
+    return s == 1 && !c->opt_no_fuse && (c->cur_gram == 4 || c->opt_gram_impl == 0);
+}
+// pipelined schedule: not at s = 1 (no Gram), and not with the recurrence kernels that want the whole chip or trigger
+// their dependents early (the grid-wide cooperative kernel, the plain-load cluster kernel)
+inline bool pipelined_mode(const casgd_ctx *c, int32_t s, int32_t b)
+{
+    if (c->opt_overlap != 2 || s == 1 || c->num_sms < 64) return false;
     const bool fused = !c->opt_no_fuse && recurrence_fuses_update(s, b, c->ldg, c->ldy, c->rws, (int)c->opt_rec_impl);
-    if (!s1) {
+    const int k = recurrence_kernel_choice(s, b, c->ldg, c->rws, (int)c->opt_rec_impl, fused);
+    return k == 1 || k == 4;
+}
+
+// ---- the stages of one outer iteration (Alg. 1 lines 2-17), each on the stream it is given ----
+
+int stage_gather(casgd_ctx *c, cudaStream_t st, const int32_t *idx, const StepParams *ind, int64_t idx_off, int32_t sb, int buf,
+                 int sms, int64_t *kernels)
+{
+    StageTimer t(c, CASGD_STAGE_GATHER);
+    const int k = launch_gather(st, c->A, c->lda, c->y, c->m, c->n, idx, ind, idx_off, sb, c->Y + (size_t)buf * c->rows_alloc * c->ldy,
+                                c->ldy, c->yI + (size_t)buf * c->rows_alloc, c->err_flag, sms);
+    t.done(k); *kernels += k;
+    return CASGD_OK;
+}
+
+// G (and r, into `r_out`) of the rows in stage `buf`; the narrow kernel gathers them itself
+int stage_gram(casgd_ctx *c, cudaStream_t st, const int32_t *idx, const StepParams *ind, int64_t idx_off, int32_t s, int32_t b,
+               int buf, float *r_out, int64_t *kernels)
+{
+    const int32_t sb = s * b;
+    uint16_t *Y = c->Y + (size_t)buf * c->rows_alloc * c->ldy;
+    float *yI = c->yI + (size_t)buf * c->rows_alloc;
+    float *G = c->G + (size_t)buf * c->rows_alloc * c->rows_alloc;
+    const int32_t row_base = buf * c->rows_alloc;
+    const S1Fuse s1f{c->loss, yI, c->z, c->u};
+    int k;
+    StageTimer t(c, CASGD_STAGE_GRAM);
+    // r_out == nullptr: no margin wanted (pipelined schedule). The tcgen05 tile kernels then leave the x_bf rows out;
+    // the narrow and CUDA-core kernels write theirs (of a stale x) to a scratch vector
+    if (!r_out && (c->cur_gram == 4 || c->cur_gram == 1)) r_out = c->r_scratch;
+    if (c->cur_gram == 4) {
+        k = launch_gram_narrow(st, c->A, c->lda, c->y, c->m, c->n, idx, ind, idx_off, sb, b, c->xbf, c->ldxb, Y, c->ldy,
+                               yI, G, c->ldg, r_out, (int)c->opt_full_lower, c->err_flag, step_is_s1(c, s) ? &s1f : nullptr);
+        if (k < 0) return fail(c, CASGD_ECUDA, "gram_narrow launch: %s", cudaGetErrorString(cudaGetLastError()));
+    } else if (c->cur_gram == 1) {
+        k = launch_gram_simt(st, Y, c->ldy, c->n, sb, b, c->xbf, G, c->ldg, r_out, (int)c->opt_full_lower);
+    } else if (c->cur_gram == 3) {
+        k = launch_gram_pair(st, c->pair_plan, row_base, sb, b, G, c->ldg, r_out, (int)c->opt_full_lower, c->cur_bn,
+                             (int)c->opt_ksplit, c->err, sizeof c->err);
+        if (k < 0) return CASGD_ECUDA;
+    } else {
+        if (!c->tc_plan) {
+            c->tc_plan = gram_tc_plan_create(c->Y, c->ldy, c->n, 2 * c->rows_alloc, c->xbf, c->ldxb, c->err, sizeof c->err);
+            if (!c->tc_plan) return CASGD_ECUDA;
+        }
+        k = launch_gram_tc(st, c->tc_plan, row_base, sb, b, G, c->ldg, r_out, (int)c->opt_full_lower, (int)c->opt_ksplit, c->gram_sms, c->err, sizeof c->err);
+        if (k < 0) return CASGD_ECUDA;
+    }
+    t.done(k); *kernels += k;
+    return CASGD_OK;
+}
+
+int stage_margin(casgd_ctx *c, cudaStream_t st, int32_t sb, int buf, int64_t *kernels)
+{
+    StageTimer t(c, CASGD_STAGE_MARGIN);
+    const int k = launch_margin(st, c->Y + (size_t)buf * c->rows_alloc * c->ldy, c->ldy, sb, c->xbf, c->r, c->chain_sms);
+    t.done(k); *kernels += k;
+    return CASGD_OK;
+}
+
+// recurrence and update of the rows in stage `buf`
+int stage_chain(casgd_ctx *c, cudaStream_t st, float *x, const StepParams *ind, int32_t s, int32_t b, float alpha, int buf,
+                bool late_trigger, const std::function<void()> &after_recurrence, int64_t *kernels)
+{
+    const int32_t sb = s * b;
+    uint16_t *Y = c->Y + (size_t)buf * c->rows_alloc * c->ldy;
+    float *yI = c->yI + (size_t)buf * c->rows_alloc;
+    float *G = c->G + (size_t)buf * c->rows_alloc * c->rows_alloc;
+    int k;
+    const bool fused = !c->opt_no_fuse && recurrence_fuses_update(s, b, c->ldg, c->ldy, c->rws, (int)c->opt_rec_impl);
+    if (!step_is_s1(c, s)) {
         StageTimer t(c, CASGD_STAGE_RECURRENCE);
-        const FusedUpdate fu{c->Y, c->ldy, c->n, x, ind, c->xbf};
-        k = launch_recurrence(st, c->G, c->ldg, c->r, c->yI, s, b, alpha, c->loss, c->z, c->u, c->rws,
+        const FusedUpdate fu{Y, c->ldy, c->n, x, ind, c->xbf};
+        c->rws.late_trigger = late_trigger;
+        k = launch_recurrence(st, G, c->ldg, c->r, yI, s, b, alpha, c->loss, c->z, c->u, c->rws,
                               (int)c->opt_rec_impl, fused ? &fu : nullptr);
+        g_completion_event = nullptr;
         if (k < 0) return fail(c, CASGD_ECUDA, "recurrence launch: %s", cudaGetErrorString(cudaGetLastError()));
         t.done(k); *kernels += k;
     }
+    if (after_recurrence) after_recurrence();
     if (!fused) {
         StageTimer t(c, CASGD_STAGE_GRADIENT);
-        k = launch_gradient_bf16(st, c->Y, c->ldy, c->n, sb, c->u, alpha, x, ind, c->xbf, c->gws);
+        c->gws.num_sms = c->chain_sms;
+        k = launch_gradient_bf16(st, Y, c->ldy, c->n, sb, c->u, alpha, x, ind, c->xbf, c->gws);
         t.done(k); *kernels += k;
     }
     return CASGD_OK;
+}
+
+// Enqueue one outer iteration (Alg. 1 lines 2-17) on one stream (plus, with io.next_idx_off, the next step's gather on the
+// side branch). `ind` non-null: graph-replay addressing.
+int enqueue_step(casgd_ctx *c, cudaStream_t st, const int32_t *idx, const StepParams *ind, int64_t idx_off, float *x,
+                 int32_t s, int32_t b, float eta, int64_t *kernels, const StepIo &io = StepIo{})
+{
+    const int32_t sb = s * b;
+    const float alpha = eta / (float)b;
+    int rc;
+    c->last_buf = io.buf;
+    const bool s1 = step_is_s1(c, s);
+    const bool split_margin = pipelined_mode(c, s, b);     // same kernels as the pipelined graphs: bit-identical iterates
+    if (s1 && c->cur_gram != 4) {
+        // wide rows: gather + margin + l' in one warp-per-row kernel (there is no Gram at s = 1)
+        StageTimer t(c, CASGD_STAGE_GRAM);
+        const int k = launch_margin_s1(st, c->A, c->lda, c->y, c->m, c->n, idx, ind, idx_off, b, c->loss, c->xbf,
+                                       c->Y + (size_t)io.buf * c->rows_alloc * c->ldy, c->ldy, c->yI + (size_t)io.buf * c->rows_alloc,
+                                       c->r, c->z, c->u, c->err_flag);
+        t.done(k); *kernels += k;
+    } else {
+        if (c->cur_gram != 4 && !io.gathered && (rc = stage_gather(c, st, idx, ind, idx_off, sb, io.buf, c->gram_sms, kernels))) return rc;
+        if ((rc = stage_gram(c, st, idx, ind, idx_off, s, b, io.buf, split_margin ? nullptr : c->r, kernels))) return rc;
+        if (split_margin && (rc = stage_margin(c, st, sb, io.buf, kernels))) return rc;
+    }
+    const bool side = io.next_idx_off >= 0;
+    std::function<void()> none;
+    if (side) {
+        // the next step's rows, on the side branch of the graph being captured
+        cudaEventRecord(c->ev_fork, st);
+        cudaStreamWaitEvent(c->side_stream, c->ev_fork, 0);
+        const int saved_step = c->cur_slot_step;
+        c->cur_slot_step = saved_step + 1;              // (stamps: the gather belongs to the next step)
+        // the recurrence cluster holds up to 16 SMs: a gather sized for all SMs would leave 16 CTAs waiting for it to
+        // finish (measured: 42 us instead of 12)
+        rc = stage_gather(c, c->side_stream, idx, ind, io.next_idx_off, sb, io.buf ^ 1, c->num_sms > 32 ? c->num_sms - 16 : c->num_sms, kernels);
+        c->cur_slot_step = saved_step;
+        if (rc) return rc;
+        cudaEventRecord(c->ev_join, c->side_stream);
+    }
+    if ((rc = stage_chain(c, st, x, ind, s, b, alpha, io.buf, side, none, kernels))) return rc;
+    if (side) cudaStreamWaitEvent(st, c->ev_join, 0);   // the next Gram needs the side branch's rows
+    return CASGD_OK;
+}
+
+// CASGD_OPT_OVERLAP = 2: `len` outer iterations as a two-branch graph. G(t+1) = Y(t+1) Y(t+1)^T needs nothing iteration t
+// computes, so the side branch runs gather(t+1) -> Gram(t+1) on gram_sms SMs while the main branch runs
+// margin(t) -> recurrence(t) -> update(t) on the rest; only r(t+1) = Y(t+1) x_bf(t+1) has to wait for the update.
+//   side:  gather(h+1) after update(h-1) (it overwrites stage (h+1) & 1, last read by iteration h-1);
+//          Gram(h+1) once every CTA of recurrence(h) is running (launch-completion event: the cluster needs its 16 SMs
+//          of one GPC before the Gram's persistent CTAs fill the chip)
+//   main:  margin(h) after gather(h); recurrence(h) after Gram(h); update(h)
+// Side-branch kernels are launched without programmatic serialisation and the recurrence triggers its dependents late:
+// a kernel that becomes resident early only to wait would hold SMs the other branch needs.
+int capture_pipelined(casgd_ctx *c, int32_t s, int32_t b, float eta, int32_t len, int64_t *kernels)
+{
+    cudaStream_t M = c->capture_stream, S = c->side_stream;
+    const int32_t sb = s * b;
+    const float alpha = eta / (float)b;
+    int rc = CASGD_OK;
+    cudaEventRecord(c->ev_fork, M);
+    cudaStreamWaitEvent(S, c->ev_fork, 0);
+    auto side_step = [&](int h, bool wait_update, bool wait_rec_launch) -> int {
+        const int buf = h & 1;
+        c->cur_slot_step = h;
+        g_plain_launch = true;
+        int rc2 = CASGD_OK;
+        if (wait_update) cudaStreamWaitEvent(S, c->ev_grad, 0);
+        if (c->cur_gram != 4) {
+            rc2 = stage_gather(c, S, nullptr, c->ind, (int64_t)h * sb, sb, buf, c->gram_sms, kernels);
+            cudaEventRecord(c->ev_gather[buf], S);
+        }
+        if (wait_rec_launch) cudaStreamWaitEvent(S, c->ev_rec_launch, 0);
+        if (!rc2) rc2 = stage_gram(c, S, nullptr, c->ind, (int64_t)h * sb, s, b, buf, nullptr, kernels);
+        cudaEventRecord(c->ev_gram[buf], S);
+        if (c->cur_gram == 4) cudaEventRecord(c->ev_gather[buf], S);
+        g_plain_launch = false;
+        return rc2;
+    };
+    rc = side_step(0, false, false);
+    for (int32_t h = 0; h < len && rc == CASGD_OK; ++h) {
+        const int buf = h & 1;
+        c->cur_slot_step = h;
+        cudaStreamWaitEvent(M, c->ev_gather[buf], 0);
+        if ((rc = stage_margin(c, M, sb, buf, kernels))) break;
+        cudaStreamWaitEvent(M, c->ev_gram[buf], 0);
+        const bool more = h + 1 < len;
+        if (more) g_completion_event = c->ev_rec_launch;
+        int rc_side = CASGD_OK;
+        std::function<void()> after = [&]() {
+            if (more) rc_side = side_step(h + 1, h >= 1, true);
+            c->cur_slot_step = h;
+        };
+        rc = stage_chain(c, M, nullptr, c->ind, s, b, alpha, buf, true, after, kernels);
+        if (!rc) rc = rc_side;
+        cudaEventRecord(c->ev_grad, M);
+    }
+    c->last_buf = (len - 1) & 1;
+    c->cur_slot_step = 0;
+    g_plain_launch = false;
+    g_completion_event = nullptr;
+    return rc;
 }
 
 // Pick the Gram kernel for this shape (outside stream capture: the pair kernel's work list is uploaded here).
@@ -267,21 +437,33 @@ int choose_gram(casgd_ctx *c, int32_t s, int32_t b)
 {
     const int32_t sb = s * b;
     const int64_t opt = c->opt_gram_impl;
+    // SM budgets of the two branches. Pipelined: the chain keeps chain_sms SMs (the recurrence cluster's 16 and a few more
+    // for the margin and update streams), gather and Gram are sized for the rest -- also in single-step calls, so that
+    // every path of a mode runs identical kernels on identical grids (bit-identical iterates).
+    c->gram_sms = c->chain_sms = c->num_sms;
+    c->cur_gram = 2;                                    // (pipelined_mode asks step_is_s1, which looks at cur_gram)
+    if (pipelined_mode(c, s, b)) {
+        const int chain = c->opt_chain_sms > 0 ? (int)c->opt_chain_sms : 32;
+        c->chain_sms = std::min(std::max(chain, 16), c->num_sms - 32) & ~1;
+        c->gram_sms = c->num_sms - c->chain_sms;
+    }
     c->cur_gram = opt == 1 ? 1 : 2;
     c->cur_bn = 0;
     // gather + Gram in one kernel: wins while the tiles fit in about half a wave (measured at n = 18, b = 64: sb = 1536
     // 20.7 against 21.8 us per step, sb = 2048 29.8 against 25.7 us)
     if ((opt == 5 || (opt == 0 && sb <= 1536)) && c->n <= 64) { c->cur_gram = 4; return CASGD_OK; }
     if (opt == 5) return fail(c, CASGD_EINVAL, "the fused gather + Gram kernel needs n <= 64");
-    if (opt == 1 || opt == 2 || c->num_sms < 2) return CASGD_OK;
+    if (opt == 1 || opt == 2 || c->gram_sms < 2) return CASGD_OK;
     if (opt == 0 && (sb < 512 || c->n < 256)) return CASGD_OK;      // too little work for 256-row tiles
+    if (c->pair_plan && c->pair_plan_sms != c->gram_sms) { gram_pair_plan_destroy(c->pair_plan); c->pair_plan = nullptr; }
     if (!c->pair_plan) {
-        c->pair_plan = gram_pair_plan_create(c->Y, c->ldy, c->n, c->rows_alloc, c->xbf, c->ldxb, c->num_sms);
+        c->pair_plan_sms = c->gram_sms;
+        c->pair_plan = gram_pair_plan_create(c->Y, c->ldy, c->n, 2 * c->rows_alloc, c->xbf, c->ldxb, c->gram_sms);
         if (!c->pair_plan) return fail(c, CASGD_ECUDA, "cuTensorMapEncodeTiled failed for the pair Gram kernel");
     }
     int bn = 0;
     const int64_t span = gram_pair_prepare(c->pair_plan, sb, b, (int)c->opt_full_lower, opt == 3 ? 256 : opt == 4 ? 512 : 0,
-                                           (int)c->opt_ksplit, &bn);
+                                           (int)c->opt_ksplit, &bn, pipelined_mode(c, s, b));
     if (span < 0) {
         if (opt >= 3) return fail(c, CASGD_EINVAL, "the pair Gram kernel cannot run s*b = %d (work list too long)", sb);
         return CASGD_OK;
@@ -295,9 +477,9 @@ int choose_gram(casgd_ctx *c, int32_t s, int32_t b)
                 const int64_t last_row = std::min<int64_t>(ti * kTile + kTile, sb) - 1;
                 tiles += (ti == tj) || c->opt_full_lower || (last_row / b) > (tj * kTile / b);
             }
-        int64_t ks = std::max<int64_t>(1, std::min<int64_t>(c->num_sms / std::max<int64_t>(tiles, 1), kbt / 16));
+        int64_t ks = std::max<int64_t>(1, std::min<int64_t>(c->gram_sms / std::max<int64_t>(tiles, 1), kbt / 16));
         if (ks > 1 && kbt - kbt / ks < 24) ks = 1;
-        const int64_t span_tc = (tiles * ks + c->num_sms - 1) / c->num_sms * ((kbt + ks - 1) / ks) * 770 + 2600 + (ks > 1 ? 12000 : 0);
+        const int64_t span_tc = (tiles * ks + c->gram_sms - 1) / c->gram_sms * ((kbt + ks - 1) / ks) * 770 + 2600 + (ks > 1 ? 12000 : 0);
         // + the pair kernel's fixed cost (cluster launch, two cluster barriers, an epilogue nothing overlaps): ~12k cycles,
         // measured on one-tile-per-pair shapes (n = 2000, sb = 2048: 23 us against 18.8 us for the 128-tile kernel)
         if ((span + 12000) * 10 > span_tc * 9) return CASGD_OK;     // not clearly better: stay with the simpler kernel
@@ -333,16 +515,35 @@ int get_graph(casgd_ctx *c, int32_t s, int32_t b, float eta, int32_t len, GraphE
     int64_t kernels = 0;
     int rc = CASGD_OK;
     const int64_t saved = c->launches;
-    for (int32_t h = 0; h < len && rc == CASGD_OK; ++h) {
-        c->cur_slot_step = h;
-        rc = enqueue_step(c, c->capture_stream, nullptr, c->ind, (int64_t)h * s * b, nullptr, s, b, eta, &kernels);
+    const bool pipelined = pipelined_mode(c, s, b) && len > 1;
+    // mode 1: steps that have a gather kernel of their own gather the NEXT step's rows on a side branch (two Y stages)
+    const bool overlap = c->opt_overlap == 1 && c->cur_gram != 4 && !step_is_s1(c, s) && len > 1;
+    if ((overlap || pipelined) && !c->side_stream) {
+        cudaStreamCreateWithFlags(&c->side_stream, cudaStreamNonBlocking);
+        for (cudaEvent_t *e : {&c->ev_fork, &c->ev_join, &c->ev_gather[0], &c->ev_gather[1], &c->ev_gram[0], &c->ev_gram[1],
+                               &c->ev_grad, &c->ev_rec_launch})
+            cudaEventCreateWithFlags(e, cudaEventDisableTiming);
+    }
+    if (pipelined) {
+        rc = capture_pipelined(c, s, b, eta, len, &kernels);
+    } else {
+        for (int32_t h = 0; h < len && rc == CASGD_OK; ++h) {
+            c->cur_slot_step = h;
+            StepIo io;
+            if (overlap) {
+                io.buf = h & 1;
+                io.gathered = h > 0;
+                io.next_idx_off = h + 1 < len ? (int64_t)(h + 1) * s * b : -1;
+            }
+            rc = enqueue_step(c, c->capture_stream, nullptr, c->ind, (int64_t)h * s * b, nullptr, s, b, eta, &kernels, io);
+        }
     }
     c->cur_slot_step = 0;
     c->launches = saved;                      // capture launches nothing; replays are counted
     cudaError_t e = cudaStreamEndCapture(c->capture_stream, &graph);
     if (rc != CASGD_OK) { if (graph) cudaGraphDestroy(graph); return rc; }
     if (e != cudaSuccess) return fail(c, CASGD_ECUDA, "cudaStreamEndCapture: %s", cudaGetErrorString(e));
-    GraphEntry ge{nullptr, kernels};
+    GraphEntry ge{nullptr, kernels, c->last_buf};
     e = cudaGraphInstantiate(&ge.exec, graph, 0);
     cudaGraphDestroy(graph);
     if (e != cudaSuccess) return fail(c, CASGD_ECUDA, "cudaGraphInstantiate: %s", cudaGetErrorString(e));
@@ -390,8 +591,9 @@ int run_steps(casgd_ctx *c, const int32_t *idx, int64_t n_steps, float *x, int32
                 c->launches += launch_set_params(c->stream, c->ind, idx + done * sb, x);
                 CK(cudaGraphLaunch(ge.exec, c->stream));
                 c->launches += ge.kernels;
+                c->last_buf = ge.last_buf;
                 if (c->opt_stamps)
-                    launch_stamp_collect(c->stream, c->stamps, len * 4, c->stamps + kStampSteps * 8, c->stamps + kStampSteps * 8 + 4);
+                    launch_stamp_collect(c->stream, c->stamps, len * kSlotStages, c->stamps + kStampAcc, c->stamps + kStampAcc + 8, c->stamps + kStampRaw);
                 done += len;
             }
         }
@@ -401,7 +603,7 @@ int run_steps(casgd_ctx *c, const int32_t *idx, int64_t n_steps, float *x, int32
         rc = enqueue_step(c, c->stream, idx + done * sb, nullptr, 0, x, s, b, eta, &kernels);
         if (rc) return rc;
         if (c->opt_stamps)
-            launch_stamp_collect(c->stream, c->stamps, 4, c->stamps + kStampSteps * 8, c->stamps + kStampSteps * 8 + 4);
+            launch_stamp_collect(c->stream, c->stamps, kSlotStages, c->stamps + kStampAcc, c->stamps + kStampAcc + 8, c->stamps + kStampRaw);
     }
     CK(cudaGetLastError());
     return CASGD_OK;
@@ -561,6 +763,7 @@ int casgd_sgd_steps_fp32(casgd_ctx *c, const int32_t *idx, int64_t n_steps, floa
     rc = ensure_workspace(c, b);
     if (rc) return rc;
     c->shadow_valid = false;                  // x changes without the shadow following
+    c->gws.num_sms = c->num_sms;
     const float alpha = eta / (float)b;
     for (int64_t h = 0; h < n_steps; ++h)
         c->launches += launch_sgd32_step(c->stream, c->A32, c->lda, c->y, c->m, c->n, idx + h * b, b, alpha, c->loss, x,
@@ -615,24 +818,28 @@ int casgd_debug_export(casgd_ctx *c, int what, void *dst_host, int64_t dst_bytes
     if (!c) return CASGD_EINVAL;
     if (!dst_host) return fail(c, CASGD_EINVAL, "dst_host is null");
     const int64_t sb = (int64_t)c->last_s * c->last_b;
-    if (sb == 0 && what != CASGD_DBG_XBF) return fail(c, CASGD_EINVAL, "no outer step has run yet");
+    if (sb == 0 && what != CASGD_DBG_XBF && what != CASGD_DBG_STAMPS) return fail(c, CASGD_EINVAL, "no outer step has run yet");
     CK(cudaStreamSynchronize(c->stream));
     auto need = [&](int64_t bytes) { return dst_bytes == bytes; };
     switch (what) {
     case CASGD_DBG_Y:
         if (!need(sb * c->n * 2)) break;
-        CK(cudaMemcpy2D(dst_host, (size_t)c->n * 2, c->Y, (size_t)c->ldy * 2, (size_t)c->n * 2, (size_t)sb, cudaMemcpyDeviceToHost));
+        CK(cudaMemcpy2D(dst_host, (size_t)c->n * 2, c->Y + (size_t)c->last_buf * c->rows_alloc * c->ldy, (size_t)c->ldy * 2, (size_t)c->n * 2, (size_t)sb, cudaMemcpyDeviceToHost));
         return CASGD_OK;
     case CASGD_DBG_G:
         if (!need(sb * sb * 4)) break;
-        CK(cudaMemcpy2D(dst_host, (size_t)sb * 4, c->G, (size_t)c->ldg * 4, (size_t)sb * 4, (size_t)sb, cudaMemcpyDeviceToHost));
+        CK(cudaMemcpy2D(dst_host, (size_t)sb * 4, c->G + (size_t)c->last_buf * c->rows_alloc * c->rows_alloc, (size_t)c->ldg * 4, (size_t)sb * 4, (size_t)sb, cudaMemcpyDeviceToHost));
         return CASGD_OK;
     case CASGD_DBG_YLAB: case CASGD_DBG_R: case CASGD_DBG_Z: case CASGD_DBG_U: {
         if (!need(sb * 4)) break;
-        const float *src = what == CASGD_DBG_YLAB ? c->yI : what == CASGD_DBG_R ? c->r : what == CASGD_DBG_Z ? c->z : c->u;
+        const float *src = what == CASGD_DBG_YLAB ? c->yI + (size_t)c->last_buf * c->rows_alloc : what == CASGD_DBG_R ? c->r : what == CASGD_DBG_Z ? c->z : c->u;
         CK(cudaMemcpy(dst_host, src, (size_t)sb * 4, cudaMemcpyDeviceToHost));
         return CASGD_OK;
     }
+    case CASGD_DBG_STAMPS:
+        if (!need((int64_t)kStampSlots * 16)) break;
+        CK(cudaMemcpy(dst_host, c->stamps + kStampRaw, (size_t)kStampSlots * 16, cudaMemcpyDeviceToHost));
+        return CASGD_OK;
     case CASGD_DBG_XBF:
         if (!need((int64_t)c->n * 2)) break;
         CK(cudaMemcpy(dst_host, c->xbf, (size_t)c->n * 2, cudaMemcpyDeviceToHost));
@@ -667,9 +874,15 @@ int casgd_set_option(casgd_ctx *c, int option, int64_t value)
         c->opt_stamps = value != 0;
         // arm every slot ({~0, 0}) and clear the totals: a collect pass over all slots, then zero the accumulators
         CK(cudaStreamSynchronize(c->stream));
-        launch_stamp_collect(c->stream, c->stamps, kStampSteps * 4, c->stamps + kStampSteps * 8, c->stamps + kStampSteps * 8 + 4);
-        CK(cudaMemsetAsync(c->stamps + kStampSteps * 8, 0, sizeof(unsigned long long) * 8, c->stream));
+        launch_stamp_collect(c->stream, c->stamps, kStampSlots, c->stamps + kStampAcc, c->stamps + kStampAcc + 8, c->stamps + kStampRaw);
+        CK(cudaMemsetAsync(c->stamps + kStampAcc, 0, sizeof(unsigned long long) * 16, c->stream));
         break;
+    case CASGD_OPT_OVERLAP:
+        if (value < 0 || value > 2) return fail(c, CASGD_EINVAL, "CASGD_OPT_OVERLAP must be 0, 1 or 2");
+        c->opt_overlap = value; break;
+    case CASGD_OPT_CHAIN_SMS:
+        if (value < 0 || value > 1024) return fail(c, CASGD_EINVAL, "CASGD_OPT_CHAIN_SMS must be in [0, 1024]");
+        c->opt_chain_sms = value; break;
     case CASGD_OPT_LOSS_IMPL:
         if (value != 0 && value != 1) return fail(c, CASGD_EINVAL, "CASGD_OPT_LOSS_IMPL must be 0 or 1");
         c->opt_loss_impl = value; break;
@@ -686,18 +899,18 @@ int casgd_stage_times(casgd_ctx *c, double *ms_host, int64_t *launches_host, int
     collect_events(c);
     if (c->opt_stamps) {
         // in-graph stamps replace the event times of the four step stages
-        unsigned long long acc[8];
-        CK(cudaMemcpy(acc, c->stamps + kStampSteps * 8, sizeof acc, cudaMemcpyDeviceToHost));
-        for (int i = 0; i < 4; ++i) {
+        unsigned long long acc[16];
+        CK(cudaMemcpy(acc, c->stamps + kStampAcc, sizeof acc, cudaMemcpyDeviceToHost));
+        for (int i = 0; i <= CASGD_STAGE_MARGIN; ++i) {
             if (ms_host) ms_host[i] = (double)acc[i] * 1e-6;
-            if (launches_host) launches_host[i] = (int64_t)acc[4 + i];
+            if (launches_host) launches_host[i] = (int64_t)acc[8 + i];
         }
-        for (int i = 4; i < CASGD_NUM_STAGES; ++i) {
+        for (int i = CASGD_STAGE_MARGIN + 1; i < CASGD_NUM_STAGES; ++i) {
             if (ms_host) ms_host[i] = c->stage_ms[i];
             if (launches_host) launches_host[i] = c->stage_launches[i];
             if (reset) { c->stage_ms[i] = 0.0; c->stage_launches[i] = 0; }
         }
-        if (reset) CK(cudaMemset(c->stamps + kStampSteps * 8, 0, sizeof(unsigned long long) * 8));
+        if (reset) CK(cudaMemset(c->stamps + kStampAcc, 0, sizeof(unsigned long long) * 16));
         return CASGD_OK;
     }
     for (int i = 0; i < CASGD_NUM_STAGES; ++i) {
@@ -719,6 +932,9 @@ void casgd_destroy(casgd_ctx *c)
     collect_events(c);
     free_step_workspace(c);
     if (c->capture_stream) cudaStreamDestroy(c->capture_stream);
+    if (c->side_stream) cudaStreamDestroy(c->side_stream);
+    for (cudaEvent_t e : {c->ev_fork, c->ev_join, c->ev_gather[0], c->ev_gather[1], c->ev_gram[0], c->ev_gram[1], c->ev_grad, c->ev_rec_launch})
+        if (e) cudaEventDestroy(e);
     cudaFree(c->A_owned); cudaFree(c->A32); cudaFree(c->xbf);
     cudaFree(c->gws.partial); cudaFree(c->gws.counters); cudaFree(c->ind); cudaFree(c->err_flag);
     cudaFree(c->rws.utag); cudaFree(c->rws.epoch); cudaFree(c->stamps);

@@ -134,6 +134,12 @@ __device__ __forceinline__ void pdl_trigger() { asm volatile("griddepcontrol.lau
 // launches. The slot pointer is a kernel argument baked into the graph (null = off). A launcher reads it from the
 // thread-local g_stamp, which enqueue_step sets around each stage.
 extern thread_local unsigned long long *g_stamp;
+// Launch modifiers for the NEXT launch_pdl call(s) of this thread, set by the pipelined graph capture (casgd_api.cu):
+// g_plain_launch: no programmatic-serialisation attribute (side-branch kernels must not become resident early: their
+// waiting CTAs would hold the SMs the other branch needs); g_completion_event: record this event once all CTAs of the
+// kernel have begun execution (cudaLaunchAttributeLaunchCompletionEvent; consumed by the launch).
+extern thread_local bool g_plain_launch;
+extern thread_local cudaEvent_t g_completion_event;
 __device__ __forceinline__ unsigned long long globaltimer_ns()
 {
     unsigned long long t;
@@ -163,11 +169,20 @@ inline cudaError_t launch_pdl(void (*kern)(KArgs...), dim3 grid, dim3 block, siz
     cfg.blockDim = block;
     cfg.dynamicSmemBytes = smem;
     cfg.stream = st;
-    cudaLaunchAttribute attr[2];
+    cudaLaunchAttribute attr[3];
     int na = 0;
-    attr[na].id = cudaLaunchAttributeProgrammaticStreamSerialization;
-    attr[na].val.programmaticStreamSerializationAllowed = 1;
-    ++na;
+    if (!g_plain_launch) {
+        attr[na].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+        attr[na].val.programmaticStreamSerializationAllowed = 1;
+        ++na;
+    }
+    if (g_completion_event) {
+        attr[na].id = cudaLaunchAttributeLaunchCompletionEvent;
+        attr[na].val.launchCompletionEvent.event = g_completion_event;
+        attr[na].val.launchCompletionEvent.flags = 0;
+        ++na;
+        g_completion_event = nullptr;
+    }
     if (cluster > 1) {
         attr[na].id = cudaLaunchAttributeClusterDimension;
         attr[na].val.clusterDim.x = (unsigned)cluster;
@@ -210,6 +225,8 @@ struct RecWorkspace {
     int32_t max_ctas;              // CTAs that can be co-resident (one per SM); 0 = grid kernel unavailable
     int32_t cluster;               // CTAs per cluster of the cluster kernel (16 or 8); 0 = unavailable
     int64_t grid_threshold_bytes;  // strict block-lower G at or above this size leaves the one-CTA kernel
+    int32_t late_trigger;          // 1 = the streaming kernel releases its dependent kernel only when the chain is done
+                                   // (a side-branch gather needs the SMs the dependent's waiting CTAs would hold)
 };
 int recurrence_cluster_size();
 int recurrence_max_coresident_ctas(int num_sms);
@@ -226,6 +243,7 @@ struct FusedUpdate {
     uint16_t *xbf;
 };
 bool recurrence_fuses_update(int32_t s, int32_t b, int32_t ldg, int32_t ldy, const RecWorkspace &ws, int impl);
+int recurrence_kernel_choice(int32_t s, int32_t b, int32_t ldg, const RecWorkspace &ws, int impl, bool fused);
 int launch_recurrence(cudaStream_t st, const float *G, int32_t ldg, const float *r, const float *yI, int32_t s,
                       int32_t b, float alpha, int loss, float *z, float *u, const RecWorkspace &ws, int impl,
                       const FusedUpdate *fu);
@@ -234,7 +252,8 @@ int launch_recurrence(cudaStream_t st, const float *G, int32_t ldg, const float 
 bool recurrence_stream_ok(int32_t s, int32_t b, int32_t ldg, int cluster);
 bool recurrence_stream_fuses_update(int32_t s, int32_t b, int32_t ldy, int cluster_max);
 int launch_recurrence_stream(cudaStream_t st, const float *G, int32_t ldg, const float *r, const float *yI, int32_t s,
-                             int32_t b, float alpha, int loss, float *z, float *u, int cluster, const FusedUpdate *fu);
+                             int32_t b, float alpha, int loss, float *z, float *u, int cluster, const FusedUpdate *fu,
+                             int late_trigger);
 
 struct GradWorkspace {
     float *partial;        // [row_splits x ldp] partial column sums
@@ -248,6 +267,9 @@ int launch_gradient_bf16(cudaStream_t st, const uint16_t *Y, int32_t ldy, int32_
                          float alpha, float *x, const StepParams *ind, uint16_t *xbf, const GradWorkspace &ws);
 
 // s = 1 with wide rows: gather + margin + l' in one warp-per-row kernel (no Gram exists at s = 1); gradient.cu
+// r = Y x_bf (Alg. 1 line 3) as a kernel of its own: the pipelined schedule computes G(t+1) before x(t+1) exists
+int launch_margin(cudaStream_t st, const uint16_t *Y, int32_t ldy, int32_t sb, const uint16_t *xbf, float *r, int num_sms);
+
 int launch_margin_s1(cudaStream_t st, const uint16_t *A, int64_t lda, const float *y, int64_t m, int32_t n,
                      const int32_t *idx, const StepParams *ind, int64_t idx_off, int32_t b, int loss, const uint16_t *xbf,
                      uint16_t *Y, int32_t ldy, float *yI, float *r, float *z, float *u, int *err_flag);
@@ -266,11 +288,12 @@ int launch_shadow(cudaStream_t st, const float *x, const StepParams *ind, int32_
 int launch_widen(cudaStream_t st, const uint16_t *A, int64_t lda, int64_t m, int32_t n, float *A32, int64_t lda32, int num_sms);
 int launch_repack(cudaStream_t st, const uint16_t *X, int64_t ldx, int64_t m, int32_t n, uint16_t *A, int64_t lda, int num_sms);
 int launch_set_params(cudaStream_t st, StepParams *ind, const int32_t *idx, float *x);
-// slots: [nslots][2] {min start, max end} in %globaltimer ns, slot = 4 * step + stage; accum_ns / count: [4]
+// slots: [nslots][2] {min start, max end} in %globaltimer ns, slot = 8 * step + stage; accum_ns / count: [8]
 int launch_stamp_collect(cudaStream_t st, unsigned long long *slots, int nslots, unsigned long long *accum_ns,
-                         unsigned long long *count);
+                         unsigned long long *count, unsigned long long *raw_copy);
 
-// tcgen05 Gram + margin (gram_tc.cu). The plan owns the TMA tensor maps of the Y workspace and of the
+// tcgen05 Gram + margin (gram_tc.cu). r == nullptr: no margin (the pipelined schedule computes r in a kernel of its own).
+// The plan owns the TMA tensor maps of the Y workspace and of the
 // BF16 shadow (a [16 x ldxb] buffer: row 0 = x_bf, rows 1..15 zero). ksplit_opt <= 0: choose automatically.
 // s = 1: there is no correction, u = l'(r, y_I) -- the Gram kernels' margin epilogue can apply l' itself.
 struct S1Fuse {
@@ -282,7 +305,7 @@ struct GramTcPlan;
 GramTcPlan *gram_tc_plan_create(const uint16_t *Y, int32_t ldy, int32_t n, int32_t sb_rows_alloc,
                                 const uint16_t *xbf, int32_t ldxb, char *err, int errlen);
 void gram_tc_plan_destroy(GramTcPlan *p);
-int launch_gram_tc(cudaStream_t st, GramTcPlan *plan, int32_t sb, int32_t b, float *G, int32_t ldg, float *r,
+int launch_gram_tc(cudaStream_t st, GramTcPlan *plan, int32_t row_base, int32_t sb, int32_t b, float *G, int32_t ldg, float *r,
                    int full_lower, int ksplit_opt, int num_sms, char *err, int errlen);
 
 // gather + Gram + margin in one kernel for narrow rows (n <= 64): gram_tc.cu
@@ -297,8 +320,8 @@ struct GramPairPlan;
 GramPairPlan *gram_pair_plan_create(const uint16_t *Y, int32_t ldy, int32_t n, int32_t rows_alloc, const uint16_t *xbf,
                                     int32_t ldxb, int num_sms);
 void gram_pair_plan_destroy(GramPairPlan *p);
-int64_t gram_pair_prepare(GramPairPlan *pl, int32_t sb, int32_t b, int full_lower, int bn, int ksplit_opt, int *bn_out);
-int launch_gram_pair(cudaStream_t st, GramPairPlan *pl, int32_t sb, int32_t b, float *G, int32_t ldg, float *r,
+int64_t gram_pair_prepare(GramPairPlan *pl, int32_t sb, int32_t b, int full_lower, int bn, int ksplit_opt, int *bn_out, bool no_margin);
+int launch_gram_pair(cudaStream_t st, GramPairPlan *pl, int32_t row_base, int32_t sb, int32_t b, float *G, int32_t ldg, float *r,
                      int full_lower, int bn, int ksplit_opt, char *err, int errlen);
 
 }  // namespace casgd

@@ -232,23 +232,25 @@ int launch_repack(cudaStream_t st, const uint16_t *X, int64_t ldx, int64_t m, in
 
 // CASGD_OPT_STAMPS: fold the {first start, last end} slots of the steps just run into per-stage totals and re-arm them.
 __global__ void stamp_collect_kernel(unsigned long long *slots, int nslots, unsigned long long *accum_ns,
-                                     unsigned long long *count)
+                                     unsigned long long *count, unsigned long long *raw_copy)
 {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= nslots) return;
     const unsigned long long t0 = slots[2 * i], t1 = slots[2 * i + 1];
+    raw_copy[2 * i] = t0;                               // the timeline of the graph just replayed (CASGD_DBG_STAMPS)
+    raw_copy[2 * i + 1] = t1;
     if (t1 != 0ull && t0 != ~0ull && t1 >= t0) {
-        atomicAdd(accum_ns + (i & 3), t1 - t0);
-        atomicAdd(count + (i & 3), 1ull);
+        atomicAdd(accum_ns + (i & 7), t1 - t0);
+        atomicAdd(count + (i & 7), 1ull);
     }
     slots[2 * i] = ~0ull;
     slots[2 * i + 1] = 0ull;
 }
 
 int launch_stamp_collect(cudaStream_t st, unsigned long long *slots, int nslots, unsigned long long *accum_ns,
-                         unsigned long long *count)
+                         unsigned long long *count, unsigned long long *raw_copy)
 {
-    stamp_collect_kernel<<<(nslots + 255) / 256, 256, 0, st>>>(slots, nslots, accum_ns, count);
+    stamp_collect_kernel<<<(nslots + 255) / 256, 256, 0, st>>>(slots, nslots, accum_ns, count, raw_copy);
     return 1;
 }
 

@@ -292,6 +292,76 @@ int launch_gradient_bf16(cudaStream_t st, const uint16_t *Y, int32_t ldy, int32_
     return launch_gradient_any<uint16_t, false, true>(st, Y, ldy, nullptr, 0, n, sb, u, alpha, x, ind, xbf, ws);
 }
 
+// ------------------------------------------------------------- margin as its own kernel ---
+// r = Y x_bf (Alg. 1 line 3; BF16 inputs, FP32 accumulation and output, L231) for the pipelined
+// schedule, where the Gram of step t + 1 is computed beside the recurrence of step t, before x(t+1) exists, so that the
+// margin can no longer ride in the Gram's B operand. A warp per row, two rows and eight 16-byte loads in flight per
+// lane; Y's pad columns and the shadow buffer's are zero, so whole 16-byte vectors are summed.
+constexpr int kMgWarps = 16;
+
+__device__ __forceinline__ uint4 ld_stream_v4(const void *p)
+{
+    uint4 r;
+    asm volatile("ld.global.L1::no_allocate.v4.u32 {%0, %1, %2, %3}, [%4];"
+                 : "=r"(r.x), "=r"(r.y), "=r"(r.z), "=r"(r.w) : "l"(p) : "memory");
+    return r;
+}
+
+__device__ __forceinline__ float dot8_bf16(const uint4 &a, const uint4 &x, float acc)
+{
+    acc = fmaf(bf16lo(a.x), bf16lo(x.x), acc); acc = fmaf(bf16hi(a.x), bf16hi(x.x), acc);
+    acc = fmaf(bf16lo(a.y), bf16lo(x.y), acc); acc = fmaf(bf16hi(a.y), bf16hi(x.y), acc);
+    acc = fmaf(bf16lo(a.z), bf16lo(x.z), acc); acc = fmaf(bf16hi(a.z), bf16hi(x.z), acc);
+    acc = fmaf(bf16lo(a.w), bf16lo(x.w), acc); acc = fmaf(bf16hi(a.w), bf16hi(x.w), acc);
+    return acc;
+}
+
+__global__ void __launch_bounds__(32 * kMgWarps)
+margin_kernel(const uint16_t *Y, int32_t ldy, int32_t sb, const uint16_t *xbf, float *r, unsigned long long *stamp)
+{
+    pdl_trigger();
+    pdl_wait();                                     // x_bf comes from the previous update, Y from the gather
+    stamp_begin(stamp);
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int gw = blockIdx.x * kMgWarps + warp, W = gridDim.x * kMgWarps;
+    const int nvec = ldy >> 3;
+    for (int row = 2 * gw; row < sb; row += 2 * W) {
+        const bool two = row + 1 < sb;
+        const uint16_t *y0 = Y + (int64_t)row * ldy, *y1 = y0 + (two ? ldy : 0);
+        float a0 = 0.f, a1 = 0.f;
+        for (int cv0 = lane; cv0 < nvec; cv0 += 128) {
+            uint4 v0[4], v1[4], xv[4];
+#pragma unroll
+            for (int q = 0; q < 4; ++q) {
+                const int cv = cv0 + 32 * q;
+                v0[q] = v1[q] = make_uint4(0u, 0u, 0u, 0u);
+                if (cv < nvec) { v0[q] = ld_stream_v4(y0 + cv * 8); v1[q] = ld_stream_v4(y1 + cv * 8); }
+            }
+#pragma unroll
+            for (int q = 0; q < 4; ++q) {
+                const int cv = cv0 + 32 * q;
+                xv[q] = make_uint4(0u, 0u, 0u, 0u);
+                if (cv < nvec) xv[q] = ld_dep_v4(xbf + cv * 8);
+            }
+#pragma unroll
+            for (int q = 0; q < 4; ++q) { a0 = dot8_bf16(v0[q], xv[q], a0); a1 = dot8_bf16(v1[q], xv[q], a1); }
+        }
+        a0 = warp_sum(a0);
+        a1 = warp_sum(a1);
+        if (lane == 0) { r[row] = a0; if (two) r[row + 1] = a1; }
+    }
+    stamp_end_warp(stamp);
+}
+
+int launch_margin(cudaStream_t st, const uint16_t *Y, int32_t ldy, int32_t sb, const uint16_t *xbf, float *r, int num_sms)
+{
+    const int pairs = (sb + 1) / 2;
+    // two CTAs per SM at most: 32 warps x 2 rows x 4 x 16-byte loads per lane = 128 KB in flight per SM
+    const int blocks = std::max(1, std::min(2 * num_sms, (pairs + kMgWarps - 1) / kMgWarps));
+    launch_pdl(margin_kernel, dim3(blocks), dim3(32 * kMgWarps), 0, st, 1, Y, ldy, sb, xbf, r, g_stamp);
+    return 1;
+}
+
 // ------------------------------------------------------------- s = 1 with BF16 rows ---
 // At s = 1 there is no Gram matrix and no correction: the step is plain mini-batch SGD on BF16 rows with a BF16
 // shadow of x (Alg. 1 with s = 1, L99). One warp per sampled row gathers the row from A (16-byte loads), writes it

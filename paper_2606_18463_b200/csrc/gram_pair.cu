@@ -61,6 +61,7 @@ struct PairParams {
     const PairItem *items;              // [npairs x kMaxItemsPerPair]
     const int32_t *counts;              // [npairs]
     int32_t ldg, sb, b, n, full_lower, bn, nslots, accumulate;
+    int32_t row_base;                   // first row of this step's Y buffer inside the (double-buffered) stage
     // margin items cut along K into mslices pieces: partial sums per slice, summed in slice order by the last to finish
     float *rpart;                       // [mslices x ldr]
     unsigned *rcount;                   // [2 x row tiles], zero between launches
@@ -231,12 +232,12 @@ gram_pair_kernel(const __grid_constant__ CUtensorMap tmY, const __grid_constant_
                     const uint32_t fb = mapa(full_bar(stage), 0);          // completion is counted on the leader's barrier
                     if (w.kind == 0) {
                         mbar_expect_tx_cluster(fb, kTileB * (1u + (uint32_t)w.nsub));
-                        tma_load_2d_pair(sbase + kOffAp, &tmY, fb, kb * BK, w.I * PM + (int)rank * HM);
+                        tma_load_2d_pair(sbase + kOffAp, &tmY, fb, kb * BK, p.row_base + w.I * PM + (int)rank * HM);
                         for (int sub = 0; sub < w.nsub; ++sub)
-                            tma_load_2d_pair(sbase + kOffB0 + sub * kTileB, &tmY, fb, kb * BK, w.J * p.bn + sub * PM + (int)rank * HM);
+                            tma_load_2d_pair(sbase + kOffB0 + sub * kTileB, &tmY, fb, kb * BK, p.row_base + w.J * p.bn + sub * PM + (int)rank * HM);
                     } else {
                         mbar_expect_tx_cluster(fb, kTileB + kXB);
-                        tma_load_2d_pair(sbase + kOffAp, &tmY, fb, kb * BK, w.I * PM + (int)rank * HM);
+                        tma_load_2d_pair(sbase + kOffAp, &tmY, fb, kb * BK, p.row_base + w.I * PM + (int)rank * HM);
                         tma_load_2d_pair(sbase + kOffB0, &tmX8, fb, kb * BK, (int)rank * 8);
                     }
                     if (++stage == kStagesP) { stage = 0; phase ^= 1u; }
@@ -448,8 +449,8 @@ struct PairList {
 
 // Items of one outer step's Gram + margin, dealt to `npairs` pairs longest-first. Returns false when a pair
 // would exceed kMaxItemsPerPair.
-bool build_items(int sb, int b, int n, int full_lower, int bn, int ksplit, int npairs, std::vector<std::vector<PairItem>> &per_pair,
-                 int64_t *makespan)
+bool build_items(int sb, int b, int n, int full_lower, int bn, int ksplit, int npairs, bool no_margin,
+                 std::vector<std::vector<PairItem>> &per_pair, int64_t *makespan)
 {
     const int mslices = margin_slices(n);
     const int T = (sb + PM - 1) / PM, kbt = (n + BK - 1) / BK;
@@ -471,7 +472,7 @@ bool build_items(int sb, int b, int n, int full_lower, int bn, int ksplit, int n
                 if (w.kb1 > w.kb0) all.push_back(w);
             }
         }
-        for (int ms = 0; ms < mslices; ++ms) {          // margin items: K slices (slice index in J)
+        for (int ms = 0; ms < mslices && !no_margin; ++ms) {          // margin items: K slices (slice index in J)
             PairItem mg{};
             mg.I = (int16_t)I; mg.J = (int16_t)ms; mg.kind = 1; mg.nsub = 1;
             mg.kb0 = (int16_t)((int64_t)ms * kbt / mslices);
@@ -501,7 +502,7 @@ struct GramPairPlan {
     float *rpart = nullptr;             // [4 x rows_alloc] margin partial sums
     unsigned *rcount = nullptr;         // [2 x row tiles]
     int32_t n = 0, rows_alloc = 0, npairs = 0;
-    std::map<std::tuple<int, int, int, int, int>, PairList> lists;       // (sb, b, full_lower, bn, ksplit_opt)
+    std::map<std::tuple<int, int, int, int, int, int>, PairList> lists;       // (sb, b, full_lower, bn, ksplit_opt, no_margin)
 };
 
 GramPairPlan *gram_pair_plan_create(const uint16_t *Y, int32_t ldy, int32_t n, int32_t rows_alloc, const uint16_t *xbf,
@@ -540,19 +541,19 @@ void gram_pair_plan_destroy(GramPairPlan *p)
 
 // Build (once per shape) and upload the work list. Must be called OUTSIDE stream capture; synchronous.
 // bn: 256, 512, or 0 = whichever the cost model prefers. Returns the estimated cycles of the Gram, or -1.
-int64_t gram_pair_prepare(GramPairPlan *pl, int32_t sb, int32_t b, int full_lower, int bn, int ksplit_opt, int *bn_out)
+int64_t gram_pair_prepare(GramPairPlan *pl, int32_t sb, int32_t b, int full_lower, int bn, int ksplit_opt, int *bn_out, bool no_margin)
 {
     int64_t best_span = -1, best_span_unused = 0;
     int best_bn = 0;
     for (int cand : {256, 512}) {
         if (bn != cand && !(bn == 0 && cand == 256)) continue;      // 256 x 512 tiles only on request: never faster, measured
-        auto key = std::make_tuple((int)sb, (int)b, full_lower, cand, ksplit_opt);
+        auto key = std::make_tuple((int)sb, (int)b, full_lower, cand, ksplit_opt, (int)no_margin);
         auto it = pl->lists.find(key);
         if (it == pl->lists.end()) {
             const int kbt = (pl->n + BK - 1) / BK;
             std::vector<std::vector<PairItem>> per_pair, best_pp;
             int n_g_items = 0;
-            if (build_items(sb, b, pl->n, full_lower, cand, 1, pl->npairs, per_pair, &best_span_unused))
+            if (build_items(sb, b, pl->n, full_lower, cand, 1, pl->npairs, no_margin, per_pair, &best_span_unused))
                 for (auto &v : per_pair)
                     for (auto &w : v) n_g_items += w.kind == 0;
             PairList L;
@@ -563,7 +564,7 @@ int64_t gram_pair_prepare(GramPairPlan *pl, int32_t sb, int32_t b, int full_lowe
                 if (ksplit_opt <= 0 && ks > 1 && kbt / ks < 16) break;      // keep >= 16 K blocks per slice
                 if (ksplit_opt <= 0 && ks > 1 && n_g_items * (ks - 1) >= pl->npairs) break;   // split only to fill idle pairs
                 int64_t sp = 0;
-                if (!build_items(sb, b, pl->n, full_lower, cand, ks, pl->npairs, per_pair, &sp)) continue;
+                if (!build_items(sb, b, pl->n, full_lower, cand, ks, pl->npairs, no_margin, per_pair, &sp)) continue;
                 if (ks > 1) sp += 12000;                                    // the cleared G and the red.add epilogue
                 if (span < 0 || sp < span) { span = sp; best_pp = per_pair; L.ksplit = ks; }
             }
@@ -591,10 +592,10 @@ int64_t gram_pair_prepare(GramPairPlan *pl, int32_t sb, int32_t b, int full_lowe
 }
 
 // Enqueue the pair kernel for a shape gram_pair_prepare has seen. Returns kernels + memsets launched, or -1.
-int launch_gram_pair(cudaStream_t st, GramPairPlan *pl, int32_t sb, int32_t b, float *G, int32_t ldg, float *r,
+int launch_gram_pair(cudaStream_t st, GramPairPlan *pl, int32_t row_base, int32_t sb, int32_t b, float *G, int32_t ldg, float *r,
                      int full_lower, int bn, int ksplit_opt, char *err, int errlen)
 {
-    auto it = pl->lists.find(std::make_tuple((int)sb, (int)b, full_lower, bn, ksplit_opt));
+    auto it = pl->lists.find(std::make_tuple((int)sb, (int)b, full_lower, bn, ksplit_opt, (int)(r == nullptr)));
     if (it == pl->lists.end() || it->second.makespan < 0) {
         snprintf(err, errlen, "gram_pair: no work list for sb = %d, b = %d, bn = %d", sb, b, bn);
         return -1;
@@ -604,6 +605,7 @@ int launch_gram_pair(cudaStream_t st, GramPairPlan *pl, int32_t sb, int32_t b, f
     p.G = G; p.r = r; p.items = L.items; p.counts = L.counts;
     p.ldg = ldg; p.sb = sb; p.b = b; p.n = pl->n; p.full_lower = full_lower; p.bn = bn;
     p.nslots = bn == 256 ? 2 : 1;
+    p.row_base = row_base;
     p.accumulate = L.ksplit > 1;
     p.stamp = g_stamp;
     p.rpart = pl->rpart; p.rcount = pl->rcount; p.mslices = margin_slices(pl->n); p.ldr = pl->rows_alloc;

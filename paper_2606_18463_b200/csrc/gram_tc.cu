@@ -38,6 +38,8 @@ struct GramParams {
     float *G;
     float *r;
     int32_t ldg, sb, b, n, T, ntiles, ksplit, kb_total, full_lower;
+    int32_t row_base;                   // first row of this step's Y buffer inside the (double-buffered) stage
+    int32_t no_margin;                  // pipelined schedule: r is a kernel of its own, no x_bf rows in the B operand
     unsigned long long *stamp;
 };
 
@@ -143,7 +145,7 @@ __device__ __forceinline__ Work decode_work(const GramParams &p, int w)
     }
     const int last_row = min(k.ti * BM + BM, p.sb) - 1;
     k.need_g = p.full_lower || (last_row / p.b) > ((k.tj * BN) / p.b);      // holds an entry of a block below the block diagonal
-    k.skip = !k.diag && !k.need_g;
+    k.skip = !k.need_g && (!k.diag || p.no_margin);
     k.kb0 = (int)(((int64_t)ks * p.kb_total) / p.ksplit);
     k.kb1 = (int)(((int64_t)(ks + 1) * p.kb_total) / p.ksplit);
     return k;
@@ -199,13 +201,13 @@ gram_tc_kernel(const __grid_constant__ CUtensorMap tmY, const __grid_constant__ 
                     mbar_wait(empty_bar(stage), phase ^ 1u);
                     const uint32_t sbase = smem_base + stage * kStageBytes;
                     if (k.diag) {
-                        mbar_expect_tx(full_bar(stage), kTileBytes + kXBytes);
-                        tma_load_2d(sbase + kOffB, &tmY, full_bar(stage), kb * BK, k.ti * BM);
-                        tma_load_2d(sbase + kOffX, &tmX, full_bar(stage), kb * BK, 0);
+                        mbar_expect_tx(full_bar(stage), kTileBytes + (p.no_margin ? 0u : kXBytes));
+                        tma_load_2d(sbase + kOffB, &tmY, full_bar(stage), kb * BK, p.row_base + k.ti * BM);
+                        if (!p.no_margin) tma_load_2d(sbase + kOffX, &tmX, full_bar(stage), kb * BK, 0);
                     } else {
                         mbar_expect_tx(full_bar(stage), 2 * kTileBytes);
-                        tma_load_2d(sbase + kOffB, &tmY, full_bar(stage), kb * BK, k.tj * BN);
-                        tma_load_2d(sbase + kOffA, &tmY, full_bar(stage), kb * BK, k.ti * BM);
+                        tma_load_2d(sbase + kOffB, &tmY, full_bar(stage), kb * BK, p.row_base + k.tj * BN);
+                        tma_load_2d(sbase + kOffA, &tmY, full_bar(stage), kb * BK, p.row_base + k.ti * BM);
                     }
                     if (++stage == kStages) { stage = 0; phase ^= 1u; }
                 }
@@ -229,7 +231,7 @@ gram_tc_kernel(const __grid_constant__ CUtensorMap tmY, const __grid_constant__ 
                 tc_fence_after();
                 const uint32_t d_tmem = tmem_base + slot * kAccCols;
                 // diagonal tile: A = B = the same smem tile; N = 144 (G tile + margin rows) or 16 (margin only)
-                const uint32_t ncols = k.diag ? (k.need_g ? (uint32_t)(BN + XR) : (uint32_t)XR) : (uint32_t)BN;
+                const uint32_t ncols = k.diag ? (k.need_g ? (uint32_t)(BN + (p.no_margin ? 0 : XR)) : (uint32_t)XR) : (uint32_t)BN;
                 const uint32_t idesc = umma_idesc(ncols);
                 const uint32_t offa = k.diag ? kOffB : kOffA, offb = (k.diag && !k.need_g) ? kOffX : kOffB;
                 for (int kb = k.kb0; kb < k.kb1; ++kb) {
@@ -306,7 +308,7 @@ gram_tc_kernel(const __grid_constant__ CUtensorMap tmY, const __grid_constant__ 
                     __syncwarp();
                 }
             }
-            if (k.diag) {
+            if (k.diag && !p.no_margin) {
                 const uint32_t rv = tc_ld1(t_row + (k.need_g ? BN : 0));
                 tc_wait_ld();
                 if (row_ok) {
@@ -582,11 +584,11 @@ cudaError_t gram_tc_configure()
     return cudaFuncSetAttribute(gram_narrow_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kNwSmem);
 }
 
-int launch_gram_tc(cudaStream_t st, GramTcPlan *plan, int32_t sb, int32_t b, float *G, int32_t ldg, float *r,
+int launch_gram_tc(cudaStream_t st, GramTcPlan *plan, int32_t row_base, int32_t sb, int32_t b, float *G, int32_t ldg, float *r,
                    int full_lower, int ksplit_opt, int num_sms, char *err, int errlen)
 {
     GramParams p;
-    p.G = G; p.r = r; p.ldg = ldg; p.sb = sb; p.b = b; p.n = plan->n;
+    p.G = G; p.r = r; p.ldg = ldg; p.sb = sb; p.b = b; p.n = plan->n; p.row_base = row_base; p.no_margin = r == nullptr;
     p.T = (sb + BM - 1) / BM;
     p.ntiles = p.T * (p.T + 1) / 2;
     p.kb_total = (plan->n + BK - 1) / BK;
@@ -608,7 +610,7 @@ int launch_gram_tc(cudaStream_t st, GramTcPlan *plan, int32_t sb, int32_t b, flo
     if (ksplit > 1) {
         // partial sums are added with red.global.add.f32: clear the rows of G and r this step writes
         cudaMemsetAsync(G, 0, sizeof(float) * (size_t)p.T * BM * ldg, st);
-        cudaMemsetAsync(r, 0, sizeof(float) * (size_t)p.T * BM, st);
+        if (r) cudaMemsetAsync(r, 0, sizeof(float) * (size_t)p.T * BM, st);
     }
     const int grid = std::min(p.ntiles * ksplit, num_sms);
     cudaError_t e = launch_pdl(gram_tc_kernel, dim3(grid), dim3(kThreads), kSmemBytes, st, 1, plan->tmY, plan->tmX, p);

@@ -536,9 +536,9 @@ bool recurrence_fuses_update(int32_t s, int32_t b, int32_t ldg, int32_t ldy, con
     return (impl == 4 || impl == 0) && recurrence_stream_ok(s, b, ldg, ws.cluster) && recurrence_stream_fuses_update(s, b, ldy, ws.cluster);
 }
 
-int launch_recurrence(cudaStream_t st, const float *G, int32_t ldg, const float *r, const float *yI, int32_t s,
-                      int32_t b, float alpha, int loss, float *z, float *u, const RecWorkspace &ws, int impl,
-                      const FusedUpdate *fu)
+// Which kernel launch_recurrence runs for this shape: 1 = one CTA, 2 = all SMs (cooperative), 3 = one cluster with
+// plain loads, 4 = the streaming cluster kernel.
+int recurrence_kernel_choice(int32_t s, int32_t b, int32_t ldg, const RecWorkspace &ws, int impl, bool fused)
 {
     const int64_t gl_bytes = 2ll * b * b * s * (s - 1);
     const int sb = s * b;
@@ -546,17 +546,26 @@ int launch_recurrence(cudaStream_t st, const float *G, int32_t ldg, const float 
     const bool grid_ok = ws.max_ctas > 0 && (int64_t)ws.max_ctas * kRecWarps * 16 >= sb;
     const bool cluster_ok = ws.cluster > 0 && b % 4 == 0 && ldg % 4 == 0;
     const bool stream_ok = (impl == 4 || impl == 0) && recurrence_stream_ok(s, b, ldg, ws.cluster);
-    if (stream_ok && (impl == 4 || gl_bytes >= ws.grid_threshold_bytes || fu))
-        return launch_recurrence_stream(st, G, ldg, r, yI, s, b, alpha, loss, z, u, ws.cluster, fu);
-    const bool use_cluster = cluster_ok && (impl >= 3 || (impl == 0 && gl_bytes >= ws.grid_threshold_bytes));
-    if (use_cluster) {
+    if (stream_ok && (impl == 4 || gl_bytes >= ws.grid_threshold_bytes || fused)) return 4;
+    if (cluster_ok && (impl >= 3 || (impl == 0 && gl_bytes >= ws.grid_threshold_bytes))) return 3;
+    if (grid_ok && (impl >= 2 || (impl == 0 && gl_bytes >= ws.grid_threshold_bytes))) return 2;
+    return 1;
+}
+
+int launch_recurrence(cudaStream_t st, const float *G, int32_t ldg, const float *r, const float *yI, int32_t s,
+                      int32_t b, float alpha, int loss, float *z, float *u, const RecWorkspace &ws, int impl,
+                      const FusedUpdate *fu)
+{
+    const int choice = recurrence_kernel_choice(s, b, ldg, ws, impl, fu != nullptr);
+    if (choice == 4)
+        return launch_recurrence_stream(st, G, ldg, r, yI, s, b, alpha, loss, z, u, ws.cluster, fu, ws.late_trigger);
+    if (choice == 3) {
         cudaError_t e = loss == CASGD_LOGISTIC ? launch_cluster<CASGD_LOGISTIC>(st, G, ldg, r, yI, s, b, alpha, z, u, ws.cluster)
                       : loss == CASGD_LINEAR  ? launch_cluster<CASGD_LINEAR>(st, G, ldg, r, yI, s, b, alpha, z, u, ws.cluster)
                                               : launch_cluster<CASGD_POISSON>(st, G, ldg, r, yI, s, b, alpha, z, u, ws.cluster);
         return e == cudaSuccess ? 1 : -1;
     }
-    const bool use_grid = grid_ok && (impl >= 2 || (impl == 0 && gl_bytes >= ws.grid_threshold_bytes));
-    if (use_grid) {
+    if (choice == 2) {
         cudaError_t e = loss == CASGD_LOGISTIC ? launch_grid<CASGD_LOGISTIC>(st, G, ldg, r, yI, s, b, alpha, z, u, ws)
                       : loss == CASGD_LINEAR  ? launch_grid<CASGD_LINEAR>(st, G, ldg, r, yI, s, b, alpha, z, u, ws)
                                               : launch_grid<CASGD_POISSON>(st, G, ldg, r, yI, s, b, alpha, z, u, ws);

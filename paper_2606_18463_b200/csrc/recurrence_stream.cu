@@ -149,7 +149,7 @@ __device__ __forceinline__ int num_chunks(int j, int b) { return (j * b + kChunk
 
 #ifdef CASGD_REC_TRACE
 __device__ long long g_rec_trace[8192];
-#define REC_TRACE(i) do { if (crank == 0 && warp == 0 && lane == 0 && (i) < 8192) g_rec_trace[(i)] = clock64(); } while (0)
+#define REC_TRACE(i) do { if (crank == 0 && (warp & 3) == 0 && (warp >> 2) < kCritPer && lane == 0 && (i) < 8192) g_rec_trace[(i)] = clock64(); } while (0)
 #define REC_TRACE_B(i) do { if (crank == 0 && warp == 2 && lane == 0 && (i) < 8192) g_rec_trace[(i)] = clock64(); } while (0)
 #else
 #define REC_TRACE_B(i) do { } while (0)
@@ -193,12 +193,15 @@ template <int LOSS>
 __global__ void __launch_bounds__(kThreads, 1)
 recurrence_stream_kernel(const float *G, int32_t ldg, const float *r,
                          const float *yI, int32_t s, int32_t b, float alpha, float *z,
-                         float *u, const FusedGrad fg, unsigned long long *stamp)
+                         float *u, const FusedGrad fg, unsigned long long *stamp, int late_trigger)
 {
     extern __shared__ __align__(128) unsigned char rs_smem[];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int C = (int)cluster_nctarank(), crank = (int)cluster_ctarank();
-    pdl_trigger();
+    // The dependent kernel's CTAs become resident (and wait) once every CTA here has triggered. Normally that is wanted
+    // at once; with the next step's gather on a side branch it is not: the waiting CTAs would hold the SMs the gather
+    // needs (measured: the gather took 42 us instead of 12), so the trigger then comes after the chain.
+    if (!late_trigger) pdl_trigger();
     REC_TRACE(0);
     const int qmax = (b / kQuad + C - 1) / C;           // row groups of a block per CTA at most
     const StreamLayout L = stream_layout(s, b, qmax);
@@ -442,6 +445,7 @@ recurrence_stream_kernel(const float *G, int32_t ldg, const float *r,
         cluster_sync_all();
     }
     cp_async_wait<0>();
+    if (late_trigger) pdl_trigger();
     REC_TRACE(2);
     if (fg.Y) {
         // ===== fused g = Y^T u, x <- x - alpha g, shadow =====
@@ -538,13 +542,13 @@ int stream_cluster_for(int b, int cluster_max)
 
 template <int LOSS>
 cudaError_t launch_stream(cudaStream_t st, const float *G, int32_t ldg, const float *r, const float *yI, int32_t s,
-                          int32_t b, float alpha, float *z, float *u, int cluster_max, const FusedGrad &fg)
+                          int32_t b, float alpha, float *z, float *u, int cluster_max, const FusedGrad &fg, int late_trigger)
 {
     const int smem = stream_smem_bytes(s, b, cluster_max);
     if (smem == 0) return cudaErrorInvalidConfiguration;
     auto kern = recurrence_stream_kernel<LOSS>;
     const int cluster = stream_cluster_for(b, cluster_max);
-    return launch_pdl(kern, dim3(cluster), dim3(kThreads), (size_t)smem, st, cluster, G, ldg, r, yI, s, b, alpha, z, u, fg, g_stamp);
+    return launch_pdl(kern, dim3(cluster), dim3(kThreads), (size_t)smem, st, cluster, G, ldg, r, yI, s, b, alpha, z, u, fg, g_stamp, late_trigger);
 }
 
 }  // namespace
@@ -587,13 +591,14 @@ bool recurrence_stream_fuses_update(int32_t s, int32_t b, int32_t ldy, int clust
 }
 
 int launch_recurrence_stream(cudaStream_t st, const float *G, int32_t ldg, const float *r, const float *yI, int32_t s,
-                             int32_t b, float alpha, int loss, float *z, float *u, int cluster, const FusedUpdate *fu)
+                             int32_t b, float alpha, int loss, float *z, float *u, int cluster, const FusedUpdate *fu,
+                             int late_trigger)
 {
     FusedGrad fg{};
     if (fu) fg = FusedGrad{fu->Y, fu->ldy, fu->n, fu->x, fu->ind, fu->xbf};
-    cudaError_t e = loss == CASGD_LOGISTIC ? launch_stream<CASGD_LOGISTIC>(st, G, ldg, r, yI, s, b, alpha, z, u, cluster, fg)
-                  : loss == CASGD_LINEAR  ? launch_stream<CASGD_LINEAR>(st, G, ldg, r, yI, s, b, alpha, z, u, cluster, fg)
-                                          : launch_stream<CASGD_POISSON>(st, G, ldg, r, yI, s, b, alpha, z, u, cluster, fg);
+    cudaError_t e = loss == CASGD_LOGISTIC ? launch_stream<CASGD_LOGISTIC>(st, G, ldg, r, yI, s, b, alpha, z, u, cluster, fg, late_trigger)
+                  : loss == CASGD_LINEAR  ? launch_stream<CASGD_LINEAR>(st, G, ldg, r, yI, s, b, alpha, z, u, cluster, fg, late_trigger)
+                                          : launch_stream<CASGD_POISSON>(st, G, ldg, r, yI, s, b, alpha, z, u, cluster, fg, late_trigger);
     return e == cudaSuccess ? 1 : -1;
 }
 

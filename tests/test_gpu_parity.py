@@ -10,7 +10,7 @@ import torch
 
 from paper_2606_18463_b200 import synth
 
-from gpu_common import (TOL_FINAL_LOSS, TOL_LOSS_CALL, check_step_against_oracle, device_dataset, random_x,
+from gpu_common import (TOL_FINAL_LOSS, TOL_LOSS_CALL, check_step_against_oracle, compare_last_step, device_dataset, random_x,
                         require_cuda)
 
 pytestmark = pytest.mark.gpu
@@ -335,6 +335,46 @@ def test_graph_replay_and_host_entry_point_equal_single_steps(binding):
         for h in range(steps):
             cg.outer_steps_host(torch.from_numpy(idx[h * s * b:(h + 1) * s * b].copy()), x1, s, b, cfg.eta, n_steps=1)
         assert torch.equal(xa.cpu(), x1)
+
+
+@pytest.mark.parametrize("overlap", [0, 1, 2], ids=["sequential", "gather-aside", "pipelined"])
+@pytest.mark.parametrize("ci,m,n,s,b", [(3, 6000, 520, 5, 32), (2, 5000, 1024, 3, 128)])
+def test_next_step_gather_on_the_side_branch_changes_nothing(binding, oracle_mod, ci, m, n, s, b, overlap):
+    """CASGD_OPT_OVERLAP: inside the graphs of casgd_outer_steps the next step's rows are gathered (mode 1), or gathered
+    and their Gram matrix computed (mode 2, the margin then being a kernel of its own), on a side branch beside this
+    step's recurrence and update. The iterate equals repeated casgd_outer_step bit for bit in every mode, and the last
+    step's exported intermediates (taken from the stage that step used) match oracle O1."""
+    cfg = synth.config(ci, m=m, n=n)
+    X_d, y_d, A_bits, y = device_dataset(cfg)
+    steps = 64 + 8 + 8 + 1                      # a 64-step graph, two 8-step graphs, a single
+    idx = np.concatenate([synth.epoch_indices(cfg, 42, e) for e in range(-(-steps * s * b // m) + 1)])[: steps * s * b].copy()
+    idx_d = torch.from_numpy(idx).cuda()
+    eta = cfg.eta * 0.25
+    with binding.Casgd(X_d, y_d, cfg.loss) as cg:
+        cg.set_option(binding.OPT_OVERLAP, overlap)
+        xa = torch.zeros(cfg.n, device="cuda")
+        for h in range(steps - 9):
+            cg.outer_step(idx_d[h * s * b:(h + 1) * s * b], xa, s, b, eta)
+        xb = torch.zeros(cfg.n, device="cuda")
+        cg.outer_steps(idx_d[: (steps - 9) * s * b], xb, s, b, eta)      # 64 + 8: ends on an 8-step graph (stage 1)
+        cg.sync()
+        assert torch.equal(xa, xb)
+        x0 = xb.cpu().numpy().copy()
+        cg.outer_steps(idx_d[(steps - 9) * s * b: (steps - 1) * s * b], xb, s, b, eta)
+        cg.sync()
+        for h in range(steps - 9, steps - 2):
+            cg.outer_step(idx_d[h * s * b:(h + 1) * s * b], xa, s, b, eta)
+        x_before_last = xa.cpu().numpy().copy()
+        cg.outer_step(idx_d[(steps - 2) * s * b:(steps - 1) * s * b], xa, s, b, eta)
+        cg.sync()
+        assert torch.equal(xa, xb)
+        # the last step of the 8-step graph, against the oracle from the same FP32 bits
+        xc = torch.from_numpy(x0.copy()).cuda()
+        cg.outer_steps(idx_d[(steps - 9) * s * b: (steps - 1) * s * b], xc, s, b, eta)
+        cg.sync()
+        last = idx[(steps - 2) * s * b:(steps - 1) * s * b]
+        ref = oracle_mod.outer_step_gram(A_bits, y, last, x_before_last.astype(np.float64), s, b, eta, cfg.loss, shadow=True)
+        compare_last_step(oracle_mod, cg, ref, y[last], x_before_last, xc, s, b, eta, cfg.loss, binding)
 
 
 @pytest.mark.parametrize("ci,m,n,s,b", [(1, 20000, 18, 5, 64), (4, 6000, 512, 3, 64), (0, 4097, 64, 7, 13)])
