@@ -185,12 +185,19 @@ int casgd_debug_export(casgd_ctx *c, int what, void *dst_host, int64_t dst_bytes
  *                              (CASGD_STAGE_MARGIN) instead of extra B-operand rows of the Gram.
  *   CASGD_OPT_CHAIN_SMS        SMs left to the margin / recurrence / update chain in the pipelined schedule (the Gram and
  *                              gather kernels are sized for the rest). 0 (default) = chosen per shape.
+ *   CASGD_OPT_MARGIN_SPLIT     0 (default) = Recipe C of Table 3: x enters the margin r = Y x as its BF16
+ *                              shadow (L231, "two BF16 input conversions"). 1 = the margin sees the FP32 MASTER: rows 1
+ *                              and 2 of the shadow buffer carry the BF16 residues of x (hi + lo + lo2 == x exactly), the
+ *                              fused margin sums three accumulator columns, and the stand-alone margin kernel reads x
+ *                              itself -- with A stored in BF16 this is Recipe B (u_A = b, every compute slot f): BF16 x
+ *                              BF16 products are exact in FP32, so G and g are already what FP32 compute gives. Removes
+ *                              the x half of Eq. 8's 2 u_16 term (L229) at no extra MMA.
  *   CASGD_OPT_LOSS_IMPL        0 = casgd_loss streams A through per-warp cp.async.bulk shared-memory rings
  *                              (default; n <= 8192), 1 = the plain 16-byte-load kernel. */
 typedef enum {
     CASGD_OPT_GRAM_IMPL = 0, CASGD_OPT_GRAM_FULL_LOWER = 1, CASGD_OPT_PROFILE = 2, CASGD_OPT_NO_GRAPH = 3,
     CASGD_OPT_GRAM_KSPLIT = 4, CASGD_OPT_RECURRENCE_IMPL = 5, CASGD_OPT_LOSS_IMPL = 6, CASGD_OPT_NO_FUSED_UPDATE = 7,
-    CASGD_OPT_STAMPS = 8, CASGD_OPT_OVERLAP = 9, CASGD_OPT_CHAIN_SMS = 10
+    CASGD_OPT_STAMPS = 8, CASGD_OPT_OVERLAP = 9, CASGD_OPT_CHAIN_SMS = 10, CASGD_OPT_MARGIN_SPLIT = 11
 } casgd_option;
 int casgd_set_option(casgd_ctx *c, int option, int64_t value);
 

@@ -94,7 +94,7 @@ struct casgd_ctx {
     unsigned long long *stamps = nullptr;     // CASGD_OPT_STAMPS: [kStampSteps * 8][2] slots, accum_ns[8], count[8], raw copy of the slots
     int cur_slot_step = 0;                    // step index (inside the graph being captured) the next stage stamps into
     int64_t opt_stamps = 0;
-    int64_t opt_gram_impl = 0, opt_full_lower = 0, opt_profile = 0, opt_no_graph = 0, opt_ksplit = 0, opt_rec_impl = 0, opt_loss_impl = 0, opt_no_fuse = 0, opt_overlap = 2, opt_chain_sms = 0;
+    int64_t opt_gram_impl = 0, opt_full_lower = 0, opt_profile = 0, opt_no_graph = 0, opt_ksplit = 0, opt_rec_impl = 0, opt_loss_impl = 0, opt_no_fuse = 0, opt_overlap = 2, opt_chain_sms = 0, opt_split = 0;
     GramTcPlan *tc_plan = nullptr;
     GramPairPlan *pair_plan = nullptr;
     int pair_plan_sms = 0;
@@ -273,7 +273,7 @@ int stage_gram(casgd_ctx *c, cudaStream_t st, const int32_t *idx, const StepPara
                                yI, G, c->ldg, r_out, (int)c->opt_full_lower, c->err_flag, step_is_s1(c, s) ? &s1f : nullptr);
         if (k < 0) return fail(c, CASGD_ECUDA, "gram_narrow launch: %s", cudaGetErrorString(cudaGetLastError()));
     } else if (c->cur_gram == 1) {
-        k = launch_gram_simt(st, Y, c->ldy, c->n, sb, b, c->xbf, G, c->ldg, r_out, (int)c->opt_full_lower);
+        k = launch_gram_simt(st, Y, c->ldy, c->n, sb, b, c->xbf, c->opt_split ? c->ldxb : 0, G, c->ldg, r_out, (int)c->opt_full_lower);
     } else if (c->cur_gram == 3) {
         k = launch_gram_pair(st, c->pair_plan, row_base, sb, b, G, c->ldg, r_out, (int)c->opt_full_lower, c->cur_bn,
                              (int)c->opt_ksplit, c->err, sizeof c->err);
@@ -290,10 +290,11 @@ int stage_gram(casgd_ctx *c, cudaStream_t st, const int32_t *idx, const StepPara
     return CASGD_OK;
 }
 
-int stage_margin(casgd_ctx *c, cudaStream_t st, int32_t sb, int buf, int64_t *kernels)
+int stage_margin(casgd_ctx *c, cudaStream_t st, const float *x, const StepParams *ind, int32_t sb, int buf, int64_t *kernels)
 {
     StageTimer t(c, CASGD_STAGE_MARGIN);
-    const int k = launch_margin(st, c->Y + (size_t)buf * c->rows_alloc * c->ldy, c->ldy, sb, c->xbf, c->r, c->chain_sms);
+    const int k = launch_margin(st, c->Y + (size_t)buf * c->rows_alloc * c->ldy, c->ldy, c->n, sb, c->xbf, x, ind, c->opt_split != 0,
+                                c->r, c->chain_sms);
     t.done(k); *kernels += k;
     return CASGD_OK;
 }
@@ -310,7 +311,7 @@ int stage_chain(casgd_ctx *c, cudaStream_t st, float *x, const StepParams *ind, 
     const bool fused = !c->opt_no_fuse && recurrence_fuses_update(s, b, c->ldg, c->ldy, c->rws, (int)c->opt_rec_impl);
     if (!step_is_s1(c, s)) {
         StageTimer t(c, CASGD_STAGE_RECURRENCE);
-        const FusedUpdate fu{Y, c->ldy, c->n, x, ind, c->xbf};
+        const FusedUpdate fu{Y, c->ldy, c->n, x, ind, c->xbf, c->opt_split ? c->ldxb : 0};
         c->rws.late_trigger = late_trigger;
         k = launch_recurrence(st, G, c->ldg, c->r, yI, s, b, alpha, c->loss, c->z, c->u, c->rws,
                               (int)c->opt_rec_impl, fused ? &fu : nullptr);
@@ -322,6 +323,7 @@ int stage_chain(casgd_ctx *c, cudaStream_t st, float *x, const StepParams *ind, 
     if (!fused) {
         StageTimer t(c, CASGD_STAGE_GRADIENT);
         c->gws.num_sms = c->chain_sms;
+        c->gws.split_ld = c->opt_split ? c->ldxb : 0;
         k = launch_gradient_bf16(st, Y, c->ldy, c->n, sb, c->u, alpha, x, ind, c->xbf, c->gws);
         t.done(k); *kernels += k;
     }
@@ -342,14 +344,14 @@ int enqueue_step(casgd_ctx *c, cudaStream_t st, const int32_t *idx, const StepPa
     if (s1 && c->cur_gram != 4) {
         // wide rows: gather + margin + l' in one warp-per-row kernel (there is no Gram at s = 1)
         StageTimer t(c, CASGD_STAGE_GRAM);
-        const int k = launch_margin_s1(st, c->A, c->lda, c->y, c->m, c->n, idx, ind, idx_off, b, c->loss, c->xbf,
+        const int k = launch_margin_s1(st, c->A, c->lda, c->y, c->m, c->n, idx, ind, idx_off, b, c->loss, c->xbf, c->opt_split ? c->ldxb : 0,
                                        c->Y + (size_t)io.buf * c->rows_alloc * c->ldy, c->ldy, c->yI + (size_t)io.buf * c->rows_alloc,
                                        c->r, c->z, c->u, c->err_flag);
         t.done(k); *kernels += k;
     } else {
         if (c->cur_gram != 4 && !io.gathered && (rc = stage_gather(c, st, idx, ind, idx_off, sb, io.buf, c->gram_sms, kernels))) return rc;
         if ((rc = stage_gram(c, st, idx, ind, idx_off, s, b, io.buf, split_margin ? nullptr : c->r, kernels))) return rc;
-        if (split_margin && (rc = stage_margin(c, st, sb, io.buf, kernels))) return rc;
+        if (split_margin && (rc = stage_margin(c, st, x, ind, sb, io.buf, kernels))) return rc;
     }
     const bool side = io.next_idx_off >= 0;
     std::function<void()> none;
@@ -410,7 +412,7 @@ int capture_pipelined(casgd_ctx *c, int32_t s, int32_t b, float eta, int32_t len
         const int buf = h & 1;
         c->cur_slot_step = h;
         cudaStreamWaitEvent(M, c->ev_gather[buf], 0);
-        if ((rc = stage_margin(c, M, sb, buf, kernels))) break;
+        if ((rc = stage_margin(c, M, nullptr, c->ind, sb, buf, kernels))) break;
         cudaStreamWaitEvent(M, c->ev_gram[buf], 0);
         const bool more = h + 1 < len;
         if (more) g_completion_event = c->ev_rec_launch;
@@ -494,7 +496,7 @@ int choose_gram(casgd_ctx *c, int32_t s, int32_t b)
 int ensure_shadow(casgd_ctx *c, const float *x)
 {
     StageTimer t(c, CASGD_STAGE_OTHER);
-    int k = launch_shadow(c->stream, x, nullptr, c->n, c->xbf);
+    int k = launch_shadow(c->stream, x, nullptr, c->n, c->xbf, c->ldxb, (int)c->opt_split);
     t.done(k);
     c->shadow_of = x;
     c->shadow_valid = true;
@@ -880,6 +882,7 @@ int casgd_set_option(casgd_ctx *c, int option, int64_t value)
     case CASGD_OPT_OVERLAP:
         if (value < 0 || value > 2) return fail(c, CASGD_EINVAL, "CASGD_OPT_OVERLAP must be 0, 1 or 2");
         c->opt_overlap = value; break;
+    case CASGD_OPT_MARGIN_SPLIT: c->opt_split = value != 0; break;
     case CASGD_OPT_CHAIN_SMS:
         if (value < 0 || value > 1024) return fail(c, CASGD_EINVAL, "CASGD_OPT_CHAIN_SMS must be in [0, 1024]");
         c->opt_chain_sms = value; break;

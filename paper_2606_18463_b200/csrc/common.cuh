@@ -32,6 +32,23 @@ __device__ __forceinline__ uint16_t f32_to_bf16_bits_rn(float f)
     return __bfloat16_as_ushort(__float2bfloat16_rn(f));
 }
 
+// The BF16 view of x the margin reads. Row 0 of the [16 x ldxb] shadow buffer is bf16_rne(x). With
+// CASGD_OPT_MARGIN_SPLIT (split_ld = ldxb, else 0) rows 1 and 2 carry the BF16 residues lo = bf16(x - hi) and
+// lo2 = bf16(x - hi - lo): hi + lo + lo2 == x exactly (3 x 8 significand bits), every BF16 x BF16 product is exact
+// in FP32, so the three accumulator columns of the fused margin sum to Y x with x the FP32 MASTER: the 2 u_16
+// input-conversion term of Eq. 8 (L229) loses its x half at no extra MMA (the B operand has 16 rows anyway).
+__device__ __forceinline__ void store_shadow(uint16_t *xbf, int32_t split_ld, int col, float xn)
+{
+    const __nv_bfloat16 hi = __float2bfloat16_rn(xn);
+    xbf[col] = __bfloat16_as_ushort(hi);
+    if (split_ld) {
+        const float r1 = xn - __bfloat162float(hi);
+        const __nv_bfloat16 lo = __float2bfloat16_rn(r1);
+        xbf[split_ld + col] = __bfloat16_as_ushort(lo);
+        xbf[2 * split_ld + col] = __bfloat16_as_ushort(__float2bfloat16_rn(r1 - __bfloat162float(lo)));
+    }
+}
+
 // u = dL/dr = -delta. Accurate expf (not __expf): Poisson amplifies margin error by e^z.
 template <int LOSS>
 __device__ __forceinline__ float lprime(float z, float y)
@@ -214,7 +231,7 @@ int launch_gather(cudaStream_t st, const uint16_t *A, int64_t lda, const float *
                   float *yI, int *err_flag, int num_sms);
 
 int launch_gram_simt(cudaStream_t st, const uint16_t *Y, int32_t ldy, int32_t n, int32_t sb, int32_t b,
-                     const uint16_t *xbf, float *G, int32_t ldg, float *r, int full_lower);
+                     const uint16_t *xbf, int32_t split_ld, float *G, int32_t ldg, float *r, int full_lower);
 
 // Cross-SM state of the grid-wide recurrence kernel (recurrence.cu).
 struct RecWorkspace {
@@ -241,6 +258,7 @@ struct FusedUpdate {
     float *x;
     const StepParams *ind;
     uint16_t *xbf;
+    int32_t split_ld;              // CASGD_OPT_MARGIN_SPLIT: row stride of the shadow buffer (0 = row 0 only)
 };
 bool recurrence_fuses_update(int32_t s, int32_t b, int32_t ldg, int32_t ldy, const RecWorkspace &ws, int impl);
 int recurrence_kernel_choice(int32_t s, int32_t b, int32_t ldg, const RecWorkspace &ws, int impl, bool fused);
@@ -261,6 +279,7 @@ struct GradWorkspace {
     unsigned *counters;    // one per column tile, zero between launches
     int32_t max_splits;
     int32_t num_sms;       // SMs of the context's device (grid sizing)
+    int32_t split_ld;      // CASGD_OPT_MARGIN_SPLIT: row stride of the shadow buffer (0 = row 0 only)
 };
 
 int launch_gradient_bf16(cudaStream_t st, const uint16_t *Y, int32_t ldy, int32_t n, int32_t sb, const float *u,
@@ -268,11 +287,13 @@ int launch_gradient_bf16(cudaStream_t st, const uint16_t *Y, int32_t ldy, int32_
 
 // s = 1 with wide rows: gather + margin + l' in one warp-per-row kernel (no Gram exists at s = 1); gradient.cu
 // r = Y x_bf (Alg. 1 line 3) as a kernel of its own: the pipelined schedule computes G(t+1) before x(t+1) exists
-int launch_margin(cudaStream_t st, const uint16_t *Y, int32_t ldy, int32_t sb, const uint16_t *xbf, float *r, int num_sms);
+// x32 / ind non-null (CASGD_OPT_MARGIN_SPLIT): the margin of the FP32 master itself, r = Y x
+int launch_margin(cudaStream_t st, const uint16_t *Y, int32_t ldy, int32_t n, int32_t sb, const uint16_t *xbf, const float *x32,
+                  const StepParams *ind, bool exact, float *r, int num_sms);
 
 int launch_margin_s1(cudaStream_t st, const uint16_t *A, int64_t lda, const float *y, int64_t m, int32_t n,
                      const int32_t *idx, const StepParams *ind, int64_t idx_off, int32_t b, int loss, const uint16_t *xbf,
-                     uint16_t *Y, int32_t ldy, float *yI, float *r, float *z, float *u, int *err_flag);
+                     int32_t split_ld, uint16_t *Y, int32_t ldy, float *yI, float *r, float *z, float *u, int *err_flag);
 
 int launch_sgd32_step(cudaStream_t st, const float *A32, int64_t lda32, const float *y, int64_t m, int32_t n,
                       const int32_t *idx, int32_t b, float alpha, int loss, float *x, float *u, float *z,
@@ -284,7 +305,7 @@ int launch_loss(cudaStream_t st, const uint16_t *A, int64_t lda, const uint16_t 
 
 int launch_sample_indices(cudaStream_t st, int32_t *idx, int64_t n_steps, int32_t sb, int64_t m, uint64_t seed,
                           uint64_t first_step);
-int launch_shadow(cudaStream_t st, const float *x, const StepParams *ind, int32_t n, uint16_t *xbf);
+int launch_shadow(cudaStream_t st, const float *x, const StepParams *ind, int32_t n, uint16_t *xbf, int32_t ldxb, int split);
 int launch_widen(cudaStream_t st, const uint16_t *A, int64_t lda, int64_t m, int32_t n, float *A32, int64_t lda32, int num_sms);
 int launch_repack(cudaStream_t st, const uint16_t *X, int64_t ldx, int64_t m, int32_t n, uint16_t *A, int64_t lda, int num_sms);
 int launch_set_params(cudaStream_t st, StepParams *ind, const int32_t *idx, float *x);

@@ -179,18 +179,20 @@ int launch_gather(cudaStream_t st, const uint16_t *A, int64_t lda, const float *
 
 // x_bf = bf16_rne(x): the margin kernel's view of the weights.
 __global__ void shadow_kernel(const float *x, const StepParams *ind, int32_t n,
-                              uint16_t *xbf)
+                              uint16_t *xbf, int32_t ldxb, int split)
 {
     pdl_trigger();
     pdl_wait();
     const float *xs = ind ? ind->x : x;
     int32_t k = blockIdx.x * blockDim.x + threadIdx.x;
-    if (k < n) xbf[k] = f32_to_bf16_bits_rn(xs[k]);
+    if (k >= n) return;
+    store_shadow(xbf, split ? ldxb : 0, k, xs[k]);
+    if (!split) xbf[ldxb + k] = xbf[2 * ldxb + k] = 0;      // the residue rows read as zero when the split is off
 }
 
-int launch_shadow(cudaStream_t st, const float *x, const StepParams *ind, int32_t n, uint16_t *xbf)
+int launch_shadow(cudaStream_t st, const float *x, const StepParams *ind, int32_t n, uint16_t *xbf, int32_t ldxb, int split)
 {
-    launch_pdl(shadow_kernel, dim3((n + 255) / 256), dim3(256), 0, st, 1, x, ind, n, xbf);
+    launch_pdl(shadow_kernel, dim3((n + 255) / 256), dim3(256), 0, st, 1, x, ind, n, xbf, ldxb, split);
     return 1;
 }
 

@@ -37,7 +37,7 @@ template <typename T, bool GATHER, bool SHADOW>
 __global__ void __launch_bounds__(kGradThreads)
 gradient_update_kernel(const T *base, int64_t ld, const int32_t *idx, int64_t m, int32_t n,
                        int32_t rows, int32_t rows_per_split, int32_t CV, const float *u, float alpha,
-                       float *x_direct, const StepParams *ind, uint16_t *xbf,
+                       float *x_direct, const StepParams *ind, uint16_t *xbf, int32_t split_ld,
                        float *partial, int32_t ldp, unsigned *counters, unsigned long long *stamp)
 {
     constexpr int kVec = VecTraits<T>::kVec;
@@ -107,7 +107,7 @@ gradient_update_kernel(const T *base, int64_t ld, const int32_t *idx, int64_t m,
         for (unsigned q = 0; q < gridDim.y; ++q) g += __ldcg(&partial[(int64_t)q * ldp + col]);
         const float xn = fmaf(-alpha, g, x[col]);
         x[col] = xn;
-        if (SHADOW) xbf[col] = f32_to_bf16_bits_rn(xn);
+        if (SHADOW) store_shadow(xbf, split_ld, col, xn);
     }
     if (tid == 0) counters[blockIdx.x] = 0u;
     __syncthreads();
@@ -127,7 +127,7 @@ constexpr size_t kGsSmem = (size_t)kGsWarps * kGsDepth * kGsPiece + (size_t)kGsW
 __global__ void __launch_bounds__(32 * kGsWarps, 1)
 gradient_stream_kernel(const uint16_t *Y, int32_t ldy, int32_t n, int32_t sb, int32_t rpw,
                        const float *u, float alpha, float *x_direct,
-                       const StepParams *ind, uint16_t *xbf, float *partial,
+                       const StepParams *ind, uint16_t *xbf, int32_t split_ld, float *partial,
                        int32_t ldp, unsigned *counters, unsigned long long *stamp)
 {
     extern __shared__ __align__(128) unsigned char gs_smem[];
@@ -229,12 +229,12 @@ gradient_stream_kernel(const uint16_t *Y, int32_t ldy, int32_t n, int32_t sb, in
         if (col < n) {
             const float xn = fmaf(-alpha, gx, x[col]);
             x[col] = xn;
-            xbf[col] = f32_to_bf16_bits_rn(xn);
+            store_shadow(xbf, split_ld, col, xn);
         }
         if (col + 1 < n) {
             const float xn = fmaf(-alpha, gy, x[col + 1]);
             x[col + 1] = xn;
-            xbf[col + 1] = f32_to_bf16_bits_rn(xn);
+            store_shadow(xbf, split_ld, col + 1, xn);
         }
     }
     if (threadIdx.x == 0) counters[blockIdx.x] = 0u;
@@ -258,7 +258,7 @@ static int launch_gradient_stream(cudaStream_t st, const uint16_t *Y, int32_t ld
     const int slabs = (sb + kGsWarps * rpw - 1) / (kGsWarps * rpw);
     if (slabs > ws.max_splits) return 0;
     launch_pdl(gradient_stream_kernel, dim3(col_segs, slabs), dim3(32 * kGsWarps), kGsSmem, st, 1, Y, ldy, n, sb, rpw, u, alpha, x,
-               ind, xbf, ws.partial, ws.ldp, ws.counters, g_stamp);
+               ind, xbf, ws.split_ld, ws.partial, ws.ldp, ws.counters, g_stamp);
     return 1;
 }
 
@@ -281,7 +281,7 @@ static int launch_gradient_any(cudaStream_t st, const T *base, int64_t ld, const
     splits = (rows + rows_per_split - 1) / rows_per_split;
     dim3 grid(col_tiles, splits);
     launch_pdl(gradient_update_kernel<T, GATHER, SHADOW>, grid, dim3(kGradThreads), 0, st, 1, base, ld, idx, m, n, rows,
-               rows_per_split, CV, u, alpha, x, ind, xbf, ws.partial, ws.ldp, ws.counters, SHADOW ? g_stamp : nullptr);
+               rows_per_split, CV, u, alpha, x, ind, xbf, ws.split_ld, ws.partial, ws.ldp, ws.counters, SHADOW ? g_stamp : nullptr);
     return 1;
 }
 
@@ -317,11 +317,49 @@ __device__ __forceinline__ float dot8_bf16(const uint4 &a, const uint4 &x, float
 }
 
 __global__ void __launch_bounds__(32 * kMgWarps)
-margin_kernel(const uint16_t *Y, int32_t ldy, int32_t sb, const uint16_t *xbf, float *r, unsigned long long *stamp)
+margin_kernel(const uint16_t *Y, int32_t ldy, int32_t sb, const uint16_t *xbf, const float *x32, const StepParams *ind,
+              int exact, float *r, unsigned long long *stamp)
 {
     pdl_trigger();
     pdl_wait();                                     // x_bf comes from the previous update, Y from the gather
     stamp_begin(stamp);
+    if (exact) {
+        // CASGD_OPT_MARGIN_SPLIT: the margin of the FP32 master (Recipe B's u_r = f, Table 3): r = Y x.
+        // Columns beyond n are zero in Y; x has exactly n entries, so the last vector of a row is guarded.
+        const float *xs = ind ? ind->x : x32;
+        const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+        const int gw = blockIdx.x * kMgWarps + warp, W = gridDim.x * kMgWarps;
+        const int nvec = ldy >> 3, n = exact;       // (exact carries n)
+        for (int row = gw; row < sb; row += W) {
+            const uint16_t *yr = Y + (int64_t)row * ldy;
+            float acc = 0.f;
+            for (int cv0 = lane; cv0 < nvec; cv0 += 128) {
+                uint4 v[4];
+#pragma unroll
+                for (int q = 0; q < 4; ++q) {
+                    const int cv = cv0 + 32 * q;
+                    v[q] = make_uint4(0u, 0u, 0u, 0u);
+                    if (cv < nvec) v[q] = ld_stream_v4(yr + cv * 8);
+                }
+#pragma unroll
+                for (int q = 0; q < 4; ++q) {
+                    const int col = (cv0 + 32 * q) * 8;
+                    if (col >= n) continue;
+                    float xv[8];
+#pragma unroll
+                    for (int e = 0; e < 8; ++e) xv[e] = col + e < n ? ld_dep(xs + col + e) : 0.f;
+                    acc = fmaf(bf16lo(v[q].x), xv[0], acc); acc = fmaf(bf16hi(v[q].x), xv[1], acc);
+                    acc = fmaf(bf16lo(v[q].y), xv[2], acc); acc = fmaf(bf16hi(v[q].y), xv[3], acc);
+                    acc = fmaf(bf16lo(v[q].z), xv[4], acc); acc = fmaf(bf16hi(v[q].z), xv[5], acc);
+                    acc = fmaf(bf16lo(v[q].w), xv[6], acc); acc = fmaf(bf16hi(v[q].w), xv[7], acc);
+                }
+            }
+            acc = warp_sum(acc);
+            if (lane == 0) r[row] = acc;
+        }
+        stamp_end_warp(stamp);
+        return;
+    }
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int gw = blockIdx.x * kMgWarps + warp, W = gridDim.x * kMgWarps;
     const int nvec = ldy >> 3;
@@ -353,12 +391,13 @@ margin_kernel(const uint16_t *Y, int32_t ldy, int32_t sb, const uint16_t *xbf, f
     stamp_end_warp(stamp);
 }
 
-int launch_margin(cudaStream_t st, const uint16_t *Y, int32_t ldy, int32_t sb, const uint16_t *xbf, float *r, int num_sms)
+int launch_margin(cudaStream_t st, const uint16_t *Y, int32_t ldy, int32_t n, int32_t sb, const uint16_t *xbf, const float *x32,
+                  const StepParams *ind, bool exact, float *r, int num_sms)
 {
     const int pairs = (sb + 1) / 2;
     // two CTAs per SM at most: 32 warps x 2 rows x 4 x 16-byte loads per lane = 128 KB in flight per SM
     const int blocks = std::max(1, std::min(2 * num_sms, (pairs + kMgWarps - 1) / kMgWarps));
-    launch_pdl(margin_kernel, dim3(blocks), dim3(32 * kMgWarps), 0, st, 1, Y, ldy, sb, xbf, r, g_stamp);
+    launch_pdl(margin_kernel, dim3(blocks), dim3(32 * kMgWarps), 0, st, 1, Y, ldy, sb, xbf, x32, ind, exact ? n : 0, r, g_stamp);
     return 1;
 }
 
@@ -370,7 +409,8 @@ int launch_margin(cudaStream_t st, const uint16_t *Y, int32_t ldy, int32_t sb, c
 __global__ void __launch_bounds__(256)
 margin_s1_kernel(const uint16_t *__restrict__ A, int64_t lda, const float *__restrict__ y, int64_t m, int32_t n,
                  const int32_t *idx, const StepParams *ind, int64_t idx_off, int32_t b, int loss, const uint16_t *xbf,
-                 uint16_t *Y, int32_t ldy, float *yI, float *r, float *z, float *u, int *err_flag, unsigned long long *stamp)
+                 int32_t split_ld, uint16_t *Y, int32_t ldy, float *yI, float *r, float *z, float *u, int *err_flag,
+                 unsigned long long *stamp)
 {
     pdl_trigger();
     pdl_wait();                                     // x_bf comes from the previous gradient; Y is read by it until now
@@ -415,6 +455,10 @@ margin_s1_kernel(const uint16_t *__restrict__ A, int64_t lda, const float *__res
             acc = fmaf(bf16lo(v[q].y), bf16lo(xv[q].y), acc); acc = fmaf(bf16hi(v[q].y), bf16hi(xv[q].y), acc);
             acc = fmaf(bf16lo(v[q].z), bf16lo(xv[q].z), acc); acc = fmaf(bf16hi(v[q].z), bf16hi(xv[q].z), acc);
             acc = fmaf(bf16lo(v[q].w), bf16lo(xv[q].w), acc); acc = fmaf(bf16hi(v[q].w), bf16hi(xv[q].w), acc);
+            if (split_ld) {                          // CASGD_OPT_MARGIN_SPLIT: the residue rows of the shadow
+                acc = dot8_bf16(v[q], ld_dep_v4(xbf + split_ld + col), acc);
+                acc = dot8_bf16(v[q], ld_dep_v4(xbf + 2 * split_ld + col), acc);
+            }
         }
     }
     acc = warp_sum(acc);
@@ -431,10 +475,10 @@ margin_s1_kernel(const uint16_t *__restrict__ A, int64_t lda, const float *__res
 
 int launch_margin_s1(cudaStream_t st, const uint16_t *A, int64_t lda, const float *y, int64_t m, int32_t n,
                      const int32_t *idx, const StepParams *ind, int64_t idx_off, int32_t b, int loss, const uint16_t *xbf,
-                     uint16_t *Y, int32_t ldy, float *yI, float *r, float *z, float *u, int *err_flag)
+                     int32_t split_ld, uint16_t *Y, int32_t ldy, float *yI, float *r, float *z, float *u, int *err_flag)
 {
-    launch_pdl(margin_s1_kernel, dim3((b * 32 + 255) / 256), dim3(256), 0, st, 1, A, lda, y, m, n, idx, ind, idx_off, b, loss, xbf, Y,
-               ldy, yI, r, z, u, err_flag, g_stamp);
+    launch_pdl(margin_s1_kernel, dim3((b * 32 + 255) / 256), dim3(256), 0, st, 1, A, lda, y, m, n, idx, ind, idx_off, b, loss, xbf,
+               split_ld, Y, ldy, yI, r, z, u, err_flag, g_stamp);
     return 1;
 }
 

@@ -164,6 +164,15 @@ __device__ __forceinline__ uint32_t tc_ld1(uint32_t taddr)
     return v;
 }
 __device__ __forceinline__ void tc_wait_ld() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
+__device__ __forceinline__ float tc_ld_margin(uint32_t taddr)
+{
+    // the margin's accumulator columns 0..3 = Y . (rows 0..3 of the x_bf operand): row 0 is bf16(x); rows 1 and 2 are
+    // zero, or its BF16 residues with CASGD_OPT_MARGIN_SPLIT; row 3 is zero. Their sum is r either way (c + 0 == c).
+    uint32_t a, b, c, d;
+    asm volatile("tcgen05.ld.sync.aligned.32x32b.x4.b32 {%0, %1, %2, %3}, [%4];" : "=r"(a), "=r"(b), "=r"(c), "=r"(d) : "r"(taddr) : "memory");
+    asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+    return (__uint_as_float(a) + __uint_as_float(b)) + (__uint_as_float(c) + __uint_as_float(d));
+}
 
 // K-major, 128-byte swizzle: rows of 64 BF16 (128 B), 8-row groups 1024 B apart (SBO), descriptor version 1.
 __device__ __forceinline__ uint64_t umma_desc_sw128(uint32_t saddr)
@@ -359,14 +368,13 @@ gram_pair_kernel(const __grid_constant__ CUtensorMap tmY, const __grid_constant_
                     __syncwarp();
                 }
             } else {
-                const uint32_t rv = tc_ld1(t_row);                         // column 0 of the N = 16 accumulator: Y x_bf
-                tc_wait_ld();
+                const float rv = tc_ld_margin(t_row);                      // columns 0..3 of the N = 16 accumulator: Y x_bf
                 if (p.mslices == 1) {
-                    if (row_ok) p.r[row] = __uint_as_float(rv);
+                    if (row_ok) p.r[row] = rv;
                 } else {
                     // a K slice of the margin (slice index in w.J): park the partial sum; the slice that finishes last
                     // adds the parts in slice order (deterministic) and writes r
-                    if (row_ok) p.rpart[(int64_t)w.J * p.ldr + row] = __uint_as_float(rv);
+                    if (row_ok) p.rpart[(int64_t)w.J * p.ldr + row] = rv;
                     __threadfence();
                     asm volatile("bar.sync 1, 128;" ::: "memory");             // the four epilogue warps
                     if (warp == 2 && lane == 0) {

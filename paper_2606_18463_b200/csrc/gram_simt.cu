@@ -68,24 +68,27 @@ gram_simt_kernel(const uint16_t *__restrict__ Y, int32_t ldy, int32_t n, int32_t
 
 // r = Y x_bf, one warp per row, FP32 accumulation.
 __global__ void __launch_bounds__(256)
-margin_simt_kernel(const uint16_t *__restrict__ Y, int32_t ldy, int32_t n, int32_t sb, const uint16_t *__restrict__ xbf,
+margin_simt_kernel(const uint16_t *__restrict__ Y, int32_t ldy, int32_t n, int32_t sb, const uint16_t *xbf, int32_t split_ld,
                    float *__restrict__ r)
 {
     const int warp = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
     if (warp >= sb) return;
     float acc = 0.f;
-    for (int k = lane; k < n; k += 32)
-        acc = fmaf(bf16_bits_to_f32(Y[(int64_t)warp * ldy + k]), bf16_bits_to_f32(xbf[k]), acc);
+    for (int k = lane; k < n; k += 32) {
+        float xv = bf16_bits_to_f32(xbf[k]);
+        if (split_ld) xv += bf16_bits_to_f32(xbf[split_ld + k]) + bf16_bits_to_f32(xbf[2 * split_ld + k]);   // == x, exactly
+        acc = fmaf(bf16_bits_to_f32(Y[(int64_t)warp * ldy + k]), xv, acc);
+    }
     acc = warp_sum(acc);
     if (lane == 0) r[warp] = acc;
 }
 
 int launch_gram_simt(cudaStream_t st, const uint16_t *Y, int32_t ldy, int32_t n, int32_t sb, int32_t b,
-                     const uint16_t *xbf, float *G, int32_t ldg, float *r, int full_lower)
+                     const uint16_t *xbf, int32_t split_ld, float *G, int32_t ldg, float *r, int full_lower)
 {
     const int T = (sb + ST - 1) / ST;
     int launches = 1;
-    margin_simt_kernel<<<(sb * 32 + 255) / 256, 256, 0, st>>>(Y, ldy, n, sb, xbf, r);
+    margin_simt_kernel<<<(sb * 32 + 255) / 256, 256, 0, st>>>(Y, ldy, n, sb, xbf, split_ld, r);
     if (full_lower || sb > b) {
         gram_simt_kernel<<<T * (T + 1) / 2, 256, 0, st>>>(Y, ldy, n, sb, b, G, ldg, T, full_lower);
         ++launches;

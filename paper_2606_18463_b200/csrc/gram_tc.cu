@@ -108,6 +108,15 @@ __device__ __forceinline__ uint32_t tc_ld1(uint32_t taddr)
     return v;
 }
 __device__ __forceinline__ void tc_wait_ld() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
+__device__ __forceinline__ float tc_ld_margin(uint32_t taddr)
+{
+    // the margin's accumulator columns 0..3 = Y . (rows 0..3 of the x_bf operand): row 0 is bf16(x); rows 1 and 2 are
+    // zero, or its BF16 residues with CASGD_OPT_MARGIN_SPLIT; row 3 is zero. Their sum is r either way (c + 0 == c).
+    uint32_t a, b, c, d;
+    asm volatile("tcgen05.ld.sync.aligned.32x32b.x4.b32 {%0, %1, %2, %3}, [%4];" : "=r"(a), "=r"(b), "=r"(c), "=r"(d) : "r"(taddr) : "memory");
+    asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+    return (__uint_as_float(a) + __uint_as_float(b)) + (__uint_as_float(c) + __uint_as_float(d));
+}
 
 // K-major, 128-byte swizzle: rows of 64 BF16 (128 B), 8-row groups 1024 B apart (SBO), descriptor version 1.
 __device__ __forceinline__ uint64_t umma_desc_sw128(uint32_t saddr)
@@ -309,11 +318,10 @@ gram_tc_kernel(const __grid_constant__ CUtensorMap tmY, const __grid_constant__ 
                 }
             }
             if (k.diag && !p.no_margin) {
-                const uint32_t rv = tc_ld1(t_row + (k.need_g ? BN : 0));
-                tc_wait_ld();
+                const float rv = tc_ld_margin(t_row + (k.need_g ? BN : 0));
                 if (row_ok) {
-                    if (!accumulate) p.r[row] = __uint_as_float(rv);
-                    else atomicAdd(p.r + row, __uint_as_float(rv));
+                    if (!accumulate) p.r[row] = rv;
+                    else atomicAdd(p.r + row, rv);
                 }
             }
             tc_fence_before();
@@ -500,14 +508,13 @@ gram_narrow_kernel(const NarrowParams p)
         }
     }
     if (diag) {
-        const uint32_t rv = tc_ld1(t_row + (need_g ? BN : 0));
-        tc_wait_ld();
+        const float rv = tc_ld_margin(t_row + (need_g ? BN : 0));
         const int row = ti * BM + warp * 32 + lane;
         if (row < p.sb) {
-            p.r[row] = __uint_as_float(rv);
+            p.r[row] = rv;
             if (p.s1_loss >= 0) {                   // this thread gathered this very row: its label is in a register
-                p.z[row] = __uint_as_float(rv);
-                p.u[row] = lprime_rt(p.s1_loss, __uint_as_float(rv), ylab);
+                p.z[row] = rv;
+                p.u[row] = lprime_rt(p.s1_loss, rv, ylab);
             }
         }
     }

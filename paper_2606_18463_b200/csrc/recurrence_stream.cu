@@ -120,6 +120,7 @@ struct FusedGrad {
     float *x_direct;
     const StepParams *ind;
     uint16_t *xbf;
+    int32_t split_ld;
 };
 constexpr int kFgMaxLdy = 2048;                          // columns (padded) the fused update handles
 
@@ -506,7 +507,7 @@ recurrence_stream_kernel(const float *G, int32_t ldg, const float *r,
                 for (int q = 0; q < C; ++q) g += gbuf[q * ldy + col];
                 const float xn = fmaf(-alpha, g, x[col]);
                 x[col] = xn;
-                fg.xbf[col] = f32_to_bf16_bits_rn(xn);
+                store_shadow(fg.xbf, fg.split_ld, col, xn);
             }
         }
         REC_TRACE(3);
@@ -595,7 +596,7 @@ int launch_recurrence_stream(cudaStream_t st, const float *G, int32_t ldg, const
                              int late_trigger)
 {
     FusedGrad fg{};
-    if (fu) fg = FusedGrad{fu->Y, fu->ldy, fu->n, fu->x, fu->ind, fu->xbf};
+    if (fu) fg = FusedGrad{fu->Y, fu->ldy, fu->n, fu->x, fu->ind, fu->xbf, fu->split_ld};
     cudaError_t e = loss == CASGD_LOGISTIC ? launch_stream<CASGD_LOGISTIC>(st, G, ldg, r, yI, s, b, alpha, z, u, cluster, fg, late_trigger)
                   : loss == CASGD_LINEAR  ? launch_stream<CASGD_LINEAR>(st, G, ldg, r, yI, s, b, alpha, z, u, cluster, fg, late_trigger)
                                           : launch_stream<CASGD_POISSON>(st, G, ldg, r, yI, s, b, alpha, z, u, cluster, fg, late_trigger);

@@ -78,19 +78,20 @@ def chain_bounds(ref, y_idx, z_gpu, s, b, eta, loss, bound_r, bound_g, tol_scale
 
 
 def check_step_against_oracle(oracle, cg, A_bits, y, idx, x0, s, b, eta, loss, binding, full_lower=False,
-                              check_g=True, tol_scale=1.0):
+                              check_g=True, tol_scale=1.0, shadow=True):
     """Run one casgd_outer_step from the FP32 bits x0 and compare every exported intermediate with O1."""
     idx_d = torch.from_numpy(idx).cuda()
     x_d = torch.from_numpy(x0.copy()).cuda()
     cg.invalidate_shadow()
     cg.outer_step(idx_d, x_d, s, b, eta)
     cg.sync()
-    ref = oracle.outer_step_gram(A_bits, y, idx, x0.astype(np.float64), s, b, eta, loss, shadow=True)
-    return compare_last_step(oracle, cg, ref, y[idx], x0, x_d, s, b, eta, loss, binding, full_lower, check_g, tol_scale)
+    ref = oracle.outer_step_gram(A_bits, y, idx, x0.astype(np.float64), s, b, eta, loss, shadow=shadow)
+    return compare_last_step(oracle, cg, ref, y[idx], x0, x_d, s, b, eta, loss, binding, full_lower, check_g, tol_scale,
+                             shadow=shadow)
 
 
 def compare_last_step(oracle, cg, ref, y_idx, x0, x_d, s, b, eta, loss, binding, full_lower=False, check_g=True,
-                      tol_scale=1.0):
+                      tol_scale=1.0, shadow=True):
     """Compare the intermediates of the LAST outer step the context ran (casgd_debug_export) and the iterate
     `x_d` it left with `ref`, oracle O1's result for the same rows, labels `y_idx`, indices and FP32 x0 bits."""
     sb = s * b
@@ -101,7 +102,7 @@ def compare_last_step(oracle, cg, ref, y_idx, x0, x_d, s, b, eta, loss, binding,
 
     Yf = oracle.bf16_to_f64(ref.Y_bits)
     norms = np.sqrt((Yf * Yf).sum(axis=1))
-    xhat = oracle.bf16_to_f64(oracle.f32_to_bf16(x0))
+    xhat = oracle.bf16_to_f64(oracle.f32_to_bf16(x0)) if shadow else x0.astype(np.float64)   # (False: CASGD_OPT_MARGIN_SPLIT)
     xnorm = np.sqrt((xhat * xhat).sum())
 
     # margin (line 3)

@@ -377,6 +377,40 @@ def test_next_step_gather_on_the_side_branch_changes_nothing(binding, oracle_mod
         compare_last_step(oracle_mod, cg, ref, y[last], x_before_last, xc, s, b, eta, cfg.loss, binding)
 
 
+SPLIT_SHAPES = [(0, 8192, 64, 4, 16), (1, 20000, 18, 5, 64), (2, 4200, 4096, 3, 128), (3, 5000, 2000, 9, 32), (4, 6000, 512, 6, 64),
+                (4, 6000, 512, 1, 64), (2, 5000, 1024, 6, 128)]
+
+
+@pytest.mark.parametrize("mode", ["sequential-auto", "sequential-simt", "sequential-tile128", "sequential-pair256", "pipelined"])
+@pytest.mark.parametrize("ci,m,n,s,b", SPLIT_SHAPES)
+def test_margin_of_the_fp32_master(binding, oracle_mod, ci, m, n, s, b, mode):
+    """CASGD_OPT_MARGIN_SPLIT (Eq. 8, Table 3 column B): the margin is taken of
+    the FP32 master -- as three BF16 rows hi / lo / lo2 of the fused tensor-core margin, or by the stand-alone margin kernel
+    reading x itself -- so r, and the whole step, match oracle O1 run WITHOUT the BF16 shadow (shadow=False) at the same
+    1e-5 tolerances. A negative control shows the default (shadow) margin does not."""
+    cfg = synth.config(ci, m=m, n=n)
+    X_d, y_d, A_bits, y = device_dataset(cfg)
+    idx = synth.epoch_indices(cfg, 42, 0)[: s * b].copy()
+    x0 = random_x(n, 5, 0.7)
+    gram = {"sequential-auto": 0, "sequential-simt": 1, "sequential-tile128": 2, "sequential-pair256": 3, "pipelined": 0}[mode]
+    if gram == 3 and (n < 64 or s * b < 256):
+        pytest.skip("the pair kernel needs whole 256-row tiles worth of work")
+    with binding.Casgd(X_d, y_d, cfg.loss) as cg:
+        cg.set_option(binding.OPT_OVERLAP, 2 if mode == "pipelined" else 0)
+        cg.set_option(binding.OPT_GRAM_IMPL, gram)
+        cg.set_option(binding.OPT_MARGIN_SPLIT, 1)
+        check_step_against_oracle(oracle_mod, cg, A_bits, y, idx, x0, s, b, cfg.eta, cfg.loss, binding, shadow=False)
+        # a second step from the updated iterate: the residue rows follow the fused update
+        x1 = torch.from_numpy(x0.copy()).cuda()
+        cg.outer_step(torch.from_numpy(idx).cuda(), x1, s, b, cfg.eta)
+        cg.sync()
+        check_step_against_oracle(oracle_mod, cg, A_bits, y, idx, x1.cpu().numpy(), s, b, cfg.eta, cfg.loss, binding, shadow=False)
+        # negative control: with the split off, r is the margin of bf16(x), which is NOT within 1e-5 of Y x
+        cg.set_option(binding.OPT_MARGIN_SPLIT, 0)
+        with pytest.raises(AssertionError, match="margin"):
+            check_step_against_oracle(oracle_mod, cg, A_bits, y, idx, x0, s, b, cfg.eta, cfg.loss, binding, shadow=False)
+
+
 @pytest.mark.parametrize("ci,m,n,s,b", [(1, 20000, 18, 5, 64), (4, 6000, 512, 3, 64), (0, 4097, 64, 7, 13)])
 def test_on_device_sampling_matches_the_oracle_sampler(binding, oracle_mod, ci, m, n, s, b):
     """casgd_outer_steps_sampled draws Alg. 1 line 1's indices on the device (Philox4x32-10, with replacement): the rows it
