@@ -108,6 +108,31 @@ int casgd_outer_steps_sampled(casgd_ctx *c, int64_t n_steps, float *x, int32_t s
 int casgd_outer_steps_host(casgd_ctx *c, const int32_t *idx_host, int64_t n_steps, float *x_host, int32_t s,
                            int32_t b, float eta);
 
+/* ---- P > 1 ranks, the paper's 1-D block-column partition (section 4.2; Alg. 1 line 5, L118) ----
+ * Rank p creates its context on the column slab A[:, c0:c1] (n = c1 - c0, `ldx` the full row stride) with the FULL label
+ * vector y, and owns the matching slab of x. One outer iteration is then
+ *   casgd_step_local    gather Y_loc, G_loc = Y_loc Y_loc^T, r_loc = Y_loc x_loc (the context's Gram kernels), packed into
+ *                       `payload_out`: casgd_payload_count(s, b) FP32 words, device memory, 16-byte aligned:
+ *                         [ r_0 .. r_{sb-1} | block row 1 of G (b x b) | block row 2 (b x 2b) | .. | block row s-1 ]
+ *                       entry (i, k), block(k) < block(i) = j, at  sb + b^2 j (j-1) / 2 + (i - j b) j b + k  -- r and the
+ *                       strict block-lower part of G (L180), sb + b^2 s (s-1) / 2 words: half of Table 2's sb + (sb)^2
+ *                       (L154), G being symmetric;
+ *   the sum over ranks  (line 5) either by the caller -- e.g. an NCCL AllReduce of the payload (the paper's grouped
+ *                       AllReduce, L276), then casgd_step_finish(payload_in = the reduced payload) -- or by
+ *                       casgd_reduce_peers: one kernel of this library that reads every rank's payload (device pointers,
+ *                       which may be peer-mapped memory of other GPUs reached over NVLink) and writes the sum, taken in
+ *                       rank order so that all ranks hold identical bits, straight into the context's G and r (no staging
+ *                       copy, no unpack pass); the caller orders it after every rank's casgd_step_local (events / a
+ *                       barrier), then calls casgd_step_finish(payload_in = NULL);
+ *   casgd_step_finish   the recurrence on the summed [r; G] (redundantly on every rank, L120-L132) and the update of this
+ *                       rank's slab of x (L133-L135) and its shadow.
+ * All ranks must pass the same idx, s, b, eta. ASYNCHRONOUS; errors as for casgd_outer_step. With P = 1 and
+ * payload_in = the rank's own payload the three calls equal casgd_outer_step. */
+int64_t casgd_payload_count(int32_t s, int32_t b);          /* -1 for arguments casgd_step_local would reject */
+int casgd_step_local(casgd_ctx *c, const int32_t *idx, const float *x, int32_t s, int32_t b, float *payload_out);
+int casgd_reduce_peers(casgd_ctx *c, const float *const *peer_payloads_host, int32_t P, int32_t s, int32_t b);
+int casgd_step_finish(casgd_ctx *c, float *x, int32_t s, int32_t b, float eta, const float *payload_in);
+
 /* In-library baseline: one all-FP32 mini-batch SGD step, i.e. Alg. 1 with s = 1 and every
  * precision slot FP32 ("Recipe A", Table 3): x <- x - (eta/b) Y32^T l'(Y32 x, y_I), with
  * Y32 the exact FP32 widening of the BF16 rows. The first call allocates the m x n FP32 copy of A.

@@ -172,6 +172,44 @@ def outer_step_gram(A_bits, y, idx, x, s, b, eta, loss, shadow=True) -> GramStep
     return GramStep(Yb, G, r, z, u, g, x_out)
 
 
+def slab_payload(A_bits, idx, x, s, b, cols, shadow=True):
+    """One rank's contribution to Alg. 1 line 5 in the 1-D block-column partition (L33, L141): with the
+    rank holding columns `cols` of A and x, r_loc = Y_loc x_hat_loc and G_loc = Y_loc Y_loc^T (FP64, plain numpy)."""
+    Y = bf16_to_f64(A_bits[idx][:, cols])
+    xl = np.asarray(x, np.float64)[cols]
+    xh = bf16_to_f64(f32_to_bf16(xl.astype(np.float32))) if shadow else xl
+    return Y @ xh, Y @ Y.T
+
+
+def outer_step_gram_partitioned(A_bits, y, idx, x, s, b, eta, loss, slabs, shadow=True) -> GramStep:
+    """O1 on P ranks: Algorithm 1 WITH its line 5 (section 4.2). `slabs` is a list of column
+    slices, one per rank. Each rank forms r_loc, G_loc on its slab; the AllReduce sums them (in rank order here);
+    every rank runs the same recurrence (lines 6-15); rank p updates its slab of x with its own Y_loc^T u (lines 16-17).
+    Plain numpy FP64, no blocking beyond the partition the paper states."""
+    _check_data(A_bits, y, idx)
+    m, n = A_bits.shape
+    sb = s * b
+    x = np.asarray(x, np.float64)
+    alpha = eta / b
+    r, G = np.zeros(sb), np.zeros((sb, sb))
+    for cols in slabs:                                   # line 5: the sum over ranks of [r; G]
+        rl, Gl = slab_payload(A_bits, idx, x, s, b, cols, shadow)
+        r += rl
+        G += Gl
+    yI = y[idx].astype(np.float64)
+    z, u = np.zeros(sb), np.zeros(sb)
+    for j in range(s):                                   # lines 6-15, redundantly on every rank
+        rows = slice(j * b, (j + 1) * b)
+        z[rows] = r[rows] - alpha * (G[rows, : j * b] @ u[: j * b])
+        u[rows] = [lprime(zz, yy, loss) for zz, yy in zip(z[rows], yI[rows])]
+    g, x_out = np.zeros(n), x.copy()
+    for cols in slabs:                                   # lines 16-17, each rank on its slab
+        Y = bf16_to_f64(A_bits[idx][:, cols])
+        g[cols] = Y.T @ u
+        x_out[cols] = x[cols] - alpha * g[cols]
+    return GramStep(A_bits[idx].copy(), G, r, z, u, g, x_out)
+
+
 class SeqStep(NamedTuple):
     z: np.ndarray
     u: np.ndarray

@@ -30,8 +30,13 @@ EXPORTS = (
     "casgd_sgd_step_fp32",
     "casgd_sgd_steps_fp32", "casgd_loss", "casgd_invalidate_shadow", "casgd_sync", "casgd_debug_export",
     "casgd_set_option", "casgd_stage_times", "casgd_launch_count", "casgd_last_error", "casgd_destroy",
-    "casgd_version",
+    "casgd_version", "casgd_payload_count", "casgd_step_local", "casgd_reduce_peers", "casgd_step_finish",
 )
+
+
+def payload_count(s: int, b: int) -> int:
+    """casgd_payload_count: FP32 words of one outer iteration's [r; strict block-lower G] (Alg. 1 line 5)."""
+    return int(load().casgd_payload_count(s, b))
 
 
 class CasgdError(RuntimeError):
@@ -68,6 +73,14 @@ def load() -> ctypes.CDLL:
     lib.casgd_sgd_step_fp32.argtypes = [vp, vp, vp, i32, f32]
     lib.casgd_sgd_steps_fp32.restype = ctypes.c_int
     lib.casgd_sgd_steps_fp32.argtypes = [vp, vp, i64, vp, i32, f32]
+    lib.casgd_payload_count.restype = ctypes.c_int64
+    lib.casgd_payload_count.argtypes = [i32, i32]
+    lib.casgd_step_local.restype = ctypes.c_int
+    lib.casgd_step_local.argtypes = [vp, vp, vp, i32, i32, vp]
+    lib.casgd_reduce_peers.restype = ctypes.c_int
+    lib.casgd_reduce_peers.argtypes = [vp, ctypes.POINTER(vp), i32, i32, i32]
+    lib.casgd_step_finish.restype = ctypes.c_int
+    lib.casgd_step_finish.argtypes = [vp, vp, i32, i32, f32, vp]
     lib.casgd_loss.restype = ctypes.c_int
     lib.casgd_loss.argtypes = [vp, vp, ctypes.POINTER(ctypes.c_double)]
     lib.casgd_invalidate_shadow.restype = ctypes.c_int
@@ -165,6 +178,27 @@ class Casgd:
         self._check(self._lib.casgd_outer_steps(self._ctx, _dev_ptr(idx), n_steps, _dev_ptr(x), s, b, eta))
         if n_steps:
             self._last_sb = s * b
+
+    # ---- P > 1: the two halves of an outer iteration around the sum over ranks (Alg. 1 line 5) ----
+    def step_local(self, idx: torch.Tensor, x: torch.Tensor, s: int, b: int, payload: torch.Tensor):
+        """casgd_step_local: this slab's [r; strict block-lower G] into `payload` (payload_count(s, b) float32)."""
+        assert idx.is_cuda and idx.dtype == torch.int32 and idx.is_contiguous() and idx.numel() == s * b
+        assert x.is_cuda and x.dtype == torch.float32 and x.is_contiguous() and x.numel() == self.n
+        assert payload.is_cuda and payload.dtype == torch.float32 and payload.is_contiguous()
+        assert payload.numel() == payload_count(s, b)
+        self._check(self._lib.casgd_step_local(self._ctx, _dev_ptr(idx), _dev_ptr(x), s, b, _dev_ptr(payload)))
+        self._last_sb = s * b
+
+    def reduce_peers(self, payloads, s: int, b: int):
+        """casgd_reduce_peers: sum the ranks' payloads (device tensors, possibly peer memory) into this context."""
+        arr = (ctypes.c_void_p * len(payloads))(*[_dev_ptr(p) for p in payloads])
+        self._check(self._lib.casgd_reduce_peers(self._ctx, arr, len(payloads), s, b))
+
+    def step_finish(self, x: torch.Tensor, s: int, b: int, eta: float, payload: Optional[torch.Tensor] = None):
+        """casgd_step_finish: recurrence on the summed [r; G] and the update of this slab of x."""
+        assert x.is_cuda and x.dtype == torch.float32 and x.is_contiguous() and x.numel() == self.n
+        self._check(self._lib.casgd_step_finish(self._ctx, _dev_ptr(x), s, b, eta,
+                                                _dev_ptr(payload) if payload is not None else None))
 
     def outer_steps_sampled(self, x: torch.Tensor, s: int, b: int, eta: float, n_steps: int, seed: int, first_step: int = 0):
         """casgd_outer_steps_sampled: indices drawn on the device (Philox4x32-10, with replacement)."""

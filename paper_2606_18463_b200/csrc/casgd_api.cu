@@ -301,7 +301,7 @@ int stage_margin(casgd_ctx *c, cudaStream_t st, const float *x, const StepParams
 
 // recurrence and update of the rows in stage `buf`
 int stage_chain(casgd_ctx *c, cudaStream_t st, float *x, const StepParams *ind, int32_t s, int32_t b, float alpha, int buf,
-                bool late_trigger, const std::function<void()> &after_recurrence, int64_t *kernels)
+                bool late_trigger, const std::function<void()> &after_recurrence, int64_t *kernels, bool force_recurrence = false)
 {
     const int32_t sb = s * b;
     uint16_t *Y = c->Y + (size_t)buf * c->rows_alloc * c->ldy;
@@ -309,7 +309,7 @@ int stage_chain(casgd_ctx *c, cudaStream_t st, float *x, const StepParams *ind, 
     float *G = c->G + (size_t)buf * c->rows_alloc * c->rows_alloc;
     int k;
     const bool fused = !c->opt_no_fuse && recurrence_fuses_update(s, b, c->ldg, c->ldy, c->rws, (int)c->opt_rec_impl);
-    if (!step_is_s1(c, s)) {
+    if (!step_is_s1(c, s) || force_recurrence) {
         StageTimer t(c, CASGD_STAGE_RECURRENCE);
         const FusedUpdate fu{Y, c->ldy, c->n, x, ind, c->xbf, c->opt_split ? c->ldxb : 0};
         c->rws.late_trigger = late_trigger;
@@ -752,6 +752,61 @@ int casgd_outer_steps_sampled(casgd_ctx *c, int64_t n_steps, float *x, int32_t s
     }
     if (count > 0) c->launches += launch_sample_indices(c->stream, c->idx_stage, n_steps, s * b, c->m, seed, first_step);
     return run_steps(c, c->idx_stage, n_steps, x, s, b, eta, true);
+}
+
+// ---- P > 1: the outer iteration in two halves around the sum over ranks (Alg. 1 line 5) ----
+
+int64_t casgd_payload_count(int32_t s, int32_t b)
+{
+    if (s < 1 || b < 1 || (int64_t)s * b > CASGD_MAX_SB) return -1;
+    return payload_count(s, b);
+}
+
+int casgd_step_local(casgd_ctx *c, const int32_t *idx, const float *x, int32_t s, int32_t b, float *payload_out)
+{
+    int rc = check_step_args(c, idx, x, 1, s, b, 0.f);
+    if (rc) return rc;
+    if (!payload_out || ((uintptr_t)payload_out & 15)) return fail(c, CASGD_EINVAL, "payload_out must be a 16-byte aligned device pointer");
+    const int32_t sb = s * b;
+    if ((rc = ensure_workspace(c, sb)) || (rc = choose_gram(c, s, b)) || (rc = ensure_shadow(c, x))) return rc;
+    c->last_s = s; c->last_b = b; c->last_buf = 0;
+    int64_t kernels = 0;
+    const bool narrow = c->cur_gram == 4;
+    const bool split_margin = pipelined_mode(c, s, b);
+    if (!narrow && (rc = stage_gather(c, c->stream, idx, nullptr, 0, sb, 0, c->gram_sms, &kernels))) return rc;
+    if ((narrow || s > 1) && (rc = stage_gram(c, c->stream, idx, nullptr, 0, s, b, 0, split_margin ? nullptr : c->r, &kernels))) return rc;
+    if ((split_margin || (s == 1 && !narrow)) && (rc = stage_margin(c, c->stream, x, nullptr, sb, 0, &kernels))) return rc;
+    c->launches += launch_payload_pack(c->stream, c->G, c->ldg, c->r, s, b, payload_out, c->num_sms);
+    CK(cudaGetLastError());
+    return CASGD_OK;
+}
+
+int casgd_reduce_peers(casgd_ctx *c, const float *const *peer_payloads_host, int32_t P, int32_t s, int32_t b)
+{
+    if (!c) return CASGD_EINVAL;
+    if (!peer_payloads_host || s < 1 || b < 1 || s * b > c->rows_alloc || s != c->last_s || b != c->last_b)
+        return fail(c, CASGD_EINVAL, "casgd_reduce_peers: (s, b) must be those of the casgd_step_local just run");
+    const int k = launch_reduce_unpack(c->stream, peer_payloads_host, P, c->G, c->ldg, c->r, s, b, c->num_sms);
+    if (k < 0) return fail(c, CASGD_EINVAL, "casgd_reduce_peers: P = %d must be in [1, 64] and every payload pointer non-null", P);
+    c->launches += k;
+    CK(cudaGetLastError());
+    return CASGD_OK;
+}
+
+int casgd_step_finish(casgd_ctx *c, float *x, int32_t s, int32_t b, float eta, const float *payload_in)
+{
+    int dummy = 0;
+    int rc = check_step_args(c, &dummy, x, 1, s, b, eta);
+    if (rc) return rc;
+    if (s != c->last_s || b != c->last_b || s * b > c->rows_alloc)
+        return fail(c, CASGD_EINVAL, "casgd_step_finish: (s, b) must be those of the casgd_step_local just run");
+    if (payload_in) c->launches += launch_payload_unpack(c->stream, c->G, c->ldg, c->r, s, b, payload_in, c->num_sms);
+    int64_t kernels = 0;
+    std::function<void()> none;
+    rc = stage_chain(c, c->stream, x, nullptr, s, b, eta / (float)b, 0, false, none, &kernels, true);
+    if (rc) return rc;
+    CK(cudaGetLastError());
+    return CASGD_OK;
 }
 
 int casgd_sgd_steps_fp32(casgd_ctx *c, const int32_t *idx, int64_t n_steps, float *x, int32_t b, float eta)

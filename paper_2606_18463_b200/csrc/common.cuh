@@ -313,6 +313,16 @@ int launch_set_params(cudaStream_t st, StepParams *ind, const int32_t *idx, floa
 int launch_stamp_collect(cudaStream_t st, unsigned long long *slots, int nslots, unsigned long long *accum_ns,
                          unsigned long long *count, unsigned long long *raw_copy);
 
+// P > 1 (partition.cu): the payload [r; strict block-lower G] of Alg. 1 line 5, packed / unpacked / summed over ranks
+int64_t payload_count(int32_t s, int32_t b);
+int launch_payload_pack(cudaStream_t st, const float *G, int32_t ldg, const float *r, int32_t s, int32_t b, float *payload,
+                        int num_sms);
+int launch_payload_unpack(cudaStream_t st, float *G, int32_t ldg, float *r, int32_t s, int32_t b, const float *payload,
+                          int num_sms);
+int launch_reduce_peers(cudaStream_t st, const float *const *peers_host, int32_t P, float *out, int64_t count, int num_sms);
+int launch_reduce_unpack(cudaStream_t st, const float *const *peers_host, int32_t P, float *G, int32_t ldg, float *r, int32_t s,
+                         int32_t b, int num_sms);
+
 // tcgen05 Gram + margin (gram_tc.cu). r == nullptr: no margin (the pipelined schedule computes r in a kernel of its own).
 // The plan owns the TMA tensor maps of the Y workspace and of the
 // BF16 shadow (a [16 x ldxb] buffer: row 0 = x_bf, rows 1..15 zero). ksplit_opt <= 0: choose automatically.
