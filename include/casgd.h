@@ -217,12 +217,19 @@ int casgd_debug_export(casgd_ctx *c, int what, void *dst_host, int64_t dst_bytes
  *                              itself -- with A stored in BF16 this is Recipe B (u_A = b, every compute slot f): BF16 x
  *                              BF16 products are exact in FP32, so G and g are already what FP32 compute gives. Removes
  *                              the x half of Eq. 8's 2 u_16 term (L229) at no extra MMA.
+ *   CASGD_OPT_MINI             1 (default) = steps small enough for one SM -- two stages of Y, the packed strict
+ *                              block-lower G and the vectors within one CTA's shared memory, a Gram of at most 4M
+ *                              multiply-adds: e.g. n = 64, s*b = 64; n = 18, s*b = 256; n = 512, s = 1, b = 64 -- run ALL
+ *                              the iterations of a casgd_outer_step(s) call in ONE persistent one-CTA launch (gather with
+ *                              the next iteration's rows in flight, mma.sync Gram, recurrence, update, x resident in
+ *                              shared memory), unless a kernel was asked for (CASGD_OPT_GRAM_IMPL, _RECURRENCE_IMPL,
+ *                              _NO_FUSED_UPDATE, _GRAM_FULL_LOWER, _PROFILE). 0 = always the kernel-per-stage path.
  *   CASGD_OPT_LOSS_IMPL        0 = casgd_loss streams A through per-warp cp.async.bulk shared-memory rings
  *                              (default; n <= 8192), 1 = the plain 16-byte-load kernel. */
 typedef enum {
     CASGD_OPT_GRAM_IMPL = 0, CASGD_OPT_GRAM_FULL_LOWER = 1, CASGD_OPT_PROFILE = 2, CASGD_OPT_NO_GRAPH = 3,
     CASGD_OPT_GRAM_KSPLIT = 4, CASGD_OPT_RECURRENCE_IMPL = 5, CASGD_OPT_LOSS_IMPL = 6, CASGD_OPT_NO_FUSED_UPDATE = 7,
-    CASGD_OPT_STAMPS = 8, CASGD_OPT_OVERLAP = 9, CASGD_OPT_CHAIN_SMS = 10, CASGD_OPT_MARGIN_SPLIT = 11
+    CASGD_OPT_STAMPS = 8, CASGD_OPT_OVERLAP = 9, CASGD_OPT_CHAIN_SMS = 10, CASGD_OPT_MARGIN_SPLIT = 11, CASGD_OPT_MINI = 12
 } casgd_option;
 int casgd_set_option(casgd_ctx *c, int option, int64_t value);
 

@@ -20,7 +20,7 @@ LOGISTIC, LINEAR, POISSON = 0, 1, 2
 OK, EINVAL, ENOMEM, ECUDA, EARCH, EINDEX = range(6)
 STATUS_NAMES = ("CASGD_OK", "CASGD_EINVAL", "CASGD_ENOMEM", "CASGD_ECUDA", "CASGD_EARCH", "CASGD_EINDEX")
 DBG_Y, DBG_YLAB, DBG_G, DBG_R, DBG_Z, DBG_U, DBG_XBF, DBG_STAMPS = range(8)
-OPT_GRAM_IMPL, OPT_GRAM_FULL_LOWER, OPT_PROFILE, OPT_NO_GRAPH, OPT_GRAM_KSPLIT, OPT_RECURRENCE_IMPL, OPT_LOSS_IMPL, OPT_NO_FUSED_UPDATE, OPT_STAMPS, OPT_OVERLAP, OPT_CHAIN_SMS, OPT_MARGIN_SPLIT = range(12)
+OPT_GRAM_IMPL, OPT_GRAM_FULL_LOWER, OPT_PROFILE, OPT_NO_GRAPH, OPT_GRAM_KSPLIT, OPT_RECURRENCE_IMPL, OPT_LOSS_IMPL, OPT_NO_FUSED_UPDATE, OPT_STAMPS, OPT_OVERLAP, OPT_CHAIN_SMS, OPT_MARGIN_SPLIT, OPT_MINI = range(13)
 STAGES = ("gather", "gram", "recurrence", "gradient", "margin", "other", "loss")
 MAX_SB = 16384
 

@@ -94,7 +94,7 @@ struct casgd_ctx {
     unsigned long long *stamps = nullptr;     // CASGD_OPT_STAMPS: [kStampSteps * 8][2] slots, accum_ns[8], count[8], raw copy of the slots
     int cur_slot_step = 0;                    // step index (inside the graph being captured) the next stage stamps into
     int64_t opt_stamps = 0;
-    int64_t opt_gram_impl = 0, opt_full_lower = 0, opt_profile = 0, opt_no_graph = 0, opt_ksplit = 0, opt_rec_impl = 0, opt_loss_impl = 0, opt_no_fuse = 0, opt_overlap = 2, opt_chain_sms = 0, opt_split = 0;
+    int64_t opt_gram_impl = 0, opt_full_lower = 0, opt_profile = 0, opt_no_graph = 0, opt_ksplit = 0, opt_rec_impl = 0, opt_loss_impl = 0, opt_no_fuse = 0, opt_overlap = 2, opt_chain_sms = 0, opt_split = 0, opt_mini = 1;
     GramTcPlan *tc_plan = nullptr;
     GramPairPlan *pair_plan = nullptr;
     int pair_plan_sms = 0;
@@ -574,6 +574,23 @@ int run_steps(casgd_ctx *c, const int32_t *idx, int64_t n_steps, float *x, int32
     if (n_steps == 0) return CASGD_OK;
     int rc = ensure_workspace(c, sb);
     if (rc) return rc;
+    // tiny steps: all n_steps iterations in ONE persistent one-CTA launch (mini_step.cu) -- unless a kernel was asked for
+    if (c->opt_mini && !c->opt_gram_impl && !c->opt_rec_impl && !c->opt_no_fuse && !c->opt_full_lower && !c->opt_profile &&
+        c->lda % 8 == 0 && mini_step_ok(c->n, c->ldy, s, b)) {
+        c->cur_slot_step = 0;
+        StageTimer t(c, CASGD_STAGE_GRAM);
+        const int k = launch_mini_steps(c->stream, c->A, c->lda, c->y, c->m, c->n, c->ldy, idx, n_steps, s, b, eta / (float)b, c->loss,
+                                        (int)c->opt_split, x, c->xbf, c->ldxb, (int)c->opt_split, c->Y, c->yI, c->G, c->ldg, c->r,
+                                        c->z, c->u, c->err_flag);
+        if (k < 0) return fail(c, CASGD_ECUDA, "mini_step launch: %s", cudaGetErrorString(cudaGetLastError()));
+        t.done(k);
+        if (c->opt_stamps)
+            launch_stamp_collect(c->stream, c->stamps, kSlotStages, c->stamps + kStampAcc, c->stamps + kStampAcc + 8, c->stamps + kStampRaw);
+        c->last_s = s; c->last_b = b; c->last_buf = 0;
+        c->shadow_of = x; c->shadow_valid = true;
+        CK(cudaGetLastError());
+        return CASGD_OK;
+    }
     rc = choose_gram(c, s, b);
     if (rc) return rc;
     rc = ensure_shadow(c, x);
@@ -637,7 +654,7 @@ int casgd_init(casgd_ctx **out, const uint16_t *X_bf16, int64_t ldx, const float
     // opt-in shared-memory sizes and cluster sizes are per-device function attributes: set them on this device
     if (gather_configure() != cudaSuccess || gradient_configure() != cudaSuccess || gram_tc_configure() != cudaSuccess ||
         gram_pair_configure() != cudaSuccess || loss_configure() != cudaSuccess || recurrence_configure() != cudaSuccess ||
-        recurrence_stream_configure() != cudaSuccess)
+        recurrence_stream_configure() != cudaSuccess || mini_step_configure() != cudaSuccess)
         return bail(CASGD_ECUDA);
     c->stream = (cudaStream_t)cuda_stream;
     c->y = y; c->m = m; c->n = n; c->loss = loss;
@@ -938,6 +955,7 @@ int casgd_set_option(casgd_ctx *c, int option, int64_t value)
         if (value < 0 || value > 2) return fail(c, CASGD_EINVAL, "CASGD_OPT_OVERLAP must be 0, 1 or 2");
         c->opt_overlap = value; break;
     case CASGD_OPT_MARGIN_SPLIT: c->opt_split = value != 0; break;
+    case CASGD_OPT_MINI: c->opt_mini = value != 0; break;
     case CASGD_OPT_CHAIN_SMS:
         if (value < 0 || value > 1024) return fail(c, CASGD_EINVAL, "CASGD_OPT_CHAIN_SMS must be in [0, 1024]");
         c->opt_chain_sms = value; break;

@@ -221,6 +221,7 @@ cudaError_t gram_pair_configure();
 cudaError_t loss_configure();
 cudaError_t recurrence_configure();
 cudaError_t recurrence_stream_configure();
+cudaError_t mini_step_configure();
 
 // ------------------------------------------------------------ launch prototypes ---
 // Every launcher enqueues on `st` and returns the number of kernels it launched.
@@ -312,6 +313,13 @@ int launch_set_params(cudaStream_t st, StepParams *ind, const int32_t *idx, floa
 // slots: [nslots][2] {min start, max end} in %globaltimer ns, slot = 8 * step + stage; accum_ns / count: [8]
 int launch_stamp_collect(cudaStream_t st, unsigned long long *slots, int nslots, unsigned long long *accum_ns,
                          unsigned long long *count, unsigned long long *raw_copy);
+
+// Whole outer iterations in one persistent one-CTA launch, for tiny steps (mini_step.cu)
+bool mini_step_ok(int32_t n, int32_t ldy, int32_t s, int32_t b);
+int launch_mini_steps(cudaStream_t st, const uint16_t *A, int64_t lda, const float *y, int64_t m, int32_t n, int32_t ldy,
+                      const int32_t *idx, int64_t n_steps, int32_t s, int32_t b, float alpha, int loss, int exact_margin,
+                      float *x, uint16_t *xbf, int32_t ldxb, int split, uint16_t *Y, float *yI, float *G, int32_t ldg, float *r,
+                      float *z, float *u, int *err_flag);
 
 // P > 1 (partition.cu): the payload [r; strict block-lower G] of Alg. 1 line 5, packed / unpacked / summed over ranks
 int64_t payload_count(int32_t s, int32_t b);

@@ -377,6 +377,60 @@ def test_next_step_gather_on_the_side_branch_changes_nothing(binding, oracle_mod
         compare_last_step(oracle_mod, cg, ref, y[last], x_before_last, xc, s, b, eta, cfg.loss, binding)
 
 
+MINI_SHAPES = [(0, 8192, 64, 4, 16), (1, 20000, 18, 1, 64), (1, 20000, 18, 2, 64), (4, 6000, 512, 1, 16), (0, 4097, 64, 7, 13),
+               (3, 3000, 100, 3, 24), (0, 5000, 33, 2, 5), (4, 6000, 512, 2, 16), (2, 20000, 1024, 1, 8)]
+
+
+@pytest.mark.parametrize("ci,m,n,s,b", MINI_SHAPES)
+def test_one_launch_kernel_for_tiny_steps(binding, oracle_mod, ci, m, n, s, b):
+    """mini_step.cu: steps that fit one SM run all iterations of a call in ONE launch. One
+    step against oracle O1 element by element (gather bit-exact, G, r, z, u, x); a 9-step call equals 9 single-step
+    calls bit for bit and is a single launch; the kernel-per-stage path gives the same iterate up to FP32 summation
+    order; an out-of-range index is reported, not read."""
+    cfg = synth.config(ci, m=m, n=n)
+    X_d, y_d, A_bits, y = device_dataset(cfg)
+    steps = 9
+    idx = np.concatenate([synth.epoch_indices(cfg, 42, e) for e in range(-(-steps * s * b // m) + 1)])[: steps * s * b].copy()
+    idx_d = torch.from_numpy(idx).cuda()
+    x0 = random_x(n, 11, 0.4)
+    eta = cfg.eta * 0.5
+    with binding.Casgd(X_d, y_d, cfg.loss) as cg:
+        n0 = cg.launch_count()
+        check_step_against_oracle(oracle_mod, cg, A_bits, y, idx[: s * b], x0, s, b, eta, cfg.loss, binding)
+        assert cg.launch_count() - n0 == 1, "the step did not run as one launch"
+        xa = torch.from_numpy(x0.copy()).cuda()
+        for h in range(steps):
+            cg.outer_step(idx_d[h * s * b:(h + 1) * s * b], xa, s, b, eta)
+        xc = torch.from_numpy(x0.copy()).cuda()
+        cg.outer_steps(idx_d[: (steps - 1) * s * b], xc, s, b, eta)
+        cg.sync()
+        x_before = xc.cpu().numpy().copy()
+        xb = torch.from_numpy(x0.copy()).cuda()
+        n0 = cg.launch_count()
+        cg.outer_steps(idx_d, xb, s, b, eta)
+        cg.sync()
+        assert cg.launch_count() - n0 == 1
+        assert torch.equal(xa, xb)
+        # the last step of the 9-step launch, against the oracle from the iterate before it
+        last = idx[(steps - 1) * s * b:]
+        ref = oracle_mod.outer_step_gram(A_bits, y, last, x_before.astype(np.float64), s, b, eta, cfg.loss, shadow=True)
+        compare_last_step(oracle_mod, cg, ref, y[last], x_before, xb, s, b, eta, cfg.loss, binding)
+        # kernel-per-stage path: same iterate up to summation order
+        cg.set_option(binding.OPT_MINI, 0)
+        xd = torch.from_numpy(x0.copy()).cuda()
+        cg.outer_steps(idx_d, xd, s, b, eta)
+        cg.sync()
+        assert torch.linalg.norm(xd - xb) <= 2e-5 * torch.linalg.norm(xb)
+        cg.set_option(binding.OPT_MINI, 1)
+        bad = idx[: s * b].copy()
+        bad[3] = m + 5
+        xe = torch.from_numpy(x0.copy()).cuda()
+        cg.outer_step(torch.from_numpy(bad).cuda(), xe, s, b, eta)
+        with pytest.raises(binding.CasgdError):
+            cg.sync()
+        assert torch.isfinite(xe).all()
+
+
 SPLIT_SHAPES = [(0, 8192, 64, 4, 16), (1, 20000, 18, 5, 64), (2, 4200, 4096, 3, 128), (3, 5000, 2000, 9, 32), (4, 6000, 512, 6, 64),
                 (4, 6000, 512, 1, 64), (2, 5000, 1024, 6, 128)]
 
