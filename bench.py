@@ -377,16 +377,20 @@ def timed_steps(cg, cfg, s, idx_d, x, K, W, stream, min_timed_s, clocks=None, ma
     return times, R, launches
 
 
-def stage_report(cg, binding, cfg, s, idx_d, x, W, Kp, pk, lib_version):
+def stage_report(cg, binding, cfg, s, idx_d, x, W, Kp, pk, lib_version, overlap=None):
     """Per-stage device times measured INSIDE the CUDA-graph replays (CASGD_OPT_STAMPS: first-CTA start after the PDL
     wait to last-CTA end, %globaltimer), the algorithmic work of each stage and its roofline fraction."""
     sb = s * cfg.b
+    if overlap is not None:
+        cg.set_option(binding.OPT_OVERLAP, overlap)
     cg.set_option(binding.OPT_STAMPS, 1)
     prime_graphs(cg, cfg, 7, s, sb)                         # the option rebuilt the graphs
     cg.stage_times(reset=True)
     cg.outer_steps(idx_d[W * sb:], x, s, cfg.b, cfg.eta, n_steps=Kp)
     st = cg.stage_times(reset=True)
     cg.set_option(binding.OPT_STAMPS, 0)
+    if overlap is not None:
+        cg.set_option(binding.OPT_OVERLAP, 2)
     work = stage_work(cfg.n, s, cfg.b, pk)
     # fused stages: a stage with no launch of its own ran inside its neighbour (n <= 64: gather inside the Gram
     # kernel; small steps: gradient + update inside the recurrence kernel; s = 1: l' inside the margin kernel)
@@ -397,6 +401,17 @@ def stage_report(cg, binding, cfg, s, idx_d, x, W, Kp, pk, lib_version):
             work[host]["flops"] += work[absent]["flops"]
             work[host]["fused"] = work[host].get("fused", []) + [absent]
     stages = {}
+    launched = [k for k in work if st[k][1] > 0]
+    if launched == ["gram"] and st["gram"][1] < Kp / 2:
+        # mini_step.cu: ALL iterations of the call in one persistent one-CTA launch (gather -> Gram -> recurrence ->
+        # update, x resident in shared memory): one stage, its time divided by the iterations it ran
+        per_step = st["gram"][0] / Kp
+        wk = dict(bytes=sum(w["bytes"] for w in work.values()), flops=sum(w["flops"] for w in work.values()), bound="hbm")
+        rl = roofline_of("fused_step", wk, per_step, pk, None)
+        rl["note"] = "latency-bound by design: one CTA, %d iterations per launch" % Kp
+        stages["fused_step"] = dict(ms_per_step=round(per_step, 6), launches_per_step=st["gram"][1] / Kp, roofline=rl,
+                                    alg_bytes=wk["bytes"], alg_flops=wk["flops"])
+        return stages
     for name, wk in work.items():
         tot_ms, cnt = st[name]
         if not cnt:
@@ -459,6 +474,9 @@ def run_workload(args, cfg, s, binding, pk, dist, world, rank, stream, clocks, f
                    final_loss=cg.loss(x), sb=sb)
         Kp = min(max(K, 64), 256)
         out["stages"] = stage_report(cg, binding, cfg, s, idx_d, x, W, Kp, pk, lib_version)
+        # ... and each kernel with the chip to itself (CASGD_OPT_OVERLAP = 0: kernels strictly in sequence, the margin
+        # fused into the Gram): what the kernels can do, as opposed to what they get beside one another
+        out["stages_alone"] = stage_report(cg, binding, cfg, s, idx_d, x, W, Kp, pk, lib_version, overlap=0)
         out["gemv"] = gemv_report(cg, binding, cfg, x, pk, lib_version, stream)
         if not full:
             cg.close()
@@ -571,13 +589,21 @@ def main_ours(args, cfg, s):
             e = run_workload(args, cfg2, s2, binding, pk, dist, world, rank, stream, None, full=False)
             extras[cfg2.name] = dict(config=config_dict(cfg2, s2, world), value=aggregate_rows_per_s(world, K, e["sb"], e["ms"]),
                                      unit=UNIT, ms_per_step=e["ms"] / K, repeats=e["repeats"], final_loss=e["final_loss"],
-                                     stages=e["stages"], gemv=e["gemv"])
+                                     stages=e["stages"], stages_alone=e["stages_alone"], gemv=e["gemv"])
     clk = clocks.stop()
 
     stages = r["stages"]
     # the roofline object: the dominant kernel of the headline step (for synth-linear: the tcgen05 Gram, tensor-bound)
     dominant = max(stages, key=lambda k: stages[k]["ms_per_step"])
-    roofline = stages[dominant]["roofline"]
+    roofline = dict(stages[dominant]["roofline"])
+    alone = r["stages_alone"].get(dominant)
+    if alone:
+        # the same kernel with the chip to itself (kernels in sequence): its own quality, next to what it gets when the
+        # schedule runs it on part of the SMs beside the latency-bound chain
+        roofline["alone"] = dict(achieved=alone["roofline"]["achieved"], frac=alone["roofline"]["frac"],
+                                 avg_launch_ms=alone["roofline"]["avg_launch_ms"], includes=alone["roofline"].get("includes"))
+        roofline["note"] = ("as scheduled: the pipelined graph runs this kernel on part of the SMs, sharing L2 with the chain "
+                            "of the previous iteration; `alone` is the same kernel in a strictly sequential graph")
     ms, Ke = r["ms"], r["Ke"]
     config = config_dict(cfg, s, world)
     notes = dict(l2="inputs larger than L2: rows are gathered at random from A "
@@ -601,7 +627,7 @@ def main_ours(args, cfg, s):
                 sampled_on_device=dict(value=aggregate_rows_per_s(world, K, sb, r["sampled_ms"]), unit=UNIT,
                                        ms_per_step=r["sampled_ms"] / K,
                                        sampler="Philox4x32-10, i.i.d. with replacement (PAPER.md:L111)"),
-                roofline=roofline, stages=stages, gemv=r["gemv"], sweep=r.get("sweep", {}), extras=extras)
+                roofline=roofline, stages=stages, stages_alone=r["stages_alone"], gemv=r["gemv"], sweep=r.get("sweep", {}), extras=extras)
     if "cpu_baseline" in r:
         line["cpu_baseline"] = r["cpu_baseline"]
     if rank == 0:

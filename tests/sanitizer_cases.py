@@ -54,7 +54,11 @@ def cases():
     yield "gram_pair256_ksplit", lambda: step_case("gram_pair256_ksplit", 4, 900, 136, 5, 64, [(B.OPT_GRAM_IMPL, 3), (B.OPT_GRAM_KSPLIT, 2)], eta=0.01)
     yield "gram_pair512", lambda: step_case("gram_pair512", 4, 900, 136, 9, 64, [(B.OPT_GRAM_IMPL, 4)], eta=0.01)
     yield "gram_narrow", lambda: step_case("gram_narrow", 1, 900, 18, 3, 64, [(B.OPT_GRAM_IMPL, 5)])
-    yield "gram_narrow_s1", lambda: step_case("gram_narrow_s1", 1, 900, 18, 1, 64)
+    yield "gram_narrow_s1", lambda: step_case("gram_narrow_s1", 1, 900, 18, 1, 64, [(B.OPT_MINI, 0)])
+    yield "mini_s1", lambda: step_case("mini_s1", 1, 900, 18, 1, 64, steps=5)
+    yield "mini_s4", lambda: step_case("mini_s4", 0, 900, 64, 4, 16, steps=5)
+    yield "mini_odd", lambda: step_case("mini_odd", 0, 900, 33, 3, 13, steps=3)
+    yield "mini_split", lambda: step_case("mini_split", 0, 900, 64, 4, 16, [(B.OPT_MARGIN_SPLIT, 1)], steps=3)
     yield "margin_s1", lambda: step_case("margin_s1", 4, 900, 136, 1, 64, eta=0.01)
     for impl, nm in ((1, "cta"), (2, "grid"), (3, "cluster"), (4, "stream")):
         yield f"rec_{nm}", (lambda impl=impl, nm=nm: step_case(f"rec_{nm}", 0, 900, 24, 6, 32, [(B.OPT_RECURRENCE_IMPL, impl)]))
@@ -62,6 +66,12 @@ def cases():
     yield "rec_stream_unfused", lambda: step_case("rec_stream_unfused", 0, 900, 24, 6, 32, [(B.OPT_RECURRENCE_IMPL, 4), (B.OPT_NO_FUSED_UPDATE, 1)])
     yield "rec_grid_scalar", lambda: step_case("rec_grid_scalar", 0, 900, 24, 5, 13, [(B.OPT_RECURRENCE_IMPL, 2)])
     yield "gather_bulk_gradient_stream", lambda: step_case("gather_bulk_gradient_stream", 2, 1200, 1024, 4, 128)
+    yield "graph_sequential", lambda: step_case("graph_sequential", 4, 900, 136, 3, 64, [(B.OPT_OVERLAP, 0)], steps=9, eta=0.01)
+    yield "graph_gather_aside", lambda: step_case("graph_gather_aside", 2, 1200, 1024, 3, 128, [(B.OPT_OVERLAP, 1)], steps=9)
+    yield "graph_pipelined_wide", lambda: step_case("graph_pipelined_wide", 2, 1200, 1024, 3, 128, steps=9)
+    yield "split_fused_tile128", lambda: step_case("split_fused_tile128", 3, 600, 200, 5, 32, [(B.OPT_OVERLAP, 0), (B.OPT_GRAM_IMPL, 2), (B.OPT_MARGIN_SPLIT, 1)])
+    yield "split_fused_pair", lambda: step_case("split_fused_pair", 4, 900, 136, 5, 64, [(B.OPT_OVERLAP, 0), (B.OPT_GRAM_IMPL, 3), (B.OPT_MARGIN_SPLIT, 1)], eta=0.01)
+    yield "split_margin_kernel", lambda: step_case("split_margin_kernel", 3, 600, 200, 5, 32, [(B.OPT_MARGIN_SPLIT, 1)], steps=3)
     yield "graph_replay", lambda: step_case("graph_replay", 4, 900, 136, 3, 64, steps=9, eta=0.01)
     yield "graph_replay_stamps", lambda: step_case("graph_replay_stamps", 4, 900, 136, 3, 64, [(B.OPT_STAMPS, 1)], steps=9, eta=0.01)
 
@@ -95,6 +105,28 @@ def cases():
             cg.sync()
         print("case sampled_and_host: ok", flush=True)
     yield "sampled_and_host", sampled_and_host
+
+    def partition_case():
+        from paper_2606_18463_b200 import partition
+        cfg, X, y = dataset(4, 900, 136)
+        s, b, P = 3, 64, 3
+        slabs = [partition.column_slab(cfg.n, r, P) for r in range(P)]
+        ctxs = [binding.Casgd(X[:, sl], y, cfg.loss) for sl in slabs]
+        idx = torch.from_numpy(synth.iid_indices(cfg.m, s * b, 4)).cuda()
+        xs = [torch.zeros(sl.stop - sl.start, device="cuda") for sl in slabs]
+        pays = [torch.empty(binding.payload_count(s, b), device="cuda") for _ in slabs]
+        for cg, xp, pay in zip(ctxs, xs, pays):
+            cg.step_local(idx, xp, s, b, pay)
+        for cg, xp in zip(ctxs, xs):
+            cg.reduce_peers(pays, s, b)
+            cg.step_finish(xp, s, b, 0.01, None)
+        total = torch.stack(pays).sum(0)
+        for cg, xp in zip(ctxs, xs):
+            cg.step_finish(xp, s, b, 0.01, total)
+            cg.sync()
+            cg.close()
+        print("case partition: ok", flush=True)
+    yield "partition", partition_case
 
 
 def main():

@@ -71,7 +71,7 @@ def test_second_graph_step_at_full_size_matches_the_oracle(binding, oracle_mod, 
         n0 = cg.launch_count()
         cg.outer_steps(idx_d, x2, s, b, cfg.eta, n_steps=2)
         cg.sync()
-        assert cg.launch_count() - n0 >= 2              # the library's own kernels ran (at least one per step)
+        assert cg.launch_count() - n0 >= 1              # the library's own kernels ran (tiny steps: ONE launch for both)
         A_bits, y, local = _host_rows(ds, idx[sb:])
         ref = oracle_mod.outer_step_gram(A_bits, y, local, x1_host.astype(np.float64), s, b, cfg.eta, cfg.loss, shadow=True)
         compare_last_step(oracle_mod, cg, ref, y[local], x1_host, x2, s, b, cfg.eta, cfg.loss, binding)
