@@ -160,13 +160,15 @@ int casgd_sync(casgd_ctx *c);
  *                  always; every k <= i when CASGD_OPT_GRAM_FULL_LOWER is set. The rest is unspecified.
  *   CASGD_DBG_R    sb FP32   CASGD_DBG_Z sb FP32   CASGD_DBG_U sb FP32
  *   CASGD_DBG_XBF  n  BF16 bits: the shadow AFTER the step (bf16 of the updated x)
+ *   CASGD_DBG_GUARDS  1 int64: every per-step workspace (Y, y_I, G, r, z, u) sits between two 1 KB guard bands of a known
+ *                  pattern; this is the number of guard bytes that no longer hold it (0 = no kernel wrote past a workspace)
  *   CASGD_DBG_STAMPS  64 x 8 x 2 uint64: with CASGD_OPT_STAMPS, {first-CTA start, last-CTA end} in %globaltimer ns of
  *                  stage g (CASGD_STAGE_*) of step h of the last graph casgd_outer_steps replayed, at [h][g][0..1];
  *                  {~0, 0} where a stage did not run
  * dst_bytes must equal the size implied above, else CASGD_EINVAL. */
 typedef enum {
     CASGD_DBG_Y = 0, CASGD_DBG_YLAB = 1, CASGD_DBG_G = 2, CASGD_DBG_R = 3, CASGD_DBG_Z = 4,
-    CASGD_DBG_U = 5, CASGD_DBG_XBF = 6, CASGD_DBG_STAMPS = 7
+    CASGD_DBG_U = 5, CASGD_DBG_XBF = 6, CASGD_DBG_STAMPS = 7, CASGD_DBG_GUARDS = 8
 } casgd_debug_what;
 int casgd_debug_export(casgd_ctx *c, int what, void *dst_host, int64_t dst_bytes);
 

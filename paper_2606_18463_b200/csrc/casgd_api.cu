@@ -47,8 +47,19 @@ inline int64_t round_up(int64_t v, int64_t q) { return (v + q - 1) / q * q; }
 
 }  // namespace
 
+// Guard bands: every per-step workspace is allocated with kGuardBytes of a known pattern before and after it, and
+// casgd_debug_export(CASGD_DBG_GUARDS) counts the guard bytes that changed -- an out-of-bounds write next to a workspace
+// (a ragged tail, an off-by-one row) shows up there. (compute-sanitizer is closed on the pool this was developed on.)
+constexpr size_t kGuardBytes = 1024;
+constexpr int kGuardPattern = 0xA5;
+struct Guarded {
+    unsigned char *base;                // start of the allocation (the front guard)
+    size_t bytes;                       // payload bytes
+};
+
 struct casgd_ctx {
     int device = 0;
+    std::vector<Guarded> guarded;
     cudaStream_t stream = nullptr;
     cudaStream_t capture_stream = nullptr;
     cudaStream_t side_stream = nullptr;       // graph capture only: the branch that gathers the next step's rows
@@ -145,12 +156,49 @@ void drop_graphs(casgd_ctx *c)
     c->graphs.clear();
 }
 
+template <typename T>
+cudaError_t alloc_guarded(casgd_ctx *c, T **out, size_t bytes)
+{
+    unsigned char *base = nullptr;
+    const size_t padded = (bytes + 255) & ~(size_t)255;
+    cudaError_t e = cudaMalloc(&base, padded + 2 * kGuardBytes);
+    if (e != cudaSuccess) return e;
+    cudaMemset(base, kGuardPattern, kGuardBytes);
+    cudaMemset(base + kGuardBytes + bytes, kGuardPattern, padded - bytes + kGuardBytes);
+    c->guarded.push_back(Guarded{base, bytes});
+    *out = reinterpret_cast<T *>(base + kGuardBytes);
+    return cudaSuccess;
+}
+
+void free_guarded(casgd_ctx *c)
+{
+    for (const Guarded &g : c->guarded) cudaFree(g.base);
+    c->guarded.clear();
+}
+
+// guard bytes that no longer hold the pattern
+int64_t count_guard_damage(casgd_ctx *c)
+{
+    int64_t bad = 0;
+    std::vector<unsigned char> h;
+    for (const Guarded &g : c->guarded) {
+        const size_t padded = (g.bytes + 255) & ~(size_t)255;
+        const size_t tail = padded - g.bytes + kGuardBytes;
+        h.resize(kGuardBytes + tail);
+        if (cudaMemcpy(h.data(), g.base, kGuardBytes, cudaMemcpyDeviceToHost) != cudaSuccess ||
+            cudaMemcpy(h.data() + kGuardBytes, g.base + kGuardBytes + g.bytes, tail, cudaMemcpyDeviceToHost) != cudaSuccess)
+            return -1;
+        for (unsigned char v : h) bad += v != kGuardPattern;
+    }
+    return bad;
+}
+
 void free_step_workspace(casgd_ctx *c)
 {
     drop_graphs(c);
     if (c->tc_plan) { gram_tc_plan_destroy(c->tc_plan); c->tc_plan = nullptr; }
     if (c->pair_plan) { gram_pair_plan_destroy(c->pair_plan); c->pair_plan = nullptr; }
-    cudaFree(c->Y); cudaFree(c->yI); cudaFree(c->G); cudaFree(c->r); cudaFree(c->z); cudaFree(c->u); cudaFree(c->r_scratch);
+    free_guarded(c);
     c->Y = nullptr; c->yI = c->G = c->r = c->z = c->u = c->r_scratch = nullptr;
     c->rows_alloc = 0;
 }
@@ -162,13 +210,13 @@ int ensure_workspace(casgd_ctx *c, int32_t sb)
     free_step_workspace(c);
     const int32_t rows = (int32_t)round_up(sb, 2 * kTile);   // whole 256-row pair tiles: a tile never straddles the two stages
     c->ldg = rows;
-    CK(cudaMalloc(&c->Y, sizeof(uint16_t) * (size_t)2 * rows * c->ldy));
-    CK(cudaMalloc(&c->yI, sizeof(float) * 2 * rows));
-    CK(cudaMalloc(&c->G, sizeof(float) * (size_t)2 * rows * rows));
-    CK(cudaMalloc(&c->r, sizeof(float) * rows));
-    CK(cudaMalloc(&c->r_scratch, sizeof(float) * rows));
-    CK(cudaMalloc(&c->z, sizeof(float) * rows));
-    CK(cudaMalloc(&c->u, sizeof(float) * rows));
+    CK(alloc_guarded(c, &c->Y, sizeof(uint16_t) * (size_t)2 * rows * c->ldy));
+    CK(alloc_guarded(c, &c->yI, sizeof(float) * 2 * rows));
+    CK(alloc_guarded(c, &c->G, sizeof(float) * (size_t)2 * rows * rows));
+    CK(alloc_guarded(c, &c->r, sizeof(float) * rows));
+    CK(alloc_guarded(c, &c->r_scratch, sizeof(float) * rows));
+    CK(alloc_guarded(c, &c->z, sizeof(float) * rows));
+    CK(alloc_guarded(c, &c->u, sizeof(float) * rows));
     CK(cudaMemsetAsync(c->Y, 0, sizeof(uint16_t) * (size_t)2 * rows * c->ldy, c->stream));
     CK(cudaMemsetAsync(c->G, 0, sizeof(float) * (size_t)2 * rows * rows, c->stream));
     CK(cudaMemsetAsync(c->r_scratch, 0, sizeof(float) * rows, c->stream));
@@ -634,7 +682,7 @@ int run_steps(casgd_ctx *c, const int32_t *idx, int64_t n_steps, float *x, int32
 
 extern "C" {
 
-const char *casgd_version(void) { return "casgd-b200 0.1 (sm_100a)"; }
+const char *casgd_version(void) { return "casgd-b200 0.2 (sm_100a)"; }
 
 int casgd_init(casgd_ctx **out, const uint16_t *X_bf16, int64_t ldx, const float *y, int64_t m, int32_t n, int loss,
                void *cuda_stream)
@@ -892,7 +940,7 @@ int casgd_debug_export(casgd_ctx *c, int what, void *dst_host, int64_t dst_bytes
     if (!c) return CASGD_EINVAL;
     if (!dst_host) return fail(c, CASGD_EINVAL, "dst_host is null");
     const int64_t sb = (int64_t)c->last_s * c->last_b;
-    if (sb == 0 && what != CASGD_DBG_XBF && what != CASGD_DBG_STAMPS) return fail(c, CASGD_EINVAL, "no outer step has run yet");
+    if (sb == 0 && what != CASGD_DBG_XBF && what != CASGD_DBG_STAMPS && what != CASGD_DBG_GUARDS) return fail(c, CASGD_EINVAL, "no outer step has run yet");
     CK(cudaStreamSynchronize(c->stream));
     auto need = [&](int64_t bytes) { return dst_bytes == bytes; };
     switch (what) {
@@ -908,6 +956,13 @@ int casgd_debug_export(casgd_ctx *c, int what, void *dst_host, int64_t dst_bytes
         if (!need(sb * 4)) break;
         const float *src = what == CASGD_DBG_YLAB ? c->yI + (size_t)c->last_buf * c->rows_alloc : what == CASGD_DBG_R ? c->r : what == CASGD_DBG_Z ? c->z : c->u;
         CK(cudaMemcpy(dst_host, src, (size_t)sb * 4, cudaMemcpyDeviceToHost));
+        return CASGD_OK;
+    }
+    case CASGD_DBG_GUARDS: {
+        if (!need(8)) break;
+        const int64_t bad = count_guard_damage(c);
+        if (bad < 0) return fail(c, CASGD_ECUDA, "reading the guard bands failed");
+        *reinterpret_cast<int64_t *>(dst_host) = bad;
         return CASGD_OK;
     }
     case CASGD_DBG_STAMPS:

@@ -219,7 +219,8 @@ gradient_stream_kernel(const uint16_t *Y, int32_t ldy, int32_t n, int32_t sb, in
     float *x = ind ? ind->x : x_direct;
     if (mine) {
         float gx = 0.f, gy = 0.f;
-#pragma unroll 8
+        // (all loads of a batch of 16 in flight before the first add: the tail is a chain of L2 round trips otherwise)
+#pragma unroll 16
         for (unsigned q = 0; q < gridDim.y; ++q) {
             const float2 v = __ldcg(reinterpret_cast<const float2 *>(partial + (int64_t)q * ldp + col0 + cl));
             gx += v.x;
@@ -251,10 +252,11 @@ static int launch_gradient_stream(cudaStream_t st, const uint16_t *Y, int32_t ld
                                   float alpha, float *x, const StepParams *ind, uint16_t *xbf, const GradWorkspace &ws)
 {
     const int col_segs = (ldy + kGsSegCols - 1) / kGsSegCols;
-    // rows per warp: at least 8 (fixed costs), at most 32 (one u per lane); about one CTA per SM for large steps
+    // rows per warp: at most 32 (one u per lane), at least 2; about one CTA per SM (measured on n = 2000, s*b = 2048:
+    // a floor of 8 rows left 32 CTAs for 148 SMs, 7.4 us for 8 MB)
     const int slabs_target = std::max(1, ws.num_sms / col_segs);
     int rpw = (sb + kGsWarps * slabs_target - 1) / (kGsWarps * slabs_target);
-    rpw = std::min(32, std::max(8, rpw));
+    rpw = std::min(32, std::max(2, rpw));
     const int slabs = (sb + kGsWarps * rpw - 1) / (kGsWarps * rpw);
     if (slabs > ws.max_splits) return 0;
     launch_pdl(gradient_stream_kernel, dim3(col_segs, slabs), dim3(32 * kGsWarps), kGsSmem, st, 1, Y, ldy, n, sb, rpw, u, alpha, x,

@@ -138,4 +138,6 @@ def compare_last_step(oracle, cg, ref, y_idx, x0, x_d, s, b, eta, loss, binding,
     # shadow: bf16_rne of the library's own new master, bit for bit
     xbf = cg.debug(binding.DBG_XBF)
     assert np.array_equal(xbf, oracle.f32_to_bf16(x_d.cpu().numpy())), "BF16 shadow is not bf16_rne(x)"
+    # no kernel wrote past a workspace (1 KB guard bands around Y, y_I, G, r, z, u)
+    assert int(cg.debug(binding.DBG_GUARDS)[0]) == 0, "guard bytes around the workspaces were overwritten"
     return ref, dict(r=r, z=z, u=u, x=x1)

@@ -42,7 +42,9 @@ def step_case(name, ci, m, n, s, b, opts=(), steps=1, eta=None):
             cg.outer_steps(idx, x, s, b, eta)
         cg.sync()
         assert torch.isfinite(x).all()
-    print(f"case {name}: ok", flush=True)
+        damage = int(cg.debug(binding.DBG_GUARDS)[0])
+        assert damage == 0, f"{name}: {damage} guard bytes around the workspaces were overwritten"
+    print(f"case {name}: ok, guard bands intact", flush=True)
 
 
 def cases():
