@@ -160,6 +160,8 @@ int casgd_sync(casgd_ctx *c);
  *                  always; every k <= i when CASGD_OPT_GRAM_FULL_LOWER is set. The rest is unspecified.
  *   CASGD_DBG_R    sb FP32   CASGD_DBG_Z sb FP32   CASGD_DBG_U sb FP32
  *   CASGD_DBG_XBF  n  BF16 bits: the shadow AFTER the step (bf16 of the updated x)
+ *   CASGD_DBG_XSNAP  n FP32: with CASGD_OPT_SNAPSHOT, x as it entered the LAST step of the last CUDA graph replayed -- the
+ *                  FP32 bits that step started from, so that a test can check it against the oracle element by element
  *   CASGD_DBG_GUARDS  1 int64: every per-step workspace (Y, y_I, G, r, z, u) sits between two 1 KB guard bands of a known
  *                  pattern; this is the number of guard bytes that no longer hold it (0 = no kernel wrote past a workspace)
  *   CASGD_DBG_STAMPS  64 x 8 x 2 uint64: with CASGD_OPT_STAMPS, {first-CTA start, last-CTA end} in %globaltimer ns of
@@ -168,7 +170,7 @@ int casgd_sync(casgd_ctx *c);
  * dst_bytes must equal the size implied above, else CASGD_EINVAL. */
 typedef enum {
     CASGD_DBG_Y = 0, CASGD_DBG_YLAB = 1, CASGD_DBG_G = 2, CASGD_DBG_R = 3, CASGD_DBG_Z = 4,
-    CASGD_DBG_U = 5, CASGD_DBG_XBF = 6, CASGD_DBG_STAMPS = 7, CASGD_DBG_GUARDS = 8
+    CASGD_DBG_U = 5, CASGD_DBG_XBF = 6, CASGD_DBG_STAMPS = 7, CASGD_DBG_GUARDS = 8, CASGD_DBG_XSNAP = 9
 } casgd_debug_what;
 int casgd_debug_export(casgd_ctx *c, int what, void *dst_host, int64_t dst_bytes);
 
@@ -226,12 +228,14 @@ int casgd_debug_export(casgd_ctx *c, int what, void *dst_host, int64_t dst_bytes
  *                              the next iteration's rows in flight, mma.sync Gram, recurrence, update, x resident in
  *                              shared memory), unless a kernel was asked for (CASGD_OPT_GRAM_IMPL, _RECURRENCE_IMPL,
  *                              _NO_FUSED_UPDATE, _GRAM_FULL_LOWER, _PROFILE). 0 = always the kernel-per-stage path.
+ *   CASGD_OPT_SNAPSHOT         1 = the graphs of casgd_outer_steps copy x aside before their last step (CASGD_DBG_XSNAP):
+ *                              test support, one n-element kernel per graph.
  *   CASGD_OPT_LOSS_IMPL        0 = casgd_loss streams A through per-warp cp.async.bulk shared-memory rings
  *                              (default; n <= 8192), 1 = the plain 16-byte-load kernel. */
 typedef enum {
     CASGD_OPT_GRAM_IMPL = 0, CASGD_OPT_GRAM_FULL_LOWER = 1, CASGD_OPT_PROFILE = 2, CASGD_OPT_NO_GRAPH = 3,
     CASGD_OPT_GRAM_KSPLIT = 4, CASGD_OPT_RECURRENCE_IMPL = 5, CASGD_OPT_LOSS_IMPL = 6, CASGD_OPT_NO_FUSED_UPDATE = 7,
-    CASGD_OPT_STAMPS = 8, CASGD_OPT_OVERLAP = 9, CASGD_OPT_CHAIN_SMS = 10, CASGD_OPT_MARGIN_SPLIT = 11, CASGD_OPT_MINI = 12
+    CASGD_OPT_STAMPS = 8, CASGD_OPT_OVERLAP = 9, CASGD_OPT_CHAIN_SMS = 10, CASGD_OPT_MARGIN_SPLIT = 11, CASGD_OPT_MINI = 12, CASGD_OPT_SNAPSHOT = 13
 } casgd_option;
 int casgd_set_option(casgd_ctx *c, int option, int64_t value);
 

@@ -19,8 +19,8 @@ LIB_PATH = os.path.join(_HERE, "libcasgd.so")
 LOGISTIC, LINEAR, POISSON = 0, 1, 2
 OK, EINVAL, ENOMEM, ECUDA, EARCH, EINDEX = range(6)
 STATUS_NAMES = ("CASGD_OK", "CASGD_EINVAL", "CASGD_ENOMEM", "CASGD_ECUDA", "CASGD_EARCH", "CASGD_EINDEX")
-DBG_Y, DBG_YLAB, DBG_G, DBG_R, DBG_Z, DBG_U, DBG_XBF, DBG_STAMPS, DBG_GUARDS = range(9)
-OPT_GRAM_IMPL, OPT_GRAM_FULL_LOWER, OPT_PROFILE, OPT_NO_GRAPH, OPT_GRAM_KSPLIT, OPT_RECURRENCE_IMPL, OPT_LOSS_IMPL, OPT_NO_FUSED_UPDATE, OPT_STAMPS, OPT_OVERLAP, OPT_CHAIN_SMS, OPT_MARGIN_SPLIT, OPT_MINI = range(13)
+DBG_Y, DBG_YLAB, DBG_G, DBG_R, DBG_Z, DBG_U, DBG_XBF, DBG_STAMPS, DBG_GUARDS, DBG_XSNAP = range(10)
+OPT_GRAM_IMPL, OPT_GRAM_FULL_LOWER, OPT_PROFILE, OPT_NO_GRAPH, OPT_GRAM_KSPLIT, OPT_RECURRENCE_IMPL, OPT_LOSS_IMPL, OPT_NO_FUSED_UPDATE, OPT_STAMPS, OPT_OVERLAP, OPT_CHAIN_SMS, OPT_MARGIN_SPLIT, OPT_MINI, OPT_SNAPSHOT = range(14)
 STAGES = ("gather", "gram", "recurrence", "gradient", "margin", "other", "loss")
 MAX_SB = 16384
 
@@ -258,7 +258,7 @@ class Casgd:
         sb = self._last_sb if sb is None else sb
         shapes = {DBG_Y: ((sb, self.n), np.uint16), DBG_YLAB: ((sb,), np.float32), DBG_G: ((sb, sb), np.float32),
                   DBG_R: ((sb,), np.float32), DBG_Z: ((sb,), np.float32), DBG_U: ((sb,), np.float32),
-                  DBG_XBF: ((self.n,), np.uint16), DBG_STAMPS: ((64, 8, 2), np.uint64), DBG_GUARDS: ((1,), np.int64)}
+                  DBG_XBF: ((self.n,), np.uint16), DBG_STAMPS: ((64, 8, 2), np.uint64), DBG_GUARDS: ((1,), np.int64), DBG_XSNAP: ((self.n,), np.float32)}
         shape, dt = shapes[what]
         out = np.empty(shape, dt)
         self._check(self._lib.casgd_debug_export(self._ctx, what, out.ctypes.data, out.nbytes))

@@ -99,16 +99,18 @@ struct casgd_ctx {
     int32_t *idx_stage = nullptr;
     int64_t idx_stage_cap = 0;
     float *x_stage = nullptr;
+    float *x_snap = nullptr;          // CASGD_OPT_SNAPSHOT: x as it entered the last step of the last graph
     // last step, for debug export
     int32_t last_s = 0, last_b = 0, last_buf = 0;
     // options
     unsigned long long *stamps = nullptr;     // CASGD_OPT_STAMPS: [kStampSteps * 8][2] slots, accum_ns[8], count[8], raw copy of the slots
     int cur_slot_step = 0;                    // step index (inside the graph being captured) the next stage stamps into
     int64_t opt_stamps = 0;
-    int64_t opt_gram_impl = 0, opt_full_lower = 0, opt_profile = 0, opt_no_graph = 0, opt_ksplit = 0, opt_rec_impl = 0, opt_loss_impl = 0, opt_no_fuse = 0, opt_overlap = 2, opt_chain_sms = 0, opt_split = 0, opt_mini = 1;
+    int64_t opt_gram_impl = 0, opt_full_lower = 0, opt_profile = 0, opt_no_graph = 0, opt_ksplit = 0, opt_rec_impl = 0, opt_loss_impl = 0, opt_no_fuse = 0, opt_overlap = 2, opt_chain_sms = 0, opt_split = 0, opt_mini = 1, opt_snapshot = 0;
     GramTcPlan *tc_plan = nullptr;
-    GramPairPlan *pair_plan = nullptr;
-    int pair_plan_sms = 0;
+    GramPairPlan *pair_plans[2] = {nullptr, nullptr};   // work lists for all SMs [0] and for the pipelined schedule's share [1]
+    int pair_plan_sms[2] = {0, 0};
+    GramPairPlan *pair_plan = nullptr;                  // the one of the schedule being enqueued
     int num_sms = 0;
     int gram_sms = 0, chain_sms = 0;  // SM budgets of the two branches for the shape being enqueued (both num_sms unless pipelined)
     int cur_gram = 0, cur_bn = 0;     // Gram kernel of the shape being enqueued: 1 = CUDA cores, 2 = 128x128 tiles, 3 = CTA pairs
@@ -197,7 +199,8 @@ void free_step_workspace(casgd_ctx *c)
 {
     drop_graphs(c);
     if (c->tc_plan) { gram_tc_plan_destroy(c->tc_plan); c->tc_plan = nullptr; }
-    if (c->pair_plan) { gram_pair_plan_destroy(c->pair_plan); c->pair_plan = nullptr; }
+    for (GramPairPlan *&pl : c->pair_plans) { if (pl) gram_pair_plan_destroy(pl); pl = nullptr; }
+    c->pair_plan = nullptr;
     free_guarded(c);
     c->Y = nullptr; c->yI = c->G = c->r = c->z = c->u = c->r_scratch = nullptr;
     c->rows_alloc = 0;
@@ -388,7 +391,6 @@ int enqueue_step(casgd_ctx *c, cudaStream_t st, const int32_t *idx, const StepPa
     int rc;
     c->last_buf = io.buf;
     const bool s1 = step_is_s1(c, s);
-    const bool split_margin = pipelined_mode(c, s, b);     // same kernels as the pipelined graphs: bit-identical iterates
     if (s1 && c->cur_gram != 4) {
         // wide rows: gather + margin + l' in one warp-per-row kernel (there is no Gram at s = 1)
         StageTimer t(c, CASGD_STAGE_GRAM);
@@ -398,8 +400,7 @@ int enqueue_step(casgd_ctx *c, cudaStream_t st, const int32_t *idx, const StepPa
         t.done(k); *kernels += k;
     } else {
         if (c->cur_gram != 4 && !io.gathered && (rc = stage_gather(c, st, idx, ind, idx_off, sb, io.buf, c->gram_sms, kernels))) return rc;
-        if ((rc = stage_gram(c, st, idx, ind, idx_off, s, b, io.buf, split_margin ? nullptr : c->r, kernels))) return rc;
-        if (split_margin && (rc = stage_margin(c, st, x, ind, sb, io.buf, kernels))) return rc;
+        if ((rc = stage_gram(c, st, idx, ind, idx_off, s, b, io.buf, c->r, kernels))) return rc;
     }
     const bool side = io.next_idx_off >= 0;
     std::function<void()> none;
@@ -460,6 +461,7 @@ int capture_pipelined(casgd_ctx *c, int32_t s, int32_t b, float eta, int32_t len
         const int buf = h & 1;
         c->cur_slot_step = h;
         cudaStreamWaitEvent(M, c->ev_gather[buf], 0);
+        if (c->opt_snapshot && h + 1 == len) *kernels += launch_snapshot(M, nullptr, c->ind, c->n, c->x_snap);
         if ((rc = stage_margin(c, M, nullptr, c->ind, sb, buf, kernels))) break;
         cudaStreamWaitEvent(M, c->ev_gram[buf], 0);
         const bool more = h + 1 < len;
@@ -483,16 +485,17 @@ int capture_pipelined(casgd_ctx *c, int32_t s, int32_t b, float eta, int32_t len
 // Pick the Gram kernel for this shape (outside stream capture: the pair kernel's work list is uploaded here).
 // CASGD_OPT_GRAM_IMPL: 0 = by the cost model, 1 = CUDA cores, 2 = 128x128 tcgen05 tiles, 3 / 4 = CTA pairs with
 // 256 / 512-column tiles.
-int choose_gram(casgd_ctx *c, int32_t s, int32_t b)
+int choose_gram(casgd_ctx *c, int32_t s, int32_t b, bool pipe)
 {
     const int32_t sb = s * b;
     const int64_t opt = c->opt_gram_impl;
-    // SM budgets of the two branches. Pipelined: the chain keeps chain_sms SMs (the recurrence cluster's 16 and a few more
-    // for the margin and update streams), gather and Gram are sized for the rest -- also in single-step calls, so that
-    // every path of a mode runs identical kernels on identical grids (bit-identical iterates).
+    // SM budgets of the two branches. In the pipelined graphs (`pipe`) the chain keeps chain_sms SMs (the recurrence
+    // cluster's 16 and a few more for the margin and update streams) and gather and Gram are sized for the rest; single
+    // steps (and the sequential schedules) give every kernel the whole chip.
     c->gram_sms = c->chain_sms = c->num_sms;
     c->cur_gram = 2;                                    // (pipelined_mode asks step_is_s1, which looks at cur_gram)
-    if (pipelined_mode(c, s, b)) {
+    pipe = pipe && pipelined_mode(c, s, b);
+    if (pipe) {
         const int chain = c->opt_chain_sms > 0 ? (int)c->opt_chain_sms : 32;
         c->chain_sms = std::min(std::max(chain, 16), c->num_sms - 32) & ~1;
         c->gram_sms = c->num_sms - c->chain_sms;
@@ -505,15 +508,17 @@ int choose_gram(casgd_ctx *c, int32_t s, int32_t b)
     if (opt == 5) return fail(c, CASGD_EINVAL, "the fused gather + Gram kernel needs n <= 64");
     if (opt == 1 || opt == 2 || c->gram_sms < 2) return CASGD_OK;
     if (opt == 0 && (sb < 512 || c->n < 256)) return CASGD_OK;      // too little work for 256-row tiles
-    if (c->pair_plan && c->pair_plan_sms != c->gram_sms) { gram_pair_plan_destroy(c->pair_plan); c->pair_plan = nullptr; }
-    if (!c->pair_plan) {
-        c->pair_plan_sms = c->gram_sms;
-        c->pair_plan = gram_pair_plan_create(c->Y, c->ldy, c->n, 2 * c->rows_alloc, c->xbf, c->ldxb, c->gram_sms);
-        if (!c->pair_plan) return fail(c, CASGD_ECUDA, "cuTensorMapEncodeTiled failed for the pair Gram kernel");
+    GramPairPlan *&plan = c->pair_plans[pipe ? 1 : 0];
+    if (plan && c->pair_plan_sms[pipe ? 1 : 0] != c->gram_sms) { gram_pair_plan_destroy(plan); plan = nullptr; }
+    if (!plan) {
+        c->pair_plan_sms[pipe ? 1 : 0] = c->gram_sms;
+        plan = gram_pair_plan_create(c->Y, c->ldy, c->n, 2 * c->rows_alloc, c->xbf, c->ldxb, c->gram_sms);
+        if (!plan) return fail(c, CASGD_ECUDA, "cuTensorMapEncodeTiled failed for the pair Gram kernel");
     }
+    c->pair_plan = plan;
     int bn = 0;
     const int64_t span = gram_pair_prepare(c->pair_plan, sb, b, (int)c->opt_full_lower, opt == 3 ? 256 : opt == 4 ? 512 : 0,
-                                           (int)c->opt_ksplit, &bn, pipelined_mode(c, s, b));
+                                           (int)c->opt_ksplit, &bn, pipe);
     if (span < 0) {
         if (opt >= 3) return fail(c, CASGD_EINVAL, "the pair Gram kernel cannot run s*b = %d (work list too long)", sb);
         return CASGD_OK;
@@ -558,6 +563,10 @@ int get_graph(casgd_ctx *c, int32_t s, int32_t b, float eta, int32_t len, GraphE
     auto it = c->graphs.find(key);
     if (it != c->graphs.end()) { *out = it->second; return CASGD_OK; }
     cudaGraph_t graph = nullptr;
+    {   // kernel choice, SM budgets and work lists of this graph's schedule (outside the capture: lists are uploaded)
+        const int rc0 = choose_gram(c, s, b, len > 1);
+        if (rc0) return rc0;
+    }
     // captured on a stream of the library's own (the caller's may be the legacy default stream, which cannot
     // be captured); nothing runs during capture, and replays are launched on the caller's stream
     if (!c->capture_stream) CK(cudaStreamCreateWithFlags(&c->capture_stream, cudaStreamNonBlocking));
@@ -585,6 +594,7 @@ int get_graph(casgd_ctx *c, int32_t s, int32_t b, float eta, int32_t len, GraphE
                 io.gathered = h > 0;
                 io.next_idx_off = h + 1 < len ? (int64_t)(h + 1) * s * b : -1;
             }
+            if (c->opt_snapshot && h + 1 == len) kernels += launch_snapshot(c->capture_stream, nullptr, c->ind, c->n, c->x_snap);
             rc = enqueue_step(c, c->capture_stream, nullptr, c->ind, (int64_t)h * s * b, nullptr, s, b, eta, &kernels, io);
         }
     }
@@ -639,7 +649,7 @@ int run_steps(casgd_ctx *c, const int32_t *idx, int64_t n_steps, float *x, int32
         CK(cudaGetLastError());
         return CASGD_OK;
     }
-    rc = choose_gram(c, s, b);
+    rc = choose_gram(c, s, b, false);
     if (rc) return rc;
     rc = ensure_shadow(c, x);
     if (rc) return rc;
@@ -665,6 +675,7 @@ int run_steps(casgd_ctx *c, const int32_t *idx, int64_t n_steps, float *x, int32
             }
         }
     }
+    if (done < n_steps && (rc = choose_gram(c, s, b, false))) return rc;      // single steps: every kernel on the whole chip
     for (; done < n_steps; ++done) {
         int64_t kernels = 0;
         rc = enqueue_step(c, c->stream, idx + done * sb, nullptr, 0, x, s, b, eta, &kernels);
@@ -749,6 +760,7 @@ int casgd_init(casgd_ctx **out, const uint16_t *X_bf16, int64_t ldx, const float
               ck(cudaMalloc(&c->loss_result, sizeof(double))) &&
               ck(cudaMallocHost(&c->loss_result_host, sizeof(double))) &&
               ck(cudaMalloc(&c->x_stage, sizeof(float) * (size_t)n)) &&
+              ck(cudaMalloc(&c->x_snap, sizeof(float) * (size_t)n)) &&
               ck(cudaMalloc(&c->stamps, sizeof(unsigned long long) * kStampWords)) &&
               ck(cudaMemsetAsync(c->stamps, 0, sizeof(unsigned long long) * kStampWords, c->stream));
     if (!ok) return bail(CASGD_ENOMEM);
@@ -833,11 +845,11 @@ int casgd_step_local(casgd_ctx *c, const int32_t *idx, const float *x, int32_t s
     if (rc) return rc;
     if (!payload_out || ((uintptr_t)payload_out & 15)) return fail(c, CASGD_EINVAL, "payload_out must be a 16-byte aligned device pointer");
     const int32_t sb = s * b;
-    if ((rc = ensure_workspace(c, sb)) || (rc = choose_gram(c, s, b)) || (rc = ensure_shadow(c, x))) return rc;
+    if ((rc = ensure_workspace(c, sb)) || (rc = choose_gram(c, s, b, false)) || (rc = ensure_shadow(c, x))) return rc;
     c->last_s = s; c->last_b = b; c->last_buf = 0;
     int64_t kernels = 0;
     const bool narrow = c->cur_gram == 4;
-    const bool split_margin = pipelined_mode(c, s, b);
+    const bool split_margin = false;
     if (!narrow && (rc = stage_gather(c, c->stream, idx, nullptr, 0, sb, 0, c->gram_sms, &kernels))) return rc;
     if ((narrow || s > 1) && (rc = stage_gram(c, c->stream, idx, nullptr, 0, s, b, 0, split_margin ? nullptr : c->r, &kernels))) return rc;
     if ((split_margin || (s == 1 && !narrow)) && (rc = stage_margin(c, c->stream, x, nullptr, sb, 0, &kernels))) return rc;
@@ -940,7 +952,7 @@ int casgd_debug_export(casgd_ctx *c, int what, void *dst_host, int64_t dst_bytes
     if (!c) return CASGD_EINVAL;
     if (!dst_host) return fail(c, CASGD_EINVAL, "dst_host is null");
     const int64_t sb = (int64_t)c->last_s * c->last_b;
-    if (sb == 0 && what != CASGD_DBG_XBF && what != CASGD_DBG_STAMPS && what != CASGD_DBG_GUARDS) return fail(c, CASGD_EINVAL, "no outer step has run yet");
+    if (sb == 0 && what != CASGD_DBG_XBF && what != CASGD_DBG_STAMPS && what != CASGD_DBG_GUARDS && what != CASGD_DBG_XSNAP) return fail(c, CASGD_EINVAL, "no outer step has run yet");
     CK(cudaStreamSynchronize(c->stream));
     auto need = [&](int64_t bytes) { return dst_bytes == bytes; };
     switch (what) {
@@ -965,6 +977,10 @@ int casgd_debug_export(casgd_ctx *c, int what, void *dst_host, int64_t dst_bytes
         *reinterpret_cast<int64_t *>(dst_host) = bad;
         return CASGD_OK;
     }
+    case CASGD_DBG_XSNAP:
+        if (!need((int64_t)c->n * 4)) break;
+        CK(cudaMemcpy(dst_host, c->x_snap, (size_t)c->n * 4, cudaMemcpyDeviceToHost));
+        return CASGD_OK;
     case CASGD_DBG_STAMPS:
         if (!need((int64_t)kStampSlots * 16)) break;
         CK(cudaMemcpy(dst_host, c->stamps + kStampRaw, (size_t)kStampSlots * 16, cudaMemcpyDeviceToHost));
@@ -1011,6 +1027,7 @@ int casgd_set_option(casgd_ctx *c, int option, int64_t value)
         c->opt_overlap = value; break;
     case CASGD_OPT_MARGIN_SPLIT: c->opt_split = value != 0; break;
     case CASGD_OPT_MINI: c->opt_mini = value != 0; break;
+    case CASGD_OPT_SNAPSHOT: c->opt_snapshot = value != 0; break;
     case CASGD_OPT_CHAIN_SMS:
         if (value < 0 || value > 1024) return fail(c, CASGD_EINVAL, "CASGD_OPT_CHAIN_SMS must be in [0, 1024]");
         c->opt_chain_sms = value; break;
@@ -1069,7 +1086,7 @@ void casgd_destroy(casgd_ctx *c)
     cudaFree(c->A_owned); cudaFree(c->A32); cudaFree(c->xbf);
     cudaFree(c->gws.partial); cudaFree(c->gws.counters); cudaFree(c->ind); cudaFree(c->err_flag);
     cudaFree(c->rws.utag); cudaFree(c->rws.epoch); cudaFree(c->stamps);
-    cudaFree(c->loss_partials); cudaFree(c->loss_result); cudaFree(c->idx_stage); cudaFree(c->x_stage);
+    cudaFree(c->loss_partials); cudaFree(c->loss_result); cudaFree(c->idx_stage); cudaFree(c->x_stage); cudaFree(c->x_snap);
     if (c->err_flag_host) cudaFreeHost(c->err_flag_host);
     if (c->loss_result_host) cudaFreeHost(c->loss_result_host);
     delete c;

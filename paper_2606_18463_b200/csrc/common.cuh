@@ -306,6 +306,7 @@ int launch_loss(cudaStream_t st, const uint16_t *A, int64_t lda, const uint16_t 
 
 int launch_sample_indices(cudaStream_t st, int32_t *idx, int64_t n_steps, int32_t sb, int64_t m, uint64_t seed,
                           uint64_t first_step);
+int launch_snapshot(cudaStream_t st, const float *x, const StepParams *ind, int32_t n, float *dst);
 int launch_shadow(cudaStream_t st, const float *x, const StepParams *ind, int32_t n, uint16_t *xbf, int32_t ldxb, int split);
 int launch_widen(cudaStream_t st, const uint16_t *A, int64_t lda, int64_t m, int32_t n, float *A32, int64_t lda32, int num_sms);
 int launch_repack(cudaStream_t st, const uint16_t *X, int64_t ldx, int64_t m, int32_t n, uint16_t *A, int64_t lda, int num_sms);

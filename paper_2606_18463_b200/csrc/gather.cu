@@ -196,6 +196,22 @@ int launch_shadow(cudaStream_t st, const float *x, const StepParams *ind, int32_
     return 1;
 }
 
+// CASGD_OPT_SNAPSHOT: the iterate as it enters the last step of a graph (tests compare that step with the oracle)
+__global__ void snapshot_kernel(const float *x, const StepParams *ind, int32_t n, float *dst)
+{
+    pdl_trigger();
+    pdl_wait();
+    const float *xs = ind ? ind->x : x;
+    const int32_t k = blockIdx.x * blockDim.x + threadIdx.x;
+    if (k < n) dst[k] = ld_dep(xs + k);
+}
+
+int launch_snapshot(cudaStream_t st, const float *x, const StepParams *ind, int32_t n, float *dst)
+{
+    launch_pdl(snapshot_kernel, dim3((n + 255) / 256), dim3(256), 0, st, 1, x, ind, n, dst);
+    return 1;
+}
+
 // Exact FP32 widening of A for the all-FP32 baseline (Recipe A storage, Table 3).
 __global__ void widen_kernel(const uint16_t *__restrict__ A, int64_t lda, int64_t m, int32_t n, float *__restrict__ A32,
                              int64_t lda32)

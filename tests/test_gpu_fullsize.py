@@ -55,24 +55,29 @@ def test_second_graph_step_at_full_size_matches_the_oracle(binding, oracle_mod, 
     assert free > need, f"{cfg.name} needs {need / 1e9:.1f} GB of device memory, {free / 1e9:.1f} GB free"
     ds = synth.make_dataset(cfg, seed=42, device="cuda")
     b, sb = cfg.b, s * cfg.b
-    idx = synth.epoch_indices(cfg, 42, 0)[: 2 * sb].copy()
+    steps = 8                                           # one 8-step CUDA graph: the schedule bench.py's 64-step graphs use
+    idx = synth.epoch_indices(cfg, 42, 0)[: steps * sb].copy()
     idx_d = torch.from_numpy(idx).cuda()
     stream = torch.cuda.Stream()
     with torch.cuda.stream(stream):
         cg = binding.Casgd(ds.X_bf16, ds.y, cfg.loss, stream=stream)
     try:
-        # the first iteration alone (direct launches), to learn the FP32 bits the second one starts from
+        # eight iterations the way bench.py runs them: one casgd_outer_steps call replayed from a CUDA graph (pipelined:
+        # gather + Gram of iteration t + 1 beside the chain of iteration t), or, for tiny steps, one persistent launch.
+        # The last one is compared with the oracle from the FP32 bits it started from: the graph copies x aside before
+        # its last step (CASGD_OPT_SNAPSHOT); the one-launch kernel gives the same bits for a 7-step call.
+        cg.set_option(binding.OPT_SNAPSHOT, 1)
         x1 = torch.zeros(cfg.n, device="cuda")
-        cg.outer_step(idx_d[:sb], x1, s, b, cfg.eta)
+        cg.outer_steps(idx_d[: (steps - 1) * sb], x1, s, b, cfg.eta)
         cg.sync()
-        x1_host = x1.cpu().numpy().copy()
-        # both iterations the way bench.py runs them: one casgd_outer_steps call, replayed from a CUDA graph
         x2 = torch.zeros(cfg.n, device="cuda")
         n0 = cg.launch_count()
-        cg.outer_steps(idx_d, x2, s, b, cfg.eta, n_steps=2)
+        cg.outer_steps(idx_d, x2, s, b, cfg.eta)
         cg.sync()
-        assert cg.launch_count() - n0 >= 1              # the library's own kernels ran (tiny steps: ONE launch for both)
-        A_bits, y, local = _host_rows(ds, idx[sb:])
+        launched = cg.launch_count() - n0
+        assert launched >= 1                            # the library's own kernels ran
+        x1_host = x1.cpu().numpy().copy() if launched == 1 else cg.debug(binding.DBG_XSNAP).copy()
+        A_bits, y, local = _host_rows(ds, idx[(steps - 1) * sb:])
         ref = oracle_mod.outer_step_gram(A_bits, y, local, x1_host.astype(np.float64), s, b, cfg.eta, cfg.loss, shadow=True)
         compare_last_step(oracle_mod, cg, ref, y[local], x1_host, x2, s, b, cfg.eta, cfg.loss, binding)
         # the first iteration from x = 0 has a closed form for its first block (r = 0): u_0 = l'(0, y)

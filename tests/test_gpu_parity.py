@@ -171,7 +171,10 @@ def test_grid_recurrence_replays_from_a_graph(binding):
             xb = torch.zeros(cfg.n, device="cuda")
             cg.outer_steps(idx_d, xb, s, b, cfg.eta)
             cg.sync()
-            assert torch.equal(xa, xb)
+            if impl in (2, 3):
+                assert torch.equal(xa, xb)              # sequential graphs: the very kernels of the single steps
+            else:                                       # pipelined graphs: the margin is a kernel of its own there
+                assert torch.linalg.norm(xa - xb) <= 1e-5 * torch.linalg.norm(xa)
             xs[impl] = xa
     for impl in (2, 3, 4):
         assert torch.linalg.norm(xs[1] - xs[impl]) <= 1e-5 * torch.linalg.norm(xs[1])
@@ -309,8 +312,8 @@ def test_fp32_sgd_baseline_matches_the_oracle(binding, oracle_mod, ci, m, n):
 
 
 def test_graph_replay_and_host_entry_point_equal_single_steps(binding):
-    """casgd_outer_steps (CUDA-graph replay) and casgd_outer_steps_host run the same kernels as repeated
-    casgd_outer_step: bitwise-equal x (every reduction in the library has a fixed order)."""
+    """casgd_outer_steps (CUDA-graph replay) and casgd_outer_steps_host against repeated casgd_outer_step: bitwise-equal
+    x wherever the same kernels run (every reduction in the library has a fixed order), equal to rounding otherwise."""
     cfg = synth.config(4, m=20000, n=512)
     X_d, y_d, _, _ = device_dataset(cfg)
     s, b, steps = 8, 64, 21                     # 21 = 8 + 8 + 5 singles: exercises both graph lengths
@@ -325,11 +328,19 @@ def test_graph_replay_and_host_entry_point_equal_single_steps(binding):
         cg.outer_steps(idx_d, xb, s, b, cfg.eta)
         assert cg.launch_count() > n0
         cg.sync()
-        assert torch.equal(xa, xb)
+        # the pipelined graphs compute r in a kernel of its own (FP32 FMA order instead of the tensor core's): same
+        # iterate up to rounding; with CASGD_OPT_OVERLAP = 0 the graphs replay the single steps' kernels, bit for bit
+        assert torch.linalg.norm(xa - xb) <= 1e-5 * torch.linalg.norm(xa)
+        cg.set_option(binding.OPT_OVERLAP, 0)
+        xs = torch.zeros(cfg.n, device="cuda")
+        cg.outer_steps(idx_d, xs, s, b, cfg.eta)
+        cg.sync()
+        assert torch.equal(xa, xs)
+        cg.set_option(binding.OPT_OVERLAP, 2)
         xh = torch.zeros(cfg.n).pin_memory()
         idx_h = torch.from_numpy(idx).pin_memory()
         cg.outer_steps_host(idx_h, xh, s, b, cfg.eta)
-        assert torch.equal(xa.cpu(), xh)
+        assert torch.equal(xb.cpu(), xh)
         # one step per call (the static host graph: staging copies, shadow rebuild, step, copy back), from pageable memory too
         x1 = torch.zeros(cfg.n)
         for h in range(steps):
@@ -342,8 +353,9 @@ def test_graph_replay_and_host_entry_point_equal_single_steps(binding):
 def test_next_step_gather_on_the_side_branch_changes_nothing(binding, oracle_mod, ci, m, n, s, b, overlap):
     """CASGD_OPT_OVERLAP: inside the graphs of casgd_outer_steps the next step's rows are gathered (mode 1), or gathered
     and their Gram matrix computed (mode 2, the margin then being a kernel of its own), on a side branch beside this
-    step's recurrence and update. The iterate equals repeated casgd_outer_step bit for bit in every mode, and the last
-    step's exported intermediates (taken from the stage that step used) match oracle O1."""
+    step's recurrence and update. The iterate equals repeated casgd_outer_step bit for bit in modes 0 and 1 (same
+    kernels), to rounding in mode 2 (its margin is a kernel of its own), and the last step's exported intermediates (taken
+    from the stage that step used) match oracle O1."""
     cfg = synth.config(ci, m=m, n=n)
     X_d, y_d, A_bits, y = device_dataset(cfg)
     steps = 64 + 8 + 8 + 1                      # a 64-step graph, two 8-step graphs, a single
@@ -358,7 +370,8 @@ def test_next_step_gather_on_the_side_branch_changes_nothing(binding, oracle_mod
         xb = torch.zeros(cfg.n, device="cuda")
         cg.outer_steps(idx_d[: (steps - 9) * s * b], xb, s, b, eta)      # 64 + 8: ends on an 8-step graph (stage 1)
         cg.sync()
-        assert torch.equal(xa, xb)
+        same = (lambda p, q: torch.equal(p, q)) if overlap < 2 else (lambda p, q: bool(torch.linalg.norm(p - q) <= 1e-4 * torch.linalg.norm(p)))
+        assert same(xa, xb)
         x0 = xb.cpu().numpy().copy()
         cg.outer_steps(idx_d[(steps - 9) * s * b: (steps - 1) * s * b], xb, s, b, eta)
         cg.sync()
@@ -367,7 +380,7 @@ def test_next_step_gather_on_the_side_branch_changes_nothing(binding, oracle_mod
         x_before_last = xa.cpu().numpy().copy()
         cg.outer_step(idx_d[(steps - 2) * s * b:(steps - 1) * s * b], xa, s, b, eta)
         cg.sync()
-        assert torch.equal(xa, xb)
+        assert same(xa, xb)
         # the last step of the 8-step graph, against the oracle from the same FP32 bits
         xc = torch.from_numpy(x0.copy()).cuda()
         cg.outer_steps(idx_d[(steps - 9) * s * b: (steps - 1) * s * b], xc, s, b, eta)
@@ -459,6 +472,20 @@ def test_margin_of_the_fp32_master(binding, oracle_mod, ci, m, n, s, b, mode):
         cg.outer_step(torch.from_numpy(idx).cuda(), x1, s, b, cfg.eta)
         cg.sync()
         check_step_against_oracle(oracle_mod, cg, A_bits, y, idx, x1.cpu().numpy(), s, b, cfg.eta, cfg.loss, binding, shadow=False)
+        if mode == "pipelined":
+            # the pipelined GRAPH computes r in the stand-alone margin kernel, from the FP32 x itself: its last step
+            # against the oracle from the bits it started from (CASGD_OPT_SNAPSHOT)
+            cg.set_option(binding.OPT_SNAPSHOT, 1)
+            idx8 = np.concatenate([synth.epoch_indices(cfg, 42, e) for e in range(-(-8 * s * b // m) + 1)])[: 8 * s * b].copy()
+            xg = torch.from_numpy(x0.copy()).cuda()
+            n0 = cg.launch_count()
+            cg.outer_steps(torch.from_numpy(idx8).cuda(), xg, s, b, cfg.eta * 0.25)
+            cg.sync()
+            if cg.launch_count() - n0 > 1:              # (not the one-launch kernel)
+                xs = cg.debug(binding.DBG_XSNAP).copy()
+                last = idx8[7 * s * b:]
+                ref = oracle_mod.outer_step_gram(A_bits, y, last, xs.astype(np.float64), s, b, cfg.eta * 0.25, cfg.loss, shadow=False)
+                compare_last_step(oracle_mod, cg, ref, y[last], xs, xg, s, b, cfg.eta * 0.25, cfg.loss, binding, shadow=False)
         # negative control: with the split off, r is the margin of bf16(x), which is NOT within 1e-5 of Y x
         cg.set_option(binding.OPT_MARGIN_SPLIT, 0)
         with pytest.raises(AssertionError, match="margin"):
@@ -478,7 +505,9 @@ def test_on_device_sampling_matches_the_oracle_sampler(binding, oracle_mod, ci, 
     eta = cfg.eta if cfg.loss != synth.POISSON else 0.01
     with binding.Casgd(X_d, y_d, cfg.loss) as cg:
         xa = torch.zeros(n, device="cuda")
-        cg.outer_steps(torch.from_numpy(idx).cuda(), xa, s, b, eta)
+        idx_d = torch.from_numpy(idx).cuda()
+        cg.outer_steps(idx_d[: 4 * sb], xa, s, b, eta)                      # the same split into calls as below: the same
+        cg.outer_steps(idx_d[4 * sb:], xa, s, b, eta)                      # schedules (graph lengths), hence the same kernels
         cg.sync()
         xb = torch.zeros(n, device="cuda")
         cg.outer_steps_sampled(xb, s, b, eta, n_steps=4, seed=seed, first_step=0)
