@@ -361,7 +361,8 @@ int stage_margin(casgd_ctx *c, cudaStream_t st, const float *x, const StepParams
 
 // recurrence and update of the rows in stage `buf`
 int stage_chain(casgd_ctx *c, cudaStream_t st, float *x, const StepParams *ind, int32_t s, int32_t b, float alpha, int buf,
-                bool late_trigger, const std::function<void()> &after_recurrence, int64_t *kernels, bool force_recurrence = false)
+                bool late_trigger, const std::function<void()> &after_recurrence, int64_t *kernels, bool force_recurrence = false,
+                bool fuse_margin = false)
 {
     const int32_t sb = s * b;
     uint16_t *Y = c->Y + (size_t)buf * c->rows_alloc * c->ldy;
@@ -371,7 +372,7 @@ int stage_chain(casgd_ctx *c, cudaStream_t st, float *x, const StepParams *ind, 
     const bool fused = !c->opt_no_fuse && recurrence_fuses_update(s, b, c->ldg, c->ldy, c->rws, (int)c->opt_rec_impl);
     if (!step_is_s1(c, s) || force_recurrence) {
         StageTimer t(c, CASGD_STAGE_RECURRENCE);
-        const FusedUpdate fu{Y, c->ldy, c->n, x, ind, c->xbf, c->opt_split ? c->ldxb : 0};
+        const FusedUpdate fu{Y, c->ldy, c->n, x, ind, c->xbf, c->opt_split ? c->ldxb : 0, fuse_margin ? c->r : nullptr};
         c->rws.late_trigger = late_trigger;
         k = launch_recurrence(st, G, c->ldg, c->r, yI, s, b, alpha, c->loss, c->z, c->u, c->rws,
                               (int)c->opt_rec_impl, fused ? &fu : nullptr);
@@ -471,7 +472,12 @@ int capture_pipelined(casgd_ctx *c, int32_t s, int32_t b, float eta, int32_t len
         c->cur_slot_step = h;
         cudaStreamWaitEvent(M, c->ev_gather[buf], 0);
         if (c->opt_snapshot && h + 1 == len) *kernels += launch_snapshot(M, nullptr, c->ind, c->n, c->x_snap);
-        if ((rc = stage_margin(c, M, nullptr, c->ind, sb, buf, kernels))) break;
+        // small Y (the shapes whose update the recurrence cluster does itself): the cluster computes its rows' margin too
+        // -- while a CTA's share of Y is a few KB (measured: n = 18, s*b = 2048, 8 KB per CTA: 21.1 -> 20.6 us per step;
+        // n = 512, 128 KB per CTA: 26.3 -> 27.4, the 16 SMs of the cluster are slower at it than a kernel on 32)
+        const bool fuse_margin = !c->opt_no_fuse && recurrence_fuses_update(s, b, c->ldg, c->ldy, c->rws, (int)c->opt_rec_impl) &&
+                                 (int64_t)sb * c->ldy * 2 <= (int64_t)16 * 1024 * std::max(1, c->rws.cluster);
+        if (!fuse_margin && (rc = stage_margin(c, M, nullptr, c->ind, sb, buf, kernels))) break;
         cudaStreamWaitEvent(M, c->ev_gram[buf], 0);
         const bool more = h + 1 < len;
         if (more) g_completion_event = c->ev_rec_launch;
@@ -480,7 +486,7 @@ int capture_pipelined(casgd_ctx *c, int32_t s, int32_t b, float eta, int32_t len
             if (more) rc_side = side_step(h + 1, h >= 1, true);
             c->cur_slot_step = h;
         };
-        rc = stage_chain(c, M, nullptr, c->ind, s, b, alpha, buf, true, after, kernels);
+        rc = stage_chain(c, M, nullptr, c->ind, s, b, alpha, buf, true, after, kernels, false, fuse_margin);
         if (!rc) rc = rc_side;
         cudaEventRecord(c->ev_grad, M);
     }

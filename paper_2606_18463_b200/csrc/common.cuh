@@ -113,6 +113,16 @@ __device__ __forceinline__ float dot8(const uint4 &a, const float4 &x0, const fl
     return acc;
 }
 
+// dot of 8 BF16 with 8 BF16 (two 16-byte vectors), FP32 accumulation
+__device__ __forceinline__ float dot8_bf16(const uint4 &a, const uint4 &x, float acc)
+{
+    acc = fmaf(bf16lo(a.x), bf16lo(x.x), acc); acc = fmaf(bf16hi(a.x), bf16hi(x.x), acc);
+    acc = fmaf(bf16lo(a.y), bf16lo(x.y), acc); acc = fmaf(bf16hi(a.y), bf16hi(x.y), acc);
+    acc = fmaf(bf16lo(a.z), bf16lo(x.z), acc); acc = fmaf(bf16hi(a.z), bf16hi(x.z), acc);
+    acc = fmaf(bf16lo(a.w), bf16lo(x.w), acc); acc = fmaf(bf16hi(a.w), bf16hi(x.w), acc);
+    return acc;
+}
+
 __device__ __forceinline__ uint4 ldg_nc_v4(const void *p)
 {
     uint4 r;
@@ -260,6 +270,7 @@ struct FusedUpdate {
     const StepParams *ind;
     uint16_t *xbf;
     int32_t split_ld;              // CASGD_OPT_MARGIN_SPLIT: row stride of the shadow buffer (0 = row 0 only)
+    float *r_fused;                // non-null: the kernel also computes r = Y x_bf (Alg. 1 line 3) for its own rows first
 };
 bool recurrence_fuses_update(int32_t s, int32_t b, int32_t ldg, int32_t ldy, const RecWorkspace &ws, int impl);
 int recurrence_kernel_choice(int32_t s, int32_t b, int32_t ldg, const RecWorkspace &ws, int impl, bool fused);

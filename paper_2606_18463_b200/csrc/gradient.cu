@@ -309,14 +309,6 @@ __device__ __forceinline__ uint4 ld_stream_v4(const void *p)
     return r;
 }
 
-__device__ __forceinline__ float dot8_bf16(const uint4 &a, const uint4 &x, float acc)
-{
-    acc = fmaf(bf16lo(a.x), bf16lo(x.x), acc); acc = fmaf(bf16hi(a.x), bf16hi(x.x), acc);
-    acc = fmaf(bf16lo(a.y), bf16lo(x.y), acc); acc = fmaf(bf16hi(a.y), bf16hi(x.y), acc);
-    acc = fmaf(bf16lo(a.z), bf16lo(x.z), acc); acc = fmaf(bf16hi(a.z), bf16hi(x.z), acc);
-    acc = fmaf(bf16lo(a.w), bf16lo(x.w), acc); acc = fmaf(bf16hi(a.w), bf16hi(x.w), acc);
-    return acc;
-}
 
 __global__ void __launch_bounds__(32 * kMgWarps)
 margin_kernel(const uint16_t *Y, int32_t ldy, int32_t sb, const uint16_t *xbf, const float *x32, const StepParams *ind,

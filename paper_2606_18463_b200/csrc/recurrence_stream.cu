@@ -121,6 +121,7 @@ struct FusedGrad {
     const StepParams *ind;
     uint16_t *xbf;
     int32_t split_ld;
+    float *r_fused;             // pipelined schedule, small Y: the margin of this CTA's rows is computed here (no margin kernel)
 };
 constexpr int kFgMaxLdy = 2048;                          // columns (padded) the fused update handles
 
@@ -225,6 +226,52 @@ recurrence_stream_kernel(const float *G, int32_t ldg, const float *r,
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     pdl_wait();                                         // G, r and y_I come from the Gram and gather kernels
     stamp_begin(stamp);
+    if (fg.r_fused) {
+        // Alg. 1 line 3 for the rows THIS CTA's critical warps own (row group q -> CTA q mod C, every block): r = Y x_bf,
+        // a warp per row -- the pipelined schedule's stand-alone margin kernel folded in when Y is small (one launch and
+        // its gap less on the chain). With CASGD_OPT_MARGIN_SPLIT the residue rows of the shadow are added (== FP32 x).
+        const int mine = s * qpc * kQuad;
+        const int nvec = fg.ldy >> 3;
+        int LG = 1;
+        while (LG < nvec && LG < 32) LG <<= 1;          // lanes side by side on a row; 32 / LG rows per warp and pass
+        const int sub = lane % LG, rsub = lane / LG, RP = 32 / LG;
+        auto row_of = [&](int t) {
+            const int j = t / (qpc * kQuad), rem = t - j * (qpc * kQuad);
+            return j * b + kQuad * (crank + (rem >> 2) * C) + (rem & 3);
+        };
+        // four passes at once: four row loads per lane in flight (a pass per L2 round trip was 3 us of prologue)
+        for (int t0 = warp * RP * 4; t0 < mine; t0 += kWarps * RP * 4) {
+            float acc[4] = {0.f, 0.f, 0.f, 0.f};
+            const uint16_t *yr[4];
+            bool on[4];
+#pragma unroll
+            for (int q = 0; q < 4; ++q) {
+                const int t = t0 + q * RP + rsub;
+                on[q] = t < mine;
+                yr[q] = fg.Y + (int64_t)row_of(on[q] ? t : 0) * fg.ldy;
+            }
+            for (int cv = sub; cv < nvec; cv += LG) {
+                uint4 v[4];
+#pragma unroll
+                for (int q = 0; q < 4; ++q) v[q] = on[q] ? ld_dep_v4(yr[q] + cv * 8) : make_uint4(0u, 0u, 0u, 0u);
+                const uint4 x0 = ld_dep_v4(fg.xbf + cv * 8);
+#pragma unroll
+                for (int q = 0; q < 4; ++q) acc[q] = dot8_bf16(v[q], x0, acc[q]);
+                if (fg.split_ld) {
+                    const uint4 x1 = ld_dep_v4(fg.xbf + fg.split_ld + cv * 8), x2 = ld_dep_v4(fg.xbf + 2 * fg.split_ld + cv * 8);
+#pragma unroll
+                    for (int q = 0; q < 4; ++q) acc[q] = dot8_bf16(v[q], x2, dot8_bf16(v[q], x1, acc[q]));
+                }
+            }
+#pragma unroll
+            for (int q = 0; q < 4; ++q) {
+                for (int o = LG >> 1; o > 0; o >>= 1) acc[q] += __shfl_xor_sync(0xffffffffu, acc[q], o);
+                if (on[q] && sub == 0) fg.r_fused[row_of(t0 + q * RP + rsub)] = acc[q];
+            }
+        }
+        __threadfence_block();
+        __syncthreads();                                // the critical warps below read r through ld_dep
+    }
 
     // Warp w runs on scheduler w & 3. Critical warps: (group gamma, parity e) -> warp gamma + 4 e.
     const int wsched = warp & 3, wslot = warp >> 2;
@@ -596,7 +643,7 @@ int launch_recurrence_stream(cudaStream_t st, const float *G, int32_t ldg, const
                              int late_trigger)
 {
     FusedGrad fg{};
-    if (fu) fg = FusedGrad{fu->Y, fu->ldy, fu->n, fu->x, fu->ind, fu->xbf, fu->split_ld};
+    if (fu) fg = FusedGrad{fu->Y, fu->ldy, fu->n, fu->x, fu->ind, fu->xbf, fu->split_ld, fu->r_fused};
     cudaError_t e = loss == CASGD_LOGISTIC ? launch_stream<CASGD_LOGISTIC>(st, G, ldg, r, yI, s, b, alpha, z, u, cluster, fg, late_trigger)
                   : loss == CASGD_LINEAR  ? launch_stream<CASGD_LINEAR>(st, G, ldg, r, yI, s, b, alpha, z, u, cluster, fg, late_trigger)
                                           : launch_stream<CASGD_POISSON>(st, G, ldg, r, yI, s, b, alpha, z, u, cluster, fg, late_trigger);
