@@ -373,7 +373,10 @@ int stage_chain(casgd_ctx *c, cudaStream_t st, float *x, const StepParams *ind, 
     if (!step_is_s1(c, s) || force_recurrence) {
         StageTimer t(c, CASGD_STAGE_RECURRENCE);
         const FusedUpdate fu{Y, c->ldy, c->n, x, ind, c->xbf, c->opt_split ? c->ldxb : 0, fuse_margin ? c->r : nullptr};
-        c->rws.late_trigger = late_trigger;
+        // late trigger: keep the dependent GRADIENT kernel's CTAs from becoming resident (and waiting) on SMs the side
+        // branch needs. With the update fused in, the dependent is the next recurrence (after its Gram, a full edge):
+        // let it launch early -- its launch latency is then off the chain (1.5 us per step on the chain-bound shapes)
+        c->rws.late_trigger = late_trigger && !fused;
         k = launch_recurrence(st, G, c->ldg, c->r, yI, s, b, alpha, c->loss, c->z, c->u, c->rws,
                               (int)c->opt_rec_impl, fused ? &fu : nullptr);
         g_completion_event = nullptr;
