@@ -68,7 +68,8 @@ struct casgd_ctx {
     cudaStream_t capture_stream = nullptr;
     cudaStream_t side_stream = nullptr;       // graph capture only: the branch that gathers the next step's rows
     cudaEvent_t ev_fork = nullptr, ev_join = nullptr;
-    cudaEvent_t ev_gather[2] = {nullptr, nullptr}, ev_gram[2] = {nullptr, nullptr}, ev_grad = nullptr, ev_rec_launch = nullptr;
+    cudaStream_t gather_stream = nullptr;     // ... and the branch that gathers the rows of the step after next
+    cudaEvent_t ev_gather[3] = {nullptr, nullptr, nullptr}, ev_gram[2] = {nullptr, nullptr}, ev_grad = nullptr, ev_rec_launch = nullptr;
     // dataset
     const uint16_t *A = nullptr;      // BF16 bits, row stride lda (borrowed or owned)
     uint16_t *A_owned = nullptr;
@@ -83,8 +84,8 @@ struct casgd_ctx {
     // per-step workspaces, sized for rows_alloc rows
     int32_t rows_alloc = 0;
     int32_t ldy = 0, ldg = 0;
-    uint16_t *Y = nullptr;            // TWO stages of rows_alloc rows: step h of a graph uses stage h & 1, so that the
-                                      // next step's gather can run beside this step's recurrence and update
+    uint16_t *Y = nullptr;            // THREE stages of rows_alloc rows (and of y_I), two of G: in the pipelined graphs step h
+                                      // uses Y stage h % 3 and G stage h & 1 (a stage index below is y | g << 2)
     float *yI = nullptr, *G = nullptr, *r = nullptr, *z = nullptr, *u = nullptr;     // G, y_I: two stages as well
     float *r_scratch = nullptr;       // pipelined schedule: where the Gram kernels' fused margin (of a stale x) goes
     uint16_t *xbf = nullptr;          // BF16 shadow of x: [16 x ldxb], row 0 = bf16(x), the rest zero
@@ -222,17 +223,17 @@ int ensure_workspace(casgd_ctx *c, int32_t sb)
     free_step_workspace(c);
     const int32_t rows = (int32_t)round_up(sb, 2 * kTile);   // whole 256-row pair tiles: a tile never straddles the two stages
     c->ldg = rows;
-    CK(alloc_guarded(c, &c->Y, sizeof(uint16_t) * (size_t)2 * rows * c->ldy));
-    CK(alloc_guarded(c, &c->yI, sizeof(float) * 2 * rows));
+    CK(alloc_guarded(c, &c->Y, sizeof(uint16_t) * (size_t)3 * rows * c->ldy));
+    CK(alloc_guarded(c, &c->yI, sizeof(float) * 3 * rows));
     CK(alloc_guarded(c, &c->G, sizeof(float) * (size_t)2 * rows * rows));
     CK(alloc_guarded(c, &c->r, sizeof(float) * rows));
     CK(alloc_guarded(c, &c->r_scratch, sizeof(float) * rows));
     CK(alloc_guarded(c, &c->z, sizeof(float) * rows));
     CK(alloc_guarded(c, &c->u, sizeof(float) * rows));
-    CK(cudaMemsetAsync(c->Y, 0, sizeof(uint16_t) * (size_t)2 * rows * c->ldy, c->stream));
+    CK(cudaMemsetAsync(c->Y, 0, sizeof(uint16_t) * (size_t)3 * rows * c->ldy, c->stream));
     CK(cudaMemsetAsync(c->G, 0, sizeof(float) * (size_t)2 * rows * rows, c->stream));
     CK(cudaMemsetAsync(c->r_scratch, 0, sizeof(float) * rows, c->stream));
-    CK(cudaMemsetAsync(c->yI, 0, sizeof(float) * 2 * rows, c->stream));
+    CK(cudaMemsetAsync(c->yI, 0, sizeof(float) * 3 * rows, c->stream));
     CK(cudaMemsetAsync(c->r, 0, sizeof(float) * rows, c->stream));
     CK(cudaMemsetAsync(c->z, 0, sizeof(float) * rows, c->stream));
     CK(cudaMemsetAsync(c->u, 0, sizeof(float) * rows, c->stream));
@@ -307,8 +308,9 @@ int stage_gather(casgd_ctx *c, cudaStream_t st, const int32_t *idx, const StepPa
                  int sms, int64_t *kernels)
 {
     StageTimer t(c, CASGD_STAGE_GATHER);
-    const int k = launch_gather(st, c->A, c->lda, c->y, c->m, c->n, idx, ind, idx_off, sb, c->Y + (size_t)buf * c->rows_alloc * c->ldy,
-                                c->ldy, c->yI + (size_t)buf * c->rows_alloc, c->err_flag, sms);
+    const int yb = buf & 3;
+    const int k = launch_gather(st, c->A, c->lda, c->y, c->m, c->n, idx, ind, idx_off, sb, c->Y + (size_t)yb * c->rows_alloc * c->ldy,
+                                c->ldy, c->yI + (size_t)yb * c->rows_alloc, c->err_flag, sms);
     t.done(k); *kernels += k;
     return CASGD_OK;
 }
@@ -318,10 +320,11 @@ int stage_gram(casgd_ctx *c, cudaStream_t st, const int32_t *idx, const StepPara
                int buf, float *r_out, int64_t *kernels)
 {
     const int32_t sb = s * b;
-    uint16_t *Y = c->Y + (size_t)buf * c->rows_alloc * c->ldy;
-    float *yI = c->yI + (size_t)buf * c->rows_alloc;
-    float *G = c->G + (size_t)buf * c->rows_alloc * c->rows_alloc;
-    const int32_t row_base = buf * c->rows_alloc;
+    const int yb = buf & 3, gb = buf >> 2;
+    uint16_t *Y = c->Y + (size_t)yb * c->rows_alloc * c->ldy;
+    float *yI = c->yI + (size_t)yb * c->rows_alloc;
+    float *G = c->G + (size_t)gb * c->rows_alloc * c->rows_alloc;
+    const int32_t row_base = yb * c->rows_alloc;
     const S1Fuse s1f{c->loss, yI, c->z, c->u};
     int k;
     StageTimer t(c, CASGD_STAGE_GRAM);
@@ -340,7 +343,7 @@ int stage_gram(casgd_ctx *c, cudaStream_t st, const int32_t *idx, const StepPara
         if (k < 0) return CASGD_ECUDA;
     } else {
         if (!c->tc_plan) {
-            c->tc_plan = gram_tc_plan_create(c->Y, c->ldy, c->n, 2 * c->rows_alloc, c->xbf, c->ldxb, c->err, sizeof c->err);
+            c->tc_plan = gram_tc_plan_create(c->Y, c->ldy, c->n, 3 * c->rows_alloc, c->xbf, c->ldxb, c->err, sizeof c->err);
             if (!c->tc_plan) return CASGD_ECUDA;
         }
         k = launch_gram_tc(st, c->tc_plan, row_base, sb, b, G, c->ldg, r_out, (int)c->opt_full_lower, (int)c->opt_ksplit, c->gram_sms, c->err, sizeof c->err);
@@ -353,7 +356,7 @@ int stage_gram(casgd_ctx *c, cudaStream_t st, const int32_t *idx, const StepPara
 int stage_margin(casgd_ctx *c, cudaStream_t st, const float *x, const StepParams *ind, int32_t sb, int buf, int64_t *kernels)
 {
     StageTimer t(c, CASGD_STAGE_MARGIN);
-    const int k = launch_margin(st, c->Y + (size_t)buf * c->rows_alloc * c->ldy, c->ldy, c->n, sb, c->xbf, x, ind, c->opt_split != 0,
+    const int k = launch_margin(st, c->Y + (size_t)(buf & 3) * c->rows_alloc * c->ldy, c->ldy, c->n, sb, c->xbf, x, ind, c->opt_split != 0,
                                 c->r, c->chain_sms);
     t.done(k); *kernels += k;
     return CASGD_OK;
@@ -365,9 +368,9 @@ int stage_chain(casgd_ctx *c, cudaStream_t st, float *x, const StepParams *ind, 
                 bool fuse_margin = false)
 {
     const int32_t sb = s * b;
-    uint16_t *Y = c->Y + (size_t)buf * c->rows_alloc * c->ldy;
-    float *yI = c->yI + (size_t)buf * c->rows_alloc;
-    float *G = c->G + (size_t)buf * c->rows_alloc * c->rows_alloc;
+    uint16_t *Y = c->Y + (size_t)(buf & 3) * c->rows_alloc * c->ldy;
+    float *yI = c->yI + (size_t)(buf & 3) * c->rows_alloc;
+    float *G = c->G + (size_t)(buf >> 2) * c->rows_alloc * c->rows_alloc;
     int k;
     const bool fused = !c->opt_no_fuse && recurrence_fuses_update(s, b, c->ldg, c->ldy, c->rws, (int)c->opt_rec_impl);
     if (!step_is_s1(c, s) || force_recurrence) {
@@ -408,7 +411,7 @@ int enqueue_step(casgd_ctx *c, cudaStream_t st, const int32_t *idx, const StepPa
         // wide rows: gather + margin + l' in one warp-per-row kernel (there is no Gram at s = 1)
         StageTimer t(c, CASGD_STAGE_GRAM);
         const int k = launch_margin_s1(st, c->A, c->lda, c->y, c->m, c->n, idx, ind, idx_off, b, c->loss, c->xbf, c->opt_split ? c->ldxb : 0,
-                                       c->Y + (size_t)io.buf * c->rows_alloc * c->ldy, c->ldy, c->yI + (size_t)io.buf * c->rows_alloc,
+                                       c->Y + (size_t)(io.buf & 3) * c->rows_alloc * c->ldy, c->ldy, c->yI + (size_t)(io.buf & 3) * c->rows_alloc,
                                        c->r, c->z, c->u, c->err_flag);
         t.done(k); *kernels += k;
     } else {
@@ -425,7 +428,7 @@ int enqueue_step(casgd_ctx *c, cudaStream_t st, const int32_t *idx, const StepPa
         c->cur_slot_step = saved_step + 1;              // (stamps: the gather belongs to the next step)
         // the recurrence cluster holds up to 16 SMs: a gather sized for all SMs would leave 16 CTAs waiting for it to
         // finish (measured: 42 us instead of 12)
-        rc = stage_gather(c, c->side_stream, idx, ind, io.next_idx_off, sb, io.buf ^ 1, c->num_sms > 32 ? c->num_sms - 16 : c->num_sms, kernels);
+        rc = stage_gather(c, c->side_stream, idx, ind, io.next_idx_off, sb, (io.buf & 3) ^ 1, c->num_sms > 32 ? c->num_sms - 16 : c->num_sms, kernels);
         c->cur_slot_step = saved_step;
         if (rc) return rc;
         cudaEventRecord(c->ev_join, c->side_stream);
@@ -446,34 +449,46 @@ int enqueue_step(casgd_ctx *c, cudaStream_t st, const int32_t *idx, const StepPa
 // a kernel that becomes resident early only to wait would hold SMs the other branch needs.
 int capture_pipelined(casgd_ctx *c, int32_t s, int32_t b, float eta, int32_t len, int64_t *kernels)
 {
-    cudaStream_t M = c->capture_stream, S = c->side_stream;
+    cudaStream_t M = c->capture_stream, S = c->side_stream, T = c->gather_stream;
     const int32_t sb = s * b;
     const float alpha = eta / (float)b;
+    const bool has_gather = c->cur_gram != 4;           // (narrow rows: the Gram kernel gathers them itself)
     int rc = CASGD_OK;
+    auto stage_of = [](int h) { return (h % 3) | ((h & 1) << 2); };      // Y stage h % 3, G stage h & 1
     cudaEventRecord(c->ev_fork, M);
     cudaStreamWaitEvent(S, c->ev_fork, 0);
-    auto side_step = [&](int h, bool wait_update, bool wait_rec_launch) -> int {
-        const int buf = h & 1;
+    cudaStreamWaitEvent(T, c->ev_fork, 0);
+    // gather(h) on the gather branch. h < 2: up front, on the Gram's share of the SMs; later ones run beside recurrence(h-2),
+    // on the chain's SMs the cluster leaves free (so the side branch is the Gram alone)
+    auto gather_step = [&](int h, bool beside_recurrence) -> int {
+        if (!has_gather) return CASGD_OK;
         c->cur_slot_step = h;
         g_plain_launch = true;
-        int rc2 = CASGD_OK;
-        if (wait_update) cudaStreamWaitEvent(S, c->ev_grad, 0);
-        if (c->cur_gram != 4) {
-            rc2 = stage_gather(c, S, nullptr, c->ind, (int64_t)h * sb, sb, buf, c->gram_sms, kernels);
-            cudaEventRecord(c->ev_gather[buf], S);
-        }
-        if (wait_rec_launch) cudaStreamWaitEvent(S, c->ev_rec_launch, 0);
-        if (!rc2) rc2 = stage_gram(c, S, nullptr, c->ind, (int64_t)h * sb, s, b, buf, nullptr, kernels);
-        cudaEventRecord(c->ev_gram[buf], S);
-        if (c->cur_gram == 4) cudaEventRecord(c->ev_gather[buf], S);
+        if (beside_recurrence) cudaStreamWaitEvent(T, c->ev_rec_launch, 0);
+        const int sms = beside_recurrence ? std::max(8, c->chain_sms - 16) : c->gram_sms;
+        const int rc2 = stage_gather(c, T, nullptr, c->ind, (int64_t)h * sb, sb, stage_of(h), sms, kernels);
+        cudaEventRecord(c->ev_gather[h % 3], T);
         g_plain_launch = false;
         return rc2;
     };
-    rc = side_step(0, false, false);
-    for (int32_t h = 0; h < len && rc == CASGD_OK; ++h) {
-        const int buf = h & 1;
+    auto gram_step = [&](int h, bool wait_rec_launch) -> int {
         c->cur_slot_step = h;
-        cudaStreamWaitEvent(M, c->ev_gather[buf], 0);
+        g_plain_launch = true;
+        if (has_gather) cudaStreamWaitEvent(S, c->ev_gather[h % 3], 0);
+        if (wait_rec_launch) cudaStreamWaitEvent(S, c->ev_rec_launch, 0);
+        const int rc2 = stage_gram(c, S, nullptr, c->ind, (int64_t)h * sb, s, b, stage_of(h), nullptr, kernels);
+        cudaEventRecord(c->ev_gram[h & 1], S);
+        if (!has_gather) cudaEventRecord(c->ev_gather[h % 3], S);
+        g_plain_launch = false;
+        return rc2;
+    };
+    rc = gather_step(0, false);
+    if (!rc && len > 1) rc = gather_step(1, false);
+    if (!rc) rc = gram_step(0, false);
+    for (int32_t h = 0; h < len && rc == CASGD_OK; ++h) {
+        const int buf = stage_of(h);
+        c->cur_slot_step = h;
+        cudaStreamWaitEvent(M, c->ev_gather[h % 3], 0);
         if (c->opt_snapshot && h + 1 == len) *kernels += launch_snapshot(M, nullptr, c->ind, c->n, c->x_snap);
         // small Y (the shapes whose update the recurrence cluster does itself): the cluster computes its rows' margin too
         // -- while a CTA's share of Y is a few KB (measured: n = 18, s*b = 2048, 8 KB per CTA: 21.1 -> 20.6 us per step;
@@ -481,19 +496,25 @@ int capture_pipelined(casgd_ctx *c, int32_t s, int32_t b, float eta, int32_t len
         const bool fuse_margin = !c->opt_no_fuse && recurrence_fuses_update(s, b, c->ldg, c->ldy, c->rws, (int)c->opt_rec_impl) &&
                                  (int64_t)sb * c->ldy * 2 <= (int64_t)16 * 1024 * std::max(1, c->rws.cluster);
         if (!fuse_margin && (rc = stage_margin(c, M, nullptr, c->ind, sb, buf, kernels))) break;
-        cudaStreamWaitEvent(M, c->ev_gram[buf], 0);
+        cudaStreamWaitEvent(M, c->ev_gram[h & 1], 0);
         const bool more = h + 1 < len;
         if (more) g_completion_event = c->ev_rec_launch;
         int rc_side = CASGD_OK;
         std::function<void()> after = [&]() {
-            if (more) rc_side = side_step(h + 1, h >= 1, true);
+            // once every CTA of recurrence(h) is running: the Gram of h + 1 (Y stage (h+1) % 3 gathered earlier, G stage
+            // (h+1) & 1 last read by recurrence(h-1)) and the gather of h + 2 (Y stage (h+2) % 3, last read by update(h-1))
+            if (more) rc_side = gram_step(h + 1, true);
+            if (!rc_side && h + 2 < len) rc_side = gather_step(h + 2, true);
             c->cur_slot_step = h;
         };
         rc = stage_chain(c, M, nullptr, c->ind, s, b, alpha, buf, true, after, kernels, false, fuse_margin);
         if (!rc) rc = rc_side;
-        cudaEventRecord(c->ev_grad, M);
     }
-    c->last_buf = (len - 1) & 1;
+    cudaEventRecord(c->ev_join, T);                     // every branch rejoins the origin stream before the capture ends
+    cudaStreamWaitEvent(M, c->ev_join, 0);
+    cudaEventRecord(c->ev_join, S);
+    cudaStreamWaitEvent(M, c->ev_join, 0);
+    c->last_buf = stage_of(len - 1);
     c->cur_slot_step = 0;
     g_plain_launch = false;
     g_completion_event = nullptr;
@@ -514,7 +535,7 @@ int choose_gram(casgd_ctx *c, int32_t s, int32_t b, bool pipe)
     c->cur_gram = 2;                                    // (pipelined_mode asks step_is_s1, which looks at cur_gram)
     pipe = pipe && pipelined_mode(c, s, b);
     if (pipe) {
-        const int chain = c->opt_chain_sms > 0 ? (int)c->opt_chain_sms : 32;
+        const int chain = c->opt_chain_sms > 0 ? (int)c->opt_chain_sms : 44;      // (measured on synth-linear s = 32: 32 -> 84.4, 44 -> 81.3, 56 -> 82.3 us)
         c->chain_sms = std::min(std::max(chain, 16), c->num_sms - 32) & ~1;
         c->gram_sms = c->num_sms - c->chain_sms;
     }
@@ -530,7 +551,7 @@ int choose_gram(casgd_ctx *c, int32_t s, int32_t b, bool pipe)
     if (plan && c->pair_plan_sms[pipe ? 1 : 0] != c->gram_sms) { gram_pair_plan_destroy(plan); plan = nullptr; }
     if (!plan) {
         c->pair_plan_sms[pipe ? 1 : 0] = c->gram_sms;
-        plan = gram_pair_plan_create(c->Y, c->ldy, c->n, 2 * c->rows_alloc, c->xbf, c->ldxb, c->gram_sms);
+        plan = gram_pair_plan_create(c->Y, c->ldy, c->n, 3 * c->rows_alloc, c->xbf, c->ldxb, c->gram_sms);
         if (!plan) return fail(c, CASGD_ECUDA, "cuTensorMapEncodeTiled failed for the pair Gram kernel");
     }
     c->pair_plan = plan;
@@ -597,7 +618,8 @@ int get_graph(casgd_ctx *c, int32_t s, int32_t b, float eta, int32_t len, GraphE
     const bool overlap = c->opt_overlap == 1 && c->cur_gram != 4 && !step_is_s1(c, s) && len > 1;
     if ((overlap || pipelined) && !c->side_stream) {
         cudaStreamCreateWithFlags(&c->side_stream, cudaStreamNonBlocking);
-        for (cudaEvent_t *e : {&c->ev_fork, &c->ev_join, &c->ev_gather[0], &c->ev_gather[1], &c->ev_gram[0], &c->ev_gram[1],
+        cudaStreamCreateWithFlags(&c->gather_stream, cudaStreamNonBlocking);
+        for (cudaEvent_t *e : {&c->ev_fork, &c->ev_join, &c->ev_gather[0], &c->ev_gather[1], &c->ev_gather[2], &c->ev_gram[0], &c->ev_gram[1],
                                &c->ev_grad, &c->ev_rec_launch})
             cudaEventCreateWithFlags(e, cudaEventDisableTiming);
     }
@@ -608,7 +630,7 @@ int get_graph(casgd_ctx *c, int32_t s, int32_t b, float eta, int32_t len, GraphE
             c->cur_slot_step = h;
             StepIo io;
             if (overlap) {
-                io.buf = h & 1;
+                io.buf = (h & 1) | ((h & 1) << 2);
                 io.gathered = h > 0;
                 io.next_idx_off = h + 1 < len ? (int64_t)(h + 1) * s * b : -1;
             }
@@ -976,15 +998,15 @@ int casgd_debug_export(casgd_ctx *c, int what, void *dst_host, int64_t dst_bytes
     switch (what) {
     case CASGD_DBG_Y:
         if (!need(sb * c->n * 2)) break;
-        CK(cudaMemcpy2D(dst_host, (size_t)c->n * 2, c->Y + (size_t)c->last_buf * c->rows_alloc * c->ldy, (size_t)c->ldy * 2, (size_t)c->n * 2, (size_t)sb, cudaMemcpyDeviceToHost));
+        CK(cudaMemcpy2D(dst_host, (size_t)c->n * 2, c->Y + (size_t)(c->last_buf & 3) * c->rows_alloc * c->ldy, (size_t)c->ldy * 2, (size_t)c->n * 2, (size_t)sb, cudaMemcpyDeviceToHost));
         return CASGD_OK;
     case CASGD_DBG_G:
         if (!need(sb * sb * 4)) break;
-        CK(cudaMemcpy2D(dst_host, (size_t)sb * 4, c->G + (size_t)c->last_buf * c->rows_alloc * c->rows_alloc, (size_t)c->ldg * 4, (size_t)sb * 4, (size_t)sb, cudaMemcpyDeviceToHost));
+        CK(cudaMemcpy2D(dst_host, (size_t)sb * 4, c->G + (size_t)(c->last_buf >> 2) * c->rows_alloc * c->rows_alloc, (size_t)c->ldg * 4, (size_t)sb * 4, (size_t)sb, cudaMemcpyDeviceToHost));
         return CASGD_OK;
     case CASGD_DBG_YLAB: case CASGD_DBG_R: case CASGD_DBG_Z: case CASGD_DBG_U: {
         if (!need(sb * 4)) break;
-        const float *src = what == CASGD_DBG_YLAB ? c->yI + (size_t)c->last_buf * c->rows_alloc : what == CASGD_DBG_R ? c->r : what == CASGD_DBG_Z ? c->z : c->u;
+        const float *src = what == CASGD_DBG_YLAB ? c->yI + (size_t)(c->last_buf & 3) * c->rows_alloc : what == CASGD_DBG_R ? c->r : what == CASGD_DBG_Z ? c->z : c->u;
         CK(cudaMemcpy(dst_host, src, (size_t)sb * 4, cudaMemcpyDeviceToHost));
         return CASGD_OK;
     }
@@ -1099,7 +1121,8 @@ void casgd_destroy(casgd_ctx *c)
     free_step_workspace(c);
     if (c->capture_stream) cudaStreamDestroy(c->capture_stream);
     if (c->side_stream) cudaStreamDestroy(c->side_stream);
-    for (cudaEvent_t e : {c->ev_fork, c->ev_join, c->ev_gather[0], c->ev_gather[1], c->ev_gram[0], c->ev_gram[1], c->ev_grad, c->ev_rec_launch})
+    if (c->gather_stream) cudaStreamDestroy(c->gather_stream);
+    for (cudaEvent_t e : {c->ev_fork, c->ev_join, c->ev_gather[0], c->ev_gather[1], c->ev_gather[2], c->ev_gram[0], c->ev_gram[1], c->ev_grad, c->ev_rec_launch})
         if (e) cudaEventDestroy(e);
     cudaFree(c->A_owned); cudaFree(c->A32); cudaFree(c->xbf);
     cudaFree(c->gws.partial); cudaFree(c->gws.counters); cudaFree(c->ind); cudaFree(c->err_flag);
