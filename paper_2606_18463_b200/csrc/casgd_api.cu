@@ -689,6 +689,22 @@ int run_steps(casgd_ctx *c, const int32_t *idx, int64_t n_steps, float *x, int32
         CK(cudaGetLastError());
         return CASGD_OK;
     }
+    // s = 1 with wide rows: likewise one persistent launch, of one cluster that splits the columns (s1_cluster.cu)
+    if (s == 1 && c->opt_mini && !c->opt_gram_impl && !c->opt_rec_impl && !c->opt_no_fuse && !c->opt_profile && c->lda % 8 == 0 &&
+        s1_cluster_ok(c->n, c->ldy, b, c->rws.cluster)) {
+        c->cur_slot_step = 0;
+        StageTimer t(c, CASGD_STAGE_GRAM);
+        const int k = launch_s1_cluster(c->stream, c->A, c->lda, c->y, c->m, c->n, c->ldy, idx, n_steps, b, eta / (float)b, c->loss,
+                                        (int)c->opt_split, x, c->xbf, c->ldxb, (int)c->opt_split, c->Y, c->yI, c->r, c->z, c->u,
+                                        c->err_flag);
+        if (k < 0) return fail(c, CASGD_ECUDA, "s1_cluster launch: %s", cudaGetErrorString(cudaGetLastError()));
+        t.done(k);
+        if (c->opt_stamps)
+            launch_stamp_collect(c->stream, c->stamps, kSlotStages, c->stamps + kStampAcc, c->stamps + kStampAcc + 8, c->stamps + kStampRaw);
+        c->last_s = s; c->last_b = b; c->last_buf = 0;
+        CK(cudaGetLastError());
+        return CASGD_OK;
+    }
     rc = choose_gram(c, s, b, false);
     if (rc) return rc;
     rc = ensure_shadow(c, x);
@@ -753,7 +769,7 @@ int casgd_init(casgd_ctx **out, const uint16_t *X_bf16, int64_t ldx, const float
     // opt-in shared-memory sizes and cluster sizes are per-device function attributes: set them on this device
     if (gather_configure() != cudaSuccess || gradient_configure() != cudaSuccess || gram_tc_configure() != cudaSuccess ||
         gram_pair_configure() != cudaSuccess || loss_configure() != cudaSuccess || recurrence_configure() != cudaSuccess ||
-        recurrence_stream_configure() != cudaSuccess || mini_step_configure() != cudaSuccess)
+        recurrence_stream_configure() != cudaSuccess || mini_step_configure() != cudaSuccess || s1_cluster_configure() != cudaSuccess)
         return bail(CASGD_ECUDA);
     c->stream = (cudaStream_t)cuda_stream;
     c->y = y; c->m = m; c->n = n; c->loss = loss;

@@ -232,6 +232,7 @@ cudaError_t loss_configure();
 cudaError_t recurrence_configure();
 cudaError_t recurrence_stream_configure();
 cudaError_t mini_step_configure();
+cudaError_t s1_cluster_configure();
 
 // ------------------------------------------------------------ launch prototypes ---
 // Every launcher enqueues on `st` and returns the number of kernels it launched.
@@ -332,6 +333,12 @@ int launch_mini_steps(cudaStream_t st, const uint16_t *A, int64_t lda, const flo
                       const int32_t *idx, int64_t n_steps, int32_t s, int32_t b, float alpha, int loss, int exact_margin,
                       float *x, uint16_t *xbf, int32_t ldxb, int split, uint16_t *Y, float *yI, float *G, int32_t ldg, float *r,
                       float *z, float *u, int *err_flag);
+
+// s = 1 with wide rows: all iterations of a call in one persistent launch of one column-split cluster (s1_cluster.cu)
+bool s1_cluster_ok(int32_t n, int32_t ldy, int32_t b, int cluster_max);
+int launch_s1_cluster(cudaStream_t st, const uint16_t *A, int64_t lda, const float *y, int64_t m, int32_t n, int32_t ldy,
+                      const int32_t *idx, int64_t n_steps, int32_t b, float alpha, int loss, int exact_margin, float *x,
+                      uint16_t *xbf, int32_t ldxb, int split, uint16_t *Y, float *yI, float *r, float *z, float *u, int *err_flag);
 
 // P > 1 (partition.cu): the payload [r; strict block-lower G] of Alg. 1 line 5, packed / unpacked / summed over ranks
 int64_t payload_count(int32_t s, int32_t b);

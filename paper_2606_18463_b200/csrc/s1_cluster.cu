@@ -1,0 +1,262 @@
+// s1_cluster.cu -- s = 1 (plain mini-batch SGD on BF16 rows with a BF16 shadow, PAPER.md:L99 with Recipe C's storage) for
+// rows too wide for mini_step.cu's one CTA: ALL iterations of a call in one persistent launch of ONE thread-block cluster
+// that splits the COLUMNS (the paper's own block-column idea, L141, across the SMs of a GPC instead of across GPUs).
+//
+// CTA c of C holds columns [c0, c1) of x in shared memory for the whole call and, per iteration,
+//   gathers its column slice of the b sampled rows (Alg. 1 line 2; 16-byte cp.async, the next iteration's slice in flight),
+//   forms the partial margins  p_c[i] = Y[i, c0:c1] . x_hat[c0:c1]  (line 3) and stores them into EVERY CTA of the cluster
+//   (distributed shared memory) -- the one exchange of an iteration, b floats per CTA pair --
+//   after a cluster barrier adds the C partials in rank order (every CTA gets the same bits), applies l' (lines 6-15 at
+//   s = 1), and updates its own columns: x[c0:c1] -= alpha * Y[:, c0:c1]^T u (lines 16-17).
+// No Gram, no recurrence, no global-memory round trip between the margin and the update, no kernel boundary per step:
+// the kernel-per-stage path needs two launches and ~7-11 us per step here, and so does the FP32 baseline.
+#include "common.cuh"
+
+namespace casgd {
+
+namespace {
+
+constexpr int kScThreads = 256, kScWarps = 8;
+constexpr int kScMaxB = 256;
+
+struct S1Params {
+    const uint16_t *A;
+    int64_t lda, m;
+    const float *y;
+    const int32_t *idx;
+    int64_t n_steps;
+    int32_t n, ldy, b, loss, exact_margin, cpc;     // cpc: columns per CTA (a multiple of 8)
+    float alpha;
+    float *x;
+    uint16_t *xbf;
+    int32_t ldxb, split;
+    uint16_t *Y;                                    // exports of the last iteration
+    float *yI, *r, *z, *u;
+    int *err_flag;
+    unsigned long long *stamp;
+};
+
+struct S1Layout {
+    uint32_t x, u, yl[2], idx[2], recv[2], red, Y[2], total;
+    int32_t lds;                                    // row stride of a Y slice in elements
+};
+
+__host__ __device__ inline S1Layout s1_layout(int b, int cpc, int C)
+{
+    S1Layout L;
+    L.lds = cpc + 8;
+    uint32_t o = 0;
+    auto take = [&](uint32_t bytes) { const uint32_t at = o; o += (bytes + 15u) & ~15u; return at; };
+    L.x = take(4u * cpc);
+    L.u = take(4u * b);
+    for (int q = 0; q < 2; ++q) L.yl[q] = take(4u * b);
+    for (int q = 0; q < 2; ++q) L.idx[q] = take(4u * b);
+    for (int q = 0; q < 2; ++q) L.recv[q] = take(4u * (uint32_t)C * b);      // [rank][row]
+    L.red = take(4u * kScWarps * cpc);
+    for (int q = 0; q < 2; ++q) L.Y[q] = take(2u * (uint32_t)b * L.lds);
+    L.total = o;
+    return L;
+}
+
+__device__ __forceinline__ uint32_t sc_rank() { uint32_t v; asm volatile("mov.u32 %0, %%cluster_ctarank;" : "=r"(v)); return v; }
+__device__ __forceinline__ uint32_t sc_size() { uint32_t v; asm volatile("mov.u32 %0, %%cluster_nctarank;" : "=r"(v)); return v; }
+__device__ __forceinline__ void sc_cluster_sync()
+{
+    asm volatile("barrier.cluster.arrive.release.aligned;\n\tbarrier.cluster.wait.acquire.aligned;" ::: "memory");
+}
+
+__global__ void __launch_bounds__(kScThreads, 1)
+s1_cluster_kernel(const S1Params p)
+{
+    extern __shared__ __align__(128) unsigned char sc_smem[];
+    pdl_trigger();
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int C = (int)sc_size(), crank = (int)sc_rank();
+    const int b = p.b, n = p.n, cpc = p.cpc;
+    const S1Layout L = s1_layout(b, cpc, C);
+    const int lds = L.lds;
+    const int c0 = crank * cpc;                          // first column of this CTA
+    const int ncol = max(0, min(cpc, p.ldy - c0));       // columns of the (padded) row this CTA holds
+    const int chunks = ncol >> 3;
+    float *xs = reinterpret_cast<float *>(sc_smem + L.x);
+    float *us = reinterpret_cast<float *>(sc_smem + L.u);
+    float *red = reinterpret_cast<float *>(sc_smem + L.red);
+    const uint32_t smem0 = (uint32_t)__cvta_generic_to_shared(sc_smem);
+
+    for (uint32_t o = L.Y[0] + 16u * tid; o < L.total; o += 16u * kScThreads)
+        *reinterpret_cast<uint4 *>(sc_smem + o) = make_uint4(0u, 0u, 0u, 0u);
+    pdl_wait();
+    stamp_begin(p.stamp);
+    for (int k = tid; k < cpc; k += kScThreads) xs[k] = c0 + k < n ? p.x[c0 + k] : 0.f;
+    for (int q = 0; q < 2; ++q)
+        if (q < p.n_steps)
+            for (int i = tid; i < b; i += kScThreads)
+                reinterpret_cast<int32_t *>(sc_smem + L.idx[q])[i] = p.idx[(int64_t)q * b + i];
+    __syncthreads();
+
+    auto issue_gather = [&](int64_t step) {
+        const int buf = (int)(step & 1);
+        const int32_t *I = reinterpret_cast<const int32_t *>(sc_smem + L.idx[buf]);
+        for (int t = tid; t < b * chunks; t += kScThreads) {
+            const int row = t / chunks, c = t - row * chunks;
+            const int64_t src = I[row];
+            const uint32_t dst = smem0 + L.Y[buf] + 2u * (uint32_t)(row * lds + c * 8);
+            if (src >= 0 && src < p.m) asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(dst), "l"(p.A + src * p.lda + c0 + c * 8) : "memory");
+            else *reinterpret_cast<uint4 *>(sc_smem + (dst - smem0)) = make_uint4(0u, 0u, 0u, 0u);
+        }
+        for (int i = tid; i < b; i += kScThreads) {
+            const int64_t src = I[i];
+            if (src >= 0 && src < p.m) asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"(smem0 + L.yl[buf] + 4u * i), "l"(p.y + src) : "memory");
+            else { reinterpret_cast<float *>(sc_smem + L.yl[buf])[i] = 0.f; if (crank == 0) atomicOr(p.err_flag, 1); }
+        }
+        asm volatile("cp.async.commit_group;" ::: "memory");
+    };
+    if (p.n_steps > 0) issue_gather(0);
+    sc_cluster_sync();                                  // every CTA's receive buffers exist (and are zero) before anyone stores
+
+    int LG = 1;
+    while (LG < chunks && LG < 32) LG <<= 1;            // lanes side by side on a row slice
+    const int rows_per_pass = kScThreads / LG, sub = tid % LG;
+    const uint32_t recv_rank_off = 4u * (uint32_t)(crank * b);
+
+    for (int64_t step = 0; step < p.n_steps; ++step) {
+        const int buf = (int)(step & 1);
+        const bool last = step + 1 == p.n_steps;
+        if (!last) issue_gather(step + 1); else asm volatile("cp.async.commit_group;" ::: "memory");
+        int32_t idx_next = 0;
+        if (step + 2 < p.n_steps && tid < b) idx_next = p.idx[(step + 2) * b + tid];
+        asm volatile("cp.async.wait_group 1;" ::: "memory");
+        __syncthreads();
+        uint16_t *Ys = reinterpret_cast<uint16_t *>(sc_smem + L.Y[buf]);
+        const float *yl = reinterpret_cast<const float *>(sc_smem + L.yl[buf]);
+        if ((n & 7) && c0 + ncol > n) {                 // the CTA that holds the row's last chunk: pad columns are zero
+            for (int i = tid; i < b; i += kScThreads)
+                for (int c = n - c0; c < ncol; ++c) Ys[i * lds + c] = 0;
+            __syncthreads();
+        }
+
+        // ---- partial margins of this column slice, into every CTA's receive buffer
+        for (int i0 = 0; i0 < b; i0 += rows_per_pass) {
+            const int i = i0 + tid / LG;
+            float acc = 0.f;
+            for (int c = sub; c < chunks && i < b; c += LG) {
+                const uint4 v = *reinterpret_cast<const uint4 *>(Ys + i * lds + c * 8);
+                const float *xv = xs + c * 8;
+                float xe[8];
+#pragma unroll
+                for (int e = 0; e < 8; ++e) xe[e] = p.exact_margin ? xv[e] : __bfloat162float(__float2bfloat16_rn(xv[e]));
+                acc = fmaf(bf16lo(v.x), xe[0], acc); acc = fmaf(bf16hi(v.x), xe[1], acc);
+                acc = fmaf(bf16lo(v.y), xe[2], acc); acc = fmaf(bf16hi(v.y), xe[3], acc);
+                acc = fmaf(bf16lo(v.z), xe[4], acc); acc = fmaf(bf16hi(v.z), xe[5], acc);
+                acc = fmaf(bf16lo(v.w), xe[6], acc); acc = fmaf(bf16hi(v.w), xe[7], acc);
+            }
+            for (int o = LG >> 1; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
+            // lane `sub` of the row's group stores to CTA sub, sub + LG, ...: the C remote stores of a row are spread over its lanes
+            if (i < b)
+                for (int dstc = sub; dstc < C; dstc += LG) {
+                    uint32_t remote;
+                    asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(remote) : "r"(smem0 + L.recv[buf] + recv_rank_off + 4u * (uint32_t)i), "r"((uint32_t)dstc));
+                    asm volatile("st.shared::cluster.f32 [%0], %1;" ::"r"(remote), "f"(acc) : "memory");
+                }
+        }
+        sc_cluster_sync();                              // all partials of this iteration have landed everywhere
+
+        // ---- r = sum over ranks (rank order: identical bits in every CTA), u = l'(r, y_I)
+        const float *rv = reinterpret_cast<const float *>(sc_smem + L.recv[buf]);
+        for (int i = tid; i < b; i += kScThreads) {
+            float rr = 0.f;
+            for (int q = 0; q < C; ++q) rr += rv[q * b + i];
+            const float uu = lprime_rt(p.loss, rr, yl[i]);
+            us[i] = uu;
+            if (last && crank == 0) { p.yI[i] = yl[i]; p.r[i] = rr; p.z[i] = rr; p.u[i] = uu; }
+        }
+        __syncthreads();
+
+        // ---- update of this CTA's columns: a warp per group of rows, 8 columns per lane and pass
+        for (int cb = 0; cb < chunks; cb += 32) {
+            const int c = cb + lane;
+            float acc[8] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
+            if (c < chunks)
+                for (int i = warp; i < b; i += kScWarps) {
+                    const uint4 v = *reinterpret_cast<const uint4 *>(Ys + i * lds + c * 8);
+                    const float uu = us[i];
+                    acc[0] = fmaf(bf16lo(v.x), uu, acc[0]); acc[1] = fmaf(bf16hi(v.x), uu, acc[1]);
+                    acc[2] = fmaf(bf16lo(v.y), uu, acc[2]); acc[3] = fmaf(bf16hi(v.y), uu, acc[3]);
+                    acc[4] = fmaf(bf16lo(v.z), uu, acc[4]); acc[5] = fmaf(bf16hi(v.z), uu, acc[5]);
+                    acc[6] = fmaf(bf16lo(v.w), uu, acc[6]); acc[7] = fmaf(bf16hi(v.w), uu, acc[7]);
+                }
+            if (c < chunks) {
+#pragma unroll
+                for (int e = 0; e < 8; ++e) red[warp * cpc + c * 8 + e] = acc[e];
+            }
+        }
+        __syncthreads();
+        for (int k = tid; k < ncol; k += kScThreads) {
+            float g = 0.f;
+#pragma unroll
+            for (int w = 0; w < kScWarps; ++w) g += red[w * cpc + k];
+            xs[k] = fmaf(-p.alpha, g, xs[k]);
+        }
+        if (last)
+            for (int t = tid; t < b * chunks; t += kScThreads) {
+                const int row = t / chunks, c = t - row * chunks;
+                *reinterpret_cast<uint4 *>(p.Y + (int64_t)row * p.ldy + c0 + c * 8) = *reinterpret_cast<const uint4 *>(Ys + row * lds + c * 8);
+            }
+        if (step + 2 < p.n_steps && tid < b) reinterpret_cast<int32_t *>(sc_smem + L.idx[buf])[tid] = idx_next;
+        __syncthreads();
+    }
+    asm volatile("cp.async.wait_group 0;" ::: "memory");
+    for (int k = tid; k < ncol; k += kScThreads)
+        if (c0 + k < n) {
+            p.x[c0 + k] = xs[k];
+            store_shadow(p.xbf, p.split ? p.ldxb : 0, c0 + k, xs[k]);
+        }
+    sc_cluster_sync();                                  // no CTA leaves while another may still store into it
+    stamp_end(p.stamp);
+}
+
+constexpr int kScSmemCap = 200 * 1024;
+
+// cluster size and columns per CTA for a row of ldy (padded) columns
+void s1_cluster_shape(int32_t ldy, int *C, int *cpc)
+{
+    int c = ldy >= 16 * 64 ? 16 : 8;
+    int per = ((ldy + c - 1) / c + 7) & ~7;
+    *C = c;
+    *cpc = per;
+}
+
+}  // namespace
+
+cudaError_t s1_cluster_configure()
+{
+    cudaError_t e = cudaFuncSetAttribute(s1_cluster_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kScSmemCap);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(s1_cluster_kernel, cudaFuncAttributeNonPortableClusterSizeAllowed, 1);
+    return e;
+}
+
+// s = 1, rows of >= 512 bytes that mini_step.cu does not take, b <= 256, everything of a CTA within its shared memory
+bool s1_cluster_ok(int32_t n, int32_t ldy, int32_t b, int cluster_max)
+{
+    if (ldy != ((n + 7) & ~7) || ldy * 2 < 512 || b < 1 || b > kScMaxB) return false;
+    int C, cpc;
+    s1_cluster_shape(ldy, &C, &cpc);
+    if (C > cluster_max) return false;
+    return s1_layout(b, cpc, C).total <= (uint32_t)kScSmemCap;
+}
+
+int launch_s1_cluster(cudaStream_t st, const uint16_t *A, int64_t lda, const float *y, int64_t m, int32_t n, int32_t ldy,
+                      const int32_t *idx, int64_t n_steps, int32_t b, float alpha, int loss, int exact_margin, float *x,
+                      uint16_t *xbf, int32_t ldxb, int split, uint16_t *Y, float *yI, float *r, float *z, float *u, int *err_flag)
+{
+    S1Params p;
+    int C;
+    s1_cluster_shape(ldy, &C, &p.cpc);
+    p.A = A; p.lda = lda; p.m = m; p.y = y; p.idx = idx; p.n_steps = n_steps; p.n = n; p.ldy = ldy; p.b = b; p.loss = loss;
+    p.exact_margin = exact_margin; p.alpha = alpha; p.x = x; p.xbf = xbf; p.ldxb = ldxb; p.split = split;
+    p.Y = Y; p.yI = yI; p.r = r; p.z = z; p.u = u; p.err_flag = err_flag; p.stamp = g_stamp;
+    const S1Layout L = s1_layout(b, p.cpc, C);
+    return launch_pdl(s1_cluster_kernel, dim3(C), dim3(kScThreads), (size_t)L.total, st, C, p) == cudaSuccess ? 1 : -1;
+}
+
+}  // namespace casgd

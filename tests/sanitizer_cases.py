@@ -61,7 +61,9 @@ def cases():
     yield "mini_s4", lambda: step_case("mini_s4", 0, 900, 64, 4, 16, steps=5)
     yield "mini_odd", lambda: step_case("mini_odd", 0, 900, 33, 3, 13, steps=3)
     yield "mini_split", lambda: step_case("mini_split", 0, 900, 64, 4, 16, [(B.OPT_MARGIN_SPLIT, 1)], steps=3)
-    yield "margin_s1", lambda: step_case("margin_s1", 4, 900, 136, 1, 64, eta=0.01)
+    yield "margin_s1", lambda: step_case("margin_s1", 4, 900, 136, 1, 64, [(B.OPT_MINI, 0)], eta=0.01)
+    yield "s1_cluster", lambda: step_case("s1_cluster", 4, 900, 520, 1, 64, steps=5, eta=0.01)
+    yield "s1_cluster_odd", lambda: step_case("s1_cluster_odd", 3, 900, 1001, 1, 40, steps=3)
     for impl, nm in ((1, "cta"), (2, "grid"), (3, "cluster"), (4, "stream")):
         yield f"rec_{nm}", (lambda impl=impl, nm=nm: step_case(f"rec_{nm}", 0, 900, 24, 6, 32, [(B.OPT_RECURRENCE_IMPL, impl)]))
     yield "rec_stream_two_groups", lambda: step_case("rec_stream_two_groups", 0, 1200, 24, 3, 128, [(B.OPT_RECURRENCE_IMPL, 4)])

@@ -391,12 +391,15 @@ def test_next_step_gather_on_the_side_branch_changes_nothing(binding, oracle_mod
 
 
 MINI_SHAPES = [(0, 8192, 64, 4, 16), (1, 20000, 18, 1, 64), (1, 20000, 18, 2, 64), (4, 6000, 512, 1, 16), (0, 4097, 64, 7, 13),
-               (3, 3000, 100, 3, 24), (0, 5000, 33, 2, 5), (4, 6000, 512, 2, 16), (2, 20000, 1024, 1, 8)]
+               (3, 3000, 100, 3, 24), (0, 5000, 33, 2, 5), (4, 6000, 512, 2, 16), (2, 20000, 1024, 1, 8),
+               # s = 1 with wide rows: one launch of one column-split cluster (s1_cluster.cu)
+               (4, 6000, 512, 1, 64), (3, 5000, 2000, 1, 32), (2, 20000, 4096, 1, 128), (3, 5000, 1001, 1, 40)]
 
 
 @pytest.mark.parametrize("ci,m,n,s,b", MINI_SHAPES)
 def test_one_launch_kernel_for_tiny_steps(binding, oracle_mod, ci, m, n, s, b):
-    """mini_step.cu: steps that fit one SM run all iterations of a call in ONE launch. One
+    """mini_step.cu / s1_cluster.cu: steps that fit one SM, and s = 1 steps with wide rows (one
+    column-split cluster), run all iterations of a call in ONE launch. One
     step against oracle O1 element by element (gather bit-exact, G, r, z, u, x); a 9-step call equals 9 single-step
     calls bit for bit and is a single launch; the kernel-per-stage path gives the same iterate up to FP32 summation
     order; an out-of-range index is reported, not read."""
