@@ -88,8 +88,11 @@ int casgd_init(casgd_ctx **out, const uint16_t *X_bf16, int64_t ldx, const float
 int casgd_outer_step(casgd_ctx *c, const int32_t *idx, float *x, int32_t s, int32_t b, float eta);
 
 /* n_steps consecutive outer iterations; step h uses idx[h*s*b .. (h+1)*s*b). ASYNCHRONOUS.
- * Same result as n_steps calls of casgd_outer_step, without per-call launch cost (the step's
- * kernels are replayed from a CUDA graph). An extension of the paper's two CUDA graphs (L278). */
+ * The same iterations as n_steps calls of casgd_outer_step without per-call launch cost: replayed from CUDA graphs of 64
+ * and 8 steps (an extension of the paper's two CUDA graphs, L278) that pipeline consecutive iterations (CASGD_OPT_OVERLAP),
+ * or, for steps small enough, run in ONE persistent launch (CASGD_OPT_MINI). Equal to the single-step calls bit for bit
+ * where the same kernels run (CASGD_OPT_OVERLAP 0 and 1, the one-launch kernels), to FP32 rounding in the pipelined
+ * graphs, whose margin is a kernel of its own. */
 int casgd_outer_steps(casgd_ctx *c, const int32_t *idx, int64_t n_steps, float *x, int32_t s, int32_t b,
                       float eta);
 
@@ -203,17 +206,18 @@ int casgd_debug_export(casgd_ctx *c, int what, void *dst_host, int64_t dst_bytes
  *                              launches of (last end - first start) -- measured INSIDE the CUDA-graph replays that
  *                              casgd_outer_steps runs (unlike CASGD_OPT_PROFILE, which launches directly). Setting the
  *                              option (to 0 or 1) clears the totals.
- *   CASGD_OPT_OVERLAP          how the CUDA graphs of casgd_outer_steps schedule consecutive outer iterations (two Y / G
- *                              stages; results do not depend on the graph length or on single-step calls in a mode):
- *                              0 = kernels strictly in sequence; 1 = a step that has a gather kernel gathers the NEXT
- *                              step's rows (Alg. 1 line 2 of iteration t + 1 needs no result of iteration t) on a side
- *                              branch, beside its own recurrence and update; 2 (default) = pipelined: G(t+1) = Y Y^T
- *                              needs no result of iteration t either, so gather + Gram of iteration t + 1 run on a side
- *                              branch (on all but CASGD_OPT_CHAIN_SMS SMs) beside margin -> recurrence -> update of
- *                              iteration t; the margin r = Y x_bf, which does need x(t+1), is then a kernel of its own
- *                              (CASGD_STAGE_MARGIN) instead of extra B-operand rows of the Gram.
+ *   CASGD_OPT_OVERLAP          how the CUDA graphs of casgd_outer_steps schedule consecutive outer iterations (three Y and
+ *                              two G stages): 0 = kernels strictly in sequence; 1 = a step that has a gather kernel
+ *                              gathers the NEXT step's rows (Alg. 1 line 2 of iteration t + 1 needs no result of
+ *                              iteration t) on a side branch, beside its own recurrence and update; 2 (default) =
+ *                              pipelined: G(t+1) = Y Y^T needs no result of iteration t either, so the Gram of iteration
+ *                              t + 1 runs on a branch of its own (on all but CASGD_OPT_CHAIN_SMS SMs) beside margin ->
+ *                              recurrence -> update of iteration t, and the gather of iteration t + 2 beside that
+ *                              recurrence; the margin r = Y x_bf, which does need x(t+1), is then a kernel of its own
+ *                              (CASGD_STAGE_MARGIN) instead of extra B-operand rows of the Gram. Single-step calls run
+ *                              the sequential kernels on the whole chip in every mode.
  *   CASGD_OPT_CHAIN_SMS        SMs left to the margin / recurrence / update chain in the pipelined schedule (the Gram and
- *                              gather kernels are sized for the rest). 0 (default) = chosen per shape.
+ *                              gather kernels are sized for the rest). 0 (default) = 44.
  *   CASGD_OPT_MARGIN_SPLIT     0 (default) = Recipe C of Table 3: x enters the margin r = Y x as its BF16
  *                              shadow (L231, "two BF16 input conversions"). 1 = the margin sees the FP32 MASTER: rows 1
  *                              and 2 of the shadow buffer carry the BF16 residues of x (hi + lo + lo2 == x exactly), the
@@ -222,12 +226,14 @@ int casgd_debug_export(casgd_ctx *c, int what, void *dst_host, int64_t dst_bytes
  *                              BF16 products are exact in FP32, so G and g are already what FP32 compute gives. Removes
  *                              the x half of Eq. 8's 2 u_16 term (L229) at no extra MMA.
  *   CASGD_OPT_MINI             1 (default) = steps small enough for one SM -- two stages of Y, the packed strict
- *                              block-lower G and the vectors within one CTA's shared memory, a Gram of at most 4M
- *                              multiply-adds: e.g. n = 64, s*b = 64; n = 18, s*b = 256; n = 512, s = 1, b = 64 -- run ALL
- *                              the iterations of a casgd_outer_step(s) call in ONE persistent one-CTA launch (gather with
+ *                              block-lower G and the vectors within one CTA's shared memory, s*b <= 128, a Gram of at
+ *                              most 256K multiply-adds: e.g. n = 64, s*b = 64; at s = 1 a step of <= 16 KB of rows -- run
+ *                              ALL the iterations of a casgd_outer_step(s) call in ONE persistent one-CTA launch (gather with
  *                              the next iteration's rows in flight, mma.sync Gram, recurrence, update, x resident in
  *                              shared memory), unless a kernel was asked for (CASGD_OPT_GRAM_IMPL, _RECURRENCE_IMPL,
- *                              _NO_FUSED_UPDATE, _GRAM_FULL_LOWER, _PROFILE). 0 = always the kernel-per-stage path.
+ *                              _NO_FUSED_UPDATE, _GRAM_FULL_LOWER, _PROFILE); and s = 1 steps with rows of >= 512 bytes run
+ *                              them in one persistent launch of one thread-block cluster that splits the columns
+ *                              (s1_cluster.cu). 0 = always the kernel-per-stage path.
  *   CASGD_OPT_SNAPSHOT         1 = the graphs of casgd_outer_steps copy x aside before their last step (CASGD_DBG_XSNAP):
  *                              test support, one n-element kernel per graph.
  *   CASGD_OPT_LOSS_IMPL        0 = casgd_loss streams A through per-warp cp.async.bulk shared-memory rings

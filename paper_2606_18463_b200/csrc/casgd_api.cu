@@ -438,13 +438,14 @@ int enqueue_step(casgd_ctx *c, cudaStream_t st, const int32_t *idx, const StepPa
     return CASGD_OK;
 }
 
-// CASGD_OPT_OVERLAP = 2: `len` outer iterations as a two-branch graph. G(t+1) = Y(t+1) Y(t+1)^T needs nothing iteration t
-// computes, so the side branch runs gather(t+1) -> Gram(t+1) on gram_sms SMs while the main branch runs
-// margin(t) -> recurrence(t) -> update(t) on the rest; only r(t+1) = Y(t+1) x_bf(t+1) has to wait for the update.
-//   side:  gather(h+1) after update(h-1) (it overwrites stage (h+1) & 1, last read by iteration h-1);
-//          Gram(h+1) once every CTA of recurrence(h) is running (launch-completion event: the cluster needs its 16 SMs
-//          of one GPC before the Gram's persistent CTAs fill the chip)
-//   main:  margin(h) after gather(h); recurrence(h) after Gram(h); update(h)
+// CASGD_OPT_OVERLAP = 2: `len` outer iterations as a three-branch graph. G(t+1) = Y(t+1) Y(t+1)^T and Y(t+2) = A[I(t+2), :]
+// need nothing iteration t computes, so the Gram branch runs Gram(t+1) on gram_sms SMs and the gather branch gather(t+2)
+// on the chain's spare SMs while the main branch runs margin(t) -> recurrence(t) -> update(t); only r(t+1) = Y(t+1)
+// x_bf(t+1) has to wait for the update. Three Y / y_I stages (h % 3), two G stages (h & 1).
+//   Gram branch:    Gram(h+1) after gather(h+1), once every CTA of recurrence(h) is running (launch-completion event: the
+//                   cluster needs its 16 SMs of one GPC before the Gram's persistent CTAs fill the chip)
+//   gather branch:  gather(h+2) once recurrence(h) is running (hence after update(h-1), the last reader of its stage)
+//   main:           margin(h) after gather(h); recurrence(h) after Gram(h); update(h)
 // Side-branch kernels are launched without programmatic serialisation and the recurrence triggers its dependents late:
 // a kernel that becomes resident early only to wait would hold SMs the other branch needs.
 int capture_pipelined(casgd_ctx *c, int32_t s, int32_t b, float eta, int32_t len, int64_t *kernels)
