@@ -390,6 +390,49 @@ def test_next_step_gather_on_the_side_branch_changes_nothing(binding, oracle_mod
         compare_last_step(oracle_mod, cg, ref, y[last], x_before_last, xc, s, b, eta, cfg.loss, binding)
 
 
+def _random_shapes(count, seed):
+    rng = np.random.default_rng(seed)
+    out = []
+    for _ in range(count):
+        loss_cfg = int(rng.choice([0, 2, 4]))               # logistic, linear, Poisson generators
+        n = int(rng.choice([9, 18, 40, 64, 100, 257, 520, 777, 1024, 1500]))
+        b = int(rng.choice([4, 8, 13, 16, 24, 32, 48, 64, 100, 128]))
+        s = int(rng.choice([1, 1, 2, 3, 5, 8, 12]))
+        while s * b > 1200:
+            s = max(1, s // 2)
+        out.append((loss_cfg, n, s, b))
+    return out
+
+
+@pytest.mark.parametrize("ci,n,s,b", _random_shapes(28, 2026))
+def test_default_paths_on_random_shapes(binding, oracle_mod, ci, n, s, b):
+    """Whatever kernels the library picks by itself for a shape (one-launch kernels, narrow / 128-tile / pair Gram, each
+    recurrence kernel, fused or stand-alone update): one step against oracle O1, then an 8-step call (pipelined graph or
+    one launch) whose last step is checked from the bits it started from."""
+    m = 3000
+    cfg = synth.config(ci, m=m, n=n)
+    X_d, y_d, A_bits, y = device_dataset(cfg)
+    rng = np.random.default_rng(n * 1000 + s * 10 + b)
+    idx = rng.integers(0, m, 8 * s * b).astype(np.int32)                   # with duplicates
+    eta = min(cfg.eta, 0.05)
+    x0 = random_x(n, 17, 0.3)
+    with binding.Casgd(X_d, y_d, cfg.loss) as cg:
+        check_step_against_oracle(oracle_mod, cg, A_bits, y, idx[: s * b], x0, s, b, eta, cfg.loss, binding)
+        cg.set_option(binding.OPT_SNAPSHOT, 1)
+        x7 = torch.from_numpy(x0.copy()).cuda()
+        cg.outer_steps(torch.from_numpy(idx[: 7 * s * b]).cuda(), x7, s, b, eta)
+        cg.sync()
+        x8 = torch.from_numpy(x0.copy()).cuda()
+        n0 = cg.launch_count()
+        cg.outer_steps(torch.from_numpy(idx).cuda(), x8, s, b, eta)
+        cg.sync()
+        one_launch = cg.launch_count() - n0 == 1
+        x_before = x7.cpu().numpy().copy() if one_launch else cg.debug(binding.DBG_XSNAP).copy()
+        last = idx[7 * s * b:]
+        ref = oracle_mod.outer_step_gram(A_bits, y, last, x_before.astype(np.float64), s, b, eta, cfg.loss, shadow=True)
+        compare_last_step(oracle_mod, cg, ref, y[last], x_before, x8, s, b, eta, cfg.loss, binding)
+
+
 MINI_SHAPES = [(0, 8192, 64, 4, 16), (1, 20000, 18, 1, 64), (1, 20000, 18, 2, 64), (4, 6000, 512, 1, 16), (0, 4097, 64, 7, 13),
                (3, 3000, 100, 3, 24), (0, 5000, 33, 2, 5), (4, 6000, 512, 2, 16), (2, 20000, 1024, 1, 8),
                # s = 1 with wide rows: one launch of one column-split cluster (s1_cluster.cu)
