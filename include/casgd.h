@@ -132,6 +132,16 @@ int casgd_outer_steps_host(casgd_ctx *c, const int32_t *idx_host, int64_t n_step
  * All ranks must pass the same idx, s, b, eta. ASYNCHRONOUS; errors as for casgd_outer_step. With P = 1 and
  * payload_in = the rank's own payload the three calls equal casgd_outer_step. */
 int64_t casgd_payload_count(int32_t s, int32_t b);          /* -1 for arguments casgd_step_local would reject */
+/* Payload buffers other PROCESSES can read (one process per GPU: each rank's casgd_reduce_peers reads every rank's
+ * payload). casgd_payload_alloc makes a dedicated device allocation of `count` FP32 words (freed by casgd_payload_free);
+ * casgd_ipc_export writes its 64-byte CUDA IPC handle to handle_host, which the caller sends to the other ranks by any
+ * means; casgd_ipc_open maps a peer's handle into this process (a device pointer usable in casgd_reduce_peers' list;
+ * over NVLink when the peer is another GPU), casgd_ipc_close unmaps it. */
+int casgd_payload_alloc(int64_t count, float **payload_dev);
+int casgd_payload_free(float *payload_dev);
+int casgd_ipc_export(const float *payload_dev, void *handle_host /* 64 bytes */);
+int casgd_ipc_open(const void *handle_host /* 64 bytes */, float **peer_payload_dev);
+int casgd_ipc_close(float *peer_payload_dev);
 int casgd_step_local(casgd_ctx *c, const int32_t *idx, const float *x, int32_t s, int32_t b, float *payload_out);
 int casgd_reduce_peers(casgd_ctx *c, const float *const *peer_payloads_host, int32_t P, int32_t s, int32_t b);
 int casgd_step_finish(casgd_ctx *c, float *x, int32_t s, int32_t b, float eta, const float *payload_in);

@@ -31,6 +31,7 @@ EXPORTS = (
     "casgd_sgd_steps_fp32", "casgd_loss", "casgd_invalidate_shadow", "casgd_sync", "casgd_debug_export",
     "casgd_set_option", "casgd_stage_times", "casgd_launch_count", "casgd_last_error", "casgd_destroy",
     "casgd_version", "casgd_payload_count", "casgd_step_local", "casgd_reduce_peers", "casgd_step_finish",
+    "casgd_payload_alloc", "casgd_payload_free", "casgd_ipc_export", "casgd_ipc_open", "casgd_ipc_close",
 )
 
 
@@ -75,6 +76,16 @@ def load() -> ctypes.CDLL:
     lib.casgd_sgd_steps_fp32.argtypes = [vp, vp, i64, vp, i32, f32]
     lib.casgd_payload_count.restype = ctypes.c_int64
     lib.casgd_payload_count.argtypes = [i32, i32]
+    lib.casgd_payload_alloc.restype = ctypes.c_int
+    lib.casgd_payload_alloc.argtypes = [i64, ctypes.POINTER(vp)]
+    lib.casgd_payload_free.restype = ctypes.c_int
+    lib.casgd_payload_free.argtypes = [vp]
+    lib.casgd_ipc_export.restype = ctypes.c_int
+    lib.casgd_ipc_export.argtypes = [vp, ctypes.c_char_p]
+    lib.casgd_ipc_open.restype = ctypes.c_int
+    lib.casgd_ipc_open.argtypes = [ctypes.c_char_p, ctypes.POINTER(vp)]
+    lib.casgd_ipc_close.restype = ctypes.c_int
+    lib.casgd_ipc_close.argtypes = [vp]
     lib.casgd_step_local.restype = ctypes.c_int
     lib.casgd_step_local.argtypes = [vp, vp, vp, i32, i32, vp]
     lib.casgd_reduce_peers.restype = ctypes.c_int
@@ -109,7 +120,57 @@ def version() -> str:
     return load().casgd_version().decode()
 
 
-def _dev_ptr(t: torch.Tensor) -> int:
+class DevBuf:
+    """A device buffer of float32 words that is not a torch tensor: a payload allocated by casgd_payload_alloc (a
+    dedicated allocation, so that its CUDA IPC handle can be exported) or a peer's payload opened from such a handle."""
+    is_cuda = True
+    dtype = torch.float32
+
+    def __init__(self, ptr: int, numel: int, owned: bool):
+        self.ptr, self._numel, self.owned = ptr, numel, owned
+
+    def data_ptr(self) -> int:
+        return self.ptr
+
+    def numel(self) -> int:
+        return self._numel
+
+    def is_contiguous(self) -> bool:
+        return True
+
+    def export_handle(self) -> bytes:
+        h = ctypes.create_string_buffer(64)
+        rc = load().casgd_ipc_export(self.ptr, h)
+        if rc != OK:
+            raise CasgdError(rc, "casgd_ipc_export failed")
+        return h.raw
+
+    def close(self):
+        if self.ptr:
+            (load().casgd_payload_free if self.owned else load().casgd_ipc_close)(self.ptr)
+            self.ptr = 0
+
+
+def payload_alloc(s: int, b: int) -> DevBuf:
+    """casgd_payload_alloc: an IPC-exportable payload buffer on the current device."""
+    p = ctypes.c_void_p()
+    n = payload_count(s, b)
+    rc = load().casgd_payload_alloc(n, ctypes.byref(p))
+    if rc != OK:
+        raise CasgdError(rc, "casgd_payload_alloc failed")
+    return DevBuf(p.value, n, True)
+
+
+def ipc_open(handle: bytes, numel: int) -> DevBuf:
+    """casgd_ipc_open: map another process's payload into this one."""
+    p = ctypes.c_void_p()
+    rc = load().casgd_ipc_open(handle, ctypes.byref(p))
+    if rc != OK:
+        raise CasgdError(rc, "casgd_ipc_open failed")
+    return DevBuf(p.value, numel, False)
+
+
+def _dev_ptr(t) -> int:
     assert t.is_cuda and t.is_contiguous(), "device tensors must be contiguous CUDA tensors"
     return t.data_ptr()
 
@@ -185,7 +246,7 @@ class Casgd:
         assert idx.is_cuda and idx.dtype == torch.int32 and idx.is_contiguous() and idx.numel() == s * b
         assert x.is_cuda and x.dtype == torch.float32 and x.is_contiguous() and x.numel() == self.n
         assert payload.is_cuda and payload.dtype == torch.float32 and payload.is_contiguous()
-        assert payload.numel() == payload_count(s, b)
+        assert payload.numel() == payload_count(s, b)      # (a torch tensor or a DevBuf)
         self._check(self._lib.casgd_step_local(self._ctx, _dev_ptr(idx), _dev_ptr(x), s, b, _dev_ptr(payload)))
         self._last_sb = s * b
 

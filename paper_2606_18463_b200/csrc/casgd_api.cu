@@ -896,6 +896,42 @@ int64_t casgd_payload_count(int32_t s, int32_t b)
     return payload_count(s, b);
 }
 
+int casgd_payload_alloc(int64_t count, float **payload_dev)
+{
+    if (!payload_dev || count < 1) return CASGD_EINVAL;
+    *payload_dev = nullptr;
+    const cudaError_t e = cudaMalloc(payload_dev, sizeof(float) * (size_t)count);
+    return e == cudaSuccess ? CASGD_OK : e == cudaErrorMemoryAllocation ? CASGD_ENOMEM : CASGD_ECUDA;
+}
+
+int casgd_payload_free(float *payload_dev) { return cudaFree(payload_dev) == cudaSuccess ? CASGD_OK : CASGD_ECUDA; }
+
+int casgd_ipc_export(const float *payload_dev, void *handle_host)
+{
+    static_assert(sizeof(cudaIpcMemHandle_t) == 64, "CUDA IPC handles are 64 bytes");
+    if (!payload_dev || !handle_host) return CASGD_EINVAL;
+    cudaIpcMemHandle_t h;
+    if (cudaIpcGetMemHandle(&h, const_cast<float *>(payload_dev)) != cudaSuccess) return CASGD_ECUDA;
+    memcpy(handle_host, &h, sizeof h);
+    return CASGD_OK;
+}
+
+int casgd_ipc_open(const void *handle_host, float **peer_payload_dev)
+{
+    if (!handle_host || !peer_payload_dev) return CASGD_EINVAL;
+    cudaIpcMemHandle_t h;
+    memcpy(&h, handle_host, sizeof h);
+    void *p = nullptr;
+    if (cudaIpcOpenMemHandle(&p, h, cudaIpcMemLazyEnablePeerAccess) != cudaSuccess) return CASGD_ECUDA;
+    *peer_payload_dev = static_cast<float *>(p);
+    return CASGD_OK;
+}
+
+int casgd_ipc_close(float *peer_payload_dev)
+{
+    return cudaIpcCloseMemHandle(peer_payload_dev) == cudaSuccess ? CASGD_OK : CASGD_ECUDA;
+}
+
 int casgd_step_local(casgd_ctx *c, const int32_t *idx, const float *x, int32_t s, int32_t b, float *payload_out)
 {
     int rc = check_step_args(c, idx, x, 1, s, b, 0.f);

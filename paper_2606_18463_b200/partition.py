@@ -97,3 +97,47 @@ class PartitionedCasgd:
             # have been created on that stream (binding.Casgd's default)
             dist.all_reduce(payload, op=dist.ReduceOp.SUM, group=self.group)
         self.backend.finish(x_slab, s, b, eta, payload)
+
+
+class PeerPartitionedCasgd:
+    """The same outer iteration with the library's OWN sum over ranks instead of a collective call: every rank's payload
+    lives in a dedicated device allocation whose CUDA IPC handle the ranks exchange once (through `group`, any backend);
+    per iteration each rank's `casgd_reduce_peers` kernel reads all P payloads -- peer memory over NVLink when the ranks
+    sit on different GPUs -- and writes the rank-ordered sum straight into its recurrence's G and r.
+
+    Ordering between the ranks is kept on the host here, the simplest correct protocol: a barrier after every rank's
+    local half has finished on its stream (payloads complete), and another after every rank's reduce has finished
+    (payloads may be overwritten). Device-side flags would remove both host round trips; they need one GPU per rank to
+    be measured, which this build's test box does not have."""
+
+    def __init__(self, backend: "CudaSlab", group):
+        import torch.distributed as dist
+        from . import binding
+        self.backend, self.group, self._dist, self._binding = backend, group, dist, binding
+        self._bufs = {}
+
+    def _setup(self, s, b):
+        mine = self._binding.payload_alloc(s, b)
+        handles = [None] * self._dist.get_world_size(self.group)
+        self._dist.all_gather_object(handles, mine.export_handle(), group=self.group)
+        rank = self._dist.get_rank(self.group)
+        peers = [mine if q == rank else self._binding.ipc_open(h, mine.numel()) for q, h in enumerate(handles)]
+        self._bufs[(s, b)] = (mine, peers)
+        return mine, peers
+
+    def outer_step(self, idx, x_slab, s: int, b: int, eta: float):
+        mine, peers = self._bufs.get((s, b)) or self._setup(s, b)
+        cg = self.backend.cg
+        cg.step_local(idx, x_slab, s, b, mine)
+        cg.sync()
+        self._dist.barrier(group=self.group)            # every rank's payload is complete
+        cg.reduce_peers(peers, s, b)
+        cg.step_finish(x_slab, s, b, eta, None)
+        cg.sync()
+        self._dist.barrier(group=self.group)            # every rank has read every payload
+
+    def close(self):
+        for mine, peers in self._bufs.values():
+            for p in peers:
+                p.close()
+        self._bufs = {}

@@ -145,3 +145,68 @@ def test_partitioned_step_over_nccl_world_of_one(binding, oracle_mod):
         back.close()
     finally:
         dist.destroy_process_group()
+
+
+def _peer_worker(rank, world, port, out):
+    import torch.distributed as dist
+    os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port), RANK=str(rank), WORLD_SIZE=str(world))
+    dist.init_process_group("gloo", rank=rank, world_size=world)       # control plane only: handles and barriers
+    try:
+        import oracle
+        from paper_2606_18463_b200 import binding
+        torch.cuda.set_device(0)
+        cfg = synth.config(4, m=6000, n=520)
+        X_d, y_d, A_bits, y = device_dataset(cfg)
+        s, b = 6, 64
+        idx = synth.epoch_indices(cfg, 42, 0)[: 2 * s * b].copy()
+        x0 = random_x(cfg.n, 21, 0.4)
+        sl = partition.column_slab(cfg.n, rank, world)
+        back = partition.CudaSlab(X_d[:, sl], y_d, cfg.loss)
+        step = partition.PeerPartitionedCasgd(back, dist.group.WORLD)
+        x = torch.from_numpy(x0[sl].copy()).cuda()
+        xs = []
+        for h in range(2):
+            step.outer_step(torch.from_numpy(idx[h * s * b:(h + 1) * s * b]).cuda(), x, s, b, cfg.eta)
+            xs.append(x.cpu().numpy().copy())
+        u_bits = back.cg.debug(binding.DBG_U).tobytes()
+        out.put((rank, sl.start, sl.stop, xs, u_bits))
+        dist.barrier()
+        step.close()
+        back.close()
+    finally:
+        dist.destroy_process_group()
+
+
+def test_two_processes_sum_their_payloads_through_peer_memory(oracle_mod):
+    """Two PROCESSES (one column slab each, both on this box's one GPU, gloo for the control plane): the payloads are
+    dedicated allocations shared by CUDA IPC handles, each process's casgd_reduce_peers kernel reads both and writes
+    the rank-ordered sum into its own G and r -- the library's own one-shot all-reduce, no NCCL. Two outer iterations
+    against oracle O1 on the unpartitioned matrix; both processes end with identical u bits."""
+    import torch.multiprocessing as mp
+    ctx = mp.get_context("spawn")
+    out = ctx.Queue()
+    with socket.socket() as sk:
+        sk.bind(("127.0.0.1", 0))
+        port = sk.getsockname()[1]
+    procs = [ctx.Process(target=_peer_worker, args=(r, 2, port, out)) for r in range(2)]
+    for p in procs:
+        p.start()
+    res = sorted(out.get(timeout=300) for _ in procs)
+    for p in procs:
+        p.join(timeout=120)
+        assert p.exitcode == 0
+    cfg = synth.config(4, m=6000, n=520)
+    ds = synth.make_dataset(cfg, seed=42, device="cpu")
+    A_bits, y = ds.X_bits_numpy(), ds.y_numpy()
+    s, b = 6, 64
+    idx = synth.epoch_indices(cfg, 42, 0)[: 2 * s * b].copy()
+    x_prev = random_x(cfg.n, 21, 0.4)
+    assert res[0][1] == 0 and res[0][2] == res[1][1] and res[1][2] == cfg.n
+    for h in range(2):
+        ref = oracle_mod.outer_step_gram(A_bits, y, idx[h * s * b:(h + 1) * s * b], x_prev.astype(np.float64), s, b, cfg.eta,
+                                         cfg.loss, shadow=True)
+        got = np.concatenate([r[3][h] for r in res])
+        rel = np.linalg.norm(got.astype(np.float64) - ref.x_out) / np.linalg.norm(ref.x_out)
+        assert rel <= TOL_X, f"iteration {h}: relative error {rel:.3g}"
+        x_prev = got                                     # the next iteration starts from the library's own FP32 bits
+    assert res[0][4] == res[1][4]                        # rank-ordered sum: identical u on both ranks
