@@ -433,6 +433,44 @@ def test_default_paths_on_random_shapes(binding, oracle_mod, ci, n, s, b):
         compare_last_step(oracle_mod, cg, ref, y[last], x_before, x8, s, b, eta, cfg.loss, binding)
 
 
+def test_pipelined_graphs_of_two_contexts_and_shapes_interleaved(binding):
+    """Robustness of the graph plumbing: two contexts on one device, each replaying pipelined graphs of two different
+    (s, b) in alternation, with a workspace growth in between -- every call must give what the same call gives on a fresh
+    context in the sequential schedule (to FP32 rounding: the pipelined margin is a kernel of its own)."""
+    cfgs = [synth.config(4, m=6000, n=512), synth.config(3, m=5000, n=1000)]
+    data = [device_dataset(c) for c in cfgs]
+    shapes = [(3, 64), (8, 32), (5, 64), (12, 32)]                 # the last one grows the workspaces
+    steps = 16
+    rng = np.random.default_rng(8)
+    idxs = {(ci, sh): torch.from_numpy(rng.integers(0, cfgs[ci].m, steps * sh[0] * sh[1]).astype(np.int32)).cuda()
+            for ci in range(2) for sh in shapes}
+
+    def run(schedule, interleaved):
+        out = {}
+        ctxs = [binding.Casgd(d[0], d[1], c.loss) for d, c in zip(data, cfgs)]
+        try:
+            for cg in ctxs:
+                cg.set_option(binding.OPT_OVERLAP, schedule)
+            order = [(ci, sh) for sh in shapes for ci in range(2)] if interleaved else [(ci, sh) for ci in range(2) for sh in shapes]
+            for rep in range(2):
+                for ci, sh in order:
+                    x = torch.full((cfgs[ci].n,), 0.01 * (rep + 1), device="cuda")
+                    ctxs[ci].outer_steps(idxs[(ci, sh)], x, sh[0], sh[1], min(cfgs[ci].eta, 0.02))
+                    out[(ci, sh, rep)] = x
+            for cg in ctxs:
+                cg.sync()
+        finally:
+            for cg in ctxs:
+                cg.close()
+        return out
+
+    ref = run(0, False)
+    got = run(2, True)
+    for k in ref:
+        assert torch.isfinite(got[k]).all()
+        assert torch.linalg.norm(got[k] - ref[k]) <= 2e-5 * torch.linalg.norm(ref[k]), k
+
+
 MINI_SHAPES = [(0, 8192, 64, 4, 16), (1, 20000, 18, 1, 64), (1, 20000, 18, 2, 64), (4, 6000, 512, 1, 16), (0, 4097, 64, 7, 13),
                (3, 3000, 100, 3, 24), (0, 5000, 33, 2, 5), (4, 6000, 512, 2, 16), (2, 20000, 1024, 1, 8),
                # s = 1 with wide rows: one launch of one column-split cluster (s1_cluster.cu)
