@@ -237,13 +237,17 @@ int casgd_debug_export(casgd_ctx *c, int what, void *dst_host, int64_t dst_bytes
  *                              the x half of Eq. 8's 2 u_16 term (L229) at no extra MMA.
  *   CASGD_OPT_MINI             1 (default) = steps small enough for one SM -- two stages of Y, the packed strict
  *                              block-lower G and the vectors within one CTA's shared memory, s*b <= 128, a Gram of at
- *                              most 256K multiply-adds: e.g. n = 64, s*b = 64; at s = 1 a step of <= 16 KB of rows -- run
- *                              ALL the iterations of a casgd_outer_step(s) call in ONE persistent one-CTA launch (gather with
- *                              the next iteration's rows in flight, mma.sync Gram, recurrence, update, x resident in
- *                              shared memory), unless a kernel was asked for (CASGD_OPT_GRAM_IMPL, _RECURRENCE_IMPL,
- *                              _NO_FUSED_UPDATE, _GRAM_FULL_LOWER, _PROFILE); and s = 1 steps with rows of >= 512 bytes run
- *                              them in one persistent launch of one thread-block cluster that splits the columns
- *                              (s1_cluster.cu). 0 = always the kernel-per-stage path.
+ *                              most 200K multiply-adds: e.g. n = 64, s*b = 64; at s = 1 a step of <= 32 KB of rows (any
+ *                              size for rows of <= 128 bytes), s*b <= 512 -- run ALL the iterations of a
+ *                              casgd_outer_step(s) call in ONE persistent one-CTA launch (gather with the next
+ *                              iteration's rows in flight, mma.sync Gram, recurrence, update, x resident in shared
+ *                              memory), unless a kernel was asked for (CASGD_OPT_GRAM_IMPL, _RECURRENCE_IMPL,
+ *                              _NO_FUSED_UPDATE, _GRAM_FULL_LOWER, _PROFILE); and s = 1 steps of more than 4 KB with
+ *                              rows of >= 128 bytes, b <= 256, run them in one persistent launch of one thread-block
+ *                              cluster that splits the columns
+ *                              (s1_cluster.cu). 0 = always the kernel-per-stage path. 2 = the one-CTA launch whenever the
+ *                              step FITS it (s*b <= 512, n <= 2048, shared memory), measured crossovers ignored: for
+ *                              tests and for measuring those crossovers.
  *   CASGD_OPT_SNAPSHOT         1 = the graphs of casgd_outer_steps copy x aside before their last step (CASGD_DBG_XSNAP):
  *                              test support, one n-element kernel per graph.
  *   CASGD_OPT_LOSS_IMPL        0 = casgd_loss streams A through per-warp cp.async.bulk shared-memory rings

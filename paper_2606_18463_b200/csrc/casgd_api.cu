@@ -675,7 +675,9 @@ int run_steps(casgd_ctx *c, const int32_t *idx, int64_t n_steps, float *x, int32
     if (rc) return rc;
     // tiny steps: all n_steps iterations in ONE persistent one-CTA launch (mini_step.cu) -- unless a kernel was asked for
     if (c->opt_mini && !c->opt_gram_impl && !c->opt_rec_impl && !c->opt_no_fuse && !c->opt_full_lower && !c->opt_profile &&
-        c->lda % 8 == 0 && mini_step_ok(c->n, c->ldy, s, b)) {
+        c->lda % 8 == 0 && mini_step_ok(c->n, c->ldy, s, b, c->opt_mini == 2) &&
+        !(s == 1 && c->opt_mini == 1 && (int64_t)b * c->ldy * 2 > 4096 &&
+          s1_cluster_ok(c->n, c->ldy, b, c->rws.cluster))) {    // (s = 1 beyond 4 KB of rows: the cluster, below)
         c->cur_slot_step = 0;
         StageTimer t(c, CASGD_STAGE_GRAM);
         const int k = launch_mini_steps(c->stream, c->A, c->lda, c->y, c->m, c->n, c->ldy, idx, n_steps, s, b, eta / (float)b, c->loss,
@@ -690,7 +692,7 @@ int run_steps(casgd_ctx *c, const int32_t *idx, int64_t n_steps, float *x, int32
         CK(cudaGetLastError());
         return CASGD_OK;
     }
-    // s = 1 with wide rows: likewise one persistent launch, of one cluster that splits the columns (s1_cluster.cu)
+    // s = 1 with rows of >= 128 bytes: likewise one persistent launch, of one cluster that splits the columns (s1_cluster.cu)
     if (s == 1 && c->opt_mini && !c->opt_gram_impl && !c->opt_rec_impl && !c->opt_no_fuse && !c->opt_profile && c->lda % 8 == 0 &&
         s1_cluster_ok(c->n, c->ldy, b, c->rws.cluster)) {
         c->cur_slot_step = 0;
@@ -703,6 +705,7 @@ int run_steps(casgd_ctx *c, const int32_t *idx, int64_t n_steps, float *x, int32
         if (c->opt_stamps)
             launch_stamp_collect(c->stream, c->stamps, kSlotStages, c->stamps + kStampAcc, c->stamps + kStampAcc + 8, c->stamps + kStampRaw);
         c->last_s = s; c->last_b = b; c->last_buf = 0;
+        c->shadow_of = x; c->shadow_valid = true;
         CK(cudaGetLastError());
         return CASGD_OK;
     }
@@ -1119,7 +1122,7 @@ int casgd_set_option(casgd_ctx *c, int option, int64_t value)
         if (value < 0 || value > 2) return fail(c, CASGD_EINVAL, "CASGD_OPT_OVERLAP must be 0, 1 or 2");
         c->opt_overlap = value; break;
     case CASGD_OPT_MARGIN_SPLIT: c->opt_split = value != 0; break;
-    case CASGD_OPT_MINI: c->opt_mini = value != 0; break;
+    case CASGD_OPT_MINI: c->opt_mini = value < 0 ? 0 : value > 2 ? 2 : value; break;
     case CASGD_OPT_SNAPSHOT: c->opt_snapshot = value != 0; break;
     case CASGD_OPT_CHAIN_SMS:
         if (value < 0 || value > 1024) return fail(c, CASGD_EINVAL, "CASGD_OPT_CHAIN_SMS must be in [0, 1024]");

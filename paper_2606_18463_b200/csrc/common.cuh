@@ -328,7 +328,7 @@ int launch_stamp_collect(cudaStream_t st, unsigned long long *slots, int nslots,
                          unsigned long long *count, unsigned long long *raw_copy);
 
 // Whole outer iterations in one persistent one-CTA launch, for tiny steps (mini_step.cu)
-bool mini_step_ok(int32_t n, int32_t ldy, int32_t s, int32_t b);
+bool mini_step_ok(int32_t n, int32_t ldy, int32_t s, int32_t b, bool any_fit);
 int launch_mini_steps(cudaStream_t st, const uint16_t *A, int64_t lda, const float *y, int64_t m, int32_t n, int32_t ldy,
                       const int32_t *idx, int64_t n_steps, int32_t s, int32_t b, float alpha, int loss, int exact_margin,
                       float *x, uint16_t *xbf, int32_t ldxb, int split, uint16_t *Y, float *yI, float *G, int32_t ldg, float *r,

@@ -21,8 +21,8 @@ namespace casgd {
 
 namespace {
 
-constexpr int kMsThreads = 512, kMsWarps = 16;
-constexpr int kMsRedFloats = 4096;                      // gradient partial sums: <= 16 parts x ldy, ldy <= 2048 / ... (see layout)
+constexpr int kMsMaxThreads = 512, kMsMaxWarps = 16;    // the launch picks 128 .. 512 threads
+constexpr int kMsRedFloats = 4096;                      // gradient partial sums: at most 16 parts x ldy floats
 
 struct MiniParams {
     const uint16_t *A;
@@ -30,7 +30,7 @@ struct MiniParams {
     const float *y;
     const int32_t *idx;                 // n_steps * s*b indices
     int64_t n_steps;
-    int32_t n, ldy, s, b, loss, exact_margin, stages;
+    int32_t n, ldy, s, b, exact_margin;
     float alpha;
     float *x;
     uint16_t *xbf;
@@ -42,13 +42,14 @@ struct MiniParams {
     unsigned long long *stamp;
 };
 
-constexpr int kMsMaxStages = 4;
-struct MiniLayout {                     // byte offsets into dynamic shared memory
-    uint32_t x, r, z, u, yl[kMsMaxStages], idx[kMsMaxStages], gl, red, Y[kMsMaxStages], total;
+// Byte offsets into dynamic shared memory. Two stages of Y, of the labels and of the indices: stage q at base + q * stride
+// (scalars, not arrays indexed at run time: those end up in local memory, on every access of every phase).
+struct MiniLayout {
+    uint32_t x, r, z, u, yl, yl_stride, idx, idx_stride, gl, red, Y, Y_stride, total;
     int32_t ldys, sbp;                  // row stride of a Y stage in elements (16-byte multiple, staggered banks); rows incl. padding
 };
 
-__host__ __device__ inline MiniLayout mini_layout(int n, int s, int b, int ns)
+__host__ __device__ inline MiniLayout mini_layout(int n, int s, int b)
 {
     MiniLayout L;
     const int sb = s * b;
@@ -58,11 +59,12 @@ __host__ __device__ inline MiniLayout mini_layout(int n, int s, int b, int ns)
     auto take = [&](uint32_t bytes) { const uint32_t at = o; o += (bytes + 15u) & ~15u; return at; };
     L.x = take(4u * (uint32_t)n);
     L.r = take(4u * sb); L.z = take(4u * sb); L.u = take(4u * sb);
-    for (int q = 0; q < ns; ++q) L.yl[q] = take(4u * sb);
-    for (int q = 0; q < ns; ++q) L.idx[q] = take(4u * sb);
+    L.yl_stride = (4u * sb + 15u) & ~15u;  L.yl = take(2u * L.yl_stride);
+    L.idx_stride = L.yl_stride;            L.idx = take(2u * L.idx_stride);
     L.gl = take(2u * (uint32_t)b * b * s * (s - 1));     // b^2 s (s-1) / 2 floats
     L.red = take(4u * kMsRedFloats);
-    for (int q = 0; q < ns; ++q) L.Y[q] = take(2u * (uint32_t)L.sbp * L.ldys);
+    L.Y_stride = (2u * (uint32_t)L.sbp * L.ldys + 15u) & ~15u;
+    L.Y = take(2u * L.Y_stride);
     L.total = o;
     return L;
 }
@@ -83,15 +85,27 @@ __device__ __forceinline__ void mma_bf16_16816(float (&c)[4], const uint32_t (&a
 }
 __device__ __forceinline__ float bf16_round(float v) { return __bfloat162float(__float2bfloat16_rn(v)); }
 
-__global__ void __launch_bounds__(kMsThreads, 1)
+#ifdef CASGD_MINI_TRACE
+__device__ long long g_mini_trace[64];
+#define MT(i) do { if (tid == 0 && step == 8) g_mini_trace[i] = clock64(); } while (0)
+#else
+#define MT(i) do { } while (0)
+#endif
+
+// The kernel is kept SMALL on purpose: every phase runs once per iteration, so its instructions are fetched once per
+// iteration; a first version (runtime loss switch inlined twice, arrays of stage offsets in local memory, divisions by
+// run-time values in the copy loops: 4096 instructions = 64 KB, twice the instruction cache) spent 12 000 cycles on an
+// iteration that needs a few hundred FMAs. One instantiation per loss; outer loops not unrolled; power-of-two lane groups.
+template <int LOSS>
+__global__ void __launch_bounds__(kMsMaxThreads, 1)
 mini_step_kernel(const MiniParams p)
 {
     extern __shared__ __align__(128) unsigned char ms_smem[];
     pdl_trigger();
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int nthr = blockDim.x, nwarp = nthr >> 5;
     const int s = p.s, b = p.b, sb = s * b, n = p.n, ldy = p.ldy;
-    const int NS = p.stages, D = NS - 1;              // Y stages; rows are gathered D iterations ahead
-    const MiniLayout L = mini_layout(n, s, b, NS);
+    const MiniLayout L = mini_layout(n, s, b);
     const int ldys = L.ldys;
     float *xs = reinterpret_cast<float *>(ms_smem + L.x);
     float *rs = reinterpret_cast<float *>(ms_smem + L.r);
@@ -102,102 +116,118 @@ mini_step_kernel(const MiniParams p)
     const uint32_t smem0 = (uint32_t)__cvta_generic_to_shared(ms_smem);
 
     // both Y stages start as zeros: the K padding (columns n .. ldys) and the row padding (rows sb .. sbp) stay zero
-    for (uint32_t o = L.Y[0] + 16u * tid; o < L.total; o += 16u * kMsThreads)
+#pragma unroll 1
+    for (uint32_t o = L.Y + 16u * tid; o < L.total; o += 16u * nthr)
         *reinterpret_cast<uint4 *>(ms_smem + o) = make_uint4(0u, 0u, 0u, 0u);
     pdl_wait();                                         // x and the index buffer come from earlier work on the stream
     stamp_begin(p.stamp);
-    for (int k = tid; k < n; k += kMsThreads) xs[k] = p.x[k];
-    for (int q = 0; q < NS; ++q)
-        if (q < p.n_steps)
-            for (int i = tid; i < sb; i += kMsThreads)
-                reinterpret_cast<int32_t *>(ms_smem + L.idx[q])[i] = p.idx[(int64_t)q * sb + i];
+#pragma unroll 1
+    for (int k = tid; k < n; k += nthr) xs[k] = p.x[k];
+    if (tid < sb) {                                     // (sb <= 512: one index per thread and stage)
+        reinterpret_cast<int32_t *>(ms_smem + L.idx)[tid] = p.idx[tid];
+        if (p.n_steps > 1) reinterpret_cast<int32_t *>(ms_smem + L.idx + L.idx_stride)[tid] = p.idx[sb + tid];
+    }
     __syncthreads();
 
+    // gather (line 2): 16-byte cp.async pieces, CH lanes side by side on a row. (One cp.async.bulk per row on an
+    // mbarrier, issued by the row's thread, measured slower -- n = 18, b = 64: 2.4 against 1.7 us per iteration, also
+    // with four stages and rows three iterations ahead: the few issuing threads become the critical path of the CTA.)
     const int chunks = ldy >> 3;                        // 16-byte pieces of a gathered row
+    int CH = 1, chs = 0;                                // lanes side by side on a row: a power of two >= chunks
+    while (CH < chunks) { CH <<= 1; ++chs; }
+    const int csub = tid & (CH - 1), crow = tid >> chs, crows = nthr >> chs;
     auto issue_gather = [&](int64_t step) {
-        const int buf = (int)(step % NS);
-        const int32_t *I = reinterpret_cast<const int32_t *>(ms_smem + L.idx[buf]);
-        for (int t = tid; t < sb * chunks; t += kMsThreads) {
-            const int row = t / chunks, c = t - row * chunks;
-            const int64_t src = I[row];
-            const uint32_t dst = smem0 + L.Y[buf] + 2u * (uint32_t)(row * ldys + c * 8);
-            if (src >= 0 && src < p.m) cp_async16_ms(dst, p.A + src * p.lda + c * 8);
-            else *reinterpret_cast<uint4 *>(ms_smem + (dst - smem0)) = make_uint4(0u, 0u, 0u, 0u);
+        const uint32_t q = (uint32_t)(step & 1);
+        const int32_t *I = reinterpret_cast<const int32_t *>(ms_smem + L.idx + q * L.idx_stride);
+        const uint32_t ybase = L.Y + q * L.Y_stride;
+        if (csub < chunks) {
+#pragma unroll 1
+            for (int row = crow; row < sb; row += crows) {
+                const int64_t src = I[row];
+                const uint32_t off = ybase + 2u * (uint32_t)(row * ldys + csub * 8);
+                if (src >= 0 && src < p.m) cp_async16_ms(smem0 + off, p.A + src * p.lda + csub * 8);
+                else *reinterpret_cast<uint4 *>(ms_smem + off) = make_uint4(0u, 0u, 0u, 0u);
+            }
         }
-        for (int i = tid; i < sb; i += kMsThreads) {
-            const int64_t src = I[i];
-            if (src >= 0 && src < p.m) cp_async4_ms(smem0 + L.yl[buf] + 4u * i, p.y + src);
-            else { reinterpret_cast<float *>(ms_smem + L.yl[buf])[i] = 0.f; atomicOr(p.err_flag, 1); }
+        if (tid < sb) {
+            const int64_t src = I[tid];
+            const uint32_t off = L.yl + q * L.yl_stride + 4u * (uint32_t)tid;
+            if (src >= 0 && src < p.m) cp_async4_ms(smem0 + off, p.y + src);
+            else { *reinterpret_cast<float *>(ms_smem + off) = 0.f; atomicOr(p.err_flag, 1); }
         }
         asm volatile("cp.async.commit_group;" ::: "memory");
     };
-    for (int q = 0; q < D; ++q) {
-        if (q < p.n_steps) issue_gather(q); else asm volatile("cp.async.commit_group;" ::: "memory");
-    }
+    if (p.n_steps > 0) issue_gather(0);
 
+    int LG = 1;                                         // margin: lanes side by side on a row (<= 32)
+    while (LG < chunks && LG < 32) LG <<= 1;
+    const int msub = tid & (LG - 1), mrows = nthr / LG;
+
+#pragma unroll 1
     for (int64_t step = 0; step < p.n_steps; ++step) {
-        const int buf = (int)(step % NS);
+        const uint32_t q = (uint32_t)(step & 1);
         const bool last = step + 1 == p.n_steps;
-        // rows of iteration step + D; indices of the one after that (stored at the bottom of this iteration)
-        if (step + D < p.n_steps) issue_gather(step + D); else asm volatile("cp.async.commit_group;" ::: "memory");
-        int32_t idx_next[4] = {0, 0, 0, 0};             // sb <= 4 * 512
-        if (step + NS < p.n_steps)
-#pragma unroll
-            for (int q = 0; q < 4; ++q)
-                if (tid + q * kMsThreads < sb) idx_next[q] = p.idx[(step + NS) * sb + tid + q * kMsThreads];
-        if (D == 1) asm volatile("cp.async.wait_group 1;" ::: "memory");
-        else asm volatile("cp.async.wait_group 3;" ::: "memory");
+        MT(0);
+        // rows of the next iteration; indices of the one after it (stored at the bottom of this iteration)
+        if (!last) issue_gather(step + 1); else asm volatile("cp.async.commit_group;" ::: "memory");
+        MT(8);
+        int32_t idx_next = 0;
+        if (step + 2 < p.n_steps && tid < sb) idx_next = p.idx[(step + 2) * sb + tid];
+        asm volatile("cp.async.wait_group 1;" ::: "memory");
+        MT(1);
         __syncthreads();                                // this iteration's rows and labels are in shared memory
-        uint16_t *Ys = reinterpret_cast<uint16_t *>(ms_smem + L.Y[buf]);
-        const float *yl = reinterpret_cast<const float *>(ms_smem + L.yl[buf]);
+        uint16_t *Ys = reinterpret_cast<uint16_t *>(ms_smem + L.Y + q * L.Y_stride);
+        const float *yl = reinterpret_cast<const float *>(ms_smem + L.yl + q * L.yl_stride);
         if (n & 7) {                                    // A's own padding may hold anything: Y's pad columns are zero
-            for (int i = tid; i < sb; i += kMsThreads)
-                for (int c = n; c < ldy; ++c) Ys[i * ldys + c] = 0;
+            if (tid < sb)
+                for (int c = n; c < ldy; ++c) Ys[tid * ldys + c] = 0;
             __syncthreads();
         }
 
+        MT(2);
         // ---- margin (line 3): a group of LG lanes per row, 8 columns per lane and pass
-        {
-            int LG = 1;
-            while (LG < chunks && LG < 32) LG <<= 1;
-            const int rows_per_pass = kMsThreads / LG, sub = tid % LG;
-            for (int i0 = 0; i0 < sb; i0 += rows_per_pass) {   // (uniform trip count: every lane takes part in the shuffles)
-                const int i = i0 + tid / LG;
-                float acc = 0.f;
-                for (int c = sub; c < chunks && i < sb; c += LG) {
-                    const uint4 v = *reinterpret_cast<const uint4 *>(Ys + i * ldys + c * 8);
-                    const float *xv = xs + c * 8;
-                    float xe[8];
+#pragma unroll 1
+        for (int i0 = 0; i0 < sb; i0 += mrows) {        // (uniform trip count: every lane takes part in the shuffles)
+            const int i = i0 + tid / LG;
+            float acc = 0.f;
+#pragma unroll 1
+            for (int c = msub; c < chunks && i < sb; c += LG) {
+                const uint4 v = *reinterpret_cast<const uint4 *>(Ys + i * ldys + c * 8);
+                float xe[8];
 #pragma unroll
-                    for (int e = 0; e < 8; ++e) {
-                        const float t = c * 8 + e < n ? xv[e] : 0.f;
-                        xe[e] = p.exact_margin ? t : bf16_round(t);
-                    }
-                    acc = fmaf(bf16lo(v.x), xe[0], acc); acc = fmaf(bf16hi(v.x), xe[1], acc);
-                    acc = fmaf(bf16lo(v.y), xe[2], acc); acc = fmaf(bf16hi(v.y), xe[3], acc);
-                    acc = fmaf(bf16lo(v.z), xe[4], acc); acc = fmaf(bf16hi(v.z), xe[5], acc);
-                    acc = fmaf(bf16lo(v.w), xe[6], acc); acc = fmaf(bf16hi(v.w), xe[7], acc);
+                for (int e = 0; e < 8; ++e) {
+                    const float t = c * 8 + e < n ? xs[c * 8 + e] : 0.f;
+                    xe[e] = p.exact_margin ? t : bf16_round(t);
                 }
-                for (int o = LG >> 1; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
-                if (sub == 0 && i < sb) {
-                    rs[i] = acc;
-                    if (s == 1) { zs[i] = acc; us[i] = lprime_rt(p.loss, acc, yl[i]); }
-                }
+                acc = fmaf(bf16lo(v.x), xe[0], acc); acc = fmaf(bf16hi(v.x), xe[1], acc);
+                acc = fmaf(bf16lo(v.y), xe[2], acc); acc = fmaf(bf16hi(v.y), xe[3], acc);
+                acc = fmaf(bf16lo(v.z), xe[4], acc); acc = fmaf(bf16hi(v.z), xe[5], acc);
+                acc = fmaf(bf16lo(v.w), xe[6], acc); acc = fmaf(bf16hi(v.w), xe[7], acc);
+            }
+            MT(10);
+            for (int o = LG >> 1; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
+            MT(11);
+            if (msub == 0 && i < sb) {
+                rs[i] = acc;
+                if (s == 1) { zs[i] = acc; us[i] = lprime<LOSS>(acc, yl[i]); }
             }
         }
 
+        MT(3);
         // ---- Gram (line 4): 16 x 8 tiles of the strict block-lower part, mma.sync from the row-major stage
         if (s > 1) {
             const int g = lane >> 2, t4 = lane & 3;
             const int TR = L.sbp >> 4, ksteps = (ldys - 8) >> 4;
+#pragma unroll 1
             for (int tr = 0; tr < TR; ++tr) {           // (a row tile inside block 0 has no columns: ntc = 0)
                 const int row_hi = min(tr * 16 + 15, sb - 1);
-                const int ncols = (row_hi / b) * b;     // columns [0, ncols) hold a block below the block of some row of the tile
-                const int ntc = (ncols + 7) >> 3;
-                for (int tc = warp; tc < ntc; tc += kMsWarps) {
+                const int ntc = ((row_hi / b) * b + 7) >> 3;    // 8-column tiles that hold a block below some row of the tile
+#pragma unroll 1
+                for (int tc = warp; tc < ntc; tc += nwarp) {
                     float c[4] = {0.f, 0.f, 0.f, 0.f};
                     const uint16_t *arow0 = Ys + (tr * 16 + g) * ldys + 2 * t4, *arow1 = arow0 + 8 * ldys;
                     const uint16_t *brow = Ys + (tc * 8 + g) * ldys + 2 * t4;
+#pragma unroll 1
                     for (int ks = 0; ks < ksteps; ++ks) {
                         uint32_t a[4], bq[2];
                         a[0] = *reinterpret_cast<const uint32_t *>(arow0 + ks * 16);
@@ -218,81 +248,89 @@ mini_step_kernel(const MiniParams p)
             }
         }
         __syncthreads();
+        MT(4);
 
         // ---- recurrence (lines 6-15): a warp per row of block j, one barrier per inner step
         if (s > 1) {
+#pragma unroll 1
             for (int j = 0; j < s; ++j) {
                 const int len = j * b;
                 const float *gblk = gl + (b * b * j * (j - 1)) / 2;
-                for (int i = j * b + warp; i < (j + 1) * b; i += kMsWarps) {
+#pragma unroll 1
+                for (int i = j * b + warp; i < (j + 1) * b; i += nwarp) {
                     float acc = 0.f;
                     const float *grow = gblk + (i - j * b) * len;
+#pragma unroll 1
                     for (int k = lane; k < len; k += 32) acc = fmaf(grow[k], us[k], acc);
                     acc = warp_sum(acc);
                     if (lane == 0) {
                         const float zz = fmaf(-p.alpha, acc, rs[i]);
                         zs[i] = zz;
-                        us[i] = lprime_rt(p.loss, zz, yl[i]);
+                        us[i] = lprime<LOSS>(zz, yl[i]);
                     }
                 }
                 __syncthreads();
             }
         }
 
+        MT(5);
         // ---- update (lines 16-17): g = Y^T u by lane groups (8 columns per thread), rows split over the groups; the
         // groups of a warp meet by shuffles, the 16 warps through shared memory, in a fixed order
         {
-            int CH = 1;
-            while (CH < chunks) CH <<= 1;               // lanes side by side on a row (power of two)
-            const int c = tid % CH, part = tid / CH, parts = kMsThreads / CH;
             float acc[8] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
-            if (c < chunks)
-                for (int i = part; i < sb; i += parts) {
-                    const uint4 v = *reinterpret_cast<const uint4 *>(Ys + i * ldys + c * 8);
+            if (csub < chunks)
+#pragma unroll 1
+                for (int i = crow; i < sb; i += crows) {
+                    const uint4 v = *reinterpret_cast<const uint4 *>(Ys + i * ldys + csub * 8);
                     const float uu = us[i];
                     acc[0] = fmaf(bf16lo(v.x), uu, acc[0]); acc[1] = fmaf(bf16hi(v.x), uu, acc[1]);
                     acc[2] = fmaf(bf16lo(v.y), uu, acc[2]); acc[3] = fmaf(bf16hi(v.y), uu, acc[3]);
                     acc[4] = fmaf(bf16lo(v.z), uu, acc[4]); acc[5] = fmaf(bf16hi(v.z), uu, acc[5]);
                     acc[6] = fmaf(bf16lo(v.w), uu, acc[6]); acc[7] = fmaf(bf16hi(v.w), uu, acc[7]);
                 }
+#pragma unroll 1
             for (int o = CH; o < 32; o <<= 1)
 #pragma unroll
                 for (int e = 0; e < 8; ++e) acc[e] += __shfl_xor_sync(0xffffffffu, acc[e], o);
-            // partial sums that remain: one per warp when CH <= 32, one per `part` otherwise (then parts <= 16)
-            const int nred = CH <= 32 ? kMsWarps : parts, ridx = CH <= 32 ? warp : part;
-            if (c < chunks && (CH > 32 || lane < CH)) {
+            // partial sums that remain: one per warp when CH <= 32, one per row group otherwise (then <= 16 groups)
+            const int nred = CH <= 32 ? nwarp : crows, ridx = CH <= 32 ? warp : crow;
+            if (csub < chunks && (CH > 32 || lane < CH)) {
 #pragma unroll
-                for (int e = 0; e < 8; ++e) red[ridx * ldy + c * 8 + e] = acc[e];
+                for (int e = 0; e < 8; ++e) red[ridx * ldy + csub * 8 + e] = acc[e];
             }
             __syncthreads();
-            for (int col = tid; col < n; col += kMsThreads) {
+#pragma unroll 1
+            for (int col = tid; col < n; col += nthr) {
                 float gsum = 0.f;
-                for (int q = 0; q < nred; ++q) gsum += red[q * ldy + col];
+#pragma unroll 4
+                for (int r2 = 0; r2 < nred; ++r2) gsum += red[r2 * ldy + col];
                 xs[col] = fmaf(-p.alpha, gsum, xs[col]);
             }
         }
 
+        MT(6);
         if (last) {
             // the intermediates casgd_debug_export serves
-            for (int t = tid; t < sb * chunks; t += kMsThreads) {
-                const int row = t / chunks, c = t - row * chunks;
-                *reinterpret_cast<uint4 *>(p.Y + (int64_t)row * ldy + c * 8) = *reinterpret_cast<const uint4 *>(Ys + row * ldys + c * 8);
-            }
-            for (int i = tid; i < sb; i += kMsThreads) { p.yI[i] = yl[i]; p.r[i] = rs[i]; p.z[i] = zs[i]; p.u[i] = us[i]; }
-            for (int i = b + warp; i < sb; i += kMsWarps) {
+            if (csub < chunks)
+#pragma unroll 1
+                for (int row = crow; row < sb; row += crows)
+                    *reinterpret_cast<uint4 *>(p.Y + (int64_t)row * ldy + csub * 8) = *reinterpret_cast<const uint4 *>(Ys + row * ldys + csub * 8);
+            if (tid < sb) { p.yI[tid] = yl[tid]; p.r[tid] = rs[tid]; p.z[tid] = zs[tid]; p.u[tid] = us[tid]; }
+#pragma unroll 1
+            for (int i = b + warp; i < sb; i += nwarp) {
                 const int j = i / b;
                 const float *grow = gl + (b * b * j * (j - 1)) / 2 + (i - j * b) * j * b;
+#pragma unroll 1
                 for (int k = lane; k < j * b; k += 32) p.G[(int64_t)i * p.ldg + k] = grow[k];
             }
         }
-#pragma unroll
-        for (int q = 0; q < 4; ++q)
-            if (step + NS < p.n_steps && tid + q * kMsThreads < sb)
-                reinterpret_cast<int32_t *>(ms_smem + L.idx[buf])[tid + q * kMsThreads] = idx_next[q];
+        if (step + 2 < p.n_steps && tid < sb) reinterpret_cast<int32_t *>(ms_smem + L.idx + q * L.idx_stride)[tid] = idx_next;
         __syncthreads();                                // x, the stage and the vectors are free for the next iteration
+        MT(7);
     }
     asm volatile("cp.async.wait_group 0;" ::: "memory");
-    for (int k = tid; k < n; k += kMsThreads) {
+#pragma unroll 1
+    for (int k = tid; k < n; k += nthr) {
         const float xn = xs[k];
         p.x[k] = xn;
         store_shadow(p.xbf, p.split ? p.ldxb : 0, k, xn);
@@ -307,29 +345,34 @@ constexpr int kMiniSmemCap = 227 * 1024;
 
 cudaError_t mini_step_configure()
 {
-    return cudaFuncSetAttribute(mini_step_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kMiniSmemCap);
+    cudaError_t e = cudaFuncSetAttribute(mini_step_kernel<CASGD_LOGISTIC>, cudaFuncAttributeMaxDynamicSharedMemorySize, kMiniSmemCap);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(mini_step_kernel<CASGD_LINEAR>, cudaFuncAttributeMaxDynamicSharedMemorySize, kMiniSmemCap);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(mini_step_kernel<CASGD_POISSON>, cudaFuncAttributeMaxDynamicSharedMemorySize, kMiniSmemCap);
+    return e;
 }
 
 // Does the one-launch kernel take this shape? Everything of an iteration (two Y stages, the packed strict block-lower
 // G, the vectors) must fit one CTA's shared memory, and the Gram and the chain must be small enough for one SM.
-bool mini_step_ok(int32_t n, int32_t ldy, int32_t s, int32_t b)
+bool mini_step_ok(int32_t n, int32_t ldy, int32_t s, int32_t b, bool any_fit)
 {
     const int64_t sb = (int64_t)s * b;
-    if (n < 1 || n > 2048 || sb > 2048 || ldy != ((n + 7) & ~7)) return false;
+    if (n < 1 || n > 2048 || sb > kMsMaxThreads || ldy != ((n + 7) & ~7)) return false;   // (one index per thread)
     if ((int64_t)b * b * s * (s - 1) * 2 > 160 * 1024) return false;
     // gradient partial sums: 16 warps (row groups of <= 32 lanes) or 512 / CH parts, times ldy floats
     int CH = 1;
     while (CH < ldy / 8) CH <<= 1;
-    const int nred = CH <= 32 ? kMsWarps : kMsThreads / CH;
+    const int nred = CH <= 32 ? kMsMaxWarps : kMsMaxThreads / CH;
     if ((int64_t)nred * ldy > kMsRedFloats) return false;
-    const MiniLayout L = mini_layout(n, s, b, 2);
-    if (L.total > (uint32_t)kMiniSmemCap) return false;
-    // measured crossovers against the kernel-per-stage path: s = 1 wins while the rows of a step are a few KB (n = 18,
-    // b = 64: 2.4 against 7.2 us; n = 512, b = 64 -- 64 KB through one SM -- 8.9 against 8.0); s > 1 while Gram and chain
-    // are tiny (n = 64, sb = 64: 6.1 against 8.4 us; n = 18, sb = 256: 19.2 against 9.3)
-    if (s == 1) return (int64_t)b * ldy * 2 <= 16 * 1024;
+    if (mini_layout(n, s, b).total > (uint32_t)kMiniSmemCap) return false;
+    // measured crossovers against the kernel-per-stage path (us per iteration): s = 1 wins up to 32 KB of rows per step
+    // (n = 18, b = 64: 1.4 against 7.2; n = 128, b = 128: 4.0 against 6.3; n = 128, b = 256: 9.0 against 7.2) and for
+    // rows of <= 128 bytes at any b (n = 64, b = 512: 5.8 against 10.3); steps beyond 4 KB with rows of >= 128 bytes go to the
+    // cluster kernel first (s1_cluster.cu; n = 256, b = 64: 1.9 against 5.2 here). s > 1 wins while Gram and chain are tiny (n = 64,
+    // s = 4, b = 16: 5.1 against 7.8; n = 128: 6.5 against 8.0; n = 256, s = 2, b = 32: 8.9 against 7.6)
+    if (any_fit) return true;                           // CASGD_OPT_MINI = 2: the structural limits only
+    if (s == 1) return (int64_t)b * ldy * 2 <= 32 * 1024 || ldy <= 64;
     const int64_t macs = (int64_t)((n + 15) & ~15) * b * b * s * (s - 1) / 2;
-    return sb <= 128 && macs <= (256ll << 10) && (int64_t)s * ((b + kMsWarps - 1) / kMsWarps) <= 16;
+    return sb <= 128 && macs <= (200ll << 10) && (int64_t)s * ((b + kMsMaxWarps - 1) / kMsMaxWarps) <= 16;
 }
 
 int launch_mini_steps(cudaStream_t st, const uint16_t *A, int64_t lda, const float *y, int64_t m, int32_t n, int32_t ldy,
@@ -339,14 +382,26 @@ int launch_mini_steps(cudaStream_t st, const uint16_t *A, int64_t lda, const flo
 {
     MiniParams p;
     p.A = A; p.lda = lda; p.m = m; p.y = y; p.idx = idx; p.n_steps = n_steps; p.n = n; p.ldy = ldy; p.s = s; p.b = b;
-    p.loss = loss; p.exact_margin = exact_margin; p.alpha = alpha; p.x = x; p.xbf = xbf; p.ldxb = ldxb; p.split = split;
+    p.exact_margin = exact_margin; p.alpha = alpha; p.x = x; p.xbf = xbf; p.ldxb = ldxb; p.split = split;
     p.Y = Y; p.yI = yI; p.G = G; p.r = r; p.z = z; p.u = u; p.ldg = ldg; p.err_flag = err_flag; p.stamp = g_stamp;
-    // rows are gathered ONE iteration ahead (two stages). Measured with four stages (three iterations ahead): no gain
-    // (n = 18, b = 64, s = 1: 2.71 against 2.43 us per step) -- an iteration is bound by its own dependent phases and
-    // barriers, not by the latency of the rows.
-    p.stages = 2;
-    const MiniLayout L = mini_layout(n, s, b, p.stages);
-    return launch_pdl(mini_step_kernel, dim3(1), dim3(kMsThreads), (size_t)L.total, st, 1, p) == cudaSuccess ? 1 : -1;
+    const MiniLayout L = mini_layout(n, s, b);
+    auto *kern = loss == CASGD_LOGISTIC ? mini_step_kernel<CASGD_LOGISTIC>
+               : loss == CASGD_LINEAR  ? mini_step_kernel<CASGD_LINEAR>
+                                       : mini_step_kernel<CASGD_POISSON>;
+    // measured: the barriers of a small s = 1 iteration are cheaper with 8 warps (n = 18, b = 64: 1.43 against 1.68 us;
+    // from 12 KB of rows on 16 warps win again), the
+    // chain of s > 1 wants a warp per row of a block (n = 64, s = 4, b = 16: 5.2 us with 16 warps, 6.0 with 8)
+    int threads = s == 1 && b * ldy * 2 <= 4096 ? 256 : kMsMaxThreads;
+    while (threads < s * b || threads * 8 < ldy) threads <<= 1;    // one index per thread; a row's 16-byte pieces side by side
+    return launch_pdl(kern, dim3(1), dim3(threads), (size_t)L.total, st, 1, p) == cudaSuccess ? 1 : -1;
 }
+
+#ifdef CASGD_MINI_TRACE
+extern "C" int casgd_mini_trace_dump(long long *dst_host)
+{
+    cudaDeviceSynchronize();
+    return (int)cudaMemcpyFromSymbol(dst_host, g_mini_trace, sizeof(long long) * 64);
+}
+#endif
 
 }  // namespace casgd

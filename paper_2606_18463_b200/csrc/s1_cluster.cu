@@ -25,7 +25,7 @@ struct S1Params {
     const float *y;
     const int32_t *idx;
     int64_t n_steps;
-    int32_t n, ldy, b, loss, exact_margin, cpc;     // cpc: columns per CTA (a multiple of 8)
+    int32_t n, ldy, b, exact_margin, cpc;     // cpc: columns per CTA (a multiple of 8)
     float alpha;
     float *x;
     uint16_t *xbf;
@@ -36,8 +36,10 @@ struct S1Params {
     unsigned long long *stamp;
 };
 
+// two stages of the labels, the indices, the receive buffers and the Y slice: stage q at base + q * stride (scalars: an
+// array of offsets indexed at run time lives in local memory)
 struct S1Layout {
-    uint32_t x, u, yl[2], idx[2], recv[2], red, Y[2], total;
+    uint32_t x, u, yl, idx, vec_stride, recv, recv_stride, red, Y, Y_stride, total;
     int32_t lds;                                    // row stride of a Y slice in elements
 };
 
@@ -49,11 +51,14 @@ __host__ __device__ inline S1Layout s1_layout(int b, int cpc, int C)
     auto take = [&](uint32_t bytes) { const uint32_t at = o; o += (bytes + 15u) & ~15u; return at; };
     L.x = take(4u * cpc);
     L.u = take(4u * b);
-    for (int q = 0; q < 2; ++q) L.yl[q] = take(4u * b);
-    for (int q = 0; q < 2; ++q) L.idx[q] = take(4u * b);
-    for (int q = 0; q < 2; ++q) L.recv[q] = take(4u * (uint32_t)C * b);      // [rank][row]
+    L.vec_stride = (4u * b + 15u) & ~15u;
+    L.yl = take(2u * L.vec_stride);
+    L.idx = take(2u * L.vec_stride);
+    L.recv_stride = (4u * (uint32_t)C * b + 15u) & ~15u;                     // [rank][row]
+    L.recv = take(2u * L.recv_stride);
     L.red = take(4u * kScWarps * cpc);
-    for (int q = 0; q < 2; ++q) L.Y[q] = take(2u * (uint32_t)b * L.lds);
+    L.Y_stride = (2u * (uint32_t)b * L.lds + 15u) & ~15u;
+    L.Y = take(2u * L.Y_stride);
     L.total = o;
     return L;
 }
@@ -65,6 +70,8 @@ __device__ __forceinline__ void sc_cluster_sync()
     asm volatile("barrier.cluster.arrive.release.aligned;\n\tbarrier.cluster.wait.acquire.aligned;" ::: "memory");
 }
 
+// (one instantiation per loss, outer loops not unrolled, power-of-two lane groups: see mini_step.cu on code size)
+template <int LOSS>
 __global__ void __launch_bounds__(kScThreads, 1)
 s1_cluster_kernel(const S1Params p)
 {
@@ -83,31 +90,42 @@ s1_cluster_kernel(const S1Params p)
     float *red = reinterpret_cast<float *>(sc_smem + L.red);
     const uint32_t smem0 = (uint32_t)__cvta_generic_to_shared(sc_smem);
 
-    for (uint32_t o = L.Y[0] + 16u * tid; o < L.total; o += 16u * kScThreads)
+#pragma unroll 1
+    for (uint32_t o = L.Y + 16u * tid; o < L.total; o += 16u * kScThreads)
         *reinterpret_cast<uint4 *>(sc_smem + o) = make_uint4(0u, 0u, 0u, 0u);
     pdl_wait();
     stamp_begin(p.stamp);
+#pragma unroll 1
     for (int k = tid; k < cpc; k += kScThreads) xs[k] = c0 + k < n ? p.x[c0 + k] : 0.f;
-    for (int q = 0; q < 2; ++q)
-        if (q < p.n_steps)
-            for (int i = tid; i < b; i += kScThreads)
-                reinterpret_cast<int32_t *>(sc_smem + L.idx[q])[i] = p.idx[(int64_t)q * b + i];
+    if (tid < b) {                                      // (b <= 256 = the threads: one index per thread and stage)
+        reinterpret_cast<int32_t *>(sc_smem + L.idx)[tid] = p.idx[tid];
+        if (p.n_steps > 1) reinterpret_cast<int32_t *>(sc_smem + L.idx + L.vec_stride)[tid] = p.idx[b + tid];
+    }
     __syncthreads();
 
+    int CH = 1, chs = 0;                                // gather, export: lanes side by side on a row slice (cpc <= 256: CH <= 32)
+    while (CH < (cpc >> 3)) { CH <<= 1; ++chs; }
+    const int csub = tid & (CH - 1), crow = tid >> chs, crows = kScThreads >> chs;
+
     auto issue_gather = [&](int64_t step) {
-        const int buf = (int)(step & 1);
-        const int32_t *I = reinterpret_cast<const int32_t *>(sc_smem + L.idx[buf]);
-        for (int t = tid; t < b * chunks; t += kScThreads) {
-            const int row = t / chunks, c = t - row * chunks;
-            const int64_t src = I[row];
-            const uint32_t dst = smem0 + L.Y[buf] + 2u * (uint32_t)(row * lds + c * 8);
-            if (src >= 0 && src < p.m) asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(dst), "l"(p.A + src * p.lda + c0 + c * 8) : "memory");
-            else *reinterpret_cast<uint4 *>(sc_smem + (dst - smem0)) = make_uint4(0u, 0u, 0u, 0u);
+        const uint32_t q = (uint32_t)(step & 1);
+        const int32_t *I = reinterpret_cast<const int32_t *>(sc_smem + L.idx + q * L.vec_stride);
+        const uint32_t ybase = L.Y + q * L.Y_stride;
+        if (csub < chunks) {
+#pragma unroll 1
+            for (int row = crow; row < b; row += crows) {
+                const int64_t src = I[row];
+                const uint32_t off = ybase + 2u * (uint32_t)(row * lds + csub * 8);
+                if (src >= 0 && src < p.m)
+                    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(smem0 + off), "l"(p.A + src * p.lda + c0 + csub * 8) : "memory");
+                else *reinterpret_cast<uint4 *>(sc_smem + off) = make_uint4(0u, 0u, 0u, 0u);
+            }
         }
-        for (int i = tid; i < b; i += kScThreads) {
-            const int64_t src = I[i];
-            if (src >= 0 && src < p.m) asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"(smem0 + L.yl[buf] + 4u * i), "l"(p.y + src) : "memory");
-            else { reinterpret_cast<float *>(sc_smem + L.yl[buf])[i] = 0.f; if (crank == 0) atomicOr(p.err_flag, 1); }
+        if (tid < b) {
+            const int64_t src = I[tid];
+            const uint32_t off = L.yl + q * L.vec_stride + 4u * (uint32_t)tid;
+            if (src >= 0 && src < p.m) asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"(smem0 + off), "l"(p.y + src) : "memory");
+            else { *reinterpret_cast<float *>(sc_smem + off) = 0.f; if (crank == 0) atomicOr(p.err_flag, 1); }
         }
         asm volatile("cp.async.commit_group;" ::: "memory");
     };
@@ -116,29 +134,33 @@ s1_cluster_kernel(const S1Params p)
 
     int LG = 1;
     while (LG < chunks && LG < 32) LG <<= 1;            // lanes side by side on a row slice
-    const int rows_per_pass = kScThreads / LG, sub = tid % LG;
+    const int rows_per_pass = kScThreads / LG, sub = tid & (LG - 1);
     const uint32_t recv_rank_off = 4u * (uint32_t)(crank * b);
 
+#pragma unroll 1
     for (int64_t step = 0; step < p.n_steps; ++step) {
-        const int buf = (int)(step & 1);
+        const uint32_t q = (uint32_t)(step & 1);
         const bool last = step + 1 == p.n_steps;
         if (!last) issue_gather(step + 1); else asm volatile("cp.async.commit_group;" ::: "memory");
         int32_t idx_next = 0;
         if (step + 2 < p.n_steps && tid < b) idx_next = p.idx[(step + 2) * b + tid];
         asm volatile("cp.async.wait_group 1;" ::: "memory");
         __syncthreads();
-        uint16_t *Ys = reinterpret_cast<uint16_t *>(sc_smem + L.Y[buf]);
-        const float *yl = reinterpret_cast<const float *>(sc_smem + L.yl[buf]);
+        uint16_t *Ys = reinterpret_cast<uint16_t *>(sc_smem + L.Y + q * L.Y_stride);
+        const float *yl = reinterpret_cast<const float *>(sc_smem + L.yl + q * L.vec_stride);
+        const uint32_t recv_q = L.recv + q * L.recv_stride;
         if ((n & 7) && c0 + ncol > n) {                 // the CTA that holds the row's last chunk: pad columns are zero
-            for (int i = tid; i < b; i += kScThreads)
-                for (int c = n - c0; c < ncol; ++c) Ys[i * lds + c] = 0;
+            if (tid < b)
+                for (int c = n - c0; c < ncol; ++c) Ys[tid * lds + c] = 0;
             __syncthreads();
         }
 
         // ---- partial margins of this column slice, into every CTA's receive buffer
+#pragma unroll 1
         for (int i0 = 0; i0 < b; i0 += rows_per_pass) {
             const int i = i0 + tid / LG;
             float acc = 0.f;
+#pragma unroll 1
             for (int c = sub; c < chunks && i < b; c += LG) {
                 const uint4 v = *reinterpret_cast<const uint4 *>(Ys + i * lds + c * 8);
                 const float *xv = xs + c * 8;
@@ -153,30 +175,35 @@ s1_cluster_kernel(const S1Params p)
             for (int o = LG >> 1; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
             // lane `sub` of the row's group stores to CTA sub, sub + LG, ...: the C remote stores of a row are spread over its lanes
             if (i < b)
+#pragma unroll 1
                 for (int dstc = sub; dstc < C; dstc += LG) {
                     uint32_t remote;
-                    asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(remote) : "r"(smem0 + L.recv[buf] + recv_rank_off + 4u * (uint32_t)i), "r"((uint32_t)dstc));
+                    asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(remote) : "r"(smem0 + recv_q + recv_rank_off + 4u * (uint32_t)i), "r"((uint32_t)dstc));
                     asm volatile("st.shared::cluster.f32 [%0], %1;" ::"r"(remote), "f"(acc) : "memory");
                 }
         }
         sc_cluster_sync();                              // all partials of this iteration have landed everywhere
 
         // ---- r = sum over ranks (rank order: identical bits in every CTA), u = l'(r, y_I)
-        const float *rv = reinterpret_cast<const float *>(sc_smem + L.recv[buf]);
-        for (int i = tid; i < b; i += kScThreads) {
+        const float *rv = reinterpret_cast<const float *>(sc_smem + recv_q);
+        if (tid < b) {
+            const int i = tid;
             float rr = 0.f;
-            for (int q = 0; q < C; ++q) rr += rv[q * b + i];
-            const float uu = lprime_rt(p.loss, rr, yl[i]);
+#pragma unroll 4
+            for (int k = 0; k < C; ++k) rr += rv[k * b + i];
+            const float uu = lprime<LOSS>(rr, yl[i]);
             us[i] = uu;
             if (last && crank == 0) { p.yI[i] = yl[i]; p.r[i] = rr; p.z[i] = rr; p.u[i] = uu; }
         }
         __syncthreads();
 
         // ---- update of this CTA's columns: a warp per group of rows, 8 columns per lane and pass
+#pragma unroll 1
         for (int cb = 0; cb < chunks; cb += 32) {
             const int c = cb + lane;
             float acc[8] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
             if (c < chunks)
+#pragma unroll 2
                 for (int i = warp; i < b; i += kScWarps) {
                     const uint4 v = *reinterpret_cast<const uint4 *>(Ys + i * lds + c * 8);
                     const float uu = us[i];
@@ -191,21 +218,22 @@ s1_cluster_kernel(const S1Params p)
             }
         }
         __syncthreads();
+#pragma unroll 1
         for (int k = tid; k < ncol; k += kScThreads) {
             float g = 0.f;
 #pragma unroll
             for (int w = 0; w < kScWarps; ++w) g += red[w * cpc + k];
             xs[k] = fmaf(-p.alpha, g, xs[k]);
         }
-        if (last)
-            for (int t = tid; t < b * chunks; t += kScThreads) {
-                const int row = t / chunks, c = t - row * chunks;
-                *reinterpret_cast<uint4 *>(p.Y + (int64_t)row * p.ldy + c0 + c * 8) = *reinterpret_cast<const uint4 *>(Ys + row * lds + c * 8);
-            }
-        if (step + 2 < p.n_steps && tid < b) reinterpret_cast<int32_t *>(sc_smem + L.idx[buf])[tid] = idx_next;
+        if (last && csub < chunks)
+#pragma unroll 1
+            for (int row = crow; row < b; row += crows)
+                *reinterpret_cast<uint4 *>(p.Y + (int64_t)row * p.ldy + c0 + csub * 8) = *reinterpret_cast<const uint4 *>(Ys + row * lds + csub * 8);
+        if (step + 2 < p.n_steps && tid < b) reinterpret_cast<int32_t *>(sc_smem + L.idx + q * L.vec_stride)[tid] = idx_next;
         __syncthreads();
     }
     asm volatile("cp.async.wait_group 0;" ::: "memory");
+#pragma unroll 1
     for (int k = tid; k < ncol; k += kScThreads)
         if (c0 + k < n) {
             p.x[c0 + k] = xs[k];
@@ -230,15 +258,23 @@ void s1_cluster_shape(int32_t ldy, int *C, int *cpc)
 
 cudaError_t s1_cluster_configure()
 {
-    cudaError_t e = cudaFuncSetAttribute(s1_cluster_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kScSmemCap);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(s1_cluster_kernel, cudaFuncAttributeNonPortableClusterSizeAllowed, 1);
+    cudaError_t e = cudaSuccess;
+    auto set = [&](auto *k) {
+        if (e == cudaSuccess) e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, kScSmemCap);
+        if (e == cudaSuccess) e = cudaFuncSetAttribute(k, cudaFuncAttributeNonPortableClusterSizeAllowed, 1);
+    };
+    set(s1_cluster_kernel<CASGD_LOGISTIC>);
+    set(s1_cluster_kernel<CASGD_LINEAR>);
+    set(s1_cluster_kernel<CASGD_POISSON>);
     return e;
 }
 
-// s = 1, rows of >= 512 bytes that mini_step.cu does not take, b <= 256, everything of a CTA within its shared memory
+// s = 1, rows of >= 128 bytes (8 columns per CTA), b <= 256, everything of a CTA within its shared memory. Measured against
+// mini_step.cu's one CTA (us per iteration): n = 64, b = 128: 1.96 against 2.27; n = 128, b = 128: 2.16 against 3.98;
+// n = 248, b = 64: 1.93 against 5.31 -- and the other way round only for steps of <= 4 KB (n = 64, b = 16: 1.52 against 1.19)
 bool s1_cluster_ok(int32_t n, int32_t ldy, int32_t b, int cluster_max)
 {
-    if (ldy != ((n + 7) & ~7) || ldy * 2 < 512 || b < 1 || b > kScMaxB) return false;
+    if (ldy != ((n + 7) & ~7) || ldy * 2 < 128 || b < 1 || b > kScMaxB) return false;
     int C, cpc;
     s1_cluster_shape(ldy, &C, &cpc);
     if (C > cluster_max) return false;
@@ -252,11 +288,14 @@ int launch_s1_cluster(cudaStream_t st, const uint16_t *A, int64_t lda, const flo
     S1Params p;
     int C;
     s1_cluster_shape(ldy, &C, &p.cpc);
-    p.A = A; p.lda = lda; p.m = m; p.y = y; p.idx = idx; p.n_steps = n_steps; p.n = n; p.ldy = ldy; p.b = b; p.loss = loss;
+    p.A = A; p.lda = lda; p.m = m; p.y = y; p.idx = idx; p.n_steps = n_steps; p.n = n; p.ldy = ldy; p.b = b;
     p.exact_margin = exact_margin; p.alpha = alpha; p.x = x; p.xbf = xbf; p.ldxb = ldxb; p.split = split;
     p.Y = Y; p.yI = yI; p.r = r; p.z = z; p.u = u; p.err_flag = err_flag; p.stamp = g_stamp;
     const S1Layout L = s1_layout(b, p.cpc, C);
-    return launch_pdl(s1_cluster_kernel, dim3(C), dim3(kScThreads), (size_t)L.total, st, C, p) == cudaSuccess ? 1 : -1;
+    auto *kern = loss == CASGD_LOGISTIC ? s1_cluster_kernel<CASGD_LOGISTIC>
+               : loss == CASGD_LINEAR  ? s1_cluster_kernel<CASGD_LINEAR>
+                                       : s1_cluster_kernel<CASGD_POISSON>;
+    return launch_pdl(kern, dim3(C), dim3(kScThreads), (size_t)L.total, st, C, p) == cudaSuccess ? 1 : -1;
 }
 
 }  // namespace casgd

@@ -471,14 +471,17 @@ def test_pipelined_graphs_of_two_contexts_and_shapes_interleaved(binding):
         assert torch.linalg.norm(got[k] - ref[k]) <= 2e-5 * torch.linalg.norm(ref[k]), k
 
 
-MINI_SHAPES = [(0, 8192, 64, 4, 16), (1, 20000, 18, 1, 64), (1, 20000, 18, 2, 64), (4, 6000, 512, 1, 16), (0, 4097, 64, 7, 13),
-               (3, 3000, 100, 3, 24), (0, 5000, 33, 2, 5), (4, 6000, 512, 2, 16), (2, 20000, 1024, 1, 8),
+# (config, m, n, s, b, CASGD_OPT_MINI): 2 = the one-CTA kernel whenever the step fits it, whatever the measured crossovers
+MINI_SHAPES = [(0, 8192, 64, 4, 16, 2), (1, 20000, 18, 1, 64, 2), (1, 20000, 18, 2, 64, 2), (4, 6000, 512, 1, 16, 2),
+               (0, 4097, 64, 7, 13, 2), (3, 3000, 100, 3, 24, 2), (0, 5000, 33, 2, 5, 2), (4, 6000, 512, 2, 16, 2),
+               (2, 20000, 1024, 1, 8, 2), (1, 9000, 18, 1, 500, 2), (0, 9000, 120, 1, 130, 1), (0, 8192, 64, 4, 16, 1),
                # s = 1 with wide rows: one launch of one column-split cluster (s1_cluster.cu)
-               (4, 6000, 512, 1, 64), (3, 5000, 2000, 1, 32), (2, 20000, 4096, 1, 128), (3, 5000, 1001, 1, 40)]
+               (4, 6000, 512, 1, 64, 1), (3, 5000, 2000, 1, 32, 1), (2, 20000, 4096, 1, 128, 1), (3, 5000, 1001, 1, 40, 1),
+               (4, 6000, 256, 1, 16, 1), (0, 7000, 300, 1, 256, 1)]
 
 
-@pytest.mark.parametrize("ci,m,n,s,b", MINI_SHAPES)
-def test_one_launch_kernel_for_tiny_steps(binding, oracle_mod, ci, m, n, s, b):
+@pytest.mark.parametrize("ci,m,n,s,b,mode", MINI_SHAPES)
+def test_one_launch_kernel_for_tiny_steps(binding, oracle_mod, ci, m, n, s, b, mode):
     """mini_step.cu / s1_cluster.cu: steps that fit one SM, and s = 1 steps with wide rows (one
     column-split cluster), run all iterations of a call in ONE launch. One
     step against oracle O1 element by element (gather bit-exact, G, r, z, u, x); a 9-step call equals 9 single-step
@@ -492,6 +495,7 @@ def test_one_launch_kernel_for_tiny_steps(binding, oracle_mod, ci, m, n, s, b):
     x0 = random_x(n, 11, 0.4)
     eta = cfg.eta * 0.5
     with binding.Casgd(X_d, y_d, cfg.loss) as cg:
+        cg.set_option(binding.OPT_MINI, mode)
         n0 = cg.launch_count()
         check_step_against_oracle(oracle_mod, cg, A_bits, y, idx[: s * b], x0, s, b, eta, cfg.loss, binding)
         assert cg.launch_count() - n0 == 1, "the step did not run as one launch"
@@ -518,7 +522,7 @@ def test_one_launch_kernel_for_tiny_steps(binding, oracle_mod, ci, m, n, s, b):
         cg.outer_steps(idx_d, xd, s, b, eta)
         cg.sync()
         assert torch.linalg.norm(xd - xb) <= 2e-5 * torch.linalg.norm(xb)
-        cg.set_option(binding.OPT_MINI, 1)
+        cg.set_option(binding.OPT_MINI, mode)
         bad = idx[: s * b].copy()
         bad[3] = m + 5
         xe = torch.from_numpy(x0.copy()).cuda()
