@@ -206,7 +206,9 @@ int casgd_debug_export(casgd_ctx *c, int what, void *dst_host, int64_t dst_bytes
  *                              L2), 3 = the cluster kernel (one 16-CTA cluster, u through distributed shared
  *                              memory, G by plain loads; needs b % 4 == 0, else falls through to 2), 4 = the
  *                              streaming cluster kernel (same cluster, G through a cp.async.bulk shared-memory
- *                              ring; needs b % 4 == 0 and b <= 128, else falls through to 3).
+ *                              ring; needs b % 4 == 0 and b <= 128, else falls through to 3), 5 = the chain-CTA
+ *                              cluster kernel (blocks of 8..64 rows, b % 4 == 0, s*b <= 4096: the dependent chain on
+ *                              ONE CTA, the older part of every sum from 15 helper CTAs; else falls through to 4).
  *   CASGD_OPT_NO_FUSED_UPDATE  1 = the outer update always runs as its own kernel. Default 0: for small steps
  *                              (at most 136 KB of Y per CTA of the cluster, 2048 columns) the streaming recurrence kernel's cluster does
  *                              g = Y^T u, the update of x and the shadow itself, right after the chain.

@@ -299,7 +299,7 @@ inline bool pipelined_mode(const casgd_ctx *c, int32_t s, int32_t b)
     if (c->opt_overlap != 2 || s == 1 || c->num_sms < 64) return false;
     const bool fused = !c->opt_no_fuse && recurrence_fuses_update(s, b, c->ldg, c->ldy, c->rws, (int)c->opt_rec_impl);
     const int k = recurrence_kernel_choice(s, b, c->ldg, c->rws, (int)c->opt_rec_impl, fused);
-    return k == 1 || k == 4;
+    return k == 1 || k == 4 || k == 5;
 }
 
 // ---- the stages of one outer iteration (Alg. 1 lines 2-17), each on the stream it is given ----
@@ -773,7 +773,7 @@ int casgd_init(casgd_ctx **out, const uint16_t *X_bf16, int64_t ldx, const float
     // opt-in shared-memory sizes and cluster sizes are per-device function attributes: set them on this device
     if (gather_configure() != cudaSuccess || gradient_configure() != cudaSuccess || gram_tc_configure() != cudaSuccess ||
         gram_pair_configure() != cudaSuccess || loss_configure() != cudaSuccess || recurrence_configure() != cudaSuccess ||
-        recurrence_stream_configure() != cudaSuccess || mini_step_configure() != cudaSuccess || s1_cluster_configure() != cudaSuccess)
+        recurrence_stream_configure() != cudaSuccess || recurrence_chain_configure() != cudaSuccess || mini_step_configure() != cudaSuccess || s1_cluster_configure() != cudaSuccess)
         return bail(CASGD_ECUDA);
     c->stream = (cudaStream_t)cuda_stream;
     c->y = y; c->m = m; c->n = n; c->loss = loss;
@@ -1108,7 +1108,7 @@ int casgd_set_option(casgd_ctx *c, int option, int64_t value)
         if (value < 0 || value > 64) return fail(c, CASGD_EINVAL, "CASGD_OPT_GRAM_KSPLIT must be in [0, 64]");
         c->opt_ksplit = value; break;
     case CASGD_OPT_RECURRENCE_IMPL:
-        if (value < 0 || value > 4) return fail(c, CASGD_EINVAL, "CASGD_OPT_RECURRENCE_IMPL must be in [0, 4]");
+        if (value < 0 || value > 5) return fail(c, CASGD_EINVAL, "CASGD_OPT_RECURRENCE_IMPL must be in [0, 5]");
         c->opt_rec_impl = value; break;
     case CASGD_OPT_NO_FUSED_UPDATE: c->opt_no_fuse = value != 0; break;
     case CASGD_OPT_STAMPS:

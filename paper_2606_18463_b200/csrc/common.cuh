@@ -231,6 +231,7 @@ cudaError_t gram_pair_configure();
 cudaError_t loss_configure();
 cudaError_t recurrence_configure();
 cudaError_t recurrence_stream_configure();
+cudaError_t recurrence_chain_configure();
 cudaError_t mini_step_configure();
 cudaError_t s1_cluster_configure();
 
@@ -278,6 +279,13 @@ int recurrence_kernel_choice(int32_t s, int32_t b, int32_t ldg, const RecWorkspa
 int launch_recurrence(cudaStream_t st, const float *G, int32_t ldg, const float *r, const float *yI, int32_t s,
                       int32_t b, float alpha, int loss, float *z, float *u, const RecWorkspace &ws, int impl,
                       const FusedUpdate *fu);
+
+// recurrence_chain.cu: one cluster for blocks of <= 64 rows -- the chain on ONE CTA (no cluster crossing per hop), the
+// older part of every row's sum from 15 helper CTAs. Kernel choice 5.
+bool recurrence_chain_ok(int32_t s, int32_t b, int32_t ldg, int cluster);
+bool recurrence_chain_fuses_update(int32_t s, int32_t b, int32_t ldy);
+int launch_recurrence_chain(cudaStream_t st, const float *G, int32_t ldg, const float *r, const float *yI, int32_t s, int32_t b,
+                            float alpha, int loss, float *z, float *u, const FusedUpdate *fu, int late_trigger);
 
 // recurrence_stream.cu: one cluster, G streamed through a shared-memory ring, u through distributed shared memory.
 bool recurrence_stream_ok(int32_t s, int32_t b, int32_t ldg, int cluster);

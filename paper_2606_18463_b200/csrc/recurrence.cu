@@ -530,14 +530,21 @@ cudaError_t recurrence_configure()
     return e;
 }
 
+// the chain-CTA kernel (5): asked for, or ... (see recurrence_kernel_choice)
+static bool chain_preferred(int32_t s, int32_t b, int32_t ldg, const RecWorkspace &ws, int impl)
+{
+    return impl == 5 && recurrence_chain_ok(s, b, ldg, ws.cluster);
+}
+
 bool recurrence_fuses_update(int32_t s, int32_t b, int32_t ldg, int32_t ldy, const RecWorkspace &ws, int impl)
 {
     // with the update fused in, the cluster kernel beats the one-CTA kernel + a gradient kernel even for tiny G (measured)
-    return (impl == 4 || impl == 0) && recurrence_stream_ok(s, b, ldg, ws.cluster) && recurrence_stream_fuses_update(s, b, ldy, ws.cluster);
+    if (chain_preferred(s, b, ldg, ws, impl)) return recurrence_chain_fuses_update(s, b, ldy);
+    return (impl >= 4 || impl == 0) && recurrence_stream_ok(s, b, ldg, ws.cluster) && recurrence_stream_fuses_update(s, b, ldy, ws.cluster);
 }
 
 // Which kernel launch_recurrence runs for this shape: 1 = one CTA, 2 = all SMs (cooperative), 3 = one cluster with
-// plain loads, 4 = the streaming cluster kernel.
+// plain loads, 4 = the streaming cluster kernel, 5 = the chain-CTA cluster kernel (small blocks).
 int recurrence_kernel_choice(int32_t s, int32_t b, int32_t ldg, const RecWorkspace &ws, int impl, bool fused)
 {
     const int64_t gl_bytes = 2ll * b * b * s * (s - 1);
@@ -545,8 +552,9 @@ int recurrence_kernel_choice(int32_t s, int32_t b, int32_t ldg, const RecWorkspa
     // MAXR = 16 rows per warp covers CASGD_MAX_SB on >= 128 SMs; on fewer co-resident CTAs fall back
     const bool grid_ok = ws.max_ctas > 0 && (int64_t)ws.max_ctas * kRecWarps * 16 >= sb;
     const bool cluster_ok = ws.cluster > 0 && b % 4 == 0 && ldg % 4 == 0;
-    const bool stream_ok = (impl == 4 || impl == 0) && recurrence_stream_ok(s, b, ldg, ws.cluster);
-    if (stream_ok && (impl == 4 || gl_bytes >= ws.grid_threshold_bytes || fused)) return 4;
+    if (chain_preferred(s, b, ldg, ws, impl)) return 5;
+    const bool stream_ok = (impl >= 4 || impl == 0) && recurrence_stream_ok(s, b, ldg, ws.cluster);
+    if (stream_ok && (impl >= 4 || gl_bytes >= ws.grid_threshold_bytes || fused)) return 4;
     if (cluster_ok && (impl >= 3 || (impl == 0 && gl_bytes >= ws.grid_threshold_bytes))) return 3;
     if (grid_ok && (impl >= 2 || (impl == 0 && gl_bytes >= ws.grid_threshold_bytes))) return 2;
     return 1;
@@ -557,6 +565,7 @@ int launch_recurrence(cudaStream_t st, const float *G, int32_t ldg, const float 
                       const FusedUpdate *fu)
 {
     const int choice = recurrence_kernel_choice(s, b, ldg, ws, impl, fu != nullptr);
+    if (choice == 5) return launch_recurrence_chain(st, G, ldg, r, yI, s, b, alpha, loss, z, u, fu, ws.late_trigger);
     if (choice == 4)
         return launch_recurrence_stream(st, G, ldg, r, yI, s, b, alpha, loss, z, u, ws.cluster, fu, ws.late_trigger);
     if (choice == 3) {

@@ -64,10 +64,11 @@ def cases():
     yield "margin_s1", lambda: step_case("margin_s1", 4, 900, 136, 1, 64, [(B.OPT_MINI, 0)], eta=0.01)
     yield "s1_cluster", lambda: step_case("s1_cluster", 4, 900, 520, 1, 64, steps=5, eta=0.01)
     yield "s1_cluster_odd", lambda: step_case("s1_cluster_odd", 3, 900, 1001, 1, 40, steps=3)
-    for impl, nm in ((1, "cta"), (2, "grid"), (3, "cluster"), (4, "stream")):
+    for impl, nm in ((1, "cta"), (2, "grid"), (3, "cluster"), (4, "stream"), (5, "chain")):
         yield f"rec_{nm}", (lambda impl=impl, nm=nm: step_case(f"rec_{nm}", 0, 900, 24, 6, 32, [(B.OPT_RECURRENCE_IMPL, impl)]))
     yield "rec_stream_two_groups", lambda: step_case("rec_stream_two_groups", 0, 1200, 24, 3, 128, [(B.OPT_RECURRENCE_IMPL, 4)])
     yield "rec_stream_unfused", lambda: step_case("rec_stream_unfused", 0, 900, 24, 6, 32, [(B.OPT_RECURRENCE_IMPL, 4), (B.OPT_NO_FUSED_UPDATE, 1)])
+    yield "rec_chain_unfused", lambda: step_case("rec_chain_unfused", 0, 900, 24, 9, 64, [(B.OPT_RECURRENCE_IMPL, 5), (B.OPT_NO_FUSED_UPDATE, 1)])
     yield "rec_grid_scalar", lambda: step_case("rec_grid_scalar", 0, 900, 24, 5, 13, [(B.OPT_RECURRENCE_IMPL, 2)])
     yield "gather_bulk_gradient_stream", lambda: step_case("gather_bulk_gradient_stream", 2, 1200, 1024, 4, 128)
     yield "graph_sequential", lambda: step_case("graph_sequential", 4, 900, 136, 3, 64, [(B.OPT_OVERLAP, 0)], steps=9, eta=0.01)

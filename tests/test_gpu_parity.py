@@ -136,11 +136,12 @@ RECURRENCE = [
 ]
 
 
-@pytest.mark.parametrize("rec_impl", [1, 2, 3, 4], ids=["cta", "grid", "cluster", "stream"])
+@pytest.mark.parametrize("rec_impl", [1, 2, 3, 4, 5], ids=["cta", "grid", "cluster", "stream", "chain"])
 @pytest.mark.parametrize("ci,m,n,s,b", RECURRENCE)
 def test_recurrence_kernels_match_the_oracle(binding, oracle_mod, ci, m, n, s, b, rec_impl):
     """Every recurrence kernel (one CTA; all SMs with tagged words through L2; one cluster with plain loads of G;
-    one cluster with G streamed through a shared-memory ring) on the same inputs, forced with
+    one cluster with G streamed through a shared-memory ring; one cluster with the chain on a single CTA and the older
+    part of every sum from 15 helper CTAs) on the same inputs, forced with
     CASGD_OPT_RECURRENCE_IMPL, twice in a row (the second launch sees the first one's retired epoch). Shapes a
     kernel does not take (b % 4 != 0, more than 8 rows of a block per CTA) fall through to the next one."""
     cfg = synth.config(ci, m=m, n=n)
@@ -163,7 +164,7 @@ def test_grid_recurrence_replays_from_a_graph(binding):
     idx_d = torch.from_numpy(synth.epoch_indices(cfg, 42, 0)[: steps * s * b].copy()).cuda()
     xs = {}
     with binding.Casgd(X_d, y_d, cfg.loss) as cg:
-        for impl in (1, 2, 3, 4):
+        for impl in (1, 2, 3, 4, 5):
             cg.set_option(binding.OPT_RECURRENCE_IMPL, impl)
             xa = torch.zeros(cfg.n, device="cuda")
             for h in range(steps):
@@ -176,7 +177,7 @@ def test_grid_recurrence_replays_from_a_graph(binding):
             else:                                       # pipelined graphs: the margin is a kernel of its own there
                 assert torch.linalg.norm(xa - xb) <= 1e-5 * torch.linalg.norm(xa)
             xs[impl] = xa
-    for impl in (2, 3, 4):
+    for impl in (2, 3, 4, 5):
         assert torch.linalg.norm(xs[1] - xs[impl]) <= 1e-5 * torch.linalg.norm(xs[1])
 
 
