@@ -95,8 +95,8 @@ struct casgd_ctx {
     GradWorkspace gws{};
     RecWorkspace rws{};
     StepParams *ind = nullptr;
-    int *err_flag = nullptr;
-    int *err_flag_host = nullptr;     // pinned
+    int *err_flag = nullptr;          // device alias of err_flag_host
+    int *err_flag_host = nullptr;     // pinned, mapped
     double *loss_partials = nullptr, *loss_result = nullptr;
     double *loss_result_host = nullptr;   // pinned
     int32_t loss_max_blocks = 0;
@@ -586,6 +586,17 @@ int choose_gram(casgd_ctx *c, int32_t s, int32_t b, bool pipe)
 
 // The BF16 shadow is rebuilt from x at the start of EVERY casgd_outer_step(s) call (one n-element kernel per call, not
 // per step): a pointer-keyed cache would be fooled by an allocator that hands a new iterate the address of a freed one.
+// after a stream synchronize: has a kernel met a row index outside [0, m)? (the flag is mapped pinned host memory)
+int index_error_check(casgd_ctx *c)
+{
+    volatile int *flag = c->err_flag_host;
+    if (*flag) {
+        *flag = 0;
+        return fail(c, CASGD_EINDEX, "a row index outside [0, %lld) was gathered", (long long)c->m);
+    }
+    return CASGD_OK;
+}
+
 int ensure_shadow(casgd_ctx *c, const float *x)
 {
     StageTimer t(c, CASGD_STAGE_OTHER);
@@ -667,7 +678,7 @@ int collect_events(casgd_ctx *c)
 }
 
 int run_steps(casgd_ctx *c, const int32_t *idx, int64_t n_steps, float *x, int32_t s, int32_t b, float eta,
-              bool allow_graph)
+              bool allow_graph, int64_t graph_from = 2)
 {
     const int32_t sb = s * b;
     if (n_steps == 0) return CASGD_OK;
@@ -716,7 +727,7 @@ int run_steps(casgd_ctx *c, const int32_t *idx, int64_t n_steps, float *x, int32
     c->last_s = s;
     c->last_b = b;
     int64_t done = 0;
-    if (allow_graph && !c->opt_profile && !c->opt_no_graph && n_steps >= 2) {
+    if (allow_graph && !c->opt_profile && !c->opt_no_graph && n_steps >= graph_from) {
         static const int32_t lens[3] = {64, 8, 1};
         for (int li = 0; li < 3; ++li) {
             const int32_t len = lens[li];
@@ -813,9 +824,8 @@ int casgd_init(casgd_ctx **out, const uint16_t *X_bf16, int64_t ldx, const float
               ck(cudaMemsetAsync(c->rws.utag, 0, sizeof(unsigned long long) * CASGD_MAX_SB * kRecReplicas, c->stream)) &&
               ck(cudaMalloc(&c->rws.epoch, 2 * sizeof(unsigned))) &&
               ck(cudaMemcpyAsync(c->rws.epoch, kEpochInit, 2 * sizeof(unsigned), cudaMemcpyHostToDevice, c->stream)) &&
-              ck(cudaMalloc(&c->err_flag, sizeof(int))) &&
-              ck(cudaMemsetAsync(c->err_flag, 0, sizeof(int), c->stream)) &&
-              ck(cudaMallocHost(&c->err_flag_host, sizeof(int))) &&
+              ck(cudaHostAlloc(&c->err_flag_host, sizeof(int), cudaHostAllocMapped)) &&
+              ck((*c->err_flag_host = 0, cudaHostGetDevicePointer(&c->err_flag, c->err_flag_host, 0))) &&
               ck(cudaMalloc(&c->loss_partials, sizeof(double) * c->loss_max_blocks)) &&
               ck(cudaMalloc(&c->loss_result, sizeof(double))) &&
               ck(cudaMallocHost(&c->loss_result_host, sizeof(double))) &&
@@ -865,11 +875,12 @@ int casgd_outer_steps_host(casgd_ctx *c, const int32_t *idx_host, int64_t n_step
     if (count > 0) CK(cudaMemcpyAsync(c->idx_stage, idx_host, sizeof(int32_t) * (size_t)count, cudaMemcpyHostToDevice, c->stream));
     CK(cudaMemcpyAsync(c->x_stage, x_host, sizeof(float) * (size_t)c->n, cudaMemcpyHostToDevice, c->stream));
     c->shadow_valid = false;                  // x_stage was overwritten from the host
-    rc = run_steps(c, c->idx_stage, n_steps, c->x_stage, s, b, eta, true);
+    // (a call of ONE step too replays a graph here: one launch instead of five on a stream the host then waits for)
+    rc = run_steps(c, c->idx_stage, n_steps, c->x_stage, s, b, eta, true, 1);
     if (rc) return rc;
     CK(cudaMemcpyAsync(x_host, c->x_stage, sizeof(float) * (size_t)c->n, cudaMemcpyDeviceToHost, c->stream));
     CK(cudaStreamSynchronize(c->stream));
-    return CASGD_OK;
+    return index_error_check(c);
 }
 
 int casgd_outer_steps_sampled(casgd_ctx *c, int64_t n_steps, float *x, int32_t s, int32_t b, float eta, uint64_t seed,
@@ -1034,13 +1045,8 @@ int casgd_invalidate_shadow(casgd_ctx *c)
 int casgd_sync(casgd_ctx *c)
 {
     if (!c) return CASGD_EINVAL;
-    CK(cudaMemcpyAsync(c->err_flag_host, c->err_flag, sizeof(int), cudaMemcpyDeviceToHost, c->stream));
     CK(cudaStreamSynchronize(c->stream));
-    if (*c->err_flag_host) {
-        CK(cudaMemsetAsync(c->err_flag, 0, sizeof(int), c->stream));
-        return fail(c, CASGD_EINDEX, "a row index outside [0, %lld) was gathered", (long long)c->m);
-    }
-    return CASGD_OK;
+    return index_error_check(c);
 }
 
 int casgd_debug_export(casgd_ctx *c, int what, void *dst_host, int64_t dst_bytes)
@@ -1181,7 +1187,7 @@ void casgd_destroy(casgd_ctx *c)
     for (cudaEvent_t e : {c->ev_fork, c->ev_join, c->ev_gather[0], c->ev_gather[1], c->ev_gather[2], c->ev_gram[0], c->ev_gram[1], c->ev_grad, c->ev_rec_launch})
         if (e) cudaEventDestroy(e);
     cudaFree(c->A_owned); cudaFree(c->A32); cudaFree(c->xbf);
-    cudaFree(c->gws.partial); cudaFree(c->gws.counters); cudaFree(c->ind); cudaFree(c->err_flag);
+    cudaFree(c->gws.partial); cudaFree(c->gws.counters); cudaFree(c->ind);
     cudaFree(c->rws.utag); cudaFree(c->rws.epoch); cudaFree(c->stamps);
     cudaFree(c->loss_partials); cudaFree(c->loss_result); cudaFree(c->idx_stage); cudaFree(c->x_stage); cudaFree(c->x_snap);
     if (c->err_flag_host) cudaFreeHost(c->err_flag_host);

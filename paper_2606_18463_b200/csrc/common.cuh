@@ -139,6 +139,9 @@ __device__ __forceinline__ uint4 ldg_nc_v4(const void *p)
 // IMPORTANT: what another kernel of the chain wrote must NOT be read through a `const T *__restrict__` pointer or
 // __ldg: the compiler treats such data as read-only for the whole kernel and may hoist the load ABOVE pdl_wait()
 // (seen: a gradient kernel summing the previous step's u). Such inputs are plain pointers, or go through ld_dep().
+// A row index outside [0, m) was met: raise the context's flag. The flag lives in MAPPED PINNED HOST memory (the host
+// reads it after a stream synchronize, no copy), so a plain store, not an atomic: every writer writes the same 1.
+__device__ __forceinline__ void flag_index_error(int *err_flag) { *reinterpret_cast<volatile int *>(err_flag) = 1; }
 __device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
 __device__ __forceinline__ uint4 ld_dep_v4(const void *p)
 {

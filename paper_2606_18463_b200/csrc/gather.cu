@@ -41,7 +41,7 @@ gather_rows_kernel(const uint16_t *__restrict__ A, int64_t lda, const float *__r
     *reinterpret_cast<uint4 *>(Y + row * (int64_t)ldy + col) = v;
     if (c == 0) {
         yI[row] = ok ? y[src] : 0.f;
-        if (!ok) atomicOr(err_flag, 1);
+        if (!ok) flag_index_error(err_flag);
     }
     stamp_end_warp(stamp);
 }
@@ -82,7 +82,7 @@ gather_bulk_kernel(const uint16_t *__restrict__ A, int64_t lda, const float *__r
         const int64_t src = I[row];
         const bool ok = src >= 0 && src < m;
         yI[row] = ok ? y[src] : 0.f;
-        if (!ok) atomicOr(err_flag, 1);
+        if (!ok) flag_index_error(err_flag);
     }
 
     const uint32_t rowB = (uint32_t)n * 2u;                                 // a multiple of 16

@@ -458,7 +458,7 @@ margin_s1_kernel(const uint16_t *__restrict__ A, int64_t lda, const float *__res
     acc = warp_sum(acc);
     if (lane == 0) {
         const float ylab = ok ? y[src] : 0.f;
-        if (!ok) atomicOr(err_flag, 1);
+        if (!ok) flag_index_error(err_flag);
         yI[row] = ylab;
         r[row] = acc;
         z[row] = acc;
@@ -490,7 +490,7 @@ sgd32_margin_kernel(const float *__restrict__ A32, int64_t lda32, const float *_
     if (warp >= b) return;
     const int64_t src = idx[warp];
     if (src < 0 || src >= m) {
-        if (lane == 0) { z[warp] = 0.f; u[warp] = 0.f; atomicOr(err_flag, 1); }
+        if (lane == 0) { z[warp] = 0.f; u[warp] = 0.f; flag_index_error(err_flag); }
         return;
     }
     const float *a = A32 + src * lda32;

@@ -416,7 +416,7 @@ gram_narrow_kernel(const NarrowParams p)
         int64_t src = -1;
         if (trow < p.sb) {
             src = I[trow];
-            if (src < 0 || src >= p.m) { src = -1; if (diag) atomicOr(p.err_flag, 1); }
+            if (src < 0 || src >= p.m) { src = -1; if (diag) flag_index_error(p.err_flag); }
         }
         const uint32_t trow_s = smem_base + (op == 0 ? kNwOffT0 : kNwOffT1) + threadIdx.x * 128u;
         uint4 v[8];

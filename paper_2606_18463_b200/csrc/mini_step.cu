@@ -153,7 +153,7 @@ mini_step_kernel(const MiniParams p)
             const int64_t src = I[tid];
             const uint32_t off = L.yl + q * L.yl_stride + 4u * (uint32_t)tid;
             if (src >= 0 && src < p.m) cp_async4_ms(smem0 + off, p.y + src);
-            else { *reinterpret_cast<float *>(ms_smem + off) = 0.f; atomicOr(p.err_flag, 1); }
+            else { *reinterpret_cast<float *>(ms_smem + off) = 0.f; flag_index_error(p.err_flag); }
         }
         asm volatile("cp.async.commit_group;" ::: "memory");
     };

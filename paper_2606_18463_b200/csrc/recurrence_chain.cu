@@ -175,52 +175,74 @@ recurrence_chain_kernel(const float *G, int32_t ldg, const float *r, const float
         cluster_sync_all();                             // every CTA's barriers exist; r of the fused margin is complete
         float rr = 0.f, yy = 0.f;
         if (owner) { rr = ld_dep(r + i); yy = ld_dep(yI + i); }
+        // running addresses: everything a hop touches moves by a constant, so the loop carries pointers, not products
+        const int b4 = b >> 2, pstep = 4 * TPR;
+        const int64_t rowstep = (int64_t)b * ldg;
+        const float *srcl = G + (int64_t)(3 * b + i) * ldg + (3 > W ? (3 - W) * b : 0) + 4 * sub;    // hop 3, this lane's piece 0
+        uint32_t uaddr = us + 16u * (uint32_t)sub;      // u of the window's first block, this lane's piece 0
+        uint32_t paddr = ps + 4u * (uint32_t)i, pb = pbar, oaddr = us + 4u * (uint32_t)i;
+        const float *rp = r + b + i, *yp = yI + b + i;
+        float *zp = z + i, *up = u + i;
+        uint32_t sl = s_loc, sr = s_rem, sb_ = s_bar;
 #pragma unroll 1
         for (int j = 0; j < s; ++j) {
             float rn = 0.f, yn = 0.f;                   // r and y of the next hop, a hop ahead
-            if (owner && j + 1 < s) { rn = ld_dep(r + (j + 1) * b + i); yn = ld_dep(yI + (j + 1) * b + i); }
+            if (owner && j + 1 < s) { rn = ld_dep(rp); yn = ld_dep(yp); }
             CT(8 * j);
 #pragma unroll
             for (int q = 0; q < kCcPieces; ++q) { g0[q] = g1[q]; g1[q] = g2[q]; g2[q] = g3[q]; }
             CT(8 * j + 1);
-            load(j + 3, g3);
+            {
+                const int jl = j + 3;
+                const int nchl = jl < s && active ? min(jl, W) * b4 : 0;
+#pragma unroll
+                for (int q = 0; q < kCcPieces; ++q)
+                    g3[q] = sub + TPR * q < nchl ? ldg_nc_f4(srcl + q * pstep) : make_float4(0.f, 0.f, 0.f, 0.f);
+                srcl += rowstep + (jl >= W ? b : 0);
+            }
             CT(8 * j + 7);
             // the older blocks' part of this hop, from the helpers: asked for now, needed after the window's dot
             uint32_t p_ok = 1u;
-            if (owner && j >= W + 1) p_ok = mbar_test(pbar + 8u * j, 0u);
+            float pv = 0.f;
+            const bool need_p = owner && j >= W + 1;
+            if (need_p) p_ok = mbar_test(pb, 0u);
             float acc = 0.f;
             if (j > 0) {
-                const int ncw = min(j, W), nch = active ? ncw * b >> 2 : 0;
-                const uint32_t urow = us + 4u * (uint32_t)((j - ncw) * b);
+                const int nch = active ? min(j, W) * b4 : 0;
+                float4 uv[kCcPieces];
 #pragma unroll
-                for (int q = 0; q < kCcPieces; ++q) {
-                    const int c = sub + TPR * q;
-                    if (c < nch) acc = dot4(g0[q], lds_f4(urow + 16u * c), acc);
-                }
+                for (int q = 0; q < kCcPieces; ++q)
+                    uv[q] = sub + TPR * q < nch ? lds_f4(uaddr + 16u * (uint32_t)(TPR * q)) : make_float4(0.f, 0.f, 0.f, 0.f);
+                const float a0 = dot4(g0[1], uv[1], dot4(g0[0], uv[0], 0.f));
+                const float a1 = dot4(g0[3], uv[3], dot4(g0[2], uv[2], 0.f));
+                acc = a0 + a1;
                 for (int o = TPR >> 1; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
             }
             CT(8 * j + 2);
             if (owner) {
-                if (j >= W + 1) {
-                    while (!p_ok) p_ok = mbar_test(pbar + 8u * j, 0u);
+                if (need_p) {
+                    while (!p_ok) p_ok = mbar_test(pb, 0u);
                     CT(8 * j + 3);
-                    acc += lds_f32(ps + 4u * (uint32_t)(j * b + i));
+                    pv = lds_f32(paddr);
                 }
-                const float zz = fmaf(-alpha, acc, rr);
+                const float zz = fmaf(-alpha, acc + pv, rr);
                 const float uu = lprime_chain<LOSS>(zz, yy);
-                sts_f32(us + 4u * (uint32_t)(j * b + i), uu);
-                z[j * b + i] = zz;
-                u[j * b + i] = uu;
+                sts_f32(oaddr, uu);
+                *zp = zz;
+                *up = uu;
             }
             rr = rn; yy = yn;
             CT(8 * j + 4);
             __syncthreads();                            // u_j is complete
             CT(8 * j + 5);
             if (sender) {
-                const uint32_t off = 4u * (uint32_t)(j * b);
-                const float4 t = lds_f4(s_loc + off);
-                st_async_v4(s_rem + off, t.x, t.y, t.z, t.w, s_bar + 8u * j);
+                const float4 t = lds_f4(sl);
+                st_async_v4(sr, t.x, t.y, t.z, t.w, sb_);
             }
+            const uint32_t bb = 4u * (uint32_t)b;
+            if (j >= W) uaddr += bb;
+            paddr += bb; oaddr += bb; pb += 8u; sl += bb; sr += bb; sb_ += 8u;
+            rp += b; yp += b; zp += b; up += b;
             CT(8 * j + 6);
         }
     } else {

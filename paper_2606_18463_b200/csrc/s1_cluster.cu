@@ -125,7 +125,7 @@ s1_cluster_kernel(const S1Params p)
             const int64_t src = I[tid];
             const uint32_t off = L.yl + q * L.vec_stride + 4u * (uint32_t)tid;
             if (src >= 0 && src < p.m) asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"(smem0 + off), "l"(p.y + src) : "memory");
-            else { *reinterpret_cast<float *>(sc_smem + off) = 0.f; if (crank == 0) atomicOr(p.err_flag, 1); }
+            else { *reinterpret_cast<float *>(sc_smem + off) = 0.f; if (crank == 0) flag_index_error(p.err_flag); }
         }
         asm volatile("cp.async.commit_group;" ::: "memory");
     };

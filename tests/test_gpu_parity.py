@@ -347,6 +347,14 @@ def test_graph_replay_and_host_entry_point_equal_single_steps(binding):
         for h in range(steps):
             cg.outer_steps_host(torch.from_numpy(idx[h * s * b:(h + 1) * s * b].copy()), x1, s, b, cfg.eta, n_steps=1)
         assert torch.equal(xa.cpu(), x1)
+        # the synchronous entry point reports a row index outside [0, m) itself; the next call is clean again
+        bad = idx[: s * b].copy()
+        bad[5] = cfg.m
+        with pytest.raises(binding.CasgdError):
+            cg.outer_steps_host(torch.from_numpy(bad), torch.zeros(cfg.n), s, b, cfg.eta, n_steps=1)
+        x2 = torch.zeros(cfg.n)
+        cg.outer_steps_host(torch.from_numpy(idx[: s * b].copy()), x2, s, b, cfg.eta, n_steps=1)
+        assert torch.isfinite(x2).all()
 
 
 @pytest.mark.parametrize("overlap", [0, 1, 2], ids=["sequential", "gather-aside", "pipelined"])
