@@ -241,7 +241,7 @@ int casgd_debug_export(casgd_ctx *c, int what, void *dst_host, int64_t dst_bytes
  *                              the x half of Eq. 8's 2 u_16 term (L229) at no extra MMA.
  *   CASGD_OPT_MINI             1 (default) = steps small enough for one SM -- two stages of Y, the packed strict
  *                              block-lower G and the vectors within one CTA's shared memory, s*b <= 128, a Gram of at
- *                              most 200K multiply-adds: e.g. n = 64, s*b = 64; at s = 1 a step of <= 32 KB of rows (any
+ *                              most 460K multiply-adds: e.g. n = 64, s*b = 64; at s = 1 a step of <= 32 KB of rows (any
  *                              size for rows of <= 128 bytes), s*b <= 512 -- run ALL the iterations of a
  *                              casgd_outer_step(s) call in ONE persistent one-CTA launch (gather with the next
  *                              iteration's rows in flight, mma.sync Gram, recurrence, update, x resident in shared

@@ -16,6 +16,7 @@
 // The last iteration's Y, y_I, G, r, z, u go to the context's workspaces (casgd_debug_export); x and its BF16 shadow
 // are written back at the end. Same arithmetic classes as the big kernels (exact BF16 products, FP32 accumulation).
 #include "common.cuh"
+#include "rec_cluster.cuh"                  // lprime_chain
 
 namespace casgd {
 
@@ -45,7 +46,7 @@ struct MiniParams {
 // Byte offsets into dynamic shared memory. Two stages of Y, of the labels and of the indices: stage q at base + q * stride
 // (scalars, not arrays indexed at run time: those end up in local memory, on every access of every phase).
 struct MiniLayout {
-    uint32_t x, r, z, u, yl, yl_stride, idx, idx_stride, gl, red, Y, Y_stride, total;
+    uint32_t x, xm, r, z, u, yl, yl_stride, idx, idx_stride, gl, red, Y, Y_stride, total;
     int32_t ldys, sbp;                  // row stride of a Y stage in elements (16-byte multiple, staggered banks); rows incl. padding
 };
 
@@ -58,6 +59,7 @@ __host__ __device__ inline MiniLayout mini_layout(int n, int s, int b)
     uint32_t o = 0;
     auto take = [&](uint32_t bytes) { const uint32_t at = o; o += (bytes + 15u) & ~15u; return at; };
     L.x = take(4u * (uint32_t)n);
+    L.xm = take(4u * (uint32_t)((n + 7) & ~7));           // the margin's view of x: bf16-rounded (or x itself), zero-padded
     L.r = take(4u * sb); L.z = take(4u * sb); L.u = take(4u * sb);
     L.yl_stride = (4u * sb + 15u) & ~15u;  L.yl = take(2u * L.yl_stride);
     L.idx_stride = L.yl_stride;            L.idx = take(2u * L.idx_stride);
@@ -108,6 +110,7 @@ mini_step_kernel(const MiniParams p)
     const MiniLayout L = mini_layout(n, s, b);
     const int ldys = L.ldys;
     float *xs = reinterpret_cast<float *>(ms_smem + L.x);
+    float *xm = reinterpret_cast<float *>(ms_smem + L.xm);
     float *rs = reinterpret_cast<float *>(ms_smem + L.r);
     float *zs = reinterpret_cast<float *>(ms_smem + L.z);
     float *us = reinterpret_cast<float *>(ms_smem + L.u);
@@ -122,7 +125,11 @@ mini_step_kernel(const MiniParams p)
     pdl_wait();                                         // x and the index buffer come from earlier work on the stream
     stamp_begin(p.stamp);
 #pragma unroll 1
-    for (int k = tid; k < n; k += nthr) xs[k] = p.x[k];
+    for (int k = tid; k < ldy; k += nthr) {
+        const float t = k < n ? p.x[k] : 0.f;
+        if (k < n) xs[k] = t;
+        xm[k] = p.exact_margin ? t : bf16_round(t);
+    }
     if (tid < sb) {                                     // (sb <= 512: one index per thread and stage)
         reinterpret_cast<int32_t *>(ms_smem + L.idx)[tid] = p.idx[tid];
         if (p.n_steps > 1) reinterpret_cast<int32_t *>(ms_smem + L.idx + L.idx_stride)[tid] = p.idx[sb + tid];
@@ -159,9 +166,10 @@ mini_step_kernel(const MiniParams p)
     };
     if (p.n_steps > 0) issue_gather(0);
 
-    int LG = 1;                                         // margin: lanes side by side on a row (<= 32)
-    while (LG < chunks && LG < 32) LG <<= 1;
-    const int msub = tid & (LG - 1), mrows = nthr / LG;
+    int LG = 1, lgs = 0;                                // margin: lanes side by side on a row (<= 32)
+    while (LG < chunks && LG < 32) { LG <<= 1; ++lgs; }
+    const int msub = tid & (LG - 1), mrow = tid >> lgs, mrows = nthr >> lgs;
+    const uint32_t inv_b = ((1u << 20) + (uint32_t)b - 1u) / (uint32_t)b;    // floor(i / b) = i * inv_b >> 20 for i b < 2^20
 
 #pragma unroll 1
     for (int64_t step = 0; step < p.n_steps; ++step) {
@@ -188,46 +196,48 @@ mini_step_kernel(const MiniParams p)
         // ---- margin (line 3): a group of LG lanes per row, 8 columns per lane and pass
 #pragma unroll 1
         for (int i0 = 0; i0 < sb; i0 += mrows) {        // (uniform trip count: every lane takes part in the shuffles)
-            const int i = i0 + tid / LG;
-            float acc = 0.f;
+            const int i = i0 + mrow;
+            float acc = 0.f, acc2 = 0.f;
 #pragma unroll 1
             for (int c = msub; c < chunks && i < sb; c += LG) {
                 const uint4 v = *reinterpret_cast<const uint4 *>(Ys + i * ldys + c * 8);
-                float xe[8];
-#pragma unroll
-                for (int e = 0; e < 8; ++e) {
-                    const float t = c * 8 + e < n ? xs[c * 8 + e] : 0.f;
-                    xe[e] = p.exact_margin ? t : bf16_round(t);
-                }
-                acc = fmaf(bf16lo(v.x), xe[0], acc); acc = fmaf(bf16hi(v.x), xe[1], acc);
-                acc = fmaf(bf16lo(v.y), xe[2], acc); acc = fmaf(bf16hi(v.y), xe[3], acc);
-                acc = fmaf(bf16lo(v.z), xe[4], acc); acc = fmaf(bf16hi(v.z), xe[5], acc);
-                acc = fmaf(bf16lo(v.w), xe[6], acc); acc = fmaf(bf16hi(v.w), xe[7], acc);
+                const float4 xa = *reinterpret_cast<const float4 *>(xm + c * 8), xb = *reinterpret_cast<const float4 *>(xm + c * 8 + 4);
+                acc = fmaf(bf16lo(v.x), xa.x, acc); acc2 = fmaf(bf16hi(v.x), xa.y, acc2);
+                acc = fmaf(bf16lo(v.y), xa.z, acc); acc2 = fmaf(bf16hi(v.y), xa.w, acc2);
+                acc = fmaf(bf16lo(v.z), xb.x, acc); acc2 = fmaf(bf16hi(v.z), xb.y, acc2);
+                acc = fmaf(bf16lo(v.w), xb.z, acc); acc2 = fmaf(bf16hi(v.w), xb.w, acc2);
             }
+            acc += acc2;
             MT(10);
             for (int o = LG >> 1; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
             MT(11);
             if (msub == 0 && i < sb) {
                 rs[i] = acc;
-                if (s == 1) { zs[i] = acc; us[i] = lprime<LOSS>(acc, yl[i]); }
+                zs[i] = acc;                            // (s > 1: the recurrence starts from z = r)
+                if (s == 1) us[i] = lprime_chain<LOSS>(acc, yl[i]);
             }
         }
 
         MT(3);
-        // ---- Gram (line 4): 16 x 8 tiles of the strict block-lower part, mma.sync from the row-major stage
+        // ---- Gram (line 4): 16 x 8 tiles of the strict block-lower part, mma.sync from the row-major stage; the tiles
+        // of all row tiles form ONE job list dealt to the warps. G lands TRANSPOSED inside each b x b block --
+        // entry (i, k), block(i) = jr > block(k) = jc, at  b^2 jr (jr-1) / 2 + jc b^2 + (k - jc b) b + (i - jr b) --
+        // so that the recurrence below reads it with consecutive threads on consecutive words.
         if (s > 1) {
             const int g = lane >> 2, t4 = lane & 3;
             const int TR = L.sbp >> 4, ksteps = (ldys - 8) >> 4;
+            int first = 0, job = warp;                  // jobs before this row tile; this warp's next job
 #pragma unroll 1
             for (int tr = 0; tr < TR; ++tr) {           // (a row tile inside block 0 has no columns: ntc = 0)
                 const int row_hi = min(tr * 16 + 15, sb - 1);
                 const int ntc = ((row_hi / b) * b + 7) >> 3;    // 8-column tiles that hold a block below some row of the tile
 #pragma unroll 1
-                for (int tc = warp; tc < ntc; tc += nwarp) {
+                for (; job < first + ntc; job += nwarp) {
+                    const int tc = job - first;
                     float c[4] = {0.f, 0.f, 0.f, 0.f};
                     const uint16_t *arow0 = Ys + (tr * 16 + g) * ldys + 2 * t4, *arow1 = arow0 + 8 * ldys;
                     const uint16_t *brow = Ys + (tc * 8 + g) * ldys + 2 * t4;
-#pragma unroll 1
+#pragma unroll 2
                     for (int ks = 0; ks < ksteps; ++ks) {
                         uint32_t a[4], bq[2];
                         a[0] = *reinterpret_cast<const uint32_t *>(arow0 + ks * 16);
@@ -241,35 +251,42 @@ mini_step_kernel(const MiniParams p)
 #pragma unroll
                     for (int e = 0; e < 4; ++e) {
                         const int i = tr * 16 + g + (e >> 1) * 8, k = tc * 8 + 2 * t4 + (e & 1);
-                        const int j = i / b;
-                        if (i < sb && k < j * b) gl[(b * b * j * (j - 1)) / 2 + (i - j * b) * j * b + k] = c[e];
+                        const int jr = (int)((uint32_t)i * inv_b >> 20), jc = (int)((uint32_t)k * inv_b >> 20);
+                        if (i < sb && jc < jr) gl[(b * b * jr * (jr - 1)) / 2 + jc * b * b + (k - jc * b) * b + (i - jr * b)] = c[e];
                     }
                 }
+                first += ntc;
             }
         }
         __syncthreads();
         MT(4);
 
-        // ---- recurrence (lines 6-15): a warp per row of block j, one barrier per inner step
+        // ---- recurrence (lines 6-15), right-looking, a THREAD per row (s b <= the threads): the margin left z = r;
+        // per inner step the rows of block j apply l', one barrier, and every later row takes block j's b columns off
+        // its own z -- the rows of block j + 1 are then final without another barrier.
         if (s > 1) {
+            const int jr = tid / b, il = tid - jr * b;  // this thread's row: block and row inside it
+            const float *gmine = gl + (b * b * jr * (jr - 1)) / 2 + il;
+            float zmine = tid < sb ? zs[tid] : 0.f;
 #pragma unroll 1
             for (int j = 0; j < s; ++j) {
-                const int len = j * b;
-                const float *gblk = gl + (b * b * j * (j - 1)) / 2;
-#pragma unroll 1
-                for (int i = j * b + warp; i < (j + 1) * b; i += nwarp) {
-                    float acc = 0.f;
-                    const float *grow = gblk + (i - j * b) * len;
-#pragma unroll 1
-                    for (int k = lane; k < len; k += 32) acc = fmaf(grow[k], us[k], acc);
-                    acc = warp_sum(acc);
-                    if (lane == 0) {
-                        const float zz = fmaf(-p.alpha, acc, rs[i]);
-                        zs[i] = zz;
-                        us[i] = lprime<LOSS>(zz, yl[i]);
-                    }
+                if (tid < sb && jr == j) {
+                    zs[tid] = zmine;
+                    us[tid] = lprime_chain<LOSS>(zmine, yl[tid]);
                 }
                 __syncthreads();
+                if (tid < sb && jr > j) {
+                    const float *gcol = gmine + j * b * b, *uj = us + j * b;
+                    float a0 = 0.f, a1 = 0.f;
+                    int k = 0;
+#pragma unroll 4
+                    for (; k + 1 < b; k += 2) {
+                        a0 = fmaf(gcol[k * b], uj[k], a0);
+                        a1 = fmaf(gcol[(k + 1) * b], uj[k + 1], a1);
+                    }
+                    if (k < b) a0 = fmaf(gcol[k * b], uj[k], a0);
+                    zmine = fmaf(-p.alpha, a0 + a1, zmine);
+                }
             }
         }
 
@@ -304,7 +321,9 @@ mini_step_kernel(const MiniParams p)
                 float gsum = 0.f;
 #pragma unroll 4
                 for (int r2 = 0; r2 < nred; ++r2) gsum += red[r2 * ldy + col];
-                xs[col] = fmaf(-p.alpha, gsum, xs[col]);
+                const float xn = fmaf(-p.alpha, gsum, xs[col]);
+                xs[col] = xn;
+                xm[col] = p.exact_margin ? xn : bf16_round(xn);
             }
         }
 
@@ -319,9 +338,9 @@ mini_step_kernel(const MiniParams p)
 #pragma unroll 1
             for (int i = b + warp; i < sb; i += nwarp) {
                 const int j = i / b;
-                const float *grow = gl + (b * b * j * (j - 1)) / 2 + (i - j * b) * j * b;
+                const float *gt = gl + (b * b * j * (j - 1)) / 2 + (i - j * b);      // (k, i) of the row block, transposed blocks
 #pragma unroll 1
-                for (int k = lane; k < j * b; k += 32) p.G[(int64_t)i * p.ldg + k] = grow[k];
+                for (int k = lane; k < j * b; k += 32) p.G[(int64_t)i * p.ldg + k] = gt[k * b];
             }
         }
         if (step + 2 < p.n_steps && tid < sb) reinterpret_cast<int32_t *>(ms_smem + L.idx + q * L.idx_stride)[tid] = idx_next;
@@ -367,12 +386,13 @@ bool mini_step_ok(int32_t n, int32_t ldy, int32_t s, int32_t b, bool any_fit)
     // measured crossovers against the kernel-per-stage path (us per iteration): s = 1 wins up to 32 KB of rows per step
     // (n = 18, b = 64: 1.4 against 7.2; n = 128, b = 128: 4.0 against 6.3; n = 128, b = 256: 9.0 against 7.2) and for
     // rows of <= 128 bytes at any b (n = 64, b = 512: 5.8 against 10.3); steps beyond 4 KB with rows of >= 128 bytes go to the
-    // cluster kernel first (s1_cluster.cu; n = 256, b = 64: 1.9 against 5.2 here). s > 1 wins while Gram and chain are tiny (n = 64,
-    // s = 4, b = 16: 5.1 against 7.8; n = 128: 6.5 against 8.0; n = 256, s = 2, b = 32: 8.9 against 7.6)
+    // cluster kernel first (s1_cluster.cu; n = 256, b = 64: 1.9 against 5.2 here). s > 1 wins while Gram and chain are tiny
+    // (n = 64, s = 4, b = 16: 3.7 against 8.0; n = 64, s = 8, b = 16: 8.5 against 9.4; n = 128, s = 4, b = 32: 9.1 against
+    // 8.0; n = 512, s = 2, b = 32: 10.7 against 8.0)
     if (any_fit) return true;                           // CASGD_OPT_MINI = 2: the structural limits only
     if (s == 1) return (int64_t)b * ldy * 2 <= 32 * 1024 || ldy <= 64;
     const int64_t macs = (int64_t)((n + 15) & ~15) * b * b * s * (s - 1) / 2;
-    return sb <= 128 && macs <= (200ll << 10) && (int64_t)s * ((b + kMsMaxWarps - 1) / kMsMaxWarps) <= 16;
+    return sb <= 128 && macs <= (460ll << 10) && (int64_t)s * ((b + kMsMaxWarps - 1) / kMsMaxWarps) <= 16;
 }
 
 int launch_mini_steps(cudaStream_t st, const uint16_t *A, int64_t lda, const float *y, int64_t m, int32_t n, int32_t ldy,
