@@ -108,7 +108,9 @@ int casgd_outer_steps_sampled(casgd_ctx *c, int64_t n_steps, float *x, int32_t s
 /* The same through HOST buffers: copies idx_host (n_steps*s*b int32) and x_host (n FP32) to the
  * device, runs the steps, copies x back into x_host, and synchronises. Pinned host memory makes the
  * copies asynchronous with respect to the host but the call still returns only when x_host is valid; a call of one
- * step replays a one-step CUDA graph (one launch on a stream the host then waits for). A row index outside [0, m) is
+ * step replays a one-step CUDA graph (one launch on a stream the host then waits for), and when both buffers are pinned
+ * MAPPED host memory (cudaHostAlloc, torch's pin_memory()) and the call moves <= 64 KB of indices, one kernel reads them
+ * in place and one writes x back -- no copy-engine round trips. A row index outside [0, m) is
  * reported here (CASGD_EINDEX; the row counts as zeros), as casgd_sync reports it for the asynchronous calls. */
 int casgd_outer_steps_host(casgd_ctx *c, const int32_t *idx_host, int64_t n_steps, float *x_host, int32_t s,
                            int32_t b, float eta);

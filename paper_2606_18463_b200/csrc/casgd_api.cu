@@ -95,6 +95,9 @@ struct casgd_ctx {
     GradWorkspace gws{};
     RecWorkspace rws{};
     StepParams *ind = nullptr;
+    bool shadow_fresh = false;        // the shadow was built by the call in progress (host entry point)
+    const int32_t *ind_idx = nullptr; // what the StepParams block on the device currently holds
+    float *ind_x = nullptr;
     int *err_flag = nullptr;          // device alias of err_flag_host
     int *err_flag_host = nullptr;     // pinned, mapped
     double *loss_partials = nullptr, *loss_result = nullptr;
@@ -586,6 +589,14 @@ int choose_gram(casgd_ctx *c, int32_t s, int32_t b, bool pipe)
 
 // The BF16 shadow is rebuilt from x at the start of EVERY casgd_outer_step(s) call (one n-element kernel per call, not
 // per step): a pointer-keyed cache would be fooled by an allocator that hands a new iterate the address of a freed one.
+// The device alias of a pinned, mapped host pointer (what torch's pin_memory() and cudaHostAlloc give), or null.
+void *mapped_alias(const void *host_ptr)
+{
+    cudaPointerAttributes at;
+    if (cudaPointerGetAttributes(&at, host_ptr) != cudaSuccess) { cudaGetLastError(); return nullptr; }
+    return at.type == cudaMemoryTypeHost ? at.devicePointer : nullptr;
+}
+
 // after a stream synchronize: has a kernel met a row index outside [0, m)? (the flag is mapped pinned host memory)
 int index_error_check(casgd_ctx *c)
 {
@@ -722,7 +733,11 @@ int run_steps(casgd_ctx *c, const int32_t *idx, int64_t n_steps, float *x, int32
     }
     rc = choose_gram(c, s, b, false);
     if (rc) return rc;
-    rc = ensure_shadow(c, x);
+    // (rebuilt on every call -- the caller may have changed x, or handed over another tensor at the same address --
+    // unless the host entry point has just built it together with its copy of x)
+    if (c->shadow_fresh && c->shadow_of == x) rc = CASGD_OK;
+    else rc = ensure_shadow(c, x);
+    c->shadow_fresh = false;
     if (rc) return rc;
     c->last_s = s;
     c->last_b = b;
@@ -736,7 +751,11 @@ int run_steps(casgd_ctx *c, const int32_t *idx, int64_t n_steps, float *x, int32
             rc = get_graph(c, s, b, eta, len, &ge);
             if (rc) return rc;
             while (n_steps - done >= len) {
-                c->launches += launch_set_params(c->stream, c->ind, idx + done * sb, x);
+                if (c->ind_idx != idx + done * sb || c->ind_x != x) {      // (the same buffers as last time: nothing to rewrite)
+                    c->launches += launch_set_params(c->stream, c->ind, idx + done * sb, x);
+                    c->ind_idx = idx + done * sb;
+                    c->ind_x = x;
+                }
                 CK(cudaGraphLaunch(ge.exec, c->stream));
                 c->launches += ge.kernels;
                 c->last_buf = ge.last_buf;
@@ -872,13 +891,30 @@ int casgd_outer_steps_host(casgd_ctx *c, const int32_t *idx_host, int64_t n_step
         CK(cudaMalloc(&c->idx_stage, sizeof(int32_t) * (size_t)count));
         c->idx_stage_cap = count;
     }
-    if (count > 0) CK(cudaMemcpyAsync(c->idx_stage, idx_host, sizeof(int32_t) * (size_t)count, cudaMemcpyHostToDevice, c->stream));
-    CK(cudaMemcpyAsync(c->x_stage, x_host, sizeof(float) * (size_t)c->n, cudaMemcpyHostToDevice, c->stream));
-    c->shadow_valid = false;                  // x_stage was overwritten from the host
+    // small steps in pinned (mapped) host memory: kernels read and write the host buffers directly
+    const int32_t *idx_alias = nullptr;
+    float *x_alias = nullptr;
+    if (count * 4 <= (64 << 10) && (int64_t)c->n * 4 <= (256 << 10)) {
+        idx_alias = static_cast<const int32_t *>(mapped_alias(idx_host));
+        x_alias = static_cast<float *>(mapped_alias(x_host));
+    }
+    const bool zero_copy = idx_alias && x_alias;
+    if (zero_copy) {
+        c->launches += launch_stage_in(c->stream, idx_alias, count, c->idx_stage, x_alias, c->n, c->x_stage, c->xbf, c->ldxb,
+                                       (int)c->opt_split);
+        c->shadow_of = c->x_stage;
+        c->shadow_valid = true;
+        c->shadow_fresh = true;
+    } else {
+        if (count > 0) CK(cudaMemcpyAsync(c->idx_stage, idx_host, sizeof(int32_t) * (size_t)count, cudaMemcpyHostToDevice, c->stream));
+        CK(cudaMemcpyAsync(c->x_stage, x_host, sizeof(float) * (size_t)c->n, cudaMemcpyHostToDevice, c->stream));
+        c->shadow_valid = false;              // x_stage was overwritten from the host
+    }
     // (a call of ONE step too replays a graph here: one launch instead of five on a stream the host then waits for)
     rc = run_steps(c, c->idx_stage, n_steps, c->x_stage, s, b, eta, true, 1);
     if (rc) return rc;
-    CK(cudaMemcpyAsync(x_host, c->x_stage, sizeof(float) * (size_t)c->n, cudaMemcpyDeviceToHost, c->stream));
+    if (zero_copy) c->launches += launch_stage_out(c->stream, c->x_stage, c->n, x_alias);
+    else CK(cudaMemcpyAsync(x_host, c->x_stage, sizeof(float) * (size_t)c->n, cudaMemcpyDeviceToHost, c->stream));
     CK(cudaStreamSynchronize(c->stream));
     return index_error_check(c);
 }

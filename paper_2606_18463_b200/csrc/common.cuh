@@ -334,6 +334,9 @@ int launch_shadow(cudaStream_t st, const float *x, const StepParams *ind, int32_
 int launch_widen(cudaStream_t st, const uint16_t *A, int64_t lda, int64_t m, int32_t n, float *A32, int64_t lda32, int num_sms);
 int launch_repack(cudaStream_t st, const uint16_t *X, int64_t ldx, int64_t m, int32_t n, uint16_t *A, int64_t lda, int num_sms);
 int launch_set_params(cudaStream_t st, StepParams *ind, const int32_t *idx, float *x);
+int launch_stage_in(cudaStream_t st, const int32_t *idx_host, int64_t count, int32_t *idx_stage, const float *x_host, int32_t n,
+                    float *x_stage, uint16_t *xbf, int32_t ldxb, int split);
+int launch_stage_out(cudaStream_t st, const float *x_stage, int32_t n, float *x_host);
 // slots: [nslots][2] {min start, max end} in %globaltimer ns, slot = 8 * step + stage; accum_ns / count: [8]
 int launch_stamp_collect(cudaStream_t st, unsigned long long *slots, int nslots, unsigned long long *accum_ns,
                          unsigned long long *count, unsigned long long *raw_copy);

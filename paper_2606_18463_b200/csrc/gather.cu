@@ -272,6 +272,48 @@ int launch_stamp_collect(cudaStream_t st, unsigned long long *slots, int nslots,
     return 1;
 }
 
+// casgd_outer_steps_host with pinned host buffers and a small step: ONE kernel reads the indices and x straight from the
+// mapped host memory (no copy-engine round trips: each cudaMemcpyAsync of 16 KB costs ~5 us of latency on a stream the
+// host is waiting for), writes the device stages and builds the BF16 shadow; a second one writes x back after the steps.
+__global__ void __launch_bounds__(256)
+stage_in_kernel(const int32_t *idx_host, int64_t count, int32_t *idx_stage, const float *x_host, int32_t n, float *x_stage,
+                uint16_t *xbf, int32_t ldxb, int split)
+{
+    pdl_trigger();
+    pdl_wait();
+    const int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x, T = (int64_t)gridDim.x * blockDim.x;
+    for (int64_t k = t; k < count; k += T) idx_stage[k] = idx_host[k];
+    for (int64_t k = t; k < n; k += T) {
+        const float v = x_host[k];
+        x_stage[k] = v;
+        store_shadow(xbf, split ? ldxb : 0, (int32_t)k, v);
+        if (!split) xbf[ldxb + k] = xbf[2 * ldxb + k] = 0;
+    }
+}
+
+__global__ void __launch_bounds__(256)
+stage_out_kernel(const float *x_stage, int32_t n, float *x_host)
+{
+    pdl_trigger();
+    pdl_wait();
+    for (int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; k < n; k += (int64_t)gridDim.x * blockDim.x) x_host[k] = ld_dep(x_stage + k);
+}
+
+int launch_stage_in(cudaStream_t st, const int32_t *idx_host, int64_t count, int32_t *idx_stage, const float *x_host, int32_t n,
+                    float *x_stage, uint16_t *xbf, int32_t ldxb, int split)
+{
+    const int64_t work = std::max<int64_t>(count, n);
+    const int blocks = (int)std::min<int64_t>(148, (work + 255) / 256);
+    launch_pdl(stage_in_kernel, dim3(blocks), dim3(256), 0, st, 1, idx_host, count, idx_stage, x_host, n, x_stage, xbf, ldxb, split);
+    return 1;
+}
+
+int launch_stage_out(cudaStream_t st, const float *x_stage, int32_t n, float *x_host)
+{
+    launch_pdl(stage_out_kernel, dim3(std::min(148, (n + 255) / 256)), dim3(256), 0, st, 1, x_stage, n, x_host);
+    return 1;
+}
+
 __global__ void set_params_kernel(StepParams *ind, const int32_t *idx, float *x)
 {
     pdl_trigger();
