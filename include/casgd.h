@@ -253,7 +253,8 @@ int casgd_debug_export(casgd_ctx *c, int what, void *dst_host, int64_t dst_bytes
  *                              cluster that splits the columns
  *                              (s1_cluster.cu). 0 = always the kernel-per-stage path. 2 = the one-CTA launch whenever the
  *                              step FITS it (s*b <= 512, n <= 2048, shared memory), measured crossovers ignored: for
- *                              tests and for measuring those crossovers.
+ *                              tests and for measuring those crossovers. 3 = likewise the cluster kernel whenever an
+ *                              s = 1 step fits it.
  *   CASGD_OPT_SNAPSHOT         1 = the graphs of casgd_outer_steps copy x aside before their last step (CASGD_DBG_XSNAP):
  *                              test support, one n-element kernel per graph.
  *   CASGD_OPT_LOSS_IMPL        0 = casgd_loss streams A through per-warp cp.async.bulk shared-memory rings

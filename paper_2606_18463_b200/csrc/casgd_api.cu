@@ -297,6 +297,7 @@ inline bool step_is_s1(const casgd_ctx *c, int32_t s)
 }
 // pipelined schedule: not at s = 1 (no Gram), and not with the recurrence kernels that want the whole chip or trigger
 // their dependents early (the grid-wide cooperative kernel, the plain-load cluster kernel)
+constexpr int64_t kClusterFromBytes = 4096;            // s = 1: steps beyond this go to s1_cluster.cu first (measured)
 inline bool pipelined_mode(const casgd_ctx *c, int32_t s, int32_t b)
 {
     if (c->opt_overlap != 2 || s == 1 || c->num_sms < 64) return false;
@@ -698,8 +699,8 @@ int run_steps(casgd_ctx *c, const int32_t *idx, int64_t n_steps, float *x, int32
     // tiny steps: all n_steps iterations in ONE persistent one-CTA launch (mini_step.cu) -- unless a kernel was asked for
     if (c->opt_mini && !c->opt_gram_impl && !c->opt_rec_impl && !c->opt_no_fuse && !c->opt_full_lower && !c->opt_profile &&
         c->lda % 8 == 0 && mini_step_ok(c->n, c->ldy, s, b, c->opt_mini == 2) &&
-        !(s == 1 && c->opt_mini == 1 && (int64_t)b * c->ldy * 2 > 4096 &&
-          s1_cluster_ok(c->n, c->ldy, b, c->rws.cluster))) {    // (s = 1 beyond 4 KB of rows: the cluster, below)
+        !(s == 1 && (c->opt_mini == 3 || (c->opt_mini == 1 && (int64_t)b * c->ldy * 2 > kClusterFromBytes)) &&
+          s1_cluster_ok(c->n, c->ldy, b, c->rws.cluster))) {    // (s = 1 beyond a few KB of rows: the cluster, below)
         c->cur_slot_step = 0;
         StageTimer t(c, CASGD_STAGE_GRAM);
         const int k = launch_mini_steps(c->stream, c->A, c->lda, c->y, c->m, c->n, c->ldy, idx, n_steps, s, b, eta / (float)b, c->loss,
@@ -1164,7 +1165,7 @@ int casgd_set_option(casgd_ctx *c, int option, int64_t value)
         if (value < 0 || value > 2) return fail(c, CASGD_EINVAL, "CASGD_OPT_OVERLAP must be 0, 1 or 2");
         c->opt_overlap = value; break;
     case CASGD_OPT_MARGIN_SPLIT: c->opt_split = value != 0; break;
-    case CASGD_OPT_MINI: c->opt_mini = value < 0 ? 0 : value > 2 ? 2 : value; break;
+    case CASGD_OPT_MINI: c->opt_mini = value < 0 ? 0 : value > 3 ? 3 : value; break;
     case CASGD_OPT_SNAPSHOT: c->opt_snapshot = value != 0; break;
     case CASGD_OPT_CHAIN_SMS:
         if (value < 0 || value > 1024) return fail(c, CASGD_EINVAL, "CASGD_OPT_CHAIN_SMS must be in [0, 1024]");

@@ -5,12 +5,13 @@
 // CTA c of C holds columns [c0, c1) of x in shared memory for the whole call and, per iteration,
 //   gathers its column slice of the b sampled rows (Alg. 1 line 2; 16-byte cp.async, the next iteration's slice in flight),
 //   forms the partial margins  p_c[i] = Y[i, c0:c1] . x_hat[c0:c1]  (line 3) and stores them into EVERY CTA of the cluster
-//   (distributed shared memory) -- the one exchange of an iteration, b floats per CTA pair --
-//   after a cluster barrier adds the C partials in rank order (every CTA gets the same bits), applies l' (lines 6-15 at
+//   (st.async into distributed shared memory, counted on the receiver's mbarrier) -- the one exchange of an iteration,
+//   b floats per CTA pair -- and, once its own C * b partials have landed, adds them in rank order (every CTA gets the same bits), applies l' (lines 6-15 at
 //   s = 1), and updates its own columns: x[c0:c1] -= alpha * Y[:, c0:c1]^T u (lines 16-17).
 // No Gram, no recurrence, no global-memory round trip between the margin and the update, no kernel boundary per step:
 // the kernel-per-stage path needs two launches and ~7-11 us per step here, and so does the FP32 baseline.
 #include "common.cuh"
+#include "rec_cluster.cuh"                  // lprime_chain
 
 namespace casgd {
 
@@ -39,7 +40,7 @@ struct S1Params {
 // two stages of the labels, the indices, the receive buffers and the Y slice: stage q at base + q * stride (scalars: an
 // array of offsets indexed at run time lives in local memory)
 struct S1Layout {
-    uint32_t x, u, yl, idx, vec_stride, recv, recv_stride, red, Y, Y_stride, total;
+    uint32_t x, xm, u, yl, idx, vec_stride, recv, recv_stride, red, Y, Y_stride, total;
     int32_t lds;                                    // row stride of a Y slice in elements
 };
 
@@ -50,6 +51,7 @@ __host__ __device__ inline S1Layout s1_layout(int b, int cpc, int C)
     uint32_t o = 0;
     auto take = [&](uint32_t bytes) { const uint32_t at = o; o += (bytes + 15u) & ~15u; return at; };
     L.x = take(4u * cpc);
+    L.xm = take(4u * cpc);                             // the margin's view of the slice: bf16-rounded, or x itself
     L.u = take(4u * b);
     L.vec_stride = (4u * b + 15u) & ~15u;
     L.yl = take(2u * L.vec_stride);
@@ -76,6 +78,7 @@ __global__ void __launch_bounds__(kScThreads, 1)
 s1_cluster_kernel(const S1Params p)
 {
     extern __shared__ __align__(128) unsigned char sc_smem[];
+    __shared__ __align__(8) unsigned long long sc_bars[2];       // one per receive buffer: C * b * 4 bytes complete a phase
     pdl_trigger();
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int C = (int)sc_size(), crank = (int)sc_rank();
@@ -86,6 +89,7 @@ s1_cluster_kernel(const S1Params p)
     const int ncol = max(0, min(cpc, p.ldy - c0));       // columns of the (padded) row this CTA holds
     const int chunks = ncol >> 3;
     float *xs = reinterpret_cast<float *>(sc_smem + L.x);
+    float *xm = reinterpret_cast<float *>(sc_smem + L.xm);
     float *us = reinterpret_cast<float *>(sc_smem + L.u);
     float *red = reinterpret_cast<float *>(sc_smem + L.red);
     const uint32_t smem0 = (uint32_t)__cvta_generic_to_shared(sc_smem);
@@ -96,7 +100,11 @@ s1_cluster_kernel(const S1Params p)
     pdl_wait();
     stamp_begin(p.stamp);
 #pragma unroll 1
-    for (int k = tid; k < cpc; k += kScThreads) xs[k] = c0 + k < n ? p.x[c0 + k] : 0.f;
+    for (int k = tid; k < cpc; k += kScThreads) {
+        const float t = c0 + k < n ? p.x[c0 + k] : 0.f;
+        xs[k] = t;
+        xm[k] = p.exact_margin ? t : __bfloat162float(__float2bfloat16_rn(t));
+    }
     if (tid < b) {                                      // (b <= 256 = the threads: one index per thread and stage)
         reinterpret_cast<int32_t *>(sc_smem + L.idx)[tid] = p.idx[tid];
         if (p.n_steps > 1) reinterpret_cast<int32_t *>(sc_smem + L.idx + L.vec_stride)[tid] = p.idx[b + tid];
@@ -130,11 +138,17 @@ s1_cluster_kernel(const S1Params p)
         asm volatile("cp.async.commit_group;" ::: "memory");
     };
     if (p.n_steps > 0) issue_gather(0);
-    sc_cluster_sync();                                  // every CTA's receive buffers exist (and are zero) before anyone stores
+    const uint32_t bar0 = (uint32_t)__cvta_generic_to_shared(sc_bars), rx_bytes = 4u * (uint32_t)(C * b);
+    if (tid == 0) {
+        mbar_init(bar0, 1); mbar_init(bar0 + 8u, 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        mbar_expect_tx(bar0, rx_bytes); mbar_expect_tx(bar0 + 8u, rx_bytes);
+    }
+    sc_cluster_sync();                                  // every CTA's receive buffers and barriers exist before anyone stores
 
-    int LG = 1;
-    while (LG < chunks && LG < 32) LG <<= 1;            // lanes side by side on a row slice
-    const int rows_per_pass = kScThreads / LG, sub = tid & (LG - 1);
+    int LG = 1, lgs = 0;
+    while (LG < chunks && LG < 32) { LG <<= 1; ++lgs; }  // lanes side by side on a row slice
+    const int rows_per_pass = kScThreads >> lgs, sub = tid & (LG - 1), mrow = tid >> lgs;
     const uint32_t recv_rank_off = 4u * (uint32_t)(crank * b);
 
 #pragma unroll 1
@@ -158,20 +172,18 @@ s1_cluster_kernel(const S1Params p)
         // ---- partial margins of this column slice, into every CTA's receive buffer
 #pragma unroll 1
         for (int i0 = 0; i0 < b; i0 += rows_per_pass) {
-            const int i = i0 + tid / LG;
-            float acc = 0.f;
+            const int i = i0 + mrow;
+            float acc = 0.f, acc2 = 0.f;
 #pragma unroll 1
             for (int c = sub; c < chunks && i < b; c += LG) {
                 const uint4 v = *reinterpret_cast<const uint4 *>(Ys + i * lds + c * 8);
-                const float *xv = xs + c * 8;
-                float xe[8];
-#pragma unroll
-                for (int e = 0; e < 8; ++e) xe[e] = p.exact_margin ? xv[e] : __bfloat162float(__float2bfloat16_rn(xv[e]));
-                acc = fmaf(bf16lo(v.x), xe[0], acc); acc = fmaf(bf16hi(v.x), xe[1], acc);
-                acc = fmaf(bf16lo(v.y), xe[2], acc); acc = fmaf(bf16hi(v.y), xe[3], acc);
-                acc = fmaf(bf16lo(v.z), xe[4], acc); acc = fmaf(bf16hi(v.z), xe[5], acc);
-                acc = fmaf(bf16lo(v.w), xe[6], acc); acc = fmaf(bf16hi(v.w), xe[7], acc);
+                const float4 xa = *reinterpret_cast<const float4 *>(xm + c * 8), xb = *reinterpret_cast<const float4 *>(xm + c * 8 + 4);
+                acc = fmaf(bf16lo(v.x), xa.x, acc); acc2 = fmaf(bf16hi(v.x), xa.y, acc2);
+                acc = fmaf(bf16lo(v.y), xa.z, acc); acc2 = fmaf(bf16hi(v.y), xa.w, acc2);
+                acc = fmaf(bf16lo(v.z), xb.x, acc); acc2 = fmaf(bf16hi(v.z), xb.y, acc2);
+                acc = fmaf(bf16lo(v.w), xb.z, acc); acc2 = fmaf(bf16hi(v.w), xb.w, acc2);
             }
+            acc += acc2;
             for (int o = LG >> 1; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
             // lane `sub` of the row's group stores to CTA sub, sub + LG, ...: the C remote stores of a row are spread over its lanes
             if (i < b)
@@ -179,10 +191,13 @@ s1_cluster_kernel(const S1Params p)
                 for (int dstc = sub; dstc < C; dstc += LG) {
                     uint32_t remote;
                     asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(remote) : "r"(smem0 + recv_q + recv_rank_off + 4u * (uint32_t)i), "r"((uint32_t)dstc));
-                    asm volatile("st.shared::cluster.f32 [%0], %1;" ::"r"(remote), "f"(acc) : "memory");
+                    st_async_b32(remote, __float_as_uint(acc), mapa_u32(bar0 + 8u * q, (uint32_t)dstc));
                 }
         }
-        sc_cluster_sync();                              // all partials of this iteration have landed everywhere
+        // all C * b partials of this iteration have landed HERE (st.async counts them on this buffer's barrier): no
+        // cluster-wide barrier per iteration -- a CTA can be at most one iteration ahead of the slowest (it needs
+        // everybody's partials to go on), which is what the two receive buffers allow
+        mbar_wait(bar0 + 8u * q, (uint32_t)(step >> 1) & 1u);
 
         // ---- r = sum over ranks (rank order: identical bits in every CTA), u = l'(r, y_I)
         const float *rv = reinterpret_cast<const float *>(sc_smem + recv_q);
@@ -191,30 +206,35 @@ s1_cluster_kernel(const S1Params p)
             float rr = 0.f;
 #pragma unroll 4
             for (int k = 0; k < C; ++k) rr += rv[k * b + i];
-            const float uu = lprime<LOSS>(rr, yl[i]);
+            const float uu = lprime_chain<LOSS>(rr, yl[i]);
             us[i] = uu;
             if (last && crank == 0) { p.yI[i] = yl[i]; p.r[i] = rr; p.z[i] = rr; p.u[i] = uu; }
         }
         __syncthreads();
+        if (tid == 0) mbar_expect_tx(bar0 + 8u * q, rx_bytes);      // this buffer's next phase (iteration step + 2), armed
+                                                                    // before this CTA's partials of step + 1 let anyone get there
 
-        // ---- update of this CTA's columns: a warp per group of rows, 8 columns per lane and pass
-#pragma unroll 1
-        for (int cb = 0; cb < chunks; cb += 32) {
-            const int c = cb + lane;
+        // ---- update of this CTA's columns: CH lanes side by side on a row slice (8 columns each), the rows dealt over
+        // the lane groups; the groups of a warp meet by shuffles, the warps through shared memory
+        {
             float acc[8] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
-            if (c < chunks)
+            if (csub < chunks)
 #pragma unroll 2
-                for (int i = warp; i < b; i += kScWarps) {
-                    const uint4 v = *reinterpret_cast<const uint4 *>(Ys + i * lds + c * 8);
+                for (int i = crow; i < b; i += crows) {
+                    const uint4 v = *reinterpret_cast<const uint4 *>(Ys + i * lds + csub * 8);
                     const float uu = us[i];
                     acc[0] = fmaf(bf16lo(v.x), uu, acc[0]); acc[1] = fmaf(bf16hi(v.x), uu, acc[1]);
                     acc[2] = fmaf(bf16lo(v.y), uu, acc[2]); acc[3] = fmaf(bf16hi(v.y), uu, acc[3]);
                     acc[4] = fmaf(bf16lo(v.z), uu, acc[4]); acc[5] = fmaf(bf16hi(v.z), uu, acc[5]);
                     acc[6] = fmaf(bf16lo(v.w), uu, acc[6]); acc[7] = fmaf(bf16hi(v.w), uu, acc[7]);
                 }
-            if (c < chunks) {
+#pragma unroll 1
+            for (int o = CH; o < 32; o <<= 1)
 #pragma unroll
-                for (int e = 0; e < 8; ++e) red[warp * cpc + c * 8 + e] = acc[e];
+                for (int e = 0; e < 8; ++e) acc[e] += __shfl_xor_sync(0xffffffffu, acc[e], o);
+            if (csub < chunks && lane < CH) {
+#pragma unroll
+                for (int e = 0; e < 8; ++e) red[warp * cpc + csub * 8 + e] = acc[e];
             }
         }
         __syncthreads();
@@ -223,7 +243,9 @@ s1_cluster_kernel(const S1Params p)
             float g = 0.f;
 #pragma unroll
             for (int w = 0; w < kScWarps; ++w) g += red[w * cpc + k];
-            xs[k] = fmaf(-p.alpha, g, xs[k]);
+            const float xn = fmaf(-p.alpha, g, xs[k]);
+            xs[k] = xn;
+            xm[k] = p.exact_margin ? xn : __bfloat162float(__float2bfloat16_rn(xn));
         }
         if (last && csub < chunks)
 #pragma unroll 1

@@ -480,13 +480,14 @@ def test_pipelined_graphs_of_two_contexts_and_shapes_interleaved(binding):
         assert torch.linalg.norm(got[k] - ref[k]) <= 2e-5 * torch.linalg.norm(ref[k]), k
 
 
-# (config, m, n, s, b, CASGD_OPT_MINI): 2 = the one-CTA kernel whenever the step fits it, whatever the measured crossovers
+# (config, m, n, s, b, CASGD_OPT_MINI): 2 / 3 = the one-CTA / the cluster kernel whenever the step fits it, whatever the
+# measured crossovers
 MINI_SHAPES = [(0, 8192, 64, 4, 16, 2), (1, 20000, 18, 1, 64, 2), (1, 20000, 18, 2, 64, 2), (4, 6000, 512, 1, 16, 2),
                (0, 4097, 64, 7, 13, 2), (3, 3000, 100, 3, 24, 2), (0, 5000, 33, 2, 5, 2), (4, 6000, 512, 2, 16, 2),
                (2, 20000, 1024, 1, 8, 2), (1, 9000, 18, 1, 500, 2), (0, 9000, 120, 1, 130, 1), (0, 8192, 64, 4, 16, 1),
                # s = 1 with wide rows: one launch of one column-split cluster (s1_cluster.cu)
                (4, 6000, 512, 1, 64, 1), (3, 5000, 2000, 1, 32, 1), (2, 20000, 4096, 1, 128, 1), (3, 5000, 1001, 1, 40, 1),
-               (4, 6000, 256, 1, 16, 1), (0, 7000, 300, 1, 256, 1)]
+               (4, 6000, 256, 1, 16, 1), (0, 7000, 300, 1, 256, 1), (0, 8192, 64, 1, 16, 3), (1, 9000, 100, 1, 7, 3)]
 
 
 @pytest.mark.parametrize("ci,m,n,s,b,mode", MINI_SHAPES)
