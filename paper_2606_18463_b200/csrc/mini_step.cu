@@ -230,7 +230,7 @@ mini_step_kernel(const MiniParams p)
 #pragma unroll 1
             for (int tr = 0; tr < TR; ++tr) {           // (a row tile inside block 0 has no columns: ntc = 0)
                 const int row_hi = min(tr * 16 + 15, sb - 1);
-                const int ntc = ((row_hi / b) * b + 7) >> 3;    // 8-column tiles that hold a block below some row of the tile
+                const int ntc = ((int)((uint32_t)row_hi * inv_b >> 20) * b + 7) >> 3;      // 8-column tiles that hold a block below some row of the tile
 #pragma unroll 1
                 for (; job < first + ntc; job += nwarp) {
                     const int tc = job - first;
@@ -248,12 +248,19 @@ mini_step_kernel(const MiniParams p)
                         bq[1] = *reinterpret_cast<const uint32_t *>(brow + ks * 16 + 8);
                         mma_bf16_16816(c, a, bq);
                     }
+                    // rows i0, i0 + 8 and columns k0, k0 + 1 of this lane: block numbers once per row and column
+                    const int i0 = tr * 16 + g, k0 = tc * 8 + 2 * t4, bb = b * b;
+                    int jrow[2], jcol[2], roff[2], coff[2];
 #pragma unroll
-                    for (int e = 0; e < 4; ++e) {
-                        const int i = tr * 16 + g + (e >> 1) * 8, k = tc * 8 + 2 * t4 + (e & 1);
-                        const int jr = (int)((uint32_t)i * inv_b >> 20), jc = (int)((uint32_t)k * inv_b >> 20);
-                        if (i < sb && jc < jr) gl[(b * b * jr * (jr - 1)) / 2 + jc * b * b + (k - jc * b) * b + (i - jr * b)] = c[e];
+                    for (int h = 0; h < 2; ++h) {
+                        jrow[h] = (int)((uint32_t)(i0 + 8 * h) * inv_b >> 20);
+                        jcol[h] = (int)((uint32_t)(k0 + h) * inv_b >> 20);
+                        roff[h] = (bb * jrow[h] * (jrow[h] - 1)) / 2 + (i0 + 8 * h - jrow[h] * b);
+                        coff[h] = jcol[h] * bb + (k0 + h - jcol[h] * b) * b;
                     }
+#pragma unroll
+                    for (int e = 0; e < 4; ++e)
+                        if (i0 + 8 * (e >> 1) < sb && jcol[e & 1] < jrow[e >> 1]) gl[roff[e >> 1] + coff[e & 1]] = c[e];
                 }
                 first += ntc;
             }
