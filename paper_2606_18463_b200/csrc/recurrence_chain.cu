@@ -7,9 +7,10 @@
 // block. Measured 0.45-0.6 us per hop, and on the narrow-row workloads (SUSY-, epsilon-, poisson-shaped: b = 64, 32, 64)
 // those hops ARE the outer iteration. Here the hop never leaves an SM:
 //   chain CTA (rank 0)  owns all b rows of every block. Per hop it needs only the NEWEST W blocks of G's row block j
-//       (b x W b floats, <= 32 KB: 16-byte cp.async, three hops ahead) and the older part of the sum as ONE
+//       (b x W b floats, <= 32 KB: straight from L2 into registers, three hops ahead) and the older part of the sum as ONE
 //       number per row: z_j = r_j - alpha (G_{j, j-W..j-1} u_{j-W..j-1} + P_j). 512/b lanes per row, a shuffle tree, l',
-//       one __syncthreads: ~400 cycles.
+//       one __syncthreads. (Planned at ~400 cycles per hop; MEASURED 1100-1400, and the helpers pace the chain at
+//       ~2600 -- slower than the streaming kernel, so this kernel is opt-in only: DESIGN.md section 6.)
 //   helpers (ranks 1..15)  own rows h, h+15, ... of every block and form P_j[i] = sum_{k <= j-W-1} G_{ik} u_k: the whole
 //       older part of the row, as soon as u_{j-W-1} has arrived
 //       from the chain CTA, and st.async it into the chain CTA W+1 hops before it is needed -- both DSMEM crossings are
@@ -29,7 +30,7 @@ constexpr int kCcSmemCap = 227 * 1024;
 constexpr int kCcPieces = 4;                            // 16-byte pieces of a hop's window one lane holds at most
 constexpr int kCcMaxSb = 4096;                          // u and P live in shared memory
 
-// Blocks of the chain CTA's window: its ring takes b * W b * 4 bytes per hop out of L2 (one SM pulls ~80 B/cycle, a hop
+// Blocks of the chain CTA's window: it takes b * W b * 4 bytes per hop out of L2 (one SM pulls ~80 B/cycle, a hop
 // is ~400 cycles), and W >= 2 is what the helpers' round trip needs.
 __host__ __device__ inline int chain_window(int b)
 {

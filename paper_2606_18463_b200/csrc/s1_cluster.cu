@@ -17,7 +17,7 @@ namespace casgd {
 
 namespace {
 
-constexpr int kScThreads = 256, kScWarps = 8;
+constexpr int kScMaxThreads = 512, kScMaxWarps = 16;     // the launch picks 256 or 512 threads
 constexpr int kScMaxB = 256;
 
 struct S1Params {
@@ -58,7 +58,7 @@ __host__ __device__ inline S1Layout s1_layout(int b, int cpc, int C)
     L.idx = take(2u * L.vec_stride);
     L.recv_stride = (4u * (uint32_t)C * b + 15u) & ~15u;                     // [rank][row]
     L.recv = take(2u * L.recv_stride);
-    L.red = take(4u * kScWarps * cpc);
+    L.red = take(4u * kScMaxWarps * cpc);
     L.Y_stride = (2u * (uint32_t)b * L.lds + 15u) & ~15u;
     L.Y = take(2u * L.Y_stride);
     L.total = o;
@@ -74,13 +74,14 @@ __device__ __forceinline__ void sc_cluster_sync()
 
 // (one instantiation per loss, outer loops not unrolled, power-of-two lane groups: see mini_step.cu on code size)
 template <int LOSS>
-__global__ void __launch_bounds__(kScThreads, 1)
+__global__ void __launch_bounds__(kScMaxThreads, 1)
 s1_cluster_kernel(const S1Params p)
 {
     extern __shared__ __align__(128) unsigned char sc_smem[];
     __shared__ __align__(8) unsigned long long sc_bars[2];       // one per receive buffer: C * b * 4 bytes complete a phase
     pdl_trigger();
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int nthr = blockDim.x, nwarp = nthr >> 5;
     const int C = (int)sc_size(), crank = (int)sc_rank();
     const int b = p.b, n = p.n, cpc = p.cpc;
     const S1Layout L = s1_layout(b, cpc, C);
@@ -95,12 +96,12 @@ s1_cluster_kernel(const S1Params p)
     const uint32_t smem0 = (uint32_t)__cvta_generic_to_shared(sc_smem);
 
 #pragma unroll 1
-    for (uint32_t o = L.Y + 16u * tid; o < L.total; o += 16u * kScThreads)
+    for (uint32_t o = L.Y + 16u * tid; o < L.total; o += 16u * nthr)
         *reinterpret_cast<uint4 *>(sc_smem + o) = make_uint4(0u, 0u, 0u, 0u);
     pdl_wait();
     stamp_begin(p.stamp);
 #pragma unroll 1
-    for (int k = tid; k < cpc; k += kScThreads) {
+    for (int k = tid; k < cpc; k += nthr) {
         const float t = c0 + k < n ? p.x[c0 + k] : 0.f;
         xs[k] = t;
         xm[k] = p.exact_margin ? t : __bfloat162float(__float2bfloat16_rn(t));
@@ -113,7 +114,7 @@ s1_cluster_kernel(const S1Params p)
 
     int CH = 1, chs = 0;                                // gather, export: lanes side by side on a row slice (cpc <= 256: CH <= 32)
     while (CH < (cpc >> 3)) { CH <<= 1; ++chs; }
-    const int csub = tid & (CH - 1), crow = tid >> chs, crows = kScThreads >> chs;
+    const int csub = tid & (CH - 1), crow = tid >> chs, crows = nthr >> chs;
 
     auto issue_gather = [&](int64_t step) {
         const uint32_t q = (uint32_t)(step & 1);
@@ -148,7 +149,7 @@ s1_cluster_kernel(const S1Params p)
 
     int LG = 1, lgs = 0;
     while (LG < chunks && LG < 32) { LG <<= 1; ++lgs; }  // lanes side by side on a row slice
-    const int rows_per_pass = kScThreads >> lgs, sub = tid & (LG - 1), mrow = tid >> lgs;
+    const int rows_per_pass = nthr >> lgs, sub = tid & (LG - 1), mrow = tid >> lgs;
     const uint32_t recv_rank_off = 4u * (uint32_t)(crank * b);
 
 #pragma unroll 1
@@ -239,10 +240,10 @@ s1_cluster_kernel(const S1Params p)
         }
         __syncthreads();
 #pragma unroll 1
-        for (int k = tid; k < ncol; k += kScThreads) {
+        for (int k = tid; k < ncol; k += nthr) {
             float g = 0.f;
-#pragma unroll
-            for (int w = 0; w < kScWarps; ++w) g += red[w * cpc + k];
+#pragma unroll 8
+            for (int w = 0; w < nwarp; ++w) g += red[w * cpc + k];
             const float xn = fmaf(-p.alpha, g, xs[k]);
             xs[k] = xn;
             xm[k] = p.exact_margin ? xn : __bfloat162float(__float2bfloat16_rn(xn));
@@ -256,7 +257,7 @@ s1_cluster_kernel(const S1Params p)
     }
     asm volatile("cp.async.wait_group 0;" ::: "memory");
 #pragma unroll 1
-    for (int k = tid; k < ncol; k += kScThreads)
+    for (int k = tid; k < ncol; k += nthr)
         if (c0 + k < n) {
             p.x[c0 + k] = xs[k];
             store_shadow(p.xbf, p.split ? p.ldxb : 0, c0 + k, xs[k]);
@@ -317,7 +318,10 @@ int launch_s1_cluster(cudaStream_t st, const uint16_t *A, int64_t lda, const flo
     auto *kern = loss == CASGD_LOGISTIC ? s1_cluster_kernel<CASGD_LOGISTIC>
                : loss == CASGD_LINEAR  ? s1_cluster_kernel<CASGD_LINEAR>
                                        : s1_cluster_kernel<CASGD_POISSON>;
-    return launch_pdl(kern, dim3(C), dim3(kScThreads), (size_t)L.total, st, C, p) == cudaSuccess ? 1 : -1;
+    // measured: 16 warps per CTA pay once a CTA's slice of a step is tens of KB (n = 4096, b = 128: 6.7 against 7.7 us);
+    // below that the barriers of 8 warps are cheaper (n = 2000, b = 32: 1.96 against 2.13)
+    const int threads = (int64_t)b * p.cpc * 2 >= (32 << 10) ? kScMaxThreads : 256;
+    return launch_pdl(kern, dim3(C), dim3(threads), (size_t)L.total, st, C, p) == cudaSuccess ? 1 : -1;
 }
 
 }  // namespace casgd
