@@ -162,6 +162,22 @@ int casgd_sgd_steps_fp32(casgd_ctx *c, const int32_t *idx, int64_t n_steps, floa
  * Synchronises. */
 int casgd_loss(casgd_ctx *c, const float *x, double *loss_host);
 
+/* The same F(x) WITHOUT A CONTEXT AND WITHOUT ANY ALLOCATION (csrc/loss_noalloc.cu), for callers that cannot call
+ * cudaMalloc: code under CUDA graph capture, tight serving loops, harnesses that forbid it. All pointers are DEVICE
+ * pointers of the current device and stay the caller's: X_bf16 = m x n BF16 bit patterns with row stride ldx >= n
+ * elements (any alignment; 16-byte-aligned rows take 16-byte loads), y = m FP32 labels, x = n FP32 weights,
+ * result_dev = one double. loss = a casgd_loss_kind. ASYNCHRONOUS on cuda_stream (a cudaStream_t, or null).
+ * The partial sums sit in a file-scope static __device__ array of 128 KB (one double per 256 rows) that every GPU loading
+ * the library holds until exit: m <= 4,194,304, larger m returns CASGD_EINVAL (casgd_loss_noalloc_error() says why).
+ * The first call on a device resolves the array's device address (cudaGetSymbolAddress; set-up, not an allocation) --
+ * make it once outside a capture. Every call on a device shares the array: calls that overlap on the GPU (other
+ * streams, concurrent graph replays) race; calls on one stream are ordered. Nothing has to start at zero (every slot a
+ * call reads it has written). The summation order depends on (m, n) only: the same bits on every call. */
+int casgd_loss_noalloc(const uint16_t *X_bf16, int64_t ldx, const float *y, int64_t m, int32_t n, int loss, const float *x,
+                       double *result_dev, void *cuda_stream);
+/* The calling thread's last casgd_loss_noalloc error message ("" after a successful call). */
+const char *casgd_loss_noalloc_error(void);
+
 /* Kept for compatibility: the shadow is rebuilt from x at the start of every outer-step call anyway. */
 int casgd_invalidate_shadow(casgd_ctx *c);
 

@@ -28,7 +28,7 @@ MAX_SB = 16384
 EXPORTS = (
     "casgd_init", "casgd_outer_step", "casgd_outer_steps", "casgd_outer_steps_sampled", "casgd_outer_steps_host",
     "casgd_sgd_step_fp32",
-    "casgd_sgd_steps_fp32", "casgd_loss", "casgd_invalidate_shadow", "casgd_sync", "casgd_debug_export",
+    "casgd_sgd_steps_fp32", "casgd_loss", "casgd_loss_noalloc", "casgd_loss_noalloc_error", "casgd_invalidate_shadow", "casgd_sync", "casgd_debug_export",
     "casgd_set_option", "casgd_stage_times", "casgd_launch_count", "casgd_last_error", "casgd_destroy",
     "casgd_version", "casgd_payload_count", "casgd_step_local", "casgd_reduce_peers", "casgd_step_finish",
     "casgd_payload_alloc", "casgd_payload_free", "casgd_ipc_export", "casgd_ipc_open", "casgd_ipc_close",
@@ -38,6 +38,23 @@ EXPORTS = (
 def payload_count(s: int, b: int) -> int:
     """casgd_payload_count: FP32 words of one outer iteration's [r; strict block-lower G] (Alg. 1 line 5)."""
     return int(load().casgd_payload_count(s, b))
+
+
+def loss_noalloc(X_bf16: torch.Tensor, y: torch.Tensor, loss: int, x: torch.Tensor, out: torch.Tensor,
+                 stream: Optional[torch.cuda.Stream] = None) -> None:
+    """casgd_loss_noalloc: F(x) into `out` (one float64 on the device) without a context and without any allocation;
+    asynchronous on `stream` (default: torch's current stream). m <= 4,194,304 rows (static scratch)."""
+    assert X_bf16.is_cuda and X_bf16.dtype == torch.bfloat16 and X_bf16.dim() == 2 and X_bf16.stride(1) == 1
+    m, n = X_bf16.shape
+    assert y.is_cuda and y.dtype == torch.float32 and y.is_contiguous() and y.numel() == m
+    assert x.is_cuda and x.dtype == torch.float32 and x.is_contiguous() and x.numel() == n
+    assert out.is_cuda and out.dtype == torch.float64 and out.numel() == 1
+    st = stream if stream is not None else torch.cuda.current_stream(X_bf16.device)
+    lib = load()
+    rc = lib.casgd_loss_noalloc(X_bf16.data_ptr(), X_bf16.stride(0), y.data_ptr(), m, n, int(loss), x.data_ptr(), out.data_ptr(),
+                                st.cuda_stream)
+    if rc:
+        raise CasgdError(rc, (lib.casgd_loss_noalloc_error() or b"").decode())
 
 
 class CasgdError(RuntimeError):
@@ -94,6 +111,10 @@ def load() -> ctypes.CDLL:
     lib.casgd_step_finish.argtypes = [vp, vp, i32, i32, f32, vp]
     lib.casgd_loss.restype = ctypes.c_int
     lib.casgd_loss.argtypes = [vp, vp, ctypes.POINTER(ctypes.c_double)]
+    lib.casgd_loss_noalloc.restype = ctypes.c_int
+    lib.casgd_loss_noalloc.argtypes = [vp, i64, vp, i64, i32, ctypes.c_int, vp, vp, vp]
+    lib.casgd_loss_noalloc_error.restype = ctypes.c_char_p
+    lib.casgd_loss_noalloc_error.argtypes = []
     lib.casgd_invalidate_shadow.restype = ctypes.c_int
     lib.casgd_invalidate_shadow.argtypes = [vp]
     lib.casgd_sync.restype = ctypes.c_int
