@@ -151,6 +151,7 @@ s1_cluster_kernel(const S1Params p)
     while (LG < chunks && LG < 32) { LG <<= 1; ++lgs; }  // lanes side by side on a row slice
     const int rows_per_pass = nthr >> lgs, sub = tid & (LG - 1), mrow = tid >> lgs;
     const uint32_t recv_rank_off = 4u * (uint32_t)(crank * b);
+    const bool wide8 = LG >= 8 && b >= 8 * rows_per_pass;
 
 #pragma unroll 1
     for (int64_t step = 0; step < p.n_steps; ++step) {
@@ -171,6 +172,50 @@ s1_cluster_kernel(const S1Params p)
         }
 
         // ---- partial margins of this column slice, into every CTA's receive buffer
+        if (wide8) {
+            // enough rows for every lane group to take EIGHT at once: the x chunk is read once per eight rows, and the eight
+            // sums meet in one transposing reduction (7-9 shuffles for eight rows instead of 3-5 per row)
+            const int o1 = LG >> 1, o2 = LG >> 2, o3 = LG >> 3;
+            const bool u1 = sub & o1, u2 = sub & o2, u3 = sub & o3;
+#pragma unroll 1
+            for (int base = 0; base < b; base += rows_per_pass * 8) {
+                const int i0 = base + mrow * 8;
+                float acc[8] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
+#pragma unroll 1
+                for (int c = sub; c < chunks; c += LG) {
+                    const float4 xa = *reinterpret_cast<const float4 *>(xm + c * 8), xb = *reinterpret_cast<const float4 *>(xm + c * 8 + 4);
+#pragma unroll
+                    for (int r8 = 0; r8 < 8; ++r8) {
+                        if (i0 + r8 < b) {
+                            const uint4 v = *reinterpret_cast<const uint4 *>(Ys + (i0 + r8) * lds + c * 8);
+                            float a = acc[r8];
+                            a = fmaf(bf16lo(v.x), xa.x, a); a = fmaf(bf16hi(v.x), xa.y, a);
+                            a = fmaf(bf16lo(v.y), xa.z, a); a = fmaf(bf16hi(v.y), xa.w, a);
+                            a = fmaf(bf16lo(v.z), xb.x, a); a = fmaf(bf16hi(v.z), xb.y, a);
+                            a = fmaf(bf16lo(v.w), xb.z, a); a = fmaf(bf16hi(v.w), xb.w, a);
+                            acc[r8] = a;
+                        }
+                    }
+                }
+                float t4[4], t2[2];
+#pragma unroll
+                for (int k = 0; k < 4; ++k)
+                    t4[k] = (u1 ? acc[k + 4] : acc[k]) + __shfl_xor_sync(0xffffffffu, u1 ? acc[k] : acc[k + 4], o1);
+#pragma unroll
+                for (int k = 0; k < 2; ++k)
+                    t2[k] = (u2 ? t4[k + 2] : t4[k]) + __shfl_xor_sync(0xffffffffu, u2 ? t4[k] : t4[k + 2], o2);
+                float tot = (u3 ? t2[1] : t2[0]) + __shfl_xor_sync(0xffffffffu, u3 ? t2[0] : t2[1], o3);
+                for (int o = o3 >> 1; o > 0; o >>= 1) tot += __shfl_xor_sync(0xffffffffu, tot, o);
+                // this lane now holds the sum of row i0 + (u1 u2 u3); the o3 lanes of a row share its C remote stores
+                const int i = i0 + (u1 ? 4 : 0) + (u2 ? 2 : 0) + (u3 ? 1 : 0);
+                if (i < b)
+#pragma unroll 1
+                    for (int dstc = sub & (o3 - 1); dstc < C; dstc += o3) {
+                        const uint32_t remote = mapa_u32(smem0 + recv_q + recv_rank_off + 4u * (uint32_t)i, (uint32_t)dstc);
+                        st_async_b32(remote, __float_as_uint(tot), mapa_u32(bar0 + 8u * q, (uint32_t)dstc));
+                    }
+            }
+        } else
 #pragma unroll 1
         for (int i0 = 0; i0 < b; i0 += rows_per_pass) {
             const int i = i0 + mrow;

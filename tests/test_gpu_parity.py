@@ -487,7 +487,9 @@ MINI_SHAPES = [(0, 8192, 64, 4, 16, 2), (1, 20000, 18, 1, 64, 2), (1, 20000, 18,
                (2, 20000, 1024, 1, 8, 2), (1, 9000, 18, 1, 500, 2), (0, 9000, 120, 1, 130, 1), (0, 8192, 64, 4, 16, 1),
                # s = 1 with wide rows: one launch of one column-split cluster (s1_cluster.cu)
                (4, 6000, 512, 1, 64, 1), (3, 5000, 2000, 1, 32, 1), (2, 20000, 4096, 1, 128, 1), (3, 5000, 1001, 1, 40, 1),
-               (4, 6000, 256, 1, 16, 1), (0, 7000, 300, 1, 256, 1), (0, 8192, 64, 1, 16, 3), (1, 9000, 100, 1, 7, 3)]
+               (4, 6000, 256, 1, 16, 1), (0, 7000, 300, 1, 256, 1), (0, 8192, 64, 1, 16, 3), (1, 9000, 100, 1, 7, 3),
+               # ... with eight rows per lane group in its margin (b >= 8 x the groups), ragged rows and chunks
+               (4, 6000, 512, 1, 256, 1), (3, 5000, 1100, 1, 200, 1)]
 
 
 @pytest.mark.parametrize("ci,m,n,s,b,mode", MINI_SHAPES)
