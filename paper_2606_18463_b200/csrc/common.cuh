@@ -72,12 +72,29 @@ __device__ __forceinline__ float lprime_rt(int loss, float z, float y)
                                  : lprime<CASGD_POISSON>(z, y);
 }
 
+// log(1 + e) for e in [0, 1] as 2 atanh(w), w = e / (2 + e) in [0, 1/3]: the odd series up to w^15 (the next term
+// is < 2e-9 of the result), relative error a few ulp for every e -- log1pf's accuracy at half its instructions (the
+// narrow-row loss kernel is issue-bound).
+__device__ __forceinline__ float log1p_unit(float e)
+{
+    const float w = __fdividef(e, 2.f + e), w2 = w * w;
+    float p = 1.f / 15.f;
+    p = fmaf(p, w2, 1.f / 13.f);
+    p = fmaf(p, w2, 1.f / 11.f);
+    p = fmaf(p, w2, 1.f / 9.f);
+    p = fmaf(p, w2, 1.f / 7.f);
+    p = fmaf(p, w2, 1.f / 5.f);
+    p = fmaf(p, w2, 1.f / 3.f);
+    p = p * w2;
+    return 2.f * fmaf(w, p, w);
+}
+
 // L(r, y) in FP32; logistic as max(-t, 0) + log1p(exp(-|t|)).
 __device__ __forceinline__ float loss_value_rt(int loss, float r, float y)
 {
     if (loss == CASGD_LOGISTIC) {
         float t = y * r;
-        return fmaxf(-t, 0.f) + log1pf(expf(-fabsf(t)));
+        return fmaxf(-t, 0.f) + log1p_unit(expf(-fabsf(t)));
     } else if (loss == CASGD_LINEAR) {
         float d = r - y;
         return 0.5f * d * d;

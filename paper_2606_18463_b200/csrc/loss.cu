@@ -160,31 +160,46 @@ loss_stream_kernel(const uint16_t *__restrict__ A, int64_t ld, const float *__re
     if (MODE == 0 || MODE == 2) {
         // unit = rows_per_slot consecutive whole rows (one contiguous piece) + their labels (a second piece)
         const int64_t nunits = (m + rows_per_slot - 1) / rows_per_slot;
-        auto issue = [&](int64_t it, int slot) {
-            const int64_t unit = gw + it * W;
-            if (unit >= nunits) return;
-            const int64_t row0 = unit * rows_per_slot;
-            const int rows = (int)min((int64_t)rows_per_slot, m - row0);
-            // the last row of the matrix ends at its n-th element (rounded up to the 16-byte vector when aligned)
-            uint32_t bytes = (uint32_t)rows * rowB;
-            if (row0 + rows == m) bytes = (uint32_t)(rows - 1) * rowB + (MODE == 0 ? (uint32_t)xpad * 2u : (uint32_t)n * 2u);
-            const uint32_t ybytes = 4u * (uint32_t)rows;
-            const uint32_t total = (((bytes | ybytes) & 15u) == 0u) ? bytes + ybytes : 1u;   // odd total: copied by the lanes
-            const uint32_t dst = ring + (uint32_t)slot * kLsSlotY;
-            fill_piece(dst, A + row0 * ld, bytes, bar0 + 8u * slot, lane, true, false, total);
-            fill_piece(dst + kLsSlot, reinterpret_cast<const uint16_t *>(y + row0), ybytes, bar0 + 8u * slot, lane, false, true, total);
+        // running state of the producer and of the consumer: this warp's next unit and where it starts (the 64-bit
+        // products per slot were a quarter of the narrow-row kernel's instructions)
+        const int64_t unit_stride_rows = W * rows_per_slot;
+        const uint32_t full_bytes = (uint32_t)rows_per_slot * rowB, full_ybytes = 4u * (uint32_t)rows_per_slot;
+        const bool full_ok = ((full_bytes | full_ybytes) & 15u) == 0u;
+        int64_t p_unit = gw;
+        const uint16_t *p_src = A + gw * rows_per_slot * ld;
+        const float *p_y = y + gw * rows_per_slot;
+        auto issue = [&](int slot) {
+            if (p_unit >= nunits) return;
+            const uint32_t dst = ring + (uint32_t)slot * kLsSlotY, bar = bar0 + 8u * slot;
+            if (p_unit + 1 < nunits && full_ok) {       // a whole unit: two bulk copies
+                if (lane == 0) {
+                    mbar_expect_tx(bar, full_bytes + full_ybytes);
+                    bulk_g2s(dst, p_src, full_bytes, bar);
+                    bulk_g2s(dst + kLsSlot, p_y, full_ybytes, bar);
+                }
+            } else {
+                const int64_t row0 = p_unit * rows_per_slot;
+                const int rows = (int)min((int64_t)rows_per_slot, m - row0);
+                // the last row of the matrix ends at its n-th element (rounded up to the 16-byte vector when aligned)
+                uint32_t bytes = (uint32_t)rows * rowB;
+                if (row0 + rows == m) bytes = (uint32_t)(rows - 1) * rowB + (MODE == 0 ? (uint32_t)xpad * 2u : (uint32_t)n * 2u);
+                const uint32_t ybytes = 4u * (uint32_t)rows;
+                const uint32_t total = (((bytes | ybytes) & 15u) == 0u) ? bytes + ybytes : 1u;   // odd total: copied by the lanes
+                fill_piece(dst, p_src, bytes, bar, lane, true, false, total);
+                fill_piece(dst + kLsSlot, reinterpret_cast<const uint16_t *>(p_y), ybytes, bar, lane, false, true, total);
+            }
+            p_unit += W;
+            p_src += unit_stride_rows * ld;
+            p_y += unit_stride_rows;
         };
 #pragma unroll 1
-        for (int d = 0; d < kLsDepth - 1; ++d) issue(d, d);
+        for (int d = 0; d < kLsDepth - 1; ++d) issue(d);
         int slot = 0;
         uint32_t phase = 0;
 #pragma unroll 1
-        for (int64_t it = 0;; ++it) {
-            const int64_t unit = gw + it * W;
-            if (unit >= nunits) break;
-            issue(it + kLsDepth - 1, slot == 0 ? kLsDepth - 1 : slot - 1);      // the slot consumed last iteration
-            const int64_t row0 = unit * rows_per_slot;
-            const int rows = (int)min((int64_t)rows_per_slot, m - row0);
+        for (int64_t unit = gw; unit < nunits; unit += W) {
+            issue(slot == 0 ? kLsDepth - 1 : slot - 1);                         // into the slot consumed last iteration
+            const int rows = unit + 1 < nunits ? rows_per_slot : (int)(m - unit * rows_per_slot);
             const uint32_t sbase = ring + (uint32_t)slot * kLsSlotY;
             mbar_wait(bar0 + 8u * slot, phase);
             if (MODE == 0) {
@@ -230,14 +245,34 @@ loss_stream_kernel(const uint16_t *__restrict__ A, int64_t ld, const float *__re
                         const uint32_t ra = sbase + (uint32_t)rr * rowB;
                         float acc = 0.f, acc2 = 0.f;
                         if (x_in_regs) {
-                            // n <= 32 and even: x lives in registers, the row's words are all loaded up front
-                            uint32_t w[16];
+                            // n <= 32 and even: x lives in registers; the row's n / 2 words in blocks of four under
+                            // UNIFORM branches (a predicated-off load or FMA still takes its issue slot, and this
+                            // kernel is issue-bound at n = 18: 16 predicated words were 106 of its 173 instructions
+                            // per 32 rows)
+                            const int nw = n >> 1;
 #pragma unroll
-                            for (int k = 0; k < 16; ++k) w[k] = (2 * k < n) ? lds_u32(ra + 4u * k) : 0u;
+                            for (int kb = 0; kb < 16; kb += 4) {
+                                if (kb < nw) {
+                                    if (kb + 4 <= nw) {
+                                        uint32_t w[4];
 #pragma unroll
-                            for (int k = 0; k < 16; ++k) {
-                                acc = fmaf(bf16lo(w[k]), xr[2 * k], acc);
-                                acc2 = fmaf(bf16hi(w[k]), xr[2 * k + 1], acc2);
+                                        for (int k = 0; k < 4; ++k) w[k] = lds_u32(ra + 4u * (kb + k));
+#pragma unroll
+                                        for (int k = 0; k < 4; ++k) {
+                                            acc = fmaf(bf16lo(w[k]), xr[2 * (kb + k)], acc);
+                                            acc2 = fmaf(bf16hi(w[k]), xr[2 * (kb + k) + 1], acc2);
+                                        }
+                                    } else {
+#pragma unroll
+                                        for (int k = 0; k < 3; ++k) {
+                                            if (kb + k < nw) {
+                                                const uint32_t w = lds_u32(ra + 4u * (kb + k));
+                                                acc = fmaf(bf16lo(w), xr[2 * (kb + k)], acc);
+                                                acc2 = fmaf(bf16hi(w), xr[2 * (kb + k) + 1], acc2);
+                                            }
+                                        }
+                                    }
+                                }
                             }
                         } else if ((ld & 1) == 0) {
                             const int nw = n >> 1;
