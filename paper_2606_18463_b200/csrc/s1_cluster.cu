@@ -73,7 +73,9 @@ __device__ __forceinline__ void sc_cluster_sync()
 }
 
 // (one instantiation per loss, outer loops not unrolled, power-of-two lane groups: see mini_step.cu on code size)
-template <int LOSS>
+// WIDE8: the margin takes eight rows per lane group (the launch checks that b and the slice width allow it; a kernel of its
+// own so that the other shapes keep their smaller loop body)
+template <int LOSS, bool WIDE8>
 __global__ void __launch_bounds__(kScMaxThreads, 1)
 s1_cluster_kernel(const S1Params p)
 {
@@ -151,7 +153,7 @@ s1_cluster_kernel(const S1Params p)
     while (LG < chunks && LG < 32) { LG <<= 1; ++lgs; }  // lanes side by side on a row slice
     const int rows_per_pass = nthr >> lgs, sub = tid & (LG - 1), mrow = tid >> lgs;
     const uint32_t recv_rank_off = 4u * (uint32_t)(crank * b);
-    const bool wide8 = LG >= 8 && b >= 8 * rows_per_pass;
+    const bool wide8 = WIDE8 && LG >= 8;                 // (a last CTA with a narrower slice takes the plain path)
 
 #pragma unroll 1
     for (int64_t step = 0; step < p.n_steps; ++step) {
@@ -172,7 +174,7 @@ s1_cluster_kernel(const S1Params p)
         }
 
         // ---- partial margins of this column slice, into every CTA's receive buffer
-        if (wide8) {
+        if (WIDE8 && wide8) {
             // enough rows for every lane group to take EIGHT at once: the x chunk is read once per eight rows, and the eight
             // sums meet in one transposing reduction (7-9 shuffles for eight rows instead of 3-5 per row)
             const int o1 = LG >> 1, o2 = LG >> 2, o3 = LG >> 3;
@@ -331,9 +333,9 @@ cudaError_t s1_cluster_configure()
         if (e == cudaSuccess) e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, kScSmemCap);
         if (e == cudaSuccess) e = cudaFuncSetAttribute(k, cudaFuncAttributeNonPortableClusterSizeAllowed, 1);
     };
-    set(s1_cluster_kernel<CASGD_LOGISTIC>);
-    set(s1_cluster_kernel<CASGD_LINEAR>);
-    set(s1_cluster_kernel<CASGD_POISSON>);
+    set(s1_cluster_kernel<CASGD_LOGISTIC, false>); set(s1_cluster_kernel<CASGD_LOGISTIC, true>);
+    set(s1_cluster_kernel<CASGD_LINEAR, false>);   set(s1_cluster_kernel<CASGD_LINEAR, true>);
+    set(s1_cluster_kernel<CASGD_POISSON, false>);  set(s1_cluster_kernel<CASGD_POISSON, true>);
     return e;
 }
 
@@ -360,12 +362,18 @@ int launch_s1_cluster(cudaStream_t st, const uint16_t *A, int64_t lda, const flo
     p.exact_margin = exact_margin; p.alpha = alpha; p.x = x; p.xbf = xbf; p.ldxb = ldxb; p.split = split;
     p.Y = Y; p.yI = yI; p.r = r; p.z = z; p.u = u; p.err_flag = err_flag; p.stamp = g_stamp;
     const S1Layout L = s1_layout(b, p.cpc, C);
-    auto *kern = loss == CASGD_LOGISTIC ? s1_cluster_kernel<CASGD_LOGISTIC>
-               : loss == CASGD_LINEAR  ? s1_cluster_kernel<CASGD_LINEAR>
-                                       : s1_cluster_kernel<CASGD_POISSON>;
     // measured: 16 warps per CTA pay once a CTA's slice of a step is tens of KB (n = 4096, b = 128: 6.7 against 7.7 us);
     // below that the barriers of 8 warps are cheaper (n = 2000, b = 32: 1.96 against 2.13)
     const int threads = (int64_t)b * p.cpc * 2 >= (32 << 10) ? kScMaxThreads : 256;
+    // eight rows per lane group in the margin: when every group of LG lanes (LG = the slice's 16-byte pieces rounded up to
+    // a power of two, 8..32) gets eight rows
+    int LG = 1;
+    while (LG < p.cpc / 8 && LG < 32) LG <<= 1;
+    const bool wide8 = LG >= 8 && b >= 8 * (threads / LG);
+    auto pick = [&](auto *narrow, auto *wide) { return wide8 ? wide : narrow; };
+    auto *kern = loss == CASGD_LOGISTIC ? pick(s1_cluster_kernel<CASGD_LOGISTIC, false>, s1_cluster_kernel<CASGD_LOGISTIC, true>)
+               : loss == CASGD_LINEAR  ? pick(s1_cluster_kernel<CASGD_LINEAR, false>, s1_cluster_kernel<CASGD_LINEAR, true>)
+                                       : pick(s1_cluster_kernel<CASGD_POISSON, false>, s1_cluster_kernel<CASGD_POISSON, true>);
     return launch_pdl(kern, dim3(C), dim3(threads), (size_t)L.total, st, C, p) == cudaSuccess ? 1 : -1;
 }
 
