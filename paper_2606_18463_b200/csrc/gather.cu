@@ -76,6 +76,9 @@ gather_bulk_kernel(const uint16_t *__restrict__ A, int64_t lda, const float *__r
     stamp_begin(stamp);
     const int32_t *I = ind ? ind->idx + idx_off : idx;
     const int gw = blockIdx.x * kGbWarps + warp, W = gridDim.x * kGbWarps;
+    // rows of A are read once per epoch: they leave L2 first (the Y and G stages of the pipelined graph are what is read again)
+    unsigned long long pol_first;
+    asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(pol_first));
 
     // labels (and the range check): one thread per sampled row
     for (int row = blockIdx.x * blockDim.x + threadIdx.x; row < sb; row += gridDim.x * blockDim.x) {
@@ -111,8 +114,8 @@ gather_bulk_kernel(const uint16_t *__restrict__ A, int64_t lda, const float *__r
                     // the store that last read this slot has finished reading it
                     asm volatile("cp.async.bulk.wait_group.read %0;" ::"n"(kGbDepth - kGbAhead - 1) : "memory");
                     asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
-                    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
-                                 ::"r"(dst), "l"(A + src * lda + off / 2), "r"(bytes), "r"(bar) : "memory");
+                    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1], %2, [%3], %4;"
+                                 ::"r"(dst), "l"(A + src * lda + off / 2), "r"(bytes), "r"(bar), "l"(pol_first) : "memory");
                 }
             } else {
                 // an out-of-range index reads as a zero row: written by the lanes, nothing goes through the ring
