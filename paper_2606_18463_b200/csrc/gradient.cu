@@ -154,12 +154,15 @@ gradient_stream_kernel(const uint16_t *Y, int32_t ldy, int32_t n, int32_t sb, in
     const int nrows = r1 - r0;                                              // <= 32
     const float u_mine = lane < nrows ? ld_dep(u + r0 + lane) : 0.f;
     const uint16_t *src = Y + (int64_t)r0 * ldy + col0;
+    // the update is the last reader of the step's rows: they may leave L2 first
+    unsigned long long pol_first;
+    asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(pol_first));
     auto issue = [&](int k) {
         if (k < nrows && lane == 0) {
             const uint32_t bar = bar0 + 8u * (k % kGsDepth);
             asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(segB) : "memory");
-            asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
-                         ::"r"(ring + (uint32_t)(k % kGsDepth) * kGsPiece), "l"(src + (int64_t)k * ldy), "r"(segB), "r"(bar) : "memory");
+            asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1], %2, [%3], %4;"
+                         ::"r"(ring + (uint32_t)(k % kGsDepth) * kGsPiece), "l"(src + (int64_t)k * ldy), "r"(segB), "r"(bar), "l"(pol_first) : "memory");
         }
     };
 #pragma unroll 1
