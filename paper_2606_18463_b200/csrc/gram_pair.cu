@@ -52,7 +52,9 @@ struct PairItem {                       // 16 bytes
     int16_t kb0, kb1;                   // K blocks [kb0, kb1)
     int16_t kind;                       // 0 = G tile, 1 = margin
     int16_t nsub;                       // 256-column sub-tiles to compute (1 or 2)
-    int32_t pad;
+    int16_t half;                       // 1 = only the tile's first 128 columns hold entries below the block diagonal (a
+                                        // diagonal tile at b = 128): N = 128, each CTA supplies 64 rows of B
+    int16_t pad;
 };
 
 struct PairParams {
@@ -188,7 +190,8 @@ __device__ __forceinline__ uint32_t umma_idesc_pair(uint32_t n_cols)
 // ------------------------------------------------------------------------------- kernel ---
 
 __global__ void __launch_bounds__(kThreadsP, 1)
-gram_pair_kernel(const __grid_constant__ CUtensorMap tmY, const __grid_constant__ CUtensorMap tmX8, const PairParams p)
+gram_pair_kernel(const __grid_constant__ CUtensorMap tmY, const __grid_constant__ CUtensorMap tmX8,
+                 const __grid_constant__ CUtensorMap tmY64, const PairParams p)
 {
     extern __shared__ uint8_t smem_raw[];
     const uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;      // same offset in both CTAs of the pair
@@ -215,6 +218,7 @@ gram_pair_kernel(const __grid_constant__ CUtensorMap tmY, const __grid_constant_
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
         asm volatile("prefetch.tensormap [%0];" ::"l"((uint64_t)&tmY) : "memory");
         asm volatile("prefetch.tensormap [%0];" ::"l"((uint64_t)&tmX8) : "memory");
+        asm volatile("prefetch.tensormap [%0];" ::"l"((uint64_t)&tmY64) : "memory");
     }
     if (warp == 1) {
         asm volatile("tcgen05.alloc.cta_group::2.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(tmem_slot), "r"(512u) : "memory");
@@ -239,7 +243,12 @@ gram_pair_kernel(const __grid_constant__ CUtensorMap tmY, const __grid_constant_
                     mbar_wait(empty_bar(stage), phase ^ 1u);
                     const uint32_t sbase = smem_base + stage * kStageB;
                     const uint32_t fb = mapa(full_bar(stage), 0);          // completion is counted on the leader's barrier
-                    if (w.kind == 0) {
+                    if (w.kind == 0 && w.half) {
+                        // N = 128: this CTA's half of B is 64 rows (columns 64 rank .. 64 rank + 63 of the tile)
+                        mbar_expect_tx_cluster(fb, kTileB + kTileB / 2);
+                        tma_load_2d_pair(sbase + kOffAp, &tmY, fb, kb * BK, p.row_base + w.I * PM + (int)rank * HM);
+                        tma_load_2d_pair(sbase + kOffB0, &tmY64, fb, kb * BK, p.row_base + w.J * p.bn + (int)rank * (HM / 2));
+                    } else if (w.kind == 0) {
                         mbar_expect_tx_cluster(fb, kTileB * (1u + (uint32_t)w.nsub));
                         tma_load_2d_pair(sbase + kOffAp, &tmY, fb, kb * BK, p.row_base + w.I * PM + (int)rank * HM);
                         for (int sub = 0; sub < w.nsub; ++sub)
@@ -272,7 +281,7 @@ gram_pair_kernel(const __grid_constant__ CUtensorMap tmY, const __grid_constant_
                 mbar_wait_cluster(acce_bar(slot), acc_phase ^ 1u);
                 tc_fence_after();
                 const uint32_t d_tmem = tmem_base + slot * 256;
-                const uint32_t idesc = umma_idesc_pair(w.kind == 0 ? 256u : 16u);
+                const uint32_t idesc = umma_idesc_pair(w.kind == 0 ? (w.half ? 128u : 256u) : 16u);
                 const bool two = w.nsub == 2;
                 for (int kb = w.kb0; kb < w.kb1; ++kb) {
                     mbar_wait(full_bar(stage), phase);
@@ -333,7 +342,7 @@ gram_pair_kernel(const __grid_constant__ CUtensorMap tmY, const __grid_constant_
             const bool row_ok = row < p.sb;
             if (w.kind == 0) {
                 const int last_row = min(half_row0 + HM, p.sb) - 1;        // last row of this CTA's half
-                const int nchunks = w.nsub * (PM / 32);
+                const int nchunks = w.half ? 4 : w.nsub * (PM / 32);
 #pragma unroll 1
                 for (int c = 0; c < nchunks; ++c) {
                     const int col0 = w.J * p.bn + c * 32, qc = col0 & ~127;
@@ -441,6 +450,7 @@ inline int64_t kblock_cost(int nsub) { return nsub == 1 ? 520 : 1300; }
 inline int64_t item_cost(const PairItem &w)
 {
     if (w.kind == 1) return (int64_t)(w.kb1 - w.kb0) * 410 + 600;
+    if (w.half) return (int64_t)(w.kb1 - w.kb0) * 400 + 3000;                    // 24 instead of 32 KB per CTA and K block, half the MMAs
     return (int64_t)(w.kb1 - w.kb0) * kblock_cost(w.nsub) + 5000 * w.nsub;      // + the epilogue (half of it overlaps on average)
 }
 
@@ -472,9 +482,13 @@ bool build_items(int sb, int b, int n, int full_lower, int bn, int ksplit, int n
                 if (c0 <= last_row && (full_lower || (last_row / b) > (c0 / b))) nsub = sub + 1;
             }
             if (nsub == 0) continue;
+            // a tile on the diagonal whose entries below the block diagonal all sit in its first 128 columns (b = 128: the
+            // one block (2I+1, 2I)): N = 128 -- half the MMAs of the tile and three quarters of its operand bytes
+            const int first_col_beyond = (last_row / b) * b - J * bn;                // tile-local; columns >= this hold no such entry
+            const bool half = bn == PM && nsub == 1 && !full_lower && J * bn + PM > last_row && first_col_beyond <= PM / 2;
             for (int ks = 0; ks < ksplit; ++ks) {
                 PairItem w{};
-                w.I = (int16_t)I; w.J = (int16_t)J; w.kind = 0; w.nsub = (int16_t)nsub;
+                w.I = (int16_t)I; w.J = (int16_t)J; w.kind = 0; w.nsub = (int16_t)nsub; w.half = half ? 1 : 0;
                 w.kb0 = (int16_t)((int64_t)ks * kbt / ksplit);
                 w.kb1 = (int16_t)((int64_t)(ks + 1) * kbt / ksplit);
                 if (w.kb1 > w.kb0) all.push_back(w);
@@ -499,6 +513,9 @@ bool build_items(int sb, int b, int n, int full_lower, int bn, int ksplit, int n
         load[best] += item_cost(w);
         if ((int)per_pair[best].size() > kMaxItemsPerPair) return false;
     }
+    // a pair runs its N = 128 items first: the last wave is then whole tiles only
+    for (auto &v : per_pair)
+        std::stable_partition(v.begin(), v.end(), [](const PairItem &w) { return w.kind == 0 && w.half; });
     *makespan = *std::max_element(load.begin(), load.end());
     return true;
 }
@@ -506,7 +523,7 @@ bool build_items(int sb, int b, int n, int full_lower, int bn, int ksplit, int n
 }  // namespace
 
 struct GramPairPlan {
-    CUtensorMap tmY, tmX8;
+    CUtensorMap tmY, tmX8, tmY64;
     float *rpart = nullptr;             // [4 x rows_alloc] margin partial sums
     unsigned *rcount = nullptr;         // [2 x row tiles]
     int32_t n = 0, rows_alloc = 0, npairs = 0;
@@ -522,6 +539,7 @@ GramPairPlan *gram_pair_plan_create(const uint16_t *Y, int32_t ldy, int32_t n, i
     pl->npairs = num_sms / 2;
     if (!make_bf16_map_p(&pl->tmY, Y, (uint64_t)n, (uint64_t)rows_alloc, (uint64_t)ldy, BK, HM) ||
         !make_bf16_map_p(&pl->tmX8, xbf, (uint64_t)n, 16, (uint64_t)ldxb, BK, 8) ||
+        !make_bf16_map_p(&pl->tmY64, Y, (uint64_t)n, (uint64_t)rows_alloc, (uint64_t)ldy, BK, HM / 2) ||
         cudaMalloc(&pl->rpart, sizeof(float) * 4 * (size_t)rows_alloc) != cudaSuccess ||
         cudaMalloc(&pl->rcount, sizeof(unsigned) * 2 * (size_t)(rows_alloc / PM + 1)) != cudaSuccess ||
         cudaMemset(pl->rcount, 0, sizeof(unsigned) * 2 * (size_t)(rows_alloc / PM + 1)) != cudaSuccess) {
@@ -621,7 +639,7 @@ int launch_gram_pair(cudaStream_t st, GramPairPlan *pl, int32_t row_base, int32_
         const int T128 = (sb + 127) / 128;
         cudaMemsetAsync(G, 0, sizeof(float) * (size_t)T128 * 128 * ldg, st);
     }
-    cudaError_t e = launch_pdl(gram_pair_kernel, dim3(2 * L.used_pairs), dim3(kThreadsP), kSmemP, st, 2, pl->tmY, pl->tmX8, p);
+    cudaError_t e = launch_pdl(gram_pair_kernel, dim3(2 * L.used_pairs), dim3(kThreadsP), kSmemP, st, 2, pl->tmY, pl->tmX8, pl->tmY64, p);
     if (e != cudaSuccess) {
         snprintf(err, errlen, "gram_pair_kernel launch: %s", cudaGetErrorString(e));
         return -1;
