@@ -36,7 +36,9 @@ namespace {
 constexpr int PM = 256;                 // rows of a pair tile (128 per CTA)
 constexpr int HM = 128;                 // rows per CTA = rows of one smem operand tile
 constexpr int BK = 64;                  // K block: 64 BF16 = one 128-byte swizzle row
-constexpr int kStagesP = 4;
+constexpr int kStagesP = 4;               // stages of 48 KB (256 x 512 tiles: A half + two B halves) ...
+constexpr int kStagesP256 = 6;            // ... or of 32 KB (256 x 256 tiles: the second B half is never loaded): same 192 KB ring, deeper
+constexpr int kMaxStagesP = 6;
 constexpr uint32_t kTileB = HM * BK * 2;                 // 16384
 constexpr uint32_t kXB = 8 * BK * 2;                     // 1024: 8 rows of the x_bf buffer
 constexpr uint32_t kStageB = 3 * kTileB;                 // A half, B half (sub 0), B half (sub 1; x box for margin items lives in sub 0)
@@ -196,11 +198,14 @@ gram_pair_kernel(const __grid_constant__ CUtensorMap tmY, const __grid_constant_
     extern __shared__ uint8_t smem_raw[];
     const uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;      // same offset in both CTAs of the pair
     const uint32_t bar_base = smem_base + kStagesP * kStageB;
+    // ring geometry: 4 stages of 48 KB for 512-column tiles, 6 stages of 32 KB otherwise
+    const int nst = p.bn == 512 ? kStagesP : kStagesP256;
+    const uint32_t stB = p.bn == 512 ? kStageB : 2 * kTileB;
     auto full_bar = [&](int s) { return bar_base + 8u * s; };
-    auto empty_bar = [&](int s) { return bar_base + 8u * (kStagesP + s); };
-    auto accf_bar = [&](int s) { return bar_base + 8u * (2 * kStagesP + s); };
-    auto acce_bar = [&](int s) { return bar_base + 8u * (2 * kStagesP + 2 + s); };
-    const uint32_t tmem_slot = bar_base + 8u * (2 * kStagesP + 4);
+    auto empty_bar = [&](int s) { return bar_base + 8u * (kMaxStagesP + s); };
+    auto accf_bar = [&](int s) { return bar_base + 8u * (2 * kMaxStagesP + s); };
+    auto acce_bar = [&](int s) { return bar_base + 8u * (2 * kMaxStagesP + 2 + s); };
+    const uint32_t tmem_slot = bar_base + 8u * (2 * kMaxStagesP + 4);
     volatile uint32_t *tmem_slot_ptr =
         reinterpret_cast<volatile uint32_t *>(smem_raw + (tmem_slot - smem_u32(smem_raw)));
     volatile uint32_t *s_last_ptr = tmem_slot_ptr + 1;
@@ -213,7 +218,7 @@ gram_pair_kernel(const __grid_constant__ CUtensorMap tmY, const __grid_constant_
     const PairItem *items = p.items + (size_t)pair * kMaxItemsPerPair;
 
     if (warp == 0 && lane == 0) {
-        for (int s = 0; s < kStagesP; ++s) { mbar_init(full_bar(s), 2); mbar_init(empty_bar(s), 1); }
+        for (int s = 0; s < nst; ++s) { mbar_init(full_bar(s), 2); mbar_init(empty_bar(s), 1); }
         for (int s = 0; s < 2; ++s) { mbar_init(accf_bar(s), 1); mbar_init(acce_bar(s), 8); }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
         asm volatile("prefetch.tensormap [%0];" ::"l"((uint64_t)&tmY) : "memory");
@@ -241,7 +246,7 @@ gram_pair_kernel(const __grid_constant__ CUtensorMap tmY, const __grid_constant_
                 const PairItem w = items[it];
                 for (int kb = w.kb0; kb < w.kb1; ++kb) {
                     mbar_wait(empty_bar(stage), phase ^ 1u);
-                    const uint32_t sbase = smem_base + stage * kStageB;
+                    const uint32_t sbase = smem_base + stage * stB;
                     const uint32_t fb = mapa(full_bar(stage), 0);          // completion is counted on the leader's barrier
                     if (w.kind == 0 && w.half) {
                         // N = 128: this CTA's half of B is 64 rows (columns 64 rank .. 64 rank + 63 of the tile)
@@ -258,13 +263,13 @@ gram_pair_kernel(const __grid_constant__ CUtensorMap tmY, const __grid_constant_
                         tma_load_2d_pair(sbase + kOffAp, &tmY, fb, kb * BK, p.row_base + w.I * PM + (int)rank * HM);
                         tma_load_2d_pair(sbase + kOffB0, &tmX8, fb, kb * BK, (int)rank * 8);
                     }
-                    if (++stage == kStagesP) { stage = 0; phase ^= 1u; }
+                    if (++stage == nst) { stage = 0; phase ^= 1u; }
                 }
             }
             // drain: the MMAs that read this CTA's last stages (and their arrivals here) are done before it exits
-            for (int i = 0; i < kStagesP; ++i) {
+            for (int i = 0; i < nst; ++i) {
                 mbar_wait(empty_bar(stage), phase ^ 1u);
-                if (++stage == kStagesP) { stage = 0; phase ^= 1u; }
+                if (++stage == nst) { stage = 0; phase ^= 1u; }
             }
         }
     } else if (warp == 1) {
@@ -286,7 +291,7 @@ gram_pair_kernel(const __grid_constant__ CUtensorMap tmY, const __grid_constant_
                 for (int kb = w.kb0; kb < w.kb1; ++kb) {
                     mbar_wait(full_bar(stage), phase);
                     tc_fence_after();
-                    const uint32_t sbase = smem_base + stage * kStageB;
+                    const uint32_t sbase = smem_base + stage * stB;
                     const uint64_t adesc = umma_desc_sw128(sbase + kOffAp);
                     const uint64_t bdesc0 = umma_desc_sw128(sbase + kOffB0);
                     const uint64_t bdesc1 = umma_desc_sw128(sbase + kOffB1);
@@ -321,7 +326,7 @@ gram_pair_kernel(const __grid_constant__ CUtensorMap tmY, const __grid_constant_
                         if (kb == w.kb1 - 1) tc_commit_pair(accf_bar(slot));   // accumulator ready, in both CTAs
                     }
                     __syncwarp();
-                    if (++stage == kStagesP) { stage = 0; phase ^= 1u; }
+                    if (++stage == nst) { stage = 0; phase ^= 1u; }
                 }
             }
         }
