@@ -249,7 +249,8 @@ int casgd_debug_export(casgd_ctx *c, int what, void *dst_host, int64_t dst_bytes
  *                              (CASGD_STAGE_MARGIN) instead of extra B-operand rows of the Gram. Single-step calls run
  *                              the sequential kernels on the whole chip in every mode.
  *   CASGD_OPT_CHAIN_SMS        SMs left to the margin / recurrence / update chain in the pipelined schedule (the Gram and
- *                              gather kernels are sized for the rest). 0 (default) = 44.
+ *                              gather kernels are sized for the rest). 0 (default) = 44, or 56 for steps of at least
+ *                              16 MB of rows (measured).
  *   CASGD_OPT_MARGIN_SPLIT     0 (default) = Recipe C of Table 3: x enters the margin r = Y x as its BF16
  *                              shadow (L231, "two BF16 input conversions"). 1 = the margin sees the FP32 MASTER: rows 1
  *                              and 2 of the shadow buffer carry the BF16 residues of x (hi + lo + lo2 == x exactly), the

@@ -540,7 +540,13 @@ int choose_gram(casgd_ctx *c, int32_t s, int32_t b, bool pipe)
     c->cur_gram = 2;                                    // (pipelined_mode asks step_is_s1, which looks at cur_gram)
     pipe = pipe && pipelined_mode(c, s, b);
     if (pipe) {
-        const int chain = c->opt_chain_sms > 0 ? (int)c->opt_chain_sms : 44;      // (measured on synth-linear s = 32: 32 -> 84.4, 44 -> 81.3, 56 -> 82.3 us)
+        // The chain's share, measured. With the pair Gram's six-stage ring the Gram branch (68 us on 52 pairs) is no longer
+        // the critical path of the headline shape; margin -> recurrence -> update is, and its two streaming kernels scale
+        // with SMs while 46 pairs still hold the work list in three waves (120 whole tiles + 16 N = 128 items): synth-linear
+        // s = 32 at 44 / 48 / 52 / 56 / 60 SMs: 76.5 / 75.6 / 74.3 / 73.8 / 82.3 us per step. Steps of a few MB gain nothing
+        // from more chain SMs (epsilon-shaped s = 64: 43.3 at 44, 43.7 at 56): 56 from 16 MB of rows per step on, else 44.
+        const int chain_default = (int64_t)sb * c->ldy * 2 >= ((int64_t)16 << 20) ? 56 : 44;
+        const int chain = c->opt_chain_sms > 0 ? (int)c->opt_chain_sms : chain_default;
         c->chain_sms = std::min(std::max(chain, 16), c->num_sms - 32) & ~1;
         c->gram_sms = c->num_sms - c->chain_sms;
     }
