@@ -790,7 +790,7 @@ int run_steps(casgd_ctx *c, const int32_t *idx, int64_t n_steps, float *x, int32
 
 extern "C" {
 
-const char *casgd_version(void) { return "casgd-b200 0.2 (sm_100a)"; }
+const char *casgd_version(void) { return "casgd-b200 0.3 (sm_100a)"; }
 
 int casgd_init(casgd_ctx **out, const uint16_t *X_bf16, int64_t ldx, const float *y, int64_t m, int32_t n, int loss,
                void *cuda_stream)
