@@ -452,7 +452,7 @@ def run_workload(args, cfg, s, binding, pk, dist, world, rank, stream, clocks, f
     seed = replica_seed(rank)                            # independent replicas
     ds = synth.make_dataset(cfg, seed=seed, device="cuda")
     K, W = args.steps, max(args.warmup, 3)
-    n_idx_steps = W + max(K, min(8 * K, 4096))
+    n_idx_steps = W + max(K, min(8 * K, 4096), min(max(K, 64), 256))   # (the stage report replays min(max(K, 64), 256) steps)
     idx_np = step_indices(cfg, seed, n_idx_steps, sb)
     out = {}
     with torch.cuda.stream(stream):                      # every allocation / fill below is ordered on the library's stream
