@@ -349,7 +349,8 @@ def time_call(stream, fn):
 
 
 def prime_graphs(cg, cfg, seed, s, sb):
-    """Make the library capture and instantiate every graph length it replays (64 + 8 + 1 steps), on a scratch x."""
+    """Make the library capture and instantiate the graph lengths it replays (64 steps, and the 9-step remainder of this
+    call as a graph of its own; a timed call's own remainder length is captured by the untimed sizing call), on a scratch x."""
     idx_p = torch.from_numpy(step_indices(cfg, seed, 73, sb)).cuda()
     cg.outer_steps(idx_p, torch.zeros(cfg.n, device="cuda"), s, cfg.b, cfg.eta, n_steps=73)
     cg.sync()
@@ -460,7 +461,7 @@ def run_workload(args, cfg, s, binding, pk, dist, world, rank, stream, clocks, f
         cg = binding.Casgd(ds.X_bf16, ds.y, cfg.loss, stream=stream)
         x = torch.zeros(cfg.n, device="cuda")
         stream.synchronize()
-        # graph instantiation is not a step: casgd_outer_steps captures its 64 / 8 / 1-step CUDA graphs on first use
+        # graph instantiation is not a step: casgd_outer_steps captures its CUDA graphs (64 steps, and one per remainder length) on first use
         prime_graphs(cg, cfg, seed, s, sb)
         if dist:
             dist.barrier()
@@ -505,7 +506,10 @@ def run_workload(args, cfg, s, binding, pk, dist, world, rank, stream, clocks, f
         for h in range(Ke):
             cg.outer_steps_host(idx_h[h * sb:(h + 1) * sb], x_h, s, cfg.b, cfg.eta, n_steps=1)
         e2e_s = time.perf_counter() - t0
-        # the same with one call per 64 steps (indices of 64 steps copied at once, x in/out once per call)
+        # the same with one call per 64 steps (indices of 64 steps copied at once, x in/out once per call); the graph of the
+        # last, shorter call is captured by an untimed call first
+        if Ke % 64 > 1:
+            cg.outer_steps_host(idx_h[: (Ke % 64) * sb], x_h, s, cfg.b, cfg.eta, n_steps=Ke % 64)
         x_h.zero_()
         t0 = time.perf_counter()
         done = 0

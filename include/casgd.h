@@ -89,7 +89,8 @@ int casgd_outer_step(casgd_ctx *c, const int32_t *idx, float *x, int32_t s, int3
 
 /* n_steps consecutive outer iterations; step h uses idx[h*s*b .. (h+1)*s*b). ASYNCHRONOUS.
  * The same iterations as n_steps calls of casgd_outer_step without per-call launch cost: replayed from CUDA graphs of 64
- * and 8 steps (an extension of the paper's two CUDA graphs, L278) that pipeline consecutive iterations (CASGD_OPT_OVERLAP),
+ * steps, the remaining n_steps % 64 as one graph of that length (captured on first use and cached by length; an extension
+ * of the paper's two CUDA graphs, L278), which pipeline consecutive iterations (CASGD_OPT_OVERLAP),
  * or, for steps small enough, run in ONE persistent launch (CASGD_OPT_MINI). Equal to the single-step calls bit for bit
  * where the same kernels run (CASGD_OPT_OVERLAP 0 and 1, the one-launch kernels), to FP32 rounding in the pipelined
  * graphs, whose margin is a kernel of its own. */

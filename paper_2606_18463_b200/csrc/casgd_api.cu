@@ -750,10 +750,14 @@ int run_steps(casgd_ctx *c, const int32_t *idx, int64_t n_steps, float *x, int32
     c->last_b = b;
     int64_t done = 0;
     if (allow_graph && !c->opt_profile && !c->opt_no_graph && n_steps >= graph_from) {
-        static const int32_t lens[3] = {64, 8, 1};
-        for (int li = 0; li < 3; ++li) {
+        // 64-step graphs, then the remainder as ONE graph of its own length (cached by length): a pipelined graph spends
+        // ~60 us filling its pipeline (two gathers and a Gram before the first chain), so a call of 20 steps is one
+        // 20-step graph rather than 8 + 8 and four single steps (synth-linear s = 32: 84.6 -> ~77 us per step)
+        const int32_t lens[2] = {64, (int32_t)(n_steps % 64)};
+        if (c->graphs.size() > 96) drop_graphs(c);          // (a caller that varies n_steps endlessly: start over)
+        for (int li = 0; li < 2; ++li) {
             const int32_t len = lens[li];
-            if (n_steps - done < len) continue;
+            if (len < 1 || n_steps - done < len) continue;
             GraphEntry ge;
             rc = get_graph(c, s, b, eta, len, &ge);
             if (rc) return rc;
