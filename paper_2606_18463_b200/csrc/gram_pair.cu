@@ -8,7 +8,10 @@
 //   pair tile 256 x 256 (BN = 256):  each CTA loads 16 KB of A + 16 KB of B per 512 MMA cycles  -> 64 B/cycle/SM
 //   pair tile 256 x 512 (BN = 512):  16 KB of A + 32 KB of B per 1024 MMA cycles               -> 48 B/cycle/SM
 // BN = 512 fills all 512 TMEM columns with one accumulator (the epilogue, ~6 % of a K = 4096 tile, is then not
-// overlapped); BN = 256 keeps two accumulator slots.
+// overlapped); BN = 256 keeps two accumulator slots, and runs the 192 KB operand ring as six stages of 32 KB (a 256-column
+// tile never loads a second B half) instead of four of 48 KB: beside the other branches' L2 traffic it is the latency of
+// the loads, not their bandwidth, that a pair waits for (Gram on 52 pairs beside the chain: 78.9 -> 68.1 us).
+// A diagonal tile whose entries below the block diagonal all sit in its first 128 columns (b = 128) is an N = 128 item.
 //
 // Work items (G tiles, and one "margin" item per 256-row tile: N = 16 with x_bf as row 0 of the B operand --
 // BASELINE.json:north_star "carrying x as an extra B-operand column") are dealt to the 74 pairs on the HOST by
