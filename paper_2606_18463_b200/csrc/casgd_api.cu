@@ -385,6 +385,7 @@ int stage_chain(casgd_ctx *c, cudaStream_t st, float *x, const StepParams *ind, 
         // branch needs. With the update fused in, the dependent is the next recurrence (after its Gram, a full edge):
         // let it launch early -- its launch latency is then off the chain (1.5 us per step on the chain-bound shapes)
         c->rws.late_trigger = late_trigger && !fused;
+        c->rws.g_protected = c->cur_gram == 3;
         k = launch_recurrence(st, G, c->ldg, c->r, yI, s, b, alpha, c->loss, c->z, c->u, c->rws,
                               (int)c->opt_rec_impl, fused ? &fu : nullptr);
         g_completion_event = nullptr;

@@ -277,6 +277,8 @@ struct RecWorkspace {
     int64_t grid_threshold_bytes;  // strict block-lower G at or above this size leaves the one-CTA kernel
     int32_t late_trigger;          // 1 = the streaming kernel releases its dependent kernel only when the chain is done
                                    // (a side-branch gather needs the SMs the dependent's waiting CTAs would hold)
+    int32_t g_protected;           // 1 = G was stored with L2::evict_last (the pair Gram kernel): the streaming kernel's
+                                   // loads of it, the only ones there are, carry evict_first
 };
 int recurrence_cluster_size();
 int recurrence_max_coresident_ctas(int num_sms);

@@ -337,6 +337,8 @@ gram_pair_kernel(const __grid_constant__ CUtensorMap tmY, const __grid_constant_
         // ===== epilogue warps: TMEM lane group (warp % 4); this CTA holds 128 of the tile's 256 rows =====
         const int q = warp & 3;
         const bool accumulate = p.accumulate != 0;
+        unsigned long long pol_keep;
+        asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(pol_keep));
         const uint32_t ebuf = bar_base + 256 + (uint32_t)(warp - 2) * kEpiBufB;
         for (int it = 0; it < nitems; ++it) {
             const PairItem w = items[it];
@@ -377,7 +379,7 @@ gram_pair_kernel(const __grid_constant__ CUtensorMap tmY, const __grid_constant_
                         const int orow = half_row0 + q * 32 + rl;
                         if (orow < p.sb) {
                             float *dst = p.G + (int64_t)orow * p.ldg + col0 + c4;
-                            if (!accumulate) *reinterpret_cast<uint4 *>(dst) = make_uint4(o0, o1, o2, o3);
+                            if (!accumulate) asm volatile("st.global.L2::cache_hint.v4.b32 [%0], {%1, %2, %3, %4}, %5;" ::"l"(dst), "r"(o0), "r"(o1), "r"(o2), "r"(o3), "l"(pol_keep) : "memory");
                             else asm volatile("red.global.add.v4.f32 [%0], {%1, %2, %3, %4};" ::"l"(dst), "f"(__uint_as_float(o0)),
                                               "f"(__uint_as_float(o1)), "f"(__uint_as_float(o2)), "f"(__uint_as_float(o3)) : "memory");
                         }

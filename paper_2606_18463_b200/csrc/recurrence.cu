@@ -567,7 +567,8 @@ int launch_recurrence(cudaStream_t st, const float *G, int32_t ldg, const float 
     const int choice = recurrence_kernel_choice(s, b, ldg, ws, impl, fu != nullptr);
     if (choice == 5) return launch_recurrence_chain(st, G, ldg, r, yI, s, b, alpha, loss, z, u, fu, ws.late_trigger);
     if (choice == 4)
-        return launch_recurrence_stream(st, G, ldg, r, yI, s, b, alpha, loss, z, u, ws.cluster, fu, ws.late_trigger);
+        return launch_recurrence_stream(st, G, ldg, r, yI, s, b, alpha, loss, z, u, ws.cluster, fu,
+                                        (ws.late_trigger ? 1 : 0) | (ws.g_protected ? 2 : 0));
     if (choice == 3) {
         cudaError_t e = loss == CASGD_LOGISTIC ? launch_cluster<CASGD_LOGISTIC>(st, G, ldg, r, yI, s, b, alpha, z, u, ws.cluster)
                       : loss == CASGD_LINEAR  ? launch_cluster<CASGD_LINEAR>(st, G, ldg, r, yI, s, b, alpha, z, u, ws.cluster)

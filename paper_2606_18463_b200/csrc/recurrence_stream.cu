@@ -107,7 +107,7 @@ recurrence_stream_kernel(const float *G, int32_t ldg, const float *r,
     // The dependent kernel's CTAs become resident (and wait) once every CTA here has triggered. Normally that is wanted
     // at once; with the next step's gather on a side branch it is not: the waiting CTAs would hold the SMs the gather
     // needs (measured: the gather took 42 us instead of 12), so the trigger then comes after the chain.
-    if (!late_trigger) pdl_trigger();
+    if (!(late_trigger & 1)) pdl_trigger();
     REC_TRACE(0);
     const int qmax = (b / kQuad + C - 1) / C;           // row groups of a block per CTA at most
     const StreamLayout L = stream_layout(s, b, qmax);
@@ -121,6 +121,10 @@ recurrence_stream_kernel(const float *G, int32_t ldg, const float *r,
     const int bshift = (b & (b - 1)) == 0 ? __ffs(b) - 1 : -1;             // b a power of two: column -> block by shift
     auto block_of = [&](int col) { return bshift >= 0 ? (col >> bshift) : col / b; };
 
+    // G is read exactly once (L180). Where the pair Gram kernel wrote it with L2::evict_last (bit 1 of late_trigger), these
+    // loads release the lines again (evict_first); elsewhere they keep the default priority (measured: the hint alone costs
+    // poisson-synth s = 32 0.8 %)
+    const unsigned long long pol_g = l2_policy((late_trigger & 2) != 0);
     const int nbulk = qmax == 1 ? 12 : 10;              // 16 warps - 3 critical warps per row group, rounded to a multiple of qmax
     for (int k = threadIdx.x; k < s; k += kThreads) {
         mbar_init(ubar + 8u * k, 1);
@@ -175,8 +179,8 @@ recurrence_stream_kernel(const float *G, int32_t ldg, const float *r,
                     if (c >= 0 && c * kChunk + lane * 4 < len) {
 #pragma unroll
                         for (int i = 0; i < kQuad; ++i)
-                            cp_async16(ring + (uint32_t)(pslot * kWin + w) * kUnitBytes + (uint32_t)i * (kChunk * 4u),
-                                       src + (int64_t)i * ldg + c * kChunk);
+                            cp_async16_hint(ring + (uint32_t)(pslot * kWin + w) * kUnitBytes + (uint32_t)i * (kChunk * 4u),
+                                            src + (int64_t)i * ldg + c * kChunk, pol_g);
                     }
                 }
                 pj += kCritPer;
@@ -305,7 +309,7 @@ recurrence_stream_kernel(const float *G, int32_t ldg, const float *r,
                 const float *src = psrc;
 #pragma unroll
                 for (int i = 0; i < kQuad; ++i) {
-                    cp_async16(dst + (uint32_t)i * (kChunk * 4u), src);
+                    cp_async16_hint(dst + (uint32_t)i * (kChunk * 4u), src, pol_g);
                     src += ldg;
                 }
                 pc += 1;
@@ -361,7 +365,7 @@ recurrence_stream_kernel(const float *G, int32_t ldg, const float *r,
         cluster_sync_all();
     }
     cp_async_wait<0>();
-    if (late_trigger) pdl_trigger();
+    if (late_trigger & 1) pdl_trigger();
     REC_TRACE(2);
     if (fg.Y) {
         // all of u is in this CTA's shared memory once every block's barrier has completed
